@@ -1,0 +1,217 @@
+"""ctypes binding of the CPU oracle (oracle/libjxo.so).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+reference legs may import this module.  It never touches the CUDA library.
+Arrays are numpy, SoA [4][ny][nx] (x fastest), float64 or float32.
+"""
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+OK, EINVAL, ENOMEM, ESTATE, ENUMERIC = 0, 1, 2, 4, 5
+BC_PERIODIC, BC_TRANSMISSIVE, BC_REFLECTIVE, BC_INFLOW = 0, 1, 2, 3
+F64, F32 = 0, 1
+_BC_NAMES = {"periodic": 0, "transmissive": 1, "reflective": 2, "inflow": 3}
+
+
+class _Bc(C.Structure):
+    _fields_ = [("xlo", C.c_int), ("xhi", C.c_int), ("ylo", C.c_int), ("yhi", C.c_int),
+                ("inflow", C.c_double * 4)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build.build())
+        vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)
+        L.jxo_create.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double,
+                                 C.c_double, C.POINTER(_Bc), C.c_int, C.POINTER(vp)]
+        L.jxo_destroy.argtypes = [vp]
+        L.jxo_destroy.restype = None
+        L.jxo_last_error.argtypes = [vp]
+        L.jxo_last_error.restype = C.c_char_p
+        L.jxo_set_ibm.argtypes = [vp, vp]
+        L.jxo_set_flux_mlp.argtypes = [vp, vp, dp, dp, C.c_int]
+        L.jxo_set_artificial_viscosity.argtypes = [vp, C.c_double]
+        L.jxo_rhs.argtypes = [vp, vp, vp]
+        L.jxo_max_wavespeed.argtypes = [vp, vp, dp]
+        L.jxo_step.argtypes = [vp, vp, C.c_double, C.c_int]
+        L.jxo_step_fixed_dt.argtypes = [vp, vp, C.c_double, C.c_int]
+        L.jxo_get_time.argtypes = [vp, dp, dp]
+        L.jxo_weno5.argtypes = [dp]
+        L.jxo_weno5.restype = C.c_double
+        L.jxo_hllc.argtypes = [dp, dp, C.c_double, dp]
+        L.jxo_hllc.restype = None
+        L.jxo_hllc_star.argtypes = [dp, dp, C.c_double, dp, dp, dp]
+        L.jxo_hllc_star.restype = None
+        L.jxo_fill_ghosts.argtypes = [vp, vp, vp]
+        L.jxo_ibm_ghosts.argtypes = [vp, ip, ip, dp, dp]
+        L.jxo_cell_types.argtypes = [vp, vp]
+        L.jxo_guard_count.argtypes = [vp]
+        L.jxo_guard_count.restype = C.c_longlong
+        L.jxo_count_ops.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
+        L.jxo_mlp_eval.argtypes = [vp, dp, dp]
+        _lib = L
+    return _lib
+
+
+def _d(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def make_bc(bc):
+    """bc: dict with xlo/xhi/ylo/yhi in {'periodic','transmissive','reflective','inflow'}
+    and optional inflow=(rho,u,v,p)."""
+    b = _Bc()
+    for side in ("xlo", "xhi", "ylo", "yhi"):
+        setattr(b, side, _BC_NAMES[bc[side]])
+    inflow = bc.get("inflow", (1.0, 0.0, 0.0, 1.0))
+    for k in range(4):
+        b.inflow[k] = float(inflow[k])
+    return b
+
+
+def weno5(v):
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    assert v.shape == (5,)
+    return lib().jxo_weno5(_d(v))
+
+
+def hllc(WL, WR, gamma):
+    WL = np.ascontiguousarray(WL, dtype=np.float64)
+    WR = np.ascontiguousarray(WR, dtype=np.float64)
+    F = np.zeros(4)
+    lib().jxo_hllc(_d(WL), _d(WR), float(gamma), _d(F))
+    return F
+
+
+def hllc_star(WL, WR, gamma):
+    WL = np.ascontiguousarray(WL, dtype=np.float64)
+    WR = np.ascontiguousarray(WR, dtype=np.float64)
+    sp, UL, UR = np.zeros(3), np.zeros(4), np.zeros(4)
+    lib().jxo_hllc_star(_d(WL), _d(WR), float(gamma), _d(sp), _d(UL), _d(UR))
+    return sp, UL, UR
+
+
+class OracleError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"jxo error {code}: {msg}")
+        self.code = code
+
+
+class Oracle:
+    def __init__(self, nx, ny, dx, dy, gamma=1.4, mu=0.0, Pr=0.72, bc=None, dtype=np.float64):
+        self.nx, self.ny = int(nx), int(ny)
+        self.dtype = np.dtype(dtype)
+        assert self.dtype in (np.float64, np.float32)
+        self._bc = make_bc(bc)
+        self._h = C.c_void_p()
+        rc = lib().jxo_create(self.nx, self.ny, dx, dy, gamma, mu, Pr, C.byref(self._bc),
+                              F64 if self.dtype == np.float64 else F32, C.byref(self._h))
+        if rc != OK:
+            raise OracleError(rc, "jxo_create")
+
+    def __del__(self):
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.jxo_destroy(self._h)
+            self._h = None
+
+    def _chk(self, rc):
+        if rc != OK:
+            raise OracleError(rc, lib().jxo_last_error(self._h).decode())
+
+    def _field(self, U):
+        U = np.ascontiguousarray(U, dtype=self.dtype)
+        assert U.shape == (4, self.ny, self.nx), U.shape
+        return U
+
+    def set_ibm(self, phi):
+        if phi is None:
+            self._chk(lib().jxo_set_ibm(self._h, None))
+            return
+        phi = np.ascontiguousarray(phi, dtype=np.float64)
+        assert phi.shape == (self.ny, self.nx)
+        self._chk(lib().jxo_set_ibm(self._h, phi.ctypes.data))
+
+    def set_flux_mlp(self, weights, in_scale=None, out_scale=None, emulate_bf16=False):
+        if weights is None:
+            self._chk(lib().jxo_set_flux_mlp(self._h, None, None, None, 0))
+            return
+        w = np.ascontiguousarray(weights, dtype=np.float32)
+        assert w.shape == (6020,)
+        a = np.ascontiguousarray(in_scale, dtype=np.float64)
+        b = np.ascontiguousarray(out_scale, dtype=np.float64)
+        self._chk(lib().jxo_set_flux_mlp(self._h, w.ctypes.data, _d(a), _d(b), int(emulate_bf16)))
+
+    def set_artificial_viscosity(self, nu):
+        self._chk(lib().jxo_set_artificial_viscosity(self._h, float(nu)))
+
+    def rhs(self, U):
+        U = self._field(U)
+        L = np.empty_like(U)
+        self._chk(lib().jxo_rhs(self._h, U.ctypes.data, L.ctypes.data))
+        return L
+
+    def max_wavespeed(self, U):
+        U = self._field(U)
+        s = C.c_double()
+        self._chk(lib().jxo_max_wavespeed(self._h, U.ctypes.data, C.byref(s)))
+        return s.value
+
+    def step(self, U, cfl, nsteps):
+        U = self._field(U).copy()
+        self._chk(lib().jxo_step(self._h, U.ctypes.data, float(cfl), int(nsteps)))
+        return U
+
+    def step_fixed_dt(self, U, dt, nsteps):
+        U = self._field(U).copy()
+        self._chk(lib().jxo_step_fixed_dt(self._h, U.ctypes.data, float(dt), int(nsteps)))
+        return U
+
+    def time(self):
+        t, dt = C.c_double(), C.c_double()
+        self._chk(lib().jxo_get_time(self._h, C.byref(t), C.byref(dt)))
+        return t.value, dt.value
+
+    def fill_ghosts(self, U):
+        U = self._field(U)
+        Up = np.empty((4, self.ny + 6, self.nx + 6), dtype=self.dtype)
+        self._chk(lib().jxo_fill_ghosts(self._h, U.ctypes.data, Up.ctypes.data))
+        return Up
+
+    def ibm_ghosts(self):
+        n = lib().jxo_ibm_ghosts(self._h, None, None, None, None)
+        cell = np.zeros(n, dtype=np.int32)
+        donors = np.zeros((n, 4), dtype=np.int32)
+        w = np.zeros((n, 4))
+        nrm = np.zeros((n, 2))
+        if n:
+            ip = C.POINTER(C.c_int)
+            lib().jxo_ibm_ghosts(self._h, cell.ctypes.data_as(ip), donors.ctypes.data_as(ip), _d(w), _d(nrm))
+        return cell, donors, w, nrm
+
+    def cell_types(self):
+        t = np.zeros((self.ny, self.nx), dtype=np.uint8)
+        self._chk(lib().jxo_cell_types(self._h, t.ctypes.data))
+        return t
+
+    def guard_count(self):
+        return int(lib().jxo_guard_count(self._h))
+
+    def count_ops(self, U):
+        U = np.ascontiguousarray(U, dtype=np.float64)
+        assert U.shape == (4, self.ny, self.nx)
+        c = (C.c_longlong * 5)()
+        self._chk(lib().jxo_count_ops(self._h, _d(U), c))
+        return dict(zip(("add", "mul", "div", "sqrt", "cmp"), [int(x) for x in c]))
+
+    def mlp_eval(self, x):
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        y = np.zeros(4)
+        self._chk(lib().jxo_mlp_eval(self._h, _d(x), _d(y)))
+        return y
