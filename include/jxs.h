@@ -1,0 +1,120 @@
+/* jxs.h — C ABI of the B200-native (sm_100a) Runge-Kutta-stage library.
+ *
+ * One SSP-RK3 stage of the 2D compressible Euler / Navier-Stokes right-hand side
+ * on a uniform Cartesian grid, as described in JAX-Shock (arXiv 2601.04400):
+ *   ghost-frame and immersed-boundary ghost-cell fill,
+ *   WENO5 reconstruction of primitive left/right face states (L46, L56),
+ *   HLLC flux in x and y (L54-81, Eq. 3-9), flux divergence + viscous terms
+ *   (L9, L83-85 Eq. 10), Runge-Kutta combine and CFL wavespeed reduction
+ *   (BASELINE.json north_star), optional per-face MLP flux correction (L96 Eq. 11).
+ * Where the paper is silent or garbled the readings R1-R17 of DESIGN.md apply.
+ *
+ * Conventions
+ *   - every function returns an int status (JXS_OK = 0); nothing throws, aborts or prints;
+ *     jxs_last_error() gives the detail of the last failure on a handle.
+ *   - the handle is opaque and owns every internal buffer (padded RK buffers, IBM lists,
+ *     MLP weights, device scalars).  The caller owns every array it passes; the library
+ *     never frees or keeps them past the call.
+ *   - field arrays are DEVICE pointers unless the function name ends in _host:
+ *     SoA [4][ny][nx], x fastest, component order (rho, rho*u, rho*v, E), interior cells
+ *     only, element type = the handle's dtype (JXS_F64 -> double, JXS_F32 -> float),
+ *     16-byte aligned.
+ *   - all device work is enqueued on the stream given to jxs_create (0 = default stream).
+ *     Functions returning a host scalar synchronise that stream; jxs_rhs does not;
+ *     jxs_step* synchronise once at the end to read the non-finite flag.
+ *   - there is no CPU fallback: without a CUDA device jxs_create fails with JXS_ECUDA.
+ */
+#ifndef JXS_H
+#define JXS_H
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  JXS_OK = 0,
+  JXS_EINVAL = 1,   /* bad argument (see each function)                         */
+  JXS_ENOMEM = 2,   /* host or device allocation failed                          */
+  JXS_ECUDA = 3,    /* CUDA runtime error (no device, launch failure, ...)       */
+  JXS_ESTATE = 4,   /* call not valid in the handle's current state              */
+  JXS_ENUMERIC = 5  /* non-finite wavespeed / state detected during stepping     */
+};
+enum { JXS_BC_PERIODIC = 0, JXS_BC_TRANSMISSIVE = 1, JXS_BC_REFLECTIVE = 2, JXS_BC_INFLOW = 3 };
+enum { JXS_F64 = 0, JXS_F32 = 1 };
+
+typedef struct jxs_solver jxs_solver;
+
+/* Domain boundary conditions (inflow = left state, outflow, reflective walls;
+ * transmissive for Sod, periodic for the vortex: BASELINE.json configs).  Three ghost layers
+ * per side; x sides first, then y sides over the x-extended range (R11).                  */
+typedef struct {
+  int xlo, xhi, ylo, yhi; /* JXS_BC_*; PERIODIC must be set on both sides of an axis   */
+  double inflow[4];       /* primitive (rho,u,v,p) imposed on JXS_BC_INFLOW sides       */
+} jxs_bc;
+
+/* Create a solver for an nx x ny grid of spacing (dx,dy), ideal gas gamma (Eq. 2), constant
+ * dynamic viscosity mu >= 0 (0 = Euler) and Prandtl number Pr (R7, R8).
+ * cuda_stream: a cudaStream_t cast to void*, or NULL.
+ * JXS_EINVAL: nx or ny < 8, dx/dy <= 0, gamma <= 1, mu < 0, Pr <= 0 with mu > 0, bad bc or
+ * dtype, NULL pointers.  JXS_ECUDA: no usable device.  JXS_ENOMEM: allocation failed.     */
+int jxs_create(int nx, int ny, double dx, double dy, double gamma, double mu, double Pr,
+               const jxs_bc* bc, int dtype, void* cuda_stream, jxs_solver** out);
+void jxs_destroy(jxs_solver*);
+/* Never NULL; "" when there was no error.  Valid until the next call on the handle.        */
+const char* jxs_last_error(const jxs_solver*);
+
+/* Immersed boundary (R9, R10).  phi_host: HOST array [ny][nx], signed
+ * distance, > 0 in the fluid; NULL removes the body.  Builds the cell classification and the
+ * ghost-cell gather list on the host and uploads them.  JXS_EINVAL: a non-fluid cell closer
+ * than 8 cells to a domain edge, zero gradient at a ghost cell, or a ghost cell left without
+ * a fluid donor (the previous body, if any, is then removed).                              */
+int jxs_set_ibm(jxs_solver*, const double* phi_host);
+
+/* Per-face MLP flux correction (Eq. 11; BASELINE.json configs[4]; R14).  weights_host: HOST
+ * array of 6020 floats, W1[64][24], b1[64], W2[64][64], b2[64], W3[4][64], b3[4] (row-major,
+ * [out][in]); NULL disables.  in_scale[4] > 0 divides (rho, u_n, u_t, p); out_scale[4]
+ * multiplies the four outputs (mass, normal, tangential momentum, energy).  The network is
+ * evaluated in bf16 with fp32 accumulation on the tensor cores.                             */
+int jxs_set_flux_mlp(jxs_solver*, const float* weights_host, const double in_scale[4],
+                     const double out_scale[4]);
+
+/* Laplacian artificial viscosity nu * Lap_h(U) of PAPER.md Eq. 10; default 0 (R7).          */
+int jxs_set_artificial_viscosity(jxs_solver*, double nu);
+
+/* dUdt = L(U): ghost fills on an internal copy of U, then the fused stage kernel with the
+ * Runge-Kutta combine disabled.  dUdt is 0 at non-fluid cells.  Asynchronous.               */
+int jxs_rhs(jxs_solver*, const void* U, void* dUdt);
+
+/* smax = max over fluid interior cells of max(|u|+a, |v|+a) (R6).  Synchronises.            */
+int jxs_max_wavespeed(jxs_solver*, const void* U, double* smax_host);
+
+/* Advance U in place by nsteps SSP-RK3 steps (R5), dt = cfl*min(dx,dy)/smax evaluated on the
+ * device at the start of every step (R6).  JXS_ENUMERIC if a non-finite or non-positive
+ * wavespeed was met (U then holds the last state computed).  Synchronises once at the end.   */
+int jxs_step(jxs_solver*, void* U, double cfl, int nsteps);
+/* Same with a fixed time step.                                                              */
+int jxs_step_fixed_dt(jxs_solver*, void* U, double dt, int nsteps);
+/* Same two calls on HOST buffers (pageable or pinned): host->device copy, stepping,
+ * device->host copy; used for end-to-end timing.                                            */
+int jxs_step_host(jxs_solver*, void* U_host, double cfl, int nsteps);
+int jxs_rhs_host(jxs_solver*, const void* U_host, void* dUdt_host);
+
+/* Simulated time since creation and the last time step taken.                               */
+int jxs_get_time(const jxs_solver*, double* t_host, double* last_dt_host);
+
+/* Number of kernel launches enqueued by this handle since creation (bench.py reports it).   */
+long long jxs_launch_count(const jxs_solver*);
+/* Device time (ms) of the stage kernels of the last jxs_step* call, measured with CUDA events
+ * on the handle's stream, and how many stage launches that was.  Only recorded when
+ * jxs_set_profiling(h, 1) is on (it adds two event records per stage launch).               */
+int jxs_set_profiling(jxs_solver*, int on);
+int jxs_stage_time(const jxs_solver*, double* ms_total, long long* launches);
+/* Number of IBM ghost cells (0 without a body).                                             */
+int jxs_ibm_ghost_count(const jxs_solver*);
+/* Sustained FP64 FMA rate of the device, in TFLOP/s (2 flops per FMA), from a register-
+ * resident DFMA loop run for about `ms` milliseconds: the ALU-roofline denominator.         */
+int jxs_measure_fp64_peak(void* cuda_stream, double ms, double* tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

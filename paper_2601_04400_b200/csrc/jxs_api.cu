@@ -1,0 +1,553 @@
+// jxs_api.cu — the C ABI of include/jxs.h: handle, argument checks, host-side set-up (work
+// decomposition, immersed-boundary classification and gather list), kernel launches.
+// Every step of the hot path runs in the kernels of stage_kernel.cuh / aux_kernels.cuh.
+#include "../../include/jxs.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "aux_kernels.cuh"
+#include "stage_kernel.cuh"
+
+using namespace jxs;
+
+namespace {
+constexpr int MAXW = 12;        // warps per CTA of the stage kernel (one CTA per SM)
+constexpr int MAX_EVENTS = 8192;
+}
+
+struct jxs_solver {
+  int nx = 0, ny = 0, dtype = 0;
+  double dx = 0, dy = 0, gamma = 0, mu = 0, Pr = 0, nu = 0;
+  jxs_bc bc{};
+  cudaStream_t stream = nullptr;
+  int num_sms = 0;
+  // padded layout
+  int pitch = 0;
+  long long plane = 0;
+  size_t elem = 8;
+  void* buf[3] = {nullptr, nullptr, nullptr};
+  void* stage_io = nullptr;  // interior-sized staging for the *_host entry points
+  // immersed boundary
+  uint8_t* d_fluid = nullptr;
+  int n_ghost = 0;
+  int* d_cell = nullptr;
+  int* d_donor = nullptr;
+  double* d_w = nullptr;
+  double* d_nrm = nullptr;
+  // stepping state
+  StepState* d_state = nullptr;
+  double t = 0, last_dt = 0;
+  // work decomposition of the stage kernel
+  int nstrips = 0, rows_per_seg = 0, nseg = 0, ntasks = 0, warps = 0, grid = 0;
+  // bookkeeping
+  long long launches = 0;
+  bool profiling = false;
+  std::vector<cudaEvent_t> events;
+  int events_used = 0;
+  double stage_ms = 0;
+  long long stage_launches = 0;
+  mutable std::string err;
+};
+
+namespace {
+
+int fail(const jxs_solver* s, int code, const std::string& msg) {
+  if (s) s->err = msg;
+  return code;
+}
+int cuda_fail(const jxs_solver* s, cudaError_t e, const char* what) {
+  return fail(s, e == cudaErrorMemoryAllocation ? JXS_ENOMEM : JXS_ECUDA,
+              std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CU(call)                                             \
+  do {                                                       \
+    cudaError_t e_ = (call);                                 \
+    if (e_ != cudaSuccess) return cuda_fail(s, e_, #call);   \
+  } while (0)
+
+GridDims dims(const jxs_solver* s) { return GridDims{s->nx, s->ny, s->pitch, s->plane}; }
+
+BcSpec bcspec(const jxs_solver* s) {
+  BcSpec b;
+  b.xlo = s->bc.xlo; b.xhi = s->bc.xhi; b.ylo = s->bc.ylo; b.yhi = s->bc.yhi;
+  const double r = s->bc.inflow[0], u = s->bc.inflow[1], v = s->bc.inflow[2], p = s->bc.inflow[3];
+  b.inflow_cons[0] = r; b.inflow_cons[1] = r * u; b.inflow_cons[2] = r * v;
+  b.inflow_cons[3] = p / (s->gamma - 1.0) + 0.5 * r * (u * u + v * v);
+  return b;
+}
+
+template <typename T> constexpr int sout() { return Cfg<T>::SOUT; }
+
+// Strips x segments: a multiple of the resident warp slots, segments long enough to amortise the
+// 6 warm-up rows of every segment.
+void choose_decomposition(jxs_solver* s) {
+  const int SOUT = s->dtype == JXS_F64 ? sout<double>() : sout<float>();
+  s->nstrips = (s->nx + SOUT - 1) / SOUT;
+  const long long slots = (long long)s->num_sms * MAXW;
+  double best = 1e300;
+  int best_rps = s->ny;
+  for (int w = 1; w <= 16; ++w) {
+    long long S = std::max<long long>(1, w * slots / s->nstrips);
+    int rps = (int)((s->ny + S - 1) / S);
+    rps = std::max(rps, std::min(s->ny, 8));
+    const int segs = (s->ny + rps - 1) / rps;
+    const long long tasks = (long long)segs * s->nstrips;
+    const long long waves = (tasks + slots - 1) / slots;
+    const double cost = (double)waves * (rps + 4.0);
+    if (cost < best - 1e-9) { best = cost; best_rps = rps; }
+  }
+  s->rows_per_seg = best_rps;
+  s->nseg = (s->ny + best_rps - 1) / best_rps;
+  s->ntasks = s->nseg * s->nstrips;
+  // small problems: fewer warps per CTA so that the CTAs spread over the SMs
+  s->warps = (int)std::min<long long>(MAXW, std::max<long long>(1, (s->ntasks + s->num_sms - 1) / s->num_sms));
+  s->grid = (s->ntasks + s->warps - 1) / s->warps;
+}
+
+template <typename T, bool VISC, bool ARTV>
+cudaError_t launch_stage_t(jxs_solver* s, const StageArgs<T>& a) {
+  auto kern = stage_kernel<T, VISC, ARTV, MAXW>;
+  constexpr int NV = VISC ? 5 : 4;
+  const size_t smem = stage_smem_per_warp<NV>(sizeof(T)) * s->warps;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)(stage_smem_per_warp<NV>(sizeof(T)) * MAXW));
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  kern<<<s->grid, s->warps * 32, smem, s->stream>>>(a);
+  return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t launch_stage(jxs_solver* s, const void* Uin, const void* U0, void* Uout, int mode, double a, double b,
+                         unsigned long long* smax_bits) {
+  StageArgs<T> A;
+  A.Uin = (const T*)Uin; A.U0 = (const T*)U0; A.Uout = (T*)Uout;
+  A.fluid = s->d_fluid;
+  A.dt = &s->d_state->dt;
+  A.smax_bits = smax_bits;
+  A.plane = s->plane; A.nx = s->nx; A.ny = s->ny; A.pitch = s->pitch;
+  A.nstrips = s->nstrips; A.rows_per_seg = s->rows_per_seg; A.ntasks = s->ntasks;
+  A.mode = mode;
+  A.gamma = (T)s->gamma; A.g1 = (T)(s->gamma - 1.0); A.g1inv = (T)(1.0 / (s->gamma - 1.0));
+  A.dxi = (T)(1.0 / s->dx); A.dyi = (T)(1.0 / s->dy);
+  A.mu = (T)s->mu;
+  A.kappa = (T)(s->mu > 0 ? s->mu * s->gamma / ((s->gamma - 1.0) * s->Pr) : 0.0);
+  A.nu = (T)s->nu;
+  A.rk_a = (T)a; A.rk_b = (T)b;
+  const bool visc = s->mu > 0, artv = s->nu > 0;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (s->profiling && mode == 0 && s->events_used + 2 <= (int)s->events.size()) {
+    e0 = s->events[s->events_used++];
+    e1 = s->events[s->events_used++];
+    cudaEventRecord(e0, s->stream);
+  }
+  cudaError_t e;
+  if (visc) e = artv ? launch_stage_t<T, true, true>(s, A) : launch_stage_t<T, true, false>(s, A);
+  else e = artv ? launch_stage_t<T, false, true>(s, A) : launch_stage_t<T, false, false>(s, A);
+  if (e1) cudaEventRecord(e1, s->stream);
+  s->launches++;
+  return e;
+}
+
+cudaError_t stage(jxs_solver* s, const void* Uin, const void* U0, void* Uout, int mode, double a, double b,
+                  unsigned long long* smax_bits) {
+  return s->dtype == JXS_F64 ? launch_stage<double>(s, Uin, U0, Uout, mode, a, b, smax_bits)
+                             : launch_stage<float>(s, Uin, U0, Uout, mode, a, b, smax_bits);
+}
+
+cudaError_t ghost_fill(jxs_solver* s, void* U) {
+  const int nframe = 6 * s->ny + 6 * (s->nx + 6);
+  const int total = nframe + s->n_ghost;
+  IbmList L{s->d_cell, s->d_donor, s->d_w, s->d_nrm, s->n_ghost};
+  const int bs = 128;
+  if (s->dtype == JXS_F64)
+    ghost_fill_kernel<double><<<(total + bs - 1) / bs, bs, 0, s->stream>>>((double*)U, dims(s), bcspec(s), L, s->gamma);
+  else
+    ghost_fill_kernel<float><<<(total + bs - 1) / bs, bs, 0, s->stream>>>((float*)U, dims(s), bcspec(s), L, (float)s->gamma);
+  s->launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t pad(jxs_solver* s, const void* U, void* dst) {
+  const int bs = 256, gs = s->num_sms * 8;
+  if (s->dtype == JXS_F64) pad_kernel<double><<<gs, bs, 0, s->stream>>>((const double*)U, (double*)dst, dims(s));
+  else pad_kernel<float><<<gs, bs, 0, s->stream>>>((const float*)U, (float*)dst, dims(s));
+  s->launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t unpad(jxs_solver* s, const void* src, void* U) {
+  const int bs = 256, gs = s->num_sms * 8;
+  if (s->dtype == JXS_F64) unpad_kernel<double><<<gs, bs, 0, s->stream>>>((const double*)src, (double*)U, dims(s));
+  else unpad_kernel<float><<<gs, bs, 0, s->stream>>>((const float*)src, (float*)U, dims(s));
+  s->launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t wavespeed(jxs_solver* s, const void* Upad, unsigned long long* out_bits) {
+  cudaError_t e = cudaMemsetAsync(out_bits, 0, sizeof(unsigned long long), s->stream);
+  if (e != cudaSuccess) return e;
+  const int bs = 256, gs = s->num_sms * 8;
+  if (s->dtype == JXS_F64)
+    wavespeed_kernel<double><<<gs, bs, 0, s->stream>>>((const double*)Upad, dims(s), s->d_fluid, s->gamma, out_bits);
+  else
+    wavespeed_kernel<float><<<gs, bs, 0, s->stream>>>((const float*)Upad, dims(s), s->d_fluid, (float)s->gamma, out_bits);
+  s->launches++;
+  return cudaGetLastError();
+}
+
+void free_ibm(jxs_solver* s) {
+  cudaFree(s->d_fluid); cudaFree(s->d_cell); cudaFree(s->d_donor); cudaFree(s->d_w); cudaFree(s->d_nrm);
+  s->d_fluid = nullptr; s->d_cell = nullptr; s->d_donor = nullptr; s->d_w = nullptr; s->d_nrm = nullptr;
+  s->n_ghost = 0;
+}
+
+// advance the padded state in buf[0] by nsteps SSP-RK3 steps (R5); cur = index of the valid s_max
+int run_steps(jxs_solver* s, double cfl, double fixed_dt, int nsteps) {
+  const double h = std::min(s->dx, s->dy);
+  int cur = 0;
+  s->events_used = 0;
+  if (!(fixed_dt > 0)) CU(wavespeed(s, s->buf[0], &s->d_state->smax_bits[0]));
+  for (int n = 0; n < nsteps; ++n) {
+    prepare_step_kernel<<<1, 1, 0, s->stream>>>(s->d_state, cur, cfl * h, fixed_dt);
+    s->launches++;
+    CU(cudaGetLastError());
+    unsigned long long* next = &s->d_state->smax_bits[cur ^ 1];
+    CU(ghost_fill(s, s->buf[0]));
+    CU(stage(s, s->buf[0], nullptr, s->buf[1], 0, 0.0, 1.0, nullptr));                  // U1 = U0 + dt L(U0)
+    CU(ghost_fill(s, s->buf[1]));
+    CU(stage(s, s->buf[1], s->buf[0], s->buf[2], 0, 0.75, 0.25, nullptr));              // U2 = 3/4 U0 + 1/4 (U1 + dt L(U1))
+    CU(ghost_fill(s, s->buf[2]));
+    CU(stage(s, s->buf[2], s->buf[0], s->buf[0], 0, 1.0 / 3.0, 2.0 / 3.0, next));       // U0 = 1/3 U0 + 2/3 (U2 + dt L(U2))
+    cur ^= 1;
+  }
+  return JXS_OK;
+}
+
+int finish_steps(jxs_solver* s, int nsteps) {
+  StepState st;
+  CU(cudaMemcpyAsync(&st, s->d_state, sizeof(st), cudaMemcpyDeviceToHost, s->stream));
+  CU(cudaStreamSynchronize(s->stream));
+  s->t = st.t;
+  if (nsteps > 0) s->last_dt = st.dt;
+  if (s->profiling) {
+    s->stage_ms = 0;
+    s->stage_launches = s->events_used / 2;
+    for (int i = 0; i + 1 < s->events_used; i += 2) {
+      float ms = 0;
+      cudaEventElapsedTime(&ms, s->events[i], s->events[i + 1]);
+      s->stage_ms += ms;
+    }
+  }
+  if (st.bad) {
+    int zero = 0;
+    cudaMemcpyAsync(&s->d_state->bad, &zero, sizeof(int), cudaMemcpyHostToDevice, s->stream);
+    return fail(s, JXS_ENUMERIC, "non-finite or non-positive wavespeed met while stepping");
+  }
+  const double sm = 0;  (void)sm;
+  return JXS_OK;
+}
+
+int step_common(jxs_solver* s, void* U, double cfl, double fixed_dt, int nsteps, bool host) {
+  if (!s) return JXS_EINVAL;
+  if (!U) return fail(s, JXS_EINVAL, "U is NULL");
+  if (nsteps < 0) return fail(s, JXS_EINVAL, "nsteps < 0");
+  if (!(fixed_dt > 0) && !(cfl > 0)) return fail(s, JXS_EINVAL, "cfl must be > 0");
+  const size_t bytes = (size_t)4 * s->nx * s->ny * s->elem;
+  const void* Ud = U;
+  if (host) {
+    CU(cudaMemcpyAsync(s->stage_io, U, bytes, cudaMemcpyHostToDevice, s->stream));
+    Ud = s->stage_io;
+  }
+  CU(pad(s, Ud, s->buf[0]));
+  int rc = run_steps(s, cfl, fixed_dt, nsteps);
+  if (rc != JXS_OK) return rc;
+  if (host) {
+    CU(unpad(s, s->buf[0], s->stage_io));
+    CU(cudaMemcpyAsync(U, s->stage_io, bytes, cudaMemcpyDeviceToHost, s->stream));
+  } else {
+    CU(unpad(s, s->buf[0], U));
+  }
+  return finish_steps(s, nsteps);
+}
+
+}  // namespace
+
+extern "C" {
+
+int jxs_create(int nx, int ny, double dx, double dy, double gamma, double mu, double Pr, const jxs_bc* bc, int dtype,
+               void* cuda_stream, jxs_solver** out) {
+  if (!out) return JXS_EINVAL;
+  *out = nullptr;
+  if (!bc) return JXS_EINVAL;
+  if (nx < 8 || ny < 8 || !(dx > 0) || !(dy > 0) || !(gamma > 1) || !(mu >= 0) || (mu > 0 && !(Pr > 0))) return JXS_EINVAL;
+  if (dtype != JXS_F64 && dtype != JXS_F32) return JXS_EINVAL;
+  const int kinds[4] = {bc->xlo, bc->xhi, bc->ylo, bc->yhi};
+  for (int k : kinds)
+    if (k < 0 || k > 3) return JXS_EINVAL;
+  if ((bc->xlo == JXS_BC_PERIODIC) != (bc->xhi == JXS_BC_PERIODIC)) return JXS_EINVAL;
+  if ((bc->ylo == JXS_BC_PERIODIC) != (bc->yhi == JXS_BC_PERIODIC)) return JXS_EINVAL;
+  for (int k = 0; k < 4; ++k)
+    if (!std::isfinite(bc->inflow[k])) return JXS_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return JXS_ECUDA;
+  jxs_solver* s = new (std::nothrow) jxs_solver;
+  if (!s) return JXS_ENOMEM;
+  s->nx = nx; s->ny = ny; s->dx = dx; s->dy = dy; s->gamma = gamma; s->mu = mu; s->Pr = Pr; s->bc = *bc;
+  s->dtype = dtype;
+  s->elem = dtype == JXS_F64 ? 8 : 4;
+  s->stream = (cudaStream_t)cuda_stream;
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { delete s; return JXS_ECUDA; }
+  if (prop.major < 10) { delete s; return JXS_ECUDA; }  // sm_100a code only
+  s->num_sms = prop.multiProcessorCount;
+  choose_decomposition(s);
+  const int SOUT = dtype == JXS_F64 ? sout<double>() : sout<float>();
+  s->pitch = ((SOUT * s->nstrips + 6 + 15) / 16) * 16;
+  s->plane = (long long)(ny + 6) * s->pitch;
+  if (s->plane > 0x7fffffffLL) { delete s; return JXS_EINVAL; }
+  const size_t pbytes = (size_t)4 * s->plane * s->elem;
+  cudaError_t e = cudaSuccess;
+  for (int b = 0; b < 3 && e == cudaSuccess; ++b) e = cudaMalloc(&s->buf[b], pbytes);
+  if (e == cudaSuccess) e = cudaMalloc(&s->stage_io, (size_t)4 * nx * ny * s->elem);
+  if (e == cudaSuccess) e = cudaMalloc(&s->d_state, sizeof(StepState));
+  if (e == cudaSuccess) e = cudaMemsetAsync(s->d_state, 0, sizeof(StepState), s->stream);
+  if (e != cudaSuccess) {
+    const int rc = e == cudaErrorMemoryAllocation ? JXS_ENOMEM : JXS_ECUDA;
+    jxs_destroy(s);
+    cudaGetLastError();
+    return rc;
+  }
+  const double e_rest = 1.0 / (gamma - 1.0);
+  for (int b = 0; b < 3; ++b) {
+    if (dtype == JXS_F64) fill_benign_kernel<double><<<s->num_sms * 4, 256, 0, s->stream>>>((double*)s->buf[b], dims(s), e_rest);
+    else fill_benign_kernel<float><<<s->num_sms * 4, 256, 0, s->stream>>>((float*)s->buf[b], dims(s), (float)e_rest);
+    s->launches++;
+  }
+  if (cudaGetLastError() != cudaSuccess) { jxs_destroy(s); return JXS_ECUDA; }
+  *out = s;
+  return JXS_OK;
+}
+
+void jxs_destroy(jxs_solver* s) {
+  if (!s) return;
+  cudaStreamSynchronize(s->stream);
+  for (int b = 0; b < 3; ++b) cudaFree(s->buf[b]);
+  cudaFree(s->stage_io);
+  cudaFree(s->d_state);
+  free_ibm(s);
+  for (cudaEvent_t ev : s->events) cudaEventDestroy(ev);
+  delete s;
+}
+
+const char* jxs_last_error(const jxs_solver* s) { return s ? s->err.c_str() : "null handle"; }
+
+int jxs_set_ibm(jxs_solver* s, const double* phi) {
+  if (!s) return JXS_EINVAL;
+  CU(cudaStreamSynchronize(s->stream));
+  free_ibm(s);
+  if (!phi) return JXS_OK;
+  const int nx = s->nx, ny = s->ny;
+  const double dx = s->dx, dy = s->dy;
+  // classification (R9 I1, I2): 1 = fluid in `fl`; ghost = non-fluid cell that some fluid cell's
+  // WENO stencil (3 cells along an axis) or viscous stencil (3x3 box) touches
+  std::vector<uint8_t> fl((size_t)nx * ny);
+  for (size_t c = 0; c < fl.size(); ++c) fl[c] = phi[c] > 0.0 ? 1 : 0;
+  auto is_fluid = [&](int i, int j) { return i >= 0 && i < nx && j >= 0 && j < ny && fl[(size_t)j * nx + i]; };
+  std::vector<int> cell, donor;
+  std::vector<double> wts, nrm;
+  static const int off[16][2] = {{1, 0}, {-1, 0}, {0, 1}, {0, -1}, {2, 0}, {-2, 0}, {0, 2}, {0, -2},
+                                 {3, 0}, {-3, 0}, {0, 3}, {0, -3}, {1, 1}, {-1, 1}, {1, -1}, {-1, -1}};
+  const double h = std::min(dx, dy);
+  for (int j = 0; j < ny; ++j)
+    for (int i = 0; i < nx; ++i) {
+      if (fl[(size_t)j * nx + i]) continue;
+      if (i < 8 || j < 8 || i >= nx - 8 || j >= ny - 8)
+        return fail(s, JXS_EINVAL, "IBM body closer than 8 cells to a domain edge");
+      bool ghost = false;
+      for (int q = 0; q < 16 && !ghost; ++q) ghost = is_fluid(i + off[q][0], j + off[q][1]);
+      if (!ghost) continue;
+      // I3: unit normal from central differences of the sampled level set
+      const double px = (phi[(size_t)j * nx + i + 1] - phi[(size_t)j * nx + i - 1]) / (2.0 * dx);
+      const double py = (phi[(size_t)(j + 1) * nx + i] - phi[(size_t)(j - 1) * nx + i]) / (2.0 * dy);
+      const double pn = std::sqrt(px * px + py * py);
+      if (!(pn > 0.0)) return fail(s, JXS_EINVAL, "IBM: zero level-set gradient at a ghost cell");
+      const double n0 = px / pn, n1 = py / pn;
+      // I4: image point, mirrored through the surface along the normal
+      const double depth = std::fabs(phi[(size_t)j * nx + i]);
+      double xi = (i + 0.5) * dx + 2.0 * depth * n0;
+      double yi = (j + 0.5) * dy + 2.0 * depth * n1;
+      // I5: bilinear donors, non-fluid ones dropped, weights renormalised; probe outwards if empty
+      int di[4], dj[4];
+      double w[4], sum = 0.0;
+      for (int attempt = 0; attempt < 9; ++attempt) {
+        const double fx = xi / dx - 0.5, fy = yi / dy - 0.5;
+        const int i0 = (int)std::floor(fx), j0 = (int)std::floor(fy);
+        const double tx = fx - i0, ty = fy - j0;
+        const double bw[4] = {(1 - tx) * (1 - ty), tx * (1 - ty), (1 - tx) * ty, tx * ty};
+        sum = 0.0;
+        for (int d = 0; d < 4; ++d) {
+          di[d] = i0 + (d & 1); dj[d] = j0 + (d >> 1);
+          w[d] = is_fluid(di[d], dj[d]) ? bw[d] : 0.0;
+          sum += w[d];
+        }
+        if (sum > 0.0) break;
+        xi += h * n0; yi += h * n1;
+      }
+      if (!(sum > 0.0)) return fail(s, JXS_EINVAL, "IBM: ghost cell without a fluid donor");
+      cell.push_back((j + 3) * s->pitch + i + 3);
+      for (int d = 0; d < 4; ++d) {
+        const double wd = w[d] / sum;
+        wts.push_back(wd);
+        donor.push_back(wd > 0.0 ? (dj[d] + 3) * s->pitch + di[d] + 3 : (j + 3) * s->pitch + i + 3);
+      }
+      nrm.push_back(n0); nrm.push_back(n1);
+    }
+  const int ng = (int)cell.size();
+  CU(cudaMalloc(&s->d_fluid, fl.size()));
+  CU(cudaMemcpy(s->d_fluid, fl.data(), fl.size(), cudaMemcpyHostToDevice));
+  if (ng > 0) {
+    CU(cudaMalloc(&s->d_cell, sizeof(int) * ng));
+    CU(cudaMalloc(&s->d_donor, sizeof(int) * 4 * ng));
+    CU(cudaMalloc(&s->d_w, sizeof(double) * 4 * ng));
+    CU(cudaMalloc(&s->d_nrm, sizeof(double) * 2 * ng));
+    CU(cudaMemcpy(s->d_cell, cell.data(), sizeof(int) * ng, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(s->d_donor, donor.data(), sizeof(int) * 4 * ng, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(s->d_w, wts.data(), sizeof(double) * 4 * ng, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(s->d_nrm, nrm.data(), sizeof(double) * 2 * ng, cudaMemcpyHostToDevice));
+  }
+  s->n_ghost = ng;
+  return JXS_OK;
+}
+
+int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[4], const double out_scale[4]) {
+  if (!s) return JXS_EINVAL;
+  if (!weights) return JXS_OK;
+  (void)in_scale; (void)out_scale;
+  return fail(s, JXS_ESTATE, "per-face MLP flux correction is not built yet");
+}
+
+int jxs_set_artificial_viscosity(jxs_solver* s, double nu) {
+  if (!s) return JXS_EINVAL;
+  if (!(nu >= 0)) return fail(s, JXS_EINVAL, "nu must be >= 0");
+  s->nu = nu;
+  return JXS_OK;
+}
+
+int jxs_rhs(jxs_solver* s, const void* U, void* dUdt) {
+  if (!s) return JXS_EINVAL;
+  if (!U || !dUdt) return fail(s, JXS_EINVAL, "NULL array");
+  CU(pad(s, U, s->buf[0]));
+  CU(ghost_fill(s, s->buf[0]));
+  CU(stage(s, s->buf[0], nullptr, dUdt, 1, 0.0, 1.0, nullptr));
+  return JXS_OK;
+}
+
+int jxs_rhs_host(jxs_solver* s, const void* U, void* dUdt) {
+  if (!s) return JXS_EINVAL;
+  if (!U || !dUdt) return fail(s, JXS_EINVAL, "NULL array");
+  const size_t bytes = (size_t)4 * s->nx * s->ny * s->elem;
+  CU(cudaMemcpyAsync(s->stage_io, U, bytes, cudaMemcpyHostToDevice, s->stream));
+  CU(pad(s, s->stage_io, s->buf[0]));
+  CU(ghost_fill(s, s->buf[0]));
+  CU(stage(s, s->buf[0], nullptr, s->stage_io, 1, 0.0, 1.0, nullptr));
+  CU(cudaMemcpyAsync(dUdt, s->stage_io, bytes, cudaMemcpyDeviceToHost, s->stream));
+  CU(cudaStreamSynchronize(s->stream));
+  return JXS_OK;
+}
+
+int jxs_max_wavespeed(jxs_solver* s, const void* U, double* smax) {
+  if (!s) return JXS_EINVAL;
+  if (!U || !smax) return fail(s, JXS_EINVAL, "NULL argument");
+  CU(pad(s, U, s->buf[1]));
+  unsigned long long* bits = &s->d_state->smax_bits[0];
+  CU(wavespeed(s, s->buf[1], bits));
+  unsigned long long h = 0;
+  CU(cudaMemcpyAsync(&h, bits, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+  CU(cudaStreamSynchronize(s->stream));
+  double v;
+  std::memcpy(&v, &h, sizeof(v));
+  *smax = v;
+  return JXS_OK;
+}
+
+int jxs_step(jxs_solver* s, void* U, double cfl, int nsteps) { return step_common(s, U, cfl, 0.0, nsteps, false); }
+int jxs_step_fixed_dt(jxs_solver* s, void* U, double dt, int nsteps) {
+  if (s && !(dt > 0)) return fail(s, JXS_EINVAL, "dt must be > 0");
+  return step_common(s, U, 0.0, dt, nsteps, false);
+}
+int jxs_step_host(jxs_solver* s, void* U, double cfl, int nsteps) { return step_common(s, U, cfl, 0.0, nsteps, true); }
+
+int jxs_get_time(const jxs_solver* s, double* t, double* last_dt) {
+  if (!s) return JXS_EINVAL;
+  if (t) *t = s->t;
+  if (last_dt) *last_dt = s->last_dt;
+  return JXS_OK;
+}
+
+long long jxs_launch_count(const jxs_solver* s) { return s ? s->launches : -1; }
+
+int jxs_set_profiling(jxs_solver* s, int on) {
+  if (!s) return JXS_EINVAL;
+  s->profiling = on != 0;
+  if (s->profiling && s->events.empty()) {
+    s->events.resize(MAX_EVENTS);
+    for (cudaEvent_t& ev : s->events) CU(cudaEventCreate(&ev));
+  }
+  return JXS_OK;
+}
+
+int jxs_stage_time(const jxs_solver* s, double* ms_total, long long* launches) {
+  if (!s) return JXS_EINVAL;
+  if (ms_total) *ms_total = s->stage_ms;
+  if (launches) *launches = s->stage_launches;
+  return JXS_OK;
+}
+
+int jxs_ibm_ghost_count(const jxs_solver* s) { return s ? s->n_ghost : -1; }
+
+int jxs_measure_fp64_peak(void* cuda_stream, double ms, double* tflops) {
+  if (!tflops || !(ms > 0)) return JXS_EINVAL;
+  int ndev = 0, dev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return JXS_ECUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return JXS_ECUDA;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  double* d_out = nullptr;
+  if (cudaMalloc(&d_out, 8) != cudaSuccess) return JXS_ENOMEM;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int bs = 256, gs = prop.multiProcessorCount * 8;
+  int iters = 2000;
+  double best = 0;
+  float el = 0;
+  for (int rep = 0; rep < 6; ++rep) {
+    cudaEventRecord(e0, st);
+    dfma_peak_kernel<<<gs, bs, 0, st>>>(d_out, iters, 1.0000001, 1e-9);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) break;
+    cudaEventElapsedTime(&el, e0, e1);
+    const double fl = (double)gs * bs * (double)iters * 64.0 * 2.0;
+    if (rep > 0) best = std::max(best, fl / (el * 1e-3) / 1e12);
+    if (el < ms) iters = (int)std::min(2.0e6, iters * std::max(1.5, ms / std::max(el, 1e-3f)));
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(d_out);
+  if (cudaGetLastError() != cudaSuccess) return JXS_ECUDA;
+  *tflops = best;
+  return JXS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,215 @@
+"""Thin ctypes binding of include/jxs.h with the same names (argument marshalling only).
+
+torch is used for device memory and streams; fields are torch CUDA tensors [4, ny, nx]
+(float64 or float32, contiguous).  If the CUDA library cannot be built or loaded, or there
+is no CUDA device, this module raises: there is no CPU fallback and it never touches oracle/.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENUMERIC = 0, 1, 2, 3, 4, 5
+BC_PERIODIC, BC_TRANSMISSIVE, BC_REFLECTIVE, BC_INFLOW = 0, 1, 2, 3
+F64, F32 = 0, 1
+_BC_NAMES = {"periodic": 0, "transmissive": 1, "reflective": 2, "inflow": 3}
+
+EXPORTS = ("jxs_create", "jxs_destroy", "jxs_last_error", "jxs_set_ibm", "jxs_set_flux_mlp",
+           "jxs_set_artificial_viscosity", "jxs_rhs", "jxs_max_wavespeed", "jxs_step", "jxs_step_fixed_dt",
+           "jxs_step_host", "jxs_rhs_host", "jxs_get_time", "jxs_launch_count", "jxs_set_profiling",
+           "jxs_stage_time", "jxs_ibm_ghost_count", "jxs_measure_fp64_peak")
+
+
+class jxs_bc(C.Structure):
+    _fields_ = [("xlo", C.c_int), ("xhi", C.c_int), ("ylo", C.c_int), ("yhi", C.c_int),
+                ("inflow", C.c_double * 4)]
+
+
+class JxsError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"jxs error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load (building first if the sources are newer) paper_2601_04400_b200/libjxs.so."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if os.path.exists(os.path.join(_build.CSRC, "jxs_api.cu")):
+            try:
+                path = _build.build()
+            except Exception:
+                if not os.path.exists(path):
+                    raise
+        L = C.CDLL(path)
+        vp, dp = C.c_void_p, C.POINTER(C.c_double)
+        L.jxs_create.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
+                                 C.POINTER(jxs_bc), C.c_int, vp, C.POINTER(vp)]
+        L.jxs_destroy.argtypes = [vp]
+        L.jxs_destroy.restype = None
+        L.jxs_last_error.argtypes = [vp]
+        L.jxs_last_error.restype = C.c_char_p
+        L.jxs_set_ibm.argtypes = [vp, vp]
+        L.jxs_set_flux_mlp.argtypes = [vp, vp, dp, dp]
+        L.jxs_set_artificial_viscosity.argtypes = [vp, C.c_double]
+        L.jxs_rhs.argtypes = [vp, vp, vp]
+        L.jxs_rhs_host.argtypes = [vp, vp, vp]
+        L.jxs_max_wavespeed.argtypes = [vp, vp, dp]
+        L.jxs_step.argtypes = [vp, vp, C.c_double, C.c_int]
+        L.jxs_step_fixed_dt.argtypes = [vp, vp, C.c_double, C.c_int]
+        L.jxs_step_host.argtypes = [vp, vp, C.c_double, C.c_int]
+        L.jxs_get_time.argtypes = [vp, dp, dp]
+        L.jxs_launch_count.argtypes = [vp]
+        L.jxs_launch_count.restype = C.c_longlong
+        L.jxs_set_profiling.argtypes = [vp, C.c_int]
+        L.jxs_stage_time.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
+        L.jxs_ibm_ghost_count.argtypes = [vp]
+        L.jxs_measure_fp64_peak.argtypes = [vp, C.c_double, dp]
+        _lib = L
+    return _lib
+
+
+def make_bc(bc):
+    b = jxs_bc()
+    for side in ("xlo", "xhi", "ylo", "yhi"):
+        setattr(b, side, _BC_NAMES[bc[side]])
+    inflow = bc.get("inflow", (1.0, 0.0, 0.0, 1.0))
+    for k in range(4):
+        b.inflow[k] = float(inflow[k])
+    return b
+
+
+def measure_fp64_peak(ms=200.0, stream=None):
+    t = C.c_double()
+    st = stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream
+    rc = lib().jxs_measure_fp64_peak(C.c_void_p(st), float(ms), C.byref(t))
+    if rc != OK:
+        raise JxsError(rc, "jxs_measure_fp64_peak")
+    return t.value
+
+
+class Solver:
+    """One jxs_solver handle.  Methods are the C calls of include/jxs.h, name for name."""
+
+    def __init__(self, nx, ny, dx, dy, gamma=1.4, mu=0.0, Pr=0.72, bc=None, dtype=torch.float64, stream=None):
+        if not torch.cuda.is_available():
+            raise JxsError(ECUDA, "no CUDA device: jxs has no CPU fallback")
+        self.nx, self.ny = int(nx), int(ny)
+        self.dtype = dtype
+        assert dtype in (torch.float64, torch.float32)
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        self._bc = make_bc(bc)
+        self._h = C.c_void_p()
+        rc = lib().jxs_create(self.nx, self.ny, float(dx), float(dy), float(gamma), float(mu), float(Pr),
+                              C.byref(self._bc), F64 if dtype == torch.float64 else F32,
+                              C.c_void_p(self.stream.cuda_stream), C.byref(self._h))
+        if rc != OK:
+            raise JxsError(rc, "jxs_create")
+
+    @classmethod
+    def from_case(cls, case, dtype=torch.float64, stream=None):
+        s = cls(case["nx"], case["ny"], case["dx"], case["dy"], case["gamma"], case["mu"], case["Pr"], case["bc"],
+                dtype=dtype, stream=stream)
+        if case.get("phi") is not None:
+            s.set_ibm(case["phi"])
+        return s
+
+    def close(self):
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.jxs_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def _chk(self, rc):
+        if rc != OK:
+            raise JxsError(rc, lib().jxs_last_error(self._h).decode())
+
+    def _dev(self, U):
+        assert isinstance(U, torch.Tensor) and U.is_cuda and U.is_contiguous(), "device tensor expected"
+        assert U.dtype == self.dtype and tuple(U.shape) == (4, self.ny, self.nx), (U.dtype, tuple(U.shape))
+        return C.c_void_p(U.data_ptr())
+
+    def _host(self, U):
+        assert isinstance(U, torch.Tensor) and not U.is_cuda and U.is_contiguous(), "host tensor expected"
+        assert U.dtype == self.dtype and tuple(U.shape) == (4, self.ny, self.nx)
+        return C.c_void_p(U.data_ptr())
+
+    def set_ibm(self, phi):
+        if phi is None:
+            self._chk(lib().jxs_set_ibm(self._h, None))
+            return
+        phi = np.ascontiguousarray(phi, dtype=np.float64)
+        assert phi.shape == (self.ny, self.nx)
+        self._chk(lib().jxs_set_ibm(self._h, phi.ctypes.data))
+
+    def set_flux_mlp(self, weights, in_scale=None, out_scale=None):
+        if weights is None:
+            self._chk(lib().jxs_set_flux_mlp(self._h, None, None, None))
+            return
+        w = np.ascontiguousarray(weights, dtype=np.float32)
+        assert w.shape == (6020,)
+        a = np.ascontiguousarray(in_scale, dtype=np.float64)
+        b = np.ascontiguousarray(out_scale, dtype=np.float64)
+        dp = C.POINTER(C.c_double)
+        self._chk(lib().jxs_set_flux_mlp(self._h, w.ctypes.data, a.ctypes.data_as(dp), b.ctypes.data_as(dp)))
+
+    def set_artificial_viscosity(self, nu):
+        self._chk(lib().jxs_set_artificial_viscosity(self._h, float(nu)))
+
+    def rhs(self, U, dUdt=None):
+        if dUdt is None:
+            dUdt = torch.empty_like(U)
+        self._chk(lib().jxs_rhs(self._h, self._dev(U), self._dev(dUdt)))
+        return dUdt
+
+    def rhs_host(self, U, dUdt=None):
+        if dUdt is None:
+            dUdt = torch.empty_like(U)
+        self._chk(lib().jxs_rhs_host(self._h, self._host(U), self._host(dUdt)))
+        return dUdt
+
+    def max_wavespeed(self, U):
+        s = C.c_double()
+        self._chk(lib().jxs_max_wavespeed(self._h, self._dev(U), C.byref(s)))
+        return s.value
+
+    def step(self, U, cfl, nsteps):
+        """In place on the device tensor U."""
+        self._chk(lib().jxs_step(self._h, self._dev(U), float(cfl), int(nsteps)))
+        return U
+
+    def step_fixed_dt(self, U, dt, nsteps):
+        self._chk(lib().jxs_step_fixed_dt(self._h, self._dev(U), float(dt), int(nsteps)))
+        return U
+
+    def step_host(self, U, cfl, nsteps):
+        """In place on the host tensor U (copies inside the call)."""
+        self._chk(lib().jxs_step_host(self._h, self._host(U), float(cfl), int(nsteps)))
+        return U
+
+    def time(self):
+        t, dt = C.c_double(), C.c_double()
+        self._chk(lib().jxs_get_time(self._h, C.byref(t), C.byref(dt)))
+        return t.value, dt.value
+
+    def launch_count(self):
+        return int(lib().jxs_launch_count(self._h))
+
+    def set_profiling(self, on=True):
+        self._chk(lib().jxs_set_profiling(self._h, int(bool(on))))
+
+    def stage_time(self):
+        ms, n = C.c_double(), C.c_longlong()
+        self._chk(lib().jxs_stage_time(self._h, C.byref(ms), C.byref(n)))
+        return ms.value, int(n.value)
+
+    def ibm_ghost_count(self):
+        return int(lib().jxs_ibm_ghost_count(self._h))
