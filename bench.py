@@ -1,0 +1,275 @@
+#!/usr/bin/env python
+"""bench.py — fp64 Mcell-stage updates/s of the fused WENO5+HLLC(+viscous,+IBM) SSP-RK3 stage on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--dtype f64|f32] [--impl reference]
+
+A "step" is one SSP-RK3 time step = 3 passes of the whole hot path (ghost fills, fused stage kernel,
+CFL reduction) over the 4096x2048 throughput case of BASELINE.json configs[3].  Prints ONE JSON line.
+N > 1 runs N independent replicas (the path does not shard: DESIGN.md section 7), one process per GPU.
+`--impl reference` times the CPU oracle, as it stands, on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "fp64 Mcell-stage updates/s (WENO5+HLLC RHS) and % of stage roofline on 1 B200"
+UNIT = "Mcell-stage/s"
+# algorithmic flops per cell-stage of the Navier-Stokes stage (SURVEY.md section 8(d), low end of the
+# minimal-work count; derivation in DESIGN.md section 6) and compulsory bytes per cell-stage
+ALG_FLOP = {"ns": 1090.0, "euler": 1000.0}
+ALG_BYTES = {"f64": 85.33, "f32": 42.67}
+# FP64 ALU peak derived from unit counts and clocks (B200_PROFILING.md / DESIGN.md section 6):
+# 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz
+PEAK_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+PEAK_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_rate(case, nsteps):
+    """Mcell-stage/s of the CPU oracle (single thread) on `case` for nsteps RK3 steps."""
+    from oracle import jxo
+    o = jxo.Oracle(case["nx"], case["ny"], case["dx"], case["dy"], case["gamma"], case["mu"], case["Pr"], case["bc"])
+    if case.get("phi") is not None:
+        o.set_ibm(case["phi"])
+    t0 = time.perf_counter()
+    o.step(case["U0"], 0.4, nsteps)
+    dt = time.perf_counter() - t0
+    return case["nx"] * case["ny"] * 3 * nsteps / dt / 1e6, dt
+
+
+def run_reference(args, rank):
+    """The reference arm = the oracle on the host cores; rank 0 only."""
+    if rank != 0:
+        return
+    from paper_2601_04400_b200 import workloads as wl
+    from oracle import jxo
+    nx, ny = 512, 256
+    case = wl.throughput_case(nx, ny)
+    o = jxo.Oracle(case["nx"], case["ny"], case["dx"], case["dy"], case["gamma"], case["mu"], case["Pr"], case["bc"])
+    o.set_ibm(case["phi"])
+    U = case["U0"]
+    for _ in range(args.warmup):
+        U = o.step(U, 0.4, 1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        U = o.step(U, 0.4, 1)
+    dt = time.perf_counter() - t0
+    val = nx * ny * 3 * args.steps / dt / 1e6
+    sample = (f"throughput case (8 seeded cylinders, Mach 3, Re 1e5, IBM) generated at {nx}x{ny} instead of 4096x2048; "
+              f"{args.steps} RK3 steps per run, 1 thread")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "throughput_4096x2048 (BASELINE.json configs[3]) sampled at 512x256", "cfl": 0.4},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--dtype", choices=("f64", "f32"), default="f64")
+    ap.add_argument("--impl", choices=("jxs", "reference"), default="jxs")
+    ap.add_argument("--nx", type=int, default=4096)
+    ap.add_argument("--ny", type=int, default=2048)
+    ap.add_argument("--euler", action="store_true", help="mu = 0, no IBM (not the headline config)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "jxs" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import numpy as np
+    import torch
+    from paper_2601_04400_b200 import jxs, workloads as wl
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the jxs path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    tdt = torch.float64 if args.dtype == "f64" else torch.float32
+    case = wl.throughput_case(args.nx, args.ny, viscous=not args.euler, ibm=not args.euler)
+    ncell = args.nx * args.ny
+    stream = torch.cuda.current_stream()
+    solver = jxs.Solver.from_case(case, dtype=tdt, stream=stream)
+    U = torch.tensor(case["U0"], dtype=tdt, device="cuda")
+    K, W = args.steps, args.warmup
+
+    peak_meas = jxs.measure_fp64_peak(200.0) if args.dtype == "f64" else None
+
+    # ---- device-resident timing: inputs already in HBM
+    solver.step(U, 0.4, W)
+    solver.set_profiling(True)
+    sampler = ClockSampler(local_rank)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = solver.launch_count()
+    barrier()
+    sampler.start()
+    e0.record(stream)
+    solver.step(U, 0.4, K)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    launches = solver.launch_count() - launches0
+    ms = e0.elapsed_time(e1)
+    stage_ms, stage_n = solver.stage_time()
+    solver.set_profiling(False)
+    if not bool(torch.isfinite(U).all()):
+        raise SystemExit("bench.py: non-finite state after the timed region")
+    tmax = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_max = float(tmax.item())
+    value = world * ncell * 3 * K / (ms_max * 1e-3) / 1e6
+
+    # ---- end to end through the C ABI with HOST buffers (copies inside the timed region)
+    Uh = torch.tensor(case["U0"], dtype=tdt).pin_memory()
+    solver2 = jxs.Solver.from_case(case, dtype=tdt, stream=stream)
+    solver2.step_host(Uh.clone().pin_memory(), 0.4, 3)
+    barrier()
+    e0.record(stream)
+    solver2.step_host(Uh, 0.4, K)
+    e1.record(stream)
+    barrier()
+    tm2 = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(tm2, op=dist.ReduceOp.MAX)
+    e2e_value = world * ncell * 3 * K / (float(tm2.item()) * 1e-3) / 1e6
+    nbytes = Uh.numel() * Uh.element_size()
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (the fused stage kernel): ALU-bound
+    kind = "euler" if args.euler else "ns"
+    stage_avg_ms = stage_ms / max(stage_n, 1)
+    flops_per_launch = ALG_FLOP[kind] * ncell
+    achieved = flops_per_launch / (stage_avg_ms * 1e-3) / 1e12
+    peak = PEAK_FP64_TFLOPS if args.dtype == "f64" else PEAK_FP32_TFLOPS
+    hbm_gbs = None
+    try:
+        hbm_gbs = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+    except Exception:
+        pass
+    traffic = None
+    try:
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "stage_kernel_traffic.json")))[args.dtype]
+    except Exception:
+        pass
+    roofline = {
+        "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+        "traffic": traffic,
+        "kernel": "jxs::stage_kernel", "avg_launch_ms": stage_avg_ms, "launches_timed": stage_n,
+        "share_of_step": stage_ms / ms,
+        "alg_flop_per_cell_stage": ALG_FLOP[kind], "alg_bytes_per_cell_stage": ALG_BYTES[args.dtype],
+        "peak_source": "derived: 148 SMs x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md section 6)",
+        "peak_measured_dfma_tflops": peak_meas,
+        "frac_of_measured_dfma": (achieved / peak_meas) if peak_meas else None,
+        "hbm_side": {"achieved_gbs": ALG_BYTES[args.dtype] * ncell / (stage_avg_ms * 1e-3) / 1e9,
+                     "peak_gbs": hbm_gbs, "peak_source": "MEASURED_PEAKS.json hbm_gbs" if hbm_gbs else None},
+    }
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        sample_case = wl.throughput_case(1024, 512, viscous=not args.euler, ibm=not args.euler)
+        v, secs = oracle_rate(sample_case, 4)
+        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"the same workload generated at 1024x512, 4 RK3 steps (12 stages), {secs:.1f} s, 1 thread"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": args.dtype, "data": "synthetic",
+        "config": {"workload": f"throughput_{args.nx}x{args.ny}" + ("_euler" if args.euler else
+                   " (BASELINE.json configs[3]: Mach-3 shock over 8 seeded cylinders, Navier-Stokes Re 1e5, IBM)"),
+                   "cfl": 0.4, "rk": "SSP-RK3", "cells": ncell, "stages_per_step": 3,
+                   "l2": "inputs larger than L2 (3 x 256 MiB state buffers vs 126 MB), no flush needed",
+                   "parallelism": "replicas" if world > 1 else "single GPU"},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes / K, "d2h_bytes_per_step": nbytes / K,
+                "note": f"one jxs_step_host call of {K} steps on a pinned host buffer; bytes are the call's copies / {K}"},
+        "gpu_launches": launches,
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
