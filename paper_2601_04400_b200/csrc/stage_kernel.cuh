@@ -86,6 +86,33 @@ __device__ __forceinline__ double sqrt_(double a) { return sqrt(a); }
 __device__ __forceinline__ float sqrt_(float a) { return sqrtf(a); }
 __device__ __forceinline__ double abs_(double a) { return fabs(a); }
 __device__ __forceinline__ float abs_(float a) { return fabsf(a); }
+// Branch-free reciprocal and reciprocal square root.  MUFU.RCP64H / MUFU.RSQ64H are accurate to
+// 2^-20 (measured on B200), so ONE cubic Newton step reaches 1 ulp (max rel. error 2.2e-16 /
+// 2.7e-16 measured over 2^26 arguments).  No slow path: arguments here are densities, pressures,
+// wave-speed differences and WENO denominators, all normal and far from the range limits.
+__device__ __forceinline__ double rcp_(double b) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
+  double e = fma(-b, r, 1.0);
+  e = fma(e, e, e);
+  return fma(r, e, r);
+}
+__device__ __forceinline__ float rcp_(float b) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(b));
+  return r;
+}
+__device__ __forceinline__ double rsqrt_(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double f = fma(-(0.5 * x) * y, y, 0.5);
+  return fma(y, f * fma(1.5, f, 1.0), y);
+}
+__device__ __forceinline__ float rsqrt_(float x) {
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 __device__ __forceinline__ double2 mk2(double a, double b) { return make_double2(a, b); }
 __device__ __forceinline__ float2 mk2(float a, float b) { return make_float2(a, b); }
 
@@ -117,8 +144,8 @@ __device__ __forceinline__ void weno5_cell(T a, T b, T c, T d, T e, T& vm, T& vp
   const T m2 = fma_(T(-2), d2, T(0.5) * d1);
   const T numm = fma_(P01, m0, fma_(P02, m1, P12 * m2));
   const T denm = fma_(T(3), P12, fma_(T(6), P02, P01));
-  vp = c + nump / denp;
-  vm = c + numm / denm;
+  vp = fma_(nump, rcp_(denp), c);
+  vm = fma_(numm, rcp_(denm), c);
 }
 
 // ------------------------------------------------------------------ S5: HLLC, one-sided
@@ -128,17 +155,19 @@ __device__ __forceinline__ void weno5_cell(T a, T b, T c, T d, T e, T& vm, T& vp
 template <typename T>
 __device__ __forceinline__ void hllc(T rL, T unL, T utL, T pL, T rR, T unR, T utR, T pR, T gamma, T g1inv,
                                      T& f0, T& f1, T& f2, T& f3) {
-  const T aL = sqrt_(gamma * pL / rL), aR = sqrt_(gamma * pR / rR);
+  // a = sqrt(gamma p / rho) = (gamma p) * rsqrt(gamma p rho)
+  const T gpL = gamma * pL, gpR = gamma * pR;
+  const T aL = gpL * rsqrt_(gpL * rL), aR = gpR * rsqrt_(gpR * rR);
   const T sL = min_(unL - aL, unR - aR), sR = max_(unL + aL, unR + aR);  // Eq. 6
   const T mL = rL * (sL - unL), mR = rR * (sR - unR);
-  const T sS = (pR - pL + mL * unL - mR * unR) / (mL - mR);              // Eq. 7
+  const T sS = fma_(mL, unL, fma_(-mR, unR, pR - pL)) * rcp_(mL - mR);    // Eq. 7
   const bool left = !(sS < T(0));
   const T r = left ? rL : rR, un = left ? unL : unR, ut = left ? utL : utR, p = left ? pL : pR;
   const T sk = left ? sL : sR;
   const T sc = left ? min_(T(0), sL) : max_(T(0), sR);                    // Eq. 5
   const T E = fma_(T(0.5) * r, fma_(un, un, ut * ut), p * g1inv);
   const T ru = r * un;
-  const T rinv = T(1) / (sk - sS);
+  const T rinv = rcp_(sk - sS);
   const T chi = (sk - un) * rinv;
   const T rchi = r * chi;
   const T dm = fma_(r, chi, -r);                                 // rho* - rho
@@ -236,7 +265,7 @@ __global__ void __launch_bounds__(WARPS * 32) stage_kernel(const StageArgs<T> A)
       V2* dst = ring + slot * NV * ROWV;
       auto convert = [&](int q) {
         const V2 r = raw[q], ru = raw[ROWV + q], rv = raw[2 * ROWV + q], E = raw[3 * ROWV + q];
-        const T i0 = T(1) / r.x, i1 = T(1) / r.y;
+        const T i0 = rcp_(r.x), i1 = rcp_(r.y);
         const T u0 = ru.x * i0, u1 = ru.y * i1, v0 = rv.x * i0, v1 = rv.y * i1;
         const T p0 = g1 * fma_(T(-0.5), fma_(ru.x, u0, rv.x * v0), E.x);
         const T p1 = g1 * fma_(T(-0.5), fma_(ru.y, u1, rv.y * v1), E.y);
@@ -366,10 +395,12 @@ __global__ void __launch_bounds__(WARPS * 32) stage_kernel(const StageArgs<T> A)
     for (int e = 0; e < 2; ++e) {
       const bool badR = !(Rm[0][e] > T(0)) || !(Rm[3][e] > T(0));
       const bool badL = !(Lp[0][e] > T(0)) || !(Lp[3][e] > T(0));
+      if (badR || badL) {  // rare
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        if (badR) Rm[k][e] = wc[k][e];
-        if (badL) Lp[k][e] = wc[k][e];
+        for (int k = 0; k < 4; ++k) {
+          if (badR) Rm[k][e] = wc[k][e];
+          if (badL) Lp[k][e] = wc[k][e];
+        }
       }
     }
     T Fa[4], Fb[4];
@@ -474,10 +505,11 @@ __global__ void __launch_bounds__(WARPS * 32) stage_kernel(const StageArgs<T> A)
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
           const bool use = (e == 0 ? ok0s : ok1) && (e == 0 ? fl0 : fl1);
-          const T ri = T(1) / Un[0][e];
+          const T ri = rcp_(Un[0][e]);
           const T u = Un[1][e] * ri, v = Un[2][e] * ri;
           const T p = g1 * fma_(T(-0.5), fma_(Un[1][e], u, Un[2][e] * v), Un[3][e]);
-          const T a = sqrt_(gamma * p * ri);
+          const T gp = gamma * p;
+          const T a = gp * rsqrt_(gp * Un[0][e]);
           const T s = max_(abs_(u), abs_(v)) + a;
           if (use) smax = (s > smax || s != s) ? s : smax;  // NaN propagates
         }
