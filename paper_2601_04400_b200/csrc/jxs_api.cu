@@ -19,8 +19,9 @@
 using namespace jxs;
 
 namespace {
-constexpr int MAXW = 12;        // warps per CTA of the stage kernel (one CTA per SM)
 constexpr int MAX_EVENTS = 8192;
+// resident one-warp CTAs per SM the stage kernel is compiled for (registers <= 65536/(32*minb))
+template <typename T> constexpr int stage_minb() { return sizeof(T) == 8 ? 20 : 24; }
 }
 
 struct jxs_solver {
@@ -91,7 +92,8 @@ template <typename T> constexpr int sout() { return Cfg<T>::SOUT; }
 void choose_decomposition(jxs_solver* s) {
   const int SOUT = s->dtype == JXS_F64 ? sout<double>() : sout<float>();
   s->nstrips = (s->nx + SOUT - 1) / SOUT;
-  const long long slots = (long long)s->num_sms * MAXW;
+  const int minb = s->dtype == JXS_F64 ? stage_minb<double>() : stage_minb<float>();
+  const long long slots = (long long)s->num_sms * minb;
   double best = 1e300;
   int best_rps = s->ny;
   for (int w = 1; w <= 16; ++w) {
@@ -107,20 +109,20 @@ void choose_decomposition(jxs_solver* s) {
   s->rows_per_seg = best_rps;
   s->nseg = (s->ny + best_rps - 1) / best_rps;
   s->ntasks = s->nseg * s->nstrips;
-  // small problems: fewer warps per CTA so that the CTAs spread over the SMs
-  s->warps = (int)std::min<long long>(MAXW, std::max<long long>(1, (s->ntasks + s->num_sms - 1) / s->num_sms));
-  s->grid = (s->ntasks + s->warps - 1) / s->warps;
+  s->warps = STAGE_WARPS;
+  s->grid = s->ntasks;
 }
 
 template <typename T, bool VISC, bool ARTV>
 cudaError_t launch_stage_t(jxs_solver* s, const StageArgs<T>& a) {
-  auto kern = stage_kernel<T, VISC, ARTV, MAXW>;
+  auto kern = stage_kernel<T, VISC, ARTV, stage_minb<T>()>;
   constexpr int NV = VISC ? 5 : 4;
-  const size_t smem = stage_smem_per_warp<NV>(sizeof(T)) * s->warps;
+  const size_t smem = stage_smem_per_warp<T, NV>();
   static bool configured = false;
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)(stage_smem_per_warp<NV>(sizeof(T)) * MAXW));
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
     configured = true;
   }
@@ -145,6 +147,7 @@ cudaError_t launch_stage(jxs_solver* s, const void* Uin, const void* U0, void* U
   A.kappa = (T)(s->mu > 0 ? s->mu * s->gamma / ((s->gamma - 1.0) * s->Pr) : 0.0);
   A.nu = (T)s->nu;
   A.rk_a = (T)a; A.rk_b = (T)b;
+  A.c133 = (T)(13.0 / 3.0); A.eps4 = (T)4e-6; A.sixth = (T)(1.0 / 6.0); A.c43 = (T)(4.0 / 3.0); A.c23 = (T)(2.0 / 3.0);
   const bool visc = s->mu > 0, artv = s->nu > 0;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (s->profiling && mode == 0 && s->events_used + 2 <= (int)s->events.size()) {
