@@ -77,6 +77,11 @@ int jxs_set_ibm(jxs_solver*, const double* phi_host);
 int jxs_set_flux_mlp(jxs_solver*, const float* weights_host, const double in_scale[4],
                      const double out_scale[4]);
 
+/* The corrections themselves (Eq. 11), for inspection and parity tests: Delta F = out_scale o y of
+ * every face of U after the ghost fills, as fp32 DEVICE arrays dFx[4][ny][nx+1] (face f of row j lies
+ * between cells f-1 and f) and dGy[4][ny+1][nx], components = corrections to the (rho, rho u, rho v, E)
+ * fluxes.  JXS_ESTATE without a network.  Asynchronous.                                     */
+int jxs_flux_correction(jxs_solver*, const void* U, float* dFx, float* dGy);
 /* Laplacian artificial viscosity nu * Lap_h(U) of PAPER.md Eq. 10; default 0 (R7).          */
 int jxs_set_artificial_viscosity(jxs_solver*, double nu);
 
@@ -108,6 +113,8 @@ long long jxs_launch_count(const jxs_solver*);
  * jxs_set_profiling(h, 1) is on (it adds two event records per stage launch).               */
 int jxs_set_profiling(jxs_solver*, int on);
 int jxs_stage_time(const jxs_solver*, double* ms_total, long long* launches);
+/* Same for the flux-MLP kernel (S5').                                                        */
+int jxs_flux_mlp_time(const jxs_solver*, double* ms_total, long long* launches);
 /* Number of IBM ghost cells (0 without a body).                                             */
 int jxs_ibm_ghost_count(const jxs_solver*);
 /* Sustained FP64 FMA rate of the device, in TFLOP/s (2 flops per FMA), from a register-

@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "aux_kernels.cuh"
+#include "flux_mlp_kernel.cuh"
 #include "stage_kernel.cuh"
 
 using namespace jxs;
@@ -43,6 +44,17 @@ struct jxs_solver {
   int* d_donor = nullptr;
   double* d_w = nullptr;
   double* d_nrm = nullptr;
+  // per-face MLP flux correction (S5')
+  bool mlp_on = false;
+  uint8_t* d_mlp_blob = nullptr;
+  float* d_dF = nullptr;   // [4][ny+6][pitch] network outputs at right faces
+  float* d_dG = nullptr;   // same at top faces
+  double in_scale[4] = {1, 1, 1, 1}, out_scale[4] = {1, 1, 1, 1};
+  int mlp_strips = 0, mlp_rows_per_seg = 0, mlp_grid = 0;
+  double mlp_ms = 0;
+  long long mlp_launches = 0;
+  std::vector<cudaEvent_t> mlp_events;
+  int mlp_events_used = 0;
   // stepping state
   StepState* d_state = nullptr;
   double t = 0, last_dt = 0;
@@ -113,9 +125,9 @@ void choose_decomposition(jxs_solver* s) {
   s->grid = s->ntasks;
 }
 
-template <typename T, bool VISC, bool ARTV>
+template <typename T, bool VISC, bool ARTV, bool MLP>
 cudaError_t launch_stage_t(jxs_solver* s, const StageArgs<T>& a) {
-  auto kern = stage_kernel<T, VISC, ARTV, stage_minb<T>()>;
+  auto kern = stage_kernel<T, VISC, ARTV, MLP, stage_minb<T>()>;
   constexpr int NV = VISC ? 5 : 4;
   const size_t smem = stage_smem_per_warp<T, NV>();
   static bool configured = false;
@@ -148,6 +160,9 @@ cudaError_t launch_stage(jxs_solver* s, const void* Uin, const void* U0, void* U
   A.nu = (T)s->nu;
   A.rk_a = (T)a; A.rk_b = (T)b;
   A.c133 = (T)(13.0 / 3.0); A.eps4 = (T)4e-6; A.sixth = (T)(1.0 / 6.0); A.c43 = (T)(4.0 / 3.0); A.c23 = (T)(2.0 / 3.0);
+  A.dF = s->mlp_on ? s->d_dF : nullptr;
+  A.dG = s->mlp_on ? s->d_dG : nullptr;
+  for (int k = 0; k < 4; ++k) A.oscale[k] = (T)s->out_scale[k];
   const bool visc = s->mu > 0, artv = s->nu > 0;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (s->profiling && mode == 0 && s->events_used + 2 <= (int)s->events.size()) {
@@ -156,8 +171,13 @@ cudaError_t launch_stage(jxs_solver* s, const void* Uin, const void* U0, void* U
     cudaEventRecord(e0, s->stream);
   }
   cudaError_t e;
-  if (visc) e = artv ? launch_stage_t<T, true, true>(s, A) : launch_stage_t<T, true, false>(s, A);
-  else e = artv ? launch_stage_t<T, false, true>(s, A) : launch_stage_t<T, false, false>(s, A);
+  if (s->mlp_on) {
+    if (visc) e = artv ? launch_stage_t<T, true, true, true>(s, A) : launch_stage_t<T, true, false, true>(s, A);
+    else e = artv ? launch_stage_t<T, false, true, true>(s, A) : launch_stage_t<T, false, false, true>(s, A);
+  } else {
+    if (visc) e = artv ? launch_stage_t<T, true, true, false>(s, A) : launch_stage_t<T, true, false, false>(s, A);
+    else e = artv ? launch_stage_t<T, false, true, false>(s, A) : launch_stage_t<T, false, false, false>(s, A);
+  }
   if (e1) cudaEventRecord(e1, s->stream);
   s->launches++;
   return e;
@@ -180,6 +200,59 @@ cudaError_t ghost_fill(jxs_solver* s, void* U) {
     ghost_fill_kernel<float><<<(total + bs - 1) / bs, bs, 0, s->stream>>>((float*)U, dims(s), bcspec(s), L, (float)s->gamma);
   s->launches++;
   return cudaGetLastError();
+}
+
+// S5': network outputs of every face of the padded, ghost-filled state U -> d_dF, d_dG
+template <typename T>
+cudaError_t launch_flux_mlp(jxs_solver* s, const void* U) {
+  MlpArgs<T> A;
+  A.U = (const T*)U; A.dF = s->d_dF; A.dG = s->d_dG; A.blob = s->d_mlp_blob;
+  A.plane = s->plane; A.nx = s->nx; A.ny = s->ny; A.pitch = s->pitch;
+  A.nstrips = s->mlp_strips; A.rows_per_seg = s->mlp_rows_per_seg;
+  A.g1 = (T)(s->gamma - 1.0);
+  for (int k = 0; k < 4; ++k) A.inv_scale[k] = (T)(1.0 / s->in_scale[k]);
+  auto kern = flux_mlp_kernel<T>;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, MLP_SMEM);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (s->profiling && s->mlp_events_used + 2 <= (int)s->mlp_events.size()) {
+    e0 = s->mlp_events[s->mlp_events_used++];
+    e1 = s->mlp_events[s->mlp_events_used++];
+    cudaEventRecord(e0, s->stream);
+  }
+  kern<<<s->mlp_grid, MLP_TILE, MLP_SMEM, s->stream>>>(A);
+  if (e1) cudaEventRecord(e1, s->stream);
+  s->launches++;
+  return cudaGetLastError();
+}
+cudaError_t flux_mlp(jxs_solver* s, const void* U) {
+  if (!s->mlp_on) return cudaSuccess;
+  return s->dtype == JXS_F64 ? launch_flux_mlp<double>(s, U) : launch_flux_mlp<float>(s, U);
+}
+
+// fp32 -> bf16 bits, round to nearest even (weights are finite)
+uint16_t bf16_bits(float f) {
+  uint32_t u;
+  std::memcpy(&u, &f, 4);
+  u += 0x7FFFu + ((u >> 16) & 1u);
+  return (uint16_t)(u >> 16);
+}
+// W[N][Kin] (row-major, [out][in]) -> canonical K-major no-swizzle tile [Npad x Kpad] (zero padded):
+// element (n, k) at (n/8)*128 + (k/8)*(Npad*16) + (n%8)*16 + (k%8)*2
+void pack_canonical(const float* W, int N, int Kin, int Npad, int Kpad, uint8_t* dst) {
+  std::memset(dst, 0, (size_t)Npad * Kpad * 2);
+  for (int n = 0; n < N; ++n)
+    for (int k = 0; k < Kin; ++k) {
+      const size_t off = (size_t)(n / 8) * 128 + (size_t)(k / 8) * (Npad * 16) + (n % 8) * 16 + (k % 8) * 2;
+      const uint16_t b = bf16_bits(W[(size_t)n * Kin + k]);
+      std::memcpy(dst + off, &b, 2);
+    }
 }
 
 cudaError_t pad(jxs_solver* s, const void* U, void* dst) {
@@ -221,6 +294,7 @@ int run_steps(jxs_solver* s, double cfl, double fixed_dt, int nsteps) {
   const double h = std::min(s->dx, s->dy);
   int cur = 0;
   s->events_used = 0;
+  s->mlp_events_used = 0;
   if (!(fixed_dt > 0)) CU(wavespeed(s, s->buf[0], &s->d_state->smax_bits[0]));
   for (int n = 0; n < nsteps; ++n) {
     prepare_step_kernel<<<1, 1, 0, s->stream>>>(s->d_state, cur, cfl * h, fixed_dt);
@@ -228,10 +302,13 @@ int run_steps(jxs_solver* s, double cfl, double fixed_dt, int nsteps) {
     CU(cudaGetLastError());
     unsigned long long* next = &s->d_state->smax_bits[cur ^ 1];
     CU(ghost_fill(s, s->buf[0]));
+    CU(flux_mlp(s, s->buf[0]));
     CU(stage(s, s->buf[0], nullptr, s->buf[1], 0, 0.0, 1.0, nullptr));                  // U1 = U0 + dt L(U0)
     CU(ghost_fill(s, s->buf[1]));
+    CU(flux_mlp(s, s->buf[1]));
     CU(stage(s, s->buf[1], s->buf[0], s->buf[2], 0, 0.75, 0.25, nullptr));              // U2 = 3/4 U0 + 1/4 (U1 + dt L(U1))
     CU(ghost_fill(s, s->buf[2]));
+    CU(flux_mlp(s, s->buf[2]));
     CU(stage(s, s->buf[2], s->buf[0], s->buf[0], 0, 1.0 / 3.0, 2.0 / 3.0, next));       // U0 = 1/3 U0 + 2/3 (U2 + dt L(U2))
     cur ^= 1;
   }
@@ -251,6 +328,13 @@ int finish_steps(jxs_solver* s, int nsteps) {
       float ms = 0;
       cudaEventElapsedTime(&ms, s->events[i], s->events[i + 1]);
       s->stage_ms += ms;
+    }
+    s->mlp_ms = 0;
+    s->mlp_launches = s->mlp_events_used / 2;
+    for (int i = 0; i + 1 < s->mlp_events_used; i += 2) {
+      float ms = 0;
+      cudaEventElapsedTime(&ms, s->mlp_events[i], s->mlp_events[i + 1]);
+      s->mlp_ms += ms;
     }
   }
   if (st.bad) {
@@ -351,7 +435,9 @@ void jxs_destroy(jxs_solver* s) {
   cudaFree(s->stage_io);
   cudaFree(s->d_state);
   free_ibm(s);
+  cudaFree(s->d_mlp_blob); cudaFree(s->d_dF); cudaFree(s->d_dG);
   for (cudaEvent_t ev : s->events) cudaEventDestroy(ev);
+  for (cudaEvent_t ev : s->mlp_events) cudaEventDestroy(ev);
   delete s;
 }
 
@@ -437,9 +523,38 @@ int jxs_set_ibm(jxs_solver* s, const double* phi) {
 
 int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[4], const double out_scale[4]) {
   if (!s) return JXS_EINVAL;
-  if (!weights) return JXS_OK;
-  (void)in_scale; (void)out_scale;
-  return fail(s, JXS_ESTATE, "per-face MLP flux correction is not built yet");
+  CU(cudaStreamSynchronize(s->stream));
+  if (!weights) { s->mlp_on = false; return JXS_OK; }
+  if (!in_scale || !out_scale) return fail(s, JXS_EINVAL, "in_scale / out_scale is NULL");
+  for (int k = 0; k < 4; ++k)
+    if (!(in_scale[k] > 0) || !std::isfinite(in_scale[k]) || !std::isfinite(out_scale[k]))
+      return fail(s, JXS_EINVAL, "in_scale must be > 0 and out_scale finite");
+  for (int i = 0; i < 6020; ++i)
+    if (!std::isfinite(weights[i])) return fail(s, JXS_EINVAL, "non-finite MLP weight");
+  // W1[64][24], b1[64], W2[64][64], b2[64], W3[4][64], b3[4] -> bf16 tiles in the tensor-core layout + fp32 biases
+  std::vector<uint8_t> blob(MLP_BLOB, 0);
+  const float *W1 = weights, *b1 = W1 + 64 * 24, *W2 = b1 + 64, *b2 = W2 + 64 * 64, *W3 = b2 + 64, *b3 = W3 + 4 * 64;
+  pack_canonical(W1, 64, 24, 64, 32, blob.data() + MLP_OFF_W1);
+  pack_canonical(W2, 64, 64, 64, 64, blob.data() + MLP_OFF_W2);
+  pack_canonical(W3, 4, 64, 16, 64, blob.data() + MLP_OFF_W3);
+  float* bias = reinterpret_cast<float*>(blob.data() + MLP_OFF_BIAS);
+  std::memcpy(bias, b1, 64 * 4); std::memcpy(bias + 64, b2, 64 * 4); std::memcpy(bias + 128, b3, 4 * 4);
+  const size_t fbytes = (size_t)4 * s->plane * sizeof(float);
+  if (!s->d_mlp_blob) CU(cudaMalloc(&s->d_mlp_blob, MLP_BLOB));
+  if (!s->d_dF) { CU(cudaMalloc(&s->d_dF, fbytes)); CU(cudaMemset(s->d_dF, 0, fbytes)); }
+  if (!s->d_dG) { CU(cudaMalloc(&s->d_dG, fbytes)); CU(cudaMemset(s->d_dG, 0, fbytes)); }
+  CU(cudaMemcpy(s->d_mlp_blob, blob.data(), MLP_BLOB, cudaMemcpyHostToDevice));
+  for (int k = 0; k < 4; ++k) { s->in_scale[k] = in_scale[k]; s->out_scale[k] = out_scale[k]; }
+  // strips of 128 faces x row segments: fill 3 resident CTAs per SM, 5 warm-up rows per segment
+  s->mlp_strips = (s->nx + 1 + MLP_TILE - 1) / MLP_TILE;
+  const int nrows = s->ny + 1;
+  const long long slots = (long long)s->num_sms * 3;
+  int segs = (int)std::max<long long>(1, slots / s->mlp_strips);
+  int rps = std::max((nrows + segs - 1) / segs, std::min(nrows, 16));
+  s->mlp_rows_per_seg = rps;
+  s->mlp_grid = s->mlp_strips * ((nrows + rps - 1) / rps);
+  s->mlp_on = true;
+  return JXS_OK;
 }
 
 int jxs_set_artificial_viscosity(jxs_solver* s, double nu) {
@@ -454,6 +569,7 @@ int jxs_rhs(jxs_solver* s, const void* U, void* dUdt) {
   if (!U || !dUdt) return fail(s, JXS_EINVAL, "NULL array");
   CU(pad(s, U, s->buf[0]));
   CU(ghost_fill(s, s->buf[0]));
+  CU(flux_mlp(s, s->buf[0]));
   CU(stage(s, s->buf[0], nullptr, dUdt, 1, 0.0, 1.0, nullptr));
   return JXS_OK;
 }
@@ -465,6 +581,7 @@ int jxs_rhs_host(jxs_solver* s, const void* U, void* dUdt) {
   CU(cudaMemcpyAsync(s->stage_io, U, bytes, cudaMemcpyHostToDevice, s->stream));
   CU(pad(s, s->stage_io, s->buf[0]));
   CU(ghost_fill(s, s->buf[0]));
+  CU(flux_mlp(s, s->buf[0]));
   CU(stage(s, s->buf[0], nullptr, s->stage_io, 1, 0.0, 1.0, nullptr));
   CU(cudaMemcpyAsync(dUdt, s->stage_io, bytes, cudaMemcpyDeviceToHost, s->stream));
   CU(cudaStreamSynchronize(s->stream));
@@ -508,6 +625,8 @@ int jxs_set_profiling(jxs_solver* s, int on) {
   if (s->profiling && s->events.empty()) {
     s->events.resize(MAX_EVENTS);
     for (cudaEvent_t& ev : s->events) CU(cudaEventCreate(&ev));
+    s->mlp_events.resize(MAX_EVENTS);
+    for (cudaEvent_t& ev : s->mlp_events) CU(cudaEventCreate(&ev));
   }
   return JXS_OK;
 }
@@ -520,6 +639,28 @@ int jxs_stage_time(const jxs_solver* s, double* ms_total, long long* launches) {
 }
 
 int jxs_ibm_ghost_count(const jxs_solver* s) { return s ? s->n_ghost : -1; }
+
+int jxs_flux_mlp_time(const jxs_solver* s, double* ms_total, long long* launches) {
+  if (!s) return JXS_EINVAL;
+  if (ms_total) *ms_total = s->mlp_ms;
+  if (launches) *launches = s->mlp_launches;
+  return JXS_OK;
+}
+
+int jxs_flux_correction(jxs_solver* s, const void* U, float* dFx, float* dGy) {
+  if (!s) return JXS_EINVAL;
+  if (!U || !dFx || !dGy) return fail(s, JXS_EINVAL, "NULL array");
+  if (!s->mlp_on) return fail(s, JXS_ESTATE, "no MLP set (jxs_set_flux_mlp)");
+  CU(pad(s, U, s->buf[0]));
+  CU(ghost_fill(s, s->buf[0]));
+  CU(flux_mlp(s, s->buf[0]));
+  const int bs = 256, gs = s->num_sms * 8;
+  gather_faces_kernel<<<gs, bs, 0, s->stream>>>(s->d_dF, s->d_dG, dFx, dGy, dims(s), s->out_scale[0], s->out_scale[1],
+                                                 s->out_scale[2], s->out_scale[3]);
+  s->launches++;
+  CU(cudaGetLastError());
+  return JXS_OK;
+}
 
 int jxs_measure_fp64_peak(void* cuda_stream, double ms, double* tflops) {
   if (!tflops || !(ms > 0)) return JXS_EINVAL;

@@ -52,6 +52,11 @@ struct StageArgs {
   // Literals that are not exact in the upper 32 bits of a double cannot be SASS immediates; as
   // kernel parameters they are constant-bank operands (no registers, no moves).
   T c133, eps4, sixth, c43, c23;  // 13/3, 4e-6, 1/6, 4/3, 2/3
+  // S5' (optional): network outputs y per face from flux_mlp_kernel, padded indexing [4][ny+6][pitch]:
+  // dF = right face, dG = top face of the cell; k = (mass, normal, tangential momentum, energy) (R14)
+  const float* dF;
+  const float* dG;
+  T oscale[4];
 };
 
 
@@ -207,7 +212,7 @@ __host__ __device__ constexpr size_t stage_smem_per_warp() {
 }
 
 // ------------------------------------------------------------------ the kernel
-template <typename T, bool VISC, bool ARTV, int MINB>
+template <typename T, bool VISC, bool ARTV, bool MLP, int MINB>
 __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const StageArgs<T> A) {
   constexpr int SOUT = Cfg<T>::SOUT;
   constexpr int NV = VISC ? 5 : 4;
@@ -311,6 +316,12 @@ __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const Sta
     const bool do_out = it >= 6;  // rows jo >= jbeg
     const unsigned fl = fl_next;
     if (it >= 5 && n < nlast && A.fluid && ic < A.nx) fl_next = A.fluid[(size_t)(jo + 1 - 3) * A.nx + ic];
+    float yF[4], yG[4];  // S5': network outputs at my right face and my top face (row jo)
+    if (MLP && it >= 5) {
+      const size_t o = (size_t)jo * A.pitch + (w0 + lane);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) { yF[k] = __ldg(A.dF + k * A.plane + o); yG[k] = __ldg(A.dG + k * A.plane + o); }
+    }
 
     // ---------------------------------------------------------------- S4/S5 along y
     T Ly_div[4];  // G_bottom - G_top of the output row, per component
@@ -336,6 +347,10 @@ __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const Sta
         T f0, f1, f2, f3;  // face between rows jo and jc: normal = y
         hllc(Ly[0], Ly[2], Ly[1], Ly[3], Ry[0], Ry[2], Ry[1], Ry[3], gamma, g1inv, f0, f1, f2, f3);
         T G[4] = {f0, f2, f1, f3};
+        if (MLP) {  // Eq. 11: normal momentum of a y-face is rho*v
+          G[0] = fma_(A.oscale[0], T(yG[0]), G[0]); G[1] = fma_(A.oscale[2], T(yG[2]), G[1]);
+          G[2] = fma_(A.oscale[1], T(yG[1]), G[2]); G[3] = fma_(A.oscale[3], T(yG[3]), G[3]);
+        }
         if (VISC) {  // S6 (R8): G^v = (0, tau_xy, tau_yy, u tau_xy + v tau_yy + k T_y)
           const T uB = rowB[CW + q], uC = rowC[CW + q], vB = rowB[2 * CW + q], vC = rowC[2 * CW + q];
           const T uy = (uC - uB) * A.dyi, vy = (vC - vB) * A.dyi;
@@ -380,6 +395,10 @@ __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const Sta
         }
         const T r0 = shfl_down1(Rm[0]), r1 = shfl_down1(Rm[1]), r2 = shfl_down1(Rm[2]), r3 = shfl_down1(Rm[3]);
         hllc(Lp[0], Lp[1], Lp[2], Lp[3], r0, r1, r2, r3, gamma, g1inv, F[0], F[1], F[2], F[3]);
+        if (MLP) {
+#pragma unroll
+          for (int k = 0; k < 4; ++k) F[k] = fma_(A.oscale[k], T(yF[k]), F[k]);  // Eq. 11
+        }
       }
       if (VISC) {  // S6 (R8): F^v = (0, tau_xx, tau_xy, u tau_xx + v tau_xy + k T_x) at my right face
         const T u1 = rowB[CW + q + 1], v1 = rowB[2 * CW + q + 1];

@@ -20,7 +20,8 @@ _BC_NAMES = {"periodic": 0, "transmissive": 1, "reflective": 2, "inflow": 3}
 EXPORTS = ("jxs_create", "jxs_destroy", "jxs_last_error", "jxs_set_ibm", "jxs_set_flux_mlp",
            "jxs_set_artificial_viscosity", "jxs_rhs", "jxs_max_wavespeed", "jxs_step", "jxs_step_fixed_dt",
            "jxs_step_host", "jxs_rhs_host", "jxs_get_time", "jxs_launch_count", "jxs_set_profiling",
-           "jxs_stage_time", "jxs_ibm_ghost_count", "jxs_measure_fp64_peak")
+           "jxs_stage_time", "jxs_ibm_ghost_count", "jxs_measure_fp64_peak", "jxs_flux_correction",
+           "jxs_flux_mlp_time")
 
 
 class jxs_bc(C.Structure):
@@ -72,6 +73,8 @@ def lib():
         L.jxs_stage_time.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
         L.jxs_ibm_ghost_count.argtypes = [vp]
         L.jxs_measure_fp64_peak.argtypes = [vp, C.c_double, dp]
+        L.jxs_flux_correction.argtypes = [vp, vp, vp, vp]
+        L.jxs_flux_mlp_time.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
         _lib = L
     return _lib
 
@@ -160,6 +163,19 @@ class Solver:
         b = np.ascontiguousarray(out_scale, dtype=np.float64)
         dp = C.POINTER(C.c_double)
         self._chk(lib().jxs_set_flux_mlp(self._h, w.ctypes.data, a.ctypes.data_as(dp), b.ctypes.data_as(dp)))
+
+    def flux_correction(self, U):
+        """(dFx [4, ny, nx+1], dGy [4, ny+1, nx]) fp32 device tensors: Eq. 11's Delta F at every face."""
+        dFx = torch.empty((4, self.ny, self.nx + 1), dtype=torch.float32, device=U.device)
+        dGy = torch.empty((4, self.ny + 1, self.nx), dtype=torch.float32, device=U.device)
+        self._chk(lib().jxs_flux_correction(self._h, self._dev(U), C.c_void_p(dFx.data_ptr()),
+                                            C.c_void_p(dGy.data_ptr())))
+        return dFx, dGy
+
+    def flux_mlp_time(self):
+        ms, n = C.c_double(), C.c_longlong()
+        self._chk(lib().jxs_flux_mlp_time(self._h, C.byref(ms), C.byref(n)))
+        return ms.value, int(n.value)
 
     def set_artificial_viscosity(self, nu):
         self._chk(lib().jxs_set_artificial_viscosity(self._h, float(nu)))
