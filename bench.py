@@ -29,6 +29,23 @@ ALG_BYTES = {"f64": 85.33, "f32": 42.67}
 # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz
 PEAK_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 PEAK_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+# dram__bytes_read.sum + dram__bytes_write.sum of the stage kernel, per launch, mean of the three RK stages, from
+# the `ncu --set full` capture summarised in profiles/r01b_stage_f64.md (fp64, 4096x2048); None = not captured
+NCU_TRAFFIC_BYTES = {("f64", 4096, 2048, "ns"): (528.7e6 + 821.2e6 + 800.1e6) / 3}
+
+
+def max_over_ranks(ms, dist, device):
+    """Timing of the slowest rank (torch.distributed MAX all-reduce; identity for a single process)."""
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_rate(ncell, steps, world, ms_max):
+    """Whole-job Mcell-stage/s of `world` replicas that each advanced ncell cells by `steps` RK3 steps."""
+    return world * ncell * 3 * steps / (ms_max * 1e-3) / 1e6
 
 
 class ClockSampler:
@@ -188,11 +205,8 @@ def main():
     solver.set_profiling(False)
     if not bool(torch.isfinite(U).all()):
         raise SystemExit("bench.py: non-finite state after the timed region")
-    tmax = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_max = float(tmax.item())
-    value = world * ncell * 3 * K / (ms_max * 1e-3) / 1e6
+    ms_max = max_over_ranks(ms, dist, "cuda")
+    value = aggregate_rate(ncell, K, world, ms_max)
 
     # ---- end to end through the C ABI with HOST buffers (copies inside the timed region)
     Uh = torch.tensor(case["U0"], dtype=tdt).pin_memory()
@@ -203,10 +217,7 @@ def main():
     solver2.step_host(Uh, 0.4, K)
     e1.record(stream)
     barrier()
-    tm2 = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(tm2, op=dist.ReduceOp.MAX)
-    e2e_value = world * ncell * 3 * K / (float(tm2.item()) * 1e-3) / 1e6
+    e2e_value = aggregate_rate(ncell, K, world, max_over_ranks(e0.elapsed_time(e1), dist, "cuda"))
     nbytes = Uh.numel() * Uh.element_size()
 
     if rank != 0:
@@ -225,14 +236,10 @@ def main():
         hbm_gbs = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
     except Exception:
         pass
-    traffic = None
-    try:
-        traffic = json.load(open(os.path.join(ROOT, "profiles", "stage_kernel_traffic.json")))[args.dtype]
-    except Exception:
-        pass
+    traffic = NCU_TRAFFIC_BYTES.get((args.dtype, args.nx, args.ny, kind))
     roofline = {
         "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-        "traffic": traffic,
+        "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r01b_stage_f64.md)",
         "kernel": "jxs::stage_kernel", "avg_launch_ms": stage_avg_ms, "launches_timed": stage_n,
         "share_of_step": stage_ms / ms,
         "alg_flop_per_cell_stage": ALG_FLOP[kind], "alg_bytes_per_cell_stage": ALG_BYTES[args.dtype],
