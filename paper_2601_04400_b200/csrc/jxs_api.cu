@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <new>
 #include <string>
 #include <vector>
@@ -22,7 +23,10 @@ using namespace jxs;
 namespace {
 constexpr int MAX_EVENTS = 8192;
 // resident one-warp CTAs per SM the stage kernel is compiled for (registers <= 65536/(32*minb))
-template <typename T> constexpr int stage_minb() { return sizeof(T) == 8 ? 20 : 24; }
+#ifndef JXS_MINB_F64
+#define JXS_MINB_F64 16
+#endif
+template <typename T> constexpr int stage_minb() { return sizeof(T) == 8 ? JXS_MINB_F64 : 24; }
 }
 
 struct jxs_solver {
@@ -138,7 +142,9 @@ cudaError_t launch_stage_t(jxs_solver* s, const StageArgs<T>& a) {
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  kern<<<s->grid, s->warps * 32, smem, s->stream>>>(a);
+  static const size_t extra = getenv("JXS_DBG_EXTRA_SMEM") ? (size_t)atoi(getenv("JXS_DBG_EXTRA_SMEM")) : 0;
+  if (extra) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem + extra));
+  kern<<<s->grid, s->warps * 32, smem + extra, s->stream>>>(a);
   return cudaGetLastError();
 }
 
@@ -159,7 +165,15 @@ cudaError_t launch_stage(jxs_solver* s, const void* Uin, const void* U0, void* U
   A.kappa = (T)(s->mu > 0 ? s->mu * s->gamma / ((s->gamma - 1.0) * s->Pr) : 0.0);
   A.nu = (T)s->nu;
   A.rk_a = (T)a; A.rk_b = (T)b;
-  A.c133 = (T)(13.0 / 3.0); A.eps4 = (T)4e-6; A.sixth = (T)(1.0 / 6.0); A.c43 = (T)(4.0 / 3.0); A.c23 = (T)(2.0 / 3.0);
+  A.c133 = (T)(13.0 / 3.0); A.eps4 = (T)4e-6; A.sixth = (T)(1.0 / 6.0);
+  {
+    const double mu = s->mu, kap = s->mu > 0 ? s->mu * s->gamma / ((s->gamma - 1.0) * s->Pr) : 0.0;
+    const double dxi = 1.0 / s->dx, dyi = 1.0 / s->dy;
+    A.vy_n = (T)(4.0 / 3.0 * mu * dyi); A.vy_c = (T)(2.0 / 3.0 * mu * 0.25 * dxi); A.vy_s = (T)(mu * dyi);
+    A.vy_t = (T)(mu * 0.25 * dxi); A.vy_q = (T)(kap * dyi);
+    A.vx_n = (T)(4.0 / 3.0 * mu * dxi); A.vx_c = (T)(2.0 / 3.0 * mu * 0.25 * dyi); A.vx_s = (T)(mu * dxi);
+    A.vx_t = (T)(mu * 0.25 * dyi); A.vx_q = (T)(kap * dxi);
+  }
   A.dF = s->mlp_on ? s->d_dF : nullptr;
   A.dG = s->mlp_on ? s->d_dG : nullptr;
   for (int k = 0; k < 4; ++k) A.oscale[k] = (T)s->out_scale[k];

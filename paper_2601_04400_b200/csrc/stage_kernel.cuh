@@ -51,7 +51,12 @@ struct StageArgs {
   T rk_a, rk_b;          // Uout = a*U0 + b*(Uin + dt*L)
   // Literals that are not exact in the upper 32 bits of a double cannot be SASS immediates; as
   // kernel parameters they are constant-bank operands (no registers, no moves).
-  T c133, eps4, sixth, c43, c23;  // 13/3, 4e-6, 1/6, 4/3, 2/3
+  T c133, eps4, sixth;  // 13/3, 4e-6, 1/6
+  // viscous-flux coefficients with mu, kappa, the grid spacings and the 1/4 of the averaged tangential
+  // derivative folded in (R8): normal stress, cross derivative in the normal stress, shear (normal and
+  // tangential part), heat flux; n = the face's normal direction
+  T vy_n, vy_c, vy_s, vy_t, vy_q;  // y-faces: 4/3 mu/dy, (2/3) mu/(4 dx), mu/dy, mu/(4 dx), kappa/dy
+  T vx_n, vx_c, vx_s, vx_t, vx_q;  // x-faces: 4/3 mu/dx, (2/3) mu/(4 dy), mu/dx, mu/(4 dy), kappa/dx
   // S5' (optional): network outputs y per face from flux_mlp_kernel, padded indexing [4][ny+6][pitch]:
   // dF = right face, dG = top face of the cell; k = (mass, normal, tangential momentum, energy) (R14)
   const float* dF;
@@ -84,6 +89,14 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
                  : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
   } while (!ok);
+}
+
+// one lane of the (converged) warp, chosen by the hardware: ptxas then keeps the bulk copies on the
+// uniform datapath instead of looping over "every active lane"
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n.reg .pred p;\nelect.sync _|p, 0xffffffff;\nselp.u32 %0, 1, 0, p;\n}" : "=r"(pred));
+  return pred != 0;
 }
 
 // ------------------------------------------------------------------ scalar helpers
@@ -153,9 +166,17 @@ __device__ __forceinline__ void weno5_cell(T a, T b, T c, T d, T e, const StageA
   const T denp = fma_(T(2), P01, h), denm = fma_(T(2), P12, h);
   const T A = P12 * (s0 - s1), C = P01 * (s1 - s2);
   // 6 (vp - c) = (d2 + 2 d3) + (2A + 3C)/denp,   6 (c - vm) = (d3 + 2 d2) + (2C + 3A)/denm
-  const T np = fma_(T(2), A, T(3) * C), nm = fma_(T(2), C, T(3) * A);
-  const T ep = fma_(np, rcp_(denp), fma_(T(2), d3, d2));
-  const T em = fma_(nm, rcp_(denm), fma_(T(2), d2, d3));
+  const T S = A + C;
+  const T np = fma_(T(2), S, C), nm = fma_(T(2), S, A);
+  T rp, rm;
+  if (sizeof(T) == 8) {  // one reciprocal for both sides (the product stays far inside the fp64 range)
+    const T r = rcp_(denp * denm);
+    rp = r * denm; rm = r * denp;
+  } else {
+    rp = rcp_(denp); rm = rcp_(denm);
+  }
+  const T ep = fma_(np, rp, fma_(T(2), d3, d2));
+  const T em = fma_(nm, rm, fma_(T(2), d2, d3));
   vp = fma_(K.sixth, ep, c);
   vm = fma_(-K.sixth, em, c);
 }
@@ -262,7 +283,7 @@ __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const Sta
       for (int k = 0; k < 4; ++k) tma_bulk_g2s(epi_u32 + (4 + k) * EROWB, A.U0 + o + k * A.plane, EROWB, bar_epi);
     }
   };
-  if (lane == 0) issue_row(nfirst);
+  if (elect_one()) issue_row(nfirst);
 
   const T gamma = A.gamma, g1inv = A.g1inv, g1 = A.g1;
   const T dtv = T(*A.dt);
@@ -272,44 +293,47 @@ __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const Sta
   T Gp[4];  // total y-flux (rho, rho u, rho v, E) through the face below the output row
 #pragma unroll
   for (int k = 0; k < 4; ++k) { Ly[k] = T(0); Gp[k] = T(0); }
+  T cuP = T(0), cvP = T(0);
   T smax = T(0);
   unsigned fl_next = 1;  // fluid flag of my cell in the next output row, fetched one iteration ahead
 
-  int slot = 0;  // ring slot of the newest row
+  // Ring rows as loop-carried per-lane pointers (to my column q), rotated once per iteration: the row
+  // accesses below become LDS with immediate offsets, no slot arithmetic.  pN = slot written next.
+  T* pN = ring + q;
+  const T *pA = ring + 1 * NV * CW + q, *pB = ring + 2 * NV * CW + q, *pC = ring + 3 * NV * CW + q,
+          *pD = ring + 4 * NV * CW + q;
+  const int hoff = lane < 2 ? -2 : LW - 2;  // my halo column (lanes 0-3 convert one each), relative to q
   for (int n = nfirst; n <= nlast; ++n) {
     const int it = n - nfirst;
     // ---------------------------------------------------------------- S3: new row -> primitives
     __syncwarp();  // every lane is done reading the ring slot that is overwritten now
     mbar_wait(bar_raw, it & 1);
     {
-      T* dst = ring + slot * NV * CW;
-      auto convert = [&](int c) {
-        const T r = raw[c], ru = raw[CW + c], rv = raw[2 * CW + c], E = raw[3 * CW + c];
+      auto convert = [&](int o) {  // o = column relative to q
+        const T* src = raw + q + o;
+        const T r = src[0], ru = src[CW], rv = src[2 * CW], E = src[3 * CW];
         const T ri = rcp_(r);
         const T u = ru * ri, v = rv * ri;
         const T p = g1 * fma_(T(-0.5), fma_(ru, u, rv * v), E);
-        dst[c] = r;
-        dst[CW + c] = u;
-        dst[2 * CW + c] = v;
-        dst[3 * CW + c] = p;
-        if (VISC) dst[4 * CW + c] = p * ri;
+        T* dst = pN + o;
+        dst[0] = r;
+        dst[CW] = u;
+        dst[2 * CW] = v;
+        dst[3 * CW] = p;
+        if (VISC) dst[4 * CW] = p * ri;
       };
-      convert(q);
-      if (lane < 4) convert(lane < 2 ? lane : LW + lane);
+      convert(0);
+      if (lane < 4) convert(hoff);
       __syncwarp();
-      if (lane == 0 && n < nlast) issue_row(n + 1);
+      if (n < nlast && elect_one()) issue_row(n + 1);
     }
-    // ring rows n-4 .. n  (valid once it >= 4)
-    const T *rowA, *rowB, *rowC, *rowD, *rowE;
+    // ring rows n-4 .. n  (valid once it >= 4): A = n-4, B = n-3 = jo (output row), C = n-2 = jc
+    // (centre of the y stencil), D = n-1, E = n
+    const T *rowA = pA - q, *rowB = pB - q, *rowC = pC - q, *rowD = pD - q, *rowE = pN - q;
     {
-      int s = slot;
-      rowE = ring + s * NV * CW; s = s == 0 ? RING - 1 : s - 1;  // n
-      rowD = ring + s * NV * CW; s = s == 0 ? RING - 1 : s - 1;  // n-1
-      rowC = ring + s * NV * CW; s = s == 0 ? RING - 1 : s - 1;  // n-2 = jc (centre of the y stencil)
-      rowB = ring + s * NV * CW; s = s == 0 ? RING - 1 : s - 1;  // n-3 = jo (output row)
-      rowA = ring + s * NV * CW;                                 // n-4
+      T* const oldest = const_cast<T*>(pA);
+      pA = pB; pB = pC; pC = pD; pD = pN; pN = oldest;
     }
-    slot = slot + 1 == RING ? 0 : slot + 1;
     if (it < 4) continue;
 
     const int jo = n - 3;
@@ -336,12 +360,18 @@ __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const Sta
       const bool badR = not_positive(Ry[0]) | not_positive(Ry[3]);
       const bool badL = not_positive(Lnew[0]) | not_positive(Lnew[3]);
       if (__any_sync(0xffffffffu, badR | badL)) {
+        asm volatile("" ::: "memory");  // keeps this (never taken in practice) block a branch, not 16 selects
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
           const T cv = rowC[k * CW + q];
           Ry[k] = badR ? cv : Ry[k];
           Lnew[k] = badL ? cv : Lnew[k];
         }
+      }
+      T cuC, cvC;  // x-centred differences of u, v in row jc; cuP, cvP: the same for row jo (carried)
+      if (VISC) {
+        cuC = rowC[CW + q + 1] - rowC[CW + q - 1];
+        cvC = rowC[2 * CW + q + 1] - rowC[2 * CW + q - 1];
       }
       if (it >= 5) {
         T f0, f1, f2, f3;  // face between rows jo and jc: normal = y
@@ -353,23 +383,20 @@ __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const Sta
         }
         if (VISC) {  // S6 (R8): G^v = (0, tau_xy, tau_yy, u tau_xy + v tau_yy + k T_y)
           const T uB = rowB[CW + q], uC = rowC[CW + q], vB = rowB[2 * CW + q], vC = rowC[2 * CW + q];
-          const T uy = (uC - uB) * A.dyi, vy = (vC - vB) * A.dyi;
-          const T Ty = (rowC[4 * CW + q] - rowB[4 * CW + q]) * A.dyi;
-          const T cuB = rowB[CW + q + 1] - rowB[CW + q - 1], cuC = rowC[CW + q + 1] - rowC[CW + q - 1];
-          const T cvB = rowB[2 * CW + q + 1] - rowB[2 * CW + q - 1], cvC = rowC[2 * CW + q + 1] - rowC[2 * CW + q - 1];
-          const T ux = T(0.25) * (cuB + cuC) * A.dxi, vx = T(0.25) * (cvB + cvC) * A.dxi;
-          const T tyy = A.mu * fma_(A.c43, vy, -(A.c23 * ux));
-          const T txy = A.mu * (uy + vx);
-          const T ub = T(0.5) * (uB + uC), vb = T(0.5) * (vB + vC);
+          const T dT = rowC[4 * CW + q] - rowB[4 * CW + q];
+          const T tyy = fma_(A.vy_n, vC - vB, -(A.vy_c * (cuP + cuC)));
+          const T txy = fma_(A.vy_s, uC - uB, A.vy_t * (cvP + cvC));
           G[1] -= txy;
           G[2] -= tyy;
-          G[3] -= fma_(ub, txy, fma_(vb, tyy, A.kappa * Ty));
+          const T w = fma_(vB + vC, tyy, (uB + uC) * txy);  // 2 (u tau_xy + v tau_yy) at the face
+          G[3] = fma_(-A.vy_q, dT, fma_(T(-0.5), w, G[3]));
         }
 #pragma unroll
         for (int k = 0; k < 4; ++k) { Ly_div[k] = Gp[k] - G[k]; Gp[k] = G[k]; }
       }
 #pragma unroll
       for (int k = 0; k < 4; ++k) Ly[k] = Lnew[k];
+      if (VISC) { cuP = cuC; cvP = cvC; }
     }
 
     if (do_out) {
@@ -387,6 +414,7 @@ __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const Sta
         const bool badR = not_positive(Rm[0]) | not_positive(Rm[3]);
         const bool badL = not_positive(Lp[0]) | not_positive(Lp[3]);
         if (__any_sync(0xffffffffu, badR | badL)) {
+          asm volatile("" ::: "memory");
 #pragma unroll
           for (int k = 0; k < 4; ++k) {
             Rm[k] = badR ? wc[k] : Rm[k];
@@ -402,18 +430,17 @@ __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const Sta
       }
       if (VISC) {  // S6 (R8): F^v = (0, tau_xx, tau_xy, u tau_xx + v tau_xy + k T_x) at my right face
         const T u1 = rowB[CW + q + 1], v1 = rowB[2 * CW + q + 1];
-        const T ux = (u1 - wc[1]) * A.dxi, vx = (v1 - wc[2]) * A.dxi;
-        const T Tx = (rowB[4 * CW + q + 1] - rowB[4 * CW + q]) * A.dxi;
-        // y-centred differences (rows jo+1 = jc and jo-1) at my cell and at the right neighbour
-        const T cu0 = rowC[CW + q] - rowA[CW + q], cu1 = rowC[CW + q + 1] - rowA[CW + q + 1];
-        const T cv0 = rowC[2 * CW + q] - rowA[2 * CW + q], cv1 = rowC[2 * CW + q + 1] - rowA[2 * CW + q + 1];
-        const T uy = T(0.25) * (cu0 + cu1) * A.dyi, vy = T(0.25) * (cv0 + cv1) * A.dyi;
-        const T txx = A.mu * fma_(A.c43, ux, -(A.c23 * vy));
-        const T txy = A.mu * (uy + vx);
-        const T ub = T(0.5) * (wc[1] + u1), vb = T(0.5) * (wc[2] + v1);
+        const T dT = rowB[4 * CW + q + 1] - rowB[4 * CW + q];
+        // y-centred differences (rows jo+1 = jc and jo-1) at my cell; the right neighbour's come by shuffle
+        // (lane 31 gets its own back: its face flux is not used)
+        const T cu0 = rowC[CW + q] - rowA[CW + q], cv0 = rowC[2 * CW + q] - rowA[2 * CW + q];
+        const T cu1 = shfl_down1(cu0), cv1 = shfl_down1(cv0);
+        const T txx = fma_(A.vx_n, u1 - wc[1], -(A.vx_c * (cv0 + cv1)));
+        const T txy = fma_(A.vx_s, v1 - wc[2], A.vx_t * (cu0 + cu1));
         F[1] -= txx;
         F[2] -= txy;
-        F[3] -= fma_(ub, txx, fma_(vb, txy, A.kappa * Tx));
+        const T w = fma_(wc[2] + v1, txy, (wc[1] + u1) * txx);
+        F[3] = fma_(-A.vx_q, dT, fma_(T(-0.5), w, F[3]));
       }
 
       // -------------------------------------------------------------- S7-S9: divergence, combine, store
@@ -444,10 +471,11 @@ __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const Sta
         }
       } else {
         mbar_wait(bar_epi, it & 1);
+        const T dtf = fl ? dtv : T(0);  // non-fluid cells keep their state
         T Un[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-          T v = epi[k * EW + lane + EOFF] + (fl ? dtv * Lc[k] : T(0));
+          T v = fma_(dtf, Lc[k], epi[k * EW + lane + EOFF]);
           if (use_u0) v = fma_(A.rk_a, epi[(4 + k) * EW + lane + EOFF], A.rk_b * v);
           Un[k] = v;
         }
@@ -470,7 +498,7 @@ __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const Sta
     // the Runge-Kutta operands of the next output row, one iteration ahead
     if (A.mode == 0 && it >= 5 && n < nlast) {
       __syncwarp();  // every lane has read epi
-      if (lane == 0) issue_epi(jo + 1);
+      if (elect_one()) issue_epi(jo + 1);
     }
   }
   if (A.smax_bits) {

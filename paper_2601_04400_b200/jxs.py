@@ -42,8 +42,8 @@ def lib():
     """Load (building first if the sources are newer) paper_2601_04400_b200/libjxs.so."""
     global _lib
     if _lib is None:
-        path = _build.LIB
-        if os.path.exists(os.path.join(_build.CSRC, "jxs_api.cu")):
+        path = os.environ.get("JXS_LIB") or _build.LIB  # JXS_LIB: use this prebuilt library as it is
+        if path == _build.LIB and os.path.exists(os.path.join(_build.CSRC, "jxs_api.cu")):
             try:
                 path = _build.build()
             except Exception:
