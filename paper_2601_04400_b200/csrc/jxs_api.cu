@@ -3,6 +3,7 @@
 // Every step of the hot path runs in the kernels of stage_kernel.cuh / aux_kernels.cuh.
 #include "../../include/jxs.h"
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -24,7 +25,7 @@ namespace {
 constexpr int MAX_EVENTS = 8192;
 // resident one-warp CTAs per SM the stage kernel is compiled for (registers <= 65536/(32*minb))
 #ifndef JXS_MINB_F64
-#define JXS_MINB_F64 16
+#define JXS_MINB_F64 12
 #endif
 template <typename T> constexpr int stage_minb() { return sizeof(T) == 8 ? JXS_MINB_F64 : 24; }
 }
@@ -41,6 +42,8 @@ struct jxs_solver {
   size_t elem = 8;
   void* buf[3] = {nullptr, nullptr, nullptr};
   void* stage_io = nullptr;  // interior-sized staging for the *_host entry points
+  // TMA descriptors of the three padded buffers: boxes [4][1][CW] (stencil rows) and [4][1][Epi::W] (RK operand rows)
+  CUtensorMap tm_row[3], tm_epi[3];
   // immersed boundary
   uint8_t* d_fluid = nullptr;
   int n_ghost = 0;
@@ -103,25 +106,59 @@ BcSpec bcspec(const jxs_solver* s) {
 
 template <typename T> constexpr int sout() { return Cfg<T>::SOUT; }
 
-// Strips x segments: a multiple of the resident warp slots, segments long enough to amortise the
-// 6 warm-up rows of every segment.
+// cuTensorMapEncodeTiled through the runtime's driver entry point (libcuda is not linked)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return (EncodeTiledFn)p;
+  }();
+  return fn;
+}
+// descriptor of boxes [4 variables][1 row][box_w columns] of a padded SoA buffer [4][ny+6][pitch]
+bool make_tensor_map(const jxs_solver* s, void* base, int box_w, CUtensorMap* out) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) return false;
+  const cuuint64_t gdim[3] = {(cuuint64_t)s->pitch, (cuuint64_t)(s->ny + 6), 4};
+  const cuuint64_t gstride[2] = {(cuuint64_t)s->pitch * s->elem, (cuuint64_t)s->plane * s->elem};
+  const cuuint32_t box[3] = {(cuuint32_t)box_w, 1, 4};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  return enc(out, s->dtype == JXS_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, base, gdim,
+             gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// Strips x row segments = one-warp tasks.  The warp schedulers are greedy (a warp that can issue keeps the
+// issue port), so the resident warps of an SM drift apart and a single wave of equal tasks ends ragged
+// (measured: mean task lifetime 75 % of the kernel's).  Many short tasks handed out dynamically by the
+// block scheduler keep every slot busy; the price is the ~2 row-equivalents of warm-up per task.
+// cost model: rows of work per slot, plus half a task of tail per slot
 void choose_decomposition(jxs_solver* s) {
   const int SOUT = s->dtype == JXS_F64 ? sout<double>() : sout<float>();
   s->nstrips = (s->nx + SOUT - 1) / SOUT;
   const int minb = s->dtype == JXS_F64 ? stage_minb<double>() : stage_minb<float>();
-  const long long slots = (long long)s->num_sms * minb;
+  const double slots = (double)s->num_sms * minb;
+  const int lo = std::min(s->ny, 8);
+  std::vector<double> cost(s->ny + 1, 0.0);
   double best = 1e300;
-  int best_rps = s->ny;
-  for (int w = 1; w <= 16; ++w) {
-    long long S = std::max<long long>(1, w * slots / s->nstrips);
-    int rps = (int)((s->ny + S - 1) / S);
-    rps = std::max(rps, std::min(s->ny, 8));
-    const int segs = (s->ny + rps - 1) / rps;
-    const long long tasks = (long long)segs * s->nstrips;
-    const long long waves = (tasks + slots - 1) / slots;
-    const double cost = (double)waves * (rps + 4.0);
-    if (cost < best - 1e-9) { best = cost; best_rps = rps; }
+  for (int rps = lo; rps <= s->ny; ++rps) {
+    const double tasks = (double)((s->ny + rps - 1) / rps) * s->nstrips;
+    const double len = rps + 2.0;
+    // one wave: the FP64 pipe of an SM is saturated by about 8 warps, fewer tasks run at full speed each
+    cost[rps] = tasks <= slots ? 1.15 * len * std::max(1.0, tasks / (8.0 * s->num_sms))
+                               : tasks / slots * len * (1.0 + 0.5 * slots / tasks);
+    best = std::min(best, cost[rps]);
   }
+  int best_rps = lo;
+  for (int rps = lo; rps <= s->ny; ++rps)
+    if (cost[rps] <= 1.01 * best) best_rps = rps;  // the longest segments among the near-optimal
+  if (const char* e = getenv("JXS_DBG_ROWS_PER_SEG")) best_rps = std::max(1, std::min(s->ny, atoi(e)));
   s->rows_per_seg = best_rps;
   s->nseg = (s->ny + best_rps - 1) / best_rps;
   s->ntasks = s->nseg * s->nstrips;
@@ -144,7 +181,10 @@ cudaError_t launch_stage_t(jxs_solver* s, const StageArgs<T>& a) {
   }
   static const size_t extra = getenv("JXS_DBG_EXTRA_SMEM") ? (size_t)atoi(getenv("JXS_DBG_EXTRA_SMEM")) : 0;
   if (extra) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem + extra));
-  kern<<<s->grid, s->warps * 32, smem + extra, s->stream>>>(a);
+  int bi = 0;  // which padded buffer is U_in
+  while (bi < 3 && s->buf[bi] != (const void*)a.Uin) ++bi;
+  if (bi == 3) return cudaErrorInvalidValue;
+  kern<<<s->grid, s->warps * 32, smem + extra, s->stream>>>(a, s->tm_row[bi], s->tm_epi[bi], s->tm_epi[0]);
   return cudaGetLastError();
 }
 
@@ -431,6 +471,11 @@ int jxs_create(int nx, int ny, double dx, double dy, double gamma, double mu, do
     cudaGetLastError();
     return rc;
   }
+  for (int b = 0; b < 3; ++b)
+    if (!make_tensor_map(s, s->buf[b], CW, &s->tm_row[b]) || !make_tensor_map(s, s->buf[b], dtype == JXS_F64 ? Epi<double>::W : Epi<float>::W, &s->tm_epi[b])) {
+      jxs_destroy(s);
+      return JXS_ECUDA;
+    }
   const double e_rest = 1.0 / (gamma - 1.0);
   for (int b = 0; b < 3; ++b) {
     if (dtype == JXS_F64) fill_benign_kernel<double><<<s->num_sms * 4, 256, 0, s->stream>>>((double*)s->buf[b], dims(s), e_rest);

@@ -20,6 +20,7 @@
 //     Runge-Kutta combine and (last stage) the wavespeed of the new state are fused behind.
 // Neither reconstructed states nor fluxes ever leave the SM.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -30,8 +31,10 @@ constexpr int CW = LW + 4;       // + 2 halo cells per side
 constexpr int RING = 5;          // rows of primitives kept per warp
 constexpr int STAGE_WARPS = 1;   // one warp per CTA: everything derived from blockIdx is warp-uniform
 
+// output cells per strip = lanes 1..SOUT; the first column of a TMA box must lie on a 16-byte boundary
+// (measured: a tiled copy from an unaligned column raises "illegal instruction"), so strips start on
+// multiples of 2 doubles / 4 floats
 template <typename T> struct Cfg;
-// output cells per strip = lanes 1..SOUT; strips must start on 16-byte boundaries (TMA)
 template <> struct Cfg<double> { static constexpr int SOUT = 30; };
 template <> struct Cfg<float> { static constexpr int SOUT = 28; };
 
@@ -83,6 +86,13 @@ __device__ __forceinline__ void tma_bulk_g2s(uint32_t dst, const void* src, uint
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
+// TMA tiled copy of a [4 variables][1 row][W columns] box of a padded SoA buffer (tensor map: dim 0 = column,
+// 1 = row, 2 = variable) global -> shared: ONE instruction and three integer coordinates per row instead of four
+// bulk copies with 64-bit address arithmetic each
+__device__ __forceinline__ void tma_box_g2s(uint32_t dst, const CUtensorMap* tm, int col, int row, uint32_t bar) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+               ::"r"(dst), "l"(tm), "r"(col), "r"(row), "r"(0), "r"(bar) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   uint32_t ok;
   do {
@@ -108,39 +118,88 @@ __device__ __forceinline__ double max_(double a, double b) { return fmax(a, b); 
 __device__ __forceinline__ float max_(float a, float b) { return fmaxf(a, b); }
 __device__ __forceinline__ double abs_(double a) { return fabs(a); }
 __device__ __forceinline__ float abs_(float a) { return fabsf(a); }
-// Branch-free reciprocal and reciprocal square root.  MUFU.RCP64H / MUFU.RSQ64H are accurate to
-// 2^-20 (measured on B200), so ONE cubic Newton step reaches 1 ulp (max rel. error 2.2e-16 /
-// 2.7e-16 measured over 2^26 arguments).  No slow path: arguments here are densities, pressures,
-// wave-speed differences and WENO denominators, all normal and far from the range limits.
-__device__ __forceinline__ double rcp_(double b) {
-  double r;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
-  double e = fma(-b, r, 1.0);
-  e = fma(e, e, e);
-  return fma(r, e, r);
-}
-__device__ __forceinline__ float rcp_(float b) {
-  float r;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(b));
-  return r;
-}
-__device__ __forceinline__ double rsqrt_(double x) {
-  double y;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  const double f = fma(-(0.5 * x) * y, y, 0.5);
-  return fma(y, f * fma(1.5, f, 1.0), y);
-}
-__device__ __forceinline__ float rsqrt_(float x) {
-  float y;
-  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
 // !(x > 0) on the integer pipe (the FP64 pipe is the bottleneck): true for x <= 0 and NaN
 __device__ __forceinline__ bool not_positive(double x) {
   return (unsigned long long)(__double_as_longlong(x) - 1ll) >= 0x7FF0000000000000ull;
 }
 __device__ __forceinline__ bool not_positive(float x) {
   return (unsigned)(__float_as_int(x) - 1) >= 0x7F800000u;
+}
+
+// ------------------------------------------------------------------ lock-step arithmetic
+// The FP64 pipe of sm_100 accepts one warp instruction every 2 cycles and returns it after ~8; measured
+// on B200 it only stays busy when every warp's OWN stream holds >= 4 independent
+// FP64 instructions between a result and its use - more resident warps do not make up for a shorter
+// distance (3 -> 72 %, 4 -> 92 % of the pipe).  So every routine below is written N-wide: each
+// statement is applied to N independent problems (the 4 primitive variables of a reconstruction, the
+// y- and the x-face of the Riemann solver, the cell and its halo cell of the conversion) before the
+// next statement starts, which is the order ptxas keeps.
+#define JXS_V _Pragma("unroll") for (int k = 0; k < N; ++k)
+
+// Branch-free reciprocal and reciprocal square root.  MUFU.RCP64H / MUFU.RSQ64H are accurate to
+// 2^-20 (measured on B200), so ONE cubic Newton step reaches 1 ulp (max rel. error 2.2e-16 /
+// 2.7e-16 measured over 2^26 arguments).  No slow path: arguments here are densities, pressures,
+// wave-speed differences and WENO denominators, all normal and far from the range limits.
+__device__ __forceinline__ double rcp_seed(double b) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
+  return r;
+}
+__device__ __forceinline__ float rcp_seed(float b) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(b));
+  return r;
+}
+__device__ __forceinline__ double rsqrt_seed(double b) {
+  double r;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
+  return r;
+}
+__device__ __forceinline__ float rsqrt_seed(float b) {
+  float r;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(b));
+  return r;
+}
+template <typename T, int N>
+__device__ __forceinline__ void rcp_n(const T (&b)[N], T (&r)[N]) {
+  T x[N];
+  JXS_V x[k] = rcp_seed(b[k]);
+  if (sizeof(T) == 8) {
+    T e[N];
+    JXS_V e[k] = fma_(-b[k], x[k], T(1));
+    JXS_V e[k] = fma_(e[k], e[k], e[k]);
+    JXS_V r[k] = fma_(x[k], e[k], x[k]);
+  } else {
+    JXS_V r[k] = x[k];
+  }
+}
+template <typename T, int N>
+__device__ __forceinline__ void rsqrt_n(const T (&b)[N], T (&r)[N]) {
+  T y[N];
+  JXS_V y[k] = rsqrt_seed(b[k]);
+  if (sizeof(T) == 8) {
+    T h[N], f[N], g[N];
+    JXS_V h[k] = T(0.5) * b[k];
+    JXS_V h[k] = h[k] * y[k];
+    JXS_V f[k] = fma_(-h[k], y[k], T(0.5));
+    JXS_V g[k] = fma_(T(1.5), f[k], T(1));
+    JXS_V f[k] = f[k] * g[k];
+    JXS_V r[k] = fma_(y[k], f[k], y[k]);
+  } else {
+    JXS_V r[k] = y[k];
+  }
+}
+template <typename T>
+__device__ __forceinline__ T rcp_(T b) {
+  T bb[1] = {b}, r[1];
+  rcp_n<T, 1>(bb, r);
+  return r[0];
+}
+template <typename T>
+__device__ __forceinline__ T rsqrt_(T b) {
+  T bb[1] = {b}, r[1];
+  rsqrt_n<T, 1>(bb, r);
+  return r[0];
 }
 
 // ------------------------------------------------------------------ S4: WENO5-JS, cell-centred
@@ -152,65 +211,134 @@ __device__ __forceinline__ bool not_positive(float x) {
 //   vp = q1 + [ P12 (q0-q1) + 3 P01 (q2-q1) ] / [P12 + 6 P02 + 3 P01],   Pjk = (Bj Bk)^2,
 //   q0-q1 = (s0-s1)/3,  q2-q1 = (s1-s2)/6,  q1 = c + (d2 + 2 d3)/6   (sk = second differences)
 // and the mirror image for vm; with A = P12 (s0-s1), C = P01 (s1-s2) everything is in sixths.
-template <typename T>
-__device__ __forceinline__ void weno5_cell(T a, T b, T c, T d, T e, const StageArgs<T>& K, T& vm, T& vp) {
-  const T d1 = b - a, d2 = c - b, d3 = d - c, d4 = e - d;
-  const T s0 = d2 - d1, s1 = d3 - d2, s2 = d4 - d3;
-  const T t0 = fma_(T(3), d2, -d1), t1 = d2 + d3, t2 = fma_(T(-3), d3, d4);
-  const T B0 = fma_(K.c133 * s0, s0, fma_(t0, t0, K.eps4));
-  const T B1 = fma_(K.c133 * s1, s1, fma_(t1, t1, K.eps4));
-  const T B2 = fma_(K.c133 * s2, s2, fma_(t2, t2, K.eps4));
-  const T D0 = B0 * B0, D1 = B1 * B1, D2 = B2 * B2;
-  const T P12 = D1 * D2, P02 = D0 * D2, P01 = D0 * D1;
-  const T h = fma_(T(6), P02, P12 + P01);
-  const T denp = fma_(T(2), P01, h), denm = fma_(T(2), P12, h);
-  const T A = P12 * (s0 - s1), C = P01 * (s1 - s2);
+// N problems in lock step (the primitive variables).
+template <typename T, int N>
+__device__ __forceinline__ void weno5_n(const T (&a)[N], const T (&b)[N], const T (&c)[N], const T (&d)[N],
+                                        const T (&e)[N], const StageArgs<T>& K, T (&vm)[N], T (&vp)[N]) {
+  T d1[N], d2[N], d3[N], d4[N], s0[N], s1[N], s2[N], t0[N], t1[N], t2[N];
+  JXS_V d1[k] = b[k] - a[k];
+  JXS_V d2[k] = c[k] - b[k];
+  JXS_V d3[k] = d[k] - c[k];
+  JXS_V d4[k] = e[k] - d[k];
+  JXS_V s0[k] = d2[k] - d1[k];
+  JXS_V s1[k] = d3[k] - d2[k];
+  JXS_V s2[k] = d4[k] - d3[k];
+  JXS_V t0[k] = fma_(T(3), d2[k], -d1[k]);
+  JXS_V t1[k] = d2[k] + d3[k];
+  JXS_V t2[k] = fma_(T(-3), d3[k], d4[k]);
+  T B0[N], B1[N], B2[N], u0[N], u1[N], u2[N];
+  JXS_V u0[k] = K.c133 * s0[k];
+  JXS_V u1[k] = K.c133 * s1[k];
+  JXS_V u2[k] = K.c133 * s2[k];
+  JXS_V B0[k] = fma_(t0[k], t0[k], K.eps4);
+  JXS_V B1[k] = fma_(t1[k], t1[k], K.eps4);
+  JXS_V B2[k] = fma_(t2[k], t2[k], K.eps4);
+  JXS_V B0[k] = fma_(u0[k], s0[k], B0[k]);
+  JXS_V B1[k] = fma_(u1[k], s1[k], B1[k]);
+  JXS_V B2[k] = fma_(u2[k], s2[k], B2[k]);
+  JXS_V B0[k] = B0[k] * B0[k];
+  JXS_V B1[k] = B1[k] * B1[k];
+  JXS_V B2[k] = B2[k] * B2[k];
+  T P12[N], P02[N], P01[N], h[N], denp[N], denm[N], A[N], C[N], np[N], nm[N];
+  JXS_V P12[k] = B1[k] * B2[k];
+  JXS_V P02[k] = B0[k] * B2[k];
+  JXS_V P01[k] = B0[k] * B1[k];
+  JXS_V h[k] = P12[k] + P01[k];
+  JXS_V A[k] = s0[k] - s1[k];
+  JXS_V C[k] = s1[k] - s2[k];
+  JXS_V h[k] = fma_(T(6), P02[k], h[k]);
+  JXS_V A[k] = P12[k] * A[k];
+  JXS_V C[k] = P01[k] * C[k];
+  JXS_V denp[k] = fma_(T(2), P01[k], h[k]);
+  JXS_V denm[k] = fma_(T(2), P12[k], h[k]);
   // 6 (vp - c) = (d2 + 2 d3) + (2A + 3C)/denp,   6 (c - vm) = (d3 + 2 d2) + (2C + 3A)/denm
-  const T S = A + C;
-  const T np = fma_(T(2), S, C), nm = fma_(T(2), S, A);
-  T rp, rm;
+  T S[N], rp[N], rm[N], ep[N], em[N];
+  JXS_V S[k] = A[k] + C[k];
   if (sizeof(T) == 8) {  // one reciprocal for both sides (the product stays far inside the fp64 range)
-    const T r = rcp_(denp * denm);
-    rp = r * denm; rm = r * denp;
+    T dd[N], r[N];
+    JXS_V dd[k] = denp[k] * denm[k];
+    rcp_n<T, N>(dd, r);
+    JXS_V rp[k] = r[k] * denm[k];
+    JXS_V rm[k] = r[k] * denp[k];
   } else {
-    rp = rcp_(denp); rm = rcp_(denm);
+    rcp_n<T, N>(denp, rp);
+    rcp_n<T, N>(denm, rm);
   }
-  const T ep = fma_(np, rp, fma_(T(2), d3, d2));
-  const T em = fma_(nm, rm, fma_(T(2), d2, d3));
-  vp = fma_(K.sixth, ep, c);
-  vm = fma_(-K.sixth, em, c);
+  JXS_V np[k] = fma_(T(2), S[k], C[k]);
+  JXS_V nm[k] = fma_(T(2), S[k], A[k]);
+  JXS_V ep[k] = fma_(T(2), d3[k], d2[k]);
+  JXS_V em[k] = fma_(T(2), d2[k], d3[k]);
+  JXS_V ep[k] = fma_(np[k], rp[k], ep[k]);
+  JXS_V em[k] = fma_(nm[k], rm[k], em[k]);
+  JXS_V vp[k] = fma_(K.sixth, ep[k], c[k]);
+  JXS_V vm[k] = fma_(-K.sixth, em[k], c[k]);
 }
 
 // ------------------------------------------------------------------ S5: HLLC, one-sided
 // Normal velocity un, tangential ut.  Eq. 3-7 with the star state of reading R1; for s* != 0 the
 // sign blend of Eq. 3 is exact branch selection, at s* = 0 the left branch is taken (R2).
-// Returns (mass, normal momentum, tangential momentum, energy) flux.
-template <typename T>
-__device__ __forceinline__ void hllc(T rL, T unL, T utL, T pL, T rR, T unR, T utR, T pR, T gamma, T g1inv,
-                                     T& f0, T& f1, T& f2, T& f3) {
-  // a = sqrt(gamma p / rho) = (gamma p) * rsqrt(gamma p rho)
-  const T gpL = gamma * pL, gpR = gamma * pR;
-  const T aL = gpL * rsqrt_(gpL * rL), aR = gpR * rsqrt_(gpR * rR);
-  const T sL = min_(unL - aL, unR - aR), sR = max_(unL + aL, unR + aR);  // Eq. 6
-  const T mL = rL * (sL - unL), mR = rR * (sR - unR);
-  const T sS = fma_(mL, unL, fma_(-mR, unR, pR - pL)) * rcp_(mL - mR);    // Eq. 7
-  const bool left = !(sS < T(0));
-  const T r = left ? rL : rR, un = left ? unL : unR, ut = left ? utL : utR, p = left ? pL : pR;
-  const T sk = left ? sL : sR;
-  const T sc = left ? min_(T(0), sL) : max_(T(0), sR);                    // Eq. 5
-  const T E = fma_(T(0.5) * r, fma_(un, un, ut * ut), p * g1inv);
-  const T ru = r * un;
-  const T rinv = rcp_(sk - sS);
-  const T chi = (sk - un) * rinv;
-  const T rchi = r * chi;
-  const T dm = fma_(r, chi, -r);                                 // rho* - rho
-  const T dn = fma_(rchi, sS, -ru);                              // (rho u)* - rho u
-  const T dt_ = ut * dm;                                         // (rho v)* - rho v
-  const T dE = fma_(sS - un, fma_(rchi, sS, p * rinv), fma_(chi, E, -E));  // E* - E
-  f0 = fma_(sc, dm, ru);
-  f1 = fma_(sc, dn, fma_(ru, un, p));
-  f2 = fma_(sc, dt_, ru * ut);
-  f3 = fma_(sc, dE, un * (E + p));
+// Returns (mass, normal momentum, tangential momentum, energy) flux.  N faces in lock step.
+template <typename T, int N>
+__device__ __forceinline__ void hllc_n(const T (&rL)[N], const T (&unL)[N], const T (&utL)[N], const T (&pL)[N],
+                                       const T (&rR)[N], const T (&unR)[N], const T (&utR)[N], const T (&pR)[N],
+                                       T gamma, T g1inv, T (&f0)[N], T (&f1)[N], T (&f2)[N], T (&f3)[N]) {
+  // a = sqrt(gamma p / rho) = (gamma p) * rsqrt(gamma p rho): both sides of all faces in one 2N-wide pass
+  T gp[2 * N], x[2 * N], y[2 * N];
+  JXS_V gp[k] = gamma * pL[k];
+  JXS_V gp[N + k] = gamma * pR[k];
+  JXS_V x[k] = gp[k] * rL[k];
+  JXS_V x[N + k] = gp[N + k] * rR[k];
+  rsqrt_n<T, 2 * N>(x, y);
+  T aL[N], aR[N], sL[N], sR[N], mL[N], mR[N], q[N], den[N], sS[N];
+  JXS_V aL[k] = gp[k] * y[k];
+  JXS_V aR[k] = gp[N + k] * y[N + k];
+  JXS_V sL[k] = min_(unL[k] - aL[k], unR[k] - aR[k]);  // Eq. 6
+  JXS_V sR[k] = max_(unL[k] + aL[k], unR[k] + aR[k]);
+  JXS_V mL[k] = sL[k] - unL[k];
+  JXS_V mR[k] = sR[k] - unR[k];
+  JXS_V mL[k] = rL[k] * mL[k];
+  JXS_V mR[k] = rR[k] * mR[k];
+  JXS_V q[k] = pR[k] - pL[k];
+  JXS_V den[k] = mL[k] - mR[k];
+  JXS_V q[k] = fma_(-mR[k], unR[k], q[k]);
+  rcp_n<T, N>(den, den);
+  JXS_V q[k] = fma_(mL[k], unL[k], q[k]);
+  JXS_V sS[k] = q[k] * den[k];  // Eq. 7
+  T r[N], un[N], ut[N], p[N], sk[N], sc[N];
+  JXS_V {
+    const bool left = !(sS[k] < T(0));
+    r[k] = left ? rL[k] : rR[k]; un[k] = left ? unL[k] : unR[k]; ut[k] = left ? utL[k] : utR[k];
+    p[k] = left ? pL[k] : pR[k]; sk[k] = left ? sL[k] : sR[k];
+    sc[k] = left ? min_(T(0), sL[k]) : max_(T(0), sR[k]);  // Eq. 5
+  }
+  T E[N], ru[N], rinv[N], chi[N], rchi[N], w[N], dm[N], dn[N], dt_[N], dE[N], z[N];
+  JXS_V rinv[k] = sk[k] - sS[k];
+  JXS_V E[k] = ut[k] * ut[k];
+  JXS_V w[k] = T(0.5) * r[k];
+  JXS_V z[k] = p[k] * g1inv;
+  rcp_n<T, N>(rinv, rinv);
+  JXS_V E[k] = fma_(un[k], un[k], E[k]);
+  JXS_V ru[k] = r[k] * un[k];
+  JXS_V chi[k] = sk[k] - un[k];
+  JXS_V E[k] = fma_(w[k], E[k], z[k]);
+  JXS_V chi[k] = chi[k] * rinv[k];
+  JXS_V w[k] = p[k] * rinv[k];
+  JXS_V z[k] = sS[k] - un[k];
+  JXS_V rchi[k] = r[k] * chi[k];
+  JXS_V dE[k] = fma_(chi[k], E[k], -E[k]);
+  JXS_V dm[k] = fma_(r[k], chi[k], -r[k]);      // rho* - rho
+  JXS_V w[k] = fma_(rchi[k], sS[k], w[k]);
+  JXS_V dn[k] = fma_(rchi[k], sS[k], -ru[k]);   // (rho u)* - rho u
+  JXS_V dt_[k] = ut[k] * dm[k];                 // (rho v)* - rho v
+  JXS_V dE[k] = fma_(z[k], w[k], dE[k]);        // E* - E
+  JXS_V f1[k] = fma_(ru[k], un[k], p[k]);
+  JXS_V f2[k] = ru[k] * ut[k];
+  JXS_V f3[k] = E[k] + p[k];
+  JXS_V f0[k] = fma_(sc[k], dm[k], ru[k]);
+  JXS_V f3[k] = un[k] * f3[k];
+  JXS_V f1[k] = fma_(sc[k], dn[k], f1[k]);
+  JXS_V f2[k] = fma_(sc[k], dt_[k], f2[k]);
+  JXS_V f3[k] = fma_(sc[k], dE[k], f3[k]);
 }
 
 template <typename T>
@@ -223,21 +351,54 @@ __device__ __forceinline__ void atomic_max_pos(unsigned long long* addr, double 
   atomicMax(addr, (unsigned long long)__double_as_longlong(v));
 }
 
+// S6 (R8): viscous flux through N faces in lock step, subtracted from the fluxes (f1 = normal momentum,
+// f2 = tangential momentum, f3 = energy).  dn, dt_: differences of the normal / tangential velocity across
+// the face; xt, xn: sums of the two adjacent centred cross-differences of the tangential / normal
+// velocity; sn, st: sums of the two adjacent velocities; dT: temperature difference.  Coefficients
+// (StageArgs v?_*) per face: cn = 4/3 mu/h_n, cc = (2/3) mu/(4 h_t), cs = mu/h_n, ct = mu/(4 h_t), cq = kappa/h_n.
+template <typename T, int N>
+__device__ __forceinline__ void viscous_n(const T (&dn)[N], const T (&dt_)[N], const T (&xt)[N], const T (&xn)[N],
+                                          const T (&sn)[N], const T (&st)[N], const T (&dT)[N], const T (&cn)[N],
+                                          const T (&cc)[N], const T (&cs)[N], const T (&ct)[N], const T (&cq)[N],
+                                          T (&f1)[N], T (&f2)[N], T (&f3)[N]) {
+  T tnn[N], tnt[N], w[N];
+  JXS_V tnn[k] = cc[k] * xt[k];
+  JXS_V tnt[k] = ct[k] * xn[k];
+  JXS_V tnn[k] = fma_(cn[k], dn[k], -tnn[k]);
+  JXS_V tnt[k] = fma_(cs[k], dt_[k], tnt[k]);
+  JXS_V w[k] = st[k] * tnt[k];
+  JXS_V f1[k] -= tnn[k];
+  JXS_V f2[k] -= tnt[k];
+  JXS_V w[k] = fma_(sn[k], tnn[k], w[k]);  // 2 (u_n tau_nn + u_t tau_nt) at the face
+  JXS_V f3[k] = fma_(T(-0.5), w[k], f3[k]);
+  JXS_V f3[k] = fma_(-cq[k], dT[k], f3[k]);
+}
+
 // Runge-Kutta operand rows: fp64 strips start on even columns, so the 32 owned columns can be
 // fetched alone (16-byte aligned); fp32 fetches the CW-wide window like the raw rows.
 template <typename T> struct Epi { static constexpr int W = sizeof(T) == 8 ? LW : CW, OFF = sizeof(T) == 8 ? 0 : 2; };
-// per-warp shared memory: ring [RING][NV][CW] | raw row [4][CW] | RK operands [2][4][Epi::W] | 2 mbarriers
+// per-warp shared memory: raw rows 2 x [4][CW] | RK operands 2 x [4][Epi::W] | 2 mbarriers | ring [RING][NV][CW]
+// (the TMA destinations first: tiled copies need 128-byte aligned destinations)
+template <typename T> __host__ __device__ constexpr size_t stage_smem_raw() { return (size_t)4 * CW * sizeof(T); }
+template <typename T> __host__ __device__ constexpr size_t stage_smem_epihalf() {
+  return ((size_t)4 * Epi<T>::W * sizeof(T) + 127) / 128 * 128;
+}
+template <typename T> __host__ __device__ constexpr size_t stage_smem_epi() { return 2 * stage_smem_epihalf<T>(); }
+template <typename T> __host__ __device__ constexpr size_t stage_smem_rawslot() { return (stage_smem_raw<T>() + 127) / 128 * 128; }
 template <typename T, int NV>
 __host__ __device__ constexpr size_t stage_smem_per_warp() {
-  return (size_t)((RING * NV + 4) * CW + 8 * Epi<T>::W) * sizeof(T) + 16;
+  return 2 * stage_smem_rawslot<T>() + stage_smem_epi<T>() + 128 + (size_t)RING * NV * CW * sizeof(T);
 }
 
 // ------------------------------------------------------------------ the kernel
 template <typename T, bool VISC, bool ARTV, bool MLP, int MINB>
-__global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const StageArgs<T> A) {
+__global__ void __launch_bounds__(STAGE_WARPS * 32, MINB)
+stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, const __grid_constant__ CUtensorMap tm_epi,
+             const __grid_constant__ CUtensorMap tm_epi0) {
+  // tm_row: boxes [4][1][CW] of Uin; tm_epi / tm_epi0: boxes [4][1][Epi::W] of Uin / U^n
   constexpr int SOUT = Cfg<T>::SOUT;
   constexpr int NV = VISC ? 5 : 4;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
 
   constexpr int EW = Epi<T>::W, EOFF = Epi<T>::OFF;
   const int lane = threadIdx.x;
@@ -250,11 +411,13 @@ __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const Sta
   const int ic = w0 + lane - 3;     // interior x index of my cell
   const int q = lane + 2;           // my column inside the per-warp rows
 
-  T* ring = reinterpret_cast<T*>(smem_raw);  // [RING][NV][CW]
-  T* raw = ring + RING * NV * CW;            // [4][CW]
-  T* epi = raw + 4 * CW;                     // [2][4][EW]
-  const uint32_t bar_raw = smem_u32(epi + 8 * EW), bar_epi = bar_raw + 8;
+  constexpr uint32_t RAWSLOT = (uint32_t)stage_smem_rawslot<T>();
+  T* raw = reinterpret_cast<T*>(smem_raw);                                                  // [2] x [4][CW]
+  T* epi = reinterpret_cast<T*>(smem_raw + 2 * RAWSLOT);                                    // U_in rows [4][EW]
+  T* epi0 = reinterpret_cast<T*>(smem_raw + 2 * RAWSLOT + stage_smem_epihalf<T>());         // U^n rows [4][EW]
+  T* ring = reinterpret_cast<T*>(smem_raw + 2 * RAWSLOT + stage_smem_epi<T>() + 128);       // [RING][NV][CW]
   const uint32_t raw_u32 = smem_u32(raw), epi_u32 = smem_u32(epi);
+  const uint32_t bar_raw = epi_u32 + (uint32_t)stage_smem_epi<T>(), bar_epi = bar_raw + 8;
   constexpr uint32_t ROWB = CW * sizeof(T), EROWB = EW * sizeof(T);
 
   if (lane == 0) {
@@ -266,31 +429,23 @@ __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const Sta
 
   const int nfirst = jbeg - 3, nlast = jend + 2;  // rows to stream, inclusive
   const bool use_u0 = A.rk_a != T(0);
-  const size_t soff = (size_t)(w0 - 2);
-  auto issue_row = [&](int n) {  // lane 0 only: conserved row n -> raw
+  auto issue_row = [&](int n, int slot) {  // one lane: conserved row n -> raw[slot]
     mbar_expect_tx(bar_raw, 4 * ROWB);
-    const T* s = A.Uin + soff + (size_t)n * A.pitch;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) tma_bulk_g2s(raw_u32 + k * ROWB, s + k * A.plane, ROWB, bar_raw);
+    tma_box_g2s(raw_u32 + slot * RAWSLOT, &tm_row, w0 - 2, n, bar_raw);
   };
-  auto issue_epi = [&](int j) {  // lane 0 only: Runge-Kutta operands of output row j -> epi
+  auto issue_epi = [&](int j) {  // one lane: Runge-Kutta operands of output row j -> epi
     mbar_expect_tx(bar_epi, (use_u0 ? 8 : 4) * EROWB);
-    const size_t o = (size_t)(w0 - EOFF) + (size_t)j * A.pitch;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) tma_bulk_g2s(epi_u32 + k * EROWB, A.Uin + o + k * A.plane, EROWB, bar_epi);
-    if (use_u0) {
-#pragma unroll
-      for (int k = 0; k < 4; ++k) tma_bulk_g2s(epi_u32 + (4 + k) * EROWB, A.U0 + o + k * A.plane, EROWB, bar_epi);
-    }
+    tma_box_g2s(epi_u32, &tm_epi, w0 - EOFF, j, bar_epi);
+    if (use_u0) tma_box_g2s(epi_u32 + (uint32_t)stage_smem_epihalf<T>(), &tm_epi0, w0 - EOFF, j, bar_epi);
   };
-  if (elect_one()) issue_row(nfirst);
+  if (elect_one()) issue_row(nfirst, 0);
 
   const T gamma = A.gamma, g1inv = A.g1inv, g1 = A.g1;
   const T dtv = T(*A.dt);
 
   // state carried from one row to the next
   T Ly[4];  // left state (rho,u,v,p) at the face below the next centre row
-  T Gp[4];  // total y-flux (rho, rho u, rho v, E) through the face below the output row
+  T Gp[4];  // total y-flux (mass, normal = rho v, tangential = rho u, energy) through the face below the output row
 #pragma unroll
   for (int k = 0; k < 4; ++k) { Ly[k] = T(0); Gp[k] = T(0); }
   T cuP = T(0), cvP = T(0);
@@ -302,204 +457,239 @@ __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const Sta
   T* pN = ring + q;
   const T *pA = ring + 1 * NV * CW + q, *pB = ring + 2 * NV * CW + q, *pC = ring + 3 * NV * CW + q,
           *pD = ring + 4 * NV * CW + q;
-  const int hoff = lane < 2 ? -2 : LW - 2;  // my halo column (lanes 0-3 convert one each), relative to q
-  for (int n = nfirst; n <= nlast; ++n) {
-    const int it = n - nfirst;
-    // ---------------------------------------------------------------- S3: new row -> primitives
-    __syncwarp();  // every lane is done reading the ring slot that is overwritten now
-    mbar_wait(bar_raw, it & 1);
-    {
-      auto convert = [&](int o) {  // o = column relative to q
-        const T* src = raw + q + o;
-        const T r = src[0], ru = src[CW], rv = src[2 * CW], E = src[3 * CW];
-        const T ri = rcp_(r);
-        const T u = ru * ri, v = rv * ri;
-        const T p = g1 * fma_(T(-0.5), fma_(ru, u, rv * v), E);
-        T* dst = pN + o;
-        dst[0] = r;
-        dst[CW] = u;
-        dst[2 * CW] = v;
-        dst[3 * CW] = p;
-        if (VISC) dst[4 * CW] = p * ri;
-      };
-      convert(0);
-      if (lane < 4) convert(hoff);
-      __syncwarp();
-      if (n < nlast && elect_one()) issue_row(n + 1);
-    }
-    // ring rows n-4 .. n  (valid once it >= 4): A = n-4, B = n-3 = jo (output row), C = n-2 = jc
-    // (centre of the y stencil), D = n-1, E = n
-    const T *rowA = pA - q, *rowB = pB - q, *rowC = pC - q, *rowD = pD - q, *rowE = pN - q;
-    {
-      T* const oldest = const_cast<T*>(pA);
-      pA = pB; pB = pC; pC = pD; pD = pN; pN = oldest;
-    }
-    if (it < 4) continue;
+  // my halo column, relative to q (lanes 0-3 convert one each; the others redo their own and drop it)
+  const int hoff = lane < 2 ? -2 : (lane < 4 ? LW - 2 : 0);
 
+  // ---------------------------------------------------------------- S3: row n -> primitives, ring rotation
+  // One warp-level barrier per row: after it every lane is done with the ring slot, the raw-row slot and the
+  // Runge-Kutta operand rows that are overwritten next, so one elected lane issues the next TMA copies.
+  auto take_row = [&](int n, int it, bool want_epi) {
+    __syncwarp();
+    mbar_wait(bar_raw, it & 1);
+    if (elect_one()) {
+      if (n < nlast) issue_row(n + 1, (it + 1) & 1);
+      if (want_epi) issue_epi(n - 3);
+    }
+    const T* src = reinterpret_cast<const T*>(smem_raw + (it & 1) * RAWSLOT) + q;
+    constexpr int N = 2;  // my cell and my halo cell in lock step
+    T r[N], ru[N], rv[N], E[N], ri[N], u[N], v[N], p[N];
+    const int o[N] = {0, hoff};
+    JXS_V { r[k] = src[o[k]]; ru[k] = src[CW + o[k]]; rv[k] = src[2 * CW + o[k]]; E[k] = src[3 * CW + o[k]]; }
+    rcp_n<T, N>(r, ri);
+    JXS_V u[k] = ru[k] * ri[k];
+    JXS_V v[k] = rv[k] * ri[k];
+    JXS_V p[k] = rv[k] * v[k];
+    JXS_V p[k] = fma_(ru[k], u[k], p[k]);
+    JXS_V p[k] = fma_(T(-0.5), p[k], E[k]);
+    JXS_V p[k] = g1 * p[k];
+    JXS_V {
+      if (k == 0 || lane < 4) {
+        T* dst = pN + o[k];
+        dst[0] = r[k]; dst[CW] = u[k]; dst[2 * CW] = v[k]; dst[3 * CW] = p[k];
+        if (VISC) dst[4 * CW] = p[k] * ri[k];
+      }
+    }
+  };
+  // ring rows until the next rotation: pA = row n-4, pB = n-3 (output row jo), pC = n-2 (centre of the y
+  // stencil, jc), pD = n-1, pN = n (just written)
+  auto rotate = [&]() {
+    T* const oldest = const_cast<T*>(pA);
+    pA = pB; pB = pC; pC = pD; pD = pN; pN = oldest;
+  };
+
+  // ---------------------------------------------------------------- S4 along y (and the carried cross differences)
+  auto weno_y = [&](T (&Ry)[4], T (&Lnew)[4], T& cuC, T& cvC) {
+    constexpr int N = 4;
+    T a[N], b[N], c[N], d[N], e[N];
+    JXS_V { a[k] = pA[k * CW]; b[k] = pB[k * CW]; c[k] = pC[k * CW]; d[k] = pD[k * CW]; e[k] = pN[k * CW]; }
+    weno5_n<T, N>(a, b, c, d, e, A, Ry, Lnew);
+    // positivity guard (R15): a side with rho <= 0 or p <= 0 falls back to its cell (row jc);
+    // one warp vote keeps the (never taken in practice) repair off the common path
+    const bool badR = not_positive(Ry[0]) | not_positive(Ry[3]);
+    const bool badL = not_positive(Lnew[0]) | not_positive(Lnew[3]);
+    if (__any_sync(0xffffffffu, badR | badL)) {
+      asm volatile("" ::: "memory");  // keeps this (never taken in practice) block a branch, not 16 selects
+      JXS_V { Ry[k] = badR ? c[k] : Ry[k]; Lnew[k] = badL ? c[k] : Lnew[k]; }
+    }
+    if (VISC) {  // x-centred differences of u, v in row jc
+      cuC = pC[CW + 1] - pC[CW - 1];
+      cvC = pC[2 * CW + 1] - pC[2 * CW - 1];
+    }
+  };
+
+  // ---------------------------------------------------------------- prologue: rows nfirst .. nfirst+5
+  // fill the ring (rows it < 4), then the left state at the face below row jbeg (it = 4) and the flux through it (it = 5)
+#pragma unroll 1
+  for (int it = 0; it < 6; ++it) {
+    const int n = nfirst + it;
+    take_row(n, it, false);
+    if (it < 4) { rotate(); continue; }
     const int jo = n - 3;
-    const bool do_out = it >= 6;  // rows jo >= jbeg
+    T Ry[4], Lnew[4], cuC = T(0), cvC = T(0);
+    weno_y(Ry, Lnew, cuC, cvC);
+    if (it == 5) {
+      constexpr int N = 1;
+      T f0[N], f1[N], f2[N], f3[N];
+      const T rL[N] = {Ly[0]}, unL[N] = {Ly[2]}, utL[N] = {Ly[1]}, pL[N] = {Ly[3]};
+      const T rR[N] = {Ry[0]}, unR[N] = {Ry[2]}, utR[N] = {Ry[1]}, pR[N] = {Ry[3]};
+      hllc_n<T, N>(rL, unL, utL, pL, rR, unR, utR, pR, gamma, g1inv, f0, f1, f2, f3);
+      if (MLP) {  // Eq. 11
+        const size_t o = (size_t)jo * A.pitch + (w0 + lane);
+        f0[0] = fma_(A.oscale[0], T(__ldg(A.dG + o)), f0[0]);
+        f1[0] = fma_(A.oscale[1], T(__ldg(A.dG + A.plane + o)), f1[0]);
+        f2[0] = fma_(A.oscale[2], T(__ldg(A.dG + 2 * A.plane + o)), f2[0]);
+        f3[0] = fma_(A.oscale[3], T(__ldg(A.dG + 3 * A.plane + o)), f3[0]);
+      }
+      if (VISC) {
+        const T dn[N] = {pC[2 * CW] - pB[2 * CW]}, dt_[N] = {pC[CW] - pB[CW]}, xt[N] = {cuP + cuC}, xn[N] = {cvP + cvC};
+        const T sn[N] = {pB[2 * CW] + pC[2 * CW]}, st[N] = {pB[CW] + pC[CW]}, dT[N] = {pC[4 * CW] - pB[4 * CW]};
+        const T cn[N] = {A.vy_n}, cc[N] = {A.vy_c}, cs[N] = {A.vy_s}, ct[N] = {A.vy_t}, cq[N] = {A.vy_q};
+        viscous_n<T, N>(dn, dt_, xt, xn, sn, st, dT, cn, cc, cs, ct, cq, f1, f2, f3);
+      }
+      Gp[0] = f0[0]; Gp[1] = f1[0]; Gp[2] = f2[0]; Gp[3] = f3[0];
+      if (A.fluid && ic < A.nx) fl_next = A.fluid[(size_t)(jo + 1 - 3) * A.nx + ic];
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) Ly[k] = Lnew[k];
+    if (VISC) { cuP = cuC; cvP = cvC; }
+    rotate();
+  }
+
+  // ---------------------------------------------------------------- main loop: one output row per iteration
+#pragma unroll 1
+  for (int n = nfirst + 6; n <= nlast; ++n) {
+    const int it = n - nfirst;
+    take_row(n, it, A.mode == 0);
+    const int jo = n - 3;  // output row = pB; pC = jc
     const unsigned fl = fl_next;
-    if (it >= 5 && n < nlast && A.fluid && ic < A.nx) fl_next = A.fluid[(size_t)(jo + 1 - 3) * A.nx + ic];
+    if (n < nlast && A.fluid && ic < A.nx) fl_next = A.fluid[(size_t)(jo + 1 - 3) * A.nx + ic];
     float yF[4], yG[4];  // S5': network outputs at my right face and my top face (row jo)
-    if (MLP && it >= 5) {
+    if (MLP) {
       const size_t o = (size_t)jo * A.pitch + (w0 + lane);
 #pragma unroll
       for (int k = 0; k < 4; ++k) { yF[k] = __ldg(A.dF + k * A.plane + o); yG[k] = __ldg(A.dG + k * A.plane + o); }
     }
 
-    // ---------------------------------------------------------------- S4/S5 along y
-    T Ly_div[4];  // G_bottom - G_top of the output row, per component
+    // -------------------------------------------------------------- S4 along y (centre jc) and along x (row jo)
+    T Ry[4], Lnew[4], cuC = T(0), cvC = T(0);
+    weno_y(Ry, Lnew, cuC, cvC);
+    T wc[4], Rm[4], Lp[4];  // my primitives; right state at my left face, left state at my right face
     {
-      T Ry[4], Lnew[4];
+      constexpr int N = 4;
+      T a[N], b[N], d[N], e[N];
+      JXS_V { a[k] = pB[k * CW - 2]; b[k] = pB[k * CW - 1]; wc[k] = pB[k * CW]; d[k] = pB[k * CW + 1]; e[k] = pB[k * CW + 2]; }
+      weno5_n<T, N>(a, b, wc, d, e, A, Rm, Lp);
+      const bool badR = not_positive(Rm[0]) | not_positive(Rm[3]);
+      const bool badL = not_positive(Lp[0]) | not_positive(Lp[3]);
+      if (__any_sync(0xffffffffu, badR | badL)) {
+        asm volatile("" ::: "memory");
+        JXS_V { Rm[k] = badR ? wc[k] : Rm[k]; Lp[k] = badL ? wc[k] : Lp[k]; }
+      }
+    }
+
+    // -------------------------------------------------------------- S5 (+S5', S6): the face above row jo (0) and my right face (1)
+    T f0[2], f1[2], f2[2], f3[2];  // (mass, normal momentum, tangential momentum, energy)
+    {
+      constexpr int N = 2;
+      const T rL[N] = {Ly[0], Lp[0]}, unL[N] = {Ly[2], Lp[1]}, utL[N] = {Ly[1], Lp[2]}, pL[N] = {Ly[3], Lp[3]};
+      const T rR[N] = {Ry[0], shfl_down1(Rm[0])}, unR[N] = {Ry[2], shfl_down1(Rm[1])},
+              utR[N] = {Ry[1], shfl_down1(Rm[2])}, pR[N] = {Ry[3], shfl_down1(Rm[3])};
+      hllc_n<T, N>(rL, unL, utL, pL, rR, unR, utR, pR, gamma, g1inv, f0, f1, f2, f3);
+      if (MLP) {  // Eq. 11
+        f0[0] = fma_(A.oscale[0], T(yG[0]), f0[0]); f0[1] = fma_(A.oscale[0], T(yF[0]), f0[1]);
+        f1[0] = fma_(A.oscale[1], T(yG[1]), f1[0]); f1[1] = fma_(A.oscale[1], T(yF[1]), f1[1]);
+        f2[0] = fma_(A.oscale[2], T(yG[2]), f2[0]); f2[1] = fma_(A.oscale[2], T(yF[2]), f2[1]);
+        f3[0] = fma_(A.oscale[3], T(yG[3]), f3[0]); f3[1] = fma_(A.oscale[3], T(yF[3]), f3[1]);
+      }
+      if (VISC) {
+        // y-face between rows jo and jc: normal velocity v.  x-face at my right: normal velocity u; the
+        // y-centred cross differences (rows jo+1 = jc and jo-1) of the right neighbour come by shuffle
+        // (lane 31 gets its own back: its face flux is not used)
+        const T u1 = pB[CW + 1], v1 = pB[2 * CW + 1];
+        const T cu0 = pC[CW] - pA[CW], cv0 = pC[2 * CW] - pA[2 * CW];
+        const T cu1 = shfl_down1(cu0), cv1 = shfl_down1(cv0);
+        const T dn[N] = {pC[2 * CW] - pB[2 * CW], u1 - wc[1]}, dt_[N] = {pC[CW] - pB[CW], v1 - wc[2]};
+        const T xt[N] = {cuP + cuC, cv0 + cv1}, xn[N] = {cvP + cvC, cu0 + cu1};
+        const T sn[N] = {pB[2 * CW] + pC[2 * CW], wc[1] + u1}, st[N] = {pB[CW] + pC[CW], wc[2] + v1};
+        const T dT[N] = {pC[4 * CW] - pB[4 * CW], pB[4 * CW + 1] - pB[4 * CW]};
+        const T cn[N] = {A.vy_n, A.vx_n}, cc[N] = {A.vy_c, A.vx_c}, cs[N] = {A.vy_s, A.vx_s}, ct[N] = {A.vy_t, A.vx_t},
+                cq[N] = {A.vy_q, A.vx_q};
+        viscous_n<T, N>(dn, dt_, xt, xn, sn, st, dT, cn, cc, cs, ct, cq, f1, f2, f3);
+      }
+    }
+
+    // -------------------------------------------------------------- S7: divergence (conserved order rho, rho u, rho v, E)
+    T Lc[4];
+    {
+      const T Fx[4] = {f0[1], f1[1], f2[1], f3[1]};
+      const T Gy[4] = {f0[0], f2[0], f1[0], f3[0]};
+      const T Gb[4] = {Gp[0], Gp[2], Gp[1], Gp[3]};
+      T dy_[4], Fl[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) Fl[k] = shfl_up1(Fx[k]);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) dy_[k] = Gb[k] - Gy[k];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) Fl[k] = Fl[k] - Fx[k];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) dy_[k] = dy_[k] * A.dyi;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) Lc[k] = fma_(Fl[k], A.dxi, dy_[k]);
+      Gp[0] = f0[0]; Gp[1] = f1[0]; Gp[2] = f2[0]; Gp[3] = f3[0];
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) Ly[k] = Lnew[k];
+    if (VISC) { cuP = cuC; cvP = cvC; }
+
+    if (ARTV) {  // nu * Lap_h(U) on the conserved variables (Eq. 10), rebuilt from the primitives
+      auto cons = [&](const T* row, int c, T* U) {
+        const T r = row[c], u = row[CW + c], v = row[2 * CW + c], p = row[3 * CW + c];
+        U[0] = r; U[1] = r * u; U[2] = r * v; U[3] = fma_(T(0.5) * r, fma_(u, u, v * v), p * g1inv);
+      };
+      T Um[4], Uxm[4], Uxp[4], Ud[4], Uu[4];
+      cons(pB, 0, Um); cons(pB, -1, Uxm); cons(pB, 1, Uxp); cons(pA, 0, Ud); cons(pC, 0, Uu);
+      const T ax = A.nu * A.dxi * A.dxi, ay = A.nu * A.dyi * A.dyi;
 #pragma unroll
       for (int k = 0; k < 4; ++k)
-        weno5_cell(rowA[k * CW + q], rowB[k * CW + q], rowC[k * CW + q], rowD[k * CW + q], rowE[k * CW + q], A, Ry[k],
-                   Lnew[k]);
-      // positivity guard (R15): a side with rho <= 0 or p <= 0 falls back to its cell (row jc);
-      // one warp vote keeps the (never taken in practice) repair off the common path
-      const bool badR = not_positive(Ry[0]) | not_positive(Ry[3]);
-      const bool badL = not_positive(Lnew[0]) | not_positive(Lnew[3]);
-      if (__any_sync(0xffffffffu, badR | badL)) {
-        asm volatile("" ::: "memory");  // keeps this (never taken in practice) block a branch, not 16 selects
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const T cv = rowC[k * CW + q];
-          Ry[k] = badR ? cv : Ry[k];
-          Lnew[k] = badL ? cv : Lnew[k];
-        }
-      }
-      T cuC, cvC;  // x-centred differences of u, v in row jc; cuP, cvP: the same for row jo (carried)
-      if (VISC) {
-        cuC = rowC[CW + q + 1] - rowC[CW + q - 1];
-        cvC = rowC[2 * CW + q + 1] - rowC[2 * CW + q - 1];
-      }
-      if (it >= 5) {
-        T f0, f1, f2, f3;  // face between rows jo and jc: normal = y
-        hllc(Ly[0], Ly[2], Ly[1], Ly[3], Ry[0], Ry[2], Ry[1], Ry[3], gamma, g1inv, f0, f1, f2, f3);
-        T G[4] = {f0, f2, f1, f3};
-        if (MLP) {  // Eq. 11: normal momentum of a y-face is rho*v
-          G[0] = fma_(A.oscale[0], T(yG[0]), G[0]); G[1] = fma_(A.oscale[2], T(yG[2]), G[1]);
-          G[2] = fma_(A.oscale[1], T(yG[1]), G[2]); G[3] = fma_(A.oscale[3], T(yG[3]), G[3]);
-        }
-        if (VISC) {  // S6 (R8): G^v = (0, tau_xy, tau_yy, u tau_xy + v tau_yy + k T_y)
-          const T uB = rowB[CW + q], uC = rowC[CW + q], vB = rowB[2 * CW + q], vC = rowC[2 * CW + q];
-          const T dT = rowC[4 * CW + q] - rowB[4 * CW + q];
-          const T tyy = fma_(A.vy_n, vC - vB, -(A.vy_c * (cuP + cuC)));
-          const T txy = fma_(A.vy_s, uC - uB, A.vy_t * (cvP + cvC));
-          G[1] -= txy;
-          G[2] -= tyy;
-          const T w = fma_(vB + vC, tyy, (uB + uC) * txy);  // 2 (u tau_xy + v tau_yy) at the face
-          G[3] = fma_(-A.vy_q, dT, fma_(T(-0.5), w, G[3]));
-        }
-#pragma unroll
-        for (int k = 0; k < 4; ++k) { Ly_div[k] = Gp[k] - G[k]; Gp[k] = G[k]; }
-      }
-#pragma unroll
-      for (int k = 0; k < 4; ++k) Ly[k] = Lnew[k];
-      if (VISC) { cuP = cuC; cvP = cvC; }
+        Lc[k] += ax * (Uxp[k] - T(2) * Um[k] + Uxm[k]) + ay * (Uu[k] - T(2) * Um[k] + Ud[k]);
     }
 
-    if (do_out) {
-      // -------------------------------------------------------------- S4/S5 along x, row jo
-      T F[4];   // total x-flux through my right face i+1/2
-      T wc[4];  // my primitives
-      {
-        T Rm[4], Lp[4];  // right state at my left face, left state at my right face
+    // -------------------------------------------------------------- S8, S9: combine, store, wavespeed
+    const bool ok = lane >= 1 && lane <= SOUT && ic < A.nx;  // lanes 0 and > SOUT are support cells
+    if (A.mode == 1) {
+      const size_t o = (size_t)(jo - 3) * A.nx + ic, pl = (size_t)A.nx * A.ny;
+      if (ok) {
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const T* r = rowB + k * CW + q;
-          wc[k] = r[0];
-          weno5_cell(r[-2], r[-1], r[0], r[1], r[2], A, Rm[k], Lp[k]);
-        }
-        const bool badR = not_positive(Rm[0]) | not_positive(Rm[3]);
-        const bool badL = not_positive(Lp[0]) | not_positive(Lp[3]);
-        if (__any_sync(0xffffffffu, badR | badL)) {
-          asm volatile("" ::: "memory");
-#pragma unroll
-          for (int k = 0; k < 4; ++k) {
-            Rm[k] = badR ? wc[k] : Rm[k];
-            Lp[k] = badL ? wc[k] : Lp[k];
-          }
-        }
-        const T r0 = shfl_down1(Rm[0]), r1 = shfl_down1(Rm[1]), r2 = shfl_down1(Rm[2]), r3 = shfl_down1(Rm[3]);
-        hllc(Lp[0], Lp[1], Lp[2], Lp[3], r0, r1, r2, r3, gamma, g1inv, F[0], F[1], F[2], F[3]);
-        if (MLP) {
-#pragma unroll
-          for (int k = 0; k < 4; ++k) F[k] = fma_(A.oscale[k], T(yF[k]), F[k]);  // Eq. 11
-        }
+        for (int k = 0; k < 4; ++k) A.Uout[k * pl + o] = fl ? Lc[k] : T(0);
       }
-      if (VISC) {  // S6 (R8): F^v = (0, tau_xx, tau_xy, u tau_xx + v tau_xy + k T_x) at my right face
-        const T u1 = rowB[CW + q + 1], v1 = rowB[2 * CW + q + 1];
-        const T dT = rowB[4 * CW + q + 1] - rowB[4 * CW + q];
-        // y-centred differences (rows jo+1 = jc and jo-1) at my cell; the right neighbour's come by shuffle
-        // (lane 31 gets its own back: its face flux is not used)
-        const T cu0 = rowC[CW + q] - rowA[CW + q], cv0 = rowC[2 * CW + q] - rowA[2 * CW + q];
-        const T cu1 = shfl_down1(cu0), cv1 = shfl_down1(cv0);
-        const T txx = fma_(A.vx_n, u1 - wc[1], -(A.vx_c * (cv0 + cv1)));
-        const T txy = fma_(A.vx_s, v1 - wc[2], A.vx_t * (cu0 + cu1));
-        F[1] -= txx;
-        F[2] -= txy;
-        const T w = fma_(wc[2] + v1, txy, (wc[1] + u1) * txx);
-        F[3] = fma_(-A.vx_q, dT, fma_(T(-0.5), w, F[3]));
+    } else {
+      mbar_wait(bar_epi, it & 1);
+      const T dtf = fl ? dtv : T(0);  // non-fluid cells keep their state
+      T Un[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) Un[k] = fma_(dtf, Lc[k], epi[k * EW + lane + EOFF]);
+      if (use_u0) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) Un[k] = A.rk_b * Un[k];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) Un[k] = fma_(A.rk_a, epi0[k * EW + lane + EOFF], Un[k]);
       }
-
-      // -------------------------------------------------------------- S7-S9: divergence, combine, store
-      T Lc[4];
+      if (ok) {
+        T* o = A.Uout + (size_t)jo * A.pitch + (w0 + lane);
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        const T Fl = shfl_up1(F[k]);
-        Lc[k] = fma_(Fl - F[k], A.dxi, Ly_div[k] * A.dyi);
+        for (int k = 0; k < 4; ++k) o[k * A.plane] = Un[k];
       }
-      if (ARTV) {  // nu * Lap_h(U) on the conserved variables (Eq. 10), rebuilt from the primitives
-        auto cons = [&](const T* row, int c, T* U) {
-          const T r = row[c], u = row[CW + c], v = row[2 * CW + c], p = row[3 * CW + c];
-          U[0] = r; U[1] = r * u; U[2] = r * v; U[3] = fma_(T(0.5) * r, fma_(u, u, v * v), p * g1inv);
-        };
-        T Um[4], Uxm[4], Uxp[4], Ud[4], Uu[4];
-        cons(rowB, q, Um); cons(rowB, q - 1, Uxm); cons(rowB, q + 1, Uxp); cons(rowA, q, Ud); cons(rowC, q, Uu);
-        const T ax = A.nu * A.dxi * A.dxi, ay = A.nu * A.dyi * A.dyi;
-#pragma unroll
-        for (int k = 0; k < 4; ++k)
-          Lc[k] += ax * (Uxp[k] - T(2) * Um[k] + Uxm[k]) + ay * (Uu[k] - T(2) * Um[k] + Ud[k]);
-      }
-      const bool ok = lane >= 1 && lane <= SOUT && ic < A.nx;  // lanes 0 and > SOUT are support cells
-      if (A.mode == 1) {
-        const size_t o = (size_t)(jo - 3) * A.nx + ic, pl = (size_t)A.nx * A.ny;
-        if (ok) {
-#pragma unroll
-          for (int k = 0; k < 4; ++k) A.Uout[k * pl + o] = fl ? Lc[k] : T(0);
-        }
-      } else {
-        mbar_wait(bar_epi, it & 1);
-        const T dtf = fl ? dtv : T(0);  // non-fluid cells keep their state
-        T Un[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          T v = fma_(dtf, Lc[k], epi[k * EW + lane + EOFF]);
-          if (use_u0) v = fma_(A.rk_a, epi[(4 + k) * EW + lane + EOFF], A.rk_b * v);
-          Un[k] = v;
-        }
-        if (ok) {
-          T* o = A.Uout + (size_t)jo * A.pitch + (w0 + lane);
-#pragma unroll
-          for (int k = 0; k < 4; ++k) o[k * A.plane] = Un[k];
-        }
-        if (A.smax_bits) {  // S9 on the new state (it is U^n of the next step), fluid cells only
-          const T ri = rcp_(Un[0]);
-          const T u = Un[1] * ri, v = Un[2] * ri;
-          const T p = g1 * fma_(T(-0.5), fma_(Un[1], u, Un[2] * v), Un[3]);
-          const T gp = gamma * p;
-          const T a = gp * rsqrt_(gp * Un[0]);
-          const T s = max_(abs_(u), abs_(v)) + a;
-          if (ok && fl) smax = (s > smax || s != s) ? s : smax;  // NaN propagates
-        }
+      if (A.smax_bits) {  // S9 on the new state (it is U^n of the next step), fluid cells only
+        const T ri = rcp_(Un[0]);
+        const T u = Un[1] * ri, v = Un[2] * ri;
+        const T p = g1 * fma_(T(-0.5), fma_(Un[1], u, Un[2] * v), Un[3]);
+        const T gp = gamma * p;
+        const T a = gp * rsqrt_(gp * Un[0]);
+        const T s = max_(abs_(u), abs_(v)) + a;
+        if (ok && fl) smax = (s > smax || s != s) ? s : smax;  // NaN propagates
       }
     }
-    // the Runge-Kutta operands of the next output row, one iteration ahead
-    if (A.mode == 0 && it >= 5 && n < nlast) {
-      __syncwarp();  // every lane has read epi
-      if (elect_one()) issue_epi(jo + 1);
-    }
+    rotate();
   }
   if (A.smax_bits) {
 #pragma unroll
@@ -510,5 +700,7 @@ __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB) stage_kernel(const Sta
     if (lane == 0) atomic_max_pos(A.smax_bits, (double)smax);
   }
 }
+
+#undef JXS_V
 
 }  // namespace jxs
