@@ -25,7 +25,7 @@ namespace {
 constexpr int MAX_EVENTS = 8192;
 // resident one-warp CTAs per SM the stage kernel is compiled for (registers <= 65536/(32*minb))
 #ifndef JXS_MINB_F64
-#define JXS_MINB_F64 12
+#define JXS_MINB_F64 16
 #endif
 template <typename T> constexpr int stage_minb() { return sizeof(T) == 8 ? JXS_MINB_F64 : 24; }
 }

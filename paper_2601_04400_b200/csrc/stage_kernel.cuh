@@ -126,6 +126,14 @@ __device__ __forceinline__ bool not_positive(float x) {
   return (unsigned)(__float_as_int(x) - 1) >= 0x7F800000u;
 }
 
+// sign bit and halving on the integer pipe (arguments are normal numbers; -0.0 counts as negative)
+__device__ __forceinline__ bool is_negative(double x) { return __double2hiint(x) < 0; }
+__device__ __forceinline__ bool is_negative(float x) { return __float_as_int(x) < 0; }
+__device__ __forceinline__ double half_of(double x) {
+  return __hiloint2double(__double2hiint(x) - 0x00100000, __double2loint(x));
+}
+__device__ __forceinline__ float half_of(float x) { return 0.5f * x; }
+
 // ------------------------------------------------------------------ lock-step arithmetic
 // The FP64 pipe of sm_100 accepts one warp instruction every 2 cycles and returns it after ~8; measured
 // on B200 it only stays busy when every warp's OWN stream holds >= 4 independent
@@ -179,7 +187,7 @@ __device__ __forceinline__ void rsqrt_n(const T (&b)[N], T (&r)[N]) {
   JXS_V y[k] = rsqrt_seed(b[k]);
   if (sizeof(T) == 8) {
     T h[N], f[N], g[N];
-    JXS_V h[k] = T(0.5) * b[k];
+    JXS_V h[k] = half_of(b[k]);
     JXS_V h[k] = h[k] * y[k];
     JXS_V f[k] = fma_(-h[k], y[k], T(0.5));
     JXS_V g[k] = fma_(T(1.5), f[k], T(1));
@@ -306,10 +314,11 @@ __device__ __forceinline__ void hllc_n(const T (&rL)[N], const T (&unL)[N], cons
   JXS_V sS[k] = q[k] * den[k];  // Eq. 7
   T r[N], un[N], ut[N], p[N], sk[N], sc[N];
   JXS_V {
-    const bool left = !(sS[k] < T(0));
+    const bool left = !is_negative(sS[k]);
     r[k] = left ? rL[k] : rR[k]; un[k] = left ? unL[k] : unR[k]; ut[k] = left ? utL[k] : utR[k];
     p[k] = left ? pL[k] : pR[k]; sk[k] = left ? sL[k] : sR[k];
-    sc[k] = left ? min_(T(0), sL[k]) : max_(T(0), sR[k]);  // Eq. 5
+    // Eq. 5: min(0, sL) on the left, max(0, sR) on the right = the selected speed where its sign says so
+    sc[k] = is_negative(sk[k]) == left ? sk[k] : T(0);
   }
   T E[N], ru[N], rinv[N], chi[N], rchi[N], w[N], dm[N], dn[N], dt_[N], dE[N], z[N];
   JXS_V rinv[k] = sk[k] - sS[k];
