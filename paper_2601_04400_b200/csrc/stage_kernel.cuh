@@ -394,9 +394,13 @@ template <typename T> __host__ __device__ constexpr size_t stage_smem_epihalf() 
 }
 template <typename T> __host__ __device__ constexpr size_t stage_smem_epi() { return 2 * stage_smem_epihalf<T>(); }
 template <typename T> __host__ __device__ constexpr size_t stage_smem_rawslot() { return (stage_smem_raw<T>() + 127) / 128 * 128; }
+// one ring row [NV][CW], padded to 128 bytes: the first rows of a segment land in the ring directly
+template <typename T, int NV> __host__ __device__ constexpr size_t stage_smem_ringslot() {
+  return ((size_t)NV * CW * sizeof(T) + 127) / 128 * 128;
+}
 template <typename T, int NV>
 __host__ __device__ constexpr size_t stage_smem_per_warp() {
-  return 2 * stage_smem_rawslot<T>() + stage_smem_epi<T>() + 128 + (size_t)RING * NV * CW * sizeof(T);
+  return 2 * stage_smem_rawslot<T>() + stage_smem_epi<T>() + 128 + (size_t)RING * stage_smem_ringslot<T, NV>();
 }
 
 // ------------------------------------------------------------------ the kernel
@@ -447,7 +451,15 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
     tma_box_g2s(epi_u32, &tm_epi, w0 - EOFF, j, bar_epi);
     if (use_u0) tma_box_g2s(epi_u32 + (uint32_t)stage_smem_epihalf<T>(), &tm_epi0, w0 - EOFF, j, bar_epi);
   };
-  if (elect_one()) issue_row(nfirst, 0);
+  // The first five rows of the segment go straight into the ring (phase 0 of bar_epi), the sixth into raw slot 1
+  // (phase 0 of bar_raw): one memory latency for the whole warm-up instead of one per row.
+  if (elect_one()) {
+    mbar_expect_tx(bar_epi, 5 * 4 * ROWB);
+#pragma unroll
+    for (int r = 0; r < 5; ++r)
+      tma_box_g2s(smem_u32(ring) + r * (uint32_t)stage_smem_ringslot<T, NV>(), &tm_row, w0 - 2, nfirst + r, bar_epi);
+    issue_row(nfirst + 5, 1);
+  }
 
   const T gamma = A.gamma, g1inv = A.g1inv, g1 = A.g1;
   const T dtv = T(*A.dt);
@@ -463,9 +475,9 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
 
   // Ring rows as loop-carried per-lane pointers (to my column q), rotated once per iteration: the row
   // accesses below become LDS with immediate offsets, no slot arithmetic.  pN = slot written next.
-  T* pN = ring + q;
-  const T *pA = ring + 1 * NV * CW + q, *pB = ring + 2 * NV * CW + q, *pC = ring + 3 * NV * CW + q,
-          *pD = ring + 4 * NV * CW + q;
+  constexpr int RS = (int)(stage_smem_ringslot<T, NV>() / sizeof(T));  // ring slot stride in elements
+  const T *pA = ring + q, *pB = ring + 1 * RS + q, *pC = ring + 2 * RS + q, *pD = ring + 3 * RS + q;
+  T* pN = ring + 4 * RS + q;
   // my halo column, relative to q (lanes 0-3 convert one each; the others redo their own and drop it)
   const int hoff = lane < 2 ? -2 : (lane < 4 ? LW - 2 : 0);
 
@@ -474,7 +486,7 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
   // Runge-Kutta operand rows that are overwritten next, so one elected lane issues the next TMA copies.
   auto take_row = [&](int n, int it, bool want_epi) {
     __syncwarp();
-    mbar_wait(bar_raw, it & 1);
+    mbar_wait(bar_raw, (it + 1) & 1);  // row nfirst+5 was phase 0
     if (elect_one()) {
       if (n < nlast) issue_row(n + 1, (it + 1) & 1);
       if (want_epi) issue_epi(n - 3);
@@ -527,12 +539,38 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
   };
 
   // ---------------------------------------------------------------- prologue: rows nfirst .. nfirst+5
-  // fill the ring (rows it < 4), then the left state at the face below row jbeg (it = 4) and the flux through it (it = 5)
+  // rows nfirst .. nfirst+4 are converted in place in the ring (5 rows in lock step, then their halo columns);
+  // then the left state at the face below row jbeg (it = 4) and the flux through it (it = 5)
+  mbar_wait(bar_epi, 0);
+  {
+    constexpr int N = 5;
+#pragma unroll
+    for (int pass = 0; pass < 2; ++pass) {
+      const int o = pass == 0 ? 0 : hoff;
+      T* const base = ring + q + o;
+      T r[N], ru[N], rv[N], E[N], ri[N], u[N], v[N], p[N];
+      JXS_V { const T* src = base + k * RS; r[k] = src[0]; ru[k] = src[CW]; rv[k] = src[2 * CW]; E[k] = src[3 * CW]; }
+      rcp_n<T, N>(r, ri);
+      JXS_V u[k] = ru[k] * ri[k];
+      JXS_V v[k] = rv[k] * ri[k];
+      JXS_V p[k] = rv[k] * v[k];
+      JXS_V p[k] = fma_(ru[k], u[k], p[k]);
+      JXS_V p[k] = fma_(T(-0.5), p[k], E[k]);
+      JXS_V p[k] = g1 * p[k];
+      if (pass == 0 || lane < 4) {
+        JXS_V {
+          T* dst = base + k * RS;
+          dst[CW] = u[k]; dst[2 * CW] = v[k]; dst[3 * CW] = p[k];
+          if (VISC) dst[4 * CW] = p[k] * ri[k];
+        }
+      }
+    }
+  }
+  __syncwarp();  // the cross differences below read the neighbours' columns
 #pragma unroll 1
-  for (int it = 0; it < 6; ++it) {
+  for (int it = 4; it < 6; ++it) {
     const int n = nfirst + it;
-    take_row(n, it, false);
-    if (it < 4) { rotate(); continue; }
+    if (it == 5) take_row(n, it, false);
     const int jo = n - 3;
     T Ry[4], Lnew[4], cuC = T(0), cvC = T(0);
     weno_y(Ry, Lnew, cuC, cvC);
@@ -672,7 +710,7 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
         for (int k = 0; k < 4; ++k) A.Uout[k * pl + o] = fl ? Lc[k] : T(0);
       }
     } else {
-      mbar_wait(bar_epi, it & 1);
+      mbar_wait(bar_epi, (it + 1) & 1);  // phase 0 was the warm-up rows
       const T dtf = fl ? dtv : T(0);  // non-fluid cells keep their state
       T Un[4];
 #pragma unroll
