@@ -30,8 +30,8 @@ ALG_BYTES = {"f64": 85.33, "f32": 42.67}
 PEAK_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 PEAK_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum of the stage kernel, per launch, mean of the three RK stages, from
-# the `ncu --set full` capture summarised in profiles/r01b_stage_f64.md (fp64, 4096x2048); None = not captured
-NCU_TRAFFIC_BYTES = {("f64", 4096, 2048, "ns"): (528.7e6 + 821.2e6 + 800.1e6) / 3}
+# the `ncu --set full` capture summarised in profiles/r01d_stage_f64.md (fp64, 4096x2048); None = not captured
+NCU_TRAFFIC_BYTES = {("f64", 4096, 2048, "ns"): (550.7e6 + 849.7e6 + 824.1e6) / 3}
 
 
 def max_over_ranks(ms, dist, device):
@@ -239,7 +239,7 @@ def main():
     traffic = NCU_TRAFFIC_BYTES.get((args.dtype, args.nx, args.ny, kind))
     roofline = {
         "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-        "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r01b_stage_f64.md)",
+        "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r01d_stage_f64.md)",
         "kernel": "jxs::stage_kernel", "avg_launch_ms": stage_avg_ms, "launches_timed": stage_n,
         "share_of_step": stage_ms / ms,
         "alg_flop_per_cell_stage": ALG_FLOP[kind], "alg_bytes_per_cell_stage": ALG_BYTES[args.dtype],
