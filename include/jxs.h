@@ -40,6 +40,7 @@ enum {
 };
 enum { JXS_BC_PERIODIC = 0, JXS_BC_TRANSMISSIVE = 1, JXS_BC_REFLECTIVE = 2, JXS_BC_INFLOW = 3 };
 enum { JXS_F64 = 0, JXS_F32 = 1 };
+enum { JXS_SSPRK3 = 0, JXS_EULER = 1 };
 
 typedef struct jxs_solver jxs_solver;
 
@@ -102,6 +103,16 @@ int jxs_step_fixed_dt(jxs_solver*, void* U, double dt, int nsteps);
  * device->host copy; used for end-to-end timing.                                            */
 int jxs_step_host(jxs_solver*, void* U_host, double cfl, int nsteps);
 int jxs_rhs_host(jxs_solver*, const void* U_host, void* dUdt_host);
+/* jxs_step without the final synchronisation: only enqueues on the handle's stream, so that several handles
+ * (BASELINE.json configs[4]: 16 independent simulations, one stream each) run concurrently.  jxs_wait
+ * synchronises the stream, updates jxs_get_time and returns JXS_ENUMERIC like jxs_step would have.
+ * U must stay valid until jxs_wait returns.                                                  */
+int jxs_step_async(jxs_solver*, void* U, double cfl, int nsteps);
+int jxs_wait(jxs_solver*);
+/* Time integrator of jxs_step*: JXS_SSPRK3 (default, R5) or JXS_EULER, the forward-Euler update the paper
+ * prints (Eq. 10; with jxs_set_artificial_viscosity it is Eq. 10 term by term) = one stage
+ * with (a,b) = (0,1).  SURVEY.md section 8(f) rank 2.                                           */
+int jxs_set_time_integrator(jxs_solver*, int scheme);
 
 /* Simulated time since creation and the last time step taken.                               */
 int jxs_get_time(const jxs_solver*, double* t_host, double* last_dt_host);

@@ -65,6 +65,8 @@ struct jxs_solver {
   // stepping state
   StepState* d_state = nullptr;
   double t = 0, last_dt = 0;
+  int scheme = JXS_SSPRK3;
+  int pending_steps = 0;  // steps enqueued by jxs_step_async and not yet waited for
   // work decomposition of the stage kernel
   int nstrips = 0, rows_per_seg = 0, nseg = 0, ntasks = 0, warps = 0, grid = 0;
   // bookkeeping
@@ -343,10 +345,12 @@ void free_ibm(jxs_solver* s) {
   s->n_ghost = 0;
 }
 
-// advance the padded state in buf[0] by nsteps SSP-RK3 steps (R5); cur = index of the valid s_max
-int run_steps(jxs_solver* s, double cfl, double fixed_dt, int nsteps) {
+// advance the padded state in buf[0] by nsteps steps; returns in *where the buffer that holds the result.
+// SSP-RK3 (R5): three stages, result back in buf[0].  Forward Euler (Eq. 10 as printed): one stage
+// with (a,b) = (0,1), the two buffers swap roles every step.  cur = index of the valid s_max.
+int run_steps(jxs_solver* s, double cfl, double fixed_dt, int nsteps, int* where) {
   const double h = std::min(s->dx, s->dy);
-  int cur = 0;
+  int cur = 0, at = 0;
   s->events_used = 0;
   s->mlp_events_used = 0;
   if (!(fixed_dt > 0)) CU(wavespeed(s, s->buf[0], &s->d_state->smax_bits[0]));
@@ -355,17 +359,25 @@ int run_steps(jxs_solver* s, double cfl, double fixed_dt, int nsteps) {
     s->launches++;
     CU(cudaGetLastError());
     unsigned long long* next = &s->d_state->smax_bits[cur ^ 1];
-    CU(ghost_fill(s, s->buf[0]));
-    CU(flux_mlp(s, s->buf[0]));
-    CU(stage(s, s->buf[0], nullptr, s->buf[1], 0, 0.0, 1.0, nullptr));                  // U1 = U0 + dt L(U0)
-    CU(ghost_fill(s, s->buf[1]));
-    CU(flux_mlp(s, s->buf[1]));
-    CU(stage(s, s->buf[1], s->buf[0], s->buf[2], 0, 0.75, 0.25, nullptr));              // U2 = 3/4 U0 + 1/4 (U1 + dt L(U1))
-    CU(ghost_fill(s, s->buf[2]));
-    CU(flux_mlp(s, s->buf[2]));
-    CU(stage(s, s->buf[2], s->buf[0], s->buf[0], 0, 1.0 / 3.0, 2.0 / 3.0, next));       // U0 = 1/3 U0 + 2/3 (U2 + dt L(U2))
+    if (s->scheme == JXS_EULER) {
+      CU(ghost_fill(s, s->buf[at]));
+      CU(flux_mlp(s, s->buf[at]));
+      CU(stage(s, s->buf[at], nullptr, s->buf[at ^ 1], 0, 0.0, 1.0, next));              // U^{n+1} = U^n + dt L(U^n)
+      at ^= 1;
+    } else {
+      CU(ghost_fill(s, s->buf[0]));
+      CU(flux_mlp(s, s->buf[0]));
+      CU(stage(s, s->buf[0], nullptr, s->buf[1], 0, 0.0, 1.0, nullptr));                  // U1 = U0 + dt L(U0)
+      CU(ghost_fill(s, s->buf[1]));
+      CU(flux_mlp(s, s->buf[1]));
+      CU(stage(s, s->buf[1], s->buf[0], s->buf[2], 0, 0.75, 0.25, nullptr));              // U2 = 3/4 U0 + 1/4 (U1 + dt L(U1))
+      CU(ghost_fill(s, s->buf[2]));
+      CU(flux_mlp(s, s->buf[2]));
+      CU(stage(s, s->buf[2], s->buf[0], s->buf[0], 0, 1.0 / 3.0, 2.0 / 3.0, next));       // U0 = 1/3 U0 + 2/3 (U2 + dt L(U2))
+    }
     cur ^= 1;
   }
+  *where = at;
   return JXS_OK;
 }
 
@@ -400,7 +412,7 @@ int finish_steps(jxs_solver* s, int nsteps) {
   return JXS_OK;
 }
 
-int step_common(jxs_solver* s, void* U, double cfl, double fixed_dt, int nsteps, bool host) {
+int step_common(jxs_solver* s, void* U, double cfl, double fixed_dt, int nsteps, bool host, bool wait = true) {
   if (!s) return JXS_EINVAL;
   if (!U) return fail(s, JXS_EINVAL, "U is NULL");
   if (nsteps < 0) return fail(s, JXS_EINVAL, "nsteps < 0");
@@ -412,13 +424,18 @@ int step_common(jxs_solver* s, void* U, double cfl, double fixed_dt, int nsteps,
     Ud = s->stage_io;
   }
   CU(pad(s, Ud, s->buf[0]));
-  int rc = run_steps(s, cfl, fixed_dt, nsteps);
+  int at = 0;
+  int rc = run_steps(s, cfl, fixed_dt, nsteps, &at);
   if (rc != JXS_OK) return rc;
   if (host) {
-    CU(unpad(s, s->buf[0], s->stage_io));
+    CU(unpad(s, s->buf[at], s->stage_io));
     CU(cudaMemcpyAsync(U, s->stage_io, bytes, cudaMemcpyDeviceToHost, s->stream));
   } else {
-    CU(unpad(s, s->buf[0], U));
+    CU(unpad(s, s->buf[at], U));
+  }
+  if (!wait) {
+    s->pending_steps += nsteps;
+    return JXS_OK;
   }
   return finish_steps(s, nsteps);
 }
@@ -668,6 +685,19 @@ int jxs_step_fixed_dt(jxs_solver* s, void* U, double dt, int nsteps) {
   return step_common(s, U, 0.0, dt, nsteps, false);
 }
 int jxs_step_host(jxs_solver* s, void* U, double cfl, int nsteps) { return step_common(s, U, cfl, 0.0, nsteps, true); }
+int jxs_step_async(jxs_solver* s, void* U, double cfl, int nsteps) { return step_common(s, U, cfl, 0.0, nsteps, false, false); }
+int jxs_wait(jxs_solver* s) {
+  if (!s) return JXS_EINVAL;
+  const int n = s->pending_steps;
+  s->pending_steps = 0;
+  return finish_steps(s, n);
+}
+int jxs_set_time_integrator(jxs_solver* s, int scheme) {
+  if (!s) return JXS_EINVAL;
+  if (scheme != JXS_SSPRK3 && scheme != JXS_EULER) return fail(s, JXS_EINVAL, "unknown time integrator");
+  s->scheme = scheme;
+  return JXS_OK;
+}
 
 int jxs_get_time(const jxs_solver* s, double* t, double* last_dt) {
   if (!s) return JXS_EINVAL;

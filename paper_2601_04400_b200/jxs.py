@@ -15,13 +15,14 @@ from . import build as _build
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENUMERIC = 0, 1, 2, 3, 4, 5
 BC_PERIODIC, BC_TRANSMISSIVE, BC_REFLECTIVE, BC_INFLOW = 0, 1, 2, 3
 F64, F32 = 0, 1
+SSPRK3, EULER = 0, 1
 _BC_NAMES = {"periodic": 0, "transmissive": 1, "reflective": 2, "inflow": 3}
 
 EXPORTS = ("jxs_create", "jxs_destroy", "jxs_last_error", "jxs_set_ibm", "jxs_set_flux_mlp",
            "jxs_set_artificial_viscosity", "jxs_rhs", "jxs_max_wavespeed", "jxs_step", "jxs_step_fixed_dt",
            "jxs_step_host", "jxs_rhs_host", "jxs_get_time", "jxs_launch_count", "jxs_set_profiling",
            "jxs_stage_time", "jxs_ibm_ghost_count", "jxs_measure_fp64_peak", "jxs_flux_correction",
-           "jxs_flux_mlp_time")
+           "jxs_flux_mlp_time", "jxs_step_async", "jxs_wait", "jxs_set_time_integrator")
 
 
 class jxs_bc(C.Structure):
@@ -66,6 +67,9 @@ def lib():
         L.jxs_step.argtypes = [vp, vp, C.c_double, C.c_int]
         L.jxs_step_fixed_dt.argtypes = [vp, vp, C.c_double, C.c_int]
         L.jxs_step_host.argtypes = [vp, vp, C.c_double, C.c_int]
+        L.jxs_step_async.argtypes = [vp, vp, C.c_double, C.c_int]
+        L.jxs_wait.argtypes = [vp]
+        L.jxs_set_time_integrator.argtypes = [vp, C.c_int]
         L.jxs_get_time.argtypes = [vp, dp, dp]
         L.jxs_launch_count.argtypes = [vp]
         L.jxs_launch_count.restype = C.c_longlong
@@ -201,6 +205,17 @@ class Solver:
         """In place on the device tensor U."""
         self._chk(lib().jxs_step(self._h, self._dev(U), float(cfl), int(nsteps)))
         return U
+
+    def step_async(self, U, cfl, nsteps):
+        """Enqueue only (no synchronisation); call wait() before reading U or the time."""
+        self._chk(lib().jxs_step_async(self._h, self._dev(U), float(cfl), int(nsteps)))
+        return U
+
+    def wait(self):
+        self._chk(lib().jxs_wait(self._h))
+
+    def set_time_integrator(self, scheme):
+        self._chk(lib().jxs_set_time_integrator(self._h, int(scheme)))
 
     def step_fixed_dt(self, U, dt, nsteps):
         self._chk(lib().jxs_step_fixed_dt(self._h, self._dev(U), float(dt), int(nsteps)))
