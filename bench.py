@@ -138,6 +138,85 @@ def run_reference(args, rank):
         "gpu_launches": 0}))
 
 
+def run_c5(args, rank, world, local_rank, dist, barrier, tdt):
+    """BASELINE.json configs[4]: 16 handles x (1024x512 shock-cylinder, Mach ~ U[1.5,3]) with the bf16 flux MLP
+    fused into the fp64 HLLC flux; one stream per handle, jxs_step_async on each, aggregate Mcell-stage/s."""
+    import numpy as np
+    import torch
+    from paper_2601_04400_b200 import jxs, workloads as wl
+    cases = wl.batch_cases(16)
+    w, (ins, outs) = wl.mlp_weights(), wl.mlp_scales()
+    streams = [torch.cuda.Stream() for _ in cases]
+    solvers, Us = [], []
+    for c, st in zip(cases, streams):
+        s = jxs.Solver.from_case(c, dtype=tdt, stream=st)
+        s.set_flux_mlp(w, ins, outs)
+        solvers.append(s)
+        Us.append(torch.tensor(c["U0"], dtype=tdt, device="cuda"))
+    ncell = sum(c["nx"] * c["ny"] for c in cases)
+    K, W = args.steps, args.warmup
+    torch.cuda.synchronize()
+    for s, U in zip(solvers, Us):
+        s.step_async(U, 0.4, W)
+    for s in solvers:
+        s.wait()
+    if args.profile_kernels:  # two event records per kernel launch: only on request, the host work is not free
+        for s in solvers:
+            s.set_profiling(True)
+    sampler = ClockSampler(local_rank)
+    main_stream = torch.cuda.current_stream()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = sum(s.launch_count() for s in solvers)
+    barrier()
+    sampler.start()
+    e0.record(main_stream)
+    for st in streams:
+        st.wait_event(e0)
+    for s, U in zip(solvers, Us):
+        s.step_async(U, 0.4, K)
+    for st in streams:
+        main_stream.wait_stream(st)
+    e1.record(main_stream)
+    for s in solvers:
+        s.wait()
+    barrier()
+    clocks = sampler.stop()
+    ms = max_over_ranks(e0.elapsed_time(e1), dist, "cuda")
+    launches = sum(s.launch_count() for s in solvers) - launches0
+    if not all(bool(torch.isfinite(U).all()) for U in Us):
+        raise SystemExit("bench.py: non-finite state after the timed region")
+    value = aggregate_rate(ncell, K, world, ms)
+    stage_ms = sum(s.stage_time()[0] for s in solvers)
+    stage_n = sum(s.stage_time()[1] for s in solvers)
+    mlp_ms = sum(s.flux_mlp_time()[0] for s in solvers)
+    mlp_n = sum(s.flux_mlp_time()[1] for s in solvers)
+    if rank != 0:
+        return
+    # S5' roofline (DESIGN.md section 6): 256 tanh per cell-stage on the MUFU units, 16 per clock per SM.  The 16
+    # streams run concurrently, so per-kernel event spans overlap; the fraction is taken over the whole timed region.
+    tanh_total = 256.0 * ncell * 3 * K
+    mufu_peak = 148 * 16 * 1.965e9
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+        "config": {"workload": "batch_16x1024x512_flux_mlp (BASELINE.json configs[4]: 16 independent shock-cylinder runs, "
+                               "Mach ~ U[1.5,3], per-face MLP 24-64-64-4 in bf16 fused into the HLLC flux)",
+                   "cfl": 0.4, "rk": "SSP-RK3", "cells": ncell, "handles": len(cases), "streams": len(streams),
+                   "l2": "16 x 3 x 17 MB of state buffers = 800 MB vs 126 MB of L2, no flush needed",
+                   "parallelism": "replicas" if world > 1 else "single GPU"},
+        "clocks": clocks, "gpu_launches": launches,
+        "roofline": {"bound": "alu", "kernel": "jxs::flux_mlp_kernel (MUFU tanh) over the whole timed region",
+                     "unit": "Gtanh/s", "achieved": tanh_total / (ms * 1e-3) / 1e9, "peak": mufu_peak / 1e9,
+                     "frac": tanh_total / (ms * 1e-3) / mufu_peak, "traffic": None,
+                     "kernel_event_spans_ms": {"flux_mlp_kernel": mlp_ms / max(mlp_n, 1), "stage_kernel": stage_ms / max(stage_n, 1),
+                                               "note": "spans on 16 concurrent streams overlap each other"},
+                     "launches_timed": mlp_n,
+                     "peak_source": "derived: 148 SMs x 16 MUFU/clk x 1.965 GHz (DESIGN.md section 6)"},
+        "e2e": None, "cpu_baseline": None,
+    }
+    print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -149,6 +228,10 @@ def main():
     ap.add_argument("--ny", type=int, default=2048)
     ap.add_argument("--euler", action="store_true", help="mu = 0, no IBM (not the headline config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--profile-kernels", action="store_true", help="c5 only: per-kernel CUDA-event spans")
+    ap.add_argument("--workload", choices=("c4", "c5"), default="c4",
+                    help="c4 = the headline throughput case (default); c5 = BASELINE.json configs[4]: 16 independent "
+                         "1024x512 shock-cylinder runs with the per-face flux MLP, one stream per handle")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "jxs" else args.warmup
 
@@ -177,6 +260,9 @@ def main():
         torch.cuda.synchronize()
 
     tdt = torch.float64 if args.dtype == "f64" else torch.float32
+    if args.workload == "c5":
+        run_c5(args, rank, world, local_rank, dist, barrier, tdt)
+        return
     case = wl.throughput_case(args.nx, args.ny, viscous=not args.euler, ibm=not args.euler)
     ncell = args.nx * args.ny
     stream = torch.cuda.current_stream()

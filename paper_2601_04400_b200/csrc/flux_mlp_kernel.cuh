@@ -39,8 +39,10 @@ constexpr int MLP_OFF_W3 = MLP_OFF_W2 + 64 * 64 * 2;  // [16 x 64] 2 KB
 constexpr int MLP_WBLOB = MLP_OFF_W3 + 16 * 64 * 2;   // 14336 B of weights, then 132 floats of biases
 constexpr int MLP_OFF_BIAS = MLP_WBLOB;               // b1[64] b2[64] b3[4]
 constexpr int MLP_BLOB = MLP_OFF_BIAS + 132 * 4;      // what jxs_set_flux_mlp uploads
-constexpr int MLP_OFF_A1 = 14976;                     // 2 tiles [128 x 32] bf16, 8 KB each
-constexpr int MLP_OFF_A2 = MLP_OFF_A1 + 2 * 8192;     // 2 tiles [128 x 64] bf16, 16 KB each
+constexpr int MLP_OFF_A1 = 14976;                     // 2 tiles [128 x 32] bf16, 8 KB each ...
+constexpr int MLP_OFF_A2 = MLP_OFF_A1;                // ... inside the 2 tiles [128 x 64] bf16, 16 KB each, of the
+                                                      // hidden layers (written after layer 1 has read its operands):
+                                                      // 54 KB per CTA, 4 CTAs = 16 warps and all 512 TMEM columns per SM
 constexpr int MLP_OFF_RING = MLP_OFF_A2 + 2 * 16384;  // [6][133] uint2
 constexpr int MLP_OFF_BAR = MLP_OFF_RING + MLP_RING * MLP_RW * 8 + 8;
 constexpr int MLP_SMEM = MLP_OFF_BAR + 16;
@@ -150,7 +152,7 @@ __device__ __forceinline__ void hidden_epilogue(uint32_t taddr, const float* __r
 }
 
 template <typename T>
-__global__ void __launch_bounds__(MLP_TILE, 3) flux_mlp_kernel(const MlpArgs<T> A) {
+__global__ void __launch_bounds__(MLP_TILE, 4) flux_mlp_kernel(const MlpArgs<T> A) {
   extern __shared__ __align__(128) unsigned char sm[];
   __shared__ uint32_t tmem_slot;
   const int t = threadIdx.x, warp = t >> 5;
@@ -170,9 +172,6 @@ __global__ void __launch_bounds__(MLP_TILE, 3) flux_mlp_kernel(const MlpArgs<T> 
   // ---- one-time set-up: weights -> smem, zero the K padding of the layer-1 A tiles, TMEM, mbarrier
   for (int i = t; i < MLP_BLOB / 16; i += MLP_TILE)
     reinterpret_cast<uint4*>(sm)[i] = reinterpret_cast<const uint4*>(A.blob)[i];
-#pragma unroll
-  for (int tile = 0; tile < 2; ++tile)
-    *reinterpret_cast<uint4*>(sm + MLP_OFF_A1 + tile * 8192 + 3 * 2048 + t * 16) = make_uint4(0, 0, 0, 0);
   if (t == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(1) : "memory");
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -230,6 +229,9 @@ __global__ void __launch_bounds__(MLP_TILE, 3) flux_mlp_kernel(const MlpArgs<T> 
       const uint2* rx = ring + sr * MLP_RW + t;
       unsigned char* a1x = sm + MLP_OFF_A1 + t * 16;
       unsigned char* a1y = a1x + 8192;
+      // K = 24 padded to 32: the last chunk is zero (the hidden layers' operands overwrite it every row)
+      *reinterpret_cast<uint4*>(a1x + 3 * 2048) = make_uint4(0, 0, 0, 0);
+      *reinterpret_cast<uint4*>(a1y + 3 * 2048) = make_uint4(0, 0, 0, 0);
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
         const uint2 e0 = rx[2 * c], e1 = rx[2 * c + 1];

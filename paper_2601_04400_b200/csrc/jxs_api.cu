@@ -621,10 +621,10 @@ int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[
   if (!s->d_dG) { CU(cudaMalloc(&s->d_dG, fbytes)); CU(cudaMemset(s->d_dG, 0, fbytes)); }
   CU(cudaMemcpy(s->d_mlp_blob, blob.data(), MLP_BLOB, cudaMemcpyHostToDevice));
   for (int k = 0; k < 4; ++k) { s->in_scale[k] = in_scale[k]; s->out_scale[k] = out_scale[k]; }
-  // strips of 128 faces x row segments: fill 3 resident CTAs per SM, 5 warm-up rows per segment
+  // strips of 128 faces x row segments: fill 4 resident CTAs per SM, 5 warm-up rows per segment
   s->mlp_strips = (s->nx + 1 + MLP_TILE - 1) / MLP_TILE;
   const int nrows = s->ny + 1;
-  const long long slots = (long long)s->num_sms * 3;
+  const long long slots = (long long)s->num_sms * 4;
   int segs = (int)std::max<long long>(1, slots / s->mlp_strips);
   int rps = std::max((nrows + segs - 1) / segs, std::min(nrows, 16));
   s->mlp_rows_per_seg = rps;
