@@ -138,6 +138,55 @@ def run_reference(args, rank):
         "gpu_launches": 0}))
 
 
+def run_sod1d(args, rank, world, local_rank, dist, barrier, tdt):
+    """the paper's 1D Sod workload at 9e6 degrees of freedom (3e6 cells x 3
+    variables) through the one-dimensional stage kernel, SSP-RK3 with the CFL step on the device."""
+    import torch
+    from paper_2601_04400_b200 import jxs, workloads as wl
+    nx = 3_000_000
+    case = wl.sod1d(nx)
+    stream = torch.cuda.current_stream()
+    solver = jxs.Solver.from_case(case, dtype=tdt, stream=stream)
+    U = torch.tensor(case["U0"], dtype=tdt, device="cuda")
+    K, W = args.steps, args.warmup
+    solver.step(U, 0.4, W)
+    solver.set_profiling(True)
+    sampler = ClockSampler(local_rank)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = solver.launch_count()
+    barrier()
+    sampler.start()
+    e0.record(stream)
+    solver.step(U, 0.4, K)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = max_over_ranks(e0.elapsed_time(e1), dist, "cuda")
+    stage_ms, stage_n = solver.stage_time()
+    if not bool(torch.isfinite(U).all()):
+        raise SystemExit("bench.py: non-finite state after the timed region")
+    if rank != 0:
+        return
+    # one-dimensional stage: WENO 4 x 97 + HLLC 85 + primitives 10 + divergence 8 + RK 16 + wavespeed 8 flop, 85.33 B
+    flop = 515.0
+    avg = stage_ms / max(stage_n, 1)
+    achieved = flop * nx / (avg * 1e-3) / 1e12
+    peak = PEAK_FP64_TFLOPS if args.dtype == "f64" else PEAK_FP32_TFLOPS
+    print(json.dumps({
+        "metric": METRIC, "value": aggregate_rate(nx, K, world, ms), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
+        "data": "synthetic",
+        "config": {"workload": "sod1d_3000000 (the paper's 1D Sod tube at 9e6 degrees of freedom, PAPER.md L149)", "cfl": 0.4,
+                   "rk": "SSP-RK3", "cells": nx, "l2": "3 x 96 MB of state buffers vs 126 MB of L2, no flush needed",
+                   "parallelism": "replicas" if world > 1 else "single GPU"},
+        "clocks": clocks, "gpu_launches": solver.launch_count() - launches0,
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                     "traffic": None, "kernel": "jxs::stage1d_kernel", "avg_launch_ms": avg, "launches_timed": stage_n,
+                     "alg_flop_per_cell_stage": flop, "alg_bytes_per_cell_stage": ALG_BYTES[args.dtype],
+                     "hbm_side_gbs": ALG_BYTES[args.dtype] * nx / (avg * 1e-3) / 1e9},
+        "e2e": None, "cpu_baseline": None}))
+
+
 def run_c5(args, rank, world, local_rank, dist, barrier, tdt):
     """BASELINE.json configs[4]: 16 handles x (1024x512 shock-cylinder, Mach ~ U[1.5,3]) with the bf16 flux MLP
     fused into the fp64 HLLC flux; one stream per handle, jxs_step_async on each, aggregate Mcell-stage/s."""
@@ -229,9 +278,10 @@ def main():
     ap.add_argument("--euler", action="store_true", help="mu = 0, no IBM (not the headline config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile-kernels", action="store_true", help="c5 only: per-kernel CUDA-event spans")
-    ap.add_argument("--workload", choices=("c4", "c5"), default="c4",
+    ap.add_argument("--workload", choices=("c4", "c5", "sod1d"), default="c4",
                     help="c4 = the headline throughput case (default); c5 = BASELINE.json configs[4]: 16 independent "
-                         "1024x512 shock-cylinder runs with the per-face flux MLP, one stream per handle")
+                         "1024x512 shock-cylinder runs with the per-face flux MLP, one stream per handle; sod1d = the "
+                         "paper's 1D Sod tube at its largest size (3e6 cells = 9e6 degrees of freedom, PAPER.md L149)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "jxs" else args.warmup
 
@@ -262,6 +312,9 @@ def main():
     tdt = torch.float64 if args.dtype == "f64" else torch.float32
     if args.workload == "c5":
         run_c5(args, rank, world, local_rank, dist, barrier, tdt)
+        return
+    if args.workload == "sod1d":
+        run_sod1d(args, rank, world, local_rank, dist, barrier, tdt)
         return
     case = wl.throughput_case(args.nx, args.ny, viscous=not args.euler, ibm=not args.euler)
     ncell = args.nx * args.ny

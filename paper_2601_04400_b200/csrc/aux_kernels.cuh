@@ -106,7 +106,8 @@ template <typename T>
 __global__ void ghost_fill_kernel(T* __restrict__ U, GridDims g, BcSpec bc, IbmList ibm, T gamma) {
   const int nxp = g.nx + 6, nyp = g.ny + 6;
   const int side_cells = 6 * g.ny;            // x-ghost columns of the interior rows
-  const int nframe = side_cells + 6 * nxp;    // + full ghost rows (incl. corners)
+  // + full ghost rows (incl. corners); a one-dimensional problem (ny = 1) has no use for them
+  const int nframe = side_cells + (g.ny > 1 ? 6 * nxp : 0);
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t < nframe) {
     int ip, jp;  // padded indices in [0,nxp) x [0,nyp)

@@ -18,6 +18,7 @@
 #include "aux_kernels.cuh"
 #include "flux_mlp_kernel.cuh"
 #include "stage_kernel.cuh"
+#include "stage1d_kernel.cuh"
 
 using namespace jxs;
 
@@ -227,7 +228,10 @@ cudaError_t launch_stage(jxs_solver* s, const void* Uin, const void* U0, void* U
     cudaEventRecord(e0, s->stream);
   }
   cudaError_t e;
-  if (s->mlp_on) {
+  if (s->ny == 1) {  // one-dimensional problems: stage1d_kernel.cuh
+    stage1d_kernel<T><<<(s->nx + S1D_OUT - 1) / S1D_OUT, S1D_TB, 0, s->stream>>>(A);
+    e = cudaGetLastError();
+  } else if (s->mlp_on) {
     if (visc) e = artv ? launch_stage_t<T, true, true, true>(s, A) : launch_stage_t<T, true, false, true>(s, A);
     else e = artv ? launch_stage_t<T, false, true, true>(s, A) : launch_stage_t<T, false, false, true>(s, A);
   } else {
@@ -246,7 +250,7 @@ cudaError_t stage(jxs_solver* s, const void* Uin, const void* U0, void* Uout, in
 }
 
 cudaError_t ghost_fill(jxs_solver* s, void* U) {
-  const int nframe = 6 * s->ny + 6 * (s->nx + 6);
+  const int nframe = 6 * s->ny + (s->ny > 1 ? 6 * (s->nx + 6) : 0);
   const int total = nframe + s->n_ghost;
   IbmList L{s->d_cell, s->d_donor, s->d_w, s->d_nrm, s->n_ghost};
   const int bs = 128;
@@ -449,7 +453,9 @@ int jxs_create(int nx, int ny, double dx, double dy, double gamma, double mu, do
   if (!out) return JXS_EINVAL;
   *out = nullptr;
   if (!bc) return JXS_EINVAL;
-  if (nx < 8 || ny < 8 || !(dx > 0) || !(dy > 0) || !(gamma > 1) || !(mu >= 0) || (mu > 0 && !(Pr > 0))) return JXS_EINVAL;
+  if (nx < 8 || (ny < 8 && ny != 1) || !(dx > 0) || !(dy > 0) || !(gamma > 1) || !(mu >= 0) || (mu > 0 && !(Pr > 0)))
+    return JXS_EINVAL;
+  if (ny == 1 && mu > 0) return JXS_EINVAL;  // the one-dimensional path is Euler (+ the nu term of Eq. 10)
   if (dtype != JXS_F64 && dtype != JXS_F32) return JXS_EINVAL;
   const int kinds[4] = {bc->xlo, bc->xhi, bc->ylo, bc->yhi};
   for (int k : kinds)
@@ -463,6 +469,7 @@ int jxs_create(int nx, int ny, double dx, double dy, double gamma, double mu, do
   jxs_solver* s = new (std::nothrow) jxs_solver;
   if (!s) return JXS_ENOMEM;
   s->nx = nx; s->ny = ny; s->dx = dx; s->dy = dy; s->gamma = gamma; s->mu = mu; s->Pr = Pr; s->bc = *bc;
+  if (ny == 1) s->bc.ylo = s->bc.yhi = JXS_BC_TRANSMISSIVE;  // the ghost rows of a single row are copies of it
   s->dtype = dtype;
   s->elem = dtype == JXS_F64 ? 8 : 4;
   s->stream = (cudaStream_t)cuda_stream;
@@ -524,6 +531,7 @@ int jxs_set_ibm(jxs_solver* s, const double* phi) {
   CU(cudaStreamSynchronize(s->stream));
   free_ibm(s);
   if (!phi) return JXS_OK;
+  if (s->ny == 1) return fail(s, JXS_EINVAL, "no immersed boundary in one-dimensional problems");
   const int nx = s->nx, ny = s->ny;
   const double dx = s->dx, dy = s->dy;
   // classification (R9 I1, I2): 1 = fluid in `fl`; ghost = non-fluid cell that some fluid cell's
@@ -601,6 +609,7 @@ int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[
   if (!s) return JXS_EINVAL;
   CU(cudaStreamSynchronize(s->stream));
   if (!weights) { s->mlp_on = false; return JXS_OK; }
+  if (s->ny == 1) return fail(s, JXS_EINVAL, "no flux MLP in one-dimensional problems");
   if (!in_scale || !out_scale) return fail(s, JXS_EINVAL, "in_scale / out_scale is NULL");
   for (int k = 0; k < 4; ++k)
     if (!(in_scale[k] > 0) || !std::isfinite(in_scale[k]) || !std::isfinite(out_scale[k]))

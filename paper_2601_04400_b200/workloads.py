@@ -64,6 +64,30 @@ def sod(nx=128, ny=128, axis=0, gamma=GAMMA):
                 dx=dx, dy=dy, gamma=gamma, mu=0.0, Pr=0.72, bc=bc, phi=None)
 
 
+def sod1d(nx=500, gamma=GAMMA):
+    """The paper's 1D Sod shock tube (Eq. 17) on [0,1]: fields [4][1][nx], ny = 1, dy = dx."""
+    dx = 1.0 / nx
+    x = (np.arange(nx) + 0.5) * dx
+    left = (x < 0.5)[None, :]
+    rho = np.where(left, 1.0, 0.125)
+    p = np.where(left, 1.0, 0.1)
+    z = np.zeros_like(rho)
+    bc = dict(xlo="transmissive", xhi="transmissive", ylo="transmissive", yhi="transmissive")
+    return dict(name=f"sod1d_{nx}", U0=cons_from_prim(rho, z, z, p, gamma), nx=nx, ny=1, dx=dx, dy=dx, gamma=gamma,
+                mu=0.0, Pr=0.72, bc=bc, phi=None)
+
+
+def as_rows(case, ny=8):
+    """A 1D case repeated over ny identical rows, periodic in y: the planar 2D problem whose every row is the 1D one
+    (identical rows make the y-fluxes cancel exactly).  This is how the 2D oracle checks the 1D path."""
+    c = dict(case)
+    c["U0"] = np.ascontiguousarray(np.repeat(case["U0"], ny, axis=1))
+    c["ny"] = ny
+    c["bc"] = dict(case["bc"], ylo="periodic", yhi="periodic")
+    c["name"] = case["name"] + f"_as_{ny}_rows"
+    return c
+
+
 # --------------------------------------------------------------------------- C2
 def vortex_primitives(x, y, gamma=GAMMA, strength=5.0, xc=5.0, yc=5.0, u0=1.0, v0=1.0):
     """Isentropic vortex (config 2) point values, free stream (1, u0, v0, 1)."""

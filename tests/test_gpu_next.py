@@ -76,3 +76,72 @@ def test_async_handles_on_streams_match_synchronous_calls():
     for s, U, (want, tm) in zip(solvers, Us, ref):
         assert np.array_equal(U.cpu().numpy(), want)
         assert s.time() == tm
+
+
+# ------------------------------------------------------------------ rank 2, second half: the 1D path (ny = 1)
+def oracle_rows(case):
+    """the 2D oracle on the 1D problem repeated over 8 identical rows (periodic in y)"""
+    from oracle import jxo
+    c = wl.as_rows(case)
+    return c, jxo.Oracle(c["nx"], c["ny"], c["dx"], c["dy"], c["gamma"], c["mu"], c["Pr"], c["bc"])
+
+
+@pytest.mark.parametrize("nx", [200, 254, 255, 1021])  # one CTA short, exactly one, one cell more, ragged
+def test_1d_rhs_and_steps_match_the_planar_oracle(nx):
+    case = wl.sod1d(nx)
+    c2, o = oracle_rows(case)
+    s = jxs().Solver.from_case(case)
+    got = s.rhs(dev(case["U0"])).cpu().numpy()
+    want = o.rhs(c2["U0"])
+    assert np.array_equal(want[:, 0], want[:, 5])          # the oracle's rows stay identical
+    assert rel_err(got, want[:, :1]) <= 1e-12
+    U = dev(case["U0"])
+    s.step(U, 0.4, 60)
+    assert rel_err(U.cpu().numpy(), o.step(c2["U0"], 0.4, 60)[:, :1]) <= 1e-9
+    assert abs(s.max_wavespeed(dev(case["U0"])) / o.max_wavespeed(c2["U0"]) - 1) <= 1e-14
+
+
+def test_1d_paper_literal_euler_with_nu_and_fp32():
+    case = wl.sod1d(300)
+    c2, o = oracle_rows(case)
+    o.set_artificial_viscosity(1e-3)
+    s = jxs().Solver.from_case(case)
+    s.set_artificial_viscosity(1e-3)
+    s.set_time_integrator(jxs().EULER)
+    U = dev(case["U0"])
+    s.step(U, 0.2, 50)
+    want = oracle_forward_euler(o, c2["U0"], 0.2, 50, case["dx"])
+    assert rel_err(U.cpu().numpy(), want[:, :1]) <= 1e-9
+    s32 = jxs().Solver.from_case(case, dtype=torch.float32)
+    o2 = oracle_rows(case)[1]
+    got = s32.rhs(dev(case["U0"], torch.float32)).cpu().numpy()
+    assert rel_err(got, o2.rhs(c2["U0"])[:, :1]) <= 1e-4
+
+
+def test_1d_sod_converges_to_the_exact_solution():
+    """PAPER.md L141-147 (Fig. 2): the solution at t = 0.2 approaches the exact Riemann solution under refinement"""
+    import refs
+    errs = []
+    for nx in (500, 2000):
+        case = wl.sod1d(nx)
+        s = jxs().Solver.from_case(case)
+        U = dev(case["U0"])
+        t, dt = 0.0, 0.2 / (2 * nx)  # fixed step well inside the CFL limit (s_max ~ 2.2), lands on t = 0.2 exactly
+        s.step_fixed_dt(U, dt, 2 * nx)
+        assert abs(s.time()[0] - 0.2) < 1e-12
+        rho = U.cpu().numpy()[0, 0]
+        x = (np.arange(nx) + 0.5) / nx
+        exact = np.array([refs.riemann_sample((xx - 0.5) / 0.2, 1.0, 0.0, 1.0, 0.125, 0.0, 0.1)[0] for xx in x])
+        errs.append(np.mean(np.abs(rho - exact)))
+    assert errs[1] < 0.4 * errs[0] and errs[1] < 2e-3, errs
+
+
+def test_1d_rejects_what_it_does_not_do():
+    case = wl.sod1d(64)
+    with pytest.raises(jxs().JxsError):
+        jxs().Solver(64, 1, 1 / 64, 1 / 64, 1.4, 1e-3, 0.72, case["bc"])   # viscous 1D
+    s = jxs().Solver.from_case(case)
+    with pytest.raises(jxs().JxsError):
+        s.set_ibm(-np.ones((1, 64)))
+    with pytest.raises(jxs().JxsError):
+        s.set_flux_mlp(wl.mlp_weights(), *wl.mlp_scales())
