@@ -60,6 +60,7 @@ struct MlpArgs {
   int nstrips, rows_per_seg;
   T g1;                  // gamma - 1
   T inv_scale[4];        // 1 / in_scale of (rho, u_n, u_t, p)
+  float bias[132];       // b1[64] b2[64] b3[4]: kernel parameters, i.e. constant-bank operands of the bias adds
 };
 
 // ---- tcgen05 / TMEM wrappers (PTX ISA: tcgen05.*) ------------------------------------------------
@@ -130,7 +131,7 @@ __device__ __forceinline__ void mbar_wait_spin(uint32_t bar, uint32_t parity) {
 }
 
 // hidden layer epilogue of one tile: 64 pre-activations of my face (TMEM) -> + bias -> tanh -> bf16 -> A2 row
-__device__ __forceinline__ void hidden_epilogue(uint32_t taddr, const float* __restrict__ bias, unsigned char* a2_tile, int m) {
+__device__ __forceinline__ void hidden_epilogue(uint32_t taddr, const float (&bias)[64], unsigned char* a2_tile, int m) {
 #pragma unroll
   for (int half = 0; half < 2; ++half) {
     uint32_t v[32];
@@ -166,7 +167,9 @@ __global__ void __launch_bounds__(MLP_TILE, 4) flux_mlp_kernel(const MlpArgs<T> 
 
   const uint32_t sm_u32 = (uint32_t)__cvta_generic_to_shared(sm);
   const uint32_t bar = sm_u32 + MLP_OFF_BAR;
-  const float* bias = reinterpret_cast<const float*>(sm + MLP_OFF_BIAS);
+  float b1[64], b2[64];  // compile-time indexed below: they stay constant-bank operands
+#pragma unroll
+  for (int k = 0; k < 64; ++k) { b1[k] = A.bias[k]; b2[k] = A.bias[64 + k]; }
   uint2* ring = reinterpret_cast<uint2*>(sm + MLP_OFF_RING);
 
   // ---- one-time set-up: weights -> smem, zero the K padding of the layer-1 A tiles, TMEM, mbarrier
@@ -260,8 +263,8 @@ __global__ void __launch_bounds__(MLP_TILE, 4) flux_mlp_kernel(const MlpArgs<T> 
     tc_fence_after();
 
     // ---- hidden layer 1 -> A2, layer 2
-    hidden_epilogue(tlane, bias, sm + MLP_OFF_A2, t);
-    hidden_epilogue(tlane + 64, bias, sm + MLP_OFF_A2 + 16384, t);
+    hidden_epilogue(tlane, b1, sm + MLP_OFF_A2, t);
+    hidden_epilogue(tlane + 64, b1, sm + MLP_OFF_A2 + 16384, t);
     fence_async_smem();
     tc_fence_before();
     __syncthreads();
@@ -279,8 +282,8 @@ __global__ void __launch_bounds__(MLP_TILE, 4) flux_mlp_kernel(const MlpArgs<T> 
     tc_fence_after();
 
     // ---- hidden layer 2 -> A2 (layer 2 has finished reading it), output layer (N = 16)
-    hidden_epilogue(tlane, bias + 64, sm + MLP_OFF_A2, t);
-    hidden_epilogue(tlane + 64, bias + 64, sm + MLP_OFF_A2 + 16384, t);
+    hidden_epilogue(tlane, b2, sm + MLP_OFF_A2, t);
+    hidden_epilogue(tlane + 64, b2, sm + MLP_OFF_A2 + 16384, t);
     fence_async_smem();
     tc_fence_before();
     __syncthreads();
@@ -307,8 +310,8 @@ __global__ void __launch_bounds__(MLP_TILE, 4) flux_mlp_kernel(const MlpArgs<T> 
         const size_t o = (size_t)r * A.pitch + col;
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-          A.dF[k * A.plane + o] = __uint_as_float(yx[k]) + bias[128 + k];
-          A.dG[k * A.plane + o] = __uint_as_float(yy[k]) + bias[128 + k];
+          A.dF[k * A.plane + o] = __uint_as_float(yx[k]) + A.bias[128 + k];
+          A.dG[k * A.plane + o] = __uint_as_float(yy[k]) + A.bias[128 + k];
         }
       }
     }

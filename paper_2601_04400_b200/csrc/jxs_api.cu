@@ -58,6 +58,7 @@ struct jxs_solver {
   float* d_dF = nullptr;   // [4][ny+6][pitch] network outputs at right faces
   float* d_dG = nullptr;   // same at top faces
   double in_scale[4] = {1, 1, 1, 1}, out_scale[4] = {1, 1, 1, 1};
+  float mlp_bias[132] = {0};
   int mlp_strips = 0, mlp_rows_per_seg = 0, mlp_grid = 0;
   double mlp_ms = 0;
   long long mlp_launches = 0;
@@ -271,6 +272,7 @@ cudaError_t launch_flux_mlp(jxs_solver* s, const void* U) {
   A.nstrips = s->mlp_strips; A.rows_per_seg = s->mlp_rows_per_seg;
   A.g1 = (T)(s->gamma - 1.0);
   for (int k = 0; k < 4; ++k) A.inv_scale[k] = (T)(1.0 / s->in_scale[k]);
+  std::memcpy(A.bias, s->mlp_bias, sizeof(A.bias));
   auto kern = flux_mlp_kernel<T>;
   static bool configured = false;
   if (!configured) {
@@ -624,6 +626,7 @@ int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[
   pack_canonical(W3, 4, 64, 16, 64, blob.data() + MLP_OFF_W3);
   float* bias = reinterpret_cast<float*>(blob.data() + MLP_OFF_BIAS);
   std::memcpy(bias, b1, 64 * 4); std::memcpy(bias + 64, b2, 64 * 4); std::memcpy(bias + 128, b3, 4 * 4);
+  std::memcpy(s->mlp_bias, bias, sizeof(s->mlp_bias));
   const size_t fbytes = (size_t)4 * s->plane * sizeof(float);
   if (!s->d_mlp_blob) CU(cudaMalloc(&s->d_mlp_blob, MLP_BLOB));
   if (!s->d_dF) { CU(cudaMalloc(&s->d_dF, fbytes)); CU(cudaMemset(s->d_dF, 0, fbytes)); }
