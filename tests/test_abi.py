@@ -69,3 +69,28 @@ def test_argument_checks_do_not_need_a_device():
     assert L.jxs_create(16, 16, 0.1, 0.1, 1.4, 0.0, 0.72, None, 0, None, C.byref(h)) == jxs.EINVAL
     assert L.jxs_step(None, None, 0.4, 1) == jxs.EINVAL
     assert L.jxs_last_error(None) == b"null handle"
+
+
+def test_argument_checks_of_the_next_rows():
+    """one-dimensional path and the entry points added for SURVEY.md section 8(f): checks that need no device"""
+    from paper_2601_04400_b200 import jxs
+    L = jxs.lib()
+    h = C.c_void_p()
+    b = jxs.make_bc(dict(xlo="transmissive", xhi="transmissive", ylo="transmissive", yhi="transmissive"))
+    assert L.jxs_create(64, 5, 0.1, 0.1, 1.4, 0.0, 0.72, C.byref(b), 0, None, C.byref(h)) == jxs.EINVAL   # 1 < ny < 8
+    assert L.jxs_create(64, 1, 0.1, 0.1, 1.4, 1e-3, 0.72, C.byref(b), 0, None, C.byref(h)) == jxs.EINVAL  # viscous 1D
+    assert L.jxs_create(4, 1, 0.1, 0.1, 1.4, 0.0, 0.72, C.byref(b), 0, None, C.byref(h)) == jxs.EINVAL
+    assert L.jxs_step_async(None, None, 0.4, 1) == jxs.EINVAL
+    assert L.jxs_wait(None) == jxs.EINVAL
+    assert L.jxs_set_time_integrator(None, 0) == jxs.EINVAL
+
+
+def test_one_dimensional_workload_is_the_planar_one():
+    import numpy as np
+    from paper_2601_04400_b200 import workloads as wl
+    c1, c2 = wl.sod1d(128), wl.sod(128, 128, 0)
+    assert c1["U0"].shape == (4, 1, 128) and c1["ny"] == 1 and c1["dy"] == c1["dx"]
+    assert np.array_equal(c1["U0"][:, 0], c2["U0"][:, 17])
+    rows = wl.as_rows(c1)
+    assert rows["U0"].shape == (4, 8, 128) and rows["bc"]["ylo"] == "periodic" and rows["bc"]["xlo"] == "transmissive"
+    assert all(np.array_equal(rows["U0"][:, j], c1["U0"][:, 0]) for j in range(8))
