@@ -98,7 +98,9 @@ int jxs_max_wavespeed(jxs_solver*, const void* U, double* smax_host);
 
 /* Advance U in place by nsteps SSP-RK3 steps (R5), dt = cfl*min(dx,dy)/smax evaluated on the
  * device at the start of every step (R6).  JXS_ENUMERIC if a non-finite or non-positive
- * wavespeed was met (U then holds the last state computed).  Synchronises once at the end.   */
+ * wavespeed was met (U then holds the last state computed).  Synchronises once at the end.
+ * For nsteps >= 6 (and jxs_set_profiling off) pairs of steps are replayed from a CUDA graph
+ * captured on a private stream; results are identical to plain launches.                      */
 int jxs_step(jxs_solver*, void* U, double cfl, int nsteps);
 /* Same with a fixed time step.                                                              */
 int jxs_step_fixed_dt(jxs_solver*, void* U, double dt, int nsteps);

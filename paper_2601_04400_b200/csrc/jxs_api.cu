@@ -68,6 +68,12 @@ struct jxs_solver {
   StepState* d_state = nullptr;
   double t = 0, last_dt = 0;
   int scheme = JXS_SSPRK3;
+  // CUDA graph of TWO consecutive steps (after two steps the s_max slot and, for forward Euler, the buffer roles are
+  // back where they started), replayed by jxs_step* when per-kernel profiling is off: small grids are launch-bound
+  cudaStream_t cap_stream = nullptr;
+  cudaGraphExec_t pair_exec = nullptr;
+  double pair_cfl_h = 0, pair_fixed_dt = 0;
+  long long pair_launches = 0;
   int pending_steps = 0;  // steps enqueued by jxs_step_async and not yet waited for
   // work decomposition of the stage kernel
   int nstrips = 0, rows_per_seg = 0, nseg = 0, ntasks = 0, warps = 0, grid = 0;
@@ -351,38 +357,91 @@ void free_ibm(jxs_solver* s) {
   s->n_ghost = 0;
 }
 
-// advance the padded state in buf[0] by nsteps steps; returns in *where the buffer that holds the result.
-// SSP-RK3 (R5): three stages, result back in buf[0].  Forward Euler (Eq. 10 as printed): one stage
-// with (a,b) = (0,1), the two buffers swap roles every step.  cur = index of the valid s_max.
+// one step, enqueued on s->stream.  cur = index of the valid s_max, at = buffer that holds U^n (forward Euler swaps
+// the two buffers every step; SSP-RK3 always starts and ends in buf[0]).
+// SSP-RK3 (R5): three stages.  Forward Euler (Eq. 10 as printed): one stage with (a,b) = (0,1).
+int one_step(jxs_solver* s, double cfl_h, double fixed_dt, int& cur, int& at) {
+  prepare_step_kernel<<<1, 1, 0, s->stream>>>(s->d_state, cur, cfl_h, fixed_dt);
+  s->launches++;
+  CU(cudaGetLastError());
+  unsigned long long* next = &s->d_state->smax_bits[cur ^ 1];
+  if (s->scheme == JXS_EULER) {
+    CU(ghost_fill(s, s->buf[at]));
+    CU(flux_mlp(s, s->buf[at]));
+    CU(stage(s, s->buf[at], nullptr, s->buf[at ^ 1], 0, 0.0, 1.0, next));              // U^{n+1} = U^n + dt L(U^n)
+    at ^= 1;
+  } else {
+    CU(ghost_fill(s, s->buf[0]));
+    CU(flux_mlp(s, s->buf[0]));
+    CU(stage(s, s->buf[0], nullptr, s->buf[1], 0, 0.0, 1.0, nullptr));                  // U1 = U0 + dt L(U0)
+    CU(ghost_fill(s, s->buf[1]));
+    CU(flux_mlp(s, s->buf[1]));
+    CU(stage(s, s->buf[1], s->buf[0], s->buf[2], 0, 0.75, 0.25, nullptr));              // U2 = 3/4 U0 + 1/4 (U1 + dt L(U1))
+    CU(ghost_fill(s, s->buf[2]));
+    CU(flux_mlp(s, s->buf[2]));
+    CU(stage(s, s->buf[2], s->buf[0], s->buf[0], 0, 1.0 / 3.0, 2.0 / 3.0, next));       // U0 = 1/3 U0 + 2/3 (U2 + dt L(U2))
+  }
+  cur ^= 1;
+  return JXS_OK;
+}
+
+void drop_graph(jxs_solver* s) {
+  if (s->pair_exec) cudaGraphExecDestroy(s->pair_exec);
+  s->pair_exec = nullptr;
+}
+
+// capture two steps (from the state cur = 0, at = 0) on a private stream; false = use plain launches
+bool capture_pair(jxs_solver* s, double cfl_h, double fixed_dt) {
+  drop_graph(s);
+  if (!s->cap_stream && cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  cudaStream_t user = s->stream;
+  const long long l0 = s->launches;
+  s->stream = s->cap_stream;
+  bool ok = cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+  int cur = 0, at = 0;
+  if (ok) {
+    ok = one_step(s, cfl_h, fixed_dt, cur, at) == JXS_OK && one_step(s, cfl_h, fixed_dt, cur, at) == JXS_OK;
+    cudaGraph_t g = nullptr;
+    if (cudaStreamEndCapture(s->cap_stream, &g) != cudaSuccess) ok = false;
+    if (ok && cudaGraphInstantiate(&s->pair_exec, g, 0) != cudaSuccess) ok = false;
+    if (g) cudaGraphDestroy(g);
+  }
+  s->stream = user;
+  s->pair_launches = s->launches - l0;
+  s->launches = l0;
+  if (!ok) {
+    cudaGetLastError();
+    drop_graph(s);
+    return false;
+  }
+  s->pair_cfl_h = cfl_h;
+  s->pair_fixed_dt = fixed_dt;
+  return true;
+}
+
+// advance the padded state in buf[0] by nsteps steps; returns in *where the buffer that holds the result
 int run_steps(jxs_solver* s, double cfl, double fixed_dt, int nsteps, int* where) {
-  const double h = std::min(s->dx, s->dy);
+  const double cfl_h = cfl * std::min(s->dx, s->dy);
   int cur = 0, at = 0;
   s->events_used = 0;
   s->mlp_events_used = 0;
   if (!(fixed_dt > 0)) CU(wavespeed(s, s->buf[0], &s->d_state->smax_bits[0]));
-  for (int n = 0; n < nsteps; ++n) {
-    prepare_step_kernel<<<1, 1, 0, s->stream>>>(s->d_state, cur, cfl * h, fixed_dt);
-    s->launches++;
-    CU(cudaGetLastError());
-    unsigned long long* next = &s->d_state->smax_bits[cur ^ 1];
-    if (s->scheme == JXS_EULER) {
-      CU(ghost_fill(s, s->buf[at]));
-      CU(flux_mlp(s, s->buf[at]));
-      CU(stage(s, s->buf[at], nullptr, s->buf[at ^ 1], 0, 0.0, 1.0, next));              // U^{n+1} = U^n + dt L(U^n)
-      at ^= 1;
-    } else {
-      CU(ghost_fill(s, s->buf[0]));
-      CU(flux_mlp(s, s->buf[0]));
-      CU(stage(s, s->buf[0], nullptr, s->buf[1], 0, 0.0, 1.0, nullptr));                  // U1 = U0 + dt L(U0)
-      CU(ghost_fill(s, s->buf[1]));
-      CU(flux_mlp(s, s->buf[1]));
-      CU(stage(s, s->buf[1], s->buf[0], s->buf[2], 0, 0.75, 0.25, nullptr));              // U2 = 3/4 U0 + 1/4 (U1 + dt L(U1))
-      CU(ghost_fill(s, s->buf[2]));
-      CU(flux_mlp(s, s->buf[2]));
-      CU(stage(s, s->buf[2], s->buf[0], s->buf[0], 0, 1.0 / 3.0, 2.0 / 3.0, next));       // U0 = 1/3 U0 + 2/3 (U2 + dt L(U2))
+  int n = 0;
+  static const bool no_graph = getenv("JXS_NO_GRAPH") != nullptr;
+  if (!s->profiling && !no_graph && nsteps >= 6) {
+    // the first pair runs as plain launches (it also configures the kernels' attributes outside any capture)
+    for (; n < 2; ++n) { const int rc = one_step(s, cfl_h, fixed_dt, cur, at); if (rc != JXS_OK) return rc; }
+    if ((s->pair_exec && s->pair_cfl_h == cfl_h && s->pair_fixed_dt == fixed_dt) || capture_pair(s, cfl_h, fixed_dt)) {
+      for (; n + 2 <= nsteps; n += 2) {
+        CU(cudaGraphLaunch(s->pair_exec, s->stream));
+        s->launches += s->pair_launches;
+      }
     }
-    cur ^= 1;
   }
+  for (; n < nsteps; ++n) { const int rc = one_step(s, cfl_h, fixed_dt, cur, at); if (rc != JXS_OK) return rc; }
   *where = at;
   return JXS_OK;
 }
@@ -516,6 +575,8 @@ int jxs_create(int nx, int ny, double dx, double dy, double gamma, double mu, do
 void jxs_destroy(jxs_solver* s) {
   if (!s) return;
   cudaStreamSynchronize(s->stream);
+  drop_graph(s);
+  if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
   for (int b = 0; b < 3; ++b) cudaFree(s->buf[b]);
   cudaFree(s->stage_io);
   cudaFree(s->d_state);
@@ -530,6 +591,7 @@ const char* jxs_last_error(const jxs_solver* s) { return s ? s->err.c_str() : "n
 
 int jxs_set_ibm(jxs_solver* s, const double* phi) {
   if (!s) return JXS_EINVAL;
+  drop_graph(s);
   CU(cudaStreamSynchronize(s->stream));
   free_ibm(s);
   if (!phi) return JXS_OK;
@@ -609,6 +671,7 @@ int jxs_set_ibm(jxs_solver* s, const double* phi) {
 
 int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[4], const double out_scale[4]) {
   if (!s) return JXS_EINVAL;
+  drop_graph(s);
   CU(cudaStreamSynchronize(s->stream));
   if (!weights) { s->mlp_on = false; return JXS_OK; }
   if (s->ny == 1) return fail(s, JXS_EINVAL, "no flux MLP in one-dimensional problems");
@@ -647,6 +710,7 @@ int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[
 
 int jxs_set_artificial_viscosity(jxs_solver* s, double nu) {
   if (!s) return JXS_EINVAL;
+  drop_graph(s);
   if (!(nu >= 0)) return fail(s, JXS_EINVAL, "nu must be >= 0");
   s->nu = nu;
   return JXS_OK;
@@ -706,6 +770,7 @@ int jxs_wait(jxs_solver* s) {
 }
 int jxs_set_time_integrator(jxs_solver* s, int scheme) {
   if (!s) return JXS_EINVAL;
+  drop_graph(s);
   if (scheme != JXS_SSPRK3 && scheme != JXS_EULER) return fail(s, JXS_EINVAL, "unknown time integrator");
   s->scheme = scheme;
   return JXS_OK;
