@@ -168,7 +168,7 @@ void choose_decomposition(jxs_solver* s) {
   int best_rps = lo;
   for (int rps = lo; rps <= s->ny; ++rps)
     if (cost[rps] <= 1.01 * best) best_rps = rps;  // the longest segments among the near-optimal
-  if (const char* e = getenv("JXS_DBG_ROWS_PER_SEG")) best_rps = std::max(1, std::min(s->ny, atoi(e)));
+  if (const char* e = getenv("JXS_ROWS_PER_SEG")) best_rps = std::max(1, std::min(s->ny, atoi(e)));
   s->rows_per_seg = best_rps;
   s->nseg = (s->ny + best_rps - 1) / best_rps;
   s->ntasks = s->nseg * s->nstrips;
@@ -189,12 +189,10 @@ cudaError_t launch_stage_t(jxs_solver* s, const StageArgs<T>& a) {
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  static const size_t extra = getenv("JXS_DBG_EXTRA_SMEM") ? (size_t)atoi(getenv("JXS_DBG_EXTRA_SMEM")) : 0;
-  if (extra) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem + extra));
   int bi = 0;  // which padded buffer is U_in
   while (bi < 3 && s->buf[bi] != (const void*)a.Uin) ++bi;
   if (bi == 3) return cudaErrorInvalidValue;
-  kern<<<s->grid, s->warps * 32, smem + extra, s->stream>>>(a, s->tm_row[bi], s->tm_epi[bi], s->tm_epi[0]);
+  kern<<<s->grid, s->warps * 32, smem, s->stream>>>(a, s->tm_row[bi], s->tm_epi[bi], s->tm_epi[0]);
   return cudaGetLastError();
 }
 
