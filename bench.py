@@ -200,6 +200,7 @@ def run_c5(args, rank, world, local_rank, dist, barrier, tdt):
     for c, st in zip(cases, streams):
         s = jxs.Solver.from_case(c, dtype=tdt, stream=st)
         s.set_flux_mlp(w, ins, outs)
+        s.set_concurrent_handles(len(cases))
         solvers.append(s)
         Us.append(torch.tensor(c["U0"], dtype=tdt, device="cuda"))
     ncell = sum(c["nx"] * c["ny"] for c in cases)

@@ -114,6 +114,10 @@ int jxs_rhs_host(jxs_solver*, const void* U_host, void* dUdt_host);
  * U must stay valid until jxs_wait returns.                                                  */
 int jxs_step_async(jxs_solver*, void* U, double cfl, int nsteps);
 int jxs_wait(jxs_solver*);
+/* Performance hint for such ensembles: n handles of about this size step concurrently, so this handle sizes
+ * its tasks for 1/n of the GPU (longer row segments, fewer warm-up rows) instead of trying to fill it alone.
+ * Results do not change.  Default 1.                                                           */
+int jxs_set_concurrent_handles(jxs_solver*, int n);
 /* Time integrator of jxs_step*: JXS_SSPRK3 (default, R5) or JXS_EULER, the forward-Euler update the paper
  * prints (Eq. 10; with jxs_set_artificial_viscosity it is Eq. 10 term by term) = one stage
  * with (a,b) = (0,1).  SURVEY.md section 8(f) rank 2.                                           */

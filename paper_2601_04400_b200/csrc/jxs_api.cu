@@ -77,6 +77,7 @@ struct jxs_solver {
   int pending_steps = 0;  // steps enqueued by jxs_step_async and not yet waited for
   // work decomposition of the stage kernel
   int nstrips = 0, rows_per_seg = 0, nseg = 0, ntasks = 0, warps = 0, grid = 0;
+  int share = 1;  // handles of about this size that step concurrently (jxs_set_concurrent_handles)
   // bookkeeping
   long long launches = 0;
   bool profiling = false;
@@ -153,7 +154,7 @@ void choose_decomposition(jxs_solver* s) {
   const int SOUT = s->dtype == JXS_F64 ? sout<double>() : sout<float>();
   s->nstrips = (s->nx + SOUT - 1) / SOUT;
   const int minb = s->dtype == JXS_F64 ? stage_minb<double>() : stage_minb<float>();
-  const double slots = (double)s->num_sms * minb;
+  const double slots = std::max(1.0, (double)s->num_sms * minb / s->share);  // this handle's share of the warp slots
   const int lo = std::min(s->ny, 8);
   std::vector<double> cost(s->ny + 1, 0.0);
   double best = 1e300;
@@ -161,7 +162,7 @@ void choose_decomposition(jxs_solver* s) {
     const double tasks = (double)((s->ny + rps - 1) / rps) * s->nstrips;
     const double len = rps + 2.0;
     // one wave: the FP64 pipe of an SM is saturated by about 8 warps, fewer tasks run at full speed each
-    cost[rps] = tasks <= slots ? 1.15 * len * std::max(1.0, tasks / (8.0 * s->num_sms))
+    cost[rps] = tasks <= slots ? 1.15 * len * std::max(1.0, tasks * s->share / (8.0 * s->num_sms))
                                : tasks / slots * len * (1.0 + 0.5 * slots / tasks);
     best = std::min(best, cost[rps]);
   }
@@ -765,6 +766,14 @@ int jxs_wait(jxs_solver* s) {
   const int n = s->pending_steps;
   s->pending_steps = 0;
   return finish_steps(s, n);
+}
+int jxs_set_concurrent_handles(jxs_solver* s, int n) {
+  if (!s) return JXS_EINVAL;
+  if (n < 1) return fail(s, JXS_EINVAL, "n must be >= 1");
+  drop_graph(s);
+  s->share = n;
+  choose_decomposition(s);  // the padded layout depends on the strips only, not on the row segments
+  return JXS_OK;
 }
 int jxs_set_time_integrator(jxs_solver* s, int scheme) {
   if (!s) return JXS_EINVAL;

@@ -22,7 +22,8 @@ EXPORTS = ("jxs_create", "jxs_destroy", "jxs_last_error", "jxs_set_ibm", "jxs_se
            "jxs_set_artificial_viscosity", "jxs_rhs", "jxs_max_wavespeed", "jxs_step", "jxs_step_fixed_dt",
            "jxs_step_host", "jxs_rhs_host", "jxs_get_time", "jxs_launch_count", "jxs_set_profiling",
            "jxs_stage_time", "jxs_ibm_ghost_count", "jxs_measure_fp64_peak", "jxs_flux_correction",
-           "jxs_flux_mlp_time", "jxs_step_async", "jxs_wait", "jxs_set_time_integrator")
+           "jxs_flux_mlp_time", "jxs_step_async", "jxs_wait", "jxs_set_time_integrator",
+           "jxs_set_concurrent_handles")
 
 
 class jxs_bc(C.Structure):
@@ -70,6 +71,7 @@ def lib():
         L.jxs_step_async.argtypes = [vp, vp, C.c_double, C.c_int]
         L.jxs_wait.argtypes = [vp]
         L.jxs_set_time_integrator.argtypes = [vp, C.c_int]
+        L.jxs_set_concurrent_handles.argtypes = [vp, C.c_int]
         L.jxs_get_time.argtypes = [vp, dp, dp]
         L.jxs_launch_count.argtypes = [vp]
         L.jxs_launch_count.restype = C.c_longlong
@@ -213,6 +215,9 @@ class Solver:
 
     def wait(self):
         self._chk(lib().jxs_wait(self._h))
+
+    def set_concurrent_handles(self, n):
+        self._chk(lib().jxs_set_concurrent_handles(self._h, int(n)))
 
     def set_time_integrator(self, scheme):
         self._chk(lib().jxs_set_time_integrator(self._h, int(scheme)))

@@ -64,6 +64,8 @@ def test_async_handles_on_streams_match_synchronous_calls():
         s.step(U, 0.4, 12)
         ref.append((U.cpu().numpy(), s.time()))
     solvers = [jxs().Solver.from_case(c, stream=st) for c, st in zip(cases, streams)]
+    for s in solvers:
+        s.set_concurrent_handles(len(solvers))  # a performance hint: results must not change
     torch.cuda.synchronize()
     Us = [dev(c["U0"]) for c in cases]
     torch.cuda.synchronize()
