@@ -30,6 +30,13 @@ __global__ void __launch_bounds__(S1D_TB) stage1d_kernel(const StageArgs<T> A) {
   const T* row = A.Uin + 3 * (size_t)A.pitch;  // the one interior row of the padded buffer
   const T g1 = A.g1, g1inv = A.g1inv, gamma = A.gamma;
 
+  // U^n of my cell for the Runge-Kutta combine: requested first, used last
+  T U0c[4] = {T(0), T(0), T(0), T(0)};
+  if (A.mode == 0 && A.rk_a != T(0)) {
+    const T* row0 = A.U0 + 3 * (size_t)A.pitch + min(col, A.pitch - 1);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) U0c[k] = row0[k * A.plane];
+  }
   // ---- S3: conserved -> primitives of my column and (threads 0-3) of one halo column
   T Uc[4];
   {
@@ -115,9 +122,8 @@ __global__ void __launch_bounds__(S1D_TB) stage1d_kernel(const StageArgs<T> A) {
 #pragma unroll
     for (int k = 0; k < 4; ++k) Un[k] = fma_(dtv, Lc[k], Uc[k]);
     if (A.rk_a != T(0)) {
-      const T* row0 = A.U0 + 3 * (size_t)A.pitch + min(col, A.pitch - 1);
 #pragma unroll
-      for (int k = 0; k < 4; ++k) Un[k] = fma_(A.rk_a, row0[k * A.plane], A.rk_b * Un[k]);
+      for (int k = 0; k < 4; ++k) Un[k] = fma_(A.rk_a, U0c[k], A.rk_b * Un[k]);
     }
     if (ok) {
       T* o = A.Uout + 3 * (size_t)A.pitch + col;
@@ -140,7 +146,18 @@ __global__ void __launch_bounds__(S1D_TB) stage1d_kernel(const StageArgs<T> A) {
       const T other = __shfl_xor_sync(0xffffffffu, smax, o);
       smax = (other > smax || other != other) ? other : smax;
     }
-    if ((t & 31) == 0) atomic_max_pos(A.smax_bits, (double)smax);
+    // one atomic per CTA: the warp maxima go through shared memory (rmS was last read before the previous barrier)
+    if ((t & 31) == 0) rmS[0][t >> 5] = smax;
+    __syncthreads();
+    if (t < 32) {
+      T m = t < S1D_TB / 32 ? rmS[0][t] : T(0);
+#pragma unroll
+      for (int o = 4; o > 0; o >>= 1) {
+        const T other = __shfl_xor_sync(0xffffffffu, m, o);
+        m = (other > m || other != other) ? other : m;
+      }
+      if (t == 0) atomic_max_pos(A.smax_bits, (double)m);
+    }
   }
 }
 
