@@ -257,3 +257,16 @@ def test_full_size_throughput_case_two_steps():
     fluid = o.cell_types() == 0
     assert rel_err(U.cpu().numpy(), ref, fluid) <= TOL_STEP64
     assert abs(o.time()[0] - s.time()[0]) <= 1e-12 * o.time()[0]
+
+
+def test_gpu_mirror_symmetry_of_the_shock_cylinder_case():
+    """C3 is mirror-symmetric about y = 0.5 (rho, rho u, E even, rho v odd): PAPER.md L162 ("arise symmetrically");
+    the CUDA path keeps it to round-off over a short run although it sweeps the rows upwards"""
+    case = wl.shock_cylinder(512, 256, Ms=2.0)
+    s = jxs().Solver.from_case(case)
+    U = dev(case["U0"])
+    s.step(U, 0.4, 60)
+    u = U.cpu().numpy()
+    scale = [np.abs(u[k]).max() for k in range(4)]
+    for k, sign in ((0, 1.0), (1, 1.0), (2, -1.0), (3, 1.0)):
+        assert np.abs(u[k] - sign * u[k][::-1, :]).max() <= 1e-10 * max(scale[k], scale[1])
