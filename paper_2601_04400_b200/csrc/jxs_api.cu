@@ -515,7 +515,6 @@ int jxs_create(int nx, int ny, double dx, double dy, double gamma, double mu, do
   if (!bc) return JXS_EINVAL;
   if (nx < 8 || (ny < 8 && ny != 1) || !(dx > 0) || !(dy > 0) || !(gamma > 1) || !(mu >= 0) || (mu > 0 && !(Pr > 0)))
     return JXS_EINVAL;
-  if (ny == 1 && mu > 0) return JXS_EINVAL;  // the one-dimensional path is Euler (+ the nu term of Eq. 10)
   if (dtype != JXS_F64 && dtype != JXS_F32) return JXS_EINVAL;
   const int kinds[4] = {bc->xlo, bc->xhi, bc->ylo, bc->yhi};
   for (int k : kinds)

@@ -9,6 +9,7 @@
 // Primitives of the tile (+2 halo columns per side), the right-biased states and the face fluxes go through
 // shared memory once each; nothing but U crosses HBM (24 B per cell-stage for (rho, rho u, E) would be the
 // floor; this kernel also carries rho v so that the C ABI keeps one layout: 64 / 96 B per cell-stage).
+// With mu > 0 the viscous flux of stage_kernel.cuh (R8) is added at the face, its cross terms being zero.
 #pragma once
 #include "stage_kernel.cuh"
 
@@ -21,7 +22,7 @@ constexpr int S1D_OUT = S1D_TB - 2;  // cells produced per CTA
 
 template <typename T>
 __global__ void __launch_bounds__(S1D_TB) stage1d_kernel(const StageArgs<T> A) {
-  __shared__ T prim[4][S1D_TB + 4];  // (rho, u, v, p) of padded columns c0-2 .. c0+257
+  __shared__ T prim[5][S1D_TB + 4];  // (rho, u, v, p, T) of padded columns c0-2 .. c0+257 (T only with mu > 0)
   __shared__ T rmS[4][S1D_TB];       // right-biased state at each cell's left face
   __shared__ T fS[4][S1D_TB];        // flux through each cell's right face
   const int t = threadIdx.x;
@@ -29,6 +30,7 @@ __global__ void __launch_bounds__(S1D_TB) stage1d_kernel(const StageArgs<T> A) {
   const int col = c0 + t;
   const T* row = A.Uin + 3 * (size_t)A.pitch;  // the one interior row of the padded buffer
   const T g1 = A.g1, g1inv = A.g1inv, gamma = A.gamma;
+  const bool visc = A.mu != T(0);
 
   // U^n of my cell for the Runge-Kutta combine: requested first, used last
   T U0c[4] = {T(0), T(0), T(0), T(0)};
@@ -54,9 +56,11 @@ __global__ void __launch_bounds__(S1D_TB) stage1d_kernel(const StageArgs<T> A) {
     JXS_V p[k] = fma_(T(-0.5), p[k], E[k]);
     JXS_V p[k] = g1 * p[k];
     prim[0][t + 2] = r[0]; prim[1][t + 2] = u[0]; prim[2][t + 2] = v[0]; prim[3][t + 2] = p[0];
+    if (visc) prim[4][t + 2] = p[0] * ri[0];
     if (t < 4) {
       const int o = t < 2 ? t : S1D_TB + t;
       prim[0][o] = r[1]; prim[1][o] = u[1]; prim[2][o] = v[1]; prim[3][o] = p[1];
+      if (visc) prim[4][o] = p[1] * ri[1];
     }
   }
   __syncthreads();
@@ -84,6 +88,14 @@ __global__ void __launch_bounds__(S1D_TB) stage1d_kernel(const StageArgs<T> A) {
     const T rR[N] = {rmS[0][tn]}, unR[N] = {rmS[1][tn]}, utR[N] = {rmS[2][tn]}, pR[N] = {rmS[3][tn]};
     T f0[N], f1[N], f2[N], f3[N];
     hllc_n<T, N>(rL, unL, utL, pL, rR, unR, utR, pR, gamma, g1inv, f0, f1, f2, f3);
+    if (visc) {  // S6 (R8) at my right face; the cross differences of a planar flow vanish
+      const int c = t + 2;
+      const T dn[N] = {prim[1][c + 1] - prim[1][c]}, dt_[N] = {prim[2][c + 1] - prim[2][c]}, zero[N] = {T(0)};
+      const T sn[N] = {prim[1][c] + prim[1][c + 1]}, st[N] = {prim[2][c] + prim[2][c + 1]};
+      const T dT[N] = {prim[4][c + 1] - prim[4][c]};
+      const T cn[N] = {A.vx_n}, cc[N] = {A.vx_c}, cs[N] = {A.vx_s}, ct[N] = {A.vx_t}, cq[N] = {A.vx_q};
+      viscous_n<T, N>(dn, dt_, zero, zero, sn, st, dT, cn, cc, cs, ct, cq, f1, f2, f3);
+    }
     F[0] = f0[0]; F[1] = f1[0]; F[2] = f2[0]; F[3] = f3[0];
 #pragma unroll
     for (int k = 0; k < 4; ++k) fS[k][t] = F[k];

@@ -78,7 +78,7 @@ def test_argument_checks_of_the_next_rows():
     h = C.c_void_p()
     b = jxs.make_bc(dict(xlo="transmissive", xhi="transmissive", ylo="transmissive", yhi="transmissive"))
     assert L.jxs_create(64, 5, 0.1, 0.1, 1.4, 0.0, 0.72, C.byref(b), 0, None, C.byref(h)) == jxs.EINVAL   # 1 < ny < 8
-    assert L.jxs_create(64, 1, 0.1, 0.1, 1.4, 1e-3, 0.72, C.byref(b), 0, None, C.byref(h)) == jxs.EINVAL  # viscous 1D
+    assert L.jxs_create(64, 1, 0.1, 0.1, 1.4, 1e-3, 0.0, C.byref(b), 0, None, C.byref(h)) == jxs.EINVAL   # Pr with mu > 0
     assert L.jxs_create(4, 1, 0.1, 0.1, 1.4, 0.0, 0.72, C.byref(b), 0, None, C.byref(h)) == jxs.EINVAL
     assert L.jxs_step_async(None, None, 0.4, 1) == jxs.EINVAL
     assert L.jxs_wait(None) == jxs.EINVAL
