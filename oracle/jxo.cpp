@@ -17,6 +17,8 @@
 //   O8  SSP-RK3              R5 (paper: forward Euler, Eq. 10)
 //   O9  CFL time step        R6 (paper silent)
 //   O10 per-face MLP         P:L96 Eq. 11; R14
+//   O11 CNN neural flux (2D)  P:L94 (3 conv layers, ReLU/ReLU/tanh, SAME padding, 6,388 parameters), Eq. 11-13
+//                             (shared between x and y); readings R18-R20 of DESIGN.md
 //
 // PARITY UNPINNED against the paper (no external definition exists; the rules
 // are shared definitions constrained only by invariants):
@@ -190,6 +192,43 @@ struct Mlp {
   }
 };
 
+// O11: the paper's fully convolutional neural flux: three 3x3 convolutions 4 -> 32 -> 16 -> 4 with biases
+// (1184 + 4624 + 580 = 6,388 parameters, the count the paper prints), ReLU, ReLU, tanh, zero ("SAME") padding at
+// every layer.  A field is in[c][a][b], a = index along the face's TANGENTIAL direction, b = along its NORMAL
+// direction (R19: the same weights serve x- and y-faces, Eq. 13).  Cross-correlation, as in JAX / PyTorch:
+//   out[o][a][b] = act( bias[o] + sum_c sum_{da,db = -1..1} W[o][c][da+1][db+1] * in[c][a+da][b+db] ).
+struct Cnn {
+  bool on = false, bf16 = false;
+  std::vector<double> W1, b1, W2, b2, W3, b3;  // W1[32][4][3][3], W2[16][32][3][3], W3[4][16][3][3]
+  double in_scale[4] = {1, 1, 1, 1}, out_scale[4] = {1, 1, 1, 1};
+  static void conv(const std::vector<double>& in, int cin, int na, int nb, const std::vector<double>& W,
+                   const std::vector<double>& b, int cout, int act, bool round_out, std::vector<double>& out) {
+    out.assign((size_t)cout * na * nb, 0.0);
+    for (int o = 0; o < cout; ++o)
+      for (int a = 0; a < na; ++a)
+        for (int bb = 0; bb < nb; ++bb) {
+          double s = b[o];
+          for (int c = 0; c < cin; ++c)
+            for (int da = -1; da <= 1; ++da)
+              for (int db = -1; db <= 1; ++db) {
+                const int a2 = a + da, b2 = bb + db;
+                if (a2 < 0 || a2 >= na || b2 < 0 || b2 >= nb) continue;  // zero padding
+                s += W[(((size_t)o * cin + c) * 3 + (da + 1)) * 3 + (db + 1)] * in[((size_t)c * na + a2) * nb + b2];
+              }
+          s = act == 0 ? (s > 0.0 ? s : 0.0) : std::tanh(s);
+          out[((size_t)o * na + a) * nb + bb] = round_out ? bf16_round(s) : s;
+        }
+  }
+  // in[4][na][nb] (already normalised) -> out[4][na][nb] in (-1,1)
+  void apply(const std::vector<double>& in, int na, int nb, std::vector<double>& out) const {
+    std::vector<double> x(in), h1, h2;
+    if (bf16) for (double& v : x) v = bf16_round(v);
+    conv(x, 4, na, nb, W1, b1, 32, 0, bf16, h1);
+    conv(h1, 32, na, nb, W2, b2, 16, 0, bf16, h2);
+    conv(h2, 16, na, nb, W3, b3, 4, 1, false, out);
+  }
+};
+
 struct IbmGhost {
   int i, j;          // the ghost cell
   int di[4], dj[4];  // bilinear donors (i0,j0),(i0+1,j0),(i0,j0+1),(i0+1,j0+1)
@@ -212,6 +251,7 @@ struct Core {
   const std::vector<unsigned char>& type;  // 0 fluid 1 ghost 2 solid (interior)
   const std::vector<IbmGhost>& ghosts;
   const Mlp& mlp;
+  const Cnn* cnn = nullptr;
   long long guard = 0;
   int nxp, nyp;
   size_t plane;
@@ -328,6 +368,21 @@ struct Core {
 
     // x-faces: Fx[k][j][f], f = 0..nx is the face between cells f-1 and f
     std::vector<T> Fx((size_t)4 * ny * (nx + 1)), Gy((size_t)4 * (ny + 1) * nx);
+    // O11 (R19): the network's input at a face = mean of the left and right reconstructed states, as conservative
+    // variables (rho, rho u_n, rho u_t, E), divided by in_scale.  Xx[c][j][f] (tangential j, normal f),
+    // Xy[c][i][f] (tangential i, normal f).
+    const bool cnn_on = cnn && cnn->on;
+    std::vector<double> Xx, Xy;
+    if (cnn_on) { Xx.assign((size_t)4 * ny * (nx + 1), 0.0); Xy.assign((size_t)4 * nx * (ny + 1), 0.0); }
+    auto face_input = [&](const T* SL, const T* SR, double* x4) {  // S = (rho, u_n, u_t, p)
+      double m[4] = {0, 0, 0, 0};
+      for (int side = 0; side < 2; ++side) {
+        const T* S = side == 0 ? SL : SR;
+        const double r = to_double(S[0]), un = to_double(S[1]), ut = to_double(S[2]), p = to_double(S[3]);
+        m[0] += r; m[1] += r * un; m[2] += r * ut; m[3] += p / (c.gamma - 1.0) + 0.5 * r * (un * un + ut * ut);
+      }
+      for (int k = 0; k < 4; ++k) x4[k] = 0.5 * m[k] / cnn->in_scale[k];
+    };
     for (int j = 0; j < ny; ++j)
       for (int f = 0; f <= nx; ++f) {
         const int i = f - 1;  // face i+1/2
@@ -347,6 +402,11 @@ struct Core {
             for (int k = 0; k < 4; ++k) x[4 * cc + k] = to_double(Wv(k, i - 2 + cc, j)) / mlp.in_scale[k];
           mlp.eval(x, y);
           for (int k = 0; k < 4; ++k) F[k] += T(mlp.out_scale[k] * y[k]);  // Eq. 11
+        }
+        if (cnn_on) {
+          double x4[4];
+          face_input(WL, WR, x4);
+          for (int k = 0; k < 4; ++k) Xx[((size_t)k * ny + j) * (nx + 1) + f] = x4[k];
         }
         for (int k = 0; k < 4; ++k) Fx[((size_t)k * ny + j) * (nx + 1) + f] = F[k];
       }
@@ -372,11 +432,31 @@ struct Core {
           mlp.eval(x, y);
           for (int k = 0; k < 4; ++k) F[k] += T(mlp.out_scale[k] * y[k]);
         }
+        if (cnn_on) {
+          double x4[4];
+          face_input(SL, SR, x4);
+          for (int k = 0; k < 4; ++k) Xy[((size_t)k * nx + i) * (ny + 1) + f] = x4[k];
+        }
         Gy[((size_t)0 * (ny + 1) + f) * nx + i] = F[0];
         Gy[((size_t)1 * (ny + 1) + f) * nx + i] = F[2];  // x-momentum = tangential
         Gy[((size_t)2 * (ny + 1) + f) * nx + i] = F[1];  // y-momentum = normal
         Gy[((size_t)3 * (ny + 1) + f) * nx + i] = F[3];
       }
+
+    if (cnn_on) {  // Eq. 11-13: F^Neural = out_scale o CNN(field), same weights for both directions
+      std::vector<double> Y;
+      cnn->apply(Xx, ny, nx + 1, Y);
+      for (int k = 0; k < 4; ++k)
+        for (int j = 0; j < ny; ++j)
+          for (int f = 0; f <= nx; ++f)
+            Fx[((size_t)k * ny + j) * (nx + 1) + f] += T(cnn->out_scale[k] * Y[((size_t)k * ny + j) * (nx + 1) + f]);
+      cnn->apply(Xy, nx, ny + 1, Y);
+      static const int to_cons[4] = {0, 2, 1, 3};  // (mass, normal = rho v, tangential = rho u, energy) -> conserved slot
+      for (int k = 0; k < 4; ++k)
+        for (int i = 0; i < nx; ++i)
+          for (int f = 0; f <= ny; ++f)
+            Gy[((size_t)to_cons[k] * (ny + 1) + f) * nx + i] += T(cnn->out_scale[k] * Y[((size_t)k * nx + i) * (ny + 1) + f]);
+    }
 
     // O6: viscous fluxes (R7, R8), constant mu, Stokes hypothesis, T = p/rho,
     // k = mu*gamma/((gamma-1) Pr); face-centred second-order central differences
@@ -504,6 +584,7 @@ struct jxo_solver {
   std::vector<unsigned char> type;  // interior cell types
   std::vector<IbmGhost> ghosts;
   Mlp mlp;
+  Cnn cnn;
   long long guard = 0;
   double t = 0, last_dt = 0;
   std::string err;
@@ -596,6 +677,7 @@ int build_ibm(jxo_solver* s, const double* phi) {
 template <class T>
 int do_rhs(jxo_solver* s, const void* U, void* dUdt) {
   Core<T> core(s->c, s->type, s->ghosts, s->mlp);
+  core.cnn = &s->cnn;
   std::vector<T> Up;
   core.pad((const T*)U, Up);
   core.fill_and_rhs(Up, (T*)dUdt);
@@ -606,6 +688,7 @@ int do_rhs(jxo_solver* s, const void* U, void* dUdt) {
 template <class T>
 int do_wavespeed(jxo_solver* s, const void* U, double* smax) {
   Core<T> core(s->c, s->type, s->ghosts, s->mlp);
+  core.cnn = &s->cnn;
   std::vector<T> Up;
   core.pad((const T*)U, Up);
   *smax = to_double(core.max_wavespeed(Up));
@@ -615,6 +698,7 @@ int do_wavespeed(jxo_solver* s, const void* U, double* smax) {
 template <class T>
 int do_step(jxo_solver* s, void* U, double cfl, double fixed_dt, int nsteps) {
   Core<T> core(s->c, s->type, s->ghosts, s->mlp);
+  core.cnn = &s->cnn;
   std::vector<T> Up;
   core.pad((T*)U, Up);
   int rc = JXO_OK;
@@ -754,6 +838,7 @@ int jxo_fill_ghosts(jxo_solver* s, const void* U, void* Upad) {
   if (!s || !U || !Upad) return JXO_EINVAL;
   if (s->dtype == JXO_F64) {
     Core<double> core(s->c, s->type, s->ghosts, s->mlp);
+    core.cnn = &s->cnn;
     std::vector<double> Up;
     core.pad((const double*)U, Up);
     core.fill_frame(Up);
@@ -761,6 +846,7 @@ int jxo_fill_ghosts(jxo_solver* s, const void* U, void* Upad) {
     std::memcpy(Upad, Up.data(), Up.size() * sizeof(double));
   } else {
     Core<float> core(s->c, s->type, s->ghosts, s->mlp);
+    core.cnn = &s->cnn;
     std::vector<float> Up;
     core.pad((const float*)U, Up);
     core.fill_frame(Up);
@@ -799,6 +885,7 @@ int jxo_count_ops(jxo_solver* s, const double* U, long long counts[5]) {
   std::vector<Counted> Uc(n), L(n);
   for (size_t i = 0; i < n; ++i) Uc[i] = Counted(U[i]);
   Core<Counted> core(s->c, s->type, s->ghosts, s->mlp);
+  core.cnn = &s->cnn;
   std::vector<Counted> Up;
   core.pad(Uc.data(), Up);
   core.fill_frame(Up);
@@ -812,6 +899,39 @@ int jxo_count_ops(jxo_solver* s, const double* U, long long counts[5]) {
   (void)core.max_wavespeed(Up);
   counts[0] = g_tally.add; counts[1] = g_tally.mul; counts[2] = g_tally.div;
   counts[3] = g_tally.sqrt_; counts[4] = g_tally.cmp;
+  return JXO_OK;
+}
+
+int jxo_set_flux_cnn(jxo_solver* s, const float* w, const double in_scale[4], const double out_scale[4],
+                     int emulate_bf16) {
+  if (!s) return JXO_EINVAL;
+  if (!w) { s->cnn.on = false; return JXO_OK; }
+  if (!in_scale || !out_scale) return JXO_EINVAL;
+  for (int i = 0; i < 6388; ++i)
+    if (!std::isfinite(w[i])) return JXO_EINVAL;
+  for (int k = 0; k < 4; ++k)
+    if (!(in_scale[k] > 0)) return JXO_EINVAL;
+  Cnn& m = s->cnn;
+  m.bf16 = emulate_bf16 != 0;
+  auto take = [&](std::vector<double>& dst, size_t n, bool round) {
+    dst.resize(n);
+    for (size_t i = 0; i < n; ++i) dst[i] = round && m.bf16 ? bf16_round((double)w[i]) : (double)w[i];
+    w += n;
+  };
+  // PyTorch / JAX OIHW order: W1[32][4][3][3], b1[32], W2[16][32][3][3], b2[16], W3[4][16][3][3], b3[4]
+  take(m.W1, 32 * 4 * 9, true); take(m.b1, 32, false);
+  take(m.W2, 16 * 32 * 9, true); take(m.b2, 16, false);
+  take(m.W3, 4 * 16 * 9, true); take(m.b3, 4, false);
+  for (int k = 0; k < 4; ++k) { m.in_scale[k] = in_scale[k]; m.out_scale[k] = out_scale[k]; }
+  m.on = true;
+  return JXO_OK;
+}
+
+int jxo_cnn_apply(const jxo_solver* s, const double* in, int na, int nb, double* out) {
+  if (!s || !s->cnn.on || !in || !out || na < 1 || nb < 1) return JXO_ESTATE;
+  std::vector<double> x(in, in + (size_t)4 * na * nb), y;
+  s->cnn.apply(x, na, nb, y);
+  std::copy(y.begin(), y.end(), out);
   return JXO_OK;
 }
 

@@ -39,6 +39,12 @@ int jxo_set_ibm(jxo_solver*, const double* phi_host);
  * activations to bf16 (round-to-nearest-even) and accumulates in double.      */
 int jxo_set_flux_mlp(jxo_solver*, const float* weights, const double in_scale[4],
                      const double out_scale[4], int emulate_bf16);
+/* O11: the paper's 2D CNN neural flux (Eq. 11-13): weights in OIHW order W1[32][4][3][3], b1[32],
+ * W2[16][32][3][3], b2[16], W3[4][16][3][3], b3[4] = 6388 floats; in_scale of (rho, rho u_n, rho u_t, E), out_scale
+ * of the (mass, normal, tangential momentum, energy) flux.  NULL disables.  emulate_bf16 != 0 rounds weights, inputs
+ * and the two hidden activation fields to bf16.  Can be combined with the per-face MLP (both are added).          */
+int jxo_set_flux_cnn(jxo_solver*, const float* weights, const double in_scale[4],
+                     const double out_scale[4], int emulate_bf16);
 int jxo_set_artificial_viscosity(jxo_solver*, double nu);
 
 int jxo_rhs(jxo_solver*, const void* U, void* dUdt);
@@ -70,6 +76,8 @@ long long jxo_guard_count(const jxo_solver*);
 int jxo_count_ops(jxo_solver*, const double* U, long long counts[5]);
 /* the per-face MLP alone: x[24] (already normalised) -> y[4]                    */
 int jxo_mlp_eval(const jxo_solver*, const double x[24], double y[4]);
+/* the CNN alone on a normalised field in[4][na][nb] (a tangential, b normal) -> out[4][na][nb]   */
+int jxo_cnn_apply(const jxo_solver*, const double* in, int na, int nb, double* out);
 
 #ifdef __cplusplus
 }

@@ -56,6 +56,8 @@ def lib():
         L.jxo_guard_count.restype = C.c_longlong
         L.jxo_count_ops.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
         L.jxo_mlp_eval.argtypes = [vp, dp, dp]
+        L.jxo_set_flux_cnn.argtypes = [vp, vp, dp, dp, C.c_int]
+        L.jxo_cnn_apply.argtypes = [vp, dp, C.c_int, C.c_int, dp]
         _lib = L
     return _lib
 
@@ -147,6 +149,24 @@ class Oracle:
         a = np.ascontiguousarray(in_scale, dtype=np.float64)
         b = np.ascontiguousarray(out_scale, dtype=np.float64)
         self._chk(lib().jxo_set_flux_mlp(self._h, w.ctypes.data, _d(a), _d(b), int(emulate_bf16)))
+
+    def set_flux_cnn(self, weights, in_scale=None, out_scale=None, emulate_bf16=False):
+        """O11: the paper's 2D CNN neural flux, 6388 weights in OIHW order (None disables)."""
+        if weights is None:
+            self._chk(lib().jxo_set_flux_cnn(self._h, None, None, None, 0))
+            return
+        w = np.ascontiguousarray(weights, dtype=np.float32)
+        assert w.shape == (6388,)
+        a = np.ascontiguousarray(in_scale, dtype=np.float64)
+        b = np.ascontiguousarray(out_scale, dtype=np.float64)
+        self._chk(lib().jxo_set_flux_cnn(self._h, w.ctypes.data, _d(a), _d(b), int(emulate_bf16)))
+
+    def cnn_apply(self, x):
+        """the CNN alone on a normalised field x[4][na][nb] (a tangential, b normal)"""
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        y = np.zeros_like(x)
+        self._chk(lib().jxo_cnn_apply(self._h, _d(x), x.shape[1], x.shape[2], _d(y)))
+        return y
 
     def set_artificial_viscosity(self, nu):
         self._chk(lib().jxo_set_artificial_viscosity(self._h, float(nu)))

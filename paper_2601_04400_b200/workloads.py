@@ -218,6 +218,32 @@ def mlp_scales(gamma=GAMMA, rho_ref=1.4, p_ref=1.0, out_factor=1.0e-3):
     return in_scale, out_scale
 
 
+CNN_SIZES = ((32, 4), (16, 32), (4, 16))  # (out, in) channels of the three 3x3 convolutions
+CNN_NPARAM = sum(o * i * 9 + o for o, i in CNN_SIZES)  # 6388, the count the paper prints
+
+
+def cnn_weights(seed=9, bias=0.0):
+    """Glorot-uniform 3x3 kernels in OIHW order, constant biases: W1[32][4][3][3], b1, W2[16][32][3][3], b2,
+    W3[4][16][3][3], b3 (fp32)."""
+    rng = np.random.default_rng(seed)
+    parts = []
+    for (fo, fi) in CNN_SIZES:
+        lim = math.sqrt(6.0 / (9 * (fi + fo)))
+        parts.append(rng.uniform(-lim, lim, size=(fo, fi, 3, 3)).astype(np.float32).ravel())
+        parts.append(np.full(fo, bias, dtype=np.float32))
+    w = np.concatenate(parts)
+    assert w.size == CNN_NPARAM
+    return w
+
+
+def cnn_scales(gamma=GAMMA, rho_ref=1.4, p_ref=1.0, out_factor=1.0e-3):
+    """in_scale of (rho, rho u_n, rho u_t, E) and out_scale of the flux, from the pre-shock state."""
+    a = math.sqrt(gamma * p_ref / rho_ref)
+    in_scale = np.array([rho_ref, rho_ref * a, rho_ref * a, p_ref / (gamma - 1.0)])
+    out_scale = out_factor * np.array([rho_ref * a, rho_ref * a * a, rho_ref * a * a, rho_ref * a ** 3])
+    return in_scale, out_scale
+
+
 def batch_cases(n=16, seed=16, nx=1024, ny=512):
     """Config 5: n independent shock-cylinder cases with Mach ~ U[1.5, 3] (seeded)."""
     rng = np.random.default_rng(seed)
