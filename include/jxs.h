@@ -86,6 +86,19 @@ int jxs_set_flux_mlp(jxs_solver*, const float* weights_host, const double in_sca
  * between cells f-1 and f) and dGy[4][ny+1][nx], components = corrections to the (rho, rho u, rho v, E)
  * fluxes.  JXS_ESTATE without a network.  Asynchronous.                                     */
 int jxs_flux_correction(jxs_solver*, const void* U, float* dFx, float* dGy);
+/* The paper's two-dimensional neural flux (Eq. 11-13): a fully
+ * convolutional network, three 3x3 convolutions 4 -> 32 -> 16 -> 4 with ReLU, ReLU, tanh and zero padding (6388
+ * parameters, R18), applied to the field of normalised face states of each direction with the same weights (R19)
+ * and added, times out_scale, to the HLLC flux (R20).  weights_host: 6388 floats in OIHW order W1[32][4][3][3],
+ * b1[32], W2[16][32][3][3], b2[16], W3[4][16][3][3], b3[4] (first tap index along the face's tangential direction,
+ * second along its normal); in_scale of (rho, rho u_n, rho u_t, E) > 0; out_scale of the (mass, normal momentum,
+ * tangential momentum, energy) flux.  Evaluated in bf16 with fp32 accumulation on the tensor cores.  NULL weights
+ * disable it.  JXS_ESTATE while the per-face MLP is set (one network at a time), JXS_EINVAL for ny = 1.
+ * jxs_flux_correction returns its corrections; jxs_flux_cnn_inputs (inspection) returns the network's input
+ * fields as floats, Xx[4][ny][nx+1] and Xy[4][nx][ny+1] (device pointers).                                   */
+int jxs_set_flux_cnn(jxs_solver*, const float* weights_host, const double in_scale[4], const double out_scale[4]);
+int jxs_flux_cnn_inputs(jxs_solver*, const void* U, float* Xx, float* Xy);
+
 /* Laplacian artificial viscosity nu * Lap_h(U) of PAPER.md Eq. 10; default 0 (R7).          */
 int jxs_set_artificial_viscosity(jxs_solver*, double nu);
 

@@ -252,6 +252,7 @@ struct Core {
   const std::vector<IbmGhost>& ghosts;
   const Mlp& mlp;
   const Cnn* cnn = nullptr;
+  std::vector<double>* cap[4] = {nullptr, nullptr, nullptr, nullptr};  // observers: Xx, Xy, Yx, Yy of the last rhs (O11)
   long long guard = 0;
   int nxp, nyp;
   size_t plane;
@@ -446,11 +447,13 @@ struct Core {
     if (cnn_on) {  // Eq. 11-13: F^Neural = out_scale o CNN(field), same weights for both directions
       std::vector<double> Y;
       cnn->apply(Xx, ny, nx + 1, Y);
+      if (cap[0]) { *cap[0] = Xx; *cap[1] = Xy; *cap[2] = Y; }
       for (int k = 0; k < 4; ++k)
         for (int j = 0; j < ny; ++j)
           for (int f = 0; f <= nx; ++f)
             Fx[((size_t)k * ny + j) * (nx + 1) + f] += T(cnn->out_scale[k] * Y[((size_t)k * ny + j) * (nx + 1) + f]);
       cnn->apply(Xy, nx, ny + 1, Y);
+      if (cap[3]) *cap[3] = Y;
       static const int to_cons[4] = {0, 2, 1, 3};  // (mass, normal = rho v, tangential = rho u, energy) -> conserved slot
       for (int k = 0; k < 4; ++k)
         for (int i = 0; i < nx; ++i)
@@ -924,6 +927,19 @@ int jxo_set_flux_cnn(jxo_solver* s, const float* w, const double in_scale[4], co
   take(m.W3, 4 * 16 * 9, true); take(m.b3, 4, false);
   for (int k = 0; k < 4; ++k) { m.in_scale[k] = in_scale[k]; m.out_scale[k] = out_scale[k]; }
   m.on = true;
+  return JXO_OK;
+}
+
+int jxo_cnn_fields(jxo_solver* s, const double* U, double* Xx, double* Xy, double* Yx, double* Yy) {
+  if (!s || !s->cnn.on || s->dtype != JXO_F64 || !U || !Xx || !Xy || !Yx || !Yy) return JXO_ESTATE;
+  Core<double> core(s->c, s->type, s->ghosts, s->mlp);
+  core.cnn = &s->cnn;
+  std::vector<double> f[4], Up, L((size_t)4 * s->c.nx * s->c.ny);
+  for (int q = 0; q < 4; ++q) core.cap[q] = &f[q];
+  core.pad(U, Up);
+  core.fill_and_rhs(Up, L.data());
+  double* out[4] = {Xx, Xy, Yx, Yy};
+  for (int q = 0; q < 4; ++q) std::copy(f[q].begin(), f[q].end(), out[q]);
   return JXO_OK;
 }
 

@@ -78,6 +78,9 @@ int jxo_count_ops(jxo_solver*, const double* U, long long counts[5]);
 int jxo_mlp_eval(const jxo_solver*, const double x[24], double y[4]);
 /* the CNN alone on a normalised field in[4][na][nb] (a tangential, b normal) -> out[4][na][nb]   */
 int jxo_cnn_apply(const jxo_solver*, const double* in, int na, int nb, double* out);
+/* observers of one rhs evaluation (fp64 handles): the network's input fields Xx[4][ny][nx+1], Xy[4][nx][ny+1]
+ * (R19) and its outputs before out_scale, same shapes                                              */
+int jxo_cnn_fields(jxo_solver*, const double* U, double* Xx, double* Xy, double* Yx, double* Yy);
 
 #ifdef __cplusplus
 }

@@ -58,6 +58,7 @@ def lib():
         L.jxo_mlp_eval.argtypes = [vp, dp, dp]
         L.jxo_set_flux_cnn.argtypes = [vp, vp, dp, dp, C.c_int]
         L.jxo_cnn_apply.argtypes = [vp, dp, C.c_int, C.c_int, dp]
+        L.jxo_cnn_fields.argtypes = [vp, dp, dp, dp, dp, dp]
         _lib = L
     return _lib
 
@@ -160,6 +161,14 @@ class Oracle:
         a = np.ascontiguousarray(in_scale, dtype=np.float64)
         b = np.ascontiguousarray(out_scale, dtype=np.float64)
         self._chk(lib().jxo_set_flux_cnn(self._h, w.ctypes.data, _d(a), _d(b), int(emulate_bf16)))
+
+    def cnn_fields(self, U):
+        """(Xx, Xy, Yx, Yy) of one rhs evaluation: inputs and raw outputs of the CNN at x- and y-faces"""
+        U = np.ascontiguousarray(U, dtype=np.float64)
+        shp = ((4, self.ny, self.nx + 1), (4, self.nx, self.ny + 1))
+        f = [np.zeros(shp[0]), np.zeros(shp[1]), np.zeros(shp[0]), np.zeros(shp[1])]
+        self._chk(lib().jxo_cnn_fields(self._h, _d(U), *[_d(a) for a in f]))
+        return f
 
     def cnn_apply(self, x):
         """the CNN alone on a normalised field x[4][na][nb] (a tangential, b normal)"""

@@ -1,0 +1,281 @@
+// flux_cnn_kernel.cuh — the paper's two-dimensional neural flux (Eq. 11-13; SURVEY.md section 8(f)
+// rank 1; readings R18-R20 of DESIGN.md) on the 5th-generation tensor cores of sm_100a.
+//
+//   F^Neural = out_scale o tanh(conv3x3(relu(conv3x3(relu(conv3x3(X; 4->32)); 32->16)); 16->4)),  zero padding
+//
+// where X is, at every face of one direction, the mean of the left and right WENO5 states as conservative
+// variables (rho, rho u_n, rho u_t, E) / in_scale (R19).  Three passes per direction, one kernel each:
+//
+//   cnn_recon_kernel   U (padded, ghosts filled) -> the two input fields, bf16, 16 bytes per face
+//   cnn_layer_kernel   one 3x3 convolution as an implicit GEMM on tcgen05: a CTA marches a strip of 128 faces
+//                      row by row; the last three input rows sit in shared memory in the K-major core-matrix
+//                      layout  [8-channel chunk][face][16 B], so that tap (da, db) of the convolution is ONE
+//                      tcgen05.mma whose A descriptor points at (row buffer da, 16*db bytes into it): im2col without
+//                      a copy.  9 * Cin/16 MMAs of 128 x Cout x 16 accumulate in TMEM; bias, ReLU (tanh in the last
+//                      layer) and the rounding to bf16 follow in registers.
+//
+// Activation fields in HBM use the same chunked layout with a one-face border of zeros all around (the "SAME"
+// padding of every layer is then just what the loads find): element (row r, chunk c, face p) is the uint4 at
+//   ((r + 1) * C + c) * nbp + (p + 1),      r in [-1, na], p in [-1, nbp - 2].
+// Rows are indexed along the field's first axis, faces along its second.  x-faces: rows = j (tangential), faces
+// = f (normal).  y-faces are kept in their natural order, rows = f (normal), faces = i (tangential), and use the
+// TRANSPOSED 3x3 kernels instead (packed on the host), which is the same convolution.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "flux_mlp_kernel.cuh"
+
+namespace jxs {
+
+constexpr int CNN_TILE = 128;           // faces per MMA tile = threads per CTA
+constexpr int CNN_ROWP = CNN_TILE + 8;  // faces per shared-memory row buffer (window of 130, padded)
+
+struct CnnField {      // one activation field in HBM
+  uint4* data;         // base (row -1, chunk 0, face -1)
+  int na, nb, nbp, C;  // rows, faces, padded faces per row (incl. the border), 8-channel chunks
+  __host__ __device__ size_t at(int r, int c, int p) const { return ((size_t)(r + 1) * C + c) * nbp + (p + 1); }
+};
+
+// ------------------------------------------------------------------ pass 1: the input fields
+// left-biased WENO5-JS value at the face right of c, literal form (R4)
+template <typename T>
+__device__ __forceinline__ T weno5_literal(T a, T b, T c, T d, T e) {
+  const T q0 = (T(2) * a - T(7) * b + T(11) * c) / T(6), q1 = (-b + T(5) * c + T(2) * d) / T(6),
+          q2 = (T(2) * c + T(5) * d - e) / T(6);
+  const T s0 = a - T(2) * b + c, s1 = b - T(2) * c + d, s2 = c - T(2) * d + e;
+  const T t0 = a - T(4) * b + T(3) * c, t1 = b - d, t2 = T(3) * c - T(4) * d + e;
+  const T b0 = T(13) / T(12) * s0 * s0 + T(0.25) * t0 * t0 + T(1e-6);
+  const T b1 = T(13) / T(12) * s1 * s1 + T(0.25) * t1 * t1 + T(1e-6);
+  const T b2 = T(13) / T(12) * s2 * s2 + T(0.25) * t2 * t2 + T(1e-6);
+  const T a0 = T(0.1) / (b0 * b0), a1 = T(0.6) / (b1 * b1), a2 = T(0.3) / (b2 * b2);
+  return (a0 * q0 + a1 * q1 + a2 * q2) / (a0 + a1 + a2);
+}
+
+template <typename T>
+struct CnnReconArgs {
+  const T* U;  // padded [4][ny+6][pitch], ghosts filled
+  long long plane;
+  int nx, ny, pitch;
+  T g1, g1inv;
+  T inv_scale[4];  // 1 / in_scale of (rho, rho u_n, rho u_t, E)
+  CnnField Xx, Xy; // Xx: rows j, faces f = 0..nx;  Xy: rows f = 0..ny, faces i
+};
+
+constexpr int CNN_RX = 32, CNN_RY = 8;  // cells per CTA of the reconstruction pass
+
+template <typename T>
+__global__ void __launch_bounds__(CNN_RX * CNN_RY) cnn_recon_kernel(const CnnReconArgs<T> A) {
+  __shared__ T W[4][CNN_RY + 5][CNN_RX + 5];  // primitives of cells [i0-2, i0+34] x [j0-2, j0+10]
+  const int tx = threadIdx.x % CNN_RX, ty = threadIdx.x / CNN_RX;
+  const int i0 = blockIdx.x * CNN_RX - 1, j0 = blockIdx.y * CNN_RY - 1;  // cells start at (-1,-1): see below
+  for (int q = threadIdx.x; q < (CNN_RY + 5) * (CNN_RX + 5); q += CNN_RX * CNN_RY) {
+    const int cx = q % (CNN_RX + 5), cy = q / (CNN_RX + 5);
+    const int ip = min(max(i0 - 2 + cx + 3, 0), A.nx + 5), jp = min(max(j0 - 2 + cy + 3, 0), A.ny + 5);
+    const T* s = A.U + (size_t)jp * A.pitch + ip;
+    const T r = s[0], ru = s[A.plane], rv = s[2 * A.plane], E = s[3 * A.plane];
+    const T u = ru / r, v = rv / r;
+    W[0][cy][cx] = r; W[1][cy][cx] = u; W[2][cy][cx] = v;
+    W[3][cy][cx] = A.g1 * (E - T(0.5) * (ru * u + rv * v));
+  }
+  __syncthreads();
+  // cell (i, j), i in [-1, nx-1], j in [-1, ny-1]: its right face is x-face f = i+1 of row j (needs j >= 0),
+  // its top face is y-face f = j+1 of column i (needs i >= 0)
+  const int i = i0 + tx, j = j0 + ty;
+  if (i > A.nx - 1 || j > A.ny - 1) return;
+  const int cx = tx + 2, cy = ty + 2;
+  auto face_input = [&](const T (&L)[4], const T (&R)[4]) -> uint4 {  // states (rho, u_n, u_t, p) -> 4 bf16 + 4 zeros
+    float m[4];
+    const T eL = L[3] * A.g1inv + T(0.5) * L[0] * (L[1] * L[1] + L[2] * L[2]);
+    const T eR = R[3] * A.g1inv + T(0.5) * R[0] * (R[1] * R[1] + R[2] * R[2]);
+    m[0] = (float)(T(0.5) * (L[0] + R[0]) * A.inv_scale[0]);
+    m[1] = (float)(T(0.5) * (L[0] * L[1] + R[0] * R[1]) * A.inv_scale[1]);
+    m[2] = (float)(T(0.5) * (L[0] * L[2] + R[0] * R[2]) * A.inv_scale[2]);
+    m[3] = (float)(T(0.5) * (eL + eR) * A.inv_scale[3]);
+    return make_uint4(pack_bf16(m[0], m[1]), pack_bf16(m[2], m[3]), 0u, 0u);
+  };
+  if (j >= 0) {
+    T L[4], R[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const T* w = &W[k][cy][cx];
+      L[k] = weno5_literal(w[-2], w[-1], w[0], w[1], w[2]);
+      R[k] = weno5_literal(w[3], w[2], w[1], w[0], w[-1]);
+    }
+    if (!(L[0] > T(0)) || !(L[3] > T(0))) { for (int k = 0; k < 4; ++k) L[k] = W[k][cy][cx]; }      // R15
+    if (!(R[0] > T(0)) || !(R[3] > T(0))) { for (int k = 0; k < 4; ++k) R[k] = W[k][cy][cx + 1]; }
+    A.Xx.data[A.Xx.at(j, 0, i + 1)] = face_input(L, R);
+  }
+  if (i >= 0) {
+    T L[4], R[4];
+    const int perm[4] = {0, 2, 1, 3};  // normal velocity first
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int kk = perm[k];
+      L[k] = weno5_literal(W[kk][cy - 2][cx], W[kk][cy - 1][cx], W[kk][cy][cx], W[kk][cy + 1][cx], W[kk][cy + 2][cx]);
+      R[k] = weno5_literal(W[kk][cy + 3][cx], W[kk][cy + 2][cx], W[kk][cy + 1][cx], W[kk][cy][cx], W[kk][cy - 1][cx]);
+    }
+    if (!(L[0] > T(0)) || !(L[3] > T(0))) { for (int k = 0; k < 4; ++k) L[k] = W[perm[k]][cy][cx]; }
+    if (!(R[0] > T(0)) || !(R[3] > T(0))) { for (int k = 0; k < 4; ++k) R[k] = W[perm[k]][cy + 1][cx]; }
+    A.Xy.data[A.Xy.at(j + 1, 0, i)] = face_input(L, R);
+  }
+}
+
+// test / inspection: the bf16 input fields -> float arrays in the oracle's layout, Xx[4][ny][nx+1] (row j, face f)
+// and Xy[4][nx][ny+1] (column i, face f)
+__global__ void cnn_inputs_gather_kernel(CnnField fx, CnnField fy, float* __restrict__ Xx, float* __restrict__ Xy, int nx, int ny) {
+  const long long nfx = (long long)ny * (nx + 1), nfy = (long long)nx * (ny + 1);
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < nfx + nfy; t += (long long)gridDim.x * blockDim.x) {
+    uint4 v;
+    float* dst;
+    long long stride;
+    if (t < nfx) {
+      const int j = (int)(t / (nx + 1)), f = (int)(t % (nx + 1));
+      v = fx.data[fx.at(j, 0, f)]; dst = Xx + t; stride = nfx;
+    } else {
+      const long long u = t - nfx;
+      const int i = (int)(u / (ny + 1)), f = (int)(u % (ny + 1));
+      v = fy.data[fy.at(f, 0, i)]; dst = Xy + u; stride = nfy;
+    }
+    dst[0] = __uint_as_float(v.x << 16); dst[stride] = __uint_as_float(v.x & 0xffff0000u);
+    dst[2 * stride] = __uint_as_float(v.y << 16); dst[3 * stride] = __uint_as_float(v.y & 0xffff0000u);
+  }
+}
+
+// ------------------------------------------------------------------ passes 2-4: one 3x3 convolution each
+// KC = 16-channel K steps per tap (input channels / 16, at least 1), NOUT = output channels padded to 16.
+// Weight blob of a layer (bf16, packed on the host): [9 taps][KC][NOUT x 16] tiles in the K-major no-swizzle
+// canonical layout (element (n, k) at (n/8)*128 + (k/8)*(NOUT*16) + (n%8)*16 + (k%8)*2), then NOUT fp32 biases.
+struct CnnLayerArgs {
+  CnnField in, out;      // out unused by the last layer
+  const uint8_t* blob;   // weights + biases of this layer (for this direction: y-faces use transposed taps)
+  int rows_per_seg;
+  // last layer only: y[k] -> dst[k * plane + (row + row_off) * pitch + face + col_off], fp32 (the stage kernel's dF / dG)
+  float* dst;
+  long long plane;
+  int pitch, row_off, col_off;
+};
+
+template <int KC, int NOUT>
+__host__ __device__ constexpr int cnn_wbytes() { return 9 * KC * NOUT * 16 * 2; }
+template <int KC>
+__host__ __device__ constexpr int cnn_slot_bytes() { return 2 * KC * CNN_ROWP * 16; }  // 2 chunks per K step
+template <int KC, int NOUT>
+__host__ __device__ constexpr int cnn_smem_bytes() {
+  return (cnn_wbytes<KC, NOUT>() + NOUT * 4 + 127) / 128 * 128 + 3 * cnn_slot_bytes<KC>() + 16;
+}
+
+// CIN8 = 8-channel chunks the input field really has (1 for the first layer: its second chunk stays zero)
+template <int KC, int CIN8, int NOUT, bool LAST>
+__global__ void __launch_bounds__(CNN_TILE) cnn_layer_kernel(const CnnLayerArgs A) {
+  extern __shared__ __align__(128) unsigned char sm[];
+  __shared__ uint32_t tmem_slot;
+  constexpr int WB = cnn_wbytes<KC, NOUT>();
+  constexpr int OFF_ROWS = (WB + NOUT * 4 + 127) / 128 * 128;
+  constexpr int SLOT = cnn_slot_bytes<KC>();
+  constexpr int LBO_A = CNN_ROWP * 16;  // between the two 8-channel chunks of a K step
+  const int t = threadIdx.x, warp = t >> 5;
+  const int nstrips = (A.in.nb + CNN_TILE - 1) / CNN_TILE;
+  const int strip = blockIdx.x % nstrips, seg = blockIdx.x / nstrips;
+  const int abeg = seg * A.rows_per_seg, aend = min(abeg + A.rows_per_seg, A.in.na);
+  if (abeg >= aend) return;
+  const int b0 = strip * CNN_TILE;  // first output face of the strip; the window is faces b0-1 .. b0+128
+  const uint32_t sm_u32 = (uint32_t)__cvta_generic_to_shared(sm);
+  const uint32_t bar = sm_u32 + OFF_ROWS + 3 * SLOT;
+  const float* bias = reinterpret_cast<const float*>(sm + WB);
+
+  for (int i = t; i < (WB + NOUT * 4) / 16; i += CNN_TILE)
+    reinterpret_cast<uint4*>(sm)[i] = reinterpret_cast<const uint4*>(A.blob)[i];
+  for (int i = t; i < 3 * SLOT / 16; i += CNN_TILE)  // chunks the field does not have stay zero
+    reinterpret_cast<uint4*>(sm + OFF_ROWS)[i] = make_uint4(0, 0, 0, 0);
+  if (t == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(1) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 0) tmem_alloc((uint32_t)__cvta_generic_to_shared(&tmem_slot), 32);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+  const uint32_t tlane = tmem + ((uint32_t)(32 * warp) << 16);
+  constexpr uint32_t IDESC = umma_idesc(128, NOUT);
+  uint32_t phase = 0;
+
+  // input row r -> ring slot (r + 1) % 3, window faces b0-1 .. b0+128 at buffer positions 0 .. 129
+  auto load_row = [&](int r) {
+    unsigned char* dst = sm + OFF_ROWS + ((r + 1) % 3) * SLOT;
+#pragma unroll
+    for (int c = 0; c < CIN8; ++c) {
+      const uint4* src = A.in.data + A.in.at(r, c, b0 - 1);
+      reinterpret_cast<uint4*>(dst + c * LBO_A)[t] = src[t];
+      if (t < 2) reinterpret_cast<uint4*>(dst + c * LBO_A)[CNN_TILE + t] = src[CNN_TILE + t];
+    }
+  };
+  load_row(abeg - 1);
+  load_row(abeg);
+  for (int a = abeg; a < aend; ++a) {
+    load_row(a + 1);  // rows -1 and na are the zero border of the field
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    if (t == 0) {
+      tc_fence_after();
+      uint32_t acc = 0;
+#pragma unroll
+      for (int da = 0; da < 3; ++da) {
+        const uint32_t rowbuf = sm_u32 + OFF_ROWS + ((a + da) % 3) * SLOT;  // row a + da - 1
+#pragma unroll
+        for (int db = 0; db < 3; ++db)
+#pragma unroll
+          for (int ks = 0; ks < KC; ++ks) {
+            umma_bf16(tmem, umma_desc(rowbuf + ks * 2 * LBO_A + db * 16, LBO_A, 128),
+                      umma_desc(sm_u32 + ((da * 3 + db) * KC + ks) * NOUT * 32, NOUT * 16, 128), IDESC, acc);
+            acc = 1;
+          }
+      }
+      umma_commit(bar);
+    }
+    mbar_wait_spin(bar, phase); phase ^= 1;
+    tc_fence_after();
+    const int p = b0 + t;
+    if (!LAST) {
+#pragma unroll
+      for (int h = 0; h < NOUT / 16; ++h) {
+        uint32_t v[16];
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                       "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                     : "r"(tlane + 16 * h) : "memory");
+        tmem_ld_wait();
+        if (p < A.in.nb) {
+#pragma unroll
+          for (int c = 0; c < 2; ++c) {
+            uint32_t w[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const int k = 8 * c + 2 * e;
+              const float s0 = fmaxf(__uint_as_float(v[k]) + bias[16 * h + k], 0.f);
+              const float s1 = fmaxf(__uint_as_float(v[k + 1]) + bias[16 * h + k + 1], 0.f);
+              w[e] = pack_bf16(s0, s1);
+            }
+            A.out.data[A.out.at(a, 2 * h + c, p)] = make_uint4(w[0], w[1], w[2], w[3]);
+          }
+        }
+      }
+    } else {
+      uint32_t y[4];
+      tmem_ld4(tlane, y);
+      tmem_ld_wait();
+      if (p < A.in.nb) {
+        float* o = A.dst + (size_t)(a + A.row_off) * A.pitch + p + A.col_off;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) o[k * A.plane] = tanh_f32(__uint_as_float(y[k]) + bias[k]);
+      }
+    }
+    tc_fence_before();  // the next row's MMAs overwrite the columns just read
+  }
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tmem, 32);
+}
+
+}  // namespace jxs

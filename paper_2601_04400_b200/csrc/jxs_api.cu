@@ -17,6 +17,7 @@
 
 #include "aux_kernels.cuh"
 #include "flux_mlp_kernel.cuh"
+#include "flux_cnn_kernel.cuh"
 #include "stage_kernel.cuh"
 #include "stage1d_kernel.cuh"
 
@@ -59,6 +60,12 @@ struct jxs_solver {
   float* d_dG = nullptr;   // same at top faces
   double in_scale[4] = {1, 1, 1, 1}, out_scale[4] = {1, 1, 1, 1};
   float mlp_bias[132] = {0};
+  // the paper's 2D CNN flux (flux_cnn_kernel.cuh): per direction (x, y) the input field, the two hidden fields and
+  // the three layers' weight blobs; shares d_dF / d_dG / out_scale with the MLP path (one of the two at a time)
+  bool cnn_on = false;
+  CnnField cnn_X[2] = {}, cnn_H1[2] = {}, cnn_H2[2] = {};
+  uint8_t* d_cnn_blob[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
+  double cnn_in_scale[4] = {1, 1, 1, 1};
   int mlp_strips = 0, mlp_rows_per_seg = 0, mlp_grid = 0;
   double mlp_ms = 0;
   long long mlp_launches = 0;
@@ -223,8 +230,8 @@ cudaError_t launch_stage(jxs_solver* s, const void* Uin, const void* U0, void* U
     A.vx_n = (T)(4.0 / 3.0 * mu * dxi); A.vx_c = (T)(2.0 / 3.0 * mu * 0.25 * dyi); A.vx_s = (T)(mu * dxi);
     A.vx_t = (T)(mu * 0.25 * dyi); A.vx_q = (T)(kap * dxi);
   }
-  A.dF = s->mlp_on ? s->d_dF : nullptr;
-  A.dG = s->mlp_on ? s->d_dG : nullptr;
+  A.dF = (s->mlp_on || s->cnn_on) ? s->d_dF : nullptr;
+  A.dG = (s->mlp_on || s->cnn_on) ? s->d_dG : nullptr;
   for (int k = 0; k < 4; ++k) A.oscale[k] = (T)s->out_scale[k];
   const bool visc = s->mu > 0, artv = s->nu > 0;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -237,7 +244,7 @@ cudaError_t launch_stage(jxs_solver* s, const void* Uin, const void* U0, void* U
   if (s->ny == 1) {  // one-dimensional problems: stage1d_kernel.cuh
     stage1d_kernel<T><<<(s->nx + S1D_OUT - 1) / S1D_OUT, S1D_TB, 0, s->stream>>>(A);
     e = cudaGetLastError();
-  } else if (s->mlp_on) {
+  } else if (s->mlp_on || s->cnn_on) {
     if (visc) e = artv ? launch_stage_t<T, true, true, true>(s, A) : launch_stage_t<T, true, false, true>(s, A);
     else e = artv ? launch_stage_t<T, false, true, true>(s, A) : launch_stage_t<T, false, false, true>(s, A);
   } else {
@@ -298,7 +305,56 @@ cudaError_t launch_flux_mlp(jxs_solver* s, const void* U) {
   s->launches++;
   return cudaGetLastError();
 }
-cudaError_t flux_mlp(jxs_solver* s, const void* U) {
+// the CNN flux of the padded, ghost-filled state U -> d_dF, d_dG: reconstruction pass, then three convolution
+// layers per direction
+template <int KC, int CIN8, int NOUT, bool LAST>
+cudaError_t launch_cnn_layer(jxs_solver* s, const CnnLayerArgs& A0) {
+  CnnLayerArgs A = A0;
+  auto kern = cnn_layer_kernel<KC, CIN8, NOUT, LAST>;
+  constexpr int smem = cnn_smem_bytes<KC, NOUT>();
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  const int nstrips = (A.in.nb + CNN_TILE - 1) / CNN_TILE;
+  const int segs = std::max(1, s->num_sms * 4 / nstrips);
+  A.rows_per_seg = std::max((A.in.na + segs - 1) / segs, std::min(A.in.na, 8));
+  const int grid = nstrips * ((A.in.na + A.rows_per_seg - 1) / A.rows_per_seg);
+  kern<<<grid, CNN_TILE, smem, s->stream>>>(A);
+  s->launches++;
+  return cudaGetLastError();
+}
+template <typename T>
+cudaError_t launch_flux_cnn(jxs_solver* s, const void* U) {
+  CnnReconArgs<T> R;
+  R.U = (const T*)U; R.plane = s->plane; R.nx = s->nx; R.ny = s->ny; R.pitch = s->pitch;
+  R.g1 = (T)(s->gamma - 1.0); R.g1inv = (T)(1.0 / (s->gamma - 1.0));
+  for (int k = 0; k < 4; ++k) R.inv_scale[k] = (T)(1.0 / s->cnn_in_scale[k]);
+  R.Xx = s->cnn_X[0]; R.Xy = s->cnn_X[1];
+  const dim3 grid((s->nx + 1 + CNN_RX - 1) / CNN_RX, (s->ny + 1 + CNN_RY - 1) / CNN_RY);
+  cnn_recon_kernel<T><<<grid, CNN_RX * CNN_RY, 0, s->stream>>>(R);
+  s->launches++;
+  cudaError_t e = cudaGetLastError();
+  for (int d = 0; d < 2 && e == cudaSuccess; ++d) {
+    CnnLayerArgs A{};
+    A.plane = s->plane; A.pitch = s->pitch;
+    A.in = s->cnn_X[d]; A.out = s->cnn_H1[d]; A.blob = s->d_cnn_blob[d][0];
+    e = launch_cnn_layer<1, 1, 32, false>(s, A);
+    if (e != cudaSuccess) break;
+    A.in = s->cnn_H1[d]; A.out = s->cnn_H2[d]; A.blob = s->d_cnn_blob[d][1];
+    e = launch_cnn_layer<2, 4, 16, false>(s, A);
+    if (e != cudaSuccess) break;
+    A.in = s->cnn_H2[d]; A.blob = s->d_cnn_blob[d][2];
+    A.dst = d == 0 ? s->d_dF : s->d_dG;  // x: row j -> padded row j+3, face f -> column f+2; y: face-row f -> f+2, i -> i+3
+    A.row_off = d == 0 ? 3 : 2; A.col_off = d == 0 ? 2 : 3;
+    e = launch_cnn_layer<1, 2, 16, true>(s, A);
+  }
+  return e;
+}
+cudaError_t flux_mlp(jxs_solver* s, const void* U) {  // whichever network is set
+  if (s->cnn_on) return s->dtype == JXS_F64 ? launch_flux_cnn<double>(s, U) : launch_flux_cnn<float>(s, U);
   if (!s->mlp_on) return cudaSuccess;
   return s->dtype == JXS_F64 ? launch_flux_mlp<double>(s, U) : launch_flux_mlp<float>(s, U);
 }
@@ -320,6 +376,26 @@ void pack_canonical(const float* W, int N, int Kin, int Npad, int Kpad, uint8_t*
       const uint16_t b = bf16_bits(W[(size_t)n * Kin + k]);
       std::memcpy(dst + off, &b, 2);
     }
+}
+
+// one convolution layer's blob: [9 taps][KC][NOUT x 16] canonical bf16 tiles + NOUT fp32 biases.
+// W is OIHW [cout][cin][3 tangential taps][3 normal taps]; the kernel's tap (row offset, face offset) is
+// (tangential, normal) for x-faces and (normal, tangential) for y-faces (transposed = true).
+std::vector<uint8_t> pack_cnn_layer(const float* W, const float* b, int cout, int cin, int KC, int NOUT, bool transposed) {
+  std::vector<uint8_t> blob((size_t)9 * KC * NOUT * 32 + NOUT * 4, 0);
+  std::vector<float> tile((size_t)NOUT * 16);
+  for (int dr = 0; dr < 3; ++dr)
+    for (int dp = 0; dp < 3; ++dp)
+      for (int ks = 0; ks < KC; ++ks) {
+        std::fill(tile.begin(), tile.end(), 0.f);
+        const int ta = transposed ? dp : dr, tb = transposed ? dr : dp;
+        for (int n = 0; n < cout; ++n)
+          for (int k = 0; k < 16 && 16 * ks + k < cin; ++k)
+            tile[(size_t)n * 16 + k] = W[(((size_t)n * cin + 16 * ks + k) * 3 + ta) * 3 + tb];
+        pack_canonical(tile.data(), NOUT, 16, NOUT, 16, blob.data() + ((size_t)(dr * 3 + dp) * KC + ks) * NOUT * 32);
+      }
+  std::memcpy(blob.data() + (size_t)9 * KC * NOUT * 32, b, (size_t)cout * 4);
+  return blob;
 }
 
 cudaError_t pad(jxs_solver* s, const void* U, void* dst) {
@@ -580,6 +656,10 @@ void jxs_destroy(jxs_solver* s) {
   cudaFree(s->d_state);
   free_ibm(s);
   cudaFree(s->d_mlp_blob); cudaFree(s->d_dF); cudaFree(s->d_dG);
+  for (int d = 0; d < 2; ++d) {
+    cudaFree(s->cnn_X[d].data); cudaFree(s->cnn_H1[d].data); cudaFree(s->cnn_H2[d].data);
+    for (int l = 0; l < 3; ++l) cudaFree(s->d_cnn_blob[d][l]);
+  }
   for (cudaEvent_t ev : s->events) cudaEventDestroy(ev);
   for (cudaEvent_t ev : s->mlp_events) cudaEventDestroy(ev);
   delete s;
@@ -673,6 +753,7 @@ int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[
   CU(cudaStreamSynchronize(s->stream));
   if (!weights) { s->mlp_on = false; return JXS_OK; }
   if (s->ny == 1) return fail(s, JXS_EINVAL, "no flux MLP in one-dimensional problems");
+  if (s->cnn_on) return fail(s, JXS_ESTATE, "the CNN flux is set: disable it first (jxs_set_flux_cnn(NULL))");
   if (!in_scale || !out_scale) return fail(s, JXS_EINVAL, "in_scale / out_scale is NULL");
   for (int k = 0; k < 4; ++k)
     if (!(in_scale[k] > 0) || !std::isfinite(in_scale[k]) || !std::isfinite(out_scale[k]))
@@ -703,6 +784,62 @@ int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[
   s->mlp_rows_per_seg = rps;
   s->mlp_grid = s->mlp_strips * ((nrows + rps - 1) / rps);
   s->mlp_on = true;
+  return JXS_OK;
+}
+
+int jxs_set_flux_cnn(jxs_solver* s, const float* weights, const double in_scale[4], const double out_scale[4]) {
+  if (!s) return JXS_EINVAL;
+  drop_graph(s);
+  CU(cudaStreamSynchronize(s->stream));
+  if (!weights) { s->cnn_on = false; return JXS_OK; }
+  if (s->ny == 1) return fail(s, JXS_EINVAL, "no CNN flux in one-dimensional problems");
+  if (s->mlp_on) return fail(s, JXS_ESTATE, "the flux MLP is set: disable it first (jxs_set_flux_mlp(NULL))");
+  if (!in_scale || !out_scale) return fail(s, JXS_EINVAL, "in_scale / out_scale is NULL");
+  for (int k = 0; k < 4; ++k)
+    if (!(in_scale[k] > 0) || !std::isfinite(in_scale[k]) || !std::isfinite(out_scale[k]))
+      return fail(s, JXS_EINVAL, "in_scale must be > 0 and out_scale finite");
+  for (int i = 0; i < 6388; ++i)
+    if (!std::isfinite(weights[i])) return fail(s, JXS_EINVAL, "non-finite CNN weight");
+  // OIHW: W1[32][4][3][3], b1[32], W2[16][32][3][3], b2[16], W3[4][16][3][3], b3[4]
+  const float *W1 = weights, *b1 = W1 + 32 * 4 * 9, *W2 = b1 + 32, *b2 = W2 + 16 * 32 * 9, *W3 = b2 + 16, *b3 = W3 + 4 * 16 * 9;
+  for (int d = 0; d < 2; ++d) {
+    const std::vector<uint8_t> blobs[3] = {pack_cnn_layer(W1, b1, 32, 4, 1, 32, d == 1), pack_cnn_layer(W2, b2, 16, 32, 2, 16, d == 1),
+                                           pack_cnn_layer(W3, b3, 4, 16, 1, 16, d == 1)};
+    for (int l = 0; l < 3; ++l) {
+      if (!s->d_cnn_blob[d][l]) CU(cudaMalloc(&s->d_cnn_blob[d][l], blobs[l].size()));
+      CU(cudaMemcpy(s->d_cnn_blob[d][l], blobs[l].data(), blobs[l].size(), cudaMemcpyHostToDevice));
+    }
+    // fields: x-faces rows j (ny), faces f (nx+1); y-faces rows f (ny+1), faces i (nx); zero border all around
+    const int na = d == 0 ? s->ny : s->ny + 1, nb = d == 0 ? s->nx + 1 : s->nx;
+    const int nbp = (nb + CNN_TILE - 1) / CNN_TILE * CNN_TILE + 2;
+    CnnField* f[3] = {&s->cnn_X[d], &s->cnn_H1[d], &s->cnn_H2[d]};
+    const int chunks[3] = {1, 4, 2};
+    for (int q = 0; q < 3; ++q) {
+      const size_t bytes = (size_t)(na + 2) * chunks[q] * nbp * sizeof(uint4);
+      if (!f[q]->data) CU(cudaMalloc(&f[q]->data, bytes));
+      CU(cudaMemset(f[q]->data, 0, bytes));
+      f[q]->na = na; f[q]->nb = nb; f[q]->nbp = nbp; f[q]->C = chunks[q];
+    }
+  }
+  const size_t fbytes = (size_t)4 * s->plane * sizeof(float);
+  if (!s->d_dF) { CU(cudaMalloc(&s->d_dF, fbytes)); CU(cudaMemset(s->d_dF, 0, fbytes)); }
+  if (!s->d_dG) { CU(cudaMalloc(&s->d_dG, fbytes)); CU(cudaMemset(s->d_dG, 0, fbytes)); }
+  for (int k = 0; k < 4; ++k) { s->cnn_in_scale[k] = in_scale[k]; s->out_scale[k] = out_scale[k]; }
+  s->cnn_on = true;
+  return JXS_OK;
+}
+
+int jxs_flux_cnn_inputs(jxs_solver* s, const void* U, float* Xx, float* Xy) {
+  if (!s) return JXS_EINVAL;
+  if (!U || !Xx || !Xy) return fail(s, JXS_EINVAL, "NULL array");
+  if (!s->cnn_on) return fail(s, JXS_ESTATE, "no CNN set (jxs_set_flux_cnn)");
+  CU(pad(s, U, s->buf[0]));
+  CU(ghost_fill(s, s->buf[0]));
+  CU(flux_mlp(s, s->buf[0]));
+  const int bs = 256, gs = s->num_sms * 8;
+  cnn_inputs_gather_kernel<<<gs, bs, 0, s->stream>>>(s->cnn_X[0], s->cnn_X[1], Xx, Xy, s->nx, s->ny);
+  s->launches++;
+  CU(cudaGetLastError());
   return JXS_OK;
 }
 
@@ -822,7 +959,7 @@ int jxs_flux_mlp_time(const jxs_solver* s, double* ms_total, long long* launches
 int jxs_flux_correction(jxs_solver* s, const void* U, float* dFx, float* dGy) {
   if (!s) return JXS_EINVAL;
   if (!U || !dFx || !dGy) return fail(s, JXS_EINVAL, "NULL array");
-  if (!s->mlp_on) return fail(s, JXS_ESTATE, "no MLP set (jxs_set_flux_mlp)");
+  if (!s->mlp_on && !s->cnn_on) return fail(s, JXS_ESTATE, "no flux network set (jxs_set_flux_mlp / jxs_set_flux_cnn)");
   CU(pad(s, U, s->buf[0]));
   CU(ghost_fill(s, s->buf[0]));
   CU(flux_mlp(s, s->buf[0]));

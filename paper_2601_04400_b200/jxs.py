@@ -23,7 +23,7 @@ EXPORTS = ("jxs_create", "jxs_destroy", "jxs_last_error", "jxs_set_ibm", "jxs_se
            "jxs_step_host", "jxs_rhs_host", "jxs_get_time", "jxs_launch_count", "jxs_set_profiling",
            "jxs_stage_time", "jxs_ibm_ghost_count", "jxs_measure_fp64_peak", "jxs_flux_correction",
            "jxs_flux_mlp_time", "jxs_step_async", "jxs_wait", "jxs_set_time_integrator",
-           "jxs_set_concurrent_handles")
+           "jxs_set_concurrent_handles", "jxs_set_flux_cnn", "jxs_flux_cnn_inputs")
 
 
 class jxs_bc(C.Structure):
@@ -72,6 +72,8 @@ def lib():
         L.jxs_wait.argtypes = [vp]
         L.jxs_set_time_integrator.argtypes = [vp, C.c_int]
         L.jxs_set_concurrent_handles.argtypes = [vp, C.c_int]
+        L.jxs_set_flux_cnn.argtypes = [vp, vp, dp, dp]
+        L.jxs_flux_cnn_inputs.argtypes = [vp, vp, vp, vp]
         L.jxs_get_time.argtypes = [vp, dp, dp]
         L.jxs_launch_count.argtypes = [vp]
         L.jxs_launch_count.restype = C.c_longlong
@@ -169,6 +171,25 @@ class Solver:
         b = np.ascontiguousarray(out_scale, dtype=np.float64)
         dp = C.POINTER(C.c_double)
         self._chk(lib().jxs_set_flux_mlp(self._h, w.ctypes.data, a.ctypes.data_as(dp), b.ctypes.data_as(dp)))
+
+    def set_flux_cnn(self, weights, in_scale=None, out_scale=None):
+        """The paper's 2D CNN flux: 6388 weights in OIHW order (None disables)."""
+        if weights is None:
+            self._chk(lib().jxs_set_flux_cnn(self._h, None, None, None))
+            return
+        w = np.ascontiguousarray(weights, dtype=np.float32)
+        assert w.shape == (6388,)
+        a = np.ascontiguousarray(in_scale, dtype=np.float64)
+        b = np.ascontiguousarray(out_scale, dtype=np.float64)
+        dp = C.POINTER(C.c_double)
+        self._chk(lib().jxs_set_flux_cnn(self._h, w.ctypes.data, a.ctypes.data_as(dp), b.ctypes.data_as(dp)))
+
+    def flux_cnn_inputs(self, U):
+        """(Xx [4, ny, nx+1], Xy [4, nx, ny+1]) fp32 device tensors: the CNN's normalised input fields."""
+        Xx = torch.empty((4, self.ny, self.nx + 1), dtype=torch.float32, device=U.device)
+        Xy = torch.empty((4, self.nx, self.ny + 1), dtype=torch.float32, device=U.device)
+        self._chk(lib().jxs_flux_cnn_inputs(self._h, self._dev(U), C.c_void_p(Xx.data_ptr()), C.c_void_p(Xy.data_ptr())))
+        return Xx, Xy
 
     def flux_correction(self, U):
         """(dFx [4, ny, nx+1], dGy [4, ny+1, nx]) fp32 device tensors: Eq. 11's Delta F at every face."""
