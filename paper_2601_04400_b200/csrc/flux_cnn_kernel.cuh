@@ -25,6 +25,7 @@
 #include <stdint.h>
 
 #include "flux_mlp_kernel.cuh"
+#include "stage_kernel.cuh"
 
 namespace jxs {
 
@@ -38,20 +39,6 @@ struct CnnField {      // one activation field in HBM
 };
 
 // ------------------------------------------------------------------ pass 1: the input fields
-// left-biased WENO5-JS value at the face right of c, literal form (R4)
-template <typename T>
-__device__ __forceinline__ T weno5_literal(T a, T b, T c, T d, T e) {
-  const T q0 = (T(2) * a - T(7) * b + T(11) * c) / T(6), q1 = (-b + T(5) * c + T(2) * d) / T(6),
-          q2 = (T(2) * c + T(5) * d - e) / T(6);
-  const T s0 = a - T(2) * b + c, s1 = b - T(2) * c + d, s2 = c - T(2) * d + e;
-  const T t0 = a - T(4) * b + T(3) * c, t1 = b - d, t2 = T(3) * c - T(4) * d + e;
-  const T b0 = T(13) / T(12) * s0 * s0 + T(0.25) * t0 * t0 + T(1e-6);
-  const T b1 = T(13) / T(12) * s1 * s1 + T(0.25) * t1 * t1 + T(1e-6);
-  const T b2 = T(13) / T(12) * s2 * s2 + T(0.25) * t2 * t2 + T(1e-6);
-  const T a0 = T(0.1) / (b0 * b0), a1 = T(0.6) / (b1 * b1), a2 = T(0.3) / (b2 * b2);
-  return (a0 * q0 + a1 * q1 + a2 * q2) / (a0 + a1 + a2);
-}
-
 template <typename T>
 struct CnnReconArgs {
   const T* U;  // padded [4][ny+6][pitch], ghosts filled
@@ -59,66 +46,73 @@ struct CnnReconArgs {
   int nx, ny, pitch;
   T g1, g1inv;
   T inv_scale[4];  // 1 / in_scale of (rho, rho u_n, rho u_t, E)
+  T c133, eps4, sixth;  // WENO constants of stage_kernel.cuh (13/3, 4e-6, 1/6)
   CnnField Xx, Xy; // Xx: rows j, faces f = 0..nx;  Xy: rows f = 0..ny, faces i
 };
 
-constexpr int CNN_RX = 32, CNN_RY = 8;  // cells per CTA of the reconstruction pass
+// One thread per cell of a 32 x 8 tile; neighbouring tiles overlap by one cell in each direction, so that every
+// face between two cells of a tile gets its left state from one thread and its right state from the next (through
+// shared memory): 31 x 8 x-faces and 32 x 7 y-faces per CTA.  Cell-centred WENO5 of stage_kernel.cuh (weno5_n):
+// same arithmetic as the stage kernel, the input field is rounded to bf16 anyway.
+constexpr int CNN_RX = 32, CNN_RY = 8;
 
 template <typename T>
 __global__ void __launch_bounds__(CNN_RX * CNN_RY) cnn_recon_kernel(const CnnReconArgs<T> A) {
-  __shared__ T W[4][CNN_RY + 5][CNN_RX + 5];  // primitives of cells [i0-2, i0+34] x [j0-2, j0+10]
+  __shared__ T W[4][CNN_RY + 4][CNN_RX + 4];  // primitives of cells [i0-2, i0+33] x [j0-2, j0+9]
+  __shared__ T Rx[4][CNN_RY][CNN_RX];         // right-biased state at each cell's left face (rho, u, v, p)
+  __shared__ T Ry[4][CNN_RY][CNN_RX];         // right-biased state at each cell's bottom face
   const int tx = threadIdx.x % CNN_RX, ty = threadIdx.x / CNN_RX;
-  const int i0 = blockIdx.x * CNN_RX - 1, j0 = blockIdx.y * CNN_RY - 1;  // cells start at (-1,-1): see below
-  for (int q = threadIdx.x; q < (CNN_RY + 5) * (CNN_RX + 5); q += CNN_RX * CNN_RY) {
-    const int cx = q % (CNN_RX + 5), cy = q / (CNN_RX + 5);
+  const int i0 = blockIdx.x * (CNN_RX - 1) - 1, j0 = blockIdx.y * (CNN_RY - 1) - 1;  // tile origin (cells start at -1)
+  for (int q = threadIdx.x; q < (CNN_RY + 4) * (CNN_RX + 4); q += CNN_RX * CNN_RY) {
+    const int cx = q % (CNN_RX + 4), cy = q / (CNN_RX + 4);
     const int ip = min(max(i0 - 2 + cx + 3, 0), A.nx + 5), jp = min(max(j0 - 2 + cy + 3, 0), A.ny + 5);
     const T* s = A.U + (size_t)jp * A.pitch + ip;
     const T r = s[0], ru = s[A.plane], rv = s[2 * A.plane], E = s[3 * A.plane];
-    const T u = ru / r, v = rv / r;
+    const T ri = rcp_(r);
+    const T u = ru * ri, v = rv * ri;
     W[0][cy][cx] = r; W[1][cy][cx] = u; W[2][cy][cx] = v;
-    W[3][cy][cx] = A.g1 * (E - T(0.5) * (ru * u + rv * v));
+    W[3][cy][cx] = A.g1 * fma_(T(-0.5), fma_(ru, u, rv * v), E);
   }
   __syncthreads();
-  // cell (i, j), i in [-1, nx-1], j in [-1, ny-1]: its right face is x-face f = i+1 of row j (needs j >= 0),
-  // its top face is y-face f = j+1 of column i (needs i >= 0)
-  const int i = i0 + tx, j = j0 + ty;
-  if (i > A.nx - 1 || j > A.ny - 1) return;
   const int cx = tx + 2, cy = ty + 2;
-  auto face_input = [&](const T (&L)[4], const T (&R)[4]) -> uint4 {  // states (rho, u_n, u_t, p) -> 4 bf16 + 4 zeros
-    float m[4];
-    const T eL = L[3] * A.g1inv + T(0.5) * L[0] * (L[1] * L[1] + L[2] * L[2]);
-    const T eR = R[3] * A.g1inv + T(0.5) * R[0] * (R[1] * R[1] + R[2] * R[2]);
-    m[0] = (float)(T(0.5) * (L[0] + R[0]) * A.inv_scale[0]);
-    m[1] = (float)(T(0.5) * (L[0] * L[1] + R[0] * R[1]) * A.inv_scale[1]);
-    m[2] = (float)(T(0.5) * (L[0] * L[2] + R[0] * R[2]) * A.inv_scale[2]);
-    m[3] = (float)(T(0.5) * (eL + eR) * A.inv_scale[3]);
-    return make_uint4(pack_bf16(m[0], m[1]), pack_bf16(m[2], m[3]), 0u, 0u);
+  StageArgs<T> K;  // only the three WENO constants are read
+  K.c133 = A.c133; K.eps4 = A.eps4; K.sixth = A.sixth;
+  T wc[4], Lx[4], Ly[4];  // my primitives; left-biased states at my right and top faces
+  {
+    T a[4], b[4], d[4], e[4], Rm[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { a[k] = W[k][cy][cx - 2]; b[k] = W[k][cy][cx - 1]; wc[k] = W[k][cy][cx]; d[k] = W[k][cy][cx + 1]; e[k] = W[k][cy][cx + 2]; }
+    weno5_n<T, 4>(a, b, wc, d, e, K, Rm, Lx);
+    const bool badR = not_positive(Rm[0]) | not_positive(Rm[3]), badL = not_positive(Lx[0]) | not_positive(Lx[3]);  // R15
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { Rx[k][ty][tx] = badR ? wc[k] : Rm[k]; Lx[k] = badL ? wc[k] : Lx[k]; }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { a[k] = W[k][cy - 2][cx]; b[k] = W[k][cy - 1][cx]; d[k] = W[k][cy + 1][cx]; e[k] = W[k][cy + 2][cx]; }
+    weno5_n<T, 4>(a, b, wc, d, e, K, Rm, Ly);
+    const bool badRy = not_positive(Rm[0]) | not_positive(Rm[3]), badLy = not_positive(Ly[0]) | not_positive(Ly[3]);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { Ry[k][ty][tx] = badRy ? wc[k] : Rm[k]; Ly[k] = badLy ? wc[k] : Ly[k]; }
+  }
+  __syncthreads();
+  // mean of the two states at a face as conservative variables (rho, rho u_n, rho u_t, E) / in_scale -> 4 bf16 + 4 zeros
+  auto face_input = [&](T rl, T unl, T utl, T pl, T rr, T unr, T utr, T pr) -> uint4 {
+    const T eL = fma_(T(0.5) * rl, fma_(unl, unl, utl * utl), pl * A.g1inv);
+    const T eR = fma_(T(0.5) * rr, fma_(unr, unr, utr * utr), pr * A.g1inv);
+    const float m0 = (float)(T(0.5) * (rl + rr) * A.inv_scale[0]);
+    const float m1 = (float)(T(0.5) * fma_(rl, unl, rr * unr) * A.inv_scale[1]);
+    const float m2 = (float)(T(0.5) * fma_(rl, utl, rr * utr) * A.inv_scale[2]);
+    const float m3 = (float)(T(0.5) * (eL + eR) * A.inv_scale[3]);
+    return make_uint4(pack_bf16(m0, m1), pack_bf16(m2, m3), 0u, 0u);
   };
-  if (j >= 0) {
-    T L[4], R[4];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      const T* w = &W[k][cy][cx];
-      L[k] = weno5_literal(w[-2], w[-1], w[0], w[1], w[2]);
-      R[k] = weno5_literal(w[3], w[2], w[1], w[0], w[-1]);
-    }
-    if (!(L[0] > T(0)) || !(L[3] > T(0))) { for (int k = 0; k < 4; ++k) L[k] = W[k][cy][cx]; }      // R15
-    if (!(R[0] > T(0)) || !(R[3] > T(0))) { for (int k = 0; k < 4; ++k) R[k] = W[k][cy][cx + 1]; }
-    A.Xx.data[A.Xx.at(j, 0, i + 1)] = face_input(L, R);
-  }
-  if (i >= 0) {
-    T L[4], R[4];
-    const int perm[4] = {0, 2, 1, 3};  // normal velocity first
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      const int kk = perm[k];
-      L[k] = weno5_literal(W[kk][cy - 2][cx], W[kk][cy - 1][cx], W[kk][cy][cx], W[kk][cy + 1][cx], W[kk][cy + 2][cx]);
-      R[k] = weno5_literal(W[kk][cy + 3][cx], W[kk][cy + 2][cx], W[kk][cy + 1][cx], W[kk][cy][cx], W[kk][cy - 1][cx]);
-    }
-    if (!(L[0] > T(0)) || !(L[3] > T(0))) { for (int k = 0; k < 4; ++k) L[k] = W[perm[k]][cy][cx]; }
-    if (!(R[0] > T(0)) || !(R[3] > T(0))) { for (int k = 0; k < 4; ++k) R[k] = W[perm[k]][cy + 1][cx]; }
-    A.Xy.data[A.Xy.at(j + 1, 0, i)] = face_input(L, R);
-  }
+  const int i = i0 + tx, j = j0 + ty;  // my cell
+  // x-face f = i+1 of row j, between me and my right neighbour in the tile
+  if (tx < CNN_RX - 1 && i + 1 <= A.nx && j >= 0 && j < A.ny)
+    A.Xx.data[A.Xx.at(j, 0, i + 1)] =
+        face_input(Lx[0], Lx[1], Lx[2], Lx[3], Rx[0][ty][tx + 1], Rx[1][ty][tx + 1], Rx[2][ty][tx + 1], Rx[3][ty][tx + 1]);
+  // y-face f = j+1 of column i: normal velocity v first
+  if (ty < CNN_RY - 1 && j + 1 <= A.ny && i >= 0 && i < A.nx)
+    A.Xy.data[A.Xy.at(j + 1, 0, i)] =
+        face_input(Ly[0], Ly[2], Ly[1], Ly[3], Ry[0][ty + 1][tx], Ry[2][ty + 1][tx], Ry[1][ty + 1][tx], Ry[3][ty + 1][tx]);
 }
 
 // test / inspection: the bf16 input fields -> float arrays in the oracle's layout, Xx[4][ny][nx+1] (row j, face f)

@@ -319,7 +319,7 @@ cudaError_t launch_cnn_layer(jxs_solver* s, const CnnLayerArgs& A0) {
     configured = true;
   }
   const int nstrips = (A.in.nb + CNN_TILE - 1) / CNN_TILE;
-  const int segs = std::max(1, s->num_sms * 4 / nstrips);
+  const int segs = std::max(1, s->num_sms * 8 / nstrips);
   A.rows_per_seg = std::max((A.in.na + segs - 1) / segs, std::min(A.in.na, 8));
   const int grid = nstrips * ((A.in.na + A.rows_per_seg - 1) / A.rows_per_seg);
   kern<<<grid, CNN_TILE, smem, s->stream>>>(A);
@@ -333,7 +333,9 @@ cudaError_t launch_flux_cnn(jxs_solver* s, const void* U) {
   R.g1 = (T)(s->gamma - 1.0); R.g1inv = (T)(1.0 / (s->gamma - 1.0));
   for (int k = 0; k < 4; ++k) R.inv_scale[k] = (T)(1.0 / s->cnn_in_scale[k]);
   R.Xx = s->cnn_X[0]; R.Xy = s->cnn_X[1];
-  const dim3 grid((s->nx + 1 + CNN_RX - 1) / CNN_RX, (s->ny + 1 + CNN_RY - 1) / CNN_RY);
+  R.c133 = (T)(13.0 / 3.0); R.eps4 = (T)4e-6; R.sixth = (T)(1.0 / 6.0);
+  // tiles overlap by one cell: 31 x-faces and 7 y-faces per tile and direction, cells from -1 to nx / ny
+  const dim3 grid((s->nx + 2 + CNN_RX - 2) / (CNN_RX - 1), (s->ny + 2 + CNN_RY - 2) / (CNN_RY - 1));
   cnn_recon_kernel<T><<<grid, CNN_RX * CNN_RY, 0, s->stream>>>(R);
   s->launches++;
   cudaError_t e = cudaGetLastError();
