@@ -195,20 +195,32 @@ __global__ void __launch_bounds__(CNN_TILE) cnn_layer_kernel(const CnnLayerArgs 
   constexpr uint32_t IDESC = umma_idesc(128, NOUT);
   uint32_t phase = 0;
 
-  // input row r -> ring slot (r + 1) % 3, window faces b0-1 .. b0+128 at buffer positions 0 .. 129
-  auto load_row = [&](int r) {
-    unsigned char* dst = sm + OFF_ROWS + ((r + 1) % 3) * SLOT;
+  // input row r -> ring slot (r + 1) % 3, window faces b0-1 .. b0+128 at buffer positions 0 .. 129.  The global
+  // loads of a row are issued one iteration before its stores, so their latency hides behind the MMAs and the
+  // epilogue of the row in between.
+  uint4 pre[CIN8], pre2[CIN8];  // my face (and, threads 0-1, one of the two extra faces) of the row in flight
+  auto fetch_row = [&](int r) {
 #pragma unroll
     for (int c = 0; c < CIN8; ++c) {
       const uint4* src = A.in.data + A.in.at(r, c, b0 - 1);
-      reinterpret_cast<uint4*>(dst + c * LBO_A)[t] = src[t];
-      if (t < 2) reinterpret_cast<uint4*>(dst + c * LBO_A)[CNN_TILE + t] = src[CNN_TILE + t];
+      pre[c] = src[t];
+      if (t < 2) pre2[c] = src[CNN_TILE + t];
     }
   };
-  load_row(abeg - 1);
-  load_row(abeg);
+  auto store_row = [&](int r) {
+    unsigned char* dst = sm + OFF_ROWS + ((r + 1) % 3) * SLOT;
+#pragma unroll
+    for (int c = 0; c < CIN8; ++c) {
+      reinterpret_cast<uint4*>(dst + c * LBO_A)[t] = pre[c];
+      if (t < 2) reinterpret_cast<uint4*>(dst + c * LBO_A)[CNN_TILE + t] = pre2[c];
+    }
+  };
+  fetch_row(abeg - 1); store_row(abeg - 1);
+  fetch_row(abeg); store_row(abeg);
+  fetch_row(abeg + 1);
   for (int a = abeg; a < aend; ++a) {
-    load_row(a + 1);  // rows -1 and na are the zero border of the field
+    store_row(a + 1);  // rows -1 and na are the zero border of the field
+    if (a + 1 < aend) fetch_row(a + 2);
     fence_async_smem();
     tc_fence_before();
     __syncthreads();
