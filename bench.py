@@ -187,6 +187,62 @@ def run_sod1d(args, rank, world, local_rank, dist, barrier, tdt):
         "e2e": None, "cpu_baseline": None}))
 
 
+def run_cnn(args, rank, world, local_rank, dist, barrier, tdt):
+    """the C4 grid with the paper's 2D CNN neural flux (Eq. 11-13) in
+    every stage: reconstruction pass + 3 convolution layers per direction on tcgen05, then the stage kernel."""
+    import torch
+    from paper_2601_04400_b200 import jxs, workloads as wl
+    case = wl.throughput_case(args.nx, args.ny)
+    ncell = args.nx * args.ny
+    stream = torch.cuda.current_stream()
+    solver = jxs.Solver.from_case(case, dtype=tdt, stream=stream)
+    solver.set_flux_cnn(wl.cnn_weights(), *wl.cnn_scales())
+    U = torch.tensor(case["U0"], dtype=tdt, device="cuda")
+    K, W = args.steps, args.warmup
+    solver.step(U, 0.4, W)
+    solver.set_profiling(True)
+    sampler = ClockSampler(local_rank)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = solver.launch_count()
+    barrier()
+    sampler.start()
+    e0.record(stream)
+    solver.step(U, 0.4, K)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = max_over_ranks(e0.elapsed_time(e1), dist, "cuda")
+    stage_ms, stage_n = solver.stage_time()
+    net_ms, net_n = solver.flux_mlp_time()
+    if not bool(torch.isfinite(U).all()):
+        raise SystemExit("bench.py: non-finite state after the timed region")
+    if rank != 0:
+        return
+    # network roofline: 2 (36*32 + 288*16 + 144*4) = 12 672 flop per face, 2 faces per cell, bf16 tensor cores
+    flop = 2.0 * 12672.0 * ncell
+    avg = net_ms / max(net_n, 1)
+    peak = 1376.0
+    try:
+        peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["bf16_tflops_sustained"]
+    except Exception:
+        pass
+    print(json.dumps({
+        "metric": METRIC, "value": aggregate_rate(ncell, K, world, ms), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
+        "data": "synthetic",
+        "config": {"workload": f"throughput_{args.nx}x{args.ny} with the paper's 2D CNN neural flux (6388 parameters, bf16) in every stage",
+                   "cfl": 0.4, "rk": "SSP-RK3", "cells": ncell, "l2": "state and activation fields far larger than L2, no flush needed",
+                   "parallelism": "replicas" if world > 1 else "single GPU"},
+        "clocks": clocks, "gpu_launches": solver.launch_count() - launches0,
+        "roofline": {"bound": "tensor", "achieved": flop / (avg * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
+                     "frac": flop / (avg * 1e-3) / 1e12 / peak, "traffic": None,
+                     "kernel": "jxs::cnn_recon_kernel + 6 x jxs::cnn_layer_kernel (one network pass)",
+                     "avg_launch_ms": avg, "launches_timed": net_n, "stage_kernel_avg_launch_ms": stage_ms / max(stage_n, 1),
+                     "alg_flop_per_cell_stage": 2.0 * 12672.0,
+                     "peak_source": "MEASURED_PEAKS.json bf16_tflops_sustained (dense bf16)"},
+        "e2e": None, "cpu_baseline": None}))
+
+
 def run_c5(args, rank, world, local_rank, dist, barrier, tdt):
     """BASELINE.json configs[4]: 16 handles x (1024x512 shock-cylinder, Mach ~ U[1.5,3]) with the bf16 flux MLP
     fused into the fp64 HLLC flux; one stream per handle, jxs_step_async on each, aggregate Mcell-stage/s."""
@@ -279,7 +335,7 @@ def main():
     ap.add_argument("--euler", action="store_true", help="mu = 0, no IBM (not the headline config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile-kernels", action="store_true", help="c5 only: per-kernel CUDA-event spans")
-    ap.add_argument("--workload", choices=("c4", "c5", "sod1d"), default="c4",
+    ap.add_argument("--workload", choices=("c4", "c5", "sod1d", "cnn"), default="c4",
                     help="c4 = the headline throughput case (default); c5 = BASELINE.json configs[4]: 16 independent "
                          "1024x512 shock-cylinder runs with the per-face flux MLP, one stream per handle; sod1d = the "
                          "paper's 1D Sod tube at its largest size (3e6 cells = 9e6 degrees of freedom, PAPER.md L149)")
@@ -316,6 +372,9 @@ def main():
         return
     if args.workload == "sod1d":
         run_sod1d(args, rank, world, local_rank, dist, barrier, tdt)
+        return
+    if args.workload == "cnn":
+        run_cnn(args, rank, world, local_rank, dist, barrier, tdt)
         return
     case = wl.throughput_case(args.nx, args.ny, viscous=not args.euler, ibm=not args.euler)
     ncell = args.nx * args.ny

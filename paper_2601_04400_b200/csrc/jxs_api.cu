@@ -356,7 +356,17 @@ cudaError_t launch_flux_cnn(jxs_solver* s, const void* U) {
   return e;
 }
 cudaError_t flux_mlp(jxs_solver* s, const void* U) {  // whichever network is set
-  if (s->cnn_on) return s->dtype == JXS_F64 ? launch_flux_cnn<double>(s, U) : launch_flux_cnn<float>(s, U);
+  if (s->cnn_on) {  // jxs_flux_mlp_time then reports the whole network pass (reconstruction + 6 layer launches)
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (s->profiling && s->mlp_events_used + 2 <= (int)s->mlp_events.size()) {
+      e0 = s->mlp_events[s->mlp_events_used++];
+      e1 = s->mlp_events[s->mlp_events_used++];
+      cudaEventRecord(e0, s->stream);
+    }
+    const cudaError_t e = s->dtype == JXS_F64 ? launch_flux_cnn<double>(s, U) : launch_flux_cnn<float>(s, U);
+    if (e1) cudaEventRecord(e1, s->stream);
+    return e;
+  }
   if (!s->mlp_on) return cudaSuccess;
   return s->dtype == JXS_F64 ? launch_flux_mlp<double>(s, U) : launch_flux_mlp<float>(s, U);
 }
