@@ -39,25 +39,26 @@ struct CnnField {      // one activation field in HBM
 };
 
 // ------------------------------------------------------------------ pass 1: the input fields
-template <typename T>
+template <typename S>
 struct CnnReconArgs {
-  const T* U;  // padded [4][ny+6][pitch], ghosts filled
+  const S* U;  // padded [4][ny+6][pitch], ghosts filled
   long long plane;
   int nx, ny, pitch;
-  T g1, g1inv;
-  T inv_scale[4];  // 1 / in_scale of (rho, rho u_n, rho u_t, E)
-  T c133, eps4, sixth;  // WENO constants of stage_kernel.cuh (13/3, 4e-6, 1/6)
+  float g1, g1inv;
+  float inv_scale[4];  // 1 / in_scale of (rho, rho u_n, rho u_t, E)
+  float c133, eps4, sixth;  // WENO constants of stage_kernel.cuh (13/3, 4e-6, 1/6)
   CnnField Xx, Xy; // Xx: rows j, faces f = 0..nx;  Xy: rows f = 0..ny, faces i
 };
 
 // One thread per cell of a 32 x 8 tile; neighbouring tiles overlap by one cell in each direction, so that every
 // face between two cells of a tile gets its left state from one thread and its right state from the next (through
-// shared memory): 31 x 8 x-faces and 32 x 7 y-faces per CTA.  Cell-centred WENO5 of stage_kernel.cuh (weno5_n):
-// same arithmetic as the stage kernel, the input field is rounded to bf16 anyway.
+// shared memory): 31 x 8 x-faces and 32 x 7 y-faces per CTA.  Cell-centred WENO5 of stage_kernel.cuh (weno5_n),
+// evaluated in fp32 whatever the state's type: the field is rounded to bf16 (8 significant bits) right after.
 constexpr int CNN_RX = 32, CNN_RY = 8;
 
-template <typename T>
-__global__ void __launch_bounds__(CNN_RX * CNN_RY) cnn_recon_kernel(const CnnReconArgs<T> A) {
+template <typename S>
+__global__ void __launch_bounds__(CNN_RX * CNN_RY) cnn_recon_kernel(const CnnReconArgs<S> A) {
+  using T = float;
   __shared__ T W[4][CNN_RY + 4][CNN_RX + 4];  // primitives of cells [i0-2, i0+33] x [j0-2, j0+9]
   __shared__ T Rx[4][CNN_RY][CNN_RX];         // right-biased state at each cell's left face (rho, u, v, p)
   __shared__ T Ry[4][CNN_RY][CNN_RX];         // right-biased state at each cell's bottom face
@@ -66,8 +67,8 @@ __global__ void __launch_bounds__(CNN_RX * CNN_RY) cnn_recon_kernel(const CnnRec
   for (int q = threadIdx.x; q < (CNN_RY + 4) * (CNN_RX + 4); q += CNN_RX * CNN_RY) {
     const int cx = q % (CNN_RX + 4), cy = q / (CNN_RX + 4);
     const int ip = min(max(i0 - 2 + cx + 3, 0), A.nx + 5), jp = min(max(j0 - 2 + cy + 3, 0), A.ny + 5);
-    const T* s = A.U + (size_t)jp * A.pitch + ip;
-    const T r = s[0], ru = s[A.plane], rv = s[2 * A.plane], E = s[3 * A.plane];
+    const S* s = A.U + (size_t)jp * A.pitch + ip;
+    const T r = (T)s[0], ru = (T)s[A.plane], rv = (T)s[2 * A.plane], E = (T)s[3 * A.plane];
     const T ri = rcp_(r);
     const T u = ru * ri, v = rv * ri;
     W[0][cy][cx] = r; W[1][cy][cx] = u; W[2][cy][cx] = v;

@@ -330,10 +330,10 @@ template <typename T>
 cudaError_t launch_flux_cnn(jxs_solver* s, const void* U) {
   CnnReconArgs<T> R;
   R.U = (const T*)U; R.plane = s->plane; R.nx = s->nx; R.ny = s->ny; R.pitch = s->pitch;
-  R.g1 = (T)(s->gamma - 1.0); R.g1inv = (T)(1.0 / (s->gamma - 1.0));
-  for (int k = 0; k < 4; ++k) R.inv_scale[k] = (T)(1.0 / s->cnn_in_scale[k]);
+  R.g1 = (float)(s->gamma - 1.0); R.g1inv = (float)(1.0 / (s->gamma - 1.0));
+  for (int k = 0; k < 4; ++k) R.inv_scale[k] = (float)(1.0 / s->cnn_in_scale[k]);
   R.Xx = s->cnn_X[0]; R.Xy = s->cnn_X[1];
-  R.c133 = (T)(13.0 / 3.0); R.eps4 = (T)4e-6; R.sixth = (T)(1.0 / 6.0);
+  R.c133 = (float)(13.0 / 3.0); R.eps4 = 4e-6f; R.sixth = (float)(1.0 / 6.0);
   // tiles overlap by one cell: 31 x-faces and 7 y-faces per tile and direction, cells from -1 to nx / ny
   const dim3 grid((s->nx + 2 + CNN_RX - 2) / (CNN_RX - 1), (s->ny + 2 + CNN_RY - 2) / (CNN_RY - 1));
   cnn_recon_kernel<T><<<grid, CNN_RX * CNN_RY, 0, s->stream>>>(R);
