@@ -285,4 +285,150 @@ __global__ void __launch_bounds__(CNN_TILE) cnn_layer_kernel(const CnnLayerArgs 
   if (warp == 0) tmem_dealloc(tmem, 32);
 }
 
+// ------------------------------------------------------------------ the same layer with the row taps stacked along N
+// A 128 x N x 16 MMA with N <= 32 costs ~64 cycles whatever it computes (measured: the tensor core's fetch of the
+// 4 KB activation tile), so the layer above is bound by its 9 * KC MMAs per row.  Input row r feeds THREE output
+// rows (r+1 with row tap 0, r with tap 1, r-1 with tap 2) from the same shifted windows, so one MMA with the three
+// taps' weights side by side (N = 3 * NOUT) does the work of three: 3 * KC MMAs per row.  The three accumulators
+// (TMEM column groups g = output row mod 3) are always accumulated into; the group whose output row is complete
+// after input row r (row r-1) is read by the epilogue and zeroed with tcgen05.st.  Which tap a group needs depends
+// on r mod 3, hence three permutations of the weight tiles (packed on the host):
+//   blob = [3 permutations][3 face taps db][KC][3 NOUT x 16] canonical tiles, then NOUT fp32 biases;
+//   in permutation q = r mod 3, rows g * NOUT .. of a tile hold row tap da = (q + 1 - g) mod 3.
+// Only the current input row is needed in shared memory (double-buffered).
+template <int KC, int NOUT>
+__host__ __device__ constexpr int cnn3_wbytes() { return 3 * 3 * KC * 3 * NOUT * 16 * 2; }
+template <int KC, int NOUT>
+__host__ __device__ constexpr int cnn3_smem_bytes() {
+  return (cnn3_wbytes<KC, NOUT>() + NOUT * 4 + 127) / 128 * 128 + 2 * cnn_slot_bytes<KC>() + 16;
+}
+
+template <int NCOL>
+__device__ __forceinline__ void tmem_zero(uint32_t taddr) {  // NCOL (multiple of 16) columns of my lane <- 0
+#pragma unroll
+  for (int h = 0; h < NCOL / 16; ++h)
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1};"
+                 ::"r"(taddr + 16 * h), "r"(0u) : "memory");
+  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+
+template <int KC, int CIN8, int NOUT, bool LAST>
+__global__ void __launch_bounds__(CNN_TILE) cnn_layer3_kernel(const CnnLayerArgs A) {
+  extern __shared__ __align__(128) unsigned char sm[];
+  __shared__ uint32_t tmem_slot;
+  constexpr int WB = cnn3_wbytes<KC, NOUT>();
+  constexpr int OFF_ROWS = (WB + NOUT * 4 + 127) / 128 * 128;
+  constexpr int SLOT = cnn_slot_bytes<KC>();
+  constexpr int LBO_A = CNN_ROWP * 16;
+  constexpr int N3 = 3 * NOUT;
+  constexpr int TCOLS = N3 <= 64 ? 64 : 128;
+  constexpr int PERM = 3 * KC * N3 * 32;  // bytes of one permutation of the tiles
+  const int t = threadIdx.x, warp = t >> 5;
+  const int nstrips = (A.in.nb + CNN_TILE - 1) / CNN_TILE;
+  const int strip = blockIdx.x % nstrips, seg = blockIdx.x / nstrips;
+  const int abeg = seg * A.rows_per_seg, aend = min(abeg + A.rows_per_seg, A.in.na);
+  if (abeg >= aend) return;
+  const int b0 = strip * CNN_TILE;
+  const uint32_t sm_u32 = (uint32_t)__cvta_generic_to_shared(sm);
+  const uint32_t bar = sm_u32 + OFF_ROWS + 2 * SLOT;
+  const float* bias = reinterpret_cast<const float*>(sm + WB);
+
+  for (int i = t; i < (WB + NOUT * 4) / 16; i += CNN_TILE)
+    reinterpret_cast<uint4*>(sm)[i] = reinterpret_cast<const uint4*>(A.blob)[i];
+  for (int i = t; i < 2 * SLOT / 16; i += CNN_TILE) reinterpret_cast<uint4*>(sm + OFF_ROWS)[i] = make_uint4(0, 0, 0, 0);
+  if (t == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(1) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 0) tmem_alloc((uint32_t)__cvta_generic_to_shared(&tmem_slot), TCOLS);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+  const uint32_t tlane = tmem + ((uint32_t)(32 * warp) << 16);
+  constexpr uint32_t IDESC = umma_idesc(128, N3);
+  uint32_t phase = 0;
+  tmem_zero<N3>(tlane);  // the three accumulators start at zero and are only ever added to
+
+  uint4 pre[CIN8], pre2[CIN8];
+  auto fetch_row = [&](int r) {
+#pragma unroll
+    for (int c = 0; c < CIN8; ++c) {
+      const uint4* src = A.in.data + A.in.at(r, c, b0 - 1);
+      pre[c] = src[t];
+      if (t < 2) pre2[c] = src[CNN_TILE + t];
+    }
+  };
+  auto store_row = [&](int r) {
+    unsigned char* dst = sm + OFF_ROWS + ((r + 2) & 1) * SLOT;
+#pragma unroll
+    for (int c = 0; c < CIN8; ++c) {
+      reinterpret_cast<uint4*>(dst + c * LBO_A)[t] = pre[c];
+      if (t < 2) reinterpret_cast<uint4*>(dst + c * LBO_A)[CNN_TILE + t] = pre2[c];
+    }
+  };
+  fetch_row(abeg - 1);
+  for (int r = abeg - 1; r <= aend; ++r) {  // input rows; rows -1 and na are the zero border of the field
+    store_row(r);
+    if (r < aend) fetch_row(r + 1);
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    if (t == 0) {
+      tc_fence_after();
+      const uint32_t rowbuf = sm_u32 + OFF_ROWS + ((r + 2) & 1) * SLOT;
+      const uint32_t wperm = sm_u32 + ((r + 3) % 3) * PERM;
+#pragma unroll
+      for (int db = 0; db < 3; ++db)
+#pragma unroll
+        for (int ks = 0; ks < KC; ++ks)
+          umma_bf16(tmem, umma_desc(rowbuf + ks * 2 * LBO_A + db * 16, LBO_A, 128),
+                    umma_desc(wperm + (db * KC + ks) * N3 * 32, N3 * 16, 128), IDESC, 1u);
+      umma_commit(bar);
+    }
+    mbar_wait_spin(bar, phase); phase ^= 1;
+    tc_fence_after();
+    // output row r-1 is complete: its accumulator is column group (r-1) mod 3
+    const int row = r - 1, p = b0 + t;
+    const uint32_t tg = tlane + ((row + 3) % 3) * NOUT;
+    const bool live = row >= abeg && row < aend && p < A.in.nb;
+    if (!LAST) {
+#pragma unroll
+      for (int h = 0; h < NOUT / 16; ++h) {
+        uint32_t v[16];
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                       "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                     : "r"(tg + 16 * h) : "memory");
+        tmem_ld_wait();
+        if (live) {
+#pragma unroll
+          for (int c = 0; c < 2; ++c) {
+            uint32_t w[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const int k = 8 * c + 2 * e;
+              w[e] = pack_bf16(fmaxf(__uint_as_float(v[k]) + bias[16 * h + k], 0.f), fmaxf(__uint_as_float(v[k + 1]) + bias[16 * h + k + 1], 0.f));
+            }
+            A.out.data[A.out.at(row, 2 * h + c, p)] = make_uint4(w[0], w[1], w[2], w[3]);
+          }
+        }
+      }
+    } else {
+      uint32_t y[4];
+      tmem_ld4(tg, y);
+      tmem_ld_wait();
+      if (live) {
+        float* o = A.dst + (size_t)(row + A.row_off) * A.pitch + p + A.col_off;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) o[k * A.plane] = tanh_f32(__uint_as_float(y[k]) + bias[k]);
+      }
+    }
+    tmem_zero<NOUT>(tg);  // the group starts over with output row r+2
+    tc_fence_before();
+  }
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tmem, TCOLS);
+}
+
 }  // namespace jxs

@@ -65,6 +65,7 @@ struct jxs_solver {
   bool cnn_on = false;
   CnnField cnn_X[2] = {}, cnn_H1[2] = {}, cnn_H2[2] = {};
   uint8_t* d_cnn_blob[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
+  uint8_t* d_cnn_blob3[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};  // for cnn_layer3_kernel
   double cnn_in_scale[4] = {1, 1, 1, 1};
   int mlp_strips = 0, mlp_rows_per_seg = 0, mlp_grid = 0;
   double mlp_ms = 0;
@@ -326,6 +327,25 @@ cudaError_t launch_cnn_layer(jxs_solver* s, const CnnLayerArgs& A0) {
   s->launches++;
   return cudaGetLastError();
 }
+template <int KC, int CIN8, int NOUT, bool LAST>
+cudaError_t launch_cnn_layer3(jxs_solver* s, const CnnLayerArgs& A0) {
+  CnnLayerArgs A = A0;
+  auto kern = cnn_layer3_kernel<KC, CIN8, NOUT, LAST>;
+  constexpr int smem = cnn3_smem_bytes<KC, NOUT>();
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  const int nstrips = (A.in.nb + CNN_TILE - 1) / CNN_TILE;
+  const int segs = std::max(1, s->num_sms * 8 / nstrips);
+  A.rows_per_seg = std::max((A.in.na + segs - 1) / segs, std::min(A.in.na, 8));
+  const int grid = nstrips * ((A.in.na + A.rows_per_seg - 1) / A.rows_per_seg);
+  kern<<<grid, CNN_TILE, smem, s->stream>>>(A);
+  s->launches++;
+  return cudaGetLastError();
+}
 template <typename T>
 cudaError_t launch_flux_cnn(jxs_solver* s, const void* U) {
   CnnReconArgs<T> R;
@@ -339,7 +359,22 @@ cudaError_t launch_flux_cnn(jxs_solver* s, const void* U) {
   cnn_recon_kernel<T><<<grid, CNN_RX * CNN_RY, 0, s->stream>>>(R);
   s->launches++;
   cudaError_t e = cudaGetLastError();
-  for (int d = 0; d < 2 && e == cudaSuccess; ++d) {
+  static const bool nine = getenv("JXS_CNN_NINE_TAPS") != nullptr;  // measurement: one MMA per tap (cnn_layer_kernel)
+  for (int d = 0; d < 2 && e == cudaSuccess && !nine; ++d) {
+    CnnLayerArgs A{};
+    A.plane = s->plane; A.pitch = s->pitch;
+    A.in = s->cnn_X[d]; A.out = s->cnn_H1[d]; A.blob = s->d_cnn_blob3[d][0];
+    e = launch_cnn_layer3<1, 1, 32, false>(s, A);
+    if (e != cudaSuccess) break;
+    A.in = s->cnn_H1[d]; A.out = s->cnn_H2[d]; A.blob = s->d_cnn_blob3[d][1];
+    e = launch_cnn_layer3<2, 4, 16, false>(s, A);
+    if (e != cudaSuccess) break;
+    A.in = s->cnn_H2[d]; A.blob = s->d_cnn_blob3[d][2];
+    A.dst = d == 0 ? s->d_dF : s->d_dG;
+    A.row_off = d == 0 ? 3 : 2; A.col_off = d == 0 ? 2 : 3;
+    e = launch_cnn_layer3<1, 2, 16, true>(s, A);
+  }
+  for (int d = 0; d < 2 && e == cudaSuccess && nine; ++d) {
     CnnLayerArgs A{};
     A.plane = s->plane; A.pitch = s->pitch;
     A.in = s->cnn_X[d]; A.out = s->cnn_H1[d]; A.blob = s->d_cnn_blob[d][0];
@@ -407,6 +442,29 @@ std::vector<uint8_t> pack_cnn_layer(const float* W, const float* b, int cout, in
         pack_canonical(tile.data(), NOUT, 16, NOUT, 16, blob.data() + ((size_t)(dr * 3 + dp) * KC + ks) * NOUT * 32);
       }
   std::memcpy(blob.data() + (size_t)9 * KC * NOUT * 32, b, (size_t)cout * 4);
+  return blob;
+}
+
+// the same layer for cnn_layer3_kernel: [3 permutations q][3 face taps dp][KC][3 NOUT x 16] tiles + NOUT biases; rows
+// g * NOUT .. of a tile hold row tap dr = (q + 1 - g) mod 3
+std::vector<uint8_t> pack_cnn_layer3(const float* W, const float* b, int cout, int cin, int KC, int NOUT, bool transposed) {
+  const int N3 = 3 * NOUT;
+  std::vector<uint8_t> blob((size_t)3 * 3 * KC * N3 * 32 + NOUT * 4, 0);
+  std::vector<float> tile((size_t)N3 * 16);
+  for (int q = 0; q < 3; ++q)
+    for (int dp = 0; dp < 3; ++dp)
+      for (int ks = 0; ks < KC; ++ks) {
+        std::fill(tile.begin(), tile.end(), 0.f);
+        for (int g = 0; g < 3; ++g) {
+          const int dr = ((q + 1 - g) % 3 + 3) % 3;
+          const int ta = transposed ? dp : dr, tb = transposed ? dr : dp;
+          for (int n = 0; n < cout; ++n)
+            for (int k = 0; k < 16 && 16 * ks + k < cin; ++k)
+              tile[(size_t)(g * NOUT + n) * 16 + k] = W[(((size_t)n * cin + 16 * ks + k) * 3 + ta) * 3 + tb];
+        }
+        pack_canonical(tile.data(), N3, 16, N3, 16, blob.data() + ((size_t)(q * 3 + dp) * KC + ks) * N3 * 32);
+      }
+  std::memcpy(blob.data() + (size_t)3 * 3 * KC * N3 * 32, b, (size_t)cout * 4);
   return blob;
 }
 
@@ -670,7 +728,7 @@ void jxs_destroy(jxs_solver* s) {
   cudaFree(s->d_mlp_blob); cudaFree(s->d_dF); cudaFree(s->d_dG);
   for (int d = 0; d < 2; ++d) {
     cudaFree(s->cnn_X[d].data); cudaFree(s->cnn_H1[d].data); cudaFree(s->cnn_H2[d].data);
-    for (int l = 0; l < 3; ++l) cudaFree(s->d_cnn_blob[d][l]);
+    for (int l = 0; l < 3; ++l) { cudaFree(s->d_cnn_blob[d][l]); cudaFree(s->d_cnn_blob3[d][l]); }
   }
   for (cudaEvent_t ev : s->events) cudaEventDestroy(ev);
   for (cudaEvent_t ev : s->mlp_events) cudaEventDestroy(ev);
@@ -817,9 +875,13 @@ int jxs_set_flux_cnn(jxs_solver* s, const float* weights, const double in_scale[
   for (int d = 0; d < 2; ++d) {
     const std::vector<uint8_t> blobs[3] = {pack_cnn_layer(W1, b1, 32, 4, 1, 32, d == 1), pack_cnn_layer(W2, b2, 16, 32, 2, 16, d == 1),
                                            pack_cnn_layer(W3, b3, 4, 16, 1, 16, d == 1)};
+    const std::vector<uint8_t> blobs3[3] = {pack_cnn_layer3(W1, b1, 32, 4, 1, 32, d == 1), pack_cnn_layer3(W2, b2, 16, 32, 2, 16, d == 1),
+                                            pack_cnn_layer3(W3, b3, 4, 16, 1, 16, d == 1)};
     for (int l = 0; l < 3; ++l) {
       if (!s->d_cnn_blob[d][l]) CU(cudaMalloc(&s->d_cnn_blob[d][l], blobs[l].size()));
       CU(cudaMemcpy(s->d_cnn_blob[d][l], blobs[l].data(), blobs[l].size(), cudaMemcpyHostToDevice));
+      if (!s->d_cnn_blob3[d][l]) CU(cudaMalloc(&s->d_cnn_blob3[d][l], blobs3[l].size()));
+      CU(cudaMemcpy(s->d_cnn_blob3[d][l], blobs3[l].data(), blobs3[l].size(), cudaMemcpyHostToDevice));
     }
     // fields: x-faces rows j (ny), faces f (nx+1); y-faces rows f (ny+1), faces i (nx); zero border all around
     const int na = d == 0 ? s->ny : s->ny + 1, nb = d == 0 ? s->nx + 1 : s->nx;
