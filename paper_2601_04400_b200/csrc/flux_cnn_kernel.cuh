@@ -350,27 +350,29 @@ __global__ void __launch_bounds__(CNN_TILE) cnn_layer3_kernel(const CnnLayerArgs
   uint32_t phase = 0;
   tmem_zero<N3>(tlane);  // the three accumulators start at zero and are only ever added to
 
-  uint4 pre[CIN8], pre2[CIN8];
-  auto fetch_row = [&](int r) {
+  // the global loads of a row are issued TWO iterations before its stores (registers pre[r & 1]): one iteration is
+  // shorter than the memory latency under load
+  uint4 pre[2][CIN8], pre2[2][CIN8];
+  auto fetch_row = [&](int r, int q) {
 #pragma unroll
     for (int c = 0; c < CIN8; ++c) {
       const uint4* src = A.in.data + A.in.at(r, c, b0 - 1);
-      pre[c] = src[t];
-      if (t < 2) pre2[c] = src[CNN_TILE + t];
+      pre[q][c] = src[t];
+      if (t < 2) pre2[q][c] = src[CNN_TILE + t];
     }
   };
-  auto store_row = [&](int r) {
+  auto store_row = [&](int r, int q) {
     unsigned char* dst = sm + OFF_ROWS + ((r + 2) & 1) * SLOT;
 #pragma unroll
     for (int c = 0; c < CIN8; ++c) {
-      reinterpret_cast<uint4*>(dst + c * LBO_A)[t] = pre[c];
-      if (t < 2) reinterpret_cast<uint4*>(dst + c * LBO_A)[CNN_TILE + t] = pre2[c];
+      reinterpret_cast<uint4*>(dst + c * LBO_A)[t] = pre[q][c];
+      if (t < 2) reinterpret_cast<uint4*>(dst + c * LBO_A)[CNN_TILE + t] = pre2[q][c];
     }
   };
-  fetch_row(abeg - 1);
-  for (int r = abeg - 1; r <= aend; ++r) {  // input rows; rows -1 and na are the zero border of the field
-    store_row(r);
-    if (r < aend) fetch_row(r + 1);
+  // rows are taken in pairs so that the register buffers are indexed at compile time
+  auto row_step = [&](int r, int q) {
+    store_row(r, q);
+    if (r + 2 <= aend) fetch_row(r + 2, q);
     fence_async_smem();
     tc_fence_before();
     __syncthreads();
@@ -426,6 +428,12 @@ __global__ void __launch_bounds__(CNN_TILE) cnn_layer3_kernel(const CnnLayerArgs
     }
     tmem_zero<NOUT>(tg);  // the group starts over with output row r+2
     tc_fence_before();
+  };
+  fetch_row(abeg - 1, 0);
+  fetch_row(abeg, 1);
+  for (int r = abeg - 1; r <= aend; r += 2) {  // input rows; rows -1 and na are the zero border of the field
+    row_step(r, 0);
+    if (r + 1 <= aend) row_step(r + 1, 1);
   }
   __syncthreads();
   if (warp == 0) tmem_dealloc(tmem, TCOLS);
