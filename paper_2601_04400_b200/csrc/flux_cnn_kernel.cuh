@@ -13,6 +13,9 @@
 //                      tcgen05.mma whose A descriptor points at (row buffer da, 16*db bytes into it): im2col without
 //                      a copy.  9 * Cin/16 MMAs of 128 x Cout x 16 accumulate in TMEM; bias, ReLU (tanh in the last
 //                      layer) and the rounding to bf16 follow in registers.
+//   cnn_layer3_kernel  the same layer with the three ROW taps stacked along N (one MMA feeds three output rows):
+//                      a third of the MMAs; this is the kernel the library launches, cnn_layer_kernel is kept for
+//                      measurements (JXS_CNN_NINE_TAPS).
 //
 // Activation fields in HBM use the same chunked layout with a one-face border of zeros all around (the "SAME"
 // padding of every layer is then just what the loads find): element (row r, chunk c, face p) is the uint4 at
