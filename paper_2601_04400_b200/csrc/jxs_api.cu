@@ -86,6 +86,7 @@ struct jxs_solver {
   // work decomposition of the stage kernel
   int nstrips = 0, rows_per_seg = 0, nseg = 0, ntasks = 0, warps = 0, grid = 0;
   int share = 1;  // handles of about this size that step concurrently (jxs_set_concurrent_handles)
+  bool tuned = false;  // rows_per_seg measured on this device (tune_decomposition)
   // bookkeeping
   long long launches = 0;
   bool profiling = false;
@@ -158,6 +159,13 @@ bool make_tensor_map(const jxs_solver* s, void* base, int box_w, CUtensorMap* ou
 // (measured: mean task lifetime 75 % of the kernel's).  Many short tasks handed out dynamically by the
 // block scheduler keep every slot busy; the price is the ~2 row-equivalents of warm-up per task.
 // cost model: rows of work per slot, plus half a task of tail per slot
+void set_rows_per_seg(jxs_solver* s, int rps) {
+  s->rows_per_seg = rps;
+  s->nseg = (s->ny + rps - 1) / rps;
+  s->ntasks = s->nseg * s->nstrips;
+  s->grid = s->ntasks;
+}
+
 void choose_decomposition(jxs_solver* s) {
   const int SOUT = s->dtype == JXS_F64 ? sout<double>() : sout<float>();
   s->nstrips = (s->nx + SOUT - 1) / SOUT;
@@ -178,11 +186,9 @@ void choose_decomposition(jxs_solver* s) {
   for (int rps = lo; rps <= s->ny; ++rps)
     if (cost[rps] <= 1.01 * best) best_rps = rps;  // the longest segments among the near-optimal
   if (const char* e = getenv("JXS_ROWS_PER_SEG")) best_rps = std::max(1, std::min(s->ny, atoi(e)));
-  s->rows_per_seg = best_rps;
-  s->nseg = (s->ny + best_rps - 1) / best_rps;
-  s->ntasks = s->nseg * s->nstrips;
+  set_rows_per_seg(s, best_rps);
   s->warps = STAGE_WARPS;
-  s->grid = s->ntasks;
+  s->tuned = getenv("JXS_ROWS_PER_SEG") != nullptr;
 }
 
 template <typename T, bool VISC, bool ARTV, bool MLP>
@@ -622,6 +628,47 @@ int finish_steps(jxs_solver* s, int nsteps) {
   return JXS_OK;
 }
 
+// When the tasks make several waves, how a kernel ends depends on how the last wave falls (measured on C4: 0.4057 ms
+// at 25 rows per task, 0.4188 at 26, 0.4067 at 28, 0.4177 at 29): no model predicts that, so the first jxs_step* call
+// of a handle times one stage launch for every segment length around the heuristic's choice and keeps the best.
+// The results do not depend on the segmentation (every row is computed with the same arithmetic).  buf[0] holds
+// the padded state; buf[1] is scratch here.
+int tune_decomposition(jxs_solver* s) {
+  s->tuned = true;
+  const int minb = s->dtype == JXS_F64 ? stage_minb<double>() : stage_minb<float>();
+  if (s->ny == 1 || (long long)s->ntasks < 2LL * s->num_sms * minb / s->share) return JXS_OK;  // one wave: nothing to tune
+  const int base = s->rows_per_seg;
+  const bool prof = s->profiling;
+  s->profiling = false;
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0));
+  CU(cudaEventCreate(&e1));
+  CU(ghost_fill(s, s->buf[0]));
+  int best = base;
+  float best_ms = 1e30f;
+  cudaError_t err = cudaSuccess;
+  for (int rps = std::max(8, base - 12); rps <= std::min(s->ny, base + 8) && err == cudaSuccess; ++rps) {
+    set_rows_per_seg(s, rps);
+    float ms = 1e30f;
+    for (int rep = 0; rep < 2 && err == cudaSuccess; ++rep) {  // the first launch of the loop also warms the caches
+      cudaEventRecord(e0, s->stream);
+      err = stage(s, s->buf[0], nullptr, s->buf[1], 0, 0.0, 1.0, nullptr);
+      cudaEventRecord(e1, s->stream);
+      if (err == cudaSuccess) err = cudaEventSynchronize(e1);
+      float t = 0;
+      if (err == cudaSuccess) cudaEventElapsedTime(&t, e0, e1);
+      if (rep == 1 || rps > std::max(8, base - 12)) ms = std::min(ms, t);
+    }
+    if (ms < best_ms) { best_ms = ms; best = rps; }
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  set_rows_per_seg(s, best);
+  s->profiling = prof;
+  if (err != cudaSuccess) return cuda_fail(s, err, "tune_decomposition");
+  return JXS_OK;
+}
+
 int step_common(jxs_solver* s, void* U, double cfl, double fixed_dt, int nsteps, bool host, bool wait = true) {
   if (!s) return JXS_EINVAL;
   if (!U) return fail(s, JXS_EINVAL, "U is NULL");
@@ -634,6 +681,10 @@ int step_common(jxs_solver* s, void* U, double cfl, double fixed_dt, int nsteps,
     Ud = s->stage_io;
   }
   CU(pad(s, Ud, s->buf[0]));
+  if (!s->tuned && nsteps > 0) {
+    const int rc = tune_decomposition(s);
+    if (rc != JXS_OK) return rc;
+  }
   int at = 0;
   int rc = run_steps(s, cfl, fixed_dt, nsteps, &at);
   if (rc != JXS_OK) return rc;
