@@ -113,7 +113,9 @@ int jxs_max_wavespeed(jxs_solver*, const void* U, double* smax_host);
  * device at the start of every step (R6).  JXS_ENUMERIC if a non-finite or non-positive
  * wavespeed was met (U then holds the last state computed).  Synchronises once at the end.
  * For nsteps >= 6 (and jxs_set_profiling off) pairs of steps are replayed from a CUDA graph
- * captured on a private stream; results are identical to plain launches.                      */
+ * captured on a private stream; results are identical to plain launches.  The first stepping call
+ * of a handle on a large grid also times about forty stage launches to choose the length of the row
+ * segments the grid is cut into (it synchronises the stream once; results do not depend on it).   */
 int jxs_step(jxs_solver*, void* U, double cfl, int nsteps);
 /* Same with a fixed time step.                                                              */
 int jxs_step_fixed_dt(jxs_solver*, void* U, double dt, int nsteps);
