@@ -77,6 +77,37 @@ inline double to_double(float x) { return (double)x; }
 inline double to_double(Counted x) { return x.v; }
 
 // ---------------------------------------------------------------------------
+// dual number: a value and its derivative along ONE direction of perturbation.
+// Running the solver on it applies the chain of Jacobians of PAPER.md Eq. 16,
+//   prod_j dU^{n+j}/dU^{n+j-1}  and  dU^{n+k}/d(parameter),
+// to that direction (forward-mode differentiation; R21).  Every rule below is
+// the textbook derivative of the operation; comparisons look at the value only,
+// so min / max / sign / the positivity guard take the derivative of the branch
+// the value selects, and |x| has derivative sign(x) (0 at x = 0).
+// ---------------------------------------------------------------------------
+struct Dual {
+  double v, d;
+  Dual() : v(0), d(0) {}
+  Dual(double x) : v(x), d(0) {}
+  Dual(double x, double dx) : v(x), d(dx) {}
+  explicit operator double() const { return v; }
+};
+inline Dual operator+(Dual a, Dual b) { return Dual(a.v + b.v, a.d + b.d); }
+inline Dual operator-(Dual a, Dual b) { return Dual(a.v - b.v, a.d - b.d); }
+inline Dual operator-(Dual a) { return Dual(-a.v, -a.d); }
+inline Dual operator*(Dual a, Dual b) { return Dual(a.v * b.v, a.d * b.v + a.v * b.d); }
+inline Dual operator/(Dual a, Dual b) { return Dual(a.v / b.v, (a.d * b.v - a.v * b.d) / (b.v * b.v)); }
+inline Dual& operator+=(Dual& a, Dual b) { a = a + b; return a; }
+inline Dual& operator-=(Dual& a, Dual b) { a = a - b; return a; }
+inline bool operator<(Dual a, Dual b) { return a.v < b.v; }
+inline bool operator>(Dual a, Dual b) { return a.v > b.v; }
+inline bool operator<=(Dual a, Dual b) { return a.v <= b.v; }
+inline bool operator>=(Dual a, Dual b) { return a.v >= b.v; }
+inline Dual s_sqrt(Dual x) { const double r = std::sqrt(x.v); return Dual(r, x.d / (2.0 * r)); }
+inline Dual s_abs(Dual x) { return Dual(std::fabs(x.v), x.v > 0 ? x.d : (x.v < 0 ? -x.d : 0.0)); }
+inline double to_double(Dual x) { return x.v; }
+
+// ---------------------------------------------------------------------------
 // O4  WENO5-JS, left-biased value at i+1/2 from (a,b,c,d,e) = v[i-2..i+2]
 //     ("WENO ... convex reconstruction of candidate stencils"; R4:
 //     eps = 1e-6, linear weights 0.1/0.6/0.3, classical smoothness indicators,
@@ -240,7 +271,12 @@ struct Config {
   int nx, ny;
   double dx, dy, gamma, mu, Pr, nu;
   jxo_bc bc;
+  double gamma_dot = 0;  // perturbation of gamma carried by the Dual scalar (jxo_step_fixed_dt_tangent), else unused
 };
+
+// gamma as the solver's scalar: for Dual it carries the direction of perturbation
+template <class T> inline T gamma_of(const Config& c) { return T(c.gamma); }
+template <> inline Dual gamma_of<Dual>(const Config& c) { return Dual(c.gamma, c.gamma_dot); }
 
 // ---------------------------------------------------------------------------
 // the solver, templated on the scalar
@@ -295,7 +331,7 @@ struct Core {
     {
       const T r = T(c.bc.inflow[0]), u = T(c.bc.inflow[1]), v = T(c.bc.inflow[2]), p = T(c.bc.inflow[3]);
       inflow[0] = r; inflow[1] = r * u; inflow[2] = r * v;
-      inflow[3] = p / (T(c.gamma) - T(1)) + T(0.5) * r * (u * u + v * v);
+      inflow[3] = p / (gamma_of<T>(c) - T(1)) + T(0.5) * r * (u * u + v * v);
     }
     for (int t = lo; t < hi; ++t) {
       for (int k = 0; k < 4; ++k) {
@@ -328,7 +364,7 @@ struct Core {
     const T r = Up[a], ru = Up[plane + a], rv = Up[2 * plane + a], E = Up[3 * plane + a];
     const T u = ru / r, v = rv / r;
     W[0] = r; W[1] = u; W[2] = v;
-    W[3] = (T(c.gamma) - T(1)) * (E - T(0.5) * r * (u * u + v * v));
+    W[3] = (gamma_of<T>(c) - T(1)) * (E - T(0.5) * r * (u * u + v * v));
   }
 
   // O2 / I6: gather primitives at the donors, interpolate to the image point,
@@ -349,14 +385,14 @@ struct Core {
       Up[a] = r;
       Up[plane + a] = r * u;
       Up[2 * plane + a] = r * v;
-      Up[3 * plane + a] = p / (T(c.gamma) - T(1)) + T(0.5) * r * (u * u + v * v);
+      Up[3 * plane + a] = p / (gamma_of<T>(c) - T(1)) + T(0.5) * r * (u * u + v * v);
     }
   }
 
   // L(U) on a padded, ghost-filled array.  L is interior [4][ny][nx].
   void rhs(const std::vector<T>& Up, T* L) {
     const int nx = c.nx, ny = c.ny;
-    const T gamma = T(c.gamma);
+    const T gamma = gamma_of<T>(c);
     // O3: primitives at all padded cells
     std::vector<T> W(4 * plane);
     for (int j = -NG; j < ny + NG; ++j)
@@ -534,7 +570,7 @@ struct Core {
         if (type[(size_t)j * c.nx + i] != 0) continue;
         T w[4];
         prim_at(Up, at(i, j), w);
-        const T a = s_sqrt(T(c.gamma) * w[3] / w[0]);
+        const T a = s_sqrt(gamma_of<T>(c) * w[3] / w[0]);
         smax = s_max(smax, s_max(s_abs(w[1]) + a, s_abs(w[2]) + a));
       }
     return smax;
@@ -835,6 +871,52 @@ void jxo_hllc_star(const double WL[4], const double WR[4], double gamma, double 
   hllc_x<double>(WL, WR, gamma, F, &d);
   speeds[0] = d.sL; speeds[1] = d.sR; speeds[2] = d.sS;
   for (int k = 0; k < 4; ++k) { UstarL[k] = d.UsL[k]; UstarR[k] = d.UsR[k]; }
+}
+
+// O12 (R21): the tangent of jxo_step_fixed_dt.  On return U = S^n(U; gamma) and
+//   Udot = dS^n/dU . Udot + dS^n/dgamma . gamma_dot      (the Jacobian products of PAPER.md Eq. 16),
+// computed by running the same templated solver on Dual scalars.  fp64 handles without a network.
+int jxo_step_fixed_dt_tangent(jxo_solver* s, double* U, double* Udot, double gamma_dot, double dt, int nsteps) {
+  if (!s || !U || !Udot || !(dt > 0) || nsteps < 0) return JXO_EINVAL;
+  if (s->dtype != JXO_F64) { s->err = "the tangent is fp64 only"; return JXO_EINVAL; }
+  if (s->mlp.on || s->cnn.on) { s->err = "the tangent does not differentiate the networks"; return JXO_ESTATE; }
+  const size_t n = (size_t)4 * s->c.nx * s->c.ny;
+  std::vector<Dual> Ud(n), Up;
+  for (size_t i = 0; i < n; ++i) Ud[i] = Dual(U[i], Udot[i]);
+  s->c.gamma_dot = gamma_dot;
+  Core<Dual> core(s->c, s->type, s->ghosts, s->mlp);
+  core.pad(Ud.data(), Up);
+  for (int k = 0; k < nsteps; ++k) {
+    core.rk3_step(Up, Dual(dt));
+    s->t += dt;
+    s->last_dt = dt;
+  }
+  core.unpad(Up, Ud.data());
+  s->c.gamma_dot = 0;
+  s->guard += core.guard;
+  int rc = JXO_OK;
+  for (size_t i = 0; i < n; ++i) {
+    U[i] = Ud[i].v;
+    Udot[i] = Ud[i].d;
+    if (!std::isfinite(U[i]) || !std::isfinite(Udot[i])) rc = JXO_ENUMERIC;
+  }
+  if (rc == JXO_ENUMERIC) s->err = "non-finite state or tangent";
+  return rc;
+}
+
+// pointwise tangents of O4 and O5, for the closed-form pins
+void jxo_weno5_tangent(const double v[5], const double vdot[5], double out[2]) {
+  const Dual r = weno5<Dual>(Dual(v[0], vdot[0]), Dual(v[1], vdot[1]), Dual(v[2], vdot[2]), Dual(v[3], vdot[3]),
+                             Dual(v[4], vdot[4]));
+  out[0] = r.v; out[1] = r.d;
+}
+
+void jxo_hllc_tangent(const double WL[4], const double WR[4], const double WLdot[4], const double WRdot[4],
+                      double gamma, double gamma_dot, double F[4], double Fdot[4]) {
+  Dual L[4], R[4], f[4];
+  for (int k = 0; k < 4; ++k) { L[k] = Dual(WL[k], WLdot[k]); R[k] = Dual(WR[k], WRdot[k]); }
+  hllc_x<Dual>(L, R, Dual(gamma, gamma_dot), f);
+  for (int k = 0; k < 4; ++k) { F[k] = f[k].v; Fdot[k] = f[k].d; }
 }
 
 int jxo_fill_ghosts(jxo_solver* s, const void* U, void* Upad) {

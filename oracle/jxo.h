@@ -52,6 +52,11 @@ int jxo_max_wavespeed(jxo_solver*, const void* U, double* smax);
 int jxo_step(jxo_solver*, void* U, double cfl, int nsteps);
 int jxo_step_fixed_dt(jxo_solver*, void* U, double dt, int nsteps);
 int jxo_get_time(const jxo_solver*, double* t, double* last_dt);
+/* O12: the tangent (forward-mode derivative) of jxo_step_fixed_dt: the Jacobian products of PAPER.md Eq. 16 applied
+ * to one direction.  U, Udot: [4][ny][nx] doubles, in and out.  On return U = S^n(U; gamma) and
+ * Udot = dS^n/dU . Udot + dS^n/dgamma . gamma_dot.  fp64 handles without a network (EINVAL / ESTATE).
+ * With a loss L(U) (Eq. 14) this gives dL/dgamma = <dL/dU, Udot>: the paper's gamma inference (L149, Fig. 3b). */
+int jxo_step_fixed_dt_tangent(jxo_solver*, double* U, double* Udot, double gamma_dot, double dt, int nsteps);
 
 /* ---- introspection used only by the oracle's own pins ------------------- */
 /* one left-biased WENO5-JS value at i+1/2 from (v[i-2..i+2]) in double          */
@@ -61,6 +66,10 @@ void jxo_hllc(const double WL[4], const double WR[4], double gamma, double F[4])
 /* wave speeds sL,sR,s* and the two star states (conserved) of the same solver   */
 void jxo_hllc_star(const double WL[4], const double WR[4], double gamma,
                    double speeds[3], double UstarL[4], double UstarR[4]);
+/* tangents of the two routines above: out = {value, derivative along vdot}; F, Fdot along (WLdot, WRdot, gamma_dot) */
+void jxo_weno5_tangent(const double v[5], const double vdot[5], double out[2]);
+void jxo_hllc_tangent(const double WL[4], const double WR[4], const double WLdot[4], const double WRdot[4],
+                      double gamma, double gamma_dot, double F[4], double Fdot[4]);
 /* fill domain frame + IBM ghosts of U (interior array is copied into a padded
  * array, filled, and the padded array [4][ny+6][nx+6] is returned in Upad)      */
 int jxo_fill_ghosts(jxo_solver*, const void* U, void* Upad);

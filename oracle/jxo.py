@@ -59,6 +59,11 @@ def lib():
         L.jxo_set_flux_cnn.argtypes = [vp, vp, dp, dp, C.c_int]
         L.jxo_cnn_apply.argtypes = [vp, dp, C.c_int, C.c_int, dp]
         L.jxo_cnn_fields.argtypes = [vp, dp, dp, dp, dp, dp]
+        L.jxo_step_fixed_dt_tangent.argtypes = [vp, vp, vp, C.c_double, C.c_double, C.c_int]
+        L.jxo_weno5_tangent.argtypes = [dp, dp, dp]
+        L.jxo_weno5_tangent.restype = None
+        L.jxo_hllc_tangent.argtypes = [dp, dp, dp, dp, C.c_double, C.c_double, dp, dp]
+        L.jxo_hllc_tangent.restype = None
         _lib = L
     return _lib
 
@@ -91,6 +96,31 @@ def hllc(WL, WR, gamma):
     F = np.zeros(4)
     lib().jxo_hllc(_d(WL), _d(WR), float(gamma), _d(F))
     return F
+
+
+def weno5_tangent(v, vdot):
+    """(value, derivative along vdot) of the left-biased WENO5-JS value (O4)."""
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    vdot = np.ascontiguousarray(vdot, dtype=np.float64)
+    assert v.shape == (5,) and vdot.shape == (5,)
+    out = np.zeros(2)
+    lib().jxo_weno5_tangent(_d(v), _d(vdot), _d(out))
+    return out[0], out[1]
+
+
+def hllc_tangent(WL, WR, WLdot, WRdot, gamma, gamma_dot):
+    """(F, Fdot) of the HLLC flux (O5) along the direction (WLdot, WRdot, gamma_dot)."""
+    a = [np.ascontiguousarray(x, dtype=np.float64) for x in (WL, WR, WLdot, WRdot)]
+    F, Fd = np.zeros(4), np.zeros(4)
+    lib().jxo_hllc_tangent(_d(a[0]), _d(a[1]), _d(a[2]), _d(a[3]), float(gamma), float(gamma_dot), _d(F), _d(Fd))
+    return F, Fd
+
+
+def mse_tangent(U, Udot, Utarget):
+    """Eq. 14 for one step with the mean over all entries (R22): L = mean((U - Utarget)^2) and its derivative
+    along Udot, dL = mean(2 (U - Utarget) Udot)."""
+    r = np.asarray(U, dtype=np.float64) - np.asarray(Utarget, dtype=np.float64)
+    return float(np.mean(r * r)), float(np.mean(2.0 * r * np.asarray(Udot, dtype=np.float64)))
 
 
 def hllc_star(WL, WR, gamma):
@@ -201,6 +231,15 @@ class Oracle:
         U = self._field(U).copy()
         self._chk(lib().jxo_step_fixed_dt(self._h, U.ctypes.data, float(dt), int(nsteps)))
         return U
+
+    def step_fixed_dt_tangent(self, U, Udot, gamma_dot, dt, nsteps):
+        """O12: (U, Udot) after nsteps steps of size dt; Udot is the derivative along (Udot, gamma_dot)."""
+        U = np.ascontiguousarray(self._field(U), dtype=np.float64).copy()
+        Udot = np.ascontiguousarray(Udot, dtype=np.float64).copy()
+        assert Udot.shape == U.shape
+        self._chk(lib().jxo_step_fixed_dt_tangent(self._h, U.ctypes.data, Udot.ctypes.data, float(gamma_dot),
+                                                  float(dt), int(nsteps)))
+        return U, Udot
 
     def time(self):
         t, dt = C.c_double(), C.c_double()

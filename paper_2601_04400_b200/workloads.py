@@ -29,6 +29,31 @@ def cons_from_prim(rho, u, v, p, gamma=GAMMA):
     return np.stack([rho, rho * u, rho * v, E]).astype(np.float64)
 
 
+def dcons_dgamma(U, gamma=GAMMA):
+    """Direction of perturbation of a conserved field when gamma changes at fixed primitives (rho, u, v, p):
+    only E = p/(gamma-1) + kinetic moves, dE/dgamma = -p/(gamma-1)^2 = -(E - kinetic)/(gamma-1).  The seed of the
+    gamma inference (Fig. 3b), whose initial condition Eq. 17 is given in primitives."""
+    U = np.asarray(U, dtype=np.float64)
+    kin = 0.5 * (U[1] ** 2 + U[2] ** 2) / U[0]
+    D = np.zeros_like(U)
+    D[3] = -(U[3] - kin) / (gamma - 1.0)
+    return D
+
+
+def smooth_direction(shape, seed=3, modes=3):
+    """A seeded smooth field [4][ny][nx] (a few low Fourier modes per component, amplitude about 1): a direction of
+    perturbation of the state for the tangent tests."""
+    rng = np.random.default_rng(seed)
+    _, ny, nx = shape
+    X, Y = np.meshgrid((np.arange(nx) + 0.5) / nx, (np.arange(ny) + 0.5) / ny)
+    D = np.zeros(shape)
+    for k in range(4):
+        for _ in range(modes):
+            a, kx, ky, ph = rng.normal(), rng.integers(0, 3), rng.integers(0, 3), rng.uniform(0, 2 * math.pi)
+            D[k] += a * np.cos(2 * math.pi * (kx * X + (ky if ny > 1 else 0) * Y) + ph)
+    return D
+
+
 def cell_centres(nx, ny, dx, dy, x0=0.0, y0=0.0):
     x = x0 + (np.arange(nx) + 0.5) * dx
     y = y0 + (np.arange(ny) + 0.5) * dy
