@@ -119,6 +119,29 @@ int jxs_max_wavespeed(jxs_solver*, const void* U, double* smax_host);
 int jxs_step(jxs_solver*, void* U, double cfl, int nsteps);
 /* Same with a fixed time step.                                                              */
 int jxs_step_fixed_dt(jxs_solver*, void* U, double dt, int nsteps);
+/* Tangent (forward-mode derivative) of jxs_step_fixed_dt for one-dimensional problems: PAPER.md Eq. 15-16 (the step
+ * U^{n+k} = S(U^{n+k-1}, theta) and the chain of its Jacobians) applied to ONE direction of perturbation, for the
+ * paper's inference of the specific-heat ratio from Sod data (L149, Fig. 3b; R21).
+ *   U, Udot   DEVICE pointers, [4][1][nx] doubles, read and overwritten: the state and a direction of perturbation
+ *             of it (owned by the caller; Udot = 0 differentiates with respect to gamma at fixed conserved state,
+ *             Udot[3] = -p/(gamma-1)^2 at fixed primitives)
+ *   gamma_dot perturbation of gamma along the same direction
+ *   dt        step size, a constant of the differentiation (> 0); nsteps >= 0 SSP-RK3 steps
+ * On return U = S^nsteps(U; gamma) (the same arithmetic as the tangent's value part, equal to jxs_step_fixed_dt to
+ * round-off) and Udot = dS^nsteps/dU . Udot + dS^nsteps/dgamma . gamma_dot.  Branches of the scheme (min / max of wave
+ * speeds, sign of the contact speed, positivity guard) carry the derivative of the branch taken.
+ * Errors: JXS_EINVAL for NULL pointers, dt <= 0, nsteps < 0, a non-finite gamma_dot, an fp32 handle or ny != 1;
+ * JXS_ESTATE with a network set, with the forward-Euler integrator or with steps pending (jxs_wait);
+ * JXS_ENOMEM / JXS_ECUDA from the first call's allocation of the tangent buffers.  Synchronises the stream.      */
+int jxs_step_fixed_dt_tangent(jxs_solver*, void* U, void* Udot, double gamma_dot, double dt, int nsteps);
+
+/* The loss of PAPER.md Eq. 14 for one target and its derivative along a tangent (R22):
+ *   *loss = mean((U - Utarget)^2),  *dloss = mean(2 (U - Utarget) Udot)   over the 4 nx ny entries.
+ * U, Udot, Utarget: DEVICE pointers, [4][ny][nx] doubles, read only; loss, dloss: HOST doubles.  With Udot from
+ * jxs_step_fixed_dt_tangent, *dloss = dL/dgamma.  The summation order is fixed (two launches), so the result is
+ * reproducible.  Errors: JXS_EINVAL for NULL pointers or an fp32 handle.  Synchronises the stream.               */
+int jxs_mse_tangent(jxs_solver*, const void* U, const void* Udot, const void* Utarget, double* loss, double* dloss);
+
 /* Same two calls on HOST buffers (pageable or pinned): host->device copy, stepping,
  * device->host copy; used for end-to-end timing.                                            */
 int jxs_step_host(jxs_solver*, void* U_host, double cfl, int nsteps);

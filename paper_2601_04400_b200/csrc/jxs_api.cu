@@ -20,6 +20,7 @@
 #include "flux_cnn_kernel.cuh"
 #include "stage_kernel.cuh"
 #include "stage1d_kernel.cuh"
+#include "tangent1d_kernel.cuh"
 
 using namespace jxs;
 
@@ -44,6 +45,10 @@ struct jxs_solver {
   size_t elem = 8;
   void* buf[3] = {nullptr, nullptr, nullptr};
   void* stage_io = nullptr;  // interior-sized staging for the *_host entry points
+  // tangent of the state (tangent1d_kernel.cuh): three padded buffers like buf[], allocated at the first
+  // jxs_step_fixed_dt_tangent call; d_mse = partial sums and result of jxs_mse_tangent
+  void* bufd[3] = {nullptr, nullptr, nullptr};
+  double* d_mse = nullptr;
   // TMA descriptors of the three padded buffers: boxes [4][1][CW] (stencil rows) and [4][1][Epi::W] (RK operand rows)
   CUtensorMap tm_row[3], tm_epi[3];
   // immersed boundary
@@ -701,6 +706,83 @@ int step_common(jxs_solver* s, void* U, double cfl, double fixed_dt, int nsteps,
   return finish_steps(s, nsteps);
 }
 
+// ---- tangent of the one-dimensional step (tangent1d_kernel.cuh)
+constexpr int MSE_PARTS = 1024;
+
+// ghosts of the tangent buffer: the boundary conditions are linear in the state (copies and sign flips), so the
+// same kernel fills them; the inflow state is given in primitives, so only its energy moves with gamma
+cudaError_t ghost_fill_tangent(jxs_solver* s, void* Udot, double gamma_dot) {
+  BcSpec b = bcspec(s);
+  const double g1 = s->gamma - 1.0;
+  b.inflow_cons[0] = b.inflow_cons[1] = b.inflow_cons[2] = 0.0;
+  b.inflow_cons[3] = -s->bc.inflow[3] / (g1 * g1) * gamma_dot;
+  const int total = 6 * s->ny;
+  IbmList none{nullptr, nullptr, nullptr, nullptr, 0};
+  const int bs = 128;
+  ghost_fill_kernel<double><<<(total + bs - 1) / bs, bs, 0, s->stream>>>((double*)Udot, dims(s), b, none, s->gamma);
+  s->launches++;
+  return cudaGetLastError();
+}
+
+cudaError_t tangent_stage(jxs_solver* s, int in, int out, double a, double b, double gamma_dot) {
+  Tangent1dArgs A;
+  A.Uin = (const double*)s->buf[in]; A.Uin_dot = (const double*)s->bufd[in];
+  A.U0 = (const double*)s->buf[0]; A.U0_dot = (const double*)s->bufd[0];
+  A.Uout = (double*)s->buf[out]; A.Uout_dot = (double*)s->bufd[out];
+  A.dt = &s->d_state->dt;
+  A.plane = s->plane; A.nx = s->nx; A.pitch = s->pitch;
+  A.gamma = s->gamma; A.gamma_dot = gamma_dot; A.dxi = 1.0 / s->dx;
+  A.mu = s->mu; A.Pr = s->Pr; A.nu = s->nu; A.rk_a = a; A.rk_b = b;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (s->profiling && s->events_used + 2 <= (int)s->events.size()) {
+    e0 = s->events[s->events_used++];
+    e1 = s->events[s->events_used++];
+    cudaEventRecord(e0, s->stream);
+  }
+  tangent1d_kernel<<<(s->nx + T1D_OUT - 1) / T1D_OUT, T1D_TB, 0, s->stream>>>(A);
+  if (e1) cudaEventRecord(e1, s->stream);
+  s->launches++;
+  return cudaGetLastError();
+}
+
+int tangent_common(jxs_solver* s, void* U, void* Udot, double gamma_dot, double dt, int nsteps) {
+  if (!s) return JXS_EINVAL;
+  if (!U || !Udot) return fail(s, JXS_EINVAL, "U or Udot is NULL");
+  if (nsteps < 0) return fail(s, JXS_EINVAL, "nsteps < 0");
+  if (!(dt > 0)) return fail(s, JXS_EINVAL, "dt must be > 0");
+  if (!std::isfinite(gamma_dot)) return fail(s, JXS_EINVAL, "gamma_dot is not finite");
+  if (s->dtype != JXS_F64) return fail(s, JXS_EINVAL, "the tangent is fp64 only");
+  if (s->ny != 1) return fail(s, JXS_EINVAL, "the tangent is built for one-dimensional problems (ny = 1)");
+  if (s->mlp_on || s->cnn_on) return fail(s, JXS_ESTATE, "the tangent does not differentiate the networks");
+  if (s->scheme != JXS_SSPRK3) return fail(s, JXS_ESTATE, "the tangent steps with SSP-RK3");
+  if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
+  const size_t bytes = (size_t)4 * s->plane * s->elem;
+  for (int b = 0; b < 3; ++b)
+    if (!s->bufd[b]) {
+      CU(cudaMalloc(&s->bufd[b], bytes));
+      CU(cudaMemsetAsync(s->bufd[b], 0, bytes, s->stream));
+    }
+  CU(pad(s, U, s->buf[0]));
+  CU(pad(s, Udot, s->bufd[0]));
+  s->events_used = 0;
+  s->mlp_events_used = 0;
+  for (int n = 0; n < nsteps; ++n) {
+    prepare_step_kernel<<<1, 1, 0, s->stream>>>(s->d_state, 0, 0.0, dt);
+    s->launches++;
+    CU(cudaGetLastError());
+    static const double ab[3][2] = {{0.0, 1.0}, {0.75, 0.25}, {1.0 / 3.0, 2.0 / 3.0}};  // R5
+    static const int io[3][2] = {{0, 1}, {1, 2}, {2, 0}};
+    for (int st = 0; st < 3; ++st) {
+      CU(ghost_fill(s, s->buf[io[st][0]]));
+      CU(ghost_fill_tangent(s, s->bufd[io[st][0]], gamma_dot));
+      CU(tangent_stage(s, io[st][0], io[st][1], ab[st][0], ab[st][1], gamma_dot));
+    }
+  }
+  CU(unpad(s, s->buf[0], U));
+  CU(unpad(s, s->bufd[0], Udot));
+  return finish_steps(s, nsteps);
+}
+
 }  // namespace
 
 extern "C" {
@@ -774,6 +856,8 @@ void jxs_destroy(jxs_solver* s) {
   if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
   for (int b = 0; b < 3; ++b) cudaFree(s->buf[b]);
   cudaFree(s->stage_io);
+  for (int b = 0; b < 3; ++b) cudaFree(s->bufd[b]);
+  cudaFree(s->d_mse);
   cudaFree(s->d_state);
   free_ibm(s);
   cudaFree(s->d_mlp_blob); cudaFree(s->d_dF); cudaFree(s->d_dG);
@@ -1020,6 +1104,30 @@ int jxs_step_fixed_dt(jxs_solver* s, void* U, double dt, int nsteps) {
   if (s && !(dt > 0)) return fail(s, JXS_EINVAL, "dt must be > 0");
   return step_common(s, U, 0.0, dt, nsteps, false);
 }
+int jxs_step_fixed_dt_tangent(jxs_solver* s, void* U, void* Udot, double gamma_dot, double dt, int nsteps) {
+  return tangent_common(s, U, Udot, gamma_dot, dt, nsteps);
+}
+
+int jxs_mse_tangent(jxs_solver* s, const void* U, const void* Udot, const void* Utarget, double* loss, double* dloss) {
+  if (!s) return JXS_EINVAL;
+  if (!U || !Udot || !Utarget || !loss || !dloss) return fail(s, JXS_EINVAL, "NULL argument");
+  if (s->dtype != JXS_F64) return fail(s, JXS_EINVAL, "the tangent is fp64 only");
+  if (!s->d_mse) CU(cudaMalloc(&s->d_mse, (2 * MSE_PARTS + 2) * sizeof(double)));
+  const long long n = 4LL * s->nx * s->ny;
+  const int parts = (int)std::min<long long>(MSE_PARTS, (n + MSE_TB - 1) / MSE_TB);
+  mse_partial_kernel<<<parts, MSE_TB, 0, s->stream>>>((const double*)U, (const double*)Udot, (const double*)Utarget, n,
+                                                     s->d_mse);
+  mse_final_kernel<<<1, MSE_TB, 0, s->stream>>>(s->d_mse, parts, 1.0 / (double)n, s->d_mse + 2 * MSE_PARTS);
+  s->launches += 2;
+  CU(cudaGetLastError());
+  double out[2];
+  CU(cudaMemcpyAsync(out, s->d_mse + 2 * MSE_PARTS, sizeof(out), cudaMemcpyDeviceToHost, s->stream));
+  CU(cudaStreamSynchronize(s->stream));
+  *loss = out[0];
+  *dloss = out[1];
+  return JXS_OK;
+}
+
 int jxs_step_host(jxs_solver* s, void* U, double cfl, int nsteps) { return step_common(s, U, cfl, 0.0, nsteps, true); }
 int jxs_step_async(jxs_solver* s, void* U, double cfl, int nsteps) { return step_common(s, U, cfl, 0.0, nsteps, false, false); }
 int jxs_wait(jxs_solver* s) {

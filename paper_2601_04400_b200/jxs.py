@@ -23,7 +23,8 @@ EXPORTS = ("jxs_create", "jxs_destroy", "jxs_last_error", "jxs_set_ibm", "jxs_se
            "jxs_step_host", "jxs_rhs_host", "jxs_get_time", "jxs_launch_count", "jxs_set_profiling",
            "jxs_stage_time", "jxs_ibm_ghost_count", "jxs_measure_fp64_peak", "jxs_flux_correction",
            "jxs_flux_mlp_time", "jxs_step_async", "jxs_wait", "jxs_set_time_integrator",
-           "jxs_set_concurrent_handles", "jxs_set_flux_cnn", "jxs_flux_cnn_inputs")
+           "jxs_set_concurrent_handles", "jxs_set_flux_cnn", "jxs_flux_cnn_inputs",
+           "jxs_step_fixed_dt_tangent", "jxs_mse_tangent")
 
 
 class jxs_bc(C.Structure):
@@ -74,6 +75,8 @@ def lib():
         L.jxs_set_concurrent_handles.argtypes = [vp, C.c_int]
         L.jxs_set_flux_cnn.argtypes = [vp, vp, dp, dp]
         L.jxs_flux_cnn_inputs.argtypes = [vp, vp, vp, vp]
+        L.jxs_step_fixed_dt_tangent.argtypes = [vp, vp, vp, C.c_double, C.c_double, C.c_int]
+        L.jxs_mse_tangent.argtypes = [vp, vp, vp, vp, dp, dp]
         L.jxs_get_time.argtypes = [vp, dp, dp]
         L.jxs_launch_count.argtypes = [vp]
         L.jxs_launch_count.restype = C.c_longlong
@@ -246,6 +249,19 @@ class Solver:
     def step_fixed_dt(self, U, dt, nsteps):
         self._chk(lib().jxs_step_fixed_dt(self._h, self._dev(U), float(dt), int(nsteps)))
         return U
+
+    def step_fixed_dt_tangent(self, U, Udot, gamma_dot, dt, nsteps):
+        """In place on the device tensors U and Udot (one-dimensional fp64 handles): the step and its tangent."""
+        self._chk(lib().jxs_step_fixed_dt_tangent(self._h, self._dev(U), self._dev(Udot), float(gamma_dot),
+                                                  float(dt), int(nsteps)))
+        return U, Udot
+
+    def mse_tangent(self, U, Udot, Utarget):
+        """(mean((U - Utarget)^2), its derivative along Udot), Eq. 14."""
+        loss, dloss = C.c_double(), C.c_double()
+        self._chk(lib().jxs_mse_tangent(self._h, self._dev(U), self._dev(Udot), self._dev(Utarget),
+                                        C.byref(loss), C.byref(dloss)))
+        return loss.value, dloss.value
 
     def step_host(self, U, cfl, nsteps):
         """In place on the host tensor U (copies inside the call)."""
