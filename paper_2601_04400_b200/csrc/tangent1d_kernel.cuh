@@ -69,27 +69,27 @@ __device__ __forceinline__ void weno5_dual(Dual a, Dual b, Dual c, Dual d, Dual 
   const Dual s0 = a - 2.0 * b + c, t0 = a - 4.0 * b + 3.0 * c;
   const Dual s1 = b - 2.0 * c + d, t1 = b - d;
   const Dual s2 = c - 2.0 * d + e, t2 = 3.0 * c - 4.0 * d + e;
-  const double c1312 = 13.0 / 12.0;
-  const Dual b0 = c1312 * (s0 * s0) + 0.25 * (t0 * t0);
-  const Dual b1 = c1312 * (s1 * s1) + 0.25 * (t1 * t1);
-  const Dual b2 = c1312 * (s2 * s2) + 0.25 * (t2 * t2);
-  const Dual r0 = rcp_dual(b0 + 1e-6), r1 = rcp_dual(b1 + 1e-6), r2 = rcp_dual(b2 + 1e-6);
-  const Dual w0 = r0 * r0, w1 = r1 * r1, w2 = r2 * r2;
-  const double sixth = 1.0 / 6.0;
-  {  // left-biased at i+1/2
-    const Dual q0 = sixth * (2.0 * a - 7.0 * b + 11.0 * c);
-    const Dual q1 = sixth * (5.0 * c - b + 2.0 * d);
-    const Dual q2 = sixth * (2.0 * c + 5.0 * d - e);
-    const Dual a0 = 0.1 * w0, a1 = 0.6 * w1, a2 = 0.3 * w2;
-    Lp = (a0 * q0 + a1 * q1 + a2 * q2) / (a0 + a1 + a2);
-  }
-  {  // right-biased at i-1/2: the same formula on (e, d, c, b, a)
-    const Dual q0 = sixth * (2.0 * e - 7.0 * d + 11.0 * c);
-    const Dual q1 = sixth * (5.0 * c - d + 2.0 * b);
-    const Dual q2 = sixth * (2.0 * c + 5.0 * b - a);
-    const Dual a0 = 0.1 * w2, a1 = 0.6 * w1, a2 = 0.3 * w0;
-    Rm = (a0 * q0 + a1 * q1 + a2 * q2) / (a0 + a1 + a2);
-  }
+  // (eps + beta)^2 with beta = 13/12 s^2 + 1/4 t^2, its derivative 2 (13/12 s s' + 1/4 t t') written out
+  auto eps_beta_sq = [](Dual s, Dual t) {
+    const double ms = (13.0 / 12.0) * s.v, mt = 0.25 * t.v;
+    const double x = fma(mt, t.v, fma(ms, s.v, 1e-6));
+    const double xd = 2.0 * fma(ms, s.d, mt * t.d);
+    return Dual{x * x, (x + x) * xd};
+  };
+  const Dual e0 = eps_beta_sq(s0, t0), e1 = eps_beta_sq(s1, t1), e2 = eps_beta_sq(s2, t2);
+  // alpha_k = d_k / (eps + beta_k)^2 over their sum, with the common denominator multiplied through (one division
+  // per side instead of four); the 1/6 of the candidate values is folded into the linear weights
+  const Dual w0 = e1 * e2, w1 = e0 * e2, w2 = e0 * e1;
+  auto blend = [](Dual wa, Dual wb, Dual wc, Dual qa, Dual qb, Dual qc) {  // weights 0.1, 0.6, 0.3 on (wa, wb, wc)
+    const Dual na = wa * qa, nb = wb * qb, nc = wc * qc;
+    const Dual N{fma(0.1 / 6.0, na.v, fma(0.6 / 6.0, nb.v, (0.3 / 6.0) * nc.v)),
+                 fma(0.1 / 6.0, na.d, fma(0.6 / 6.0, nb.d, (0.3 / 6.0) * nc.d))};
+    const Dual D{fma(0.1, wa.v, fma(0.6, wb.v, 0.3 * wc.v)), fma(0.1, wa.d, fma(0.6, wb.d, 0.3 * wc.d))};
+    return N / D;
+  };
+  // left-biased at i+1/2, and right-biased at i-1/2 = the same formula on (e, d, c, b, a)
+  Lp = blend(w0, w1, w2, 2.0 * a - 7.0 * b + 11.0 * c, 5.0 * c - b + 2.0 * d, 2.0 * c + 5.0 * d - e);
+  Rm = blend(w2, w1, w0, 2.0 * e - 7.0 * d + 11.0 * c, 5.0 * c - d + 2.0 * b, 2.0 * c + 5.0 * b - a);
 }
 
 // one side K of the HLLC flux (Eq. 3-4, R1): F_K + s_K^clip (U*_K - U_K) with
