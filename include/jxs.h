@@ -142,6 +142,24 @@ int jxs_step_fixed_dt_tangent(jxs_solver*, void* U, void* Udot, double gamma_dot
  * reproducible.  Errors: JXS_EINVAL for NULL pointers or an fp32 handle.  Synchronises the stream.               */
 int jxs_mse_tangent(jxs_solver*, const void* U, const void* Udot, const void* Utarget, double* loss, double* dloss);
 
+/* Reverse mode (adjoint) of jxs_step_fixed_dt for one-dimensional Euler problems: Eq. 15-16 —
+ * "backpropagation through the full sequence of unrolled solver steps" (R21, R24).
+ * Two calls: the forward sweep that records the trajectory, then the reverse sweep.
+ *
+ * jxs_step_fixed_dt_record: as jxs_step_fixed_dt (U: DEVICE pointer, [4][1][nx] doubles, advanced in place by nsteps
+ * >= 1 SSP-RK3 steps of size dt > 0), keeping the 3 stage states of every step in device memory owned by the handle
+ * (96 nx bytes per step; released by the next record call or jxs_destroy).
+ * jxs_adjoint_steps: Ubar (DEVICE pointer, [4][1][nx] doubles) holds on entry the adjoint of the final state, e.g.
+ * dL/dU^{n+m} of the loss of Eq. 14; on return the adjoint of the initial state, (dU^{n+m}/dU^n)^T Ubar.
+ * *gamma_bar (HOST) = <dU^{n+m}/dgamma at fixed initial conserved state, Ubar>.  For every direction (Udot, gamma_dot)
+ * <Ubar_in, tangent(Udot, gamma_dot)> = <Ubar_out, Udot> + gamma_bar gamma_dot with jxs_step_fixed_dt_tangent.
+ * May be called repeatedly on one recording.  Branches of the scheme carry the derivative of the branch taken.
+ * Errors: JXS_EINVAL for NULL pointers, dt <= 0, nsteps < 1, an fp32 handle or ny != 1; JXS_ESTATE with mu > 0 or
+ * nu > 0, a network, the forward-Euler integrator, steps pending, or (adjoint) nothing recorded; JXS_ENOMEM when the
+ * trajectory does not fit.  Both synchronise the stream.                                                          */
+int jxs_step_fixed_dt_record(jxs_solver*, void* U, double dt, int nsteps);
+int jxs_adjoint_steps(jxs_solver*, void* Ubar, double* gamma_bar);
+
 /* Same two calls on HOST buffers (pageable or pinned): host->device copy, stepping,
  * device->host copy; used for end-to-end timing.                                            */
 int jxs_step_host(jxs_solver*, void* U_host, double cfl, int nsteps);

@@ -241,6 +241,26 @@ class Oracle:
                                                   float(dt), int(nsteps)))
         return U, Udot
 
+    def step_fixed_dt_adjoint(self, U, Ubar, dt, nsteps, planar=False):
+        """O13: the adjoint of nsteps fixed-dt steps, from the definition of a transpose (Eq. 16 read from
+        the left): entry j of J^T Ubar is <Ubar, J e_j>, with J e_j from the tangent O12 -- one tangent run per
+        entry of the state (small cases only), and gamma_bar = <Ubar, dS/dgamma>.
+        planar: U is a field of identical rows standing for a 1D problem; the directions e_j are repeated over the
+        rows and Ubar (one row, [4][1][nx]) is paired with row 0: the 1D adjoint.  Returns (Ubar_in, gamma_bar)."""
+        U = np.ascontiguousarray(self._field(U), dtype=np.float64)
+        Ubar = np.asarray(Ubar, dtype=np.float64)
+        shape = (4, 1, self.nx) if planar else U.shape
+        assert Ubar.shape == shape
+        out = np.zeros(shape)
+        pick = (lambda D: D[:, :1]) if planar else (lambda D: D)
+        for j in range(out.size):
+            e = np.zeros(shape)
+            e.flat[j] = 1.0
+            _, D = self.step_fixed_dt_tangent(U, np.repeat(e, self.ny, axis=1) if planar else e, 0.0, dt, nsteps)
+            out.flat[j] = float(np.sum(Ubar * pick(D)))
+        _, D = self.step_fixed_dt_tangent(U, np.zeros_like(U), 1.0, dt, nsteps)
+        return out, float(np.sum(Ubar * pick(D)))
+
     def time(self):
         t, dt = C.c_double(), C.c_double()
         self._chk(lib().jxo_get_time(self._h, C.byref(t), C.byref(dt)))

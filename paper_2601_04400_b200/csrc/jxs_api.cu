@@ -21,6 +21,7 @@
 #include "stage_kernel.cuh"
 #include "stage1d_kernel.cuh"
 #include "tangent1d_kernel.cuh"
+#include "adjoint1d_kernel.cuh"
 
 using namespace jxs;
 
@@ -49,6 +50,13 @@ struct jxs_solver {
   // jxs_step_fixed_dt_tangent call; d_mse = partial sums and result of jxs_mse_tangent
   void* bufd[3] = {nullptr, nullptr, nullptr};
   double* d_mse = nullptr;
+  // recorded trajectory and adjoint buffers of the one-dimensional reverse sweep (adjoint1d_kernel.cuh), compact
+  // layout [4][pitch] per state: tape = the 3 stage inputs of every recorded step + the final state
+  double* tape = nullptr;
+  int tape_steps = 0;
+  double tape_dt = 0;
+  double* adj = nullptr;  // 4 adjoint states, then the gamma_bar partial sums, then gamma_bar
+  int adj_parts = 0;
   // TMA descriptors of the three padded buffers: boxes [4][1][CW] (stencil rows) and [4][1][Epi::W] (RK operand rows)
   CUtensorMap tm_row[3], tm_epi[3];
   // immersed boundary
@@ -783,6 +791,135 @@ int tangent_common(jxs_solver* s, void* U, void* Udot, double gamma_dot, double 
   return finish_steps(s, nsteps);
 }
 
+// ---- reverse mode of the one-dimensional Euler step (adjoint1d_kernel.cuh)
+// The tape and the adjoint states hold only the one interior row of the padded layout ([4][pitch] per state).  The
+// kernels address row 3 of a [4][7][pitch] buffer, so they are handed a pointer 3 rows before the compact state and a
+// plane stride of one row; they never touch another row when ny = 1.
+struct CompactLayout {
+  jxs_solver* s;
+  long long plane;
+  explicit CompactLayout(jxs_solver* s_) : s(s_), plane(s_->plane) { s->plane = s->pitch; }
+  ~CompactLayout() { s->plane = plane; }
+};
+double* compact_state(const jxs_solver* s, double* base, long long i) {
+  return base + i * 4 * (long long)s->pitch - 3 * (long long)s->pitch;
+}
+
+int adjoint_checks(jxs_solver* s) {
+  if (s->dtype != JXS_F64) return fail(s, JXS_EINVAL, "the adjoint is fp64 only");
+  if (s->ny != 1) return fail(s, JXS_EINVAL, "the adjoint is built for one-dimensional problems (ny = 1)");
+  if (s->mu > 0 || s->nu > 0) return fail(s, JXS_ESTATE, "the adjoint is built for the Euler equations (mu = 0, nu = 0)");
+  if (s->mlp_on || s->cnn_on) return fail(s, JXS_ESTATE, "the adjoint does not differentiate the networks");
+  if (s->scheme != JXS_SSPRK3) return fail(s, JXS_ESTATE, "the adjoint steps with SSP-RK3");
+  if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
+  return JXS_OK;
+}
+
+int record_common(jxs_solver* s, void* U, double dt, int nsteps) {
+  if (!s) return JXS_EINVAL;
+  if (!U) return fail(s, JXS_EINVAL, "U is NULL");
+  if (nsteps < 1) return fail(s, JXS_EINVAL, "nsteps < 1");
+  if (!(dt > 0)) return fail(s, JXS_EINVAL, "dt must be > 0");
+  int rc = adjoint_checks(s);
+  if (rc != JXS_OK) return rc;
+  cudaFree(s->tape);
+  s->tape = nullptr;
+  s->tape_steps = 0;
+  const size_t state = (size_t)4 * s->pitch * sizeof(double);
+  const size_t bytes = state * (3 * (size_t)nsteps + 1);
+  CU(cudaMalloc(&s->tape, bytes));
+  CU(cudaMemsetAsync(s->tape, 0, bytes, s->stream));
+  CompactLayout compact(s);
+  auto T = [&](long long i) { return (void*)compact_state(s, s->tape, i); };
+  CU(pad(s, U, T(0)));
+  s->events_used = 0;
+  s->mlp_events_used = 0;
+  for (long long n = 0; n < nsteps; ++n) {
+    prepare_step_kernel<<<1, 1, 0, s->stream>>>(s->d_state, 0, 0.0, dt);
+    s->launches++;
+    CU(cudaGetLastError());
+    CU(ghost_fill(s, T(3 * n)));
+    CU(stage(s, T(3 * n), nullptr, T(3 * n + 1), 0, 0.0, 1.0, nullptr));
+    CU(ghost_fill(s, T(3 * n + 1)));
+    CU(stage(s, T(3 * n + 1), T(3 * n), T(3 * n + 2), 0, 0.75, 0.25, nullptr));
+    CU(ghost_fill(s, T(3 * n + 2)));
+    CU(stage(s, T(3 * n + 2), T(3 * n), T(3 * n + 3), 0, 1.0 / 3.0, 2.0 / 3.0, nullptr));
+  }
+  CU(unpad(s, T(3LL * nsteps), U));
+  rc = finish_steps(s, nsteps);
+  if (rc != JXS_OK) return rc;
+  s->tape_steps = nsteps;
+  s->tape_dt = dt;
+  return JXS_OK;
+}
+
+cudaError_t adjoint_stage(jxs_solver* s, const double* U, const double* out, double* in, double b, const double* E1,
+                          double e1, const double* E2, double e2) {
+  Adjoint1dArgs A;
+  A.U = U + 3 * (long long)s->pitch; A.Ubar_out = out + 3 * (long long)s->pitch; A.Ubar_in = in + 3 * (long long)s->pitch;
+  A.E1 = E1 ? E1 + 3 * (long long)s->pitch : nullptr; A.E2 = E2 ? E2 + 3 * (long long)s->pitch : nullptr;
+  double* partial = s->adj + 4LL * 4 * s->pitch;
+  A.gbar_partial = partial;
+  A.dt = s->tape_dt; A.plane = s->pitch; A.nx = s->nx; A.pitch = s->pitch;
+  A.gamma = s->gamma; A.dxi = 1.0 / s->dx; A.b = b; A.e1 = e1; A.e2 = e2;
+  cudaEvent_t e0 = nullptr, e1v = nullptr;
+  if (s->profiling && s->events_used + 2 <= (int)s->events.size()) {
+    e0 = s->events[s->events_used++];
+    e1v = s->events[s->events_used++];
+    cudaEventRecord(e0, s->stream);
+  }
+  adjoint1d_kernel<<<s->adj_parts, A1D_TB, 0, s->stream>>>(A);
+  if (e1v) cudaEventRecord(e1v, s->stream);
+  adjoint1d_fold_kernel<<<1, 256, 0, s->stream>>>(A.Ubar_in, s->pitch, s->nx, s->bc.xlo, s->bc.xhi, s->bc.inflow[3],
+                                                   s->gamma, partial, s->adj_parts, partial + s->adj_parts);
+  s->launches += 2;
+  return cudaGetLastError();
+}
+
+int adjoint_common(jxs_solver* s, void* Ubar, double* gamma_bar) {
+  if (!s) return JXS_EINVAL;
+  if (!Ubar || !gamma_bar) return fail(s, JXS_EINVAL, "NULL argument");
+  int rc = adjoint_checks(s);
+  if (rc != JXS_OK) return rc;
+  if (!s->tape || s->tape_steps < 1) return fail(s, JXS_ESTATE, "no recorded steps: call jxs_step_fixed_dt_record first");
+  const int parts = (s->nx + 6 + A1D_OUT - 1) / A1D_OUT;
+  const size_t state = (size_t)4 * s->pitch;
+  if (!s->adj || s->adj_parts != parts) {
+    cudaFree(s->adj);
+    s->adj = nullptr;
+    CU(cudaMalloc(&s->adj, (4 * state + parts + 1) * sizeof(double)));
+    s->adj_parts = parts;
+  }
+  CU(cudaMemsetAsync(s->adj, 0, (4 * state + parts + 1) * sizeof(double), s->stream));
+  CompactLayout compact(s);
+  auto T = [&](long long i) { return compact_state(s, s->tape, i); };
+  auto B = [&](int i) { return compact_state(s, s->adj, i); };
+  CU(pad(s, Ubar, B(0)));
+  s->events_used = 0;
+  int x = 0;  // which adjoint state holds the adjoint of U^{n+1}
+  for (long long n = s->tape_steps - 1; n >= 0; --n) {
+    const int y2 = (x + 1) & 3, y1 = (x + 2) & 3, y0 = (x + 3) & 3;
+    // U^{n+1} = 1/3 U0 + 2/3 (U2 + dt L(U2));  U2 = 3/4 U0 + 1/4 (U1 + dt L(U1));  U1 = U0 + dt L(U0)   (R5)
+    CU(adjoint_stage(s, T(3 * n + 2), B(x), B(y2), 2.0 / 3.0, nullptr, 0.0, nullptr, 0.0));
+    CU(adjoint_stage(s, T(3 * n + 1), B(y2), B(y1), 0.25, nullptr, 0.0, nullptr, 0.0));
+    CU(adjoint_stage(s, T(3 * n), B(y1), B(y0), 1.0, B(x), 1.0 / 3.0, B(y2), 0.75));
+    x = y0;
+  }
+  CU(unpad(s, B(x), Ubar));
+  CU(cudaMemcpyAsync(gamma_bar, s->adj + 4 * state + parts, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+  CU(cudaStreamSynchronize(s->stream));
+  if (s->profiling) {
+    s->stage_ms = 0;
+    s->stage_launches = s->events_used / 2;
+    for (int i = 0; i + 1 < s->events_used; i += 2) {
+      float ms = 0;
+      cudaEventElapsedTime(&ms, s->events[i], s->events[i + 1]);
+      s->stage_ms += ms;
+    }
+  }
+  return JXS_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -858,6 +995,8 @@ void jxs_destroy(jxs_solver* s) {
   cudaFree(s->stage_io);
   for (int b = 0; b < 3; ++b) cudaFree(s->bufd[b]);
   cudaFree(s->d_mse);
+  cudaFree(s->tape);
+  cudaFree(s->adj);
   cudaFree(s->d_state);
   free_ibm(s);
   cudaFree(s->d_mlp_blob); cudaFree(s->d_dF); cudaFree(s->d_dG);
@@ -1107,6 +1246,9 @@ int jxs_step_fixed_dt(jxs_solver* s, void* U, double dt, int nsteps) {
 int jxs_step_fixed_dt_tangent(jxs_solver* s, void* U, void* Udot, double gamma_dot, double dt, int nsteps) {
   return tangent_common(s, U, Udot, gamma_dot, dt, nsteps);
 }
+
+int jxs_step_fixed_dt_record(jxs_solver* s, void* U, double dt, int nsteps) { return record_common(s, U, dt, nsteps); }
+int jxs_adjoint_steps(jxs_solver* s, void* Ubar, double* gamma_bar) { return adjoint_common(s, Ubar, gamma_bar); }
 
 int jxs_mse_tangent(jxs_solver* s, const void* U, const void* Udot, const void* Utarget, double* loss, double* dloss) {
   if (!s) return JXS_EINVAL;

@@ -257,6 +257,30 @@ def test_gamma_inference_recovers_the_value_behind_the_data():
     assert dloss == pytest.approx((lp[0] - lp[1]) / (2 * h), rel=1e-5)
 
 
+def test_adjoint_is_the_gradient_of_a_linear_functional():
+    # O13 against central differences of the primal oracle: phi(U0, gamma) = <c, S^n(U0; gamma)> has gradient
+    # (J^T c, <c, dS/dgamma>); sampled entries of U0
+    case = wl.vortex(8)
+    dt, ns = 0.05, 2
+    rng = np.random.default_rng(8)
+    c = rng.normal(size=case["U0"].shape)
+    grad, gbar = make(case).step_fixed_dt_adjoint(case["U0"], c, dt, ns)
+    h = 1e-7  # a one-cell perturbation: the WENO weights (eps = 1e-6) have large third derivatives
+    for j in rng.choice(c.size, 12, replace=False):
+        e = np.zeros(c.shape)
+        e.flat[j] = 1.0
+        fd = np.sum(c * central_difference(case, e, 0.0, dt, ns, h))
+        assert grad.flat[j] == pytest.approx(fd, rel=2e-6, abs=1e-8)
+    assert gbar == pytest.approx(np.sum(c * central_difference(case, 0 * c, 1.0, dt, ns, 1e-6)), rel=1e-6)
+    # planar form = the 1D adjoint: its pairing with any 1D direction equals the tangent's pairing with c
+    case = sod_rows(24)
+    c1 = rng.normal(size=(4, 1, 24))
+    d1 = rng.normal(size=(4, 1, 24))
+    g1, gb1 = make(case).step_fixed_dt_adjoint(case["U0"], c1, 0.2 * case["dx"], 2, planar=True)
+    _, D = make(case).step_fixed_dt_tangent(case["U0"], np.repeat(d1, 8, axis=1), 0.7, 0.2 * case["dx"], 2)
+    assert np.sum(c1 * D[:, :1]) == pytest.approx(np.sum(g1 * d1) + 0.7 * gb1, rel=1e-12)
+
+
 def test_tangent_argument_checks():
     case = wl.vortex(8)
     o = make(case, dtype=np.float32)
