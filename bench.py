@@ -245,6 +245,69 @@ def run_tangent1d(args, rank, world, local_rank, dist, barrier, tdt):
         "e2e": None, "cpu_baseline": None}))
 
 
+def run_adjoint1d(args, rank, world, local_rank, dist, barrier, tdt):
+    """SURVEY.md section 8(f) rank 3 (reverse mode): one iteration of the gamma inference by backpropagation
+     on the 1D Sod tube at 3e6 cells: K recorded steps, dL/dU of Eq. 14, K adjoint steps."""
+    import torch
+    from paper_2601_04400_b200 import jxs, workloads as wl
+    if args.dtype != "f64":
+        raise SystemExit("bench.py: the adjoint is fp64 only")
+    nx = 3_000_000
+    case = wl.sod1d(nx, gamma=1.3)
+    dt = 0.2 * case["dx"]
+    stream = torch.cuda.current_stream()
+    solver = jxs.Solver.from_case(case, dtype=tdt, stream=stream)
+    U0 = torch.tensor(case["U0"], dtype=tdt, device="cuda")
+    seed = torch.tensor(wl.dcons_dgamma(case["U0"], case["gamma"]), dtype=tdt, device="cuda")
+    target = torch.tensor(wl.sod1d(nx)["U0"], dtype=tdt, device="cuda")
+    K, W = args.steps, args.warmup
+
+    def iteration(n):
+        U = U0.clone()
+        solver.step_fixed_dt_record(U, dt, n)
+        B = (U - target).mul_(2.0 / U.numel())         # dL/dU of Eq. 14
+        gbar = solver.adjoint_steps(B)
+        return gbar + float((B * seed).sum())           # dL/dgamma at fixed primitives (R23)
+
+    iteration(W)
+    solver.set_profiling(True)
+    sampler = ClockSampler(local_rank)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = solver.launch_count()
+    barrier()
+    sampler.start()
+    e0.record(stream)
+    dloss = iteration(K)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = max_over_ranks(e0.elapsed_time(e1), dist, "cuda")
+    stage_ms, stage_n = solver.stage_time()            # the adjoint kernel's launches of the reverse sweep
+    if not math.isfinite(dloss):
+        raise SystemExit("bench.py: non-finite gradient after the timed region")
+    if rank != 0:
+        return
+    # adjoint of the 1D Euler stage: the stage's values recomputed (471 flop) + the reverse sweep (581) + the combine
+    # (16), DESIGN.md section 6; bytes: state, adjoint in, adjoint out (+ two more adjoints in the first stage)
+    flop, nbytes = 1068.0, (96.0 + 96.0 + 160.0) / 3.0
+    avg = stage_ms / max(stage_n, 1)
+    achieved = flop * nx / (avg * 1e-3) / 1e12
+    print(json.dumps({
+        "metric": METRIC, "value": aggregate_rate(nx, K, world, ms), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
+        "data": "synthetic",
+        "config": {"workload": "adjoint1d_3000000 (1D Sod tube: K recorded steps, dL/dU of Eq. 14, K adjoint steps; one "
+                               "cell-stage = forward + reverse; PAPER.md L115-128, L149)", "dt": dt, "rk": "SSP-RK3",
+                   "cells": nx, "l2": "the recorded trajectory (288 MB per step) streams through HBM, no flush needed",
+                   "dloss_dgamma": dloss, "parallelism": "replicas" if world > 1 else "single GPU"},
+        "clocks": clocks, "gpu_launches": solver.launch_count() - launches0,
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_FP64_TFLOPS, "unit": "TFLOP/s",
+                     "frac": achieved / PEAK_FP64_TFLOPS, "traffic": None, "kernel": "jxs::adjoint1d_kernel",
+                     "avg_launch_ms": avg, "launches_timed": stage_n, "alg_flop_per_cell_stage": flop,
+                     "alg_bytes_per_cell_stage": nbytes, "hbm_side_gbs": nbytes * nx / (avg * 1e-3) / 1e9},
+        "e2e": None, "cpu_baseline": None}))
+
+
 def run_cnn(args, rank, world, local_rank, dist, barrier, tdt):
     """the C4 grid with the paper's 2D CNN neural flux (Eq. 11-13) in
     every stage: reconstruction pass + 3 convolution layers per direction on tcgen05, then the stage kernel."""
@@ -393,7 +456,7 @@ def main():
     ap.add_argument("--euler", action="store_true", help="mu = 0, no IBM (not the headline config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile-kernels", action="store_true", help="c5 only: per-kernel CUDA-event spans")
-    ap.add_argument("--workload", choices=("c4", "c5", "sod1d", "cnn", "tangent1d"), default="c4",
+    ap.add_argument("--workload", choices=("c4", "c5", "sod1d", "cnn", "tangent1d", "adjoint1d"), default="c4",
                     help="c4 = the headline throughput case (default); c5 = BASELINE.json configs[4]: 16 independent "
                          "1024x512 shock-cylinder runs with the per-face flux MLP, one stream per handle; sod1d = the "
                          "paper's 1D Sod tube at its largest size (3e6 cells = 9e6 degrees of freedom, PAPER.md L149)")
@@ -430,6 +493,9 @@ def main():
         return
     if args.workload == "sod1d":
         run_sod1d(args, rank, world, local_rank, dist, barrier, tdt)
+        return
+    if args.workload == "adjoint1d":
+        run_adjoint1d(args, rank, world, local_rank, dist, barrier, tdt)
         return
     if args.workload == "tangent1d":
         run_tangent1d(args, rank, world, local_rank, dist, barrier, tdt)

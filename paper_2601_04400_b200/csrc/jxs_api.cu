@@ -828,7 +828,10 @@ int record_common(jxs_solver* s, void* U, double dt, int nsteps) {
   const size_t state = (size_t)4 * s->pitch * sizeof(double);
   const size_t bytes = state * (3 * (size_t)nsteps + 1);
   CU(cudaMalloc(&s->tape, bytes));
-  CU(cudaMemsetAsync(s->tape, 0, bytes, s->stream));
+  // the columns past the padded row are never written; the kernels' clamped support reads must find numbers there
+  if (s->pitch > s->nx + 6)
+    CU(cudaMemset2DAsync(s->tape + s->nx + 6, (size_t)s->pitch * sizeof(double), 0,
+                         (size_t)(s->pitch - s->nx - 6) * sizeof(double), 4 * (3 * (size_t)nsteps + 1), s->stream));
   CompactLayout compact(s);
   auto T = [&](long long i) { return (void*)compact_state(s, s->tape, i); };
   CU(pad(s, U, T(0)));
