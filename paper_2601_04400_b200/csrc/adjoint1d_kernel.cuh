@@ -324,19 +324,21 @@ __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A
 // (transposed ghost fill: periodic / transmissive copy, reflective copy with the normal momentum negated; an inflow
 // ghost is a constant of U whose energy p/(gamma-1) + ... moves with gamma), (2) gamma_bar += the launch's partial
 // sums, in a fixed order.  One CTA.
-__global__ void __launch_bounds__(256) adjoint1d_fold_kernel(double* Ubar, long long plane, int nx, int xlo, int xhi,
-                                                             double p_inflow, double gamma, const double* partial,
-                                                             int nparts, double* gamma_bar) {
-  __shared__ double red[8];
+constexpr int A1D_FOLD_TB = 1024;
+__global__ void __launch_bounds__(A1D_FOLD_TB) adjoint1d_fold_kernel(double* Ubar, long long plane, int nx, int xlo,
+                                                                     int xhi, double p_inflow, double gamma,
+                                                                     const double* partial, int nparts,
+                                                                     double* gamma_bar) {
+  __shared__ double red[A1D_FOLD_TB / 32];
   double a = 0.0;
-  for (int i = threadIdx.x; i < nparts; i += 256) a += partial[i];
+  for (int i = threadIdx.x; i < nparts; i += A1D_FOLD_TB) a += partial[i];
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
   if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = a;
   __syncthreads();
   if (threadIdx.x == 0) {
     double gb = 0.0;
-    for (int w = 0; w < 8; ++w) gb += red[w];
+    for (int w = 0; w < A1D_FOLD_TB / 32; ++w) gb += red[w];
     const double g1 = gamma - 1.0;
     for (int c = 0; c < 6; ++c) {
       const int i = c < 3 ? c - 3 : nx + (c - 3);  // interior index of the ghost cell

@@ -873,7 +873,7 @@ cudaError_t adjoint_stage(jxs_solver* s, const double* U, const double* out, dou
   }
   adjoint1d_kernel<<<s->adj_parts, A1D_TB, 0, s->stream>>>(A);
   if (e1v) cudaEventRecord(e1v, s->stream);
-  adjoint1d_fold_kernel<<<1, 256, 0, s->stream>>>(A.Ubar_in, s->pitch, s->nx, s->bc.xlo, s->bc.xhi, s->bc.inflow[3],
+  adjoint1d_fold_kernel<<<1, A1D_FOLD_TB, 0, s->stream>>>(A.Ubar_in, s->pitch, s->nx, s->bc.xlo, s->bc.xhi, s->bc.inflow[3],
                                                    s->gamma, partial, s->adj_parts, partial + s->adj_parts);
   s->launches += 2;
   return cudaGetLastError();
