@@ -285,6 +285,15 @@ __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A
 #pragma unroll
     for (int j = 0; j < 5; ++j) con[k][j][t] = g[j];
   }
+  // the U0 terms of the Shu-Osher combine: requested before the barrier, used after the gather
+  double Ex[4] = {0.0, 0.0, 0.0, 0.0};
+  if (interior && mine) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      if (A.E1) Ex[k] = A.e1 * A.E1[k * A.plane + pc];
+      if (A.E2) Ex[k] = fma(A.e2, A.E2[k * A.plane + pc], Ex[k]);
+    }
+  }
   __syncthreads();
 
   // ---- gather, reverse S3 (primitives -> conserved), S8
@@ -304,11 +313,7 @@ __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       double x = out[k];
-      if (interior) {
-        x = fma(A.b, Ub[k], x);
-        if (A.E1) x = fma(A.e1, A.E1[k * A.plane + pc], x);
-        if (A.E2) x = fma(A.e2, A.E2[k * A.plane + pc], x);
-      }
+      if (interior) x = fma(A.b, Ub[k], x) + Ex[k];
       A.Ubar_in[k * A.plane + pc] = x;
     }
   }

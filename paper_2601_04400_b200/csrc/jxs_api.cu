@@ -54,6 +54,7 @@ struct jxs_solver {
   // layout [4][pitch] per state: tape = the 3 stage inputs of every recorded step + the final state
   double* tape = nullptr;
   int tape_steps = 0;
+  size_t tape_bytes = 0;
   double tape_dt = 0;
   double* adj = nullptr;  // 4 adjoint states, then the gamma_bar partial sums, then gamma_bar
   int adj_parts = 0;
@@ -822,12 +823,16 @@ int record_common(jxs_solver* s, void* U, double dt, int nsteps) {
   if (!(dt > 0)) return fail(s, JXS_EINVAL, "dt must be > 0");
   int rc = adjoint_checks(s);
   if (rc != JXS_OK) return rc;
-  cudaFree(s->tape);
-  s->tape = nullptr;
   s->tape_steps = 0;
   const size_t state = (size_t)4 * s->pitch * sizeof(double);
   const size_t bytes = state * (3 * (size_t)nsteps + 1);
-  CU(cudaMalloc(&s->tape, bytes));
+  if (!s->tape || s->tape_bytes < bytes) {  // the tape is kept between calls and only ever grows
+    cudaFree(s->tape);
+    s->tape = nullptr;
+    s->tape_bytes = 0;
+    CU(cudaMalloc(&s->tape, bytes));
+    s->tape_bytes = bytes;
+  }
   // the columns past the padded row are never written; the kernels' clamped support reads must find numbers there
   if (s->pitch > s->nx + 6)
     CU(cudaMemset2DAsync(s->tape + s->nx + 6, (size_t)s->pitch * sizeof(double), 0,

@@ -102,6 +102,31 @@ def sod1d(nx=500, gamma=GAMMA):
                 mu=0.0, Pr=0.72, bc=bc, phi=None)
 
 
+def wavy1d(nx, gamma=GAMMA):
+    """A 1D field for parity checks at large nx on sampled windows: the Sod jump at mid-tube carrying short waves
+    (37 to 91 cells long) in every primitive, so that every window of a few dozen cells sees a different, varying
+    state.  Deterministic; transmissive ends."""
+    case = sod1d(nx, gamma)
+    i = np.arange(nx, dtype=np.float64)
+    left = i < nx // 2
+    rho = np.where(left, 1.0, 0.125) * (1.0 + 0.2 * np.sin(2 * math.pi * i / 37.0))
+    u = 0.4 * np.cos(2 * math.pi * i / 53.0)
+    v = 0.2 * np.sin(2 * math.pi * i / 91.0)
+    p = np.where(left, 1.0, 0.1) * (1.0 + 0.15 * np.cos(2 * math.pi * i / 71.0 + 0.3))
+    case["U0"] = cons_from_prim(rho[None, :], u[None, :], v[None, :], p[None, :], gamma)
+    case["name"] = f"wavy1d_{nx}"
+    return case
+
+
+def window(case, lo, hi):
+    """Cells [lo, hi) of a 1D case as a case of its own (transmissive ends)."""
+    c = dict(case)
+    c["U0"] = np.ascontiguousarray(case["U0"][:, :, lo:hi])
+    c["nx"] = hi - lo
+    c["name"] = case["name"] + f"[{lo}:{hi}]"
+    return c
+
+
 def as_rows(case, ny=8):
     """A 1D case repeated over ny identical rows, periodic in y: the planar 2D problem whose every row is the 1D one
     (identical rows make the y-fluxes cancel exactly).  This is how the 2D oracle checks the 1D path."""
