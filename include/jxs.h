@@ -142,7 +142,7 @@ int jxs_step_fixed_dt_tangent(jxs_solver*, void* U, void* Udot, double gamma_dot
  * reproducible.  Errors: JXS_EINVAL for NULL pointers or an fp32 handle.  Synchronises the stream.               */
 int jxs_mse_tangent(jxs_solver*, const void* U, const void* Udot, const void* Utarget, double* loss, double* dloss);
 
-/* Reverse mode (adjoint) of jxs_step_fixed_dt for one-dimensional Euler problems: Eq. 15-16 —
+/* Reverse mode (adjoint) of jxs_step_fixed_dt for one-dimensional problems (Euler or Navier-Stokes, nu-term): Eq. 15-16 —
  * "backpropagation through the full sequence of unrolled solver steps" (R21, R24).
  * Two calls: the forward sweep that records the trajectory, then the reverse sweep.
  *
@@ -154,8 +154,7 @@ int jxs_mse_tangent(jxs_solver*, const void* U, const void* Udot, const void* Ut
  * *gamma_bar (HOST) = <dU^{n+m}/dgamma at fixed initial conserved state, Ubar>.  For every direction (Udot, gamma_dot)
  * <Ubar_in, tangent(Udot, gamma_dot)> = <Ubar_out, Udot> + gamma_bar gamma_dot with jxs_step_fixed_dt_tangent.
  * May be called repeatedly on one recording.  Branches of the scheme carry the derivative of the branch taken.
- * Errors: JXS_EINVAL for NULL pointers, dt <= 0, nsteps < 1, an fp32 handle or ny != 1; JXS_ESTATE with mu > 0 or
- * nu > 0, a network, the forward-Euler integrator, steps pending, or (adjoint) nothing recorded; JXS_ENOMEM when the
+ * Errors: JXS_EINVAL for NULL pointers, dt <= 0, nsteps < 1, an fp32 handle or ny != 1; JXS_ESTATE with a network, the forward-Euler integrator, steps pending, or (adjoint) nothing recorded; JXS_ENOMEM when the
  * trajectory does not fit.  Both synchronise the stream.                                                          */
 int jxs_step_fixed_dt_record(jxs_solver*, void* U, double dt, int nsteps);
 int jxs_adjoint_steps(jxs_solver*, void* Ubar, double* gamma_bar);

@@ -12,7 +12,8 @@
 // copy them from by adjoint1d_fold_kernel), 128-thread CTAs that produce 122 cells: a cell's adjoint collects
 // contributions from the reconstructions of cells c-2 .. c+2, which need the flux adjoints of faces c-3+1/2 .. c+2+1/2.
 // Scatter is turned into gather through shared memory: no atomics, fixed summation order.
-// Euler only (mu = 0, nu = 0), fp64.
+// With mu > 0 the viscous flux of the 1D stage (R8, kappa depends on gamma) and with nu > 0 the nu Lap_h(U) term
+// are reversed as well.  fp64.
 #pragma once
 #include "aux_kernels.cuh"
 #include "stage_kernel.cuh"
@@ -33,6 +34,7 @@ struct Adjoint1dArgs {
   long long plane;         // pitch (compact layout)
   int nx, pitch;
   double gamma, dxi, b, e1, e2;
+  double mu, Pr, nu;       // viscous flux (R8) and the nu Lap_h(U) term of Eq. 10; 0 = absent
 };
 
 // WENO5-JS values of one variable at one cell (as weno5_dual in tangent1d_kernel.cuh, values only) and, given the
@@ -200,6 +202,7 @@ __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A
   __shared__ double LbS[4][A1D_TB];        // adjoint of L at each cell: b dt Ubar_out on interior cells, else 0
   __shared__ double rmB[4][A1D_TB + 1];    // adjoint of the right-biased state at each cell's left face
   __shared__ double con[4][5][A1D_TB];     // each cell's reconstruction adjoints for cells c-2 .. c+2
+  __shared__ double visN[4][A1D_TB + 1];   // viscous flux: adjoint of (rho, u, v, p) of the cell right of each face
   __shared__ double red[A1D_TB / 32];
   const int t = threadIdx.x;
   const int pc0 = A1D_OUT * blockIdx.x - 3;  // padded column of thread 0
@@ -227,7 +230,7 @@ __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A
   for (int k = 0; k < 4; ++k) LbS[k][t] = bdt * Ub[k];
   if (t == 0) {
 #pragma unroll
-    for (int k = 0; k < 4; ++k) rmB[k][0] = 0.0;
+    for (int k = 0; k < 4; ++k) { rmB[k][0] = 0.0; visN[k][0] = 0.0; }
   }
   __syncthreads();
 
@@ -257,19 +260,36 @@ __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A
   const bool face = pc >= 2 && pc <= A.nx + 2 && t < A1D_TB - 1;
   const bool mine = t >= 3 && t <= A1D_TB - 4 && pc <= last;  // the cells (and faces) this CTA accounts for
   double Lpb[4] = {0.0, 0.0, 0.0, 0.0}, gbar = 0.0;
+  double vo[4] = {0.0, 0.0, 0.0, 0.0};  // viscous flux of this face: adjoint of my cell's (rho, u, v, p)
   {
-    double Rnb[4] = {0.0, 0.0, 0.0, 0.0};
+    double Rnb[4] = {0.0, 0.0, 0.0, 0.0}, vn[4] = {0.0, 0.0, 0.0, 0.0};
     if (face) {
       double f[4], R[4];
 #pragma unroll
       for (int k = 0; k < 4; ++k) { f[k] = A.dxi * (LbS[k][t + 1] - LbS[k][t]); R[k] = rmS[k][t + 1]; }
-      const double gb = hllc_adjoint(Lp, R, A.gamma, f, Lpb, Rnb);
+      double gb = hllc_adjoint(Lp, R, A.gamma, f, Lpb, Rnb);
+      if (A.mu != 0.0) {
+        // F -= (0, txx, txy, ub txx + vb txy + kappa Tx), txx = 4/3 mu ux, txy = mu vx, T = p / rho (R8, 1D)
+        const int c = t + 2;
+        const double rc_ = prim[0][c], rn = prim[0][c + 1], rci = rcp_(rc_), rni = rcp_(rn);
+        const double Tc = prim[3][c] * rci, Tn = prim[3][c + 1] * rni;
+        const double kappa = A.mu / A.Pr * A.gamma * rcp_(g1);
+        const double ux = A.dxi * (prim[1][c + 1] - prim[1][c]), vx = A.dxi * (prim[2][c + 1] - prim[2][c]);
+        const double Tx = A.dxi * (Tn - Tc);
+        const double ub = 0.5 * (prim[1][c] + prim[1][c + 1]), vb = 0.5 * (prim[2][c] + prim[2][c + 1]);
+        const double txx = 4.0 / 3.0 * A.mu * ux, txy = A.mu * vx;
+        const double uxb = -(4.0 / 3.0 * A.mu) * (f[1] + f[3] * ub) * A.dxi, vxb = -A.mu * (f[2] + f[3] * vb) * A.dxi;
+        const double ubb = -0.5 * f[3] * txx, vbb = -0.5 * f[3] * txy, Txb = -f[3] * kappa * A.dxi;
+        vo[1] = ubb - uxb; vn[1] = ubb + uxb;
+        vo[2] = vbb - vxb; vn[2] = vbb + vxb;
+        vo[3] = -Txb * rci; vo[0] = Txb * Tc * rci;   // T = p / rho
+        vn[3] = Txb * rni; vn[0] = -Txb * Tn * rni;
+        gb += f[3] * Tx * (A.mu / A.Pr) * rcp_(g1 * g1);  // kappa = mu gamma / ((gamma-1) Pr)
+      }
       if (mine) gbar += gb;
     }
-    if (t < A1D_TB) {
 #pragma unroll
-      for (int k = 0; k < 4; ++k) rmB[k][t + 1] = Rnb[k];
-    }
+    for (int k = 0; k < 4; ++k) { rmB[k][t + 1] = Rnb[k]; visN[k][t + 1] = vn[k]; }
   }
   __syncthreads();
 
@@ -301,7 +321,8 @@ __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A
     double Wb[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k)
-      Wb[k] = con[k][0][t + 2] + con[k][1][t + 1] + con[k][2][t] + con[k][3][t - 1] + con[k][4][t - 2];
+      Wb[k] = con[k][0][t + 2] + con[k][1][t + 1] + con[k][2][t] + con[k][3][t - 1] + con[k][4][t - 2] +
+              (vo[k] + visN[k][t]);
     const double r = wc[0], u = wc[1], v = wc[2], p = wc[3], ri = rcp_(r);
     // u = ru / r, v = rv / r, p = g1 (E - (ru u + rv v) / 2)
     double out[4];
@@ -313,6 +334,8 @@ __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       double x = out[k];
+      if (A.nu != 0.0)  // L += nu Lap_h(U) (Eq. 10): the Laplacian is its own transpose
+        x = fma(A.nu * A.dxi * A.dxi, LbS[k][t - 1] - 2.0 * LbS[k][t] + LbS[k][t + 1], x);
       if (interior) x = fma(A.b, Ub[k], x) + Ex[k];
       A.Ubar_in[k * A.plane + pc] = x;
     }

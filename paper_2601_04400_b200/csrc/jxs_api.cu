@@ -809,7 +809,6 @@ double* compact_state(const jxs_solver* s, double* base, long long i) {
 int adjoint_checks(jxs_solver* s) {
   if (s->dtype != JXS_F64) return fail(s, JXS_EINVAL, "the adjoint is fp64 only");
   if (s->ny != 1) return fail(s, JXS_EINVAL, "the adjoint is built for one-dimensional problems (ny = 1)");
-  if (s->mu > 0 || s->nu > 0) return fail(s, JXS_ESTATE, "the adjoint is built for the Euler equations (mu = 0, nu = 0)");
   if (s->mlp_on || s->cnn_on) return fail(s, JXS_ESTATE, "the adjoint does not differentiate the networks");
   if (s->scheme != JXS_SSPRK3) return fail(s, JXS_ESTATE, "the adjoint steps with SSP-RK3");
   if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
@@ -870,6 +869,7 @@ cudaError_t adjoint_stage(jxs_solver* s, const double* U, const double* out, dou
   A.gbar_partial = partial;
   A.dt = s->tape_dt; A.plane = s->pitch; A.nx = s->nx; A.pitch = s->pitch;
   A.gamma = s->gamma; A.dxi = 1.0 / s->dx; A.b = b; A.e1 = e1; A.e2 = e2;
+  A.mu = s->mu; A.Pr = s->Pr; A.nu = s->nu;
   cudaEvent_t e0 = nullptr, e1v = nullptr;
   if (s->profiling && s->events_used + 2 <= (int)s->events.size()) {
     e0 = s->events[s->events_used++];

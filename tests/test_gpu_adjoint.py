@@ -1,4 +1,4 @@
-"""SURVEY.md section 8(f) rank 3, reverse mode: the adjoint of the one-dimensional Euler step (adjoint1d_kernel.cuh,
+"""SURVEY.md section 8(f) rank 3, reverse mode: the adjoint of the one-dimensional Euler / Navier-Stokes step (adjoint1d_kernel.cuh,
 jxs_step_fixed_dt_record / jxs_adjoint_steps) through the C ABI.  -m gpu.
 
 * element by element against the oracle's adjoint O13 (the transpose written out from its definition with the tangent
@@ -20,17 +20,24 @@ from test_gpu_tangent import PER, oracle_rows, smooth1d
 pytestmark = pytest.mark.gpu
 
 
-def gpu_adjoint(case, Ubar, dt, nsteps):
+def gpu_adjoint(case, Ubar, dt, nsteps, nu=0.0):
     s = jxs().Solver.from_case(case)
+    if nu:
+        s.set_artificial_viscosity(nu)
     U, B = dev(case["U0"]), dev(Ubar)
     s.step_fixed_dt_record(U, dt, nsteps)
     gbar = s.adjoint_steps(B)
     return U.cpu().numpy(), B.cpu().numpy(), gbar, s
 
 
-@pytest.mark.parametrize("name,nx,nsteps", [("sod", 60, 1), ("sod", 130, 2), ("smooth_periodic", 122, 2),
-                                            ("smooth_reflective", 123, 2), ("smooth_inflow", 70, 2)])
-def test_adjoint_matches_the_transposed_oracle_tangent(name, nx, nsteps):
+@pytest.mark.parametrize("name,nx,nsteps,mu,nu", [("sod", 60, 1, 0.0, 0.0), ("sod", 130, 2, 0.0, 0.0),
+                                                  ("smooth_periodic", 122, 2, 0.0, 0.0),
+                                                  ("smooth_reflective", 123, 2, 0.0, 0.0),
+                                                  ("smooth_inflow", 70, 2, 0.0, 0.0),
+                                                  ("smooth_periodic", 90, 2, 3e-3, 0.0),     # Navier-Stokes terms
+                                                  ("smooth_inflow", 125, 2, 2e-3, 1e-3),     # ... and nu Lap_h(U)
+                                                  ("sod", 64, 2, 0.0, 2e-3)])
+def test_adjoint_matches_the_transposed_oracle_tangent(name, nx, nsteps, mu, nu):
     if name == "sod":
         case = wl.sod1d(nx)
         # let the waves exist before differentiating: start from the state after 20 steps
@@ -42,12 +49,12 @@ def test_adjoint_matches_the_transposed_oracle_tangent(name, nx, nsteps):
             bc.update(xlo="reflective", xhi="reflective")
         if name == "smooth_inflow":
             bc.update(xlo="inflow", xhi="transmissive", inflow=(1.0, 0.4, 0.0, 1.0))
-        case = smooth1d(nx, 0.0, bc)
+        case = smooth1d(nx, mu, bc)
     dt = 0.2 * case["dx"]
     Ubar = np.random.default_rng(nx).normal(size=case["U0"].shape)
-    c2, o = oracle_rows(case)
+    c2, o = oracle_rows(case, nu)
     want, gwant = o.step_fixed_dt_adjoint(c2["U0"], Ubar, dt, nsteps, planar=True)
-    U, got, gbar, _ = gpu_adjoint(case, Ubar, dt, nsteps)
+    U, got, gbar, _ = gpu_adjoint(case, Ubar, dt, nsteps, nu)
     assert rel_err(U, o.step_fixed_dt(c2["U0"], dt, nsteps)[:, :1]) <= 1e-12
     assert rel_err(got, want) <= 1e-11
     assert gbar == pytest.approx(gwant, rel=1e-10, abs=1e-12 * np.abs(want).max())
@@ -108,12 +115,9 @@ def test_adjoint_rejects_what_it_does_not_do():
     for dt, n in ((0.0, 1), (1e-3, 0), (1e-3, -2)):
         with pytest.raises(E):
             s.step_fixed_dt_record(U, dt, n)
-    s.set_artificial_viscosity(1e-3)
+    s.set_time_integrator(jxs().EULER)
     with pytest.raises(E):
         s.step_fixed_dt_record(U, 1e-3, 1)
-    c2 = dict(case, mu=1e-3)
-    with pytest.raises(E):
-        jxs().Solver.from_case(c2).step_fixed_dt_record(U, 1e-3, 1)
     s32 = jxs().Solver.from_case(case, dtype=torch.float32)
     with pytest.raises(E):
         s32.step_fixed_dt_record(dev(case["U0"], torch.float32), 1e-3, 1)
