@@ -148,14 +148,16 @@ int jxs_mse_tangent(jxs_solver*, const void* U, const void* Udot, const void* Ut
  *
  * jxs_step_fixed_dt_record: as jxs_step_fixed_dt (U: DEVICE pointer, [4][1][nx] doubles, advanced in place by nsteps
  * >= 1 SSP-RK3 steps of size dt > 0), keeping the 3 stage states of every step in device memory owned by the handle
- * (96 nx bytes per step; released by the next record call or jxs_destroy).
+ * (96 nx bytes per step).
  * jxs_adjoint_steps: Ubar (DEVICE pointer, [4][1][nx] doubles) holds on entry the adjoint of the final state, e.g.
  * dL/dU^{n+m} of the loss of Eq. 14; on return the adjoint of the initial state, (dU^{n+m}/dU^n)^T Ubar.
- * *gamma_bar (HOST) = <dU^{n+m}/dgamma at fixed initial conserved state, Ubar>.  For every direction (Udot, gamma_dot)
- * <Ubar_in, tangent(Udot, gamma_dot)> = <Ubar_out, Udot> + gamma_bar gamma_dot with jxs_step_fixed_dt_tangent.
+ * *gamma_bar (HOST) = <dU^{n+m}/dgamma at fixed initial conserved state, Ubar>.  For every direction (Udot, gamma_dot),
+ * with Udot_end from jxs_step_fixed_dt_tangent: <Ubar on entry, Udot_end> = <Ubar on return, Udot> + gamma_bar gamma_dot.
  * May be called repeatedly on one recording.  Branches of the scheme carry the derivative of the branch taken.
- * Errors: JXS_EINVAL for NULL pointers, dt <= 0, nsteps < 1, an fp32 handle or ny != 1; JXS_ESTATE with a network, the forward-Euler integrator, steps pending, or (adjoint) nothing recorded; JXS_ENOMEM when the
- * trajectory does not fit.  Both synchronise the stream.                                                          */
+ * Errors: JXS_EINVAL for NULL pointers, dt <= 0, nsteps < 1, an fp32 handle or ny != 1; JXS_ESTATE with a network,
+ * the forward-Euler integrator, steps pending, or (adjoint) nothing recorded; JXS_ENOMEM when the trajectory does
+ * not fit.  The recording stays (and its memory is reused by the next record call) until jxs_destroy.  Both
+ * synchronise the stream.                                                                                         */
 int jxs_step_fixed_dt_record(jxs_solver*, void* U, double dt, int nsteps);
 int jxs_adjoint_steps(jxs_solver*, void* Ubar, double* gamma_bar);
 
