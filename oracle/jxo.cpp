@@ -19,6 +19,10 @@
 //   O10 per-face MLP         P:L96 Eq. 11; R14
 //   O11 CNN neural flux (2D)  P:L94 (3 conv layers, ReLU/ReLU/tanh, SAME padding, 6,388 parameters), Eq. 11-13
 //                             (shared between x and y); readings R18-R20 of DESIGN.md
+//   O12 tangent of the step   P:L115-128 Eq. 15-16 (the chain of Jacobians, applied to one direction), P:L149 (gamma
+//                             inference); the solver run on the Dual scalar; R21-R23
+//   O13 adjoint of the step   the transpose of O12 from its definition, one tangent run per entry (jxo.py:
+//                             Oracle.step_fixed_dt_adjoint); R24
 //
 // PARITY UNPINNED against the paper (no external definition exists; the rules
 // are shared definitions constrained only by invariants):
