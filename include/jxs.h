@@ -99,6 +99,12 @@ int jxs_flux_correction(jxs_solver*, const void* U, float* dFx, float* dGy);
 int jxs_set_flux_cnn(jxs_solver*, const float* weights_host, const double in_scale[4], const double out_scale[4]);
 int jxs_flux_cnn_inputs(jxs_solver*, const void* U, float* Xx, float* Xy);
 
+/* Change the specific-heat ratio of the handle (> 1, else JXS_EINVAL): the unknown of the paper's inference from
+ * Sod data (Fig. 3b), so an optimisation loop keeps one handle.  Everything that depends on gamma is
+ * evaluated at launch time; captured CUDA graphs and a recorded trajectory (jxs_step_fixed_dt_record) are dropped.
+ * JXS_ESTATE with steps pending (jxs_wait).                                                   */
+int jxs_set_gamma(jxs_solver*, double gamma);
+
 /* Laplacian artificial viscosity nu * Lap_h(U) of PAPER.md Eq. 10; default 0 (R7).          */
 int jxs_set_artificial_viscosity(jxs_solver*, double nu);
 
