@@ -109,6 +109,33 @@ def oracle_rate(case, nsteps):
     return case["nx"] * case["ny"] * 3 * nsteps / dt / 1e6, dt
 
 
+def oracle_rate_1d(kind, skip):
+    """cpu_baseline of the one-dimensional workloads: the oracle (one thread) on a bounded sample of the same tube,
+    as the planar problem of 8 identical rows it uses everywhere for 1D (so 8 nx cells are computed per stage).
+    kind: 'step' | 'tangent' | 'adjoint' (= one tangent run per entry of the state: the transpose from its definition)."""
+    if skip:
+        return None
+    import numpy as np
+    from oracle import jxo
+    from paper_2601_04400_b200 import workloads as wl
+    nx, ns = {"step": (40000, 20), "tangent": (20000, 15), "adjoint": (128, 6)}[kind]  # about 10 s each
+    c1 = wl.sod1d(nx, gamma=1.3)
+    c = wl.as_rows(c1)
+    o = jxo.Oracle(c["nx"], c["ny"], c["dx"], c["dy"], c["gamma"], c["mu"], c["Pr"], c["bc"])
+    dt = 0.2 * c["dx"]
+    t0 = time.perf_counter()
+    if kind == "step":
+        o.step_fixed_dt(c["U0"], dt, ns)
+    elif kind == "tangent":
+        o.step_fixed_dt_tangent(c["U0"], np.repeat(wl.dcons_dgamma(c1["U0"], 1.3), 8, axis=1), 1.0, dt, ns)
+    else:
+        o.step_fixed_dt_adjoint(c["U0"], np.ones((4, 1, nx)), dt, ns, planar=True)
+    el = time.perf_counter() - t0
+    return {"value": nx * 3 * ns / el / 1e6, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"1D Sod tube at {nx} cells (as 8 identical rows: 8 x {nx} cells computed), {ns} RK3 steps, "
+                      f"{kind}, {el:.1f} s, 1 thread"}
+
+
 def run_reference(args, rank):
     """The reference arm = the oracle on the host cores; rank 0 only."""
     if rank != 0:
@@ -185,7 +212,7 @@ def run_sod1d(args, rank, world, local_rank, dist, barrier, tdt):
                      "traffic": None, "kernel": "jxs::stage1d_kernel", "avg_launch_ms": avg, "launches_timed": stage_n,
                      "alg_flop_per_cell_stage": flop, "alg_bytes_per_cell_stage": ALG_BYTES[args.dtype],
                      "hbm_side_gbs": ALG_BYTES[args.dtype] * nx / (avg * 1e-3) / 1e9},
-        "e2e": None, "cpu_baseline": None}))
+        "e2e": None, "cpu_baseline": oracle_rate_1d("step", args.no_cpu_baseline)}))
 
 
 def run_tangent1d(args, rank, world, local_rank, dist, barrier, tdt):
@@ -242,7 +269,7 @@ def run_tangent1d(args, rank, world, local_rank, dist, barrier, tdt):
                      "frac": achieved / PEAK_FP64_TFLOPS, "traffic": None, "kernel": "jxs::tangent1d_kernel",
                      "avg_launch_ms": avg, "launches_timed": stage_n, "alg_flop_per_cell_stage": flop,
                      "alg_bytes_per_cell_stage": nbytes, "hbm_side_gbs": nbytes * nx / (avg * 1e-3) / 1e9},
-        "e2e": None, "cpu_baseline": None}))
+        "e2e": None, "cpu_baseline": oracle_rate_1d("tangent", args.no_cpu_baseline)}))
 
 
 def run_adjoint1d(args, rank, world, local_rank, dist, barrier, tdt):
@@ -305,7 +332,7 @@ def run_adjoint1d(args, rank, world, local_rank, dist, barrier, tdt):
                      "frac": achieved / PEAK_FP64_TFLOPS, "traffic": None, "kernel": "jxs::adjoint1d_kernel",
                      "avg_launch_ms": avg, "launches_timed": stage_n, "alg_flop_per_cell_stage": flop,
                      "alg_bytes_per_cell_stage": nbytes, "hbm_side_gbs": nbytes * nx / (avg * 1e-3) / 1e9},
-        "e2e": None, "cpu_baseline": None}))
+        "e2e": None, "cpu_baseline": oracle_rate_1d("adjoint", args.no_cpu_baseline)}))
 
 
 def run_cnn(args, rank, world, local_rank, dist, barrier, tdt):
