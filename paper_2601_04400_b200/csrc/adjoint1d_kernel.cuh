@@ -196,6 +196,8 @@ __device__ __forceinline__ double hllc_adjoint(const double L[4], const double R
   return gammab - gb * g * g;  // g = 1 / (gamma - 1)
 }
 
+// NS: the viscous flux and / or the nu-term are present (mu > 0 or nu > 0)
+template <bool NS>
 __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A) {
   __shared__ double prim[4][A1D_TB + 4];   // (rho, u, v, p) of padded columns pc0-2 .. pc0+129
   __shared__ double rmS[4][A1D_TB];        // right-biased state at each cell's left face (values)
@@ -268,7 +270,7 @@ __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A
 #pragma unroll
       for (int k = 0; k < 4; ++k) { f[k] = A.dxi * (LbS[k][t + 1] - LbS[k][t]); R[k] = rmS[k][t + 1]; }
       double gb = hllc_adjoint(Lp, R, A.gamma, f, Lpb, Rnb);
-      if (A.mu != 0.0) {
+      if (NS && A.mu != 0.0) {
         // F -= (0, txx, txy, ub txx + vb txy + kappa Tx), txx = 4/3 mu ux, txy = mu vx, T = p / rho (R8, 1D)
         const int c = t + 2;
         const double rc_ = prim[0][c], rn = prim[0][c + 1], rci = rcp_(rc_), rni = rcp_(rn);
@@ -289,7 +291,10 @@ __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A
       if (mine) gbar += gb;
     }
 #pragma unroll
-    for (int k = 0; k < 4; ++k) { rmB[k][t + 1] = Rnb[k]; visN[k][t + 1] = vn[k]; }
+    for (int k = 0; k < 4; ++k) {
+      rmB[k][t + 1] = Rnb[k];
+      if (NS) visN[k][t + 1] = vn[k];
+    }
   }
   __syncthreads();
 
@@ -322,7 +327,7 @@ __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A
 #pragma unroll
     for (int k = 0; k < 4; ++k)
       Wb[k] = con[k][0][t + 2] + con[k][1][t + 1] + con[k][2][t] + con[k][3][t - 1] + con[k][4][t - 2] +
-              (vo[k] + visN[k][t]);
+              (NS ? vo[k] + visN[k][t] : 0.0);
     const double r = wc[0], u = wc[1], v = wc[2], p = wc[3], ri = rcp_(r);
     // u = ru / r, v = rv / r, p = g1 (E - (ru u + rv v) / 2)
     double out[4];
@@ -334,7 +339,7 @@ __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       double x = out[k];
-      if (A.nu != 0.0)  // L += nu Lap_h(U) (Eq. 10): the Laplacian is its own transpose
+      if (NS && A.nu != 0.0)  // L += nu Lap_h(U) (Eq. 10): the Laplacian is its own transpose
         x = fma(A.nu * A.dxi * A.dxi, LbS[k][t - 1] - 2.0 * LbS[k][t] + LbS[k][t + 1], x);
       if (interior) x = fma(A.b, Ub[k], x) + Ex[k];
       A.Ubar_in[k * A.plane + pc] = x;

@@ -933,7 +933,8 @@ cudaError_t adjoint_stage(jxs_solver* s, const double* U, const double* out, dou
     e1v = s->events[s->events_used++];
     cudaEventRecord(e0, s->stream);
   }
-  adjoint1d_kernel<<<s->adj_parts, A1D_TB, 0, s->stream>>>(A);
+  if (s->mu > 0 || s->nu > 0) adjoint1d_kernel<true><<<s->adj_parts, A1D_TB, 0, s->stream>>>(A);
+  else adjoint1d_kernel<false><<<s->adj_parts, A1D_TB, 0, s->stream>>>(A);
   if (e1v) cudaEventRecord(e1v, s->stream);
   adjoint1d_fold_kernel<<<1, A1D_FOLD_TB, 0, s->stream>>>(A.Ubar_in, s->pitch, s->nx, s->bc.xlo, s->bc.xhi, s->bc.inflow[3],
                                                    s->gamma, partial, s->adj_parts, partial + s->adj_parts);
