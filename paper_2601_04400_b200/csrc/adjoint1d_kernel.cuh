@@ -39,7 +39,8 @@ struct Adjoint1dArgs {
 
 // WENO5-JS values of one variable at one cell (as weno5_dual in tangent1d_kernel.cuh, values only) and, given the
 // adjoints (Lb, Rb) of the two results, the adjoints of the five cell values
-__device__ __forceinline__ void weno5_val(double a, double b, double c, double d, double e, double& Lp, double& Rm) {
+__device__ __forceinline__ void weno5_val(double a, double b, double c, double d, double e, double& Lp, double& Rm,
+                                          double& Di, double& Ei) {
   const double s0 = a - 2.0 * b + c, t0 = a - 4.0 * b + 3.0 * c;
   const double s1 = b - 2.0 * c + d, t1 = b - d;
   const double s2 = c - 2.0 * d + e, t2 = 3.0 * c - 4.0 * d + e;
@@ -50,14 +51,16 @@ __device__ __forceinline__ void weno5_val(double a, double b, double c, double d
   const double e0 = x0 * x0, e1 = x1 * x1, e2 = x2 * x2;
   const double w0 = e1 * e2, w1 = e0 * e2, w2 = e0 * e1;
   const double k0 = 0.1 / 6.0, k1 = 0.6 / 6.0, k2 = 0.3 / 6.0;
-  Lp = (k0 * w0 * (2.0 * a - 7.0 * b + 11.0 * c) + k1 * w1 * (5.0 * c - b + 2.0 * d) + k2 * w2 * (2.0 * c + 5.0 * d - e)) *
-       rcp_(0.1 * w0 + 0.6 * w1 + 0.3 * w2);
-  Rm = (k0 * w2 * (2.0 * e - 7.0 * d + 11.0 * c) + k1 * w1 * (5.0 * c - d + 2.0 * b) + k2 * w0 * (2.0 * c + 5.0 * b - a)) *
-       rcp_(0.1 * w2 + 0.6 * w1 + 0.3 * w0);
+  Di = rcp_(0.1 * w0 + 0.6 * w1 + 0.3 * w2);  // the two reciprocals are kept for the reverse sweep
+  Ei = rcp_(0.1 * w2 + 0.6 * w1 + 0.3 * w0);
+  Lp = (k0 * w0 * (2.0 * a - 7.0 * b + 11.0 * c) + k1 * w1 * (5.0 * c - b + 2.0 * d) + k2 * w2 * (2.0 * c + 5.0 * d - e)) * Di;
+  Rm = (k0 * w2 * (2.0 * e - 7.0 * d + 11.0 * c) + k1 * w1 * (5.0 * c - d + 2.0 * b) + k2 * w0 * (2.0 * c + 5.0 * b - a)) * Ei;
 }
 
+// (Lp, Rm, Di, Ei: the forward values and reciprocals of weno5_val; they multiply Lb / Rb only, so after the
+// positivity guard, which zeroes the adjoint it replaces, any finite numbers do)
 __device__ __forceinline__ void weno5_adjoint(double a, double b, double c, double d, double e, double Lb, double Rb,
-                                              double g[5]) {
+                                              double Lp, double Rm, double Di, double Ei, double g[5]) {
   const double s0 = a - 2.0 * b + c, t0 = a - 4.0 * b + 3.0 * c;
   const double s1 = b - 2.0 * c + d, t1 = b - d;
   const double s2 = c - 2.0 * d + e, t2 = 3.0 * c - 4.0 * d + e;
@@ -70,15 +73,11 @@ __device__ __forceinline__ void weno5_adjoint(double a, double b, double c, doub
   const double k0 = 0.1 / 6.0, k1 = 0.6 / 6.0, k2 = 0.3 / 6.0;
   // left-biased value Lp = N / D
   const double Q0 = 2.0 * a - 7.0 * b + 11.0 * c, Q1 = 5.0 * c - b + 2.0 * d, Q2 = 2.0 * c + 5.0 * d - e;
-  const double Di = rcp_(0.1 * w0 + 0.6 * w1 + 0.3 * w2);
-  const double Lp = (k0 * w0 * Q0 + k1 * w1 * Q1 + k2 * w2 * Q2) * Di;
   const double Nb = Lb * Di, Db = -Nb * Lp;
   double w0b = Nb * k0 * Q0 + Db * 0.1, w1b = Nb * k1 * Q1 + Db * 0.6, w2b = Nb * k2 * Q2 + Db * 0.3;
   const double Q0b = Nb * k0 * w0, Q1b = Nb * k1 * w1, Q2b = Nb * k2 * w2;
   // right-biased value Rm = N' / D' (the mirrored stencil: w0 and w2 exchanged)
   const double P0 = 2.0 * e - 7.0 * d + 11.0 * c, P1 = 5.0 * c - d + 2.0 * b, P2 = 2.0 * c + 5.0 * b - a;
-  const double Ei = rcp_(0.1 * w2 + 0.6 * w1 + 0.3 * w0);
-  const double Rm = (k0 * w2 * P0 + k1 * w1 * P1 + k2 * w0 * P2) * Ei;
   const double Mb = Rb * Ei, Eb = -Mb * Rm;
   w2b += Mb * k0 * P0 + Eb * 0.1; w1b += Mb * k1 * P1 + Eb * 0.6; w0b += Mb * k2 * P2 + Eb * 0.3;
   const double P0b = Mb * k0 * w2, P1b = Mb * k1 * w1, P2b = Mb * k2 * w0;
@@ -99,14 +98,14 @@ __device__ __forceinline__ void weno5_adjoint(double a, double b, double c, doub
 // adjoint of one side K of the HLLC flux (hllc_side_dual in tangent1d_kernel.cuh): given the flux adjoint f, add to
 // the adjoints of the side's state W = (rho, u, v, p), of the wave speeds sK, s*, of the clipped speed sc and of
 // g = 1/(gamma-1)
-__device__ __forceinline__ void hllc_side_adjoint(const double W[4], double sK, double sS, double sc, double g,
+__device__ __forceinline__ void hllc_side_adjoint(const double W[4], double ri, double sK, double sS, double sc, double g,
                                                   const double f[4], double Wb[4], double& sKb, double& sSb, double& scb,
-                                                  double& gb) {
+                                                  double& gb) {  // ri = 1 / rho
   const double r = W[0], u = W[1], v = W[2], p = W[3];
   const double q = u * u + v * v;
   const double E = p * g + 0.5 * r * q;
   const double ru = r * u, du = sK - u, den = sK - sS;
-  const double deni = rcp_(den), ri = rcp_(r);
+  const double deni = rcp_(den);
   const double chi = du * deni, rc = r * chi;
   const double A = r * du, Ai = rcp_(A), B = p * Ai;
   const double Cc = sS + B, Dd = sS - u;
@@ -152,7 +151,7 @@ __device__ __forceinline__ double hllc_adjoint(const double L[4], const double R
   const double g = rcp_(gamma - 1.0);
   const double rLi = rcp_(L[0]), rRi = rcp_(R[0]);
   const double zL = gamma * L[3] * rLi, zR = gamma * R[3] * rRi;
-  const double aL = zL * rsqrt_(zL), aR = zR * rsqrt_(zR);
+  const double aLi = rsqrt_(zL), aRi = rsqrt_(zR), aL = zL * aLi, aR = zR * aRi;
   const double xa = L[1] - aL, xb = R[1] - aR, ya = L[1] + aL, yb = R[1] + aR;
   const bool sL_from_R = xb < xa, sR_from_R = ya < yb;
   const double sL = sL_from_R ? xb : xa, sR = sR_from_R ? yb : ya;
@@ -163,12 +162,12 @@ __device__ __forceinline__ double hllc_adjoint(const double L[4], const double R
 #pragma unroll
   for (int k = 0; k < 4; ++k) { Lb[k] = 0.0; Rb[k] = 0.0; }
   double sLb = 0.0, sRb = 0.0, sSb = 0.0, smb = 0.0, spb = 0.0, gb = 0.0;
-  if (sS > 0.0) hllc_side_adjoint(L, sL, sS, sm, g, f, Lb, sLb, sSb, smb, gb);
-  else if (sS < 0.0) hllc_side_adjoint(R, sR, sS, sp, g, f, Rb, sRb, sSb, spb, gb);
+  if (sS > 0.0) hllc_side_adjoint(L, rLi, sL, sS, sm, g, f, Lb, sLb, sSb, smb, gb);
+  else if (sS < 0.0) hllc_side_adjoint(R, rRi, sR, sS, sp, g, f, Rb, sRb, sSb, spb, gb);
   else {
     const double h[4] = {0.5 * f[0], 0.5 * f[1], 0.5 * f[2], 0.5 * f[3]};
-    hllc_side_adjoint(L, sL, sS, sm, g, h, Lb, sLb, sSb, smb, gb);
-    hllc_side_adjoint(R, sR, sS, sp, g, h, Rb, sRb, sSb, spb, gb);
+    hllc_side_adjoint(L, rLi, sL, sS, sm, g, h, Lb, sLb, sSb, smb, gb);
+    hllc_side_adjoint(R, rRi, sR, sS, sp, g, h, Rb, sRb, sSb, spb, gb);
   }
   if (sL < 0.0) sLb += smb;  // sm = min(0, sL), sp = max(0, sR)
   if (0.0 < sR) sRb += spb;
@@ -186,11 +185,11 @@ __device__ __forceinline__ double hllc_adjoint(const double L[4], const double R
   // a = sqrt(z), z = gamma p / rho
   double gammab = 0.0;
   {
-    const double zb = 0.5 * aLb * rcp_(aL);
+    const double zb = 0.5 * aLb * aLi;
     gammab += zb * L[3] * rLi; Lb[3] += zb * gamma * rLi; Lb[0] -= zb * zL * rLi;
   }
   {
-    const double zb = 0.5 * aRb * rcp_(aR);
+    const double zb = 0.5 * aRb * aRi;
     gammab += zb * R[3] * rRi; Rb[3] += zb * gamma * rRi; Rb[0] -= zb * zR * rRi;
   }
   return gammab - gb * g * g;  // g = 1 / (gamma - 1)
@@ -244,7 +243,10 @@ __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A
   for (int k = 0; k < 4; ++k) {
     wc[k] = prim[k][t + 2];
     Lp[k] = Rm[k] = wc[k];
-    if (stencil) weno5_val(prim[k][t], prim[k][t + 1], wc[k], prim[k][t + 3], prim[k][t + 4], Lp[k], Rm[k]);
+    double Di = 0.0, Ei = 0.0;
+    if (stencil) weno5_val(prim[k][t], prim[k][t + 1], wc[k], prim[k][t + 3], prim[k][t + 4], Lp[k], Rm[k], Di, Ei);
+    con[k][0][t] = Di;  // my own slots of the gather array, free until my reverse sweep fills them
+    con[k][1][t] = Ei;
   }
   if (stencil) {
     badR = !(Rm[0] > 0.0) || !(Rm[3] > 0.0);
@@ -304,7 +306,8 @@ __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A
     double g[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
     const double Rb = rmB[k][t];
     if (stencil) {
-      weno5_adjoint(prim[k][t], prim[k][t + 1], wc[k], prim[k][t + 3], prim[k][t + 4], badL ? 0.0 : Lpb[k], badR ? 0.0 : Rb, g);
+      weno5_adjoint(prim[k][t], prim[k][t + 1], wc[k], prim[k][t + 3], prim[k][t + 4], badL ? 0.0 : Lpb[k], badR ? 0.0 : Rb,
+                    Lp[k], rmS[k][t], con[k][0][t], con[k][1][t], g);
       g[2] += (badL ? Lpb[k] : 0.0) + (badR ? Rb : 0.0);
     }
 #pragma unroll
