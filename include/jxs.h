@@ -132,12 +132,13 @@ int jxs_step_fixed_dt(jxs_solver*, void* U, double dt, int nsteps);
  *             of it (owned by the caller; Udot = 0 differentiates with respect to gamma at fixed conserved state,
  *             Udot[3] = -p/(gamma-1)^2 at fixed primitives)
  *   gamma_dot perturbation of gamma along the same direction
- *   dt        step size, a constant of the differentiation (> 0); nsteps >= 0 SSP-RK3 steps
+ *   dt        step size, a constant of the differentiation (> 0); nsteps >= 0 steps of the handle's time integrator
+ *             (SSP-RK3, or the forward-Euler update of Eq. 10 with its nu-term: the update the paper differentiates)
  * On return U = S^nsteps(U; gamma) (the same arithmetic as the tangent's value part, equal to jxs_step_fixed_dt to
  * round-off) and Udot = dS^nsteps/dU . Udot + dS^nsteps/dgamma . gamma_dot.  Branches of the scheme (min / max of wave
  * speeds, sign of the contact speed, positivity guard) carry the derivative of the branch taken.
  * Errors: JXS_EINVAL for NULL pointers, dt <= 0, nsteps < 0, a non-finite gamma_dot, an fp32 handle or ny != 1;
- * JXS_ESTATE with a network set, with the forward-Euler integrator or with steps pending (jxs_wait);
+ * JXS_ESTATE with a network set or with steps pending (jxs_wait);
  * JXS_ENOMEM / JXS_ECUDA from the first call's allocation of the tangent buffers.  Synchronises the stream.      */
 int jxs_step_fixed_dt_tangent(jxs_solver*, void* U, void* Udot, double gamma_dot, double dt, int nsteps);
 
@@ -153,15 +154,15 @@ int jxs_mse_tangent(jxs_solver*, const void* U, const void* Udot, const void* Ut
  * Two calls: the forward sweep that records the trajectory, then the reverse sweep.
  *
  * jxs_step_fixed_dt_record: as jxs_step_fixed_dt (U: DEVICE pointer, [4][1][nx] doubles, advanced in place by nsteps
- * >= 1 SSP-RK3 steps of size dt > 0), keeping the 3 stage states of every step in device memory owned by the handle
- * (96 nx bytes per step).
+ * >= 1 steps of size dt > 0 of the handle's time integrator), keeping the stage states of every step (3 for SSP-RK3, 1
+ * for forward Euler) in device memory owned by the handle (32 nx bytes per state).
  * jxs_adjoint_steps: Ubar (DEVICE pointer, [4][1][nx] doubles) holds on entry the adjoint of the final state, e.g.
  * dL/dU^{n+m} of the loss of Eq. 14; on return the adjoint of the initial state, (dU^{n+m}/dU^n)^T Ubar.
  * *gamma_bar (HOST) = <dU^{n+m}/dgamma at fixed initial conserved state, Ubar>.  For every direction (Udot, gamma_dot),
  * with Udot_end from jxs_step_fixed_dt_tangent: <Ubar on entry, Udot_end> = <Ubar on return, Udot> + gamma_bar gamma_dot.
  * May be called repeatedly on one recording.  Branches of the scheme carry the derivative of the branch taken.
  * Errors: JXS_EINVAL for NULL pointers, dt <= 0, nsteps < 1, an fp32 handle or ny != 1; JXS_ESTATE with a network,
- * the forward-Euler integrator, steps pending, or (adjoint) nothing recorded; JXS_ENOMEM when the trajectory does
+ * steps pending, or (adjoint) nothing recorded; JXS_ENOMEM when the trajectory does
  * not fit.  The recording stays (and its memory is reused by the next record call) until jxs_destroy.  Both
  * synchronise the stream.                                                                                         */
 int jxs_step_fixed_dt_record(jxs_solver*, void* U, double dt, int nsteps);

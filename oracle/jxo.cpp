@@ -908,6 +908,25 @@ int jxo_step_fixed_dt_tangent(jxo_solver* s, double* U, double* Udot, double gam
   return rc;
 }
 
+// L(U) and its tangent: the building block of O12 for a caller-written time integrator (the forward-Euler update of
+// PAPER.md Eq. 10 written out in jxo.py).  L, Ldot: [4][ny][nx] doubles, out.
+int jxo_rhs_tangent(jxo_solver* s, const double* U, const double* Udot, double gamma_dot, double* L, double* Ldot) {
+  if (!s || !U || !Udot || !L || !Ldot) return JXO_EINVAL;
+  if (s->dtype != JXO_F64) { s->err = "the tangent is fp64 only"; return JXO_EINVAL; }
+  if (s->mlp.on || s->cnn.on) { s->err = "the tangent does not differentiate the networks"; return JXO_ESTATE; }
+  const size_t n = (size_t)4 * s->c.nx * s->c.ny;
+  std::vector<Dual> Ud(n), Ld(n), Up;
+  for (size_t i = 0; i < n; ++i) Ud[i] = Dual(U[i], Udot[i]);
+  s->c.gamma_dot = gamma_dot;
+  Core<Dual> core(s->c, s->type, s->ghosts, s->mlp);
+  core.pad(Ud.data(), Up);
+  core.fill_and_rhs(Up, Ld.data());
+  s->c.gamma_dot = 0;
+  s->guard += core.guard;
+  for (size_t i = 0; i < n; ++i) { L[i] = Ld[i].v; Ldot[i] = Ld[i].d; }
+  return JXO_OK;
+}
+
 // pointwise tangents of O4 and O5, for the closed-form pins
 void jxo_weno5_tangent(const double v[5], const double vdot[5], double out[2]) {
   const Dual r = weno5<Dual>(Dual(v[0], vdot[0]), Dual(v[1], vdot[1]), Dual(v[2], vdot[2]), Dual(v[3], vdot[3]),

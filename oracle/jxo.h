@@ -57,6 +57,9 @@ int jxo_get_time(const jxo_solver*, double* t, double* last_dt);
  * Udot = dS^n/dU . Udot + dS^n/dgamma . gamma_dot.  fp64 handles without a network (EINVAL / ESTATE).
  * With a loss L(U) (Eq. 14) this gives dL/dgamma = <dL/dU, Udot>: the paper's gamma inference (L149, Fig. 3b). */
 int jxo_step_fixed_dt_tangent(jxo_solver*, double* U, double* Udot, double gamma_dot, double dt, int nsteps);
+/* L(U) and its tangent along (Udot, gamma_dot), [4][ny][nx] doubles each: for the forward-Euler update of Eq. 10,
+ * which jxo.py writes out with it.                                                                            */
+int jxo_rhs_tangent(jxo_solver*, const double* U, const double* Udot, double gamma_dot, double* L, double* Ldot);
 
 /* ---- introspection used only by the oracle's own pins ------------------- */
 /* one left-biased WENO5-JS value at i+1/2 from (v[i-2..i+2]) in double          */

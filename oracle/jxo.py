@@ -60,6 +60,7 @@ def lib():
         L.jxo_cnn_apply.argtypes = [vp, dp, C.c_int, C.c_int, dp]
         L.jxo_cnn_fields.argtypes = [vp, dp, dp, dp, dp, dp]
         L.jxo_step_fixed_dt_tangent.argtypes = [vp, vp, vp, C.c_double, C.c_double, C.c_int]
+        L.jxo_rhs_tangent.argtypes = [vp, vp, vp, C.c_double, vp, vp]
         L.jxo_weno5_tangent.argtypes = [dp, dp, dp]
         L.jxo_weno5_tangent.restype = None
         L.jxo_hllc_tangent.argtypes = [dp, dp, dp, dp, C.c_double, C.c_double, dp, dp]
@@ -232,16 +233,34 @@ class Oracle:
         self._chk(lib().jxo_step_fixed_dt(self._h, U.ctypes.data, float(dt), int(nsteps)))
         return U
 
-    def step_fixed_dt_tangent(self, U, Udot, gamma_dot, dt, nsteps):
-        """O12: (U, Udot) after nsteps steps of size dt; Udot is the derivative along (Udot, gamma_dot)."""
+    def rhs_tangent(self, U, Udot, gamma_dot):
+        """(L(U), its derivative along (Udot, gamma_dot))."""
+        U = np.ascontiguousarray(self._field(U), dtype=np.float64)
+        Udot = np.ascontiguousarray(Udot, dtype=np.float64)
+        assert Udot.shape == U.shape
+        L, Ld = np.empty_like(U), np.empty_like(U)
+        self._chk(lib().jxo_rhs_tangent(self._h, U.ctypes.data, Udot.ctypes.data, float(gamma_dot), L.ctypes.data,
+                                        Ld.ctypes.data))
+        return L, Ld
+
+    def step_fixed_dt_tangent(self, U, Udot, gamma_dot, dt, nsteps, scheme="ssprk3"):
+        """O12: (U, Udot) after nsteps steps of size dt; Udot is the derivative along (Udot, gamma_dot).
+        scheme "euler": the update of PAPER.md Eq. 10 as printed, U <- U + dt L(U), written out here."""
         U = np.ascontiguousarray(self._field(U), dtype=np.float64).copy()
         Udot = np.ascontiguousarray(Udot, dtype=np.float64).copy()
         assert Udot.shape == U.shape
+        if scheme == "euler":
+            for _ in range(int(nsteps)):
+                L, Ld = self.rhs_tangent(U, Udot, gamma_dot)
+                U = U + dt * L
+                Udot = Udot + dt * Ld
+            return U, Udot
+        assert scheme == "ssprk3"
         self._chk(lib().jxo_step_fixed_dt_tangent(self._h, U.ctypes.data, Udot.ctypes.data, float(gamma_dot),
                                                   float(dt), int(nsteps)))
         return U, Udot
 
-    def step_fixed_dt_adjoint(self, U, Ubar, dt, nsteps, planar=False):
+    def step_fixed_dt_adjoint(self, U, Ubar, dt, nsteps, planar=False, scheme="ssprk3"):
         """O13: the adjoint of nsteps fixed-dt steps, from the definition of a transpose (Eq. 16 read from
         the left): entry j of J^T Ubar is <Ubar, J e_j>, with J e_j from the tangent O12 -- one tangent run per
         entry of the state (small cases only), and gamma_bar = <Ubar, dS/dgamma>.
@@ -256,9 +275,9 @@ class Oracle:
         for j in range(out.size):
             e = np.zeros(shape)
             e.flat[j] = 1.0
-            _, D = self.step_fixed_dt_tangent(U, np.repeat(e, self.ny, axis=1) if planar else e, 0.0, dt, nsteps)
+            _, D = self.step_fixed_dt_tangent(U, np.repeat(e, self.ny, axis=1) if planar else e, 0.0, dt, nsteps, scheme)
             out.flat[j] = float(np.sum(Ubar * pick(D)))
-        _, D = self.step_fixed_dt_tangent(U, np.zeros_like(U), 1.0, dt, nsteps)
+        _, D = self.step_fixed_dt_tangent(U, np.zeros_like(U), 1.0, dt, nsteps, scheme)
         return out, float(np.sum(Ubar * pick(D)))
 
     def time(self):

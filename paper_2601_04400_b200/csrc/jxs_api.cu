@@ -57,6 +57,7 @@ struct jxs_solver {
   // layout [4][pitch] per state: tape = the 3 stage inputs of every recorded step + the final state
   double* tape = nullptr;
   int tape_steps = 0;
+  int tape_scheme = JXS_SSPRK3;  // the integrator the recording was made with
   size_t tape_bytes = 0;
   double tape_dt = 0;
   double* adj = nullptr;  // 4 adjoint states, then the gamma_bar partial sums, then gamma_bar
@@ -815,7 +816,6 @@ int tangent_common(jxs_solver* s, void* U, void* Udot, double gamma_dot, double 
   if (s->dtype != JXS_F64) return fail(s, JXS_EINVAL, "the tangent is fp64 only");
   if (s->ny != 1) return fail(s, JXS_EINVAL, "the tangent is built for one-dimensional problems (ny = 1)");
   if (s->mlp_on || s->cnn_on) return fail(s, JXS_ESTATE, "the tangent does not differentiate the networks");
-  if (s->scheme != JXS_SSPRK3) return fail(s, JXS_ESTATE, "the tangent steps with SSP-RK3");
   if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
   const size_t bytes = (size_t)4 * s->plane * s->elem;
   for (int b = 0; b < 3; ++b)
@@ -828,6 +828,20 @@ int tangent_common(jxs_solver* s, void* U, void* Udot, double gamma_dot, double 
   s->events_used = 0;
   s->mlp_events_used = 0;
   int n = 0;
+  if (s->scheme == JXS_EULER) {  // Eq. 10 as printed: one stage with (a, b) = (0, 1); the two buffers swap roles
+    int at = 0;
+    for (; n < nsteps; ++n, at ^= 1) {
+      prepare_step_kernel<<<1, 1, 0, s->stream>>>(s->d_state, 0, 0.0, dt);
+      s->launches++;
+      CU(cudaGetLastError());
+      CU(ghost_fill(s, s->buf[at]));
+      CU(ghost_fill_tangent(s, s->bufd[at], gamma_dot));
+      CU(tangent_stage(s, at, at ^ 1, 0.0, 1.0, gamma_dot));
+    }
+    CU(unpad(s, s->buf[at], U));
+    CU(unpad(s, s->bufd[at], Udot));
+    return finish_steps(s, nsteps);
+  }
   static const bool no_graph = getenv("JXS_NO_GRAPH") != nullptr;
   if (!s->profiling && !no_graph && nsteps >= 4) {
     // the first step runs as plain launches; the rest replay one captured step (the buffers' roles return after it)
@@ -867,7 +881,6 @@ int adjoint_checks(jxs_solver* s) {
   if (s->dtype != JXS_F64) return fail(s, JXS_EINVAL, "the adjoint is fp64 only");
   if (s->ny != 1) return fail(s, JXS_EINVAL, "the adjoint is built for one-dimensional problems (ny = 1)");
   if (s->mlp_on || s->cnn_on) return fail(s, JXS_ESTATE, "the adjoint does not differentiate the networks");
-  if (s->scheme != JXS_SSPRK3) return fail(s, JXS_ESTATE, "the adjoint steps with SSP-RK3");
   if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
   return JXS_OK;
 }
@@ -881,7 +894,8 @@ int record_common(jxs_solver* s, void* U, double dt, int nsteps) {
   if (rc != JXS_OK) return rc;
   s->tape_steps = 0;
   const size_t state = (size_t)4 * s->pitch * sizeof(double);
-  const size_t bytes = state * (3 * (size_t)nsteps + 1);
+  const int per_step = s->scheme == JXS_EULER ? 1 : 3;  // recorded states per step
+  const size_t bytes = state * (per_step * (size_t)nsteps + 1);
   if (!s->tape || s->tape_bytes < bytes) {  // the tape is kept between calls and only ever grows
     cudaFree(s->tape);
     s->tape = nullptr;
@@ -892,7 +906,7 @@ int record_common(jxs_solver* s, void* U, double dt, int nsteps) {
   // the columns past the padded row are never written; the kernels' clamped support reads must find numbers there
   if (s->pitch > s->nx + 6)
     CU(cudaMemset2DAsync(s->tape + s->nx + 6, (size_t)s->pitch * sizeof(double), 0,
-                         (size_t)(s->pitch - s->nx - 6) * sizeof(double), 4 * (3 * (size_t)nsteps + 1), s->stream));
+                         (size_t)(s->pitch - s->nx - 6) * sizeof(double), 4 * (per_step * (size_t)nsteps + 1), s->stream));
   CompactLayout compact(s);
   auto T = [&](long long i) { return (void*)compact_state(s, s->tape, i); };
   CU(pad(s, U, T(0)));
@@ -902,6 +916,11 @@ int record_common(jxs_solver* s, void* U, double dt, int nsteps) {
     prepare_step_kernel<<<1, 1, 0, s->stream>>>(s->d_state, 0, 0.0, dt);
     s->launches++;
     CU(cudaGetLastError());
+    if (per_step == 1) {  // forward Euler (Eq. 10)
+      CU(ghost_fill(s, T(n)));
+      CU(stage(s, T(n), nullptr, T(n + 1), 0, 0.0, 1.0, nullptr));
+      continue;
+    }
     CU(ghost_fill(s, T(3 * n)));
     CU(stage(s, T(3 * n), nullptr, T(3 * n + 1), 0, 0.0, 1.0, nullptr));
     CU(ghost_fill(s, T(3 * n + 1)));
@@ -909,10 +928,11 @@ int record_common(jxs_solver* s, void* U, double dt, int nsteps) {
     CU(ghost_fill(s, T(3 * n + 2)));
     CU(stage(s, T(3 * n + 2), T(3 * n), T(3 * n + 3), 0, 1.0 / 3.0, 2.0 / 3.0, nullptr));
   }
-  CU(unpad(s, T(3LL * nsteps), U));
+  CU(unpad(s, T((long long)per_step * nsteps), U));
   rc = finish_steps(s, nsteps);
   if (rc != JXS_OK) return rc;
   s->tape_steps = nsteps;
+  s->tape_scheme = s->scheme;
   s->tape_dt = dt;
   return JXS_OK;
 }
@@ -964,6 +984,11 @@ int adjoint_common(jxs_solver* s, void* Ubar, double* gamma_bar) {
   s->events_used = 0;
   int x = 0;  // which adjoint state holds the adjoint of U^{n+1}
   for (long long n = s->tape_steps - 1; n >= 0; --n) {
+    if (s->tape_scheme == JXS_EULER) {  // U^{n+1} = U^n + dt L(U^n)
+      CU(adjoint_stage(s, T(n), B(x), B(x ^ 1), 1.0, nullptr, 0.0, nullptr, 0.0));
+      x ^= 1;
+      continue;
+    }
     const int y2 = (x + 1) & 3, y1 = (x + 2) & 3, y0 = (x + 3) & 3;
     // U^{n+1} = 1/3 U0 + 2/3 (U2 + dt L(U2));  U2 = 3/4 U0 + 1/4 (U1 + dt L(U1));  U1 = U0 + dt L(U0)   (R5)
     CU(adjoint_stage(s, T(3 * n + 2), B(x), B(y2), 2.0 / 3.0, nullptr, 0.0, nullptr, 0.0));

@@ -281,6 +281,41 @@ def test_adjoint_is_the_gradient_of_a_linear_functional():
     assert np.sum(c1 * D[:, :1]) == pytest.approx(np.sum(g1 * d1) + 0.7 * gb1, rel=1e-12)
 
 
+def test_rhs_tangent_and_the_euler_update():
+    case = wl.shock_cylinder(nx=64, ny=32, Ms=2.0, Re=200.0)
+    Udir = wl.dcons_dgamma(case["U0"], G) + 0.1 * wl.smooth_direction(case["U0"].shape, seed=12)
+    o = make(case)
+    L, Ld = o.rhs_tangent(case["U0"], Udir, 1.0)
+    assert np.array_equal(L, o.rhs(case["U0"]))
+    h = 1e-7
+    fd = (make(case, gamma=G + h).rhs(case["U0"] + h * Udir) - make(case, gamma=G - h).rhs(case["U0"] - h * Udir)) / (2 * h)
+    fluid = (case["phi"] > 0)[None]
+    assert rel(Ld * fluid, fd * fluid) < 5e-6
+    # SSP-RK3 composed from rhs_tangent by hand is O12
+    dt = 1e-3
+    def stage(U, D):
+        L, Ld = o.rhs_tangent(U, D, 1.0)
+        return U + dt * L, D + dt * Ld
+    U1, D1 = stage(case["U0"], Udir)
+    U2, D2 = stage(U1, D1)
+    U2, D2 = 0.75 * case["U0"] + 0.25 * U2, 0.75 * Udir + 0.25 * D2
+    U3, D3 = stage(U2, D2)
+    U3, D3 = case["U0"] / 3 + 2 * U3 / 3, Udir / 3 + 2 * D3 / 3
+    Us, Ds = o.step_fixed_dt_tangent(case["U0"], Udir, 1.0, dt, 1)
+    # (fluid cells: the step also leaves its IBM ghost fill in the non-fluid cells it returns)
+    assert rel(U3 * fluid, Us * fluid) < 1e-14 and rel(D3 * fluid, Ds * fluid) < 1e-12
+    # Eq. 10: two Euler steps against central differences of the same update written with the primal L
+    def euler(c, g, U, n):
+        oo = make(c, gamma=g)
+        for _ in range(n):
+            U = U + dt * oo.rhs(U)
+        return U
+    Ue, De = o.step_fixed_dt_tangent(case["U0"], Udir, 1.0, dt, 2, scheme="euler")
+    assert np.array_equal(Ue, euler(case, G, case["U0"], 2))
+    fd = (euler(case, G + h, case["U0"] + h * Udir, 2) - euler(case, G - h, case["U0"] - h * Udir, 2)) / (2 * h)
+    assert rel(De * fluid, fd * fluid) < 5e-6
+
+
 def test_tangent_argument_checks():
     case = wl.vortex(8)
     o = make(case, dtype=np.float32)
