@@ -167,6 +167,11 @@ int jxs_mse_tangent(jxs_solver*, const void* U, const void* Udot, const void* Ut
  * synchronise the stream.                                                                                         */
 int jxs_step_fixed_dt_record(jxs_solver*, void* U, double dt, int nsteps);
 int jxs_adjoint_steps(jxs_solver*, void* Ubar, double* gamma_bar);
+/* Checkpointing of the recording (default off): with on != 0 an SSP-RK3 recording keeps only U^n of every step (32 nx
+ * bytes per step instead of 96) and jxs_adjoint_steps recomputes the two inner stage states of a step before it
+ * reverses them: one third of the memory for two more stage launches per step, bit-identical results.  Applies to
+ * recordings made after the call.                                                                                 */
+int jxs_set_adjoint_checkpointing(jxs_solver*, int on);
 
 /* Same two calls on HOST buffers (pageable or pinned): host->device copy, stepping,
  * device->host copy; used for end-to-end timing.                                            */

@@ -58,6 +58,9 @@ struct jxs_solver {
   double* tape = nullptr;
   int tape_steps = 0;
   int tape_scheme = JXS_SSPRK3;  // the integrator the recording was made with
+  int checkpoint = 0;            // jxs_set_adjoint_checkpointing: keep one state per step, recompute the stages
+  int tape_ckpt = 0;             // ... as the recording was made
+  double* ckpt = nullptr;        // the two recomputed stage states (compact layout)
   size_t tape_bytes = 0;
   double tape_dt = 0;
   double* adj = nullptr;  // 4 adjoint states, then the gamma_bar partial sums, then gamma_bar
@@ -894,7 +897,12 @@ int record_common(jxs_solver* s, void* U, double dt, int nsteps) {
   if (rc != JXS_OK) return rc;
   s->tape_steps = 0;
   const size_t state = (size_t)4 * s->pitch * sizeof(double);
-  const int per_step = s->scheme == JXS_EULER ? 1 : 3;  // recorded states per step
+  const bool ckpt = s->checkpoint && s->scheme == JXS_SSPRK3;
+  const int per_step = (s->scheme == JXS_EULER || ckpt) ? 1 : 3;  // recorded states per step
+  if (ckpt && !s->ckpt) {
+    CU(cudaMalloc(&s->ckpt, 2 * state));
+    CU(cudaMemsetAsync(s->ckpt, 0, 2 * state, s->stream));
+  }
   const size_t bytes = state * (per_step * (size_t)nsteps + 1);
   if (!s->tape || s->tape_bytes < bytes) {  // the tape is kept between calls and only ever grows
     cudaFree(s->tape);
@@ -916,6 +924,17 @@ int record_common(jxs_solver* s, void* U, double dt, int nsteps) {
     prepare_step_kernel<<<1, 1, 0, s->stream>>>(s->d_state, 0, 0.0, dt);
     s->launches++;
     CU(cudaGetLastError());
+    if (ckpt) {  // SSP-RK3 with only U^n kept: the two inner stage states live in scratch and are recomputed later
+      void* S0 = compact_state(s, s->ckpt, 0);
+      void* S1 = compact_state(s, s->ckpt, 1);
+      CU(ghost_fill(s, T(n)));
+      CU(stage(s, T(n), nullptr, S0, 0, 0.0, 1.0, nullptr));
+      CU(ghost_fill(s, S0));
+      CU(stage(s, S0, T(n), S1, 0, 0.75, 0.25, nullptr));
+      CU(ghost_fill(s, S1));
+      CU(stage(s, S1, T(n), T(n + 1), 0, 1.0 / 3.0, 2.0 / 3.0, nullptr));
+      continue;
+    }
     if (per_step == 1) {  // forward Euler (Eq. 10)
       CU(ghost_fill(s, T(n)));
       CU(stage(s, T(n), nullptr, T(n + 1), 0, 0.0, 1.0, nullptr));
@@ -933,6 +952,7 @@ int record_common(jxs_solver* s, void* U, double dt, int nsteps) {
   if (rc != JXS_OK) return rc;
   s->tape_steps = nsteps;
   s->tape_scheme = s->scheme;
+  s->tape_ckpt = ckpt;
   s->tape_dt = dt;
   return JXS_OK;
 }
@@ -984,6 +1004,21 @@ int adjoint_common(jxs_solver* s, void* Ubar, double* gamma_bar) {
   s->events_used = 0;
   int x = 0;  // which adjoint state holds the adjoint of U^{n+1}
   for (long long n = s->tape_steps - 1; n >= 0; --n) {
+    if (s->tape_ckpt) {  // recompute the step's inner stage states from the kept U^n, then reverse the three stages
+      double* S0 = compact_state(s, s->ckpt, 0);
+      double* S1 = compact_state(s, s->ckpt, 1);
+      CU(cudaMemcpyAsync(&s->d_state->dt, &s->tape_dt, sizeof(double), cudaMemcpyHostToDevice, s->stream));
+      CU(stage(s, T(n), nullptr, S0, 0, 0.0, 1.0, nullptr));
+      CU(ghost_fill(s, S0));
+      CU(stage(s, S0, T(n), S1, 0, 0.75, 0.25, nullptr));
+      CU(ghost_fill(s, S1));
+      const int y2 = (x + 1) & 3, y1 = (x + 2) & 3, y0 = (x + 3) & 3;
+      CU(adjoint_stage(s, S1, B(x), B(y2), 2.0 / 3.0, nullptr, 0.0, nullptr, 0.0));
+      CU(adjoint_stage(s, S0, B(y2), B(y1), 0.25, nullptr, 0.0, nullptr, 0.0));
+      CU(adjoint_stage(s, T(n), B(y1), B(y0), 1.0, B(x), 1.0 / 3.0, B(y2), 0.75));
+      x = y0;
+      continue;
+    }
     if (s->tape_scheme == JXS_EULER) {  // U^{n+1} = U^n + dt L(U^n)
       CU(adjoint_stage(s, T(n), B(x), B(x ^ 1), 1.0, nullptr, 0.0, nullptr, 0.0));
       x ^= 1;
@@ -1088,6 +1123,7 @@ void jxs_destroy(jxs_solver* s) {
   if (s->tan_exec) cudaGraphExecDestroy(s->tan_exec);
   cudaFree(s->d_mse);
   cudaFree(s->tape);
+  cudaFree(s->ckpt);
   cudaFree(s->adj);
   cudaFree(s->d_state);
   free_ibm(s);
@@ -1351,6 +1387,12 @@ int jxs_step_fixed_dt_tangent(jxs_solver* s, void* U, void* Udot, double gamma_d
 
 int jxs_step_fixed_dt_record(jxs_solver* s, void* U, double dt, int nsteps) { return record_common(s, U, dt, nsteps); }
 int jxs_adjoint_steps(jxs_solver* s, void* Ubar, double* gamma_bar) { return adjoint_common(s, Ubar, gamma_bar); }
+
+int jxs_set_adjoint_checkpointing(jxs_solver* s, int on) {
+  if (!s) return JXS_EINVAL;
+  s->checkpoint = on != 0;
+  return JXS_OK;
+}
 
 int jxs_mse_tangent(jxs_solver* s, const void* U, const void* Udot, const void* Utarget, double* loss, double* dloss) {
   if (!s) return JXS_EINVAL;

@@ -24,7 +24,8 @@ EXPORTS = ("jxs_create", "jxs_destroy", "jxs_last_error", "jxs_set_ibm", "jxs_se
            "jxs_stage_time", "jxs_ibm_ghost_count", "jxs_measure_fp64_peak", "jxs_flux_correction",
            "jxs_flux_mlp_time", "jxs_step_async", "jxs_wait", "jxs_set_time_integrator",
            "jxs_set_concurrent_handles", "jxs_set_flux_cnn", "jxs_flux_cnn_inputs",
-           "jxs_step_fixed_dt_tangent", "jxs_mse_tangent", "jxs_step_fixed_dt_record", "jxs_adjoint_steps", "jxs_set_gamma")
+           "jxs_step_fixed_dt_tangent", "jxs_mse_tangent", "jxs_step_fixed_dt_record", "jxs_adjoint_steps", "jxs_set_gamma",
+           "jxs_set_adjoint_checkpointing")
 
 
 class jxs_bc(C.Structure):
@@ -80,6 +81,7 @@ def lib():
         L.jxs_step_fixed_dt_record.argtypes = [vp, vp, C.c_double, C.c_int]
         L.jxs_adjoint_steps.argtypes = [vp, vp, dp]
         L.jxs_set_gamma.argtypes = [vp, C.c_double]
+        L.jxs_set_adjoint_checkpointing.argtypes = [vp, C.c_int]
         L.jxs_get_time.argtypes = [vp, dp, dp]
         L.jxs_launch_count.argtypes = [vp]
         L.jxs_launch_count.restype = C.c_longlong
@@ -268,6 +270,9 @@ class Solver:
 
     def set_gamma(self, gamma):
         self._chk(lib().jxs_set_gamma(self._h, float(gamma)))
+
+    def set_adjoint_checkpointing(self, on):
+        self._chk(lib().jxs_set_adjoint_checkpointing(self._h, int(bool(on))))
 
     def step_fixed_dt_record(self, U, dt, nsteps):
         """jxs_step_fixed_dt that keeps the trajectory for adjoint_steps (one-dimensional fp64 Euler handles)."""

@@ -103,6 +103,21 @@ def test_adjoint_pairs_with_the_tangent_kernel(nx, nsteps):
     assert s2.adjoint_steps(B2) == gbar and np.array_equal(B2.cpu().numpy(), got)
 
 
+def test_checkpointed_recording_gives_the_same_adjoint_bit_for_bit():
+    case = smooth1d(3000, 1e-5, dict(PER, xlo="inflow", xhi="transmissive", inflow=(1.0, 0.4, 0.0, 1.0)))
+    dt = 0.2 * case["dx"]   # (mu small enough for the explicit viscous step at this dx)
+    Ubar = np.random.default_rng(5).normal(size=case["U0"].shape)
+    U, full, gfull, s = gpu_adjoint(case, Ubar, dt, 12)
+    s.step_fixed_dt(dev(case["U0"]), 0.5 * dt, 3)        # another call in between must not disturb the reverse sweep
+    s.set_adjoint_checkpointing(True)
+    U2, B = dev(case["U0"]), dev(Ubar)
+    s.step_fixed_dt_record(U2, dt, 12)
+    s.step_fixed_dt(dev(case["U0"]), 0.5 * dt, 3)
+    g = s.adjoint_steps(B)
+    assert np.isfinite(full).all() and np.abs(full).max() > 0.1
+    assert np.array_equal(U2.cpu().numpy(), U) and np.array_equal(B.cpu().numpy(), full) and g == gfull
+
+
 def test_loss_gradient_by_backpropagation_equals_forward_mode():
     """dL/dgamma of Eq. 14 for the Sod inference, initial condition given in primitives (R23)"""
     nx, ns, g = 500, 60, 1.3
