@@ -167,6 +167,18 @@ int jxs_mse_tangent(jxs_solver*, const void* U, const void* Udot, const void* Ut
  * synchronise the stream.                                                                                         */
 int jxs_step_fixed_dt_record(jxs_solver*, void* U, double dt, int nsteps);
 int jxs_adjoint_steps(jxs_solver*, void* Ubar, double* gamma_bar);
+/* One-dimensional handles accept jxs_set_flux_mlp as well ("For the one-dimensional Sod shock-tube
+ * simulation, a multilayer perceptron (MLP) network is used to predict the neural flux"): same parameters, input
+ * and output conventions as in 2D (R14), evaluated per face in fp64 and added to the HLLC flux of every stage (Eq. 11)
+ * by all the stepping calls, jxs_rhs and jxs_step_fixed_dt_record.  jxs_adjoint_steps then also differentiates
+ * through the network — its input's dependence on the state and on gamma enters Ubar and *gamma_bar — and accumulates
+ * the weights' gradient (Eq. 16), which jxs_flux_mlp_gradient copies out:
+ *   grad  HOST, 6020 doubles in the order of the weights: d<Ubar on entry, U^{n+m}>/d(theta) of the last
+ *         jxs_adjoint_steps call (zero before any).  Sums over faces use fp64 atomics: reproducible to round-off.
+ * JXS_ESTATE without a flux MLP on a one-dimensional handle, JXS_EINVAL for NULL.  The forward-mode tangent does not
+ * cover the network (JXS_ESTATE).                                                                                  */
+int jxs_flux_mlp_gradient(jxs_solver*, double* grad);
+
 /* Checkpointing of the recording (default off): with on != 0 an SSP-RK3 recording keeps only U^n of every step (32 nx
  * bytes per step instead of 96) and jxs_adjoint_steps recomputes the two inner stage states of a step before it
  * reverses them: one third of the memory for two more stage launches per step, bit-identical results.  Applies to

@@ -29,6 +29,7 @@ struct Adjoint1dArgs {
   double* Ubar_in;         // adjoint of the stage's input, same layout, ghost columns included
   const double* E1;        // optional: Ubar_in += e1 E1 + e2 E2 on interior cells (the a U0 terms of later stages)
   const double* E2;
+  const double* Wmlp;      // optional: adjoint of the primitives through the network input (mlp1d_backward_kernel)
   double* gbar_partial;    // [gridDim.x] this launch's contributions to gamma_bar
   double dt;               // the step size (a constant of the differentiation)
   long long plane;         // pitch (compact layout)
@@ -331,6 +332,10 @@ __global__ void __launch_bounds__(A1D_TB) adjoint1d_kernel(const Adjoint1dArgs A
     for (int k = 0; k < 4; ++k)
       Wb[k] = con[k][0][t + 2] + con[k][1][t + 1] + con[k][2][t] + con[k][3][t - 1] + con[k][4][t - 2] +
               (NS ? vo[k] + visN[k][t] : 0.0);
+    if (A.Wmlp) {
+#pragma unroll
+      for (int k = 0; k < 4; ++k) Wb[k] += A.Wmlp[k * A.plane + pc];
+    }
     const double r = wc[0], u = wc[1], v = wc[2], p = wc[3], ri = rcp_(r);
     // u = ru / r, v = rv / r, p = g1 (E - (ru u + rv v) / 2)
     double out[4];

@@ -22,6 +22,7 @@
 #include "stage1d_kernel.cuh"
 #include "tangent1d_kernel.cuh"
 #include "adjoint1d_kernel.cuh"
+#include "mlp1d_kernel.cuh"
 
 using namespace jxs;
 
@@ -50,6 +51,13 @@ struct jxs_solver {
   // jxs_step_fixed_dt_tangent call; d_mse = partial sums and result of jxs_mse_tangent
   void* bufd[3] = {nullptr, nullptr, nullptr};
   double* d_mse = nullptr;
+  // per-face MLP flux of one-dimensional problems (mlp1d_kernel.cuh): parameters, flux corrections, and for the
+  // reverse sweep the weights' gradient and the adjoint of the primitives through the network input
+  bool mlp1d_on = false;
+  double* d_theta = nullptr;
+  double* d_dF1d = nullptr;
+  double* d_theta_bar = nullptr;
+  double* d_Wmlp = nullptr;
   cudaGraphExec_t tan_exec = nullptr;  // one tangent step (10 launches), replayed: small grids are launch-bound
   double tan_dt = 0, tan_gdot = 0;
   long long tan_launches = 0;
@@ -261,6 +269,7 @@ cudaError_t launch_stage(jxs_solver* s, const void* Uin, const void* U0, void* U
   A.dF = (s->mlp_on || s->cnn_on) ? s->d_dF : nullptr;
   A.dG = (s->mlp_on || s->cnn_on) ? s->d_dG : nullptr;
   for (int k = 0; k < 4; ++k) A.oscale[k] = (T)s->out_scale[k];
+  A.dF1d = s->mlp1d_on ? s->d_dF1d : nullptr;
   const bool visc = s->mu > 0, artv = s->nu > 0;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (s->profiling && mode == 0 && s->events_used + 2 <= (int)s->events.size()) {
@@ -417,7 +426,23 @@ cudaError_t launch_flux_cnn(jxs_solver* s, const void* U) {
   }
   return e;
 }
+Mlp1dArgs mlp1d_args(const jxs_solver* s, const void* U) {
+  Mlp1dArgs A{};
+  A.U = U; A.theta = s->d_theta; A.dF = s->d_dF1d; A.plane = s->plane; A.nx = s->nx; A.pitch = s->pitch;
+  A.g1 = s->gamma - 1.0;
+  for (int k = 0; k < 4; ++k) { A.inv_in[k] = 1.0 / s->in_scale[k]; A.out_scale[k] = s->out_scale[k]; }
+  return A;
+}
+int mlp1d_grid(const jxs_solver* s) { return std::min((s->nx + 1 + 3) / 4, s->num_sms * 16); }
+
 cudaError_t flux_mlp(jxs_solver* s, const void* U) {  // whichever network is set
+  if (s->mlp1d_on) {  // one-dimensional problems: mlp1d_kernel.cuh, one warp per face
+    const Mlp1dArgs A = mlp1d_args(s, U);
+    if (s->dtype == JXS_F64) mlp1d_kernel<double><<<mlp1d_grid(s), 128, 0, s->stream>>>(A);
+    else mlp1d_kernel<float><<<mlp1d_grid(s), 128, 0, s->stream>>>(A);
+    s->launches++;
+    return cudaGetLastError();
+  }
   if (s->cnn_on) {  // jxs_flux_mlp_time then reports the whole network pass (reconstruction + 6 layer launches)
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (s->profiling && s->mlp_events_used + 2 <= (int)s->mlp_events.size()) {
@@ -818,7 +843,7 @@ int tangent_common(jxs_solver* s, void* U, void* Udot, double gamma_dot, double 
   if (!std::isfinite(gamma_dot)) return fail(s, JXS_EINVAL, "gamma_dot is not finite");
   if (s->dtype != JXS_F64) return fail(s, JXS_EINVAL, "the tangent is fp64 only");
   if (s->ny != 1) return fail(s, JXS_EINVAL, "the tangent is built for one-dimensional problems (ny = 1)");
-  if (s->mlp_on || s->cnn_on) return fail(s, JXS_ESTATE, "the tangent does not differentiate the networks");
+  if (s->mlp_on || s->cnn_on || s->mlp1d_on) return fail(s, JXS_ESTATE, "the tangent does not differentiate the networks");
   if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
   const size_t bytes = (size_t)4 * s->plane * s->elem;
   for (int b = 0; b < 3; ++b)
@@ -883,7 +908,6 @@ double* compact_state(const jxs_solver* s, double* base, long long i) {
 int adjoint_checks(jxs_solver* s) {
   if (s->dtype != JXS_F64) return fail(s, JXS_EINVAL, "the adjoint is fp64 only");
   if (s->ny != 1) return fail(s, JXS_EINVAL, "the adjoint is built for one-dimensional problems (ny = 1)");
-  if (s->mlp_on || s->cnn_on) return fail(s, JXS_ESTATE, "the adjoint does not differentiate the networks");
   if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
   return JXS_OK;
 }
@@ -928,23 +952,30 @@ int record_common(jxs_solver* s, void* U, double dt, int nsteps) {
       void* S0 = compact_state(s, s->ckpt, 0);
       void* S1 = compact_state(s, s->ckpt, 1);
       CU(ghost_fill(s, T(n)));
+      CU(flux_mlp(s, T(n)));
       CU(stage(s, T(n), nullptr, S0, 0, 0.0, 1.0, nullptr));
       CU(ghost_fill(s, S0));
+      CU(flux_mlp(s, S0));
       CU(stage(s, S0, T(n), S1, 0, 0.75, 0.25, nullptr));
       CU(ghost_fill(s, S1));
+      CU(flux_mlp(s, S1));
       CU(stage(s, S1, T(n), T(n + 1), 0, 1.0 / 3.0, 2.0 / 3.0, nullptr));
       continue;
     }
     if (per_step == 1) {  // forward Euler (Eq. 10)
       CU(ghost_fill(s, T(n)));
+      CU(flux_mlp(s, T(n)));
       CU(stage(s, T(n), nullptr, T(n + 1), 0, 0.0, 1.0, nullptr));
       continue;
     }
     CU(ghost_fill(s, T(3 * n)));
+    CU(flux_mlp(s, T(3 * n)));
     CU(stage(s, T(3 * n), nullptr, T(3 * n + 1), 0, 0.0, 1.0, nullptr));
     CU(ghost_fill(s, T(3 * n + 1)));
+    CU(flux_mlp(s, T(3 * n + 1)));
     CU(stage(s, T(3 * n + 1), T(3 * n), T(3 * n + 2), 0, 0.75, 0.25, nullptr));
     CU(ghost_fill(s, T(3 * n + 2)));
+    CU(flux_mlp(s, T(3 * n + 2)));
     CU(stage(s, T(3 * n + 2), T(3 * n), T(3 * n + 3), 0, 1.0 / 3.0, 2.0 / 3.0, nullptr));
   }
   CU(unpad(s, T((long long)per_step * nsteps), U));
@@ -967,6 +998,16 @@ cudaError_t adjoint_stage(jxs_solver* s, const double* U, const double* out, dou
   A.dt = s->tape_dt; A.plane = s->pitch; A.nx = s->nx; A.pitch = s->pitch;
   A.gamma = s->gamma; A.dxi = 1.0 / s->dx; A.b = b; A.e1 = e1; A.e2 = e2;
   A.mu = s->mu; A.Pr = s->Pr; A.nu = s->nu;
+  A.Wmlp = nullptr;
+  if (s->mlp1d_on) {  // the network's reverse first: weights' gradient, and the adjoint of its input for the kernel below
+    Mlp1dArgs M = mlp1d_args(s, U);  // (compact layout: U is the virtual pointer 3 rows before the state)
+    M.Ubar_out = out; M.Wbar = s->d_Wmlp; M.theta_bar = s->d_theta_bar; M.bdt = b * s->tape_dt; M.dxi = 1.0 / s->dx;
+    cudaError_t e = cudaMemsetAsync(s->d_Wmlp, 0, (size_t)4 * 4 * s->pitch * sizeof(double), s->stream);
+    if (e != cudaSuccess) return e;
+    mlp1d_backward_kernel<<<mlp1d_grid(s), 128, 0, s->stream>>>(M);
+    s->launches++;
+    A.Wmlp = s->d_Wmlp + 3 * (long long)s->pitch;
+  }
   cudaEvent_t e0 = nullptr, e1v = nullptr;
   if (s->profiling && s->events_used + 2 <= (int)s->events.size()) {
     e0 = s->events[s->events_used++];
@@ -1001,6 +1042,7 @@ int adjoint_common(jxs_solver* s, void* Ubar, double* gamma_bar) {
   auto T = [&](long long i) { return compact_state(s, s->tape, i); };
   auto B = [&](int i) { return compact_state(s, s->adj, i); };
   CU(pad(s, Ubar, B(0)));
+  if (s->mlp1d_on) CU(cudaMemsetAsync(s->d_theta_bar, 0, MLP1D_NPARAM * sizeof(double), s->stream));
   s->events_used = 0;
   int x = 0;  // which adjoint state holds the adjoint of U^{n+1}
   for (long long n = s->tape_steps - 1; n >= 0; --n) {
@@ -1008,8 +1050,10 @@ int adjoint_common(jxs_solver* s, void* Ubar, double* gamma_bar) {
       double* S0 = compact_state(s, s->ckpt, 0);
       double* S1 = compact_state(s, s->ckpt, 1);
       CU(cudaMemcpyAsync(&s->d_state->dt, &s->tape_dt, sizeof(double), cudaMemcpyHostToDevice, s->stream));
+      CU(flux_mlp(s, T(n)));
       CU(stage(s, T(n), nullptr, S0, 0, 0.0, 1.0, nullptr));
       CU(ghost_fill(s, S0));
+      CU(flux_mlp(s, S0));
       CU(stage(s, S0, T(n), S1, 0, 0.75, 0.25, nullptr));
       CU(ghost_fill(s, S1));
       const int y2 = (x + 1) & 3, y1 = (x + 2) & 3, y0 = (x + 3) & 3;
@@ -1122,6 +1166,7 @@ void jxs_destroy(jxs_solver* s) {
   for (int b = 0; b < 3; ++b) cudaFree(s->bufd[b]);
   if (s->tan_exec) cudaGraphExecDestroy(s->tan_exec);
   cudaFree(s->d_mse);
+  cudaFree(s->d_theta); cudaFree(s->d_dF1d); cudaFree(s->d_theta_bar); cudaFree(s->d_Wmlp);
   cudaFree(s->tape);
   cudaFree(s->ckpt);
   cudaFree(s->adj);
@@ -1223,8 +1268,7 @@ int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[
   if (!s) return JXS_EINVAL;
   drop_graph(s);
   CU(cudaStreamSynchronize(s->stream));
-  if (!weights) { s->mlp_on = false; return JXS_OK; }
-  if (s->ny == 1) return fail(s, JXS_EINVAL, "no flux MLP in one-dimensional problems");
+  if (!weights) { s->mlp_on = false; s->mlp1d_on = false; s->tape_steps = 0; return JXS_OK; }
   if (s->cnn_on) return fail(s, JXS_ESTATE, "the CNN flux is set: disable it first (jxs_set_flux_cnn(NULL))");
   if (!in_scale || !out_scale) return fail(s, JXS_EINVAL, "in_scale / out_scale is NULL");
   for (int k = 0; k < 4; ++k)
@@ -1232,6 +1276,21 @@ int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[
       return fail(s, JXS_EINVAL, "in_scale must be > 0 and out_scale finite");
   for (int i = 0; i < 6020; ++i)
     if (!std::isfinite(weights[i])) return fail(s, JXS_EINVAL, "non-finite MLP weight");
+  if (s->ny == 1) {  // one-dimensional problems: the fp64 per-face MLP of mlp1d_kernel.cuh
+    std::vector<double> th(MLP1D_NPARAM);
+    for (int i = 0; i < MLP1D_NPARAM; ++i) th[i] = (double)weights[i];
+    const size_t fbytes = (size_t)4 * s->plane * sizeof(double);
+    if (!s->d_theta) CU(cudaMalloc(&s->d_theta, MLP1D_NPARAM * sizeof(double)));
+    if (!s->d_theta_bar) CU(cudaMalloc(&s->d_theta_bar, MLP1D_NPARAM * sizeof(double)));
+    if (!s->d_dF1d) { CU(cudaMalloc(&s->d_dF1d, fbytes)); CU(cudaMemset(s->d_dF1d, 0, fbytes)); }
+    if (!s->d_Wmlp) { CU(cudaMalloc(&s->d_Wmlp, fbytes)); CU(cudaMemset(s->d_Wmlp, 0, fbytes)); }
+    CU(cudaMemcpy(s->d_theta, th.data(), MLP1D_NPARAM * sizeof(double), cudaMemcpyHostToDevice));
+    CU(cudaMemset(s->d_theta_bar, 0, MLP1D_NPARAM * sizeof(double)));
+    for (int k = 0; k < 4; ++k) { s->in_scale[k] = in_scale[k]; s->out_scale[k] = out_scale[k]; }
+    s->mlp1d_on = true;
+    s->tape_steps = 0;
+    return JXS_OK;
+  }
   // W1[64][24], b1[64], W2[64][64], b2[64], W3[4][64], b3[4] -> bf16 tiles in the tensor-core layout + fp32 biases
   std::vector<uint8_t> blob(MLP_BLOB, 0);
   const float *W1 = weights, *b1 = W1 + 64 * 24, *W2 = b1 + 64, *b2 = W2 + 64 * 64, *W3 = b2 + 64, *b3 = W3 + 4 * 64;
@@ -1387,6 +1446,15 @@ int jxs_step_fixed_dt_tangent(jxs_solver* s, void* U, void* Udot, double gamma_d
 
 int jxs_step_fixed_dt_record(jxs_solver* s, void* U, double dt, int nsteps) { return record_common(s, U, dt, nsteps); }
 int jxs_adjoint_steps(jxs_solver* s, void* Ubar, double* gamma_bar) { return adjoint_common(s, Ubar, gamma_bar); }
+
+int jxs_flux_mlp_gradient(jxs_solver* s, double* grad) {
+  if (!s) return JXS_EINVAL;
+  if (!grad) return fail(s, JXS_EINVAL, "grad is NULL");
+  if (!s->mlp1d_on) return fail(s, JXS_ESTATE, "no flux MLP set on a one-dimensional handle");
+  CU(cudaMemcpyAsync(grad, s->d_theta_bar, MLP1D_NPARAM * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+  CU(cudaStreamSynchronize(s->stream));
+  return JXS_OK;
+}
 
 int jxs_set_adjoint_checkpointing(jxs_solver* s, int on) {
   if (!s) return JXS_EINVAL;

@@ -97,6 +97,11 @@ __global__ void __launch_bounds__(S1D_TB) stage1d_kernel(const StageArgs<T> A) {
       viscous_n<T, N>(dn, dt_, zero, zero, sn, st, dT, cn, cc, cs, ct, cq, f1, f2, f3);
     }
     F[0] = f0[0]; F[1] = f1[0]; F[2] = f2[0]; F[3] = f3[0];
+    if (A.dF1d) {  // Eq. 11: + F^Neural of this face (mlp1d_kernel.cuh)
+      const size_t o = 3 * (size_t)A.pitch + min(col, A.pitch - 1);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) F[k] += T(A.dF1d[k * A.plane + o]);
+    }
 #pragma unroll
     for (int k = 0; k < 4; ++k) fS[k][t] = F[k];
   }

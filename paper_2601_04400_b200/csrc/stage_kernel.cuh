@@ -65,6 +65,9 @@ struct StageArgs {
   const float* dF;
   const float* dG;
   T oscale[4];
+  // one-dimensional problems (stage1d_kernel.cuh): the per-face MLP's flux correction from mlp1d_kernel.cuh, already
+  // scaled, indexed like U (right face of the cell); nullptr = none
+  const double* dF1d;
 };
 
 

@@ -25,7 +25,7 @@ EXPORTS = ("jxs_create", "jxs_destroy", "jxs_last_error", "jxs_set_ibm", "jxs_se
            "jxs_flux_mlp_time", "jxs_step_async", "jxs_wait", "jxs_set_time_integrator",
            "jxs_set_concurrent_handles", "jxs_set_flux_cnn", "jxs_flux_cnn_inputs",
            "jxs_step_fixed_dt_tangent", "jxs_mse_tangent", "jxs_step_fixed_dt_record", "jxs_adjoint_steps", "jxs_set_gamma",
-           "jxs_set_adjoint_checkpointing")
+           "jxs_set_adjoint_checkpointing", "jxs_flux_mlp_gradient")
 
 
 class jxs_bc(C.Structure):
@@ -82,6 +82,7 @@ def lib():
         L.jxs_adjoint_steps.argtypes = [vp, vp, dp]
         L.jxs_set_gamma.argtypes = [vp, C.c_double]
         L.jxs_set_adjoint_checkpointing.argtypes = [vp, C.c_int]
+        L.jxs_flux_mlp_gradient.argtypes = [vp, vp]
         L.jxs_get_time.argtypes = [vp, dp, dp]
         L.jxs_launch_count.argtypes = [vp]
         L.jxs_launch_count.restype = C.c_longlong
@@ -270,6 +271,13 @@ class Solver:
 
     def set_gamma(self, gamma):
         self._chk(lib().jxs_set_gamma(self._h, float(gamma)))
+
+    def flux_mlp_gradient(self):
+        """The weights' gradient accumulated by the last adjoint_steps (one-dimensional handles), float64[6020]."""
+        import numpy as np
+        g = np.zeros(6020)
+        self._chk(lib().jxs_flux_mlp_gradient(self._h, g.ctypes.data))
+        return g
 
     def set_adjoint_checkpointing(self, on):
         self._chk(lib().jxs_set_adjoint_checkpointing(self._h, int(bool(on))))

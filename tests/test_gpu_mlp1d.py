@@ -1,0 +1,104 @@
+"""The per-face MLP neural flux of one-dimensional problems (Fig. 1b; Eq. 11) and its training gradient
+(Eq. 14-16): mlp1d_kernel.cuh through the C ABI.  -m gpu.
+
+* forward: RHS and steps against the oracle's exact (fp64) MLP mode on the planar problem of 8 identical rows (the
+  y-face corrections of identical rows cancel in the divergence): <= 1e-12 / <= 1e-9;
+* reverse: phi = <c, S^n(U0; theta)> has gradient (J^T c, dphi/dtheta); the adjoint of the state and the weights'
+  gradient against central differences of the ORACLE's primal run at sampled entries (the oracle's network is not
+  differentiated, SURVEY 8(f) rank 3 says as much: "finite differences"): 1e-5 of the gradient's scale.
+"""
+import numpy as np
+import pytest
+
+from oracle import jxo
+from paper_2601_04400_b200 import workloads as wl
+from test_gpu_parity import dev, jxs, rel_err
+from test_gpu_tangent import PER, smooth1d
+
+pytestmark = pytest.mark.gpu
+
+W = wl.mlp_weights(7)
+SC = wl.mlp_scales(out_factor=5e-2)   # corrections of a few per cent of the flux: the network matters
+
+
+def oracle_rows(case, w=W):
+    c = wl.as_rows(case)
+    o = jxo.Oracle(c["nx"], c["ny"], c["dx"], c["dy"], c["gamma"], c["mu"], c["Pr"], c["bc"])
+    o.set_flux_mlp(w, *SC, emulate_bf16=False)
+    return c, o
+
+
+def gpu(case, w=W):
+    s = jxs().Solver.from_case(case)
+    s.set_flux_mlp(w, *SC)
+    return s
+
+
+@pytest.mark.parametrize("nx,bc", [(100, None), (255, dict(PER)), (381, dict(PER, xlo="reflective", xhi="transmissive"))])
+def test_mlp1d_forward_matches_the_exact_oracle_mlp(nx, bc):
+    case = wl.sod1d(nx) if bc is None else smooth1d(nx, 1e-4, bc)
+    c2, o = oracle_rows(case)
+    s = gpu(case)
+    got = s.rhs(dev(case["U0"])).cpu().numpy()
+    want = o.rhs(c2["U0"])[:, :1]
+    assert rel_err(got, want) <= 1e-12
+    plain = jxs().Solver.from_case(case).rhs(dev(case["U0"])).cpu().numpy()
+    assert rel_err(got, plain) > 1e-4                      # the network does change the result
+    U = dev(case["U0"])
+    s.step(U, 0.3, 25)
+    assert rel_err(U.cpu().numpy(), o.step(c2["U0"], 0.3, 25)[:, :1]) <= 1e-9
+    s.set_flux_mlp(None)
+    assert np.array_equal(s.rhs(dev(case["U0"])).cpu().numpy(), plain)
+
+
+def test_mlp1d_training_gradient_against_differences_of_the_oracle():
+    nx, ns = 96, 2
+    case = smooth1d(nx, 0.0, dict(PER, xlo="transmissive", xhi="transmissive"))
+    dt = 0.2 * case["dx"]
+    rng = np.random.default_rng(4)
+    c = rng.normal(size=case["U0"].shape)
+    s = gpu(case)
+    U, B = dev(case["U0"]), dev(c)
+    s.step_fixed_dt_record(U, dt, ns)
+    c2, o = oracle_rows(case)
+    assert rel_err(U.cpu().numpy(), o.step_fixed_dt(c2["U0"], dt, ns)[:, :1]) <= 1e-12
+    gbar = s.adjoint_steps(B)
+    grad_u, grad_w = B.cpu().numpy(), s.flux_mlp_gradient()
+    assert np.isfinite(grad_w).all() and np.abs(grad_w).max() > 0
+
+    def phi(U0, w=W, gamma=None):
+        cc = dict(case, U0=U0) if gamma is None else dict(case, U0=U0, gamma=gamma)
+        c3, oo = oracle_rows(cc, w)
+        return float(np.sum(c * oo.step_fixed_dt(c3["U0"], dt, ns)[:, :1]))
+
+    # the weights: perturb the float32 parameter and divide by the step actually taken
+    scale = np.abs(grad_w).max()
+    picks = [0, 5, 24 * 31 + 7, 1536 + 3, 1600 + 64 * 10 + 20, 1600 + 64 * 63 + 63, 5696 + 40, 5760 + 64 + 9, 6016 + 2]
+    picks += [int(j) for j in rng.integers(0, 6020, 8)]
+    for j in picks:
+        wp, wm = W.copy(), W.copy()
+        h = np.float32(max(abs(W[j]), 0.05) * 2e-3)
+        wp[j] += h
+        wm[j] -= h
+        fd = (phi(case["U0"], wp) - phi(case["U0"], wm)) / (float(wp[j]) - float(wm[j]))
+        assert abs(grad_w[j] - fd) <= 1e-5 * scale + 1e-6 * abs(fd), (j, grad_w[j], fd)
+    # the state, through the solver and through the network's input
+    h = 1e-6
+    for j in rng.choice(c.size, 10, replace=False):
+        e = np.zeros(c.shape)
+        e.flat[j] = 1.0
+        fd = (phi(case["U0"] + h * e) - phi(case["U0"] - h * e)) / (2 * h)
+        assert grad_u.flat[j] == pytest.approx(fd, rel=2e-5, abs=1e-7 * np.abs(grad_u).max())
+    # gamma (the network's pressure input depends on it too)
+    fd = (phi(case["U0"], gamma=1.4 + h) - phi(case["U0"], gamma=1.4 - h)) / (2 * h)
+    assert gbar == pytest.approx(fd, rel=2e-5)
+
+
+def test_mlp1d_rejects_what_it_does_not_do():
+    case = wl.sod1d(64)
+    s = gpu(case)
+    with pytest.raises(jxs().JxsError):
+        s.step_fixed_dt_tangent(dev(case["U0"]), dev(case["U0"]), 1.0, 1e-3, 1)   # forward mode: no network
+    s2 = jxs().Solver.from_case(case)
+    with pytest.raises(jxs().JxsError):
+        s2.flux_mlp_gradient()

@@ -162,4 +162,4 @@ def test_1d_rejects_what_it_does_not_do():
     with pytest.raises(jxs().JxsError):
         s.set_ibm(-np.ones((1, 64)))
     with pytest.raises(jxs().JxsError):
-        s.set_flux_mlp(wl.mlp_weights(), *wl.mlp_scales())
+        s.set_flux_cnn(wl.cnn_weights(), *wl.cnn_scales())
