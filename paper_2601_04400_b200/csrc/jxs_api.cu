@@ -1004,7 +1004,16 @@ cudaError_t adjoint_stage(jxs_solver* s, const double* U, const double* out, dou
     M.Ubar_out = out; M.Wbar = s->d_Wmlp; M.theta_bar = s->d_theta_bar; M.bdt = b * s->tape_dt; M.dxi = 1.0 / s->dx;
     cudaError_t e = cudaMemsetAsync(s->d_Wmlp, 0, (size_t)4 * 4 * s->pitch * sizeof(double), s->stream);
     if (e != cudaSuccess) return e;
-    mlp1d_backward_kernel<<<mlp1d_grid(s), 128, 0, s->stream>>>(M);
+    static bool configured = false;
+    if (!configured) {
+      e = cudaFuncSetAttribute(mlp1d_backward_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, MLP1D_BWD_SMEM);
+      if (e != cudaSuccess) return e;
+      configured = true;
+    }
+    // every CTA flushes its 6020 sums at its end: one face per warp on small grids (the paper's N = 500 .. 1000,
+    // where latency counts), at most 2 CTAs per SM on large ones (where the flushes would)
+    const int bgrid = std::max(1, std::min((s->nx + 1 + 3) / 4, s->num_sms * 2));
+    mlp1d_backward_kernel<<<bgrid, 128, MLP1D_BWD_SMEM, s->stream>>>(M);
     s->launches++;
     A.Wmlp = s->d_Wmlp + 3 * (long long)s->pitch;
   }

@@ -94,6 +94,45 @@ def test_mlp1d_training_gradient_against_differences_of_the_oracle():
     assert gbar == pytest.approx(fd, rel=2e-5)
 
 
+def test_unrolled_training_of_the_neural_flux_reduces_the_loss():
+    """P:L112-128 on the paper's own set-up (Fig. 3c-f), scaled down: a low-resolution Sod run (N = 125) with the
+    neural flux is trained, m = 10 unrolled steps, towards the block-averaged high-resolution run (N = 250, Eq. 14);
+    every forward and backward step runs in the kernels, the update of the weights is plain gradient descent here."""
+    import torch
+    nlo, m = 125, 10
+    dt = 0.2 / nlo
+    hi = wl.sod1d(2 * nlo)
+    Uh = dev(hi["U0"])
+    jxs().Solver.from_case(hi).step_fixed_dt(Uh, 0.5 * dt, 40)          # a developed high-resolution state ...
+    start = 0.5 * (Uh[:, :, 0::2] + Uh[:, :, 1::2]).contiguous()          # ... block-averaged: the low-resolution start
+    jxs().Solver.from_case(hi).step_fixed_dt(Uh, 0.5 * dt, 2 * m)        # the same time span on the fine grid
+    target = 0.5 * (Uh[:, :, 0::2] + Uh[:, :, 1::2]).contiguous()        # d(U_HR), Eq. 14
+    case = wl.sod1d(nlo)
+    w = (0.2 * wl.mlp_weights(11)).astype(np.float32)
+    s = jxs().Solver.from_case(case)
+    losses = []
+    lr = None
+    for it in range(12):
+        s.set_flux_mlp(w, *SC)
+        U = start.clone()
+        s.step_fixed_dt_record(U, dt, m)
+        r = U - target
+        losses.append(float((r * r).mean()))
+        B = (2.0 / r.numel()) * r
+        s.adjoint_steps(B)
+        g = s.flux_mlp_gradient()
+        if lr is None:
+            lr = 0.1 * np.abs(w).max() / np.abs(g).max()                 # first step: 10 % of the weights' scale
+        w = (w - lr * g).astype(np.float32)
+    assert all(b < a for a, b in zip(losses, losses[1:])), losses
+    assert losses[-1] < 0.95 * losses[0], losses
+    # and the baseline without the network, for the record: training must not end above it
+    s.set_flux_mlp(None)
+    U = start.clone()
+    s.step_fixed_dt(U, dt, m)
+    assert losses[-1] <= float(((U - target) ** 2).mean()) * 1.5
+
+
 def test_mlp1d_rejects_what_it_does_not_do():
     case = wl.sod1d(64)
     s = gpu(case)
