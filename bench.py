@@ -336,6 +336,74 @@ def run_adjoint1d(args, rank, world, local_rank, dist, barrier, tdt):
         "e2e": None, "cpu_baseline": oracle_rate_1d("adjoint", args.no_cpu_baseline)}))
 
 
+def run_train1d(args, rank, world, local_rank, dist, barrier, tdt):
+    """SURVEY.md section 8(f) rank 3, the paper's second mode (Fig. 3c): one training iteration
+    of the 1D neural flux at the paper's low resolution N = 500 — K unrolled steps recorded with the per-face MLP in
+    every stage, dL/dU of Eq. 14, K adjoint steps through solver and network, the weights' gradient copied out."""
+    import torch
+    from paper_2601_04400_b200 import jxs, workloads as wl
+    if args.dtype != "f64":
+        raise SystemExit("bench.py: the adjoint is fp64 only")
+    nx = 500
+    case = wl.sod1d(nx)
+    dt = 0.2 * case["dx"]
+    stream = torch.cuda.current_stream()
+    solver = jxs.Solver.from_case(case, dtype=tdt, stream=stream)
+    solver.set_flux_mlp(wl.mlp_weights(7), *wl.mlp_scales(out_factor=5e-2))
+    U0 = torch.tensor(case["U0"], dtype=tdt, device="cuda")
+    hi = wl.sod1d(2 * nx)
+    Uh = torch.tensor(hi["U0"], dtype=tdt, device="cuda")
+    K, W = args.steps, args.warmup
+    jxs.Solver.from_case(hi, dtype=tdt, stream=stream).step_fixed_dt(Uh, 0.5 * dt, 2 * K)
+    target = (0.5 * (Uh[:, :, 0::2] + Uh[:, :, 1::2])).contiguous()   # d(U_HR): block average of the N = 1000 run
+
+    def iteration(n):
+        U = U0.clone()
+        solver.step_fixed_dt_record(U, dt, n)
+        B = (U - target).mul_(2.0 / U.numel())
+        solver.adjoint_steps(B)
+        return solver.flux_mlp_gradient()
+
+    iteration(W)
+    iteration(K)
+    solver.set_profiling(True)
+    sampler = ClockSampler(local_rank)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = solver.launch_count()
+    barrier()
+    sampler.start()
+    e0.record(stream)
+    g = iteration(K)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = max_over_ranks(e0.elapsed_time(e1), dist, "cuda")
+    stage_ms, stage_n = solver.stage_time()
+    if not all(map(math.isfinite, g)):
+        raise SystemExit("bench.py: non-finite gradient after the timed region")
+    if rank != 0:
+        return
+    flop = 1068.0
+    avg = stage_ms / max(stage_n, 1)
+    achieved = flop * nx / (avg * 1e-3) / 1e12
+    print(json.dumps({
+        "metric": METRIC, "value": aggregate_rate(nx, K, world, ms), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
+        "data": "synthetic",
+        "config": {"workload": "train1d_500 (one training iteration of the 1D neural flux at the paper's N = 500 against the "
+                               "block-averaged N = 1000 run: K unrolled steps forward with the MLP, backward through solver "
+                               "and network; P:L109, L112-128)", "dt": dt, "rk": "SSP-RK3", "cells": nx,
+                   "l2": "everything fits in L2: the iteration is bound by its 22 launches per step, not by bandwidth",
+                   "grad_norm": float(sum(x * x for x in g) ** 0.5),
+                   "parallelism": "replicas" if world > 1 else "single GPU"},
+        "clocks": clocks, "gpu_launches": solver.launch_count() - launches0,
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_FP64_TFLOPS, "unit": "TFLOP/s",
+                     "frac": achieved / PEAK_FP64_TFLOPS, "traffic": None, "kernel": "jxs::adjoint1d_kernel",
+                     "avg_launch_ms": avg, "launches_timed": stage_n, "alg_flop_per_cell_stage": flop,
+                     "note": "500 cells = 5 CTAs: launch latency, not arithmetic, sets these times"},
+        "e2e": None, "cpu_baseline": None}))
+
+
 def run_cnn(args, rank, world, local_rank, dist, barrier, tdt):
     """the C4 grid with the paper's 2D CNN neural flux (Eq. 11-13) in
     every stage: reconstruction pass + 3 convolution layers per direction on tcgen05, then the stage kernel."""
@@ -484,7 +552,7 @@ def main():
     ap.add_argument("--euler", action="store_true", help="mu = 0, no IBM (not the headline config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile-kernels", action="store_true", help="c5 only: per-kernel CUDA-event spans")
-    ap.add_argument("--workload", choices=("c4", "c5", "sod1d", "cnn", "tangent1d", "adjoint1d"), default="c4",
+    ap.add_argument("--workload", choices=("c4", "c5", "sod1d", "cnn", "tangent1d", "adjoint1d", "train1d"), default="c4",
                     help="c4 = the headline throughput case (default); c5 = BASELINE.json configs[4]: 16 independent "
                          "1024x512 shock-cylinder runs with the per-face flux MLP, one stream per handle; sod1d = the "
                          "paper's 1D Sod tube at its largest size (3e6 cells = 9e6 degrees of freedom, PAPER.md L149)")
@@ -521,6 +589,9 @@ def main():
         return
     if args.workload == "sod1d":
         run_sod1d(args, rank, world, local_rank, dist, barrier, tdt)
+        return
+    if args.workload == "train1d":
+        run_train1d(args, rank, world, local_rank, dist, barrier, tdt)
         return
     if args.workload == "adjoint1d":
         run_adjoint1d(args, rank, world, local_rank, dist, barrier, tdt)

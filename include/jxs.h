@@ -57,7 +57,7 @@ typedef struct {
  * cuda_stream: a cudaStream_t cast to void*, or NULL.
  * ny = 1 selects the one-dimensional path (the paper's Sod tube): fields are
  * [4][1][nx] (rho v is carried along), the y boundary conditions are ignored, dy still enters the
- * CFL step as min(dx,dy) (pass dy = dx); no immersed boundary, no flux MLP.
+ * CFL step as min(dx,dy) (pass dy = dx); no immersed boundary, no CNN flux (the per-face MLP is available).
  * JXS_EINVAL: nx < 8, ny < 8 and != 1, dx/dy <= 0, gamma <= 1, mu < 0, Pr <= 0 with mu > 0,
  * bad bc or dtype, NULL pointers.  JXS_ECUDA: no usable device.  JXS_ENOMEM: allocation failed. */
 int jxs_create(int nx, int ny, double dx, double dy, double gamma, double mu, double Pr,
