@@ -36,6 +36,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 namespace {
@@ -108,6 +109,7 @@ inline bool operator>(Dual a, Dual b) { return a.v > b.v; }
 inline bool operator<=(Dual a, Dual b) { return a.v <= b.v; }
 inline bool operator>=(Dual a, Dual b) { return a.v >= b.v; }
 inline Dual s_sqrt(Dual x) { const double r = std::sqrt(x.v); return Dual(r, x.d / (2.0 * r)); }
+inline Dual s_tanh(Dual x) { const double t = std::tanh(x.v); return Dual(t, (1.0 - t * t) * x.d); }
 inline Dual s_abs(Dual x) { return Dual(std::fabs(x.v), x.v > 0 ? x.d : (x.v < 0 ? -x.d : 0.0)); }
 inline double to_double(Dual x) { return x.v; }
 
@@ -203,6 +205,29 @@ struct Mlp {
   bool on = false, bf16 = false;
   std::vector<double> W1, b1, W2, b2, W3, b3;  // W1[64][24], W2[64][64], W3[4][64]
   double in_scale[4] = {1, 1, 1, 1}, out_scale[4] = {1, 1, 1, 1};
+  // direction of perturbation of the parameters for the tangent O12 (same layout; empty = the parameters do not move)
+  std::vector<double> dW1, db1, dW2, db2, dW3, db3;
+  // O10 on the dual scalar (exact mode only): the same three layers, every parameter carrying its direction
+  void eval_dual(const Dual x[24], Dual y[4]) const {
+    const bool dir = !dW1.empty();
+    auto par = [&](const std::vector<double>& w, const std::vector<double>& d, size_t i) { return Dual(w[i], dir ? d[i] : 0.0); };
+    Dual h1[64], h2[64];
+    for (int o = 0; o < 64; ++o) {
+      Dual s = par(b1, db1, o);
+      for (int k = 0; k < 24; ++k) s += par(W1, dW1, o * 24 + k) * x[k];
+      h1[o] = s_tanh(s);
+    }
+    for (int o = 0; o < 64; ++o) {
+      Dual s = par(b2, db2, o);
+      for (int k = 0; k < 64; ++k) s += par(W2, dW2, o * 64 + k) * h1[k];
+      h2[o] = s_tanh(s);
+    }
+    for (int o = 0; o < 4; ++o) {
+      Dual s = par(b3, db3, o);
+      for (int k = 0; k < 64; ++k) s += par(W3, dW3, o * 64 + k) * h2[k];
+      y[o] = s;
+    }
+  }
   // O10: h1 = tanh(W1 x + b1), h2 = tanh(W2 h1 + b2), y = W3 h2 + b3 (linear)
   void eval(const double x_in[24], double y[4]) const {
     double x[24], h1[64], h2[64];
@@ -438,11 +463,19 @@ struct Core {
         T F[4];
         hllc_x(WL, WR, gamma, F);
         if (mlp.on) {  // O10: cells i-2..i+3, each (rho,u,v,p)/in_scale
-          double x[24], y[4];
-          for (int cc = 0; cc < 6; ++cc)
-            for (int k = 0; k < 4; ++k) x[4 * cc + k] = to_double(Wv(k, i - 2 + cc, j)) / mlp.in_scale[k];
-          mlp.eval(x, y);
-          for (int k = 0; k < 4; ++k) F[k] += T(mlp.out_scale[k] * y[k]);  // Eq. 11
+          if constexpr (std::is_same<T, Dual>::value) {  // O12: the network's inputs and parameters carry their directions
+            Dual x[24], y[4];
+            for (int cc = 0; cc < 6; ++cc)
+              for (int k = 0; k < 4; ++k) x[4 * cc + k] = Wv(k, i - 2 + cc, j) / Dual(mlp.in_scale[k]);
+            mlp.eval_dual(x, y);
+            for (int k = 0; k < 4; ++k) F[k] += Dual(mlp.out_scale[k]) * y[k];
+          } else {
+            double x[24], y[4];
+            for (int cc = 0; cc < 6; ++cc)
+              for (int k = 0; k < 4; ++k) x[4 * cc + k] = to_double(Wv(k, i - 2 + cc, j)) / mlp.in_scale[k];
+            mlp.eval(x, y);
+            for (int k = 0; k < 4; ++k) F[k] += T(mlp.out_scale[k] * y[k]);  // Eq. 11
+          }
         }
         if (cnn_on) {
           double x4[4];
@@ -467,11 +500,19 @@ struct Core {
         hllc_x(SL, SR, gamma, F);
         if (mlp.on) {  // normal velocity first: (rho, v, u, p)
           static const int perm[4] = {0, 2, 1, 3};
-          double x[24], y[4];
-          for (int cc = 0; cc < 6; ++cc)
-            for (int k = 0; k < 4; ++k) x[4 * cc + k] = to_double(Wv(perm[k], i, j - 2 + cc)) / mlp.in_scale[k];
-          mlp.eval(x, y);
-          for (int k = 0; k < 4; ++k) F[k] += T(mlp.out_scale[k] * y[k]);
+          if constexpr (std::is_same<T, Dual>::value) {
+            Dual x[24], y[4];
+            for (int cc = 0; cc < 6; ++cc)
+              for (int k = 0; k < 4; ++k) x[4 * cc + k] = Wv(perm[k], i, j - 2 + cc) / Dual(mlp.in_scale[k]);
+            mlp.eval_dual(x, y);
+            for (int k = 0; k < 4; ++k) F[k] += Dual(mlp.out_scale[k]) * y[k];
+          } else {
+            double x[24], y[4];
+            for (int cc = 0; cc < 6; ++cc)
+              for (int k = 0; k < 4; ++k) x[4 * cc + k] = to_double(Wv(perm[k], i, j - 2 + cc)) / mlp.in_scale[k];
+            mlp.eval(x, y);
+            for (int k = 0; k < 4; ++k) F[k] += T(mlp.out_scale[k] * y[k]);
+          }
         }
         if (cnn_on) {
           double x4[4];
@@ -825,7 +866,19 @@ int jxo_set_flux_mlp(jxo_solver* s, const float* w, const double in_scale[4], co
     m.in_scale[k] = in_scale[k];
     m.out_scale[k] = out_scale[k];
   }
+  m.dW1.clear(); m.db1.clear(); m.dW2.clear(); m.db2.clear(); m.dW3.clear(); m.db3.clear();
   m.on = true;
+  return JXO_OK;
+}
+
+// direction of perturbation of the MLP's parameters for O12 (6020 doubles in the order of the weights); NULL = none.
+// jxo_set_flux_mlp clears it.
+int jxo_set_flux_mlp_direction(jxo_solver* s, const double* d) {
+  if (!s) return JXO_EINVAL;
+  Mlp& m = s->mlp;
+  if (!d) { m.dW1.clear(); m.db1.clear(); m.dW2.clear(); m.db2.clear(); m.dW3.clear(); m.db3.clear(); return JXO_OK; }
+  auto take = [&](std::vector<double>& dst, size_t n) { dst.assign(d, d + n); d += n; };
+  take(m.dW1, 64 * 24); take(m.db1, 64); take(m.dW2, 64 * 64); take(m.db2, 64); take(m.dW3, 4 * 64); take(m.db3, 4);
   return JXO_OK;
 }
 
@@ -883,7 +936,7 @@ void jxo_hllc_star(const double WL[4], const double WR[4], double gamma, double 
 int jxo_step_fixed_dt_tangent(jxo_solver* s, double* U, double* Udot, double gamma_dot, double dt, int nsteps) {
   if (!s || !U || !Udot || !(dt > 0) || nsteps < 0) return JXO_EINVAL;
   if (s->dtype != JXO_F64) { s->err = "the tangent is fp64 only"; return JXO_EINVAL; }
-  if (s->mlp.on || s->cnn.on) { s->err = "the tangent does not differentiate the networks"; return JXO_ESTATE; }
+  if ((s->mlp.on && s->mlp.bf16) || s->cnn.on) { s->err = "the tangent differentiates the exact (fp64) MLP only"; return JXO_ESTATE; }
   const size_t n = (size_t)4 * s->c.nx * s->c.ny;
   std::vector<Dual> Ud(n), Up;
   for (size_t i = 0; i < n; ++i) Ud[i] = Dual(U[i], Udot[i]);
@@ -913,7 +966,7 @@ int jxo_step_fixed_dt_tangent(jxo_solver* s, double* U, double* Udot, double gam
 int jxo_rhs_tangent(jxo_solver* s, const double* U, const double* Udot, double gamma_dot, double* L, double* Ldot) {
   if (!s || !U || !Udot || !L || !Ldot) return JXO_EINVAL;
   if (s->dtype != JXO_F64) { s->err = "the tangent is fp64 only"; return JXO_EINVAL; }
-  if (s->mlp.on || s->cnn.on) { s->err = "the tangent does not differentiate the networks"; return JXO_ESTATE; }
+  if ((s->mlp.on && s->mlp.bf16) || s->cnn.on) { s->err = "the tangent differentiates the exact (fp64) MLP only"; return JXO_ESTATE; }
   const size_t n = (size_t)4 * s->c.nx * s->c.ny;
   std::vector<Dual> Ud(n), Ld(n), Up;
   for (size_t i = 0; i < n; ++i) Ud[i] = Dual(U[i], Udot[i]);

@@ -45,6 +45,9 @@ int jxo_set_flux_mlp(jxo_solver*, const float* weights, const double in_scale[4]
  * and the two hidden activation fields to bf16.  Can be combined with the per-face MLP (both are added).          */
 int jxo_set_flux_cnn(jxo_solver*, const float* weights, const double in_scale[4],
                      const double out_scale[4], int emulate_bf16);
+/* O12 through the exact (emulate_bf16 = 0) MLP: direction of perturbation of its 6020 parameters, doubles in the
+ * order of the weights; NULL = the parameters do not move (default; jxo_set_flux_mlp resets it).                */
+int jxo_set_flux_mlp_direction(jxo_solver*, const double* direction);
 int jxo_set_artificial_viscosity(jxo_solver*, double nu);
 
 int jxo_rhs(jxo_solver*, const void* U, void* dUdt);

@@ -61,6 +61,7 @@ def lib():
         L.jxo_cnn_fields.argtypes = [vp, dp, dp, dp, dp, dp]
         L.jxo_step_fixed_dt_tangent.argtypes = [vp, vp, vp, C.c_double, C.c_double, C.c_int]
         L.jxo_rhs_tangent.argtypes = [vp, vp, vp, C.c_double, vp, vp]
+        L.jxo_set_flux_mlp_direction.argtypes = [vp, vp]
         L.jxo_weno5_tangent.argtypes = [dp, dp, dp]
         L.jxo_weno5_tangent.restype = None
         L.jxo_hllc_tangent.argtypes = [dp, dp, dp, dp, C.c_double, C.c_double, dp, dp]
@@ -232,6 +233,15 @@ class Oracle:
         U = self._field(U).copy()
         self._chk(lib().jxo_step_fixed_dt(self._h, U.ctypes.data, float(dt), int(nsteps)))
         return U
+
+    def set_flux_mlp_direction(self, direction):
+        """Direction of perturbation of the MLP's 6020 parameters for the tangent O12; None = none."""
+        if direction is None:
+            self._chk(lib().jxo_set_flux_mlp_direction(self._h, None))
+            return
+        d = np.ascontiguousarray(direction, dtype=np.float64)
+        assert d.shape == (6020,)
+        self._chk(lib().jxo_set_flux_mlp_direction(self._h, d.ctypes.data))
 
     def rhs_tangent(self, U, Udot, gamma_dot):
         """(L(U), its derivative along (Udot, gamma_dot))."""

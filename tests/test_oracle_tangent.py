@@ -316,12 +316,50 @@ def test_rhs_tangent_and_the_euler_update():
     assert rel(De * fluid, fd * fluid) < 5e-6
 
 
+def test_tangent_through_the_exact_mlp_matches_central_differences():
+    # O12 with the network: its inputs' dependence on the state and on gamma, and a direction in its 6020 parameters
+    case = wl.vortex(12)
+    w = wl.mlp_weights(3)
+    sc = wl.mlp_scales(out_factor=5e-2)
+    dt, ns = 0.04, 2
+    rng = np.random.default_rng(14)
+    wdir = rng.normal(size=6020)
+
+    def run(U0, g, ww):
+        o = make(case, gamma=g)
+        o.set_flux_mlp(ww, *sc, emulate_bf16=False)
+        return o.step_fixed_dt(U0, dt, ns)
+
+    o = make(case)
+    o.set_flux_mlp(w, *sc, emulate_bf16=False)
+    assert rel(run(case["U0"], G, w), make(case).step_fixed_dt(case["U0"], dt, ns)) > 1e-4   # the network acts
+    Udir = wl.smooth_direction(case["U0"].shape, seed=15)
+    h = 2e-7   # a coarse grid: the third derivatives of the WENO weights are large
+    # state and gamma
+    U, Ud = o.step_fixed_dt_tangent(case["U0"], Udir, 0.7, dt, ns)
+    assert np.array_equal(U, run(case["U0"], G, w))
+    fd = (run(case["U0"] + h * Udir, G + 0.7 * h, w) - run(case["U0"] - h * Udir, G - 0.7 * h, w)) / (2 * h)
+    assert rel(Ud, fd) < 5e-7
+    # the parameters: float32 weights perturbed along a float32 direction, the quotient taken with the step made
+    hw = np.float32(2.0 ** -12)
+    wd32 = wdir.astype(np.float32)
+    wp, wm = (w + hw * wd32).astype(np.float32), (w - hw * wd32).astype(np.float32)
+    actual = (wp.astype(np.float64) - wm.astype(np.float64)) / (2.0 * float(hw))   # the direction really taken
+    o.set_flux_mlp_direction(actual)
+    _, Ud = o.step_fixed_dt_tangent(case["U0"], np.zeros_like(Udir), 0.0, dt, ns)
+    fd = (run(case["U0"], G, wp) - run(case["U0"], G, wm)) / (2.0 * float(hw))
+    assert np.abs(Ud).max() > 1e-6 and rel(Ud, fd) < 1e-5
+    o.set_flux_mlp_direction(None)
+    _, Ud = o.step_fixed_dt_tangent(case["U0"], np.zeros_like(Udir), 0.0, dt, ns)
+    assert np.all(Ud == 0.0)
+
+
 def test_tangent_argument_checks():
     case = wl.vortex(8)
     o = make(case, dtype=np.float32)
     with pytest.raises(jxo.OracleError):
         o.step_fixed_dt_tangent(case["U0"].astype(np.float32), np.zeros_like(case["U0"]), 1.0, 0.01, 1)
     o = make(case)
-    o.set_flux_mlp(wl.mlp_weights(), *wl.mlp_scales())
+    o.set_flux_mlp(wl.mlp_weights(), *wl.mlp_scales(), emulate_bf16=True)   # only the exact MLP is differentiated
     with pytest.raises(jxo.OracleError):
         o.step_fixed_dt_tangent(case["U0"], np.zeros_like(case["U0"]), 1.0, 0.01, 1)
