@@ -3,9 +3,10 @@
 
 * forward: RHS and steps against the oracle's exact (fp64) MLP mode on the planar problem of 8 identical rows (the
   y-face corrections of identical rows cancel in the divergence): <= 1e-12 / <= 1e-9;
-* reverse: phi = <c, S^n(U0; theta)> has gradient (J^T c, dphi/dtheta); the adjoint of the state and the weights'
-  gradient against central differences of the ORACLE's primal run at sampled entries (the oracle's network is not
-  differentiated, SURVEY 8(f) rank 3 says as much: "finite differences"): 1e-5 of the gradient's scale.
+* reverse: phi = <c, S^n(U0; theta)> has gradient (J^T c, dphi/dtheta).  Exact parity against the oracle's tangent
+  (O12 runs the exact MLP on the dual scalar, with a direction in its parameters): the state's adjoint and gamma_bar
+  element by element against O13, the weights' gradient at sampled entries, <= 1e-11; and, independently of the
+  oracle's derivative code, against central differences of its primal run (1e-5).
 """
 import numpy as np
 import pytest
@@ -92,6 +93,42 @@ def test_mlp1d_training_gradient_against_differences_of_the_oracle():
     # gamma (the network's pressure input depends on it too)
     fd = (phi(case["U0"], gamma=1.4 + h) - phi(case["U0"], gamma=1.4 - h)) / (2 * h)
     assert gbar == pytest.approx(fd, rel=2e-5)
+
+
+def test_mlp1d_adjoint_and_weights_gradient_match_the_transposed_oracle_tangent():
+    """exact parity: O13 (the transpose of the oracle's tangent, which covers the exact MLP) for the state and gamma,
+    and <Ubar, dS/dtheta_j> from the oracle's tangent along unit directions in the parameters, sampled"""
+    nx, ns = 80, 2
+    case = smooth1d(nx, 1e-4, dict(PER, xlo="reflective", xhi="transmissive"))
+    dt = 0.2 * case["dx"]
+    rng = np.random.default_rng(6)
+    Ubar = rng.normal(size=case["U0"].shape)
+    c2, o = oracle_rows(case)
+    want, gwant = o.step_fixed_dt_adjoint(c2["U0"], Ubar, dt, ns, planar=True)
+    s = gpu(case)
+    U, B = dev(case["U0"]), dev(Ubar)
+    s.step_fixed_dt_record(U, dt, ns)
+    gbar = s.adjoint_steps(B)
+    assert rel_err(B.cpu().numpy(), want) <= 1e-11
+    assert gbar == pytest.approx(gwant, rel=1e-10)
+    grad = s.flux_mlp_gradient()
+    scale = np.abs(grad).max()
+    picks = [3, 24 * 40 + 11, 1536 + 63, 1600 + 64 * 5 + 50, 5696 + 1, 5760 + 3 * 64 + 33, 6016] + \
+            [int(j) for j in rng.integers(0, 6020, 10)]
+    zero = np.zeros_like(c2["U0"])
+    for j in picks:
+        e = np.zeros(6020)
+        e[j] = 1.0
+        o.set_flux_mlp_direction(e)
+        _, D = o.step_fixed_dt_tangent(c2["U0"], zero, 0.0, dt, ns)
+        assert abs(grad[j] - float(np.sum(Ubar * D[:, :1]))) <= 1e-11 * scale, j
+    # checkpointed recording: the same numbers to round-off (with the network the sums over faces are atomic)
+    s.set_adjoint_checkpointing(True)
+    U2, B2 = dev(case["U0"]), dev(Ubar)
+    s.step_fixed_dt_record(U2, dt, ns)
+    assert s.adjoint_steps(B2) == pytest.approx(gbar, rel=1e-12)
+    assert np.array_equal(U2.cpu().numpy(), U.cpu().numpy()) and rel_err(B2.cpu().numpy(), B.cpu().numpy()) <= 1e-13
+    assert np.abs(s.flux_mlp_gradient() - grad).max() <= 1e-13 * scale
 
 
 def test_unrolled_training_of_the_neural_flux_reduces_the_loss():
