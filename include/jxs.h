@@ -7,7 +7,11 @@
  *   HLLC flux in x and y (L54-81, Eq. 3-9), flux divergence + viscous terms
  *   (L9, L83-85 Eq. 10), Runge-Kutta combine and CFL wavespeed reduction
  *   (BASELINE.json north_star), optional per-face MLP flux correction (L96 Eq. 11).
- * Where the paper is silent or garbled the readings R1-R17 of DESIGN.md apply.
+ * Widened since: the paper's 2D CNN flux (L94, Eq. 11-13), the forward-Euler update of Eq. 10,
+ * one-dimensional problems (ny = 1: the Sod tube of L132-149) with their per-face MLP flux (L109), and for those
+ * the derivatives the paper obtains from JAX (L92, L112-128, L149): the tangent of the step, its adjoint with the
+ * trajectory kept in HBM, the loss of Eq. 14 and the gradient with respect to gamma and to the network's weights.
+ * Where the paper is silent or garbled the readings R1-R24 of DESIGN.md apply.
  *
  * Conventions
  *   - every function returns an int status (JXS_OK = 0); nothing throws, aborts or prints;
