@@ -93,18 +93,23 @@ __global__ void __launch_bounds__(128) mlp1d_kernel(const Mlp1dArgs A) {
 // with Lbar = b dt Ubar_out (as in adjoint1d_kernel); ybar = out_scale o Fbar; then layer by layer:
 //   W3bar += ybar h2^T, h2bar = W3^T ybar, z2bar = h2bar (1 - h2^2), W2bar += z2bar h1^T, h1bar = W2^T z2bar, ...
 // and xbar / in_scale is the adjoint of the six cells' primitives (added to Wbar for adjoint1d_kernel to convert).
-// Sums over faces go through fp64 atomics — a CTA first adds the weights' gradient of all its faces up in shared
-// memory (6020 doubles, dynamic), then adds that to the global one once — so the order of the additions is not
+// The weights' gradient: every warp adds the contributions of its faces into a slot of its own in shared memory
+// (4 x 6020 doubles, dynamic; plain stores, every entry belongs to one lane), the CTA sums its four slots and adds
+// the result to the global gradient with one fp64 atomic per parameter; the adjoint of the network's input, which
+// neighbouring faces share, goes through fp64 atomics as well (24 per face).  The order of those additions is not
 // fixed: results agree to round-off.
-constexpr int MLP1D_BWD_SMEM = MLP1D_NPARAM * (int)sizeof(double);
+constexpr int MLP1D_BWD_SMEM = 4 * MLP1D_NPARAM * (int)sizeof(double);
 
 __global__ void __launch_bounds__(128) mlp1d_backward_kernel(const Mlp1dArgs A) {
-  extern __shared__ double tb[];  // this CTA's share of theta_bar
+  extern __shared__ double slots[];
   const int lane = threadIdx.x & 31;
   const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
   const double* th = A.theta;
-  for (int i = threadIdx.x; i < MLP1D_NPARAM; i += blockDim.x) tb[i] = 0.0;
-  __syncthreads();
+  double* tb = slots + (threadIdx.x >> 5) * MLP1D_NPARAM;  // this warp's slot
+  bool first = true;  // the first face of a warp writes its slot, the later ones add to it (every face touches all of it)
+  if (2 + warp > A.nx + 2)
+    for (int i = lane; i < MLP1D_NPARAM; i += 32) tb[i] = 0.0;  // a warp without a face
+  auto add = [&](double* p, double v) { *p = first ? v : *p + v; };
   for (int c = 2 + warp; c <= A.nx + 2; c += nwarps) {
     double r, u, v, h1a, h1b, h2a, h2b, y[4];
     const double x = mlp1d_input<double>(A, c, lane, r, u, v);
@@ -122,36 +127,36 @@ __global__ void __launch_bounds__(128) mlp1d_backward_kernel(const Mlp1dArgs A) 
     double h2ab = 0.0, h2bb = 0.0;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-      atomicAdd(tb + MLP1D_W3 + k * 64 + lane, yb[k] * h2a);
-      atomicAdd(tb + MLP1D_W3 + k * 64 + lane + 32, yb[k] * h2b);
+      add(tb + MLP1D_W3 + k * 64 + lane, yb[k] * h2a);
+      add(tb + MLP1D_W3 + k * 64 + lane + 32, yb[k] * h2b);
       h2ab = fma(th[MLP1D_W3 + k * 64 + lane], yb[k], h2ab);
       h2bb = fma(th[MLP1D_W3 + k * 64 + lane + 32], yb[k], h2bb);
     }
-    if (lane < 4) atomicAdd(tb + MLP1D_B3 + lane, yb[lane]);
+    if (lane < 4) add(tb + MLP1D_B3 + lane, yb[lane]);
     // second hidden layer: my units j = lane, lane + 32
     const double z2a = h2ab * (1.0 - h2a * h2a), z2b = h2bb * (1.0 - h2b * h2b);
-    atomicAdd(tb + MLP1D_B2 + lane, z2a);
-    atomicAdd(tb + MLP1D_B2 + lane + 32, z2b);
+    add(tb + MLP1D_B2 + lane, z2a);
+    add(tb + MLP1D_B2 + lane + 32, z2b);
     double h1ab = 0.0, h1bb = 0.0;  // adjoint of h1 units lane, lane + 32: sum over all 64 units j of W2[j][.] z2bar_j
     for (int i = 0; i < 32; ++i) {
       const double a = __shfl_sync(0xffffffffu, h1a, i), b = __shfl_sync(0xffffffffu, h1b, i);
-      atomicAdd(tb + MLP1D_W2 + lane * 64 + i, z2a * a);
-      atomicAdd(tb + MLP1D_W2 + lane * 64 + 32 + i, z2a * b);
-      atomicAdd(tb + MLP1D_W2 + (lane + 32) * 64 + i, z2b * a);
-      atomicAdd(tb + MLP1D_W2 + (lane + 32) * 64 + 32 + i, z2b * b);
+      add(tb + MLP1D_W2 + lane * 64 + i, z2a * a);
+      add(tb + MLP1D_W2 + lane * 64 + 32 + i, z2a * b);
+      add(tb + MLP1D_W2 + (lane + 32) * 64 + i, z2b * a);
+      add(tb + MLP1D_W2 + (lane + 32) * 64 + 32 + i, z2b * b);
       const double za = __shfl_sync(0xffffffffu, z2a, i), zb = __shfl_sync(0xffffffffu, z2b, i);  // units i, i + 32
       h1ab = fma(th[MLP1D_W2 + i * 64 + lane], za, fma(th[MLP1D_W2 + (i + 32) * 64 + lane], zb, h1ab));
       h1bb = fma(th[MLP1D_W2 + i * 64 + lane + 32], za, fma(th[MLP1D_W2 + (i + 32) * 64 + lane + 32], zb, h1bb));
     }
     // first hidden layer
     const double z1a = h1ab * (1.0 - h1a * h1a), z1b = h1bb * (1.0 - h1b * h1b);
-    atomicAdd(tb + MLP1D_B1 + lane, z1a);
-    atomicAdd(tb + MLP1D_B1 + lane + 32, z1b);
+    add(tb + MLP1D_B1 + lane, z1a);
+    add(tb + MLP1D_B1 + lane + 32, z1b);
     double xb = 0.0;  // adjoint of input lane (< 24)
     for (int i = 0; i < 24; ++i) {
       const double xi = __shfl_sync(0xffffffffu, x, i);
-      atomicAdd(tb + MLP1D_W1 + lane * 24 + i, z1a * xi);
-      atomicAdd(tb + MLP1D_W1 + (lane + 32) * 24 + i, z1b * xi);
+      add(tb + MLP1D_W1 + lane * 24 + i, z1a * xi);
+      add(tb + MLP1D_W1 + (lane + 32) * 24 + i, z1b * xi);
     }
     for (int j = 0; j < 32; ++j) {
       const double za = __shfl_sync(0xffffffffu, z1a, j), zb = __shfl_sync(0xffffffffu, z1b, j);  // units j, j + 32
@@ -161,9 +166,12 @@ __global__ void __launch_bounds__(128) mlp1d_backward_kernel(const Mlp1dArgs A) 
       const int var = lane & 3;
       atomicAdd(A.Wbar + var * A.plane + 3 * (size_t)A.pitch + (c - 2 + (lane >> 2)), xb * A.inv_in[var]);
     }
+    first = false;
+    __syncwarp();
   }
   __syncthreads();
-  for (int i = threadIdx.x; i < MLP1D_NPARAM; i += blockDim.x) atomicAdd(A.theta_bar + i, tb[i]);
+  for (int i = threadIdx.x; i < MLP1D_NPARAM; i += blockDim.x)
+    atomicAdd(A.theta_bar + i, (slots[i] + slots[MLP1D_NPARAM + i]) + (slots[2 * MLP1D_NPARAM + i] + slots[3 * MLP1D_NPARAM + i]));
 }
 
 }  // namespace jxs
