@@ -377,21 +377,34 @@ __global__ void __launch_bounds__(A1D_FOLD_TB) adjoint1d_fold_kernel(double* Uba
   for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
   if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = a;
   __syncthreads();
+  // ghost columns: one thread per (side, component); its three ghost cells are read together, then added to their
+  // source cells one after the other (all three may share one: a transmissive end)
+  __shared__ double gin[8];
+  if (threadIdx.x < 8) {
+    const int side = threadIdx.x >> 2, k = threadIdx.x & 3;
+    const double g1 = gamma - 1.0;
+    double x[3], gi = 0.0;
+    int idx[3];
+#pragma unroll
+    for (int g = 0; g < 3; ++g) {
+      idx[g] = side == 0 ? g - 3 : nx + g;  // interior index of the ghost cell
+      x[g] = Ubar[k * plane + idx[g] + 3];
+      Ubar[k * plane + idx[g] + 3] = 0.0;
+    }
+#pragma unroll
+    for (int g = 0; g < 3; ++g) {
+      int src, sgn;
+      bc_map(idx[g], nx, xlo, xhi, src, sgn);
+      if (src < 0) { if (k == 3) gi -= x[g] * p_inflow / (g1 * g1); }
+      else Ubar[k * plane + src + 3] += (k == 1 && sgn < 0) ? -x[g] : x[g];
+    }
+    gin[threadIdx.x] = gi;
+  }
+  __syncthreads();
   if (threadIdx.x == 0) {
     double gb = 0.0;
     for (int w = 0; w < A1D_FOLD_TB / 32; ++w) gb += red[w];
-    const double g1 = gamma - 1.0;
-    for (int c = 0; c < 6; ++c) {
-      const int i = c < 3 ? c - 3 : nx + (c - 3);  // interior index of the ghost cell
-      int src, sgn;
-      bc_map(i, nx, xlo, xhi, src, sgn);
-      for (int k = 0; k < 4; ++k) {
-        const double x = Ubar[k * plane + i + 3];
-        Ubar[k * plane + i + 3] = 0.0;
-        if (src < 0) { if (k == 3) gb -= x * p_inflow / (g1 * g1); }
-        else Ubar[k * plane + src + 3] += (k == 1 && sgn < 0) ? -x : x;
-      }
-    }
+    for (int w = 0; w < 8; ++w) gb += gin[w];
     *gamma_bar += gb;
   }
 }
