@@ -171,6 +171,17 @@ int jxs_mse_tangent(jxs_solver*, const void* U, const void* Udot, const void* Ut
  * synchronise the stream.                                                                                         */
 int jxs_step_fixed_dt_record(jxs_solver*, void* U, double dt, int nsteps);
 int jxs_adjoint_steps(jxs_solver*, void* Ubar, double* gamma_bar);
+/* The reverse sweep driven by the loss of PAPER.md Eq. 14 itself, the mean over the m recorded steps of the mean
+ * squared error against one target per step (R22):  L = (1/m) sum_{s=1..m} mean((U^{n+s} - targets[s-1])^2).
+ *   targets  DEVICE, [m][4][1][nx] doubles, m = the nsteps of the last jxs_step_fixed_dt_record: the downsampled
+ *            reference states U~^{n+s} (read only)
+ *   Ubar     DEVICE, [4][1][nx] doubles, OUT: dL/dU^n
+ *   loss, gamma_bar  HOST, OUT: L and dL/dgamma at fixed U^n; the weights' gradient dL/dtheta is read with
+ *            jxs_flux_mlp_gradient
+ * Every intermediate loss L_s enters the sweep where its state does (Eq. 16 summed over s), so the cost is that of
+ * one jxs_adjoint_steps.  Errors as jxs_adjoint_steps, JXS_EINVAL for NULL.  Synchronises the stream.            */
+int jxs_adjoint_steps_mse(jxs_solver*, const void* targets, void* Ubar, double* loss, double* gamma_bar);
+
 /* One-dimensional handles accept jxs_set_flux_mlp as well ("For the one-dimensional Sod shock-tube
  * simulation, a multilayer perceptron (MLP) network is used to predict the neural flux"): same parameters, input
  * and output conventions as in 2D (R14), evaluated per face in fp64 and added to the HLLC flux of every stage (Eq. 11)

@@ -409,4 +409,30 @@ __global__ void __launch_bounds__(A1D_FOLD_TB) adjoint1d_fold_kernel(double* Uba
   }
 }
 
+// The loss of PAPER.md Eq. 14 inside the reverse sweep: L = (1/m) sum_s mean((U^{n+s} - target_s)^2).  For one s:
+// Ubar (+)= coef (U - target), coef = 2 / (m 4 nx), on the interior cells of the compact padded row, and
+// loss_acc += sum (U - target)^2 (one fp64 atomic per CTA).  target: [4][nx] interior layout.
+__global__ void __launch_bounds__(256) mse_inject_kernel(const double* __restrict__ Urow, long long plane,
+                                                         const double* __restrict__ target, int nx, double coef,
+                                                         double* Xrow, int accumulate, double* loss_acc) {
+  __shared__ double red[8];
+  double a = 0.0;
+  for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < 4LL * nx; i += (long long)gridDim.x * 256) {
+    const int k = (int)(i / nx), c = (int)(i - (long long)k * nx);
+    const double r = Urow[k * plane + c + 3] - target[i];
+    double* x = Xrow + k * plane + c + 3;
+    *x = accumulate ? fma(coef, r, *x) : coef * r;
+    a = fma(r, r, a);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = a;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int w = 0; w < 8; ++w) t += red[w];
+    atomicAdd(loss_acc, t);
+  }
+}
+
 }  // namespace jxs

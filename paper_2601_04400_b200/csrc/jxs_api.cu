@@ -1032,9 +1032,10 @@ cudaError_t adjoint_stage(jxs_solver* s, const double* U, const double* out, dou
   return cudaGetLastError();
 }
 
-int adjoint_common(jxs_solver* s, void* Ubar, double* gamma_bar) {
+// targets != nullptr: the loss of Eq. 14 over the recorded steps drives the sweep (Ubar is output only, *loss too)
+int adjoint_common(jxs_solver* s, void* Ubar, double* gamma_bar, const double* targets = nullptr, double* loss = nullptr) {
   if (!s) return JXS_EINVAL;
-  if (!Ubar || !gamma_bar) return fail(s, JXS_EINVAL, "NULL argument");
+  if (!Ubar || !gamma_bar || (targets && !loss)) return fail(s, JXS_EINVAL, "NULL argument");
   int rc = adjoint_checks(s);
   if (rc != JXS_OK) return rc;
   if (!s->tape || s->tape_steps < 1) return fail(s, JXS_ESTATE, "no recorded steps: call jxs_step_fixed_dt_record first");
@@ -1043,18 +1044,33 @@ int adjoint_common(jxs_solver* s, void* Ubar, double* gamma_bar) {
   if (!s->adj || s->adj_parts != parts) {
     cudaFree(s->adj);
     s->adj = nullptr;
-    CU(cudaMalloc(&s->adj, (4 * state + parts + 1) * sizeof(double)));
+    CU(cudaMalloc(&s->adj, (4 * state + parts + 2) * sizeof(double)));
     s->adj_parts = parts;
   }
-  CU(cudaMemsetAsync(s->adj, 0, (4 * state + parts + 1) * sizeof(double), s->stream));
+  CU(cudaMemsetAsync(s->adj, 0, (4 * state + parts + 2) * sizeof(double), s->stream));
   CompactLayout compact(s);
   auto T = [&](long long i) { return compact_state(s, s->tape, i); };
   auto B = [&](int i) { return compact_state(s, s->adj, i); };
-  CU(pad(s, Ubar, B(0)));
+  const int per_step = (s->tape_scheme == JXS_EULER || s->tape_ckpt) ? 1 : 3;
+  const long long ncell4 = 4LL * s->nx;
+  double* loss_acc = s->adj + 4 * state + parts + 1;
+  // Eq. 14: the state after recorded step n is tape state per_step * n; its target is targets[n - 1]
+  auto inject = [&](long long n, int into, int accumulate) {
+    const int gs = (int)std::min<long long>((ncell4 + 255) / 256, s->num_sms * 4);
+    mse_inject_kernel<<<gs, 256, 0, s->stream>>>(T(per_step * n) + 3 * (long long)s->pitch, s->pitch,
+                                                 targets + (n - 1) * ncell4, s->nx, 2.0 / (s->tape_steps * (double)ncell4),
+                                                 B(into) + 3 * (long long)s->pitch, accumulate, loss_acc);
+    s->launches++;
+    return cudaGetLastError();
+  };
+  if (targets) CU(inject(s->tape_steps, 0, 0));
+  else CU(pad(s, Ubar, B(0)));
   if (s->mlp1d_on) CU(cudaMemsetAsync(s->d_theta_bar, 0, MLP1D_NPARAM * sizeof(double), s->stream));
   s->events_used = 0;
   int x = 0;  // which adjoint state holds the adjoint of U^{n+1}
   for (long long n = s->tape_steps - 1; n >= 0; --n) {
+    // (Eq. 14) the adjoint of U^{n+1} so far comes from the later steps: add this state's own term of the loss
+    if (targets && n + 1 < s->tape_steps) CU(inject(n + 1, x, 1));
     if (s->tape_ckpt) {  // recompute the step's inner stage states from the kept U^n, then reverse the three stages
       double* S0 = compact_state(s, s->ckpt, 0);
       double* S1 = compact_state(s, s->ckpt, 1);
@@ -1085,8 +1101,11 @@ int adjoint_common(jxs_solver* s, void* Ubar, double* gamma_bar) {
     x = y0;
   }
   CU(unpad(s, B(x), Ubar));
-  CU(cudaMemcpyAsync(gamma_bar, s->adj + 4 * state + parts, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+  double out[2];
+  CU(cudaMemcpyAsync(out, s->adj + 4 * state + parts, sizeof(out), cudaMemcpyDeviceToHost, s->stream));
   CU(cudaStreamSynchronize(s->stream));
+  *gamma_bar = out[0];
+  if (loss) *loss = out[1] / (s->tape_steps * (double)ncell4);
   if (s->profiling) {
     s->stage_ms = 0;
     s->stage_launches = s->events_used / 2;
@@ -1455,6 +1474,10 @@ int jxs_step_fixed_dt_tangent(jxs_solver* s, void* U, void* Udot, double gamma_d
 
 int jxs_step_fixed_dt_record(jxs_solver* s, void* U, double dt, int nsteps) { return record_common(s, U, dt, nsteps); }
 int jxs_adjoint_steps(jxs_solver* s, void* Ubar, double* gamma_bar) { return adjoint_common(s, Ubar, gamma_bar); }
+int jxs_adjoint_steps_mse(jxs_solver* s, const void* targets, void* Ubar, double* loss, double* gamma_bar) {
+  if (s && !targets) return fail(s, JXS_EINVAL, "targets is NULL");
+  return adjoint_common(s, Ubar, gamma_bar, (const double*)targets, loss);
+}
 
 int jxs_flux_mlp_gradient(jxs_solver* s, double* grad) {
   if (!s) return JXS_EINVAL;

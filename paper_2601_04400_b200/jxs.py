@@ -25,7 +25,7 @@ EXPORTS = ("jxs_create", "jxs_destroy", "jxs_last_error", "jxs_set_ibm", "jxs_se
            "jxs_flux_mlp_time", "jxs_step_async", "jxs_wait", "jxs_set_time_integrator",
            "jxs_set_concurrent_handles", "jxs_set_flux_cnn", "jxs_flux_cnn_inputs",
            "jxs_step_fixed_dt_tangent", "jxs_mse_tangent", "jxs_step_fixed_dt_record", "jxs_adjoint_steps", "jxs_set_gamma",
-           "jxs_set_adjoint_checkpointing", "jxs_flux_mlp_gradient")
+           "jxs_set_adjoint_checkpointing", "jxs_flux_mlp_gradient", "jxs_adjoint_steps_mse")
 
 
 class jxs_bc(C.Structure):
@@ -83,6 +83,7 @@ def lib():
         L.jxs_set_gamma.argtypes = [vp, C.c_double]
         L.jxs_set_adjoint_checkpointing.argtypes = [vp, C.c_int]
         L.jxs_flux_mlp_gradient.argtypes = [vp, vp]
+        L.jxs_adjoint_steps_mse.argtypes = [vp, vp, vp, dp, dp]
         L.jxs_get_time.argtypes = [vp, dp, dp]
         L.jxs_launch_count.argtypes = [vp]
         L.jxs_launch_count.restype = C.c_longlong
@@ -271,6 +272,16 @@ class Solver:
 
     def set_gamma(self, gamma):
         self._chk(lib().jxs_set_gamma(self._h, float(gamma)))
+
+    def adjoint_steps_mse(self, targets, Ubar):
+        """Eq. 14 over the recorded steps: fills Ubar with dL/dU^n; returns (loss, gamma_bar).
+        targets: device tensor [m][4][1][nx] float64, m = the recorded step count."""
+        assert targets.is_cuda and targets.is_contiguous() and targets.dtype == torch.float64
+        assert tuple(targets.shape[1:]) == (4, self.ny, self.nx)
+        loss, g = C.c_double(), C.c_double()
+        self._chk(lib().jxs_adjoint_steps_mse(self._h, C.c_void_p(targets.data_ptr()), self._dev(Ubar),
+                                              C.byref(loss), C.byref(g)))
+        return loss.value, g.value
 
     def flux_mlp_gradient(self):
         """The weights' gradient accumulated by the last adjoint_steps (one-dimensional handles), float64[6020]."""

@@ -131,6 +131,48 @@ def test_mlp1d_adjoint_and_weights_gradient_match_the_transposed_oracle_tangent(
     assert np.abs(s.flux_mlp_gradient() - grad).max() <= 1e-13 * scale
 
 
+@pytest.mark.parametrize("ckpt", [False, True])
+def test_eq14_loss_over_the_unrolled_steps_and_its_gradients(ckpt):
+    """jxs_adjoint_steps_mse: L = (1/m) sum_s mean((U^{n+s} - target_s)^2), Eq. 14 with its intermediate losses.
+    Against the oracle: the value from its primal trajectory, dL/dgamma and dL/dtheta_j from its tangents at every
+    step (L' = (1/m) sum_s mean(2 (U_s - target_s) Udot_s)), dL/dU^n from the transposes O13 of the s-step maps."""
+    import torch
+    nx, m = 48, 3
+    case = smooth1d(nx, 0.0, dict(PER))
+    dt = 0.2 * case["dx"]
+    rng = np.random.default_rng(9)
+    targets = case["U0"][None] + 0.05 * rng.normal(size=(m,) + case["U0"].shape)
+    s = gpu(case)
+    s.set_adjoint_checkpointing(ckpt)
+    U, B = dev(case["U0"]), dev(np.zeros_like(case["U0"]))
+    s.step_fixed_dt_record(U, dt, m)
+    loss, gbar = s.adjoint_steps_mse(torch.tensor(targets, device="cuda"), B)
+    grad = s.flux_mlp_gradient()
+    c2, o = oracle_rows(case)
+    # the oracle's trajectory and residuals
+    res = []
+    for k in range(1, m + 1):
+        res.append(o.step_fixed_dt(c2["U0"], dt, k)[:, :1] - targets[k - 1])
+    n = res[0].size
+    assert loss == pytest.approx(sum(float(np.mean(r * r)) for r in res) / m, rel=1e-12)
+    zero = np.zeros_like(c2["U0"])
+
+    def dloss(Udot, gdot):
+        return sum(float(np.sum(2.0 * r * o.step_fixed_dt_tangent(c2["U0"], Udot, gdot, dt, k + 1)[1][:, :1]))
+                   for k, r in enumerate(res)) / (m * n)
+
+    assert gbar == pytest.approx(dloss(zero, 1.0), rel=1e-10)
+    scale = np.abs(grad).max()
+    for j in [7, 1536 + 20, 1600 + 64 * 33 + 2, 5760 + 100, 6019]:
+        e = np.zeros(6020)
+        e[j] = 1.0
+        o.set_flux_mlp_direction(e)
+        assert abs(grad[j] - dloss(zero, 0.0)) <= 1e-11 * scale, j
+    o.set_flux_mlp_direction(None)
+    want = sum(o.step_fixed_dt_adjoint(c2["U0"], 2.0 * r / (m * n), dt, k + 1, planar=True)[0] for k, r in enumerate(res))
+    assert rel_err(B.cpu().numpy(), want) <= 1e-11
+
+
 def test_unrolled_training_of_the_neural_flux_reduces_the_loss():
     """P:L112-128 on the paper's own set-up (Fig. 3c-f), scaled down: a low-resolution Sod run (N = 125) with the
     neural flux is trained, m = 10 unrolled steps, towards the block-averaged high-resolution run (N = 250, Eq. 14);
