@@ -339,7 +339,8 @@ def run_adjoint1d(args, rank, world, local_rank, dist, barrier, tdt):
 def run_train1d(args, rank, world, local_rank, dist, barrier, tdt):
     """SURVEY.md section 8(f) rank 3, the paper's second mode (Fig. 3c): one training iteration
     of the 1D neural flux at the paper's low resolution N = 500 — K unrolled steps recorded with the per-face MLP in
-    every stage, dL/dU of Eq. 14, K adjoint steps through solver and network, the weights' gradient copied out."""
+    every stage, then the reverse sweep driven by Eq. 14 with one block-averaged N = 1000 target per unrolled step
+    (jxs_adjoint_steps_mse) through solver and network, the weights' gradient copied out."""
     import torch
     from paper_2601_04400_b200 import jxs, workloads as wl
     if args.dtype != "f64":
@@ -354,14 +355,17 @@ def run_train1d(args, rank, world, local_rank, dist, barrier, tdt):
     hi = wl.sod1d(2 * nx)
     Uh = torch.tensor(hi["U0"], dtype=tdt, device="cuda")
     K, W = args.steps, args.warmup
-    jxs.Solver.from_case(hi, dtype=tdt, stream=stream).step_fixed_dt(Uh, 0.5 * dt, 2 * K)
-    target = (0.5 * (Uh[:, :, 0::2] + Uh[:, :, 1::2])).contiguous()   # d(U_HR): block average of the N = 1000 run
+    fine = jxs.Solver.from_case(hi, dtype=tdt, stream=stream)
+    targets = torch.empty((max(K, W), 4, 1, nx), dtype=tdt, device="cuda")
+    for k in range(max(K, W)):   # d(U_HR^{n+s}), s = 1 .. K: block averages of the N = 1000 run, one per unrolled step
+        fine.step_fixed_dt(Uh, 0.5 * dt, 2)
+        targets[k] = 0.5 * (Uh[:, :, 0::2] + Uh[:, :, 1::2])
+    B = torch.empty_like(U0)
 
     def iteration(n):
         U = U0.clone()
         solver.step_fixed_dt_record(U, dt, n)
-        B = (U - target).mul_(2.0 / U.numel())
-        solver.adjoint_steps(B)
+        solver.adjoint_steps_mse(targets[:n].contiguous(), B)     # Eq. 14 over the n unrolled steps and its gradients
         return solver.flux_mlp_gradient()
 
     iteration(W)
