@@ -1305,14 +1305,18 @@ int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[
   for (int i = 0; i < 6020; ++i)
     if (!std::isfinite(weights[i])) return fail(s, JXS_EINVAL, "non-finite MLP weight");
   if (s->ny == 1) {  // one-dimensional problems: the fp64 per-face MLP of mlp1d_kernel.cuh
-    std::vector<double> th(MLP1D_NPARAM);
+    std::vector<double> th(MLP1D_NDEV);
     for (int i = 0; i < MLP1D_NPARAM; ++i) th[i] = (double)weights[i];
+    for (int j = 0; j < 64; ++j) {  // the transposed copies the forward pass reads
+      for (int i = 0; i < 24; ++i) th[MLP1D_W1T + i * 64 + j] = th[MLP1D_W1 + j * 24 + i];
+      for (int i = 0; i < 64; ++i) th[MLP1D_W2T + i * 64 + j] = th[MLP1D_W2 + j * 64 + i];
+    }
     const size_t fbytes = (size_t)4 * s->plane * sizeof(double);
-    if (!s->d_theta) CU(cudaMalloc(&s->d_theta, MLP1D_NPARAM * sizeof(double)));
+    if (!s->d_theta) CU(cudaMalloc(&s->d_theta, MLP1D_NDEV * sizeof(double)));
     if (!s->d_theta_bar) CU(cudaMalloc(&s->d_theta_bar, MLP1D_NPARAM * sizeof(double)));
     if (!s->d_dF1d) { CU(cudaMalloc(&s->d_dF1d, fbytes)); CU(cudaMemset(s->d_dF1d, 0, fbytes)); }
     if (!s->d_Wmlp) { CU(cudaMalloc(&s->d_Wmlp, fbytes)); CU(cudaMemset(s->d_Wmlp, 0, fbytes)); }
-    CU(cudaMemcpy(s->d_theta, th.data(), MLP1D_NPARAM * sizeof(double), cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(s->d_theta, th.data(), MLP1D_NDEV * sizeof(double), cudaMemcpyHostToDevice));
     CU(cudaMemset(s->d_theta_bar, 0, MLP1D_NPARAM * sizeof(double)));
     for (int k = 0; k < 4; ++k) { s->in_scale[k] = in_scale[k]; s->out_scale[k] = out_scale[k]; }
     s->mlp1d_on = true;

@@ -15,10 +15,13 @@ namespace jxs {
 
 constexpr int MLP1D_NPARAM = 6020;  // W1[64][24], b1[64], W2[64][64], b2[64], W3[4][64], b3[4]
 constexpr int MLP1D_W1 = 0, MLP1D_B1 = 1536, MLP1D_W2 = 1600, MLP1D_B2 = 5696, MLP1D_W3 = 5760, MLP1D_B3 = 6016;
+// the device copy of the parameters carries W1 and W2 a second time, transposed (W1T[24][64], W2T[64][64]): with lane
+// l owning hidden units l and l + 32 the forward pass reads a column of W per step, which is a row of the transpose
+constexpr int MLP1D_W1T = 6020, MLP1D_W2T = 6020 + 1536, MLP1D_NDEV = 6020 + 1536 + 4096;
 
 struct Mlp1dArgs {
   const void* U;        // padded state, ghosts filled (row 3 of [4][.][pitch])
-  const double* theta;  // the 6020 parameters, in the order of jxs_set_flux_mlp
+  const double* theta;  // MLP1D_NDEV doubles: the 6020 parameters in the order of jxs_set_flux_mlp, then W1T, W2T
   double* dF;           // [4] planes, same indexing as U: the correction of the flux through the RIGHT face of a cell
   long long plane;
   int nx, pitch;
@@ -55,16 +58,16 @@ __device__ __forceinline__ void mlp1d_forward(const double* __restrict__ th, dou
 #pragma unroll
   for (int i = 0; i < 24; ++i) {
     const double xi = __shfl_sync(0xffffffffu, x, i);
-    z0 = fma(th[MLP1D_W1 + lane * 24 + i], xi, z0);
-    z1 = fma(th[MLP1D_W1 + (lane + 32) * 24 + i], xi, z1);
+    z0 = fma(th[MLP1D_W1T + i * 64 + lane], xi, z0);
+    z1 = fma(th[MLP1D_W1T + i * 64 + lane + 32], xi, z1);
   }
   h1a = tanh(z0); h1b = tanh(z1);
   z0 = th[MLP1D_B2 + lane]; z1 = th[MLP1D_B2 + lane + 32];
 #pragma unroll 8
   for (int i = 0; i < 32; ++i) {
     const double a = __shfl_sync(0xffffffffu, h1a, i), b = __shfl_sync(0xffffffffu, h1b, i);
-    z0 = fma(th[MLP1D_W2 + lane * 64 + i], a, fma(th[MLP1D_W2 + lane * 64 + 32 + i], b, z0));
-    z1 = fma(th[MLP1D_W2 + (lane + 32) * 64 + i], a, fma(th[MLP1D_W2 + (lane + 32) * 64 + 32 + i], b, z1));
+    z0 = fma(th[MLP1D_W2T + i * 64 + lane], a, fma(th[MLP1D_W2T + (i + 32) * 64 + lane], b, z0));
+    z1 = fma(th[MLP1D_W2T + i * 64 + lane + 32], a, fma(th[MLP1D_W2T + (i + 32) * 64 + lane + 32], b, z1));
   }
   h2a = tanh(z0); h2b = tanh(z1);
 #pragma unroll
@@ -140,10 +143,11 @@ __global__ void __launch_bounds__(128) mlp1d_backward_kernel(const Mlp1dArgs A) 
     double h1ab = 0.0, h1bb = 0.0;  // adjoint of h1 units lane, lane + 32: sum over all 64 units j of W2[j][.] z2bar_j
     for (int i = 0; i < 32; ++i) {
       const double a = __shfl_sync(0xffffffffu, h1a, i), b = __shfl_sync(0xffffffffu, h1b, i);
-      add(tb + MLP1D_W2 + lane * 64 + i, z2a * a);
-      add(tb + MLP1D_W2 + lane * 64 + 32 + i, z2a * b);
-      add(tb + MLP1D_W2 + (lane + 32) * 64 + i, z2b * a);
-      add(tb + MLP1D_W2 + (lane + 32) * 64 + 32 + i, z2b * b);
+      // (the slot keeps W1 and W2 transposed, [input][unit]: neighbouring lanes, neighbouring words)
+      add(tb + MLP1D_W2 + i * 64 + lane, z2a * a);
+      add(tb + MLP1D_W2 + (i + 32) * 64 + lane, z2a * b);
+      add(tb + MLP1D_W2 + i * 64 + lane + 32, z2b * a);
+      add(tb + MLP1D_W2 + (i + 32) * 64 + lane + 32, z2b * b);
       const double za = __shfl_sync(0xffffffffu, z2a, i), zb = __shfl_sync(0xffffffffu, z2b, i);  // units i, i + 32
       h1ab = fma(th[MLP1D_W2 + i * 64 + lane], za, fma(th[MLP1D_W2 + (i + 32) * 64 + lane], zb, h1ab));
       h1bb = fma(th[MLP1D_W2 + i * 64 + lane + 32], za, fma(th[MLP1D_W2 + (i + 32) * 64 + lane + 32], zb, h1bb));
@@ -155,8 +159,8 @@ __global__ void __launch_bounds__(128) mlp1d_backward_kernel(const Mlp1dArgs A) 
     double xb = 0.0;  // adjoint of input lane (< 24)
     for (int i = 0; i < 24; ++i) {
       const double xi = __shfl_sync(0xffffffffu, x, i);
-      add(tb + MLP1D_W1 + lane * 24 + i, z1a * xi);
-      add(tb + MLP1D_W1 + (lane + 32) * 24 + i, z1b * xi);
+      add(tb + MLP1D_W1 + i * 64 + lane, z1a * xi);
+      add(tb + MLP1D_W1 + i * 64 + lane + 32, z1b * xi);
     }
     for (int j = 0; j < 32; ++j) {
       const double za = __shfl_sync(0xffffffffu, z1a, j), zb = __shfl_sync(0xffffffffu, z1b, j);  // units j, j + 32
@@ -170,8 +174,12 @@ __global__ void __launch_bounds__(128) mlp1d_backward_kernel(const Mlp1dArgs A) 
     __syncwarp();
   }
   __syncthreads();
-  for (int i = threadIdx.x; i < MLP1D_NPARAM; i += blockDim.x)
-    atomicAdd(A.theta_bar + i, (slots[i] + slots[MLP1D_NPARAM + i]) + (slots[2 * MLP1D_NPARAM + i] + slots[3 * MLP1D_NPARAM + i]));
+  for (int q = threadIdx.x; q < MLP1D_NPARAM; q += blockDim.x) {
+    int p = q;  // slot position -> parameter: the W1 and W2 blocks of a slot are transposed
+    if (q < MLP1D_B1) p = MLP1D_W1 + (q & 63) * 24 + (q >> 6);
+    else if (q >= MLP1D_W2 && q < MLP1D_B2) p = MLP1D_W2 + ((q - MLP1D_W2) & 63) * 64 + ((q - MLP1D_W2) >> 6);
+    atomicAdd(A.theta_bar + p, (slots[q] + slots[MLP1D_NPARAM + q]) + (slots[2 * MLP1D_NPARAM + q] + slots[3 * MLP1D_NPARAM + q]));
+  }
 }
 
 }  // namespace jxs
