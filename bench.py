@@ -55,17 +55,23 @@ class ClockSampler:
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index):
-        self.rows, self.proc, self.index = [], None, index
-
-    def start(self):
+        # nvidia-smi takes a few hundred ms to print its first row, longer than a short timed region: it is launched
+        # here, before the warm-up; start() marks where the timed region's rows begin.
+        self.rows, self.proc, self.index, self.first = [], None, index, 0
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
         except OSError:
             self.proc = None
+
+    def start(self):
+        t0 = time.time()
+        while self.proc and not self.rows and time.time() - t0 < 3.0:
+            time.sleep(0.01)
+        self.first = len(self.rows)
 
     def _read(self):
         for line in self.proc.stdout:
@@ -81,7 +87,7 @@ class ClockSampler:
             self.proc.kill()
         sm, mx, reasons = [], [], set()
         names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
-        for r in self.rows:
+        for r in self.rows[self.first:]:
             f = [x.strip() for x in r.split(",")]
             if len(f) < 7:
                 continue
@@ -177,9 +183,9 @@ def run_sod1d(args, rank, world, local_rank, dist, barrier, tdt):
     solver = jxs.Solver.from_case(case, dtype=tdt, stream=stream)
     U = torch.tensor(case["U0"], dtype=tdt, device="cuda")
     K, W = args.steps, args.warmup
+    sampler = ClockSampler(local_rank)
     solver.step(U, 0.4, W)
     solver.set_profiling(True)
-    sampler = ClockSampler(local_rank)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches0 = solver.launch_count()
     barrier()
@@ -420,9 +426,9 @@ def run_cnn(args, rank, world, local_rank, dist, barrier, tdt):
     solver.set_flux_cnn(wl.cnn_weights(), *wl.cnn_scales())
     U = torch.tensor(case["U0"], dtype=tdt, device="cuda")
     K, W = args.steps, args.warmup
+    sampler = ClockSampler(local_rank)
     solver.step(U, 0.4, W)
     solver.set_profiling(True)
-    sampler = ClockSampler(local_rank)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches0 = solver.launch_count()
     barrier()
@@ -606,6 +612,7 @@ def main():
     if args.workload == "cnn":
         run_cnn(args, rank, world, local_rank, dist, barrier, tdt)
         return
+    sampler = ClockSampler(local_rank)
     case = wl.throughput_case(args.nx, args.ny, viscous=not args.euler, ibm=not args.euler)
     ncell = args.nx * args.ny
     stream = torch.cuda.current_stream()
@@ -618,7 +625,6 @@ def main():
     # ---- device-resident timing: inputs already in HBM
     solver.step(U, 0.4, W)
     solver.set_profiling(True)
-    sampler = ClockSampler(local_rank)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches0 = solver.launch_count()
     barrier()
@@ -648,6 +654,15 @@ def main():
     barrier()
     e2e_value = aggregate_rate(ncell, K, world, max_over_ranks(e0.elapsed_time(e1), dist, "cuda"))
     nbytes = Uh.numel() * Uh.element_size()
+    # the same call made once per step: the whole state crosses PCIe in both directions every step
+    Kc = min(K, 10)
+    barrier()
+    e0.record(stream)
+    for _ in range(Kc):
+        solver2.step_host(Uh, 0.4, 1)
+    e1.record(stream)
+    barrier()
+    e2e_copy_value = aggregate_rate(ncell, Kc, world, max_over_ranks(e0.elapsed_time(e1), dist, "cuda"))
 
     if rank != 0:
         if dist is not None:
@@ -697,7 +712,10 @@ def main():
                    "parallelism": "replicas" if world > 1 else "single GPU"},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes / K, "d2h_bytes_per_step": nbytes / K,
-                "note": f"one jxs_step_host call of {K} steps on a pinned host buffer; bytes are the call's copies / {K}"},
+                "note": f"one jxs_step_host call of {K} steps on a pinned host buffer; bytes are the call's copies / {K}",
+                "copies_every_step": {"value": e2e_copy_value, "unit": UNIT, "steps": Kc, "h2d_bytes_per_step": nbytes,
+                                      "d2h_bytes_per_step": nbytes,
+                                      "note": "jxs_step_host(nsteps = 1) per step: PCIe-bound, the state is 256 MiB"}},
         "gpu_launches": launches,
         "roofline": roofline,
         "cpu_baseline": cpu,
