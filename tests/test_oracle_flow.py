@@ -230,6 +230,127 @@ def test_cfl_time_step_rule():
     assert o.time()[1] == pytest.approx(0.4 * min(case["dx"], case["dy"]) / smax, rel=1e-15)
 
 
+def _uniform_with(n, m, base, cells):
+    """Conserved field, uniform primitive state `base` except the listed (i, j) -> (rho, u, v, p)."""
+    W = np.empty((4, m, n))
+    for k in range(4):
+        W[k] = base[k]
+    for (i, j), w in cells.items():
+        W[:, j, i] = w
+    return wl.cons_from_prim(W[0], W[1], W[2], W[3])
+
+
+def test_max_wavespeed_closed_form_on_moving_states():
+    """O9 / R6: s_max = max over fluid cells of max(|u| + a, |v| + a), a = sqrt(gamma p / rho).  Hand-built states in
+    which the maximum is taken (a) by a cell moving in -x (|u| matters, not u), (b) by the v-branch, (c) by a slow cell
+    with a large sound speed; each number is written out with math.sqrt here.  A rule that drops the absolute value,
+    ignores v, or uses |u| + |v| + a or sqrt(u^2 + v^2) + a gives another value in at least one of them."""
+    n, m = 12, 10
+    base = (1.0, 0.1, -0.2, 1.0)
+    a0 = math.sqrt(G * 1.0 / 1.0)
+    o = jxo.Oracle(n, m, 0.1, 0.1, G, 0.0, 0.72, TRN)
+    # uniform: the v-branch wins (|v| = 0.2 > |u| = 0.1)
+    assert o.max_wavespeed(_uniform_with(n, m, base, {})) == pytest.approx(0.2 + a0, rel=1e-15)
+    # (a) one cell with u = -3 (and v = +1: |u| + a, not |u| + |v| + a, not hypot(u, v) + a)
+    fast = (2.0, -3.0, 1.0, 0.5)
+    a = math.sqrt(G * 0.5 / 2.0)
+    got = o.max_wavespeed(_uniform_with(n, m, base, {(4, 7): fast}))
+    assert got == pytest.approx(3.0 + a, rel=1e-15)
+    assert abs(got - (4.0 + a)) > 0.5 and abs(got - (math.hypot(3.0, 1.0) + a)) > 0.1 and abs(got - (1.0 + a)) > 1.0
+    # (b) the v-branch with a negative v, at the last cell of the grid (loop bounds)
+    fastv = (0.5, 0.3, -2.5, 2.0)
+    av = math.sqrt(G * 2.0 / 0.5)
+    assert o.max_wavespeed(_uniform_with(n, m, base, {(n - 1, m - 1): fastv})) == pytest.approx(2.5 + av, rel=1e-15)
+    # (c) a cell at rest with the largest sound speed, at the first cell
+    hot = (0.1, 0.0, 0.0, 10.0)
+    assert o.max_wavespeed(_uniform_with(n, m, base, {(0, 0): hot})) == pytest.approx(math.sqrt(G * 10.0 / 0.1), rel=1e-15)
+    # gamma enters through E -> p and through a: the same primitives with gamma = 1.67
+    o2 = jxo.Oracle(n, m, 0.1, 0.1, 1.67, 0.0, 0.72, TRN)
+    full = tuple(np.full((m, n), w) for w in fast)
+    U2 = wl.cons_from_prim(*full, gamma=1.67)
+    assert o2.max_wavespeed(U2) == pytest.approx(3.0 + math.sqrt(1.67 * 0.5 / 2.0), rel=1e-15)
+
+
+def test_max_wavespeed_ignores_cells_inside_a_body():
+    """O9: "fluid interior cells": the fastest cell placed inside the body (solid), and in its
+    ghost layer, must not count; the same cell outside the body does."""
+    n, m = 48, 40
+    dx = 1.0 / n
+    x = (np.arange(n) + 0.5) * dx
+    y = (np.arange(m) + 0.5) * dx
+    X, Y = np.meshgrid(x, y)
+    phi = np.hypot(X - 0.5, Y - 20.5 * dx) - 6.0 * dx
+    o = jxo.Oracle(n, m, dx, dx, G, 0.0, 0.72, TRN)
+    o.set_ibm(phi)
+    types = o.cell_types()
+    base = (1.0, 0.4, 0.0, 1.0)
+    a0 = math.sqrt(G)
+    fast = (1.0, -5.0, 0.5, 4.0)
+    af = math.sqrt(G * 4.0)
+    centre = (24, 20)                                   # deep inside: solid
+    assert types[centre[1], centre[0]] != 0 and phi[centre[1], centre[0]] < -3 * dx
+    gj, gi = [(j, i) for j in range(m) for i in range(n) if types[j, i] != 0 and phi[j, i] > -1.2 * dx][0]
+    assert types[gj, gi] != 0                           # a non-fluid cell next to the surface: ghost
+    fj, fi = 20, 40                                     # far outside: fluid
+    assert types[fj, fi] == 0
+    assert o.max_wavespeed(_uniform_with(n, m, base, {})) == pytest.approx(0.4 + a0, rel=1e-15)
+    assert o.max_wavespeed(_uniform_with(n, m, base, {centre: fast})) == pytest.approx(0.4 + a0, rel=1e-15)
+    assert o.max_wavespeed(_uniform_with(n, m, base, {(gi, gj): fast})) == pytest.approx(0.4 + a0, rel=1e-15)
+    assert o.max_wavespeed(_uniform_with(n, m, base, {(fi, fj): fast})) == pytest.approx(5.0 + af, rel=1e-15)
+    # without the body the same cell counts
+    o.set_ibm(None)
+    assert o.max_wavespeed(_uniform_with(n, m, base, {centre: fast})) == pytest.approx(5.0 + af, rel=1e-15)
+
+
+@pytest.mark.parametrize("dx,dy", [(0.05, 0.02), (0.01, 0.04)])
+def test_cfl_time_step_uses_the_smaller_spacing(dx, dy):
+    """R6: dt = cfl min(dx, dy) / s_max, with dx != dy either way round, on a moving state."""
+    n, m = 16, 12
+    U = _uniform_with(n, m, (1.0, -0.7, 0.3, 1.0), {(5, 5): (1.5, 0.2, 2.0, 3.0)})
+    smax = max(0.7 + math.sqrt(G), 2.0 + math.sqrt(G * 3.0 / 1.5))
+    o = jxo.Oracle(n, m, dx, dy, G, 0.0, 0.72, PER)
+    assert o.max_wavespeed(U) == pytest.approx(smax, rel=1e-15)
+    o.step(U, 0.3, 1)
+    t, dt = o.time()
+    assert dt == pytest.approx(0.3 * min(dx, dy) / smax, rel=1e-15) and t == dt
+
+
+def test_operation_tally_of_the_literal_evaluation():
+    """The counting scalar (jxo_count_ops): operations of ONE literal evaluation of L(U), one general RK combine and
+    one wavespeed pass on the 512x256 throughput case, per interior cell.  These are the figures DESIGN.md section 6
+    quotes next to the minimal-work count the roofline uses (the oracle shares nothing between faces and evaluates both
+    HLLC sides, so its count is the larger one)."""
+    case = wl.throughput_case(512, 256)
+    o = make(case)
+    c = o.count_ops(case["U0"])
+    n = 512 * 256
+    per = {k: v / n for k, v in c.items()}
+    # literal WENO5 (two sides x 4 variables x 2 directions), both-sided HLLC at every face, viscous fluxes, divergence,
+    # combine, wavespeed; the face counts exceed the cell count by the boundary faces, hence the tolerances
+    assert 660 < per["add"] < 670 and 686 < per["mul"] < 696, per
+    assert 206 < per["div"] < 212 and 4.9 < per["sqrt"] < 5.1, per
+    total = per["add"] + per["mul"] + per["div"] + per["sqrt"]
+    assert 1560 < total < 1580, total
+
+
+def test_float_oracle_agrees_with_the_double_oracle():
+    """The float instantiation of the oracle (JXO_F32): a uniform state gives L == 0 exactly (identical arithmetic at
+    every face), and on the smooth vortex its RHS is within float round-off of the double oracle's."""
+    n = 32
+    U = _uniform_with(n, n, (1.0, 0.5, -0.25, 2.0), {})
+    o32 = jxo.Oracle(n, n, 0.1, 0.1, G, 0.0, 0.72, PER, dtype=np.float32)
+    L = o32.rhs(U.astype(np.float32))
+    assert L.dtype == np.float32 and np.array_equal(L, np.zeros_like(L))
+    case = wl.vortex(64)
+    Ld = make(case).rhs(case["U0"])
+    Lf = make(case, dtype=np.float32).rhs(case["U0"].astype(np.float32))
+    for k in range(4):
+        assert np.max(np.abs(Lf[k] - Ld[k])) <= 1e-5 * np.max(np.abs(Ld[k])) + 1e-5, k
+    sd = make(case).max_wavespeed(case["U0"])
+    sf = make(case, dtype=np.float32).max_wavespeed(case["U0"].astype(np.float32))
+    assert abs(sf - sd) <= 1e-6 * sd
+
+
 # -------------------------------------------------------------------- viscous
 def _viscous_part(n, mu=0.05, Pr=0.72):
     rho, u, v, p = smooth_periodic_field(n, n, seed=6)
