@@ -30,9 +30,14 @@ ALG_BYTES = {"f64": 85.33, "f32": 42.67}
 # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz
 PEAK_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 PEAK_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
-# dram__bytes_read.sum + dram__bytes_write.sum of the stage kernel, per launch, mean of the three RK stages, from
-# the `ncu --set full` capture summarised in profiles/r01d_stage_f64.md (fp64, 4096x2048); None = not captured
-NCU_TRAFFIC_BYTES = {("f64", 4096, 2048, "ns"): (550.7e6 + 849.7e6 + 824.1e6) / 3}
+# dram__bytes_read.sum + dram__bytes_write.sum of the stage kernel, per launch, mean of the three RK stages of one
+# step, from an `ncu --set full` capture (never measured inside a bench run: a number taken under a profiler is not a
+# bench value).  Each entry names the profile it was read from and the commit whose kernel was captured, so that a
+# reader can tell whether it still describes the kernel being timed; None = not captured for this configuration.
+NCU_TRAFFIC = {
+    ("f64", 4096, 2048, "ns"): {"bytes": (550.7e6 + 849.7e6 + 824.1e6) / 3, "profile": "profiles/r01d_stage_f64.md",
+                                "kernel_commit": "6acb3c3"},
+}
 
 
 def max_over_ranks(ms, dist, device):
@@ -50,57 +55,113 @@ def aggregate_rate(ncell, steps, world, ms_max):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    """SM clock, power and throttle reasons of one GPU sampled DURING the timed region.
+
+    Source: NVML in-process (the library nvidia-smi itself reads), polled every ~2 ms from a thread, so that a timed
+    region of a few tens of ms still holds samples; if NVML cannot be loaded, `nvidia-smi -lms 10` as a subprocess."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    PERIOD_S = 0.002
 
     def __init__(self, index):
-        # nvidia-smi takes a few hundred ms to print its first row, longer than a short timed region: it is launched
-        # here, before the warm-up; start() marks where the timed region's rows begin.
         self.rows, self.proc, self.index, self.first = [], None, index, 0
+        self.source, self._stop, self.thread, self.nv, self.h = None, threading.Event(), None, None, None
         try:
+            import pynvml as nv
+            nv.nvmlInit()
+            self.h = self._nvml_handle(nv, index)
+            self.nv, self.source = nv, "nvml"
+            self.max_mhz = float(nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM))
+            self.thread = threading.Thread(target=self._poll_nvml, daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.nv = None
+        try:
+            # nvidia-smi takes a few hundred ms to print its first row: launched here, before the warm-up
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                          "--format=csv,noheader,nounits", "-lms", "10"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.source = "nvidia-smi -lms 10"
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
         except OSError:
             self.proc = None
 
+    @staticmethod
+    def _nvml_handle(nv, index):
+        """NVML handle of torch's device `index` (CUDA_VISIBLE_DEVICES may renumber: match by UUID)."""
+        try:
+            import torch
+            uuid = str(torch.cuda.get_device_properties(index).uuid)
+            if not uuid.startswith("GPU-"):
+                uuid = "GPU-" + uuid
+            return nv.nvmlDeviceGetHandleByUUID(uuid)
+        except Exception:
+            return nv.nvmlDeviceGetHandleByIndex(index)
+
+    def _poll_nvml(self):
+        nv, h = self.nv, self.h
+        R = nv
+        bits = (("hw_slowdown", getattr(R, "nvmlClocksEventReasonHwSlowdown", 0x8)),
+                ("hw_thermal_slowdown", getattr(R, "nvmlClocksEventReasonHwThermalSlowdown", 0x40)),
+                ("sw_thermal_slowdown", getattr(R, "nvmlClocksEventReasonSwThermalSlowdown", 0x20)),
+                ("sw_power_cap", getattr(R, "nvmlClocksEventReasonSwPowerCap", 0x4)))
+        reasons_fn = getattr(nv, "nvmlDeviceGetCurrentClocksEventReasons", None) or nv.nvmlDeviceGetCurrentClocksThrottleReasons
+        while not self._stop.is_set():
+            try:
+                mhz = float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                mask = int(reasons_fn(h))
+                watts = nv.nvmlDeviceGetPowerUsage(h) / 1000.0
+                self.rows.append((mhz, self.max_mhz, watts, tuple(n for n, b in bits if mask & b)))
+            except Exception:
+                pass
+            time.sleep(self.PERIOD_S)
+
     def start(self):
         t0 = time.time()
-        while self.proc and not self.rows and time.time() - t0 < 3.0:
-            time.sleep(0.01)
+        while (self.proc or self.nv) and not self.rows and time.time() - t0 < 3.0:
+            time.sleep(0.005)
         self.first = len(self.rows)
 
     def _read(self):
-        for line in self.proc.stdout:
-            self.rows.append(line.strip())
-
-    def stop(self):
-        if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=5)
-        except subprocess.TimeoutExpired:
-            self.proc.kill()
-        sm, mx, reasons = [], [], set()
         names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
-        for r in self.rows[self.first:]:
-            f = [x.strip() for x in r.split(",")]
+        for line in self.proc.stdout:
+            f = [x.strip() for x in line.strip().split(",")]
             if len(f) < 7:
                 continue
             try:
-                sm.append(float(f[0])); mx.append(float(f[1]))
+                self.rows.append((float(f[0]), float(f[1]), float(f[2]),
+                                  tuple(n for n, v in zip(names, f[3:7]) if v.lower().startswith("active"))))
             except ValueError:
                 continue
-            for n, v in zip(names, f[3:7]):
-                if v.lower().startswith("active"):
-                    reasons.add(n)
-        sm.sort()
-        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "samples": len(sm), "reasons": sorted(reasons)}
+
+    def stop(self):
+        if not self.proc and not self.nv:
+            return {"sm_mhz": None, "sm_max_mhz": None, "samples": 0, "reasons": ["nvml and nvidia-smi unavailable"]}
+        n_end = len(self.rows)
+        self._stop.set()
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self.proc.kill()
+        rows = self.rows[self.first:n_end]
+        sm = sorted(r[0] for r in rows)
+        reasons = sorted({n for r in rows for n in r[3]})
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max((r[1] for r in rows), default=None),
+                "sm_min_mhz": sm[0] if sm else None, "power_w_max": max((r[2] for r in rows), default=None),
+                "samples": len(sm), "reasons": reasons, "source": self.source}
+
+
+MIN_REGION_S = 0.25   # a timed region shorter than this is repeated back to back (see repeats_for)
+
+
+def repeats_for(ms_one_call):
+    """How many back-to-back repetitions of the K-step call make the timed region span MIN_REGION_S, so that the clock
+    sampler sees the region (a 20-step region lasts 26 ms); the mean over the repetitions is reported."""
+    return max(1, int(math.ceil(MIN_REGION_S * 1e3 / max(ms_one_call, 1e-3))))
 
 
 def oracle_rate(case, nsteps):
@@ -562,6 +623,9 @@ def main():
     ap.add_argument("--euler", action="store_true", help="mu = 0, no IBM (not the headline config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile-kernels", action="store_true", help="c5 only: per-kernel CUDA-event spans")
+    ap.add_argument("--rows-per-segment", type=int, default=0,
+                    help="fix the stage kernel's row-segment length (jxs_set_rows_per_segment) instead of measuring it at the "
+                         "first step call: used for ncu captures, which would otherwise land in the ~40 tuning launches")
     ap.add_argument("--workload", choices=("c4", "c5", "sod1d", "cnn", "tangent1d", "adjoint1d", "train1d"), default="c4",
                     help="c4 = the headline throughput case (default); c5 = BASELINE.json configs[4]: 16 independent "
                          "1024x512 shock-cylinder runs with the per-face flux MLP, one stream per handle; sod1d = the "
@@ -617,26 +681,37 @@ def main():
     ncell = args.nx * args.ny
     stream = torch.cuda.current_stream()
     solver = jxs.Solver.from_case(case, dtype=tdt, stream=stream)
+    if args.rows_per_segment > 0:
+        solver.set_rows_per_segment(args.rows_per_segment)
     U = torch.tensor(case["U0"], dtype=tdt, device="cuda")
     K, W = args.steps, args.warmup
 
     peak_meas = jxs.measure_fp64_peak(200.0) if args.dtype == "f64" else None
 
     # ---- device-resident timing: inputs already in HBM
-    solver.step(U, 0.4, W)
-    solver.set_profiling(True)
+    solver.step(U, 0.4, W)            # warm-up; the first call also measures the row-segment length (jxs_tune)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    solver.step(U, 0.4, K)            # untimed: how long one K-step call lasts decides the repetitions below
+    e1.record(stream)
+    torch.cuda.synchronize()
+    R = repeats_for(max_over_ranks(e0.elapsed_time(e1), dist, "cuda"))
+    solver.set_profiling(True)
     launches0 = solver.launch_count()
+    stage_ms, stage_n = 0.0, 0
     barrier()
     sampler.start()
     e0.record(stream)
-    solver.step(U, 0.4, K)
+    for _ in range(R):                # R back-to-back calls of EXACTLY K steps each; the mean call is reported
+        solver.step(U, 0.4, K)
+        m, n = solver.stage_time()
+        stage_ms, stage_n = stage_ms + m, stage_n + n
     e1.record(stream)
     barrier()
     clocks = sampler.stop()
-    launches = solver.launch_count() - launches0
-    ms = e0.elapsed_time(e1)
-    stage_ms, stage_n = solver.stage_time()
+    launches = (solver.launch_count() - launches0) // R
+    ms = e0.elapsed_time(e1) / R
+    stage_ms, stage_n = stage_ms / R, stage_n // R
     solver.set_profiling(False)
     if not bool(torch.isfinite(U).all()):
         raise SystemExit("bench.py: non-finite state after the timed region")
@@ -646,13 +721,16 @@ def main():
     # ---- end to end through the C ABI with HOST buffers (copies inside the timed region)
     Uh = torch.tensor(case["U0"], dtype=tdt).pin_memory()
     solver2 = jxs.Solver.from_case(case, dtype=tdt, stream=stream)
+    if args.rows_per_segment > 0:
+        solver2.set_rows_per_segment(args.rows_per_segment)
     solver2.step_host(Uh.clone().pin_memory(), 0.4, 3)
     barrier()
     e0.record(stream)
-    solver2.step_host(Uh, 0.4, K)
+    for _ in range(R):
+        solver2.step_host(Uh, 0.4, K)
     e1.record(stream)
     barrier()
-    e2e_value = aggregate_rate(ncell, K, world, max_over_ranks(e0.elapsed_time(e1), dist, "cuda"))
+    e2e_value = aggregate_rate(ncell, K, world, max_over_ranks(e0.elapsed_time(e1) / R, dist, "cuda"))
     nbytes = Uh.numel() * Uh.element_size()
     # the same call made once per step: the whole state crosses PCIe in both directions every step
     Kc = min(K, 10)
@@ -680,10 +758,13 @@ def main():
         hbm_gbs = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
     except Exception:
         pass
-    traffic = NCU_TRAFFIC_BYTES.get((args.dtype, args.nx, args.ny, kind))
+    traffic_rec = NCU_TRAFFIC.get((args.dtype, args.nx, args.ny, kind))
+    traffic = traffic_rec["bytes"] if traffic_rec else None
     roofline = {
         "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-        "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r01d_stage_f64.md)",
+        "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
+        "traffic_source": ({"profile": traffic_rec["profile"], "kernel_commit": traffic_rec["kernel_commit"]}
+                           if traffic_rec else None),
         "kernel": "jxs::stage_kernel", "avg_launch_ms": stage_avg_ms, "launches_timed": stage_n,
         "share_of_step": stage_ms / ms,
         "alg_flop_per_cell_stage": ALG_FLOP[kind], "alg_bytes_per_cell_stage": ALG_BYTES[args.dtype],
@@ -708,11 +789,15 @@ def main():
         "config": {"workload": f"throughput_{args.nx}x{args.ny}" + ("_euler" if args.euler else
                    " (BASELINE.json configs[3]: Mach-3 shock over 8 seeded cylinders, Navier-Stokes Re 1e5, IBM)"),
                    "cfl": 0.4, "rk": "SSP-RK3", "cells": ncell, "stages_per_step": 3,
+                   "timed_region": f"{R} back-to-back jxs_step calls of {K} steps each (>= {MIN_REGION_S} s in all, so that "
+                                   f"the clock sampler sees the region); ms_per_step, value and e2e are the mean call",
+                   "repeats": R,
                    "l2": "inputs larger than L2 (3 x 256 MiB state buffers vs 126 MB), no flush needed",
                    "parallelism": "replicas" if world > 1 else "single GPU"},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes / K, "d2h_bytes_per_step": nbytes / K,
-                "note": f"one jxs_step_host call of {K} steps on a pinned host buffer; bytes are the call's copies / {K}",
+                "note": f"jxs_step_host calls of {K} steps on a pinned host buffer ({R} back to back, mean); bytes are one "
+                        f"call's copies / {K}",
                 "copies_every_step": {"value": e2e_copy_value, "unit": UNIT, "steps": Kc, "h2d_bytes_per_step": nbytes,
                                       "d2h_bytes_per_step": nbytes,
                                       "note": "jxs_step_host(nsteps = 1) per step: PCIe-bound, the state is 256 MiB"}},

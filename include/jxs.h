@@ -26,7 +26,9 @@
  *   - all device work is enqueued on the stream given to jxs_create (0 = default stream).
  *     Functions returning a host scalar synchronise that stream; jxs_rhs does not;
  *     jxs_step* synchronise once at the end to read the non-finite flag.
- *   - there is no CPU fallback: without a CUDA device jxs_create fails with JXS_ECUDA.
+ *   - there is no CPU fallback: without a CUDA device jxs_create fails with JXS_ECUDA (also on a device that is
+ *     not compute capability 10.0: the library holds sm_100a code only).  A handle belongs to the device that was
+ *     current at jxs_create; calls made with another device current return JXS_ESTATE.
  */
 #ifndef JXS_H
 #define JXS_H
@@ -109,7 +111,8 @@ int jxs_flux_cnn_inputs(jxs_solver*, const void* U, float* Xx, float* Xy);
  * JXS_ESTATE with steps pending (jxs_wait).                                                   */
 int jxs_set_gamma(jxs_solver*, double gamma);
 
-/* Laplacian artificial viscosity nu * Lap_h(U) of PAPER.md Eq. 10; default 0 (R7).          */
+/* Laplacian artificial viscosity nu * Lap_h(U) of PAPER.md Eq. 10; default 0 (R7).  Drops a recorded
+ * trajectory.  JXS_EINVAL for nu < 0 or non-finite (nothing changes), JXS_ESTATE with steps pending. */
 int jxs_set_artificial_viscosity(jxs_solver*, double nu);
 
 /* dUdt = L(U): ghost fills on an internal copy of U, then the fused stage kernel with the
@@ -123,9 +126,10 @@ int jxs_max_wavespeed(jxs_solver*, const void* U, double* smax_host);
  * device at the start of every step (R6).  JXS_ENUMERIC if a non-finite or non-positive
  * wavespeed was met (U then holds the last state computed).  Synchronises once at the end.
  * For nsteps >= 6 (and jxs_set_profiling off) pairs of steps are replayed from a CUDA graph
- * captured on a private stream; results are identical to plain launches.  The first stepping call
- * of a handle on a large grid also times about forty stage launches to choose the length of the row
- * segments the grid is cut into (it synchronises the stream once; results do not depend on it).   */
+ * captured on a private stream; results are identical to plain launches (jxs_set_graph_replay(h, 0) turns
+ * the replay off).  The first synchronous stepping call of a handle on a large grid also times about forty
+ * stage launches to choose the length of the row segments the grid is cut into (jxs_tune, below; it
+ * synchronises the stream once; results do not depend on it).                                        */
 int jxs_step(jxs_solver*, void* U, double cfl, int nsteps);
 /* Same with a fixed time step.                                                              */
 int jxs_step_fixed_dt(jxs_solver*, void* U, double dt, int nsteps);
@@ -165,9 +169,9 @@ int jxs_mse_tangent(jxs_solver*, const void* U, const void* Udot, const void* Ut
  * *gamma_bar (HOST) = <dU^{n+m}/dgamma at fixed initial conserved state, Ubar>.  For every direction (Udot, gamma_dot),
  * with Udot_end from jxs_step_fixed_dt_tangent: <Ubar on entry, Udot_end> = <Ubar on return, Udot> + gamma_bar gamma_dot.
  * May be called repeatedly on one recording.  Branches of the scheme carry the derivative of the branch taken.
- * Errors: JXS_EINVAL for NULL pointers, dt <= 0, nsteps < 1, an fp32 handle or ny != 1; JXS_ESTATE with a network,
- * steps pending, or (adjoint) nothing recorded; JXS_ENOMEM when the trajectory does
- * not fit.  The recording stays (and its memory is reused by the next record call) until jxs_destroy.  Both
+ * Errors: JXS_EINVAL for NULL pointers, dt <= 0, nsteps < 1, an fp32 handle or ny != 1; JXS_ESTATE with steps
+ * pending, or (adjoint) nothing recorded (changing gamma, nu or the network drops a recording); JXS_ENOMEM when the
+ * trajectory does not fit.  With the per-face MLP set on the handle (see jxs_flux_mlp_gradient below) both calls include it.  The recording stays (and its memory is reused by the next record call) until jxs_destroy.  Both
  * synchronise the stream.                                                                                         */
 int jxs_step_fixed_dt_record(jxs_solver*, void* U, double dt, int nsteps);
 int jxs_adjoint_steps(jxs_solver*, void* Ubar, double* gamma_bar);
@@ -210,6 +214,18 @@ int jxs_rhs_host(jxs_solver*, const void* U_host, void* dUdt_host);
  * U must stay valid until jxs_wait returns.                                                  */
 int jxs_step_async(jxs_solver*, void* U, double cfl, int nsteps);
 int jxs_wait(jxs_solver*);
+/* The work decomposition of the fused stage kernel: the grid is cut into column strips and
+ * each strip into row segments of `rows` rows, one task each.  Results never depend on it.
+ *   jxs_tune                  times one stage launch per candidate segment length around the heuristic's choice on the
+ *                             handle's own buffers (about forty launches, one stream synchronisation) and keeps the best;
+ *                             jxs_step / jxs_step_fixed_dt / jxs_step_host do this themselves on their first call,
+ *                             jxs_step_async never does (it only enqueues): call jxs_tune once before an async loop.
+ *                             JXS_ESTATE with steps pending.
+ *   jxs_set_rows_per_segment  rows > 0 fixes the segment length (no measurement); 0 returns to the heuristic + jxs_tune.
+ *   jxs_set_graph_replay      on = 0: plain launches instead of the replayed two-step CUDA graph (default on).   */
+int jxs_tune(jxs_solver*);
+int jxs_set_rows_per_segment(jxs_solver*, int rows);
+int jxs_set_graph_replay(jxs_solver*, int on);
 /* Performance hint for such ensembles: n handles of about this size step concurrently, so this handle sizes
  * its tasks for 1/n of the GPU (longer row segments, fewer warm-up rows) instead of trying to fill it alone.
  * Results do not change.  Default 1.                                                           */

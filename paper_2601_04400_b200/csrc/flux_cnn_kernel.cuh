@@ -7,15 +7,12 @@
 // variables (rho, rho u_n, rho u_t, E) / in_scale (R19).  Three passes per direction, one kernel each:
 //
 //   cnn_recon_kernel   U (padded, ghosts filled) -> the two input fields, bf16, 16 bytes per face
-//   cnn_layer_kernel   one 3x3 convolution as an implicit GEMM on tcgen05: a CTA marches a strip of 128 faces
-//                      row by row; the last three input rows sit in shared memory in the K-major core-matrix
-//                      layout  [8-channel chunk][face][16 B], so that tap (da, db) of the convolution is ONE
-//                      tcgen05.mma whose A descriptor points at (row buffer da, 16*db bytes into it): im2col without
-//                      a copy.  9 * Cin/16 MMAs of 128 x Cout x 16 accumulate in TMEM; bias, ReLU (tanh in the last
-//                      layer) and the rounding to bf16 follow in registers.
-//   cnn_layer3_kernel  the same layer with the three ROW taps stacked along N (one MMA feeds three output rows):
-//                      a third of the MMAs; this is the kernel the library launches, cnn_layer_kernel is kept for
-//                      measurements (JXS_CNN_NINE_TAPS).
+//   cnn_layer3_kernel  one 3x3 convolution as an implicit GEMM on tcgen05: a CTA marches a strip of 128 faces
+//                      row by row; the current input row sits in shared memory in the K-major core-matrix layout
+//                      [8-channel chunk][face][16 B], so that face tap db of the convolution is a tcgen05.mma whose
+//                      A descriptor points 16*db bytes into the row buffer: im2col without a copy.  The three ROW
+//                      taps are stacked along N (one MMA feeds three output rows): 3 * Cin/16 MMAs per row accumulate
+//                      in TMEM; bias, ReLU (tanh in the last layer) and the rounding to bf16 follow in registers.
 //
 // Activation fields in HBM use the same chunked layout with a one-face border of zeros all around (the "SAME"
 // padding of every layer is then just what the loads find): element (row r, chunk c, face p) is the uint4 at
@@ -154,143 +151,13 @@ struct CnnLayerArgs {
   int pitch, row_off, col_off;
 };
 
-template <int KC, int NOUT>
-__host__ __device__ constexpr int cnn_wbytes() { return 9 * KC * NOUT * 16 * 2; }
 template <int KC>
 __host__ __device__ constexpr int cnn_slot_bytes() { return 2 * KC * CNN_ROWP * 16; }  // 2 chunks per K step
-template <int KC, int NOUT>
-__host__ __device__ constexpr int cnn_smem_bytes() {
-  return (cnn_wbytes<KC, NOUT>() + NOUT * 4 + 127) / 128 * 128 + 3 * cnn_slot_bytes<KC>() + 16;
-}
+// CIN8 (below) = 8-channel chunks the input field really has (1 for the first layer: its second chunk stays zero)
 
-// CIN8 = 8-channel chunks the input field really has (1 for the first layer: its second chunk stays zero)
-template <int KC, int CIN8, int NOUT, bool LAST>
-__global__ void __launch_bounds__(CNN_TILE) cnn_layer_kernel(const CnnLayerArgs A) {
-  extern __shared__ __align__(128) unsigned char sm[];
-  __shared__ uint32_t tmem_slot;
-  constexpr int WB = cnn_wbytes<KC, NOUT>();
-  constexpr int OFF_ROWS = (WB + NOUT * 4 + 127) / 128 * 128;
-  constexpr int SLOT = cnn_slot_bytes<KC>();
-  constexpr int LBO_A = CNN_ROWP * 16;  // between the two 8-channel chunks of a K step
-  const int t = threadIdx.x, warp = t >> 5;
-  const int nstrips = (A.in.nb + CNN_TILE - 1) / CNN_TILE;
-  const int strip = blockIdx.x % nstrips, seg = blockIdx.x / nstrips;
-  const int abeg = seg * A.rows_per_seg, aend = min(abeg + A.rows_per_seg, A.in.na);
-  if (abeg >= aend) return;
-  const int b0 = strip * CNN_TILE;  // first output face of the strip; the window is faces b0-1 .. b0+128
-  const uint32_t sm_u32 = (uint32_t)__cvta_generic_to_shared(sm);
-  const uint32_t bar = sm_u32 + OFF_ROWS + 3 * SLOT;
-  const float* bias = reinterpret_cast<const float*>(sm + WB);
-
-  for (int i = t; i < (WB + NOUT * 4) / 16; i += CNN_TILE)
-    reinterpret_cast<uint4*>(sm)[i] = reinterpret_cast<const uint4*>(A.blob)[i];
-  for (int i = t; i < 3 * SLOT / 16; i += CNN_TILE)  // chunks the field does not have stay zero
-    reinterpret_cast<uint4*>(sm + OFF_ROWS)[i] = make_uint4(0, 0, 0, 0);
-  if (t == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(1) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  if (warp == 0) tmem_alloc((uint32_t)__cvta_generic_to_shared(&tmem_slot), 32);
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = tmem_slot;
-  const uint32_t tlane = tmem + ((uint32_t)(32 * warp) << 16);
-  constexpr uint32_t IDESC = umma_idesc(128, NOUT);
-  uint32_t phase = 0;
-
-  // input row r -> ring slot (r + 1) % 3, window faces b0-1 .. b0+128 at buffer positions 0 .. 129.  The global
-  // loads of a row are issued one iteration before its stores, so their latency hides behind the MMAs and the
-  // epilogue of the row in between.
-  uint4 pre[CIN8], pre2[CIN8];  // my face (and, threads 0-1, one of the two extra faces) of the row in flight
-  auto fetch_row = [&](int r) {
-#pragma unroll
-    for (int c = 0; c < CIN8; ++c) {
-      const uint4* src = A.in.data + A.in.at(r, c, b0 - 1);
-      pre[c] = src[t];
-      if (t < 2) pre2[c] = src[CNN_TILE + t];
-    }
-  };
-  auto store_row = [&](int r) {
-    unsigned char* dst = sm + OFF_ROWS + ((r + 1) % 3) * SLOT;
-#pragma unroll
-    for (int c = 0; c < CIN8; ++c) {
-      reinterpret_cast<uint4*>(dst + c * LBO_A)[t] = pre[c];
-      if (t < 2) reinterpret_cast<uint4*>(dst + c * LBO_A)[CNN_TILE + t] = pre2[c];
-    }
-  };
-  fetch_row(abeg - 1); store_row(abeg - 1);
-  fetch_row(abeg); store_row(abeg);
-  fetch_row(abeg + 1);
-  for (int a = abeg; a < aend; ++a) {
-    store_row(a + 1);  // rows -1 and na are the zero border of the field
-    if (a + 1 < aend) fetch_row(a + 2);
-    fence_async_smem();
-    tc_fence_before();
-    __syncthreads();
-    if (t == 0) {
-      tc_fence_after();
-      uint32_t acc = 0;
-#pragma unroll
-      for (int da = 0; da < 3; ++da) {
-        const uint32_t rowbuf = sm_u32 + OFF_ROWS + ((a + da) % 3) * SLOT;  // row a + da - 1
-#pragma unroll
-        for (int db = 0; db < 3; ++db)
-#pragma unroll
-          for (int ks = 0; ks < KC; ++ks) {
-            umma_bf16(tmem, umma_desc(rowbuf + ks * 2 * LBO_A + db * 16, LBO_A, 128),
-                      umma_desc(sm_u32 + ((da * 3 + db) * KC + ks) * NOUT * 32, NOUT * 16, 128), IDESC, acc);
-            acc = 1;
-          }
-      }
-      umma_commit(bar);
-    }
-    mbar_wait_spin(bar, phase); phase ^= 1;
-    tc_fence_after();
-    const int p = b0 + t;
-    if (!LAST) {
-#pragma unroll
-      for (int h = 0; h < NOUT / 16; ++h) {
-        uint32_t v[16];
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                       "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                     : "r"(tlane + 16 * h) : "memory");
-        tmem_ld_wait();
-        if (p < A.in.nb) {
-#pragma unroll
-          for (int c = 0; c < 2; ++c) {
-            uint32_t w[4];
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              const int k = 8 * c + 2 * e;
-              const float s0 = fmaxf(__uint_as_float(v[k]) + bias[16 * h + k], 0.f);
-              const float s1 = fmaxf(__uint_as_float(v[k + 1]) + bias[16 * h + k + 1], 0.f);
-              w[e] = pack_bf16(s0, s1);
-            }
-            A.out.data[A.out.at(a, 2 * h + c, p)] = make_uint4(w[0], w[1], w[2], w[3]);
-          }
-        }
-      }
-    } else {
-      uint32_t y[4];
-      tmem_ld4(tlane, y);
-      tmem_ld_wait();
-      if (p < A.in.nb) {
-        float* o = A.dst + (size_t)(a + A.row_off) * A.pitch + p + A.col_off;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) o[k * A.plane] = tanh_f32(__uint_as_float(y[k]) + bias[k]);
-      }
-    }
-    tc_fence_before();  // the next row's MMAs overwrite the columns just read
-  }
-  __syncthreads();
-  if (warp == 0) tmem_dealloc(tmem, 32);
-}
-
-// ------------------------------------------------------------------ the same layer with the row taps stacked along N
+// ------------------------------------------------------------------ the layer, with the row taps stacked along N
 // A 128 x N x 16 MMA with N <= 32 costs ~64 cycles whatever it computes (measured: the tensor core's fetch of the
-// 4 KB activation tile), so the layer above is bound by its 9 * KC MMAs per row.  Input row r feeds THREE output
+// 4 KB activation tile), so a layer with one MMA per tap is bound by its 9 * KC MMAs per row.  Input row r feeds THREE output
 // rows (r+1 with row tap 0, r with tap 1, r-1 with tap 2) from the same shifted windows, so one MMA with the three
 // taps' weights side by side (N = 3 * NOUT) does the work of three: 3 * KC MMAs per row.  The three accumulators
 // (TMEM column groups g = output row mod 3) are always accumulated into; the group whose output row is complete

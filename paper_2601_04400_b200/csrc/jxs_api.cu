@@ -41,6 +41,7 @@ struct jxs_solver {
   jxs_bc bc{};
   cudaStream_t stream = nullptr;
   int num_sms = 0;
+  int dev = 0;  // the device the handle was created on (and every call must be made on)
   // padded layout
   int pitch = 0;
   long long plane = 0;
@@ -93,7 +94,6 @@ struct jxs_solver {
   // the three layers' weight blobs; shares d_dF / d_dG / out_scale with the MLP path (one of the two at a time)
   bool cnn_on = false;
   CnnField cnn_X[2] = {}, cnn_H1[2] = {}, cnn_H2[2] = {};
-  uint8_t* d_cnn_blob[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
   uint8_t* d_cnn_blob3[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};  // for cnn_layer3_kernel
   double cnn_in_scale[4] = {1, 1, 1, 1};
   int mlp_strips = 0, mlp_rows_per_seg = 0, mlp_grid = 0;
@@ -116,6 +116,8 @@ struct jxs_solver {
   int nstrips = 0, rows_per_seg = 0, nseg = 0, ntasks = 0, warps = 0, grid = 0;
   int share = 1;  // handles of about this size that step concurrently (jxs_set_concurrent_handles)
   bool tuned = false;  // rows_per_seg measured on this device (tune_decomposition)
+  int rows_fixed = 0;  // jxs_set_rows_per_segment: > 0 overrides the heuristic and the measurement
+  bool use_graph = true;  // jxs_set_graph_replay
   // bookkeeping
   long long launches = 0;
   bool profiling = false;
@@ -140,6 +142,32 @@ int cuda_fail(const jxs_solver* s, cudaError_t e, const char* what) {
   do {                                                       \
     cudaError_t e_ = (call);                                 \
     if (e_ != cudaSuccess) return cuda_fail(s, e_, #call);   \
+  } while (0)
+
+// cudaFuncSetAttribute is per device: one flag per (kernel instantiation, device)
+constexpr int MAX_DEVICES = 64;
+template <typename K>
+cudaError_t configure_smem(const jxs_solver* s, K kern, bool (&done)[MAX_DEVICES], int smem) {
+  const int d = s->dev;
+  if (d < 0 || d >= MAX_DEVICES) return cudaErrorInvalidDevice;
+  if (done[d]) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  if (e == cudaSuccess) done[d] = true;
+  return e;
+}
+// every entry point that enqueues work checks that the caller is on the handle's device
+int check_device(const jxs_solver* s) {
+  int d = -1;
+  if (cudaGetDevice(&d) != cudaSuccess) return fail(s, JXS_ECUDA, "cudaGetDevice failed");
+  if (d != s->dev) return fail(s, JXS_ESTATE, "the current CUDA device is not the one the handle was created on");
+  return JXS_OK;
+}
+#define DEV(s)                              \
+  do {                                      \
+    const int rc_ = check_device(s);        \
+    if (rc_ != JXS_OK) return rc_;          \
   } while (0)
 
 GridDims dims(const jxs_solver* s) { return GridDims{s->nx, s->ny, s->pitch, s->plane}; }
@@ -214,10 +242,10 @@ void choose_decomposition(jxs_solver* s) {
   int best_rps = lo;
   for (int rps = lo; rps <= s->ny; ++rps)
     if (cost[rps] <= 1.01 * best) best_rps = rps;  // the longest segments among the near-optimal
-  if (const char* e = getenv("JXS_ROWS_PER_SEG")) best_rps = std::max(1, std::min(s->ny, atoi(e)));
+  if (s->rows_fixed > 0) best_rps = std::max(1, std::min(s->ny, s->rows_fixed));
   set_rows_per_seg(s, best_rps);
   s->warps = STAGE_WARPS;
-  s->tuned = getenv("JXS_ROWS_PER_SEG") != nullptr;
+  s->tuned = s->rows_fixed > 0;
 }
 
 template <typename T, bool VISC, bool ARTV, bool MLP>
@@ -225,14 +253,8 @@ cudaError_t launch_stage_t(jxs_solver* s, const StageArgs<T>& a) {
   auto kern = stage_kernel<T, VISC, ARTV, MLP, stage_minb<T>()>;
   constexpr int NV = VISC ? 5 : 4;
   const size_t smem = stage_smem_per_warp<T, NV>();
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  static bool configured[MAX_DEVICES] = {false};
+  if (cudaError_t e = configure_smem(s, kern, configured, (int)smem); e != cudaSuccess) return e;
   int bi = 0;  // which padded buffer is U_in
   while (bi < 3 && s->buf[bi] != (const void*)a.Uin) ++bi;
   if (bi == 3) return cudaErrorInvalidValue;
@@ -323,14 +345,8 @@ cudaError_t launch_flux_mlp(jxs_solver* s, const void* U) {
   for (int k = 0; k < 4; ++k) A.inv_scale[k] = (T)(1.0 / s->in_scale[k]);
   std::memcpy(A.bias, s->mlp_bias, sizeof(A.bias));
   auto kern = flux_mlp_kernel<T>;
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, MLP_SMEM);
-    if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  static bool configured[MAX_DEVICES] = {false};
+  if (cudaError_t e = configure_smem(s, kern, configured, MLP_SMEM); e != cudaSuccess) return e;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (s->profiling && s->mlp_events_used + 2 <= (int)s->mlp_events.size()) {
     e0 = s->mlp_events[s->mlp_events_used++];
@@ -345,35 +361,12 @@ cudaError_t launch_flux_mlp(jxs_solver* s, const void* U) {
 // the CNN flux of the padded, ghost-filled state U -> d_dF, d_dG: reconstruction pass, then three convolution
 // layers per direction
 template <int KC, int CIN8, int NOUT, bool LAST>
-cudaError_t launch_cnn_layer(jxs_solver* s, const CnnLayerArgs& A0) {
-  CnnLayerArgs A = A0;
-  auto kern = cnn_layer_kernel<KC, CIN8, NOUT, LAST>;
-  constexpr int smem = cnn_smem_bytes<KC, NOUT>();
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
-  const int nstrips = (A.in.nb + CNN_TILE - 1) / CNN_TILE;
-  const int segs = std::max(1, s->num_sms * 8 / nstrips);
-  A.rows_per_seg = std::max((A.in.na + segs - 1) / segs, std::min(A.in.na, 8));
-  const int grid = nstrips * ((A.in.na + A.rows_per_seg - 1) / A.rows_per_seg);
-  kern<<<grid, CNN_TILE, smem, s->stream>>>(A);
-  s->launches++;
-  return cudaGetLastError();
-}
-template <int KC, int CIN8, int NOUT, bool LAST>
 cudaError_t launch_cnn_layer3(jxs_solver* s, const CnnLayerArgs& A0) {
   CnnLayerArgs A = A0;
   auto kern = cnn_layer3_kernel<KC, CIN8, NOUT, LAST>;
   constexpr int smem = cnn3_smem_bytes<KC, NOUT>();
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  static bool configured[MAX_DEVICES] = {false};
+  if (cudaError_t e = configure_smem(s, kern, configured, smem); e != cudaSuccess) return e;
   const int nstrips = (A.in.nb + CNN_TILE - 1) / CNN_TILE;
   const int segs = std::max(1, s->num_sms * 8 / nstrips);
   A.rows_per_seg = std::max((A.in.na + segs - 1) / segs, std::min(A.in.na, 8));
@@ -395,8 +388,7 @@ cudaError_t launch_flux_cnn(jxs_solver* s, const void* U) {
   cnn_recon_kernel<T><<<grid, CNN_RX * CNN_RY, 0, s->stream>>>(R);
   s->launches++;
   cudaError_t e = cudaGetLastError();
-  static const bool nine = getenv("JXS_CNN_NINE_TAPS") != nullptr;  // measurement: one MMA per tap (cnn_layer_kernel)
-  for (int d = 0; d < 2 && e == cudaSuccess && !nine; ++d) {
+  for (int d = 0; d < 2 && e == cudaSuccess; ++d) {
     CnnLayerArgs A{};
     A.plane = s->plane; A.pitch = s->pitch;
     A.in = s->cnn_X[d]; A.out = s->cnn_H1[d]; A.blob = s->d_cnn_blob3[d][0];
@@ -409,20 +401,6 @@ cudaError_t launch_flux_cnn(jxs_solver* s, const void* U) {
     A.dst = d == 0 ? s->d_dF : s->d_dG;
     A.row_off = d == 0 ? 3 : 2; A.col_off = d == 0 ? 2 : 3;
     e = launch_cnn_layer3<1, 2, 16, true>(s, A);
-  }
-  for (int d = 0; d < 2 && e == cudaSuccess && nine; ++d) {
-    CnnLayerArgs A{};
-    A.plane = s->plane; A.pitch = s->pitch;
-    A.in = s->cnn_X[d]; A.out = s->cnn_H1[d]; A.blob = s->d_cnn_blob[d][0];
-    e = launch_cnn_layer<1, 1, 32, false>(s, A);
-    if (e != cudaSuccess) break;
-    A.in = s->cnn_H1[d]; A.out = s->cnn_H2[d]; A.blob = s->d_cnn_blob[d][1];
-    e = launch_cnn_layer<2, 4, 16, false>(s, A);
-    if (e != cudaSuccess) break;
-    A.in = s->cnn_H2[d]; A.blob = s->d_cnn_blob[d][2];
-    A.dst = d == 0 ? s->d_dF : s->d_dG;  // x: row j -> padded row j+3, face f -> column f+2; y: face-row f -> f+2, i -> i+3
-    A.row_off = d == 0 ? 3 : 2; A.col_off = d == 0 ? 2 : 3;
-    e = launch_cnn_layer<1, 2, 16, true>(s, A);
   }
   return e;
 }
@@ -477,27 +455,9 @@ void pack_canonical(const float* W, int N, int Kin, int Npad, int Kpad, uint8_t*
     }
 }
 
-// one convolution layer's blob: [9 taps][KC][NOUT x 16] canonical bf16 tiles + NOUT fp32 biases.
 // W is OIHW [cout][cin][3 tangential taps][3 normal taps]; the kernel's tap (row offset, face offset) is
 // (tangential, normal) for x-faces and (normal, tangential) for y-faces (transposed = true).
-std::vector<uint8_t> pack_cnn_layer(const float* W, const float* b, int cout, int cin, int KC, int NOUT, bool transposed) {
-  std::vector<uint8_t> blob((size_t)9 * KC * NOUT * 32 + NOUT * 4, 0);
-  std::vector<float> tile((size_t)NOUT * 16);
-  for (int dr = 0; dr < 3; ++dr)
-    for (int dp = 0; dp < 3; ++dp)
-      for (int ks = 0; ks < KC; ++ks) {
-        std::fill(tile.begin(), tile.end(), 0.f);
-        const int ta = transposed ? dp : dr, tb = transposed ? dr : dp;
-        for (int n = 0; n < cout; ++n)
-          for (int k = 0; k < 16 && 16 * ks + k < cin; ++k)
-            tile[(size_t)n * 16 + k] = W[(((size_t)n * cin + 16 * ks + k) * 3 + ta) * 3 + tb];
-        pack_canonical(tile.data(), NOUT, 16, NOUT, 16, blob.data() + ((size_t)(dr * 3 + dp) * KC + ks) * NOUT * 32);
-      }
-  std::memcpy(blob.data() + (size_t)9 * KC * NOUT * 32, b, (size_t)cout * 4);
-  return blob;
-}
-
-// the same layer for cnn_layer3_kernel: [3 permutations q][3 face taps dp][KC][3 NOUT x 16] tiles + NOUT biases; rows
+// one convolution layer's blob for cnn_layer3_kernel: [3 permutations q][3 face taps dp][KC][3 NOUT x 16] tiles + NOUT biases; rows
 // g * NOUT .. of a tile hold row tap dr = (q + 1 - g) mod 3
 std::vector<uint8_t> pack_cnn_layer3(const float* W, const float* b, int cout, int cin, int KC, int NOUT, bool transposed) {
   const int N3 = 3 * NOUT;
@@ -629,8 +589,7 @@ int run_steps(jxs_solver* s, double cfl, double fixed_dt, int nsteps, int* where
   s->mlp_events_used = 0;
   if (!(fixed_dt > 0)) CU(wavespeed(s, s->buf[0], &s->d_state->smax_bits[0]));
   int n = 0;
-  static const bool no_graph = getenv("JXS_NO_GRAPH") != nullptr;
-  if (!s->profiling && !no_graph && nsteps >= 6) {
+  if (!s->profiling && s->use_graph && nsteps >= 6) {
     // the first pair runs as plain launches (it also configures the kernels' attributes outside any capture)
     for (; n < 2; ++n) { const int rc = one_step(s, cfl_h, fixed_dt, cur, at); if (rc != JXS_OK) return rc; }
     if ((s->pair_exec && s->pair_cfl_h == cfl_h && s->pair_fixed_dt == fixed_dt) || capture_pair(s, cfl_h, fixed_dt)) {
@@ -719,6 +678,7 @@ int tune_decomposition(jxs_solver* s) {
 
 int step_common(jxs_solver* s, void* U, double cfl, double fixed_dt, int nsteps, bool host, bool wait = true) {
   if (!s) return JXS_EINVAL;
+  DEV(s);
   if (!U) return fail(s, JXS_EINVAL, "U is NULL");
   if (nsteps < 0) return fail(s, JXS_EINVAL, "nsteps < 0");
   if (!(fixed_dt > 0) && !(cfl > 0)) return fail(s, JXS_EINVAL, "cfl must be > 0");
@@ -729,7 +689,7 @@ int step_common(jxs_solver* s, void* U, double cfl, double fixed_dt, int nsteps,
     Ud = s->stage_io;
   }
   CU(pad(s, Ud, s->buf[0]));
-  if (!s->tuned && nsteps > 0) {
+  if (!s->tuned && nsteps > 0 && wait) {  // never inside jxs_step_async: it must only enqueue (jxs_tune does it explicitly)
     const int rc = tune_decomposition(s);
     if (rc != JXS_OK) return rc;
   }
@@ -837,6 +797,7 @@ bool capture_tangent_step(jxs_solver* s, double gamma_dot, double dt) {
 
 int tangent_common(jxs_solver* s, void* U, void* Udot, double gamma_dot, double dt, int nsteps) {
   if (!s) return JXS_EINVAL;
+  DEV(s);
   if (!U || !Udot) return fail(s, JXS_EINVAL, "U or Udot is NULL");
   if (nsteps < 0) return fail(s, JXS_EINVAL, "nsteps < 0");
   if (!(dt > 0)) return fail(s, JXS_EINVAL, "dt must be > 0");
@@ -870,8 +831,7 @@ int tangent_common(jxs_solver* s, void* U, void* Udot, double gamma_dot, double 
     CU(unpad(s, s->bufd[at], Udot));
     return finish_steps(s, nsteps);
   }
-  static const bool no_graph = getenv("JXS_NO_GRAPH") != nullptr;
-  if (!s->profiling && !no_graph && nsteps >= 4) {
+  if (!s->profiling && s->use_graph && nsteps >= 4) {
     // the first step runs as plain launches; the rest replay one captured step (the buffers' roles return after it)
     int rc = tangent_one_step(s, gamma_dot, dt);
     if (rc != JXS_OK) return rc;
@@ -914,6 +874,7 @@ int adjoint_checks(jxs_solver* s) {
 
 int record_common(jxs_solver* s, void* U, double dt, int nsteps) {
   if (!s) return JXS_EINVAL;
+  DEV(s);
   if (!U) return fail(s, JXS_EINVAL, "U is NULL");
   if (nsteps < 1) return fail(s, JXS_EINVAL, "nsteps < 1");
   if (!(dt > 0)) return fail(s, JXS_EINVAL, "dt must be > 0");
@@ -1004,12 +965,9 @@ cudaError_t adjoint_stage(jxs_solver* s, const double* U, const double* out, dou
     M.Ubar_out = out; M.Wbar = s->d_Wmlp; M.theta_bar = s->d_theta_bar; M.bdt = b * s->tape_dt; M.dxi = 1.0 / s->dx;
     cudaError_t e = cudaMemsetAsync(s->d_Wmlp, 0, (size_t)4 * 4 * s->pitch * sizeof(double), s->stream);
     if (e != cudaSuccess) return e;
-    static bool configured = false;
-    if (!configured) {
-      e = cudaFuncSetAttribute(mlp1d_backward_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, MLP1D_BWD_SMEM);
-      if (e != cudaSuccess) return e;
-      configured = true;
-    }
+    static bool configured[MAX_DEVICES] = {false};
+    e = configure_smem(s, mlp1d_backward_kernel, configured, MLP1D_BWD_SMEM);
+    if (e != cudaSuccess) return e;
     // every CTA flushes its 6020 sums at its end: one face per warp on small grids (the paper's N = 500 .. 1000,
     // where latency counts), at most 2 CTAs per SM on large ones (where the flushes would)
     const int bgrid = std::max(1, std::min((s->nx + 1 + 3) / 4, s->num_sms * 2));
@@ -1035,6 +993,7 @@ cudaError_t adjoint_stage(jxs_solver* s, const double* U, const double* out, dou
 // targets != nullptr: the loss of Eq. 14 over the recorded steps drives the sweep (Ubar is output only, *loss too)
 int adjoint_common(jxs_solver* s, void* Ubar, double* gamma_bar, const double* targets = nullptr, double* loss = nullptr) {
   if (!s) return JXS_EINVAL;
+  DEV(s);
   if (!Ubar || !gamma_bar || (targets && !loss)) return fail(s, JXS_EINVAL, "NULL argument");
   int rc = adjoint_checks(s);
   if (rc != JXS_OK) return rc;
@@ -1149,7 +1108,8 @@ int jxs_create(int nx, int ny, double dx, double dy, double gamma, double mu, do
   int dev = 0;
   cudaDeviceProp prop;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { delete s; return JXS_ECUDA; }
-  if (prop.major < 10) { delete s; return JXS_ECUDA; }  // sm_100a code only
+  if (prop.major != 10 || prop.minor != 0) { delete s; return JXS_ECUDA; }  // the library holds sm_100a code only
+  s->dev = dev;
   s->num_sms = prop.multiProcessorCount;
   choose_decomposition(s);
   const int SOUT = dtype == JXS_F64 ? sout<double>() : sout<float>();
@@ -1203,7 +1163,7 @@ void jxs_destroy(jxs_solver* s) {
   cudaFree(s->d_mlp_blob); cudaFree(s->d_dF); cudaFree(s->d_dG);
   for (int d = 0; d < 2; ++d) {
     cudaFree(s->cnn_X[d].data); cudaFree(s->cnn_H1[d].data); cudaFree(s->cnn_H2[d].data);
-    for (int l = 0; l < 3; ++l) { cudaFree(s->d_cnn_blob[d][l]); cudaFree(s->d_cnn_blob3[d][l]); }
+    for (int l = 0; l < 3; ++l) cudaFree(s->d_cnn_blob3[d][l]);
   }
   for (cudaEvent_t ev : s->events) cudaEventDestroy(ev);
   for (cudaEvent_t ev : s->mlp_events) cudaEventDestroy(ev);
@@ -1214,6 +1174,7 @@ const char* jxs_last_error(const jxs_solver* s) { return s ? s->err.c_str() : "n
 
 int jxs_set_ibm(jxs_solver* s, const double* phi) {
   if (!s) return JXS_EINVAL;
+  DEV(s);
   drop_graph(s);
   CU(cudaStreamSynchronize(s->stream));
   free_ibm(s);
@@ -1294,6 +1255,7 @@ int jxs_set_ibm(jxs_solver* s, const double* phi) {
 
 int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[4], const double out_scale[4]) {
   if (!s) return JXS_EINVAL;
+  DEV(s);
   drop_graph(s);
   CU(cudaStreamSynchronize(s->stream));
   if (!weights) { s->mlp_on = false; s->mlp1d_on = false; s->tape_steps = 0; return JXS_OK; }
@@ -1352,6 +1314,7 @@ int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[
 
 int jxs_set_flux_cnn(jxs_solver* s, const float* weights, const double in_scale[4], const double out_scale[4]) {
   if (!s) return JXS_EINVAL;
+  DEV(s);
   drop_graph(s);
   CU(cudaStreamSynchronize(s->stream));
   if (!weights) { s->cnn_on = false; return JXS_OK; }
@@ -1366,13 +1329,9 @@ int jxs_set_flux_cnn(jxs_solver* s, const float* weights, const double in_scale[
   // OIHW: W1[32][4][3][3], b1[32], W2[16][32][3][3], b2[16], W3[4][16][3][3], b3[4]
   const float *W1 = weights, *b1 = W1 + 32 * 4 * 9, *W2 = b1 + 32, *b2 = W2 + 16 * 32 * 9, *W3 = b2 + 16, *b3 = W3 + 4 * 16 * 9;
   for (int d = 0; d < 2; ++d) {
-    const std::vector<uint8_t> blobs[3] = {pack_cnn_layer(W1, b1, 32, 4, 1, 32, d == 1), pack_cnn_layer(W2, b2, 16, 32, 2, 16, d == 1),
-                                           pack_cnn_layer(W3, b3, 4, 16, 1, 16, d == 1)};
     const std::vector<uint8_t> blobs3[3] = {pack_cnn_layer3(W1, b1, 32, 4, 1, 32, d == 1), pack_cnn_layer3(W2, b2, 16, 32, 2, 16, d == 1),
                                             pack_cnn_layer3(W3, b3, 4, 16, 1, 16, d == 1)};
     for (int l = 0; l < 3; ++l) {
-      if (!s->d_cnn_blob[d][l]) CU(cudaMalloc(&s->d_cnn_blob[d][l], blobs[l].size()));
-      CU(cudaMemcpy(s->d_cnn_blob[d][l], blobs[l].data(), blobs[l].size(), cudaMemcpyHostToDevice));
       if (!s->d_cnn_blob3[d][l]) CU(cudaMalloc(&s->d_cnn_blob3[d][l], blobs3[l].size()));
       CU(cudaMemcpy(s->d_cnn_blob3[d][l], blobs3[l].data(), blobs3[l].size(), cudaMemcpyHostToDevice));
     }
@@ -1398,6 +1357,7 @@ int jxs_set_flux_cnn(jxs_solver* s, const float* weights, const double in_scale[
 
 int jxs_flux_cnn_inputs(jxs_solver* s, const void* U, float* Xx, float* Xy) {
   if (!s) return JXS_EINVAL;
+  DEV(s);
   if (!U || !Xx || !Xy) return fail(s, JXS_EINVAL, "NULL array");
   if (!s->cnn_on) return fail(s, JXS_ESTATE, "no CNN set (jxs_set_flux_cnn)");
   CU(pad(s, U, s->buf[0]));
@@ -1412,8 +1372,10 @@ int jxs_flux_cnn_inputs(jxs_solver* s, const void* U, float* Xx, float* Xy) {
 
 int jxs_set_artificial_viscosity(jxs_solver* s, double nu) {
   if (!s) return JXS_EINVAL;
+  if (!(nu >= 0) || !std::isfinite(nu)) return fail(s, JXS_EINVAL, "nu must be finite and >= 0");
+  if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
   drop_graph(s);
-  if (!(nu >= 0)) return fail(s, JXS_EINVAL, "nu must be >= 0");
+  s->tape_steps = 0;  // a recording made with another nu cannot be reversed
   s->nu = nu;
   return JXS_OK;
 }
@@ -1430,6 +1392,7 @@ int jxs_set_gamma(jxs_solver* s, double gamma) {
 
 int jxs_rhs(jxs_solver* s, const void* U, void* dUdt) {
   if (!s) return JXS_EINVAL;
+  DEV(s);
   if (!U || !dUdt) return fail(s, JXS_EINVAL, "NULL array");
   CU(pad(s, U, s->buf[0]));
   CU(ghost_fill(s, s->buf[0]));
@@ -1440,6 +1403,7 @@ int jxs_rhs(jxs_solver* s, const void* U, void* dUdt) {
 
 int jxs_rhs_host(jxs_solver* s, const void* U, void* dUdt) {
   if (!s) return JXS_EINVAL;
+  DEV(s);
   if (!U || !dUdt) return fail(s, JXS_EINVAL, "NULL array");
   const size_t bytes = (size_t)4 * s->nx * s->ny * s->elem;
   CU(cudaMemcpyAsync(s->stage_io, U, bytes, cudaMemcpyHostToDevice, s->stream));
@@ -1454,6 +1418,7 @@ int jxs_rhs_host(jxs_solver* s, const void* U, void* dUdt) {
 
 int jxs_max_wavespeed(jxs_solver* s, const void* U, double* smax) {
   if (!s) return JXS_EINVAL;
+  DEV(s);
   if (!U || !smax) return fail(s, JXS_EINVAL, "NULL argument");
   CU(pad(s, U, s->buf[1]));
   unsigned long long* bits = &s->d_state->smax_bits[0];
@@ -1500,6 +1465,7 @@ int jxs_set_adjoint_checkpointing(jxs_solver* s, int on) {
 
 int jxs_mse_tangent(jxs_solver* s, const void* U, const void* Udot, const void* Utarget, double* loss, double* dloss) {
   if (!s) return JXS_EINVAL;
+  DEV(s);
   if (!U || !Udot || !Utarget || !loss || !dloss) return fail(s, JXS_EINVAL, "NULL argument");
   if (s->dtype != JXS_F64) return fail(s, JXS_EINVAL, "the tangent is fp64 only");
   if (!s->d_mse) CU(cudaMalloc(&s->d_mse, (2 * MSE_PARTS + 2) * sizeof(double)));
@@ -1533,6 +1499,29 @@ int jxs_set_concurrent_handles(jxs_solver* s, int n) {
   s->share = n;
   choose_decomposition(s);  // the padded layout depends on the strips only, not on the row segments
   return JXS_OK;
+}
+int jxs_set_rows_per_segment(jxs_solver* s, int rows) {
+  if (!s) return JXS_EINVAL;
+  if (rows < 0) return fail(s, JXS_EINVAL, "rows must be >= 0");
+  if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
+  drop_graph(s);
+  s->rows_fixed = rows;
+  choose_decomposition(s);
+  return JXS_OK;
+}
+int jxs_set_graph_replay(jxs_solver* s, int on) {
+  if (!s) return JXS_EINVAL;
+  s->use_graph = on != 0;
+  if (!s->use_graph) drop_graph(s);
+  return JXS_OK;
+}
+int jxs_tune(jxs_solver* s) {
+  if (!s) return JXS_EINVAL;
+  DEV(s);
+  if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
+  if (s->tuned) return JXS_OK;
+  drop_graph(s);
+  return tune_decomposition(s);
 }
 int jxs_set_time_integrator(jxs_solver* s, int scheme) {
   if (!s) return JXS_EINVAL;
@@ -1581,6 +1570,7 @@ int jxs_flux_mlp_time(const jxs_solver* s, double* ms_total, long long* launches
 
 int jxs_flux_correction(jxs_solver* s, const void* U, float* dFx, float* dGy) {
   if (!s) return JXS_EINVAL;
+  DEV(s);
   if (!U || !dFx || !dGy) return fail(s, JXS_EINVAL, "NULL array");
   if (!s->mlp_on && !s->cnn_on) return fail(s, JXS_ESTATE, "no flux network set (jxs_set_flux_mlp / jxs_set_flux_cnn)");
   CU(pad(s, U, s->buf[0]));

@@ -426,6 +426,7 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
   const int w0 = 2 + SOUT * strip;  // padded column of lane 0's cell
   const int ic = w0 + lane - 3;     // interior x index of my cell
   const int q = lane + 2;           // my column inside the per-warp rows
+  const bool in_x = (unsigned)ic < (unsigned)A.nx;  // my cell is an interior column (lane 0 of strip 0 is column -1)
 
   constexpr uint32_t RAWSLOT = (uint32_t)stage_smem_rawslot<T>();
   T* raw = reinterpret_cast<T*>(smem_raw);                                                  // [2] x [4][CW]
@@ -597,7 +598,7 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
         viscous_n<T, N>(dn, dt_, xt, xn, sn, st, dT, cn, cc, cs, ct, cq, f1, f2, f3);
       }
       Gp[0] = f0[0]; Gp[1] = f1[0]; Gp[2] = f2[0]; Gp[3] = f3[0];
-      if (A.fluid && ic < A.nx) fl_next = A.fluid[(size_t)(jo + 1 - 3) * A.nx + ic];
+      if (A.fluid && in_x) fl_next = A.fluid[(size_t)(jo + 1 - 3) * A.nx + ic];
     }
 #pragma unroll
     for (int k = 0; k < 4; ++k) Ly[k] = Lnew[k];
@@ -612,7 +613,7 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
     take_row(n, it, A.mode == 0);
     const int jo = n - 3;  // output row = pB; pC = jc
     const unsigned fl = fl_next;
-    if (n < nlast && A.fluid && ic < A.nx) fl_next = A.fluid[(size_t)(jo + 1 - 3) * A.nx + ic];
+    if (n < nlast && A.fluid && in_x) fl_next = A.fluid[(size_t)(jo + 1 - 3) * A.nx + ic];
     float yF[4], yG[4];  // S5': network outputs at my right face and my top face (row jo)
     if (MLP) {
       const size_t o = (size_t)jo * A.pitch + (w0 + lane);
@@ -705,7 +706,7 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
     }
 
     // -------------------------------------------------------------- S8, S9: combine, store, wavespeed
-    const bool ok = lane >= 1 && lane <= SOUT && ic < A.nx;  // lanes 0 and > SOUT are support cells
+    const bool ok = lane >= 1 && lane <= SOUT && in_x;  // lanes 0 and > SOUT are support cells
     if (A.mode == 1) {
       const size_t o = (size_t)(jo - 3) * A.nx + ic, pl = (size_t)A.nx * A.ny;
       if (ok) {

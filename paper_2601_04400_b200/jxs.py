@@ -25,7 +25,8 @@ EXPORTS = ("jxs_create", "jxs_destroy", "jxs_last_error", "jxs_set_ibm", "jxs_se
            "jxs_flux_mlp_time", "jxs_step_async", "jxs_wait", "jxs_set_time_integrator",
            "jxs_set_concurrent_handles", "jxs_set_flux_cnn", "jxs_flux_cnn_inputs",
            "jxs_step_fixed_dt_tangent", "jxs_mse_tangent", "jxs_step_fixed_dt_record", "jxs_adjoint_steps", "jxs_set_gamma",
-           "jxs_set_adjoint_checkpointing", "jxs_flux_mlp_gradient", "jxs_adjoint_steps_mse")
+           "jxs_set_adjoint_checkpointing", "jxs_flux_mlp_gradient", "jxs_adjoint_steps_mse",
+           "jxs_tune", "jxs_set_rows_per_segment", "jxs_set_graph_replay")
 
 
 class jxs_bc(C.Structure):
@@ -48,11 +49,8 @@ def lib():
     if _lib is None:
         path = os.environ.get("JXS_LIB") or _build.LIB  # JXS_LIB: use this prebuilt library as it is
         if path == _build.LIB and os.path.exists(os.path.join(_build.CSRC, "jxs_api.cu")):
-            try:
-                path = _build.build()
-            except Exception:
-                if not os.path.exists(path):
-                    raise
+            # a failed rebuild raises: loading an older libjxs.so would validate and time code that is not HEAD
+            path = _build.build()
         L = C.CDLL(path)
         vp, dp = C.c_void_p, C.POINTER(C.c_double)
         L.jxs_create.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
@@ -74,6 +72,9 @@ def lib():
         L.jxs_wait.argtypes = [vp]
         L.jxs_set_time_integrator.argtypes = [vp, C.c_int]
         L.jxs_set_concurrent_handles.argtypes = [vp, C.c_int]
+        L.jxs_tune.argtypes = [vp]
+        L.jxs_set_rows_per_segment.argtypes = [vp, C.c_int]
+        L.jxs_set_graph_replay.argtypes = [vp, C.c_int]
         L.jxs_set_flux_cnn.argtypes = [vp, vp, dp, dp]
         L.jxs_flux_cnn_inputs.argtypes = [vp, vp, vp, vp]
         L.jxs_step_fixed_dt_tangent.argtypes = [vp, vp, vp, C.c_double, C.c_double, C.c_int]
@@ -250,6 +251,15 @@ class Solver:
     def set_concurrent_handles(self, n):
         self._chk(lib().jxs_set_concurrent_handles(self._h, int(n)))
 
+    def tune(self):
+        self._chk(lib().jxs_tune(self._h))
+
+    def set_rows_per_segment(self, rows):
+        self._chk(lib().jxs_set_rows_per_segment(self._h, int(rows)))
+
+    def set_graph_replay(self, on):
+        self._chk(lib().jxs_set_graph_replay(self._h, int(bool(on))))
+
     def set_time_integrator(self, scheme):
         self._chk(lib().jxs_set_time_integrator(self._h, int(scheme)))
 
@@ -294,7 +304,7 @@ class Solver:
         self._chk(lib().jxs_set_adjoint_checkpointing(self._h, int(bool(on))))
 
     def step_fixed_dt_record(self, U, dt, nsteps):
-        """jxs_step_fixed_dt that keeps the trajectory for adjoint_steps (one-dimensional fp64 Euler handles)."""
+        """jxs_step_fixed_dt that keeps the trajectory for adjoint_steps (fp64 handles; SSP-RK3 or forward Euler)."""
         self._chk(lib().jxs_step_fixed_dt_record(self._h, self._dev(U), float(dt), int(nsteps)))
         return U
 

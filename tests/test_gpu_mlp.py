@@ -62,9 +62,11 @@ def rel_net(a, b, outs):
 
 
 def rel(a, b):
-    """max-norm error per flux component, scaled by that component's max (the two momenta share one scale)."""
+    """max-norm error per component, scaled by that component's max; a momentum component that is zero up to
+    round-off in the case at hand (below 1e-9 of the other) borrows the other's scale."""
     peak = [np.max(np.abs(b[k])) for k in range(4)]
-    scale = [peak[0], max(peak[1], peak[2]), max(peak[1], peak[2]), peak[3]]
+    mom = max(peak[1], peak[2])
+    scale = [peak[0], peak[1] if peak[1] > 1e-9 * mom else mom, peak[2] if peak[2] > 1e-9 * mom else mom, peak[3]]
     return max(np.max(np.abs(a[k] - b[k])) / scale[k] for k in range(4))
 
 
