@@ -84,13 +84,13 @@ __global__ void __launch_bounds__(CNN_RX * CNN_RY) cnn_recon_kernel(const CnnRec
 #pragma unroll
     for (int k = 0; k < 4; ++k) { a[k] = W[k][cy][cx - 2]; b[k] = W[k][cy][cx - 1]; wc[k] = W[k][cy][cx]; d[k] = W[k][cy][cx + 1]; e[k] = W[k][cy][cx + 2]; }
     weno5_n<T, 4>(a, b, wc, d, e, K, Rm, Lx);
-    const bool badR = not_positive(Rm[0]) | not_positive(Rm[3]), badL = not_positive(Lx[0]) | not_positive(Lx[3]);  // R15
+    const bool badR = any_not_positive(Rm[0], Rm[3]), badL = any_not_positive(Lx[0], Lx[3]);  // R15
 #pragma unroll
     for (int k = 0; k < 4; ++k) { Rx[k][ty][tx] = badR ? wc[k] : Rm[k]; Lx[k] = badL ? wc[k] : Lx[k]; }
 #pragma unroll
     for (int k = 0; k < 4; ++k) { a[k] = W[k][cy - 2][cx]; b[k] = W[k][cy - 1][cx]; d[k] = W[k][cy + 1][cx]; e[k] = W[k][cy + 2][cx]; }
     weno5_n<T, 4>(a, b, wc, d, e, K, Rm, Ly);
-    const bool badRy = not_positive(Rm[0]) | not_positive(Rm[3]), badLy = not_positive(Ly[0]) | not_positive(Ly[3]);
+    const bool badRy = any_not_positive(Rm[0], Rm[3]), badLy = any_not_positive(Ly[0], Ly[3]);
 #pragma unroll
     for (int k = 0; k < 4; ++k) { Ry[k][ty][tx] = badRy ? wc[k] : Rm[k]; Ly[k] = badLy ? wc[k] : Ly[k]; }
   }

@@ -28,11 +28,18 @@ using namespace jxs;
 
 namespace {
 constexpr int MAX_EVENTS = 8192;
-// resident one-warp CTAs per SM the stage kernel is compiled for (registers <= 65536/(32*minb))
+// resident one-warp CTAs per SM the stage kernel is compiled for (registers <= 65536 / (32 * minb)).  Measured on
+// B200 (4096 x 2048, ms per stage launch) with the y-reconstruction's differences carried in registers: fp64 12 warps
+// at 168 registers 0.3829, 16 warps at 128 registers (spilling) 0.4975; without the carried state 16 warps at 122
+// registers 0.3975, 12 at 156 0.4026, 10 at 157 0.4121, 8 at 157 0.4091 (the FP64 pipe is fed by each warp's own
+// independent instructions, not by the number of warps).  fp32: 20 warps at 96 registers 0.2299, 24 at 80 (spilling) 0.2438.
 #ifndef JXS_MINB_F64
-#define JXS_MINB_F64 16
+#define JXS_MINB_F64 12
 #endif
-template <typename T> constexpr int stage_minb() { return sizeof(T) == 8 ? JXS_MINB_F64 : 24; }
+#ifndef JXS_MINB_F32
+#define JXS_MINB_F32 20
+#endif
+template <typename T> constexpr int stage_minb() { return sizeof(T) == 8 ? JXS_MINB_F64 : JXS_MINB_F32; }
 }
 
 struct jxs_solver {
@@ -114,9 +121,11 @@ struct jxs_solver {
   int pending_steps = 0;  // steps enqueued by jxs_step_async and not yet waited for
   // work decomposition of the stage kernel
   int nstrips = 0, rows_per_seg = 0, nseg = 0, ntasks = 0, warps = 0, grid = 0;
+  int nseg_a = 0, rows_b = 0;  // the first nseg_a segments of a strip have rows_per_seg rows, the rest rows_b (short tail tasks)
   int share = 1;  // handles of about this size that step concurrently (jxs_set_concurrent_handles)
   bool tuned = false;  // rows_per_seg measured on this device (tune_decomposition)
   int rows_fixed = 0;  // jxs_set_rows_per_segment: > 0 overrides the heuristic and the measurement
+  double tail_frac = 0.0;  // fraction of the rows cut into half-length segments (chosen by tune_decomposition)
   bool use_graph = true;  // jxs_set_graph_replay
   // bookkeeping
   long long launches = 0;
@@ -216,9 +225,21 @@ bool make_tensor_map(const jxs_solver* s, void* base, int box_w, CUtensorMap* ou
 // (measured: mean task lifetime 75 % of the kernel's).  Many short tasks handed out dynamically by the
 // block scheduler keep every slot busy; the price is the ~2 row-equivalents of warm-up per task.
 // cost model: rows of work per slot, plus half a task of tail per slot
-void set_rows_per_seg(jxs_solver* s, int rps) {
+// tail_frac > 0: the last tail_frac of the rows are cut into segments of half the length.  Tasks are handed out in
+// blockIdx order (segment-major), so these are the tasks the kernel ends on, and the time during which SMs run out of
+// work scales with their length; their extra warm-up rows are paid on that fraction only.
+void set_rows_per_seg(jxs_solver* s, int rps, double tail_frac = 0.0) {
   s->rows_per_seg = rps;
-  s->nseg = (s->ny + rps - 1) / rps;
+  s->rows_b = rps;
+  s->nseg_a = (s->ny + rps - 1) / rps;
+  int nseg_b = 0;
+  if (tail_frac > 0.0 && rps >= 16) {
+    const int rb = std::max(8, rps / 2);
+    const int na = std::max(0, (int)((1.0 - tail_frac) * s->ny) / rps);
+    const int left = s->ny - na * rps;
+    if (left > 0) { s->nseg_a = na; s->rows_b = rb; nseg_b = (left + rb - 1) / rb; }
+  }
+  s->nseg = s->nseg_a + nseg_b;
   s->ntasks = s->nseg * s->nstrips;
   s->grid = s->ntasks;
 }
@@ -272,6 +293,7 @@ cudaError_t launch_stage(jxs_solver* s, const void* Uin, const void* U0, void* U
   A.smax_bits = smax_bits;
   A.plane = s->plane; A.nx = s->nx; A.ny = s->ny; A.pitch = s->pitch;
   A.nstrips = s->nstrips; A.rows_per_seg = s->rows_per_seg; A.ntasks = s->ntasks;
+  A.nseg_a = s->nseg_a; A.rows_b = s->rows_b;
   A.mode = mode;
   A.gamma = (T)s->gamma; A.g1 = (T)(s->gamma - 1.0); A.g1inv = (T)(1.0 / (s->gamma - 1.0));
   A.dxi = (T)(1.0 / s->dx); A.dyi = (T)(1.0 / s->dy);
@@ -652,25 +674,32 @@ int tune_decomposition(jxs_solver* s) {
   CU(cudaEventCreate(&e1));
   CU(ghost_fill(s, s->buf[0]));
   int best = base;
+  double best_tail = 0.0;
   float best_ms = 1e30f;
   cudaError_t err = cudaSuccess;
-  for (int rps = std::max(8, base - 12); rps <= std::min(s->ny, base + 8) && err == cudaSuccess; ++rps) {
-    set_rows_per_seg(s, rps);
-    float ms = 1e30f;
-    for (int rep = 0; rep < 2 && err == cudaSuccess; ++rep) {  // the first launch of the loop also warms the caches
-      cudaEventRecord(e0, s->stream);
-      err = stage(s, s->buf[0], nullptr, s->buf[1], 0, 0.0, 1.0, nullptr);
-      cudaEventRecord(e1, s->stream);
-      if (err == cudaSuccess) err = cudaEventSynchronize(e1);
-      float t = 0;
-      if (err == cudaSuccess) cudaEventElapsedTime(&t, e0, e1);
-      if (rep == 1 || rps > std::max(8, base - 12)) ms = std::min(ms, t);
+  bool first = true;
+  for (int rps = std::max(8, base - 12); rps <= std::min(s->ny, base + 16) && err == cudaSuccess; ++rps)
+    for (int variant = 0; variant < 3 && err == cudaSuccess; ++variant) {
+      const double tail = variant == 0 ? 0.0 : (variant == 1 ? 0.15 : 0.3);
+      set_rows_per_seg(s, rps, tail);
+      if (variant > 0 && s->rows_b == rps) continue;  // no short segments at this length
+      float ms = 1e30f;
+      for (int rep = 0; rep < 2 && err == cudaSuccess; ++rep) {  // the very first launch also warms the caches
+        cudaEventRecord(e0, s->stream);
+        err = stage(s, s->buf[0], nullptr, s->buf[1], 0, 0.0, 1.0, nullptr);
+        cudaEventRecord(e1, s->stream);
+        if (err == cudaSuccess) err = cudaEventSynchronize(e1);
+        float t = 0;
+        if (err == cudaSuccess) cudaEventElapsedTime(&t, e0, e1);
+        if (rep == 1 || !first) ms = std::min(ms, t);
+      }
+      first = false;
+      if (ms < best_ms) { best_ms = ms; best = rps; best_tail = tail; }
     }
-    if (ms < best_ms) { best_ms = ms; best = rps; }
-  }
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
-  set_rows_per_seg(s, best);
+  set_rows_per_seg(s, best, best_tail);
+  s->tail_frac = best_tail;
   s->profiling = prof;
   if (err != cudaSuccess) return cuda_fail(s, err, "tune_decomposition");
   return JXS_OK;

@@ -72,8 +72,8 @@ __global__ void __launch_bounds__(S1D_TB) stage1d_kernel(const StageArgs<T> A) {
     T a[N], b[N], d[N], e[N];
     JXS_V { a[k] = prim[k][t]; b[k] = prim[k][t + 1]; wc[k] = prim[k][t + 2]; d[k] = prim[k][t + 3]; e[k] = prim[k][t + 4]; }
     weno5_n<T, N>(a, b, wc, d, e, A, Rm, Lp);
-    const bool badR = not_positive(Rm[0]) | not_positive(Rm[3]);  // positivity guard (R15)
-    const bool badL = not_positive(Lp[0]) | not_positive(Lp[3]);
+    const bool badR = any_not_positive(Rm[0], Rm[3]);  // positivity guard (R15)
+    const bool badL = any_not_positive(Lp[0], Lp[3]);
     JXS_V { Rm[k] = badR ? wc[k] : Rm[k]; Lp[k] = badL ? wc[k] : Lp[k]; }
     JXS_V rmS[k][t] = Rm[k];
   }

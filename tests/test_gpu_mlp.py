@@ -61,13 +61,17 @@ def rel_net(a, b, outs):
     return np.max(np.abs(a - b)) / np.max(np.abs(b))
 
 
-def rel(a, b):
-    """max-norm error per component, scaled by that component's max; a momentum component that is zero up to
-    round-off in the case at hand (below 1e-9 of the other) borrows the other's scale."""
+def rel_fields(a, b, zero_tol=1e-6):
+    """max-norm error of each component, scaled by that component's max; a momentum component that holds only
+    round-off (below zero_tol of the other) borrows the other's scale."""
     peak = [np.max(np.abs(b[k])) for k in range(4)]
     mom = max(peak[1], peak[2])
-    scale = [peak[0], peak[1] if peak[1] > 1e-9 * mom else mom, peak[2] if peak[2] > 1e-9 * mom else mom, peak[3]]
-    return max(np.max(np.abs(a[k] - b[k])) / scale[k] for k in range(4))
+    scale = [peak[0], peak[1] if peak[1] > zero_tol * mom else mom, peak[2] if peak[2] > zero_tol * mom else mom, peak[3]]
+    return [np.max(np.abs(a[k] - b[k])) / scale[k] for k in range(4)]
+
+
+def rel(a, b):
+    return max(rel_fields(a, b))
 
 
 CASES = {
@@ -184,5 +188,8 @@ def test_steps_with_mlp_stay_close():
     s.step(U, 0.4, 20)
     fluid = o.cell_types() == 0
     got = U.cpu().numpy()
-    assert rel(got[:, fluid], ref[:, fluid]) <= 1e-4
+    e = rel_fields(got[:, fluid], ref[:, fluid])
+    # rho, rho u, E: the corrections are 1e-3 of the flux, their 1e-2 errors 1e-5 of it.  rho v exists here only through
+    # the network's corrections (the shock has not reached the body), so relative to ITS max it carries the network's bound
+    assert max(e[0], e[1], e[3]) <= 1e-4 and e[2] <= 1e-2, e
     assert abs(o.time()[0] - s.time()[0]) <= 1e-6 * o.time()[0]
