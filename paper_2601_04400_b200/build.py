@@ -13,7 +13,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libjxs.so")
 SOURCES = [os.path.join(CSRC, "jxs_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("stage_kernel.cuh", "stage1d_kernel.cuh", "tangent1d_kernel.cuh", "adjoint1d_kernel.cuh", "mlp1d_kernel.cuh", "aux_kernels.cuh", "flux_mlp_kernel.cuh", "flux_cnn_kernel.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("stage_kernel.cuh", "stage1d_kernel.cuh", "tangent1d_kernel.cuh", "adjoint1d_kernel.cuh", "mlp1d_kernel.cuh", "deriv2d_kernels.cuh", "aux_kernels.cuh", "flux_mlp_kernel.cuh", "flux_cnn_kernel.cuh")] + [
     os.path.join(ROOT, "include", "jxs.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-cudart", "static"]

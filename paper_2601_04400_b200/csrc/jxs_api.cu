@@ -23,6 +23,7 @@
 #include "tangent1d_kernel.cuh"
 #include "adjoint1d_kernel.cuh"
 #include "mlp1d_kernel.cuh"
+#include "deriv2d_kernels.cuh"
 
 using namespace jxs;
 
@@ -81,6 +82,25 @@ struct jxs_solver {
   double tape_dt = 0;
   double* adj = nullptr;  // 4 adjoint states, then the gamma_bar partial sums, then gamma_bar
   int adj_parts = 0;
+  // two-dimensional derivatives (deriv2d_kernels.cuh): transposed scratch fields [4][nx+6][pitch_t], L and its tangent
+  // in the natural layout, the viscous adjoint's face coefficients, the immersed boundary's transposed gather
+  // (donor cell -> the ghost entries it feeds), the fluid mask transposed, partial sums of gamma_bar
+  int pitch_t = 0;
+  long long plane_t = 0;
+  double* tr[4] = {nullptr, nullptr, nullptr, nullptr};
+  double* Lnat[2] = {nullptr, nullptr};
+  double* visc_C = nullptr;
+  uint8_t* d_fluid_t = nullptr;
+  int n_donor = 0;
+  int* d_dcell = nullptr;
+  int* d_drows = nullptr;
+  int* d_dentry = nullptr;
+  double* d_contrib = nullptr;
+  double* d_gpart = nullptr;
+  size_t gpart_n = 0;
+  double* tape2 = nullptr;   // recorded padded states of the 2D reverse sweep (4 * plane doubles each)
+  size_t tape2_bytes = 0;
+  double* adj2 = nullptr;    // 4 padded adjoint states + gamma_bar + loss accumulator
   // TMA descriptors of the three padded buffers: boxes [4][1][CW] (stencil rows) and [4][1][Epi::W] (RK operand rows)
   CUtensorMap tm_row[3], tm_epi[3];
   // immersed boundary
@@ -534,6 +554,10 @@ void free_ibm(jxs_solver* s) {
   cudaFree(s->d_fluid); cudaFree(s->d_cell); cudaFree(s->d_donor); cudaFree(s->d_w); cudaFree(s->d_nrm);
   s->d_fluid = nullptr; s->d_cell = nullptr; s->d_donor = nullptr; s->d_w = nullptr; s->d_nrm = nullptr;
   s->n_ghost = 0;
+  cudaFree(s->d_fluid_t); cudaFree(s->d_dcell); cudaFree(s->d_drows); cudaFree(s->d_dentry); cudaFree(s->d_contrib);
+  s->d_fluid_t = nullptr; s->d_dcell = nullptr; s->d_drows = nullptr; s->d_dentry = nullptr; s->d_contrib = nullptr;
+  s->n_donor = 0;
+  s->tape_steps = 0;  // a recording made with another body cannot be reversed
 }
 
 // one step, enqueued on s->stream.  cur = index of the valid s_max, at = buffer that holds U^n (forward Euler swaps
@@ -824,6 +848,10 @@ bool capture_tangent_step(jxs_solver* s, double gamma_dot, double dt) {
   return true;
 }
 
+int tangent2d_common(jxs_solver* s, void* U, void* Udot, double gamma_dot, double dt, int nsteps);
+int record2d_common(jxs_solver* s, void* U, double dt, int nsteps);
+int adjoint2d_common(jxs_solver* s, void* Ubar, double* gamma_bar, const double* targets, double* loss);
+
 int tangent_common(jxs_solver* s, void* U, void* Udot, double gamma_dot, double dt, int nsteps) {
   if (!s) return JXS_EINVAL;
   DEV(s);
@@ -832,9 +860,9 @@ int tangent_common(jxs_solver* s, void* U, void* Udot, double gamma_dot, double 
   if (!(dt > 0)) return fail(s, JXS_EINVAL, "dt must be > 0");
   if (!std::isfinite(gamma_dot)) return fail(s, JXS_EINVAL, "gamma_dot is not finite");
   if (s->dtype != JXS_F64) return fail(s, JXS_EINVAL, "the tangent is fp64 only");
-  if (s->ny != 1) return fail(s, JXS_EINVAL, "the tangent is built for one-dimensional problems (ny = 1)");
   if (s->mlp_on || s->cnn_on || s->mlp1d_on) return fail(s, JXS_ESTATE, "the tangent does not differentiate the networks");
   if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
+  if (s->ny != 1) return tangent2d_common(s, U, Udot, gamma_dot, dt, nsteps);
   const size_t bytes = (size_t)4 * s->plane * s->elem;
   for (int b = 0; b < 3; ++b)
     if (!s->bufd[b]) {
@@ -896,7 +924,6 @@ double* compact_state(const jxs_solver* s, double* base, long long i) {
 
 int adjoint_checks(jxs_solver* s) {
   if (s->dtype != JXS_F64) return fail(s, JXS_EINVAL, "the adjoint is fp64 only");
-  if (s->ny != 1) return fail(s, JXS_EINVAL, "the adjoint is built for one-dimensional problems (ny = 1)");
   if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
   return JXS_OK;
 }
@@ -909,6 +936,7 @@ int record_common(jxs_solver* s, void* U, double dt, int nsteps) {
   if (!(dt > 0)) return fail(s, JXS_EINVAL, "dt must be > 0");
   int rc = adjoint_checks(s);
   if (rc != JXS_OK) return rc;
+  if (s->ny != 1) return record2d_common(s, U, dt, nsteps);
   s->tape_steps = 0;
   const size_t state = (size_t)4 * s->pitch * sizeof(double);
   const bool ckpt = s->checkpoint && s->scheme == JXS_SSPRK3;
@@ -1026,6 +1054,7 @@ int adjoint_common(jxs_solver* s, void* Ubar, double* gamma_bar, const double* t
   if (!Ubar || !gamma_bar || (targets && !loss)) return fail(s, JXS_EINVAL, "NULL argument");
   int rc = adjoint_checks(s);
   if (rc != JXS_OK) return rc;
+  if (s->ny != 1) return adjoint2d_common(s, Ubar, gamma_bar, targets, loss);
   if (!s->tape || s->tape_steps < 1) return fail(s, JXS_ESTATE, "no recorded steps: call jxs_step_fixed_dt_record first");
   const int parts = (s->nx + 6 + A1D_OUT - 1) / A1D_OUT;
   const size_t state = (size_t)4 * s->pitch;
@@ -1091,6 +1120,335 @@ int adjoint_common(jxs_solver* s, void* Ubar, double* gamma_bar, const double* t
   CU(unpad(s, B(x), Ubar));
   double out[2];
   CU(cudaMemcpyAsync(out, s->adj + 4 * state + parts, sizeof(out), cudaMemcpyDeviceToHost, s->stream));
+  CU(cudaStreamSynchronize(s->stream));
+  *gamma_bar = out[0];
+  if (loss) *loss = out[1] / (s->tape_steps * (double)ncell4);
+  if (s->profiling) {
+    s->stage_ms = 0;
+    s->stage_launches = s->events_used / 2;
+    for (int i = 0; i + 1 < s->events_used; i += 2) {
+      float ms = 0;
+      cudaEventElapsedTime(&ms, s->events[i], s->events[i + 1]);
+      s->stage_ms += ms;
+    }
+  }
+  return JXS_OK;
+}
+
+// ---- derivatives of the two-dimensional step (deriv2d_kernels.cuh)
+int deriv2d_scratch(jxs_solver* s) {
+  if (s->tr[0]) return JXS_OK;
+  s->pitch_t = (s->ny + 6 + 15) / 16 * 16;
+  s->plane_t = (long long)(s->nx + 6) * s->pitch_t;
+  const size_t tb = (size_t)4 * s->plane_t * sizeof(double), nb = (size_t)4 * s->plane * sizeof(double);
+  for (int q = 0; q < 4; ++q) { CU(cudaMalloc(&s->tr[q], tb)); CU(cudaMemsetAsync(s->tr[q], 0, tb, s->stream)); }
+  for (int q = 0; q < 2; ++q) { CU(cudaMalloc(&s->Lnat[q], nb)); CU(cudaMemsetAsync(s->Lnat[q], 0, nb, s->stream)); }
+  const size_t nf = (size_t)s->ny * (s->nx + 1) + (size_t)(s->ny + 1) * s->nx;
+  CU(cudaMalloc(&s->visc_C, 7 * nf * sizeof(double)));
+  // partial sums of gamma_bar: the line kernels' CTAs of both passes, the viscous kernels, the folds, the ghosts
+  const size_t lines = (size_t)((s->nx + 6 + A1D_OUT - 1) / A1D_OUT) * s->ny + (size_t)((s->ny + 6 + A1D_OUT - 1) / A1D_OUT) * s->nx;
+  s->gpart_n = lines + 2 * (size_t)s->num_sms * 8 + 4 * (size_t)(s->nx + s->ny + 16) + (size_t)s->n_ghost + 64;
+  CU(cudaMalloc(&s->d_gpart, s->gpart_n * sizeof(double)));
+  return JXS_OK;
+}
+LineSet lines_x(const jxs_solver* s) { return LineSet{s->plane, s->pitch, s->nx, s->ny}; }
+LineSet lines_y(const jxs_solver* s) { return LineSet{s->plane_t, s->pitch_t, s->ny, s->nx}; }
+
+// natural [4][ny+6][pitch] -> transposed [4][nx+6][pitch_t] (momenta exchanged), the whole padded field
+cudaError_t to_transposed(jxs_solver* s, const double* src, double* dst) {
+  TransposeArgs T{src, dst, s->plane, s->plane_t, s->pitch, s->pitch_t, 0, s->ny + 6, 0, s->nx + 6, 0};
+  const dim3 grid((s->nx + 6 + 31) / 32, (s->ny + 6 + 31) / 32, 4);
+  transpose_swap_kernel<<<grid, 256, 0, s->stream>>>(T);
+  s->launches++;
+  return cudaGetLastError();
+}
+// transposed -> natural, added: the lines 3 .. nx+2 of src (interior columns), positions [p_lo, p_hi) along them
+cudaError_t add_from_transposed(jxs_solver* s, const double* src, double* dst, int p_lo, int p_hi) {
+  TransposeArgs T{src, dst, s->plane_t, s->plane, s->pitch_t, s->pitch, 3, s->nx + 3, p_lo, p_hi, 1};
+  const dim3 grid((p_hi - p_lo + 31) / 32, (s->nx + 31) / 32, 4);
+  transpose_swap_kernel<<<grid, 256, 0, s->stream>>>(T);
+  s->launches++;
+  return cudaGetLastError();
+}
+
+// the tangent's ghosts: frame (the boundary conditions are linear; the inflow state's energy moves with gamma), then
+// the immersed-boundary fill on pairs.  U must already hold its own ghosts.
+cudaError_t ghost_fill_tangent2d(jxs_solver* s, const void* U, void* Udot, double gamma_dot) {
+  BcSpec b = bcspec(s);
+  const double g1 = s->gamma - 1.0;
+  b.inflow_cons[0] = b.inflow_cons[1] = b.inflow_cons[2] = 0.0;
+  b.inflow_cons[3] = -s->bc.inflow[3] / (g1 * g1) * gamma_dot;
+  const int total = 6 * s->ny + 6 * (s->nx + 6);
+  IbmList none{nullptr, nullptr, nullptr, nullptr, 0};
+  ghost_fill_kernel<double><<<(total + 127) / 128, 128, 0, s->stream>>>((double*)Udot, dims(s), b, none, s->gamma);
+  s->launches++;
+  if (s->n_ghost > 0) {
+    IbmList L{s->d_cell, s->d_donor, s->d_w, s->d_nrm, s->n_ghost};
+    ibm_fill_tangent_kernel<<<(s->n_ghost + 127) / 128, 128, 0, s->stream>>>((const double*)U, (double*)Udot, s->plane, L,
+                                                                             s->gamma, gamma_dot);
+    s->launches++;
+  }
+  return cudaGetLastError();
+}
+
+// one stage on pairs: (buf[in], bufd[in]) -> (buf[out], bufd[out]) = a U0 + b (U + dt L), L = Lx + Ly + Lv
+int tangent_stage2d(jxs_solver* s, int in, int out, double a, double b, double gamma_dot) {
+  const double *U = (const double*)s->buf[in], *Ud = (const double*)s->bufd[in];
+  CU(ghost_fill(s, s->buf[in]));
+  CU(ghost_fill_tangent2d(s, U, s->bufd[in], gamma_dot));
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (s->profiling && s->events_used + 2 <= (int)s->events.size()) {
+    e0 = s->events[s->events_used++];
+    e1 = s->events[s->events_used++];
+    cudaEventRecord(e0, s->stream);
+  }
+  TangentLineArgs X{U, Ud, s->Lnat[0], s->Lnat[1], lines_x(s), s->gamma, gamma_dot, 1.0 / s->dx, s->nu, 0};
+  tangent_line_kernel<<<dim3((s->nx + T1D_OUT - 1) / T1D_OUT, s->ny), T1D_TB, 0, s->stream>>>(X);
+  s->launches++;
+  CU(to_transposed(s, U, s->tr[0]));
+  CU(to_transposed(s, Ud, s->tr[1]));
+  TangentLineArgs Y{s->tr[0], s->tr[1], s->tr[2], s->tr[3], lines_y(s), s->gamma, gamma_dot, 1.0 / s->dy, s->nu, 0};
+  tangent_line_kernel<<<dim3((s->ny + T1D_OUT - 1) / T1D_OUT, s->nx), T1D_TB, 0, s->stream>>>(Y);
+  s->launches++;
+  CU(add_from_transposed(s, s->tr[2], s->Lnat[0], 3, s->ny + 3));
+  CU(add_from_transposed(s, s->tr[3], s->Lnat[1], 3, s->ny + 3));
+  if (s->mu > 0) {
+    Visc2dArgs V{U, Ud, s->Lnat[0], s->Lnat[1], s->plane, s->nx, s->ny, s->pitch, s->gamma, gamma_dot, s->mu, s->Pr,
+                 1.0 / s->dx, 1.0 / s->dy};
+    viscous2d_tangent_kernel<<<dim3((s->nx + V2_TX - 1) / V2_TX, (s->ny + V2_TY - 1) / V2_TY), V2_TX * V2_TY, 0, s->stream>>>(V);
+    s->launches++;
+  }
+  Combine2dArgs C{U, Ud, (const double*)s->buf[0], (const double*)s->bufd[0], s->Lnat[0], s->Lnat[1], (double*)s->buf[out],
+                  (double*)s->bufd[out], s->d_fluid, &s->d_state->dt, s->plane, s->nx, s->ny, s->pitch, a, b};
+  combine2d_tangent_kernel<<<s->num_sms * 8, 256, 0, s->stream>>>(C);
+  s->launches++;
+  if (e1) cudaEventRecord(e1, s->stream);
+  CU(cudaGetLastError());
+  return JXS_OK;
+}
+
+int tangent2d_common(jxs_solver* s, void* U, void* Udot, double gamma_dot, double dt, int nsteps) {
+  if (s->mlp_on || s->cnn_on) return fail(s, JXS_ESTATE, "the tangent does not differentiate the 2D networks");
+  int rc = deriv2d_scratch(s);
+  if (rc != JXS_OK) return rc;
+  const size_t bytes = (size_t)4 * s->plane * s->elem;
+  for (int b = 0; b < 3; ++b)
+    if (!s->bufd[b]) {
+      CU(cudaMalloc(&s->bufd[b], bytes));
+      CU(cudaMemsetAsync(s->bufd[b], 0, bytes, s->stream));
+    }
+  CU(pad(s, U, s->buf[0]));
+  CU(pad(s, Udot, s->bufd[0]));
+  s->events_used = 0;
+  s->mlp_events_used = 0;
+  int at = 0;
+  for (int n = 0; n < nsteps; ++n) {
+    prepare_step_kernel<<<1, 1, 0, s->stream>>>(s->d_state, 0, 0.0, dt);
+    s->launches++;
+    CU(cudaGetLastError());
+    if (s->scheme == JXS_EULER) {  // Eq. 10: one stage with (a, b) = (0, 1); the two buffers swap roles
+      rc = tangent_stage2d(s, at, at ^ 1, 0.0, 1.0, gamma_dot);
+      if (rc != JXS_OK) return rc;
+      at ^= 1;
+      continue;
+    }
+    static const double ab[3][2] = {{0.0, 1.0}, {0.75, 0.25}, {1.0 / 3.0, 2.0 / 3.0}};  // R5
+    static const int io[3][2] = {{0, 1}, {1, 2}, {2, 0}};
+    for (int st = 0; st < 3; ++st) {
+      rc = tangent_stage2d(s, io[st][0], io[st][1], ab[st][0], ab[st][1], gamma_dot);
+      if (rc != JXS_OK) return rc;
+    }
+  }
+  CU(unpad(s, s->buf[at], U));
+  CU(unpad(s, s->bufd[at], Udot));
+  return finish_steps(s, nsteps);
+}
+
+// recorded forward sweep in 2D: the padded, ghost-filled input state of every stage is kept (3 per SSP-RK3 step, 1
+// per forward-Euler step, or with checkpointing U^n only), plus the final state
+int record2d_common(jxs_solver* s, void* U, double dt, int nsteps) {
+  if (s->mlp_on || s->cnn_on) return fail(s, JXS_ESTATE, "the adjoint does not differentiate the 2D networks");
+  int rc = deriv2d_scratch(s);
+  if (rc != JXS_OK) return rc;
+  s->tape_steps = 0;
+  const size_t state = (size_t)4 * s->plane;
+  const bool ckpt = s->checkpoint && s->scheme == JXS_SSPRK3;
+  const int per_step = (s->scheme == JXS_EULER || ckpt) ? 1 : 3;
+  const size_t bytes = state * sizeof(double) * (per_step * (size_t)nsteps + 1);
+  if (!s->tape2 || s->tape2_bytes < bytes) {
+    cudaFree(s->tape2);
+    s->tape2 = nullptr;
+    s->tape2_bytes = 0;
+    if (cudaMalloc(&s->tape2, bytes) != cudaSuccess) {
+      cudaGetLastError();
+      return fail(s, JXS_ENOMEM, "the recorded trajectory does not fit in device memory");
+    }
+    s->tape2_bytes = bytes;
+  }
+  auto T = [&](long long i) { return (void*)(s->tape2 + i * state); };
+  CU(pad(s, U, s->buf[0]));
+  s->events_used = 0;
+  s->mlp_events_used = 0;
+  const size_t sb = state * sizeof(double);
+  // The fused stage kernel reads through the tensor maps of buf[0..2]; the recording therefore steps in the handle's
+  // buffers exactly like jxs_step_fixed_dt and copies each stage's (ghost-filled) input to the tape.
+  long long rec = 0;
+  for (long long n = 0; n < nsteps; ++n) {
+    prepare_step_kernel<<<1, 1, 0, s->stream>>>(s->d_state, 0, 0.0, dt);
+    s->launches++;
+    CU(cudaGetLastError());
+    if (s->scheme == JXS_EULER) {
+      const int at = (int)(n & 1);
+      CU(ghost_fill(s, s->buf[at]));
+      CU(cudaMemcpyAsync(T(rec++), s->buf[at], sb, cudaMemcpyDeviceToDevice, s->stream));
+      CU(stage(s, s->buf[at], nullptr, s->buf[at ^ 1], 0, 0.0, 1.0, nullptr));
+      continue;
+    }
+    CU(ghost_fill(s, s->buf[0]));
+    CU(cudaMemcpyAsync(T(rec++), s->buf[0], sb, cudaMemcpyDeviceToDevice, s->stream));
+    CU(stage(s, s->buf[0], nullptr, s->buf[1], 0, 0.0, 1.0, nullptr));
+    CU(ghost_fill(s, s->buf[1]));
+    if (!ckpt) CU(cudaMemcpyAsync(T(rec++), s->buf[1], sb, cudaMemcpyDeviceToDevice, s->stream));
+    CU(stage(s, s->buf[1], s->buf[0], s->buf[2], 0, 0.75, 0.25, nullptr));
+    CU(ghost_fill(s, s->buf[2]));
+    if (!ckpt) CU(cudaMemcpyAsync(T(rec++), s->buf[2], sb, cudaMemcpyDeviceToDevice, s->stream));
+    CU(stage(s, s->buf[2], s->buf[0], s->buf[0], 0, 1.0 / 3.0, 2.0 / 3.0, nullptr));
+  }
+  const int at = s->scheme == JXS_EULER ? (nsteps & 1) : 0;
+  CU(cudaMemcpyAsync(T(rec), s->buf[at], sb, cudaMemcpyDeviceToDevice, s->stream));
+  CU(unpad(s, s->buf[at], U));
+  rc = finish_steps(s, nsteps);
+  if (rc != JXS_OK) return rc;
+  s->tape_steps = nsteps;
+  s->tape_scheme = s->scheme;
+  s->tape_ckpt = ckpt;
+  s->tape_dt = dt;
+  return JXS_OK;
+}
+
+// gamma_bar accumulator: adj2 + 16 * plane; loss accumulator behind it
+double* adj2_state(const jxs_solver* s, int i) { return s->adj2 + (size_t)i * 4 * s->plane; }
+double* adj2_gbar(const jxs_solver* s) { return s->adj2 + (size_t)16 * s->plane; }
+
+cudaError_t add_partials(jxs_solver* s, long long n) {
+  sum_partials_kernel<<<1, 1024, 0, s->stream>>>(s->d_gpart, n, adj2_gbar(s));
+  s->launches++;
+  return cudaGetLastError();
+}
+
+// reverse of one 2D stage U_out = b (U + dt fl L(U)) (+ a U0): Ubar_in = b Ubar_out + b dt (dL/dU)^T (fl Ubar_out)
+// + e1 E1 + e2 E2, then the transposed immersed-boundary fill and the transposed frame fill; gamma_bar accumulates
+int adjoint_stage2d(jxs_solver* s, const double* U, const double* out, double* in, double b, const double* E1, double e1,
+                    const double* E2, double e2) {
+  const size_t sb = (size_t)4 * s->plane * sizeof(double);
+  CU(cudaMemsetAsync(in, 0, sb, s->stream));
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  if (s->profiling && s->events_used + 2 <= (int)s->events.size()) {
+    ev0 = s->events[s->events_used++];
+    ev1 = s->events[s->events_used++];
+    cudaEventRecord(ev0, s->stream);
+  }
+  // Lx: the rows
+  const int px = (s->nx + 6 + A1D_OUT - 1) / A1D_OUT, py = (s->ny + 6 + A1D_OUT - 1) / A1D_OUT;
+  AdjointLineArgs X{U, out, in, E1, E2, s->d_fluid, s->d_gpart, lines_x(s), s->tape_dt, s->gamma, 1.0 / s->dx, b, e1, e2, s->nu, 1};
+  adjoint_line_kernel<<<dim3(px, s->ny), A1D_TB, 0, s->stream>>>(X);
+  s->launches++;
+  CU(add_partials(s, (long long)px * s->ny));
+  // Ly: the rows of the transposed copies
+  CU(to_transposed(s, U, s->tr[0]));
+  CU(to_transposed(s, out, s->tr[1]));
+  AdjointLineArgs Y{s->tr[0], s->tr[1], s->tr[2], nullptr, nullptr, s->d_fluid_t, s->d_gpart, lines_y(s), s->tape_dt, s->gamma,
+                    1.0 / s->dy, b, 0.0, 0.0, s->nu, 0};
+  adjoint_line_kernel<<<dim3(py, s->nx), A1D_TB, 0, s->stream>>>(Y);
+  s->launches++;
+  CU(add_partials(s, (long long)py * s->nx));
+  CU(add_from_transposed(s, s->tr[2], in, 0, s->ny + 6));
+  // Lv
+  if (s->mu > 0) {
+    const size_t nfx = (size_t)s->ny * (s->nx + 1);
+    Visc2dAdjArgs V{U, out, s->d_fluid, s->visc_C, s->visc_C + 7 * nfx, in, s->d_gpart, s->plane, s->nx, s->ny, s->pitch,
+                    s->gamma, s->mu, s->Pr, 1.0 / s->dx, 1.0 / s->dy, b * s->tape_dt};
+    const int gs = s->num_sms * 8;
+    viscous2d_adjoint_faces_kernel<<<gs, 256, 0, s->stream>>>(V);
+    viscous2d_adjoint_gather_kernel<<<gs, 256, 0, s->stream>>>(V);
+    viscous2d_adjoint_gamma_kernel<<<gs, 256, 0, s->stream>>>(V, s->d_gpart + gs);
+    s->launches += 3;
+    CU(add_partials(s, 2LL * gs));
+  }
+  if (ev1) cudaEventRecord(ev1, s->stream);
+  // the transposed fills, in the reverse order of the fills
+  if (s->n_ghost > 0) {
+    IbmList L{s->d_cell, s->d_donor, s->d_w, s->d_nrm, s->n_ghost};
+    double* gcontrib = s->d_contrib + (size_t)16 * s->n_ghost;
+    ibm_adjoint_ghost_kernel<<<(s->n_ghost + 127) / 128, 128, 0, s->stream>>>(U, in, s->plane, L, s->gamma, s->d_contrib, gcontrib);
+    ibm_adjoint_donor_kernel<<<(s->n_donor + 127) / 128, 128, 0, s->stream>>>(in, s->plane, s->d_dcell, s->d_drows, s->d_dentry,
+                                                                           s->n_donor, s->d_contrib);
+    sum_partials_kernel<<<1, 1024, 0, s->stream>>>(gcontrib, s->n_ghost, adj2_gbar(s));
+    s->launches += 3;
+  }
+  for (int axis = 1; axis >= 0; --axis) {
+    const int nline = axis == 1 ? s->nx + 6 : s->ny;
+    frame_fold_kernel<<<(2 * nline + 127) / 128, 128, 0, s->stream>>>(in, dims(s), bcspec(s), axis, s->bc.inflow[3], s->gamma,
+                                                                      s->d_gpart);
+    s->launches++;
+    CU(add_partials(s, 2LL * nline));
+  }
+  CU(cudaGetLastError());
+  return JXS_OK;
+}
+
+int adjoint2d_common(jxs_solver* s, void* Ubar, double* gamma_bar, const double* targets, double* loss) {
+  if (!s->tape2 || s->tape_steps < 1) return fail(s, JXS_ESTATE, "no recorded steps: call jxs_step_fixed_dt_record first");
+  const size_t state = (size_t)4 * s->plane, sb = state * sizeof(double);
+  if (!s->adj2) CU(cudaMalloc(&s->adj2, (4 * state + 2) * sizeof(double)));
+  CU(cudaMemsetAsync(s->adj2, 0, (4 * state + 2) * sizeof(double), s->stream));
+  auto T = [&](long long i) { return s->tape2 + i * state; };
+  auto B = [&](int i) { return adj2_state(s, i); };
+  const int per_step = (s->tape_scheme == JXS_EULER || s->tape_ckpt) ? 1 : 3;
+  const long long ncell4 = 4LL * s->nx * s->ny;
+  double* loss_acc = adj2_gbar(s) + 1;
+  const int igs = s->num_sms * 4;
+  auto inject = [&](long long n, int into, int accumulate) -> cudaError_t {  // Eq. 14: state after step n vs targets[n-1]
+    mse_inject2d_kernel<<<igs, 256, 0, s->stream>>>(T(per_step * n), targets + (n - 1) * ncell4, B(into), dims(s),
+                                                    2.0 / (s->tape_steps * (double)ncell4), accumulate, s->d_gpart);
+    sum_partials_kernel<<<1, 1024, 0, s->stream>>>(s->d_gpart, igs, loss_acc);
+    s->launches += 2;
+    return cudaGetLastError();
+  };
+  if (targets) CU(inject(s->tape_steps, 0, 0));
+  else CU(pad(s, Ubar, B(0)));
+  s->events_used = 0;
+  int x = 0;
+  for (long long n = s->tape_steps - 1; n >= 0; --n) {
+    if (targets && n + 1 < s->tape_steps) CU(inject(n + 1, x, 1));
+    int rc;
+    if (s->tape_scheme == JXS_EULER) {
+      rc = adjoint_stage2d(s, T(n), B(x), B(x ^ 1), 1.0, nullptr, 0.0, nullptr, 0.0);
+      if (rc != JXS_OK) return rc;
+      x ^= 1;
+      continue;
+    }
+    const double *S0 = T(3 * n), *S1 = T(3 * n + 1), *S2 = T(3 * n + 2);
+    if (s->tape_ckpt) {  // recompute the two inner stage states from the kept U^n (in the handle's own buffers)
+      CU(cudaMemcpyAsync(s->buf[0], T(n), sb, cudaMemcpyDeviceToDevice, s->stream));
+      CU(cudaMemcpyAsync(&s->d_state->dt, &s->tape_dt, sizeof(double), cudaMemcpyHostToDevice, s->stream));
+      CU(stage(s, s->buf[0], nullptr, s->buf[1], 0, 0.0, 1.0, nullptr));
+      CU(ghost_fill(s, s->buf[1]));
+      CU(stage(s, s->buf[1], s->buf[0], s->buf[2], 0, 0.75, 0.25, nullptr));
+      CU(ghost_fill(s, s->buf[2]));
+      S0 = (const double*)s->buf[0]; S1 = (const double*)s->buf[1]; S2 = (const double*)s->buf[2];
+    }
+    const int y2 = (x + 1) & 3, y1 = (x + 2) & 3, y0 = (x + 3) & 3;
+    // U^{n+1} = 1/3 U0 + 2/3 (U2 + dt L(U2));  U2 = 3/4 U0 + 1/4 (U1 + dt L(U1));  U1 = U0 + dt L(U0)   (R5)
+    rc = adjoint_stage2d(s, S2, B(x), B(y2), 2.0 / 3.0, nullptr, 0.0, nullptr, 0.0);
+    if (rc == JXS_OK) rc = adjoint_stage2d(s, S1, B(y2), B(y1), 0.25, nullptr, 0.0, nullptr, 0.0);
+    if (rc == JXS_OK) rc = adjoint_stage2d(s, S0, B(y1), B(y0), 1.0, B(x), 1.0 / 3.0, B(y2), 0.75);
+    if (rc != JXS_OK) return rc;
+    x = y0;
+  }
+  CU(unpad(s, B(x), Ubar));
+  double out[2];
+  CU(cudaMemcpyAsync(out, adj2_gbar(s), sizeof(out), cudaMemcpyDeviceToHost, s->stream));
   CU(cudaStreamSynchronize(s->stream));
   *gamma_bar = out[0];
   if (loss) *loss = out[1] / (s->tape_steps * (double)ncell4);
@@ -1185,6 +1543,9 @@ void jxs_destroy(jxs_solver* s) {
   cudaFree(s->d_mse);
   cudaFree(s->d_theta); cudaFree(s->d_dF1d); cudaFree(s->d_theta_bar); cudaFree(s->d_Wmlp);
   cudaFree(s->tape);
+  cudaFree(s->tape2); cudaFree(s->adj2); cudaFree(s->visc_C); cudaFree(s->d_gpart);
+  for (int q = 0; q < 4; ++q) cudaFree(s->tr[q]);
+  cudaFree(s->Lnat[0]); cudaFree(s->Lnat[1]);
   cudaFree(s->ckpt);
   cudaFree(s->adj);
   cudaFree(s->d_state);
@@ -1279,6 +1640,37 @@ int jxs_set_ibm(jxs_solver* s, const double* phi) {
     CU(cudaMemcpy(s->d_nrm, nrm.data(), sizeof(double) * 2 * ng, cudaMemcpyHostToDevice));
   }
   s->n_ghost = ng;
+  // for the reverse sweep (deriv2d_kernels.cuh): the fluid mask transposed, and the gather list transposed —
+  // every donor cell with the entries 16 q + 4 d of the ghost cells q it feeds, in increasing order (a fixed
+  // summation order instead of atomics)
+  {
+    std::vector<uint8_t> flt((size_t)nx * ny);
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i) flt[(size_t)i * ny + j] = fl[(size_t)j * nx + i];
+    CU(cudaMalloc(&s->d_fluid_t, flt.size()));
+    CU(cudaMemcpy(s->d_fluid_t, flt.data(), flt.size(), cudaMemcpyHostToDevice));
+    std::vector<std::pair<int, int>> de;  // (donor cell offset, entry)
+    for (int q = 0; q < ng; ++q)
+      for (int d = 0; d < 4; ++d)
+        if (wts[4 * q + d] > 0.0) de.emplace_back(donor[4 * q + d], 16 * q + 4 * d);
+    std::sort(de.begin(), de.end());
+    std::vector<int> dcell, rows, entry;
+    for (size_t e = 0; e < de.size(); ++e) {
+      if (e == 0 || de[e].first != de[e - 1].first) { dcell.push_back(de[e].first); rows.push_back((int)e); }
+      entry.push_back(de[e].second);
+    }
+    rows.push_back((int)de.size());
+    s->n_donor = (int)dcell.size();
+    if (s->n_donor > 0) {
+      CU(cudaMalloc(&s->d_dcell, sizeof(int) * dcell.size()));
+      CU(cudaMalloc(&s->d_drows, sizeof(int) * rows.size()));
+      CU(cudaMalloc(&s->d_dentry, sizeof(int) * entry.size()));
+      CU(cudaMalloc(&s->d_contrib, sizeof(double) * 17 * (size_t)ng));
+      CU(cudaMemcpy(s->d_dcell, dcell.data(), sizeof(int) * dcell.size(), cudaMemcpyHostToDevice));
+      CU(cudaMemcpy(s->d_drows, rows.data(), sizeof(int) * rows.size(), cudaMemcpyHostToDevice));
+      CU(cudaMemcpy(s->d_dentry, entry.data(), sizeof(int) * entry.size(), cudaMemcpyHostToDevice));
+    }
+  }
   return JXS_OK;
 }
 
