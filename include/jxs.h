@@ -68,6 +68,20 @@ typedef struct {
  * bad bc or dtype, NULL pointers.  JXS_ECUDA: no usable device.  JXS_ENOMEM: allocation failed. */
 int jxs_create(int nx, int ny, double dx, double dy, double gamma, double mu, double Pr,
                const jxs_bc* bc, int dtype, void* cuda_stream, jxs_solver** out);
+/* A BATCH of nbatch independent simulations on grids of one size (BASELINE.json configs[4]: 16 shock-cylinder runs;
+ * SURVEY.md section 8(f) rank 4), advanced by ONE launch per kernel and stage: the members are stacked along y in the
+ * handle's padded buffers, each with its own ghost frame, immersed boundary, time step and clock.
+ *   mu[nbatch]  dynamic viscosity of every member (all zero or all positive); bc[nbatch]: the same kinds on every
+ *               member, the inflow states may differ; nx, ny >= 8 (no one-dimensional batches)
+ * On a batch handle every field argument is [nbatch][4][ny][nx] (member-major), jxs_set_ibm takes [nbatch][ny][nx]
+ * level sets, jxs_max_wavespeed writes nbatch values, jxs_step evaluates the CFL step per member (jxs_get_time_batch),
+ * the flux MLP (one set of weights) serves all members.  Results are bitwise those of nbatch separate handles.
+ * Not available on a batch (JXS_EINVAL): the CNN flux, the nu-term, the derivatives, jxs_flux_correction.          */
+int jxs_create_batch(int nbatch, int nx, int ny, double dx, double dy, double gamma, const double* mu, double Pr,
+                     const jxs_bc* bc, int dtype, void* cuda_stream, jxs_solver** out);
+int jxs_batch_size(const jxs_solver*);
+/* t_host[nbatch], last_dt_host[nbatch] (either may be NULL): every member's clock (a single handle: one value) */
+int jxs_get_time_batch(const jxs_solver*, double* t_host, double* last_dt_host);
 void jxs_destroy(jxs_solver*);
 /* Never NULL; "" when there was no error.  Valid until the next call on the handle.        */
 const char* jxs_last_error(const jxs_solver*);

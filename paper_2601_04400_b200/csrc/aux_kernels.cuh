@@ -9,31 +9,34 @@
 
 namespace jxs {
 
+// A handle holds nb >= 1 independent grids of the same size (a batch: BASELINE.json configs[4]), stacked along y in
+// one padded buffer: member m owns the padded rows [m (ny+6), (m+1) (ny+6)), each with its own ghost frame.
 struct GridDims {
   int nx, ny, pitch;
-  long long plane;  // (ny+6)*pitch
+  long long plane;  // nb*(ny+6)*pitch
+  int nb;           // members of the batch
 };
 
-// interior [4][ny][nx] -> padded [4][ny+6][pitch] (interior cell (i,j) at row j+3, column i+3)
+// interior [nb][4][ny][nx] -> padded [4][nb (ny+6)][pitch] (interior cell (i,j) of member m at row m (ny+6) + j+3,
+// column i+3)
+__device__ __forceinline__ long long padded_offset(const GridDims& g, long long t) {
+  const long long n = (long long)g.nx * g.ny;
+  const int mk = (int)(t / n), m = mk >> 2, k = mk & 3;
+  const long long r = t - mk * n;
+  const int j = (int)(r / g.nx), i = (int)(r - (long long)j * g.nx);
+  return k * g.plane + ((long long)m * (g.ny + 6) + j + 3) * g.pitch + i + 3;
+}
 template <typename T>
 __global__ void pad_kernel(const T* __restrict__ src, T* __restrict__ dst, GridDims g) {
-  const long long n = (long long)g.nx * g.ny;
-  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < 4 * n; t += (long long)gridDim.x * blockDim.x) {
-    const int k = (int)(t / n);
-    const long long r = t - k * n;
-    const int j = (int)(r / g.nx), i = (int)(r - (long long)j * g.nx);
-    dst[k * g.plane + (long long)(j + 3) * g.pitch + i + 3] = src[t];
-  }
+  const long long n = (long long)g.nx * g.ny * g.nb;
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < 4 * n; t += (long long)gridDim.x * blockDim.x)
+    dst[padded_offset(g, t)] = src[t];
 }
 template <typename T>
 __global__ void unpad_kernel(const T* __restrict__ src, T* __restrict__ dst, GridDims g) {
-  const long long n = (long long)g.nx * g.ny;
-  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < 4 * n; t += (long long)gridDim.x * blockDim.x) {
-    const int k = (int)(t / n);
-    const long long r = t - k * n;
-    const int j = (int)(r / g.nx), i = (int)(r - (long long)j * g.nx);
-    dst[t] = src[k * g.plane + (long long)(j + 3) * g.pitch + i + 3];
-  }
+  const long long n = (long long)g.nx * g.ny * g.nb;
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < 4 * n; t += (long long)gridDim.x * blockDim.x)
+    dst[t] = src[padded_offset(g, t)];
 }
 // every element of the padded buffers starts as a benign state so that support cells outside the
 // frame never feed denormals/NaNs into the division slow paths
@@ -102,14 +105,22 @@ struct IbmList {
 // threads [nframe, nframe + ibm.n) fill one IBM ghost cell each (R9 I6): gather primitives at the
 // fluid donors, interpolate to the image point, reflect the velocity, store conserved.
 // IBM donors are interior fluid cells, so the two parts do not depend on each other.
+// inflow_tab: per-member inflow states (conserved, [nb][4]) of a batch whose members differ there; nullptr = bc's
 template <typename T>
-__global__ void ghost_fill_kernel(T* __restrict__ U, GridDims g, BcSpec bc, IbmList ibm, T gamma) {
+__global__ void ghost_fill_kernel(T* __restrict__ U, GridDims g, BcSpec bc, IbmList ibm, T gamma,
+                                  const double* __restrict__ inflow_tab = nullptr) {
   const int nxp = g.nx + 6, nyp = g.ny + 6;
   const int side_cells = 6 * g.ny;            // x-ghost columns of the interior rows
   // + full ghost rows (incl. corners); a one-dimensional problem (ny = 1) has no use for them
   const int nframe = side_cells + (g.ny > 1 ? 6 * nxp : 0);
-  const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t < nframe) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < nframe * g.nb) {
+    const int member = t / nframe;
+    t -= member * nframe;
+    U += (long long)member * nyp * g.pitch;  // this member's rows
+    if (inflow_tab) {
+      for (int k = 0; k < 4; ++k) bc.inflow_cons[k] = inflow_tab[4 * member + k];
+    }
     int ip, jp;  // padded indices in [0,nxp) x [0,nyp)
     if (t < side_cells) {
       jp = 3 + t / 6;
@@ -142,7 +153,7 @@ __global__ void ghost_fill_kernel(T* __restrict__ U, GridDims g, BcSpec bc, IbmL
     (void)nyp;
     return;
   }
-  const int q = t - nframe;
+  const int q = t - nframe * g.nb;
   if (q >= ibm.n) return;
   T WI[4] = {T(0), T(0), T(0), T(0)};
   for (int d = 0; d < 4; ++d) {
@@ -168,11 +179,16 @@ __device__ __forceinline__ void atomic_max_bits(unsigned long long* addr, double
   atomicMax(addr, (unsigned long long)__double_as_longlong(v));
 }
 
-// S9 stand-alone: max over fluid interior cells of max(|u|+a, |v|+a) from a padded buffer
+// S9 stand-alone: max over fluid interior cells of max(|u|+a, |v|+a) from a padded buffer; blockIdx.y = member of the
+// batch, whose result goes to the word out_stride bytes further on
 template <typename T>
 __global__ void wavespeed_kernel(const T* __restrict__ U, GridDims g, const uint8_t* __restrict__ fluid, T gamma,
-                                 unsigned long long* out_bits) {
+                                 unsigned long long* out_bits, long long out_stride = 0) {
   const long long n = (long long)g.nx * g.ny;
+  const int member = blockIdx.y;
+  U += (long long)member * (g.ny + 6) * g.pitch;
+  if (fluid) fluid += member * n;
+  out_bits = reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(out_bits) + member * out_stride);
   T smax = T(0);
   for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
     if (fluid && !fluid[t]) continue;
@@ -214,7 +230,10 @@ struct StepState {
 
 // once per step, before stage 1: dt = cfl*h/smax (R6) or the fixed dt; advance the clock; reset the
 // accumulator the last stage of this step will fill.
-__global__ void prepare_step_kernel(StepState* st, int cur, double cfl_h, double fixed_dt) {
+__global__ void prepare_step_kernel(StepState* st, int cur, double cfl_h, double fixed_dt, int nb = 1) {
+  const int m = blockIdx.x * blockDim.x + threadIdx.x;  // one thread per member of the batch
+  if (m >= nb) return;
+  st += m;
   double dt = fixed_dt;
   if (!(fixed_dt > 0.0)) {
     const double smax = __longlong_as_double((long long)st->smax_bits[cur]);

@@ -58,6 +58,7 @@ struct MlpArgs {
   long long plane;
   int nx, ny, pitch;
   int nstrips, rows_per_seg;
+  int nseg;              // row segments per strip and member of a batch (members are stacked along y, ny+6 rows each)
   T g1;                  // gamma - 1
   T inv_scale[4];        // 1 / in_scale of (rho, u_n, u_t, p)
   float bias[132];       // b1[64] b2[64] b3[4]: kernel parameters, i.e. constant-bank operands of the bias adds
@@ -157,10 +158,12 @@ __global__ void __launch_bounds__(MLP_TILE, 4) flux_mlp_kernel(const MlpArgs<T> 
   extern __shared__ __align__(128) unsigned char sm[];
   __shared__ uint32_t tmem_slot;
   const int t = threadIdx.x, warp = t >> 5;
-  const int strip = blockIdx.x % A.nstrips, seg = blockIdx.x / A.nstrips;
-  // cell rows whose faces this CTA evaluates: padded rows [rbeg, rend) of [2, ny+3)
-  const int rbeg = 2 + seg * A.rows_per_seg;
-  const int rend = min(rbeg + A.rows_per_seg, A.ny + 3);
+  const int strip = blockIdx.x % A.nstrips, seg_all = blockIdx.x / A.nstrips;
+  const int member = seg_all / A.nseg, seg = seg_all - member * A.nseg;
+  const int rb = member * (A.ny + 6);  // first padded row of my member
+  // cell rows whose faces this CTA evaluates: padded rows [rbeg, rend) of this member's [2, ny+3)
+  const int rbeg = rb + 2 + seg * A.rows_per_seg;
+  const int rend = min(rbeg + A.rows_per_seg, rb + A.ny + 3);
   if (rbeg >= rend) return;
   const int c0 = 2 + MLP_TILE * strip;  // padded column of thread 0's cell
   const int col = c0 + t;

@@ -45,6 +45,14 @@ template <typename T> constexpr int stage_minb() { return sizeof(T) == 8 ? JXS_M
 
 struct jxs_solver {
   int nx = 0, ny = 0, dtype = 0;
+  // batch (jxs_create_batch): nb independent grids of the same size stacked along y in every padded buffer; per member
+  // the viscosity, the inflow state, the immersed boundary, the time step and the clock
+  int nb = 1;
+  std::vector<double> mu_b, t_b, dt_b;
+  std::vector<jxs_bc> bc_b;
+  double* d_inflow_tab = nullptr;  // [nb][4] conserved inflow states
+  void* d_vtab = nullptr;          // [nb][10] viscous coefficients in the handle's dtype
+  int mlp_nseg = 1;
   double dx = 0, dy = 0, gamma = 0, mu = 0, Pr = 0, nu = 0;
   jxs_bc bc{};
   cudaStream_t stream = nullptr;
@@ -199,7 +207,7 @@ int check_device(const jxs_solver* s) {
     if (rc_ != JXS_OK) return rc_;          \
   } while (0)
 
-GridDims dims(const jxs_solver* s) { return GridDims{s->nx, s->ny, s->pitch, s->plane}; }
+GridDims dims(const jxs_solver* s) { return GridDims{s->nx, s->ny, s->pitch, s->plane, s->nb}; }
 
 BcSpec bcspec(const jxs_solver* s) {
   BcSpec b;
@@ -231,7 +239,7 @@ EncodeTiledFn encode_tiled_fn() {
 bool make_tensor_map(const jxs_solver* s, void* base, int box_w, CUtensorMap* out) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return false;
-  const cuuint64_t gdim[3] = {(cuuint64_t)s->pitch, (cuuint64_t)(s->ny + 6), 4};
+  const cuuint64_t gdim[3] = {(cuuint64_t)s->pitch, (cuuint64_t)s->nb * (s->ny + 6), 4};
   const cuuint64_t gstride[2] = {(cuuint64_t)s->pitch * s->elem, (cuuint64_t)s->plane * s->elem};
   const cuuint32_t box[3] = {(cuuint32_t)box_w, 1, 4};
   const cuuint32_t estr[3] = {1, 1, 1};
@@ -260,7 +268,7 @@ void set_rows_per_seg(jxs_solver* s, int rps, double tail_frac = 0.0) {
     if (left > 0) { s->nseg_a = na; s->rows_b = rb; nseg_b = (left + rb - 1) / rb; }
   }
   s->nseg = s->nseg_a + nseg_b;
-  s->ntasks = s->nseg * s->nstrips;
+  s->ntasks = s->nseg * s->nstrips * s->nb;
   s->grid = s->ntasks;
 }
 
@@ -273,7 +281,7 @@ void choose_decomposition(jxs_solver* s) {
   std::vector<double> cost(s->ny + 1, 0.0);
   double best = 1e300;
   for (int rps = lo; rps <= s->ny; ++rps) {
-    const double tasks = (double)((s->ny + rps - 1) / rps) * s->nstrips;
+    const double tasks = (double)((s->ny + rps - 1) / rps) * s->nstrips * s->nb;
     const double len = rps + 2.0;
     // one wave: the FP64 pipe of an SM is saturated by about 8 warps, fewer tasks run at full speed each
     cost[rps] = tasks <= slots ? 1.15 * len * std::max(1.0, tasks * s->share / (8.0 * s->num_sms))
@@ -289,9 +297,9 @@ void choose_decomposition(jxs_solver* s) {
   s->tuned = s->rows_fixed > 0;
 }
 
-template <typename T, bool VISC, bool ARTV, bool MLP>
+template <typename T, bool VISC, bool ARTV, bool MLP, bool BATCH = false>
 cudaError_t launch_stage_t(jxs_solver* s, const StageArgs<T>& a) {
-  auto kern = stage_kernel<T, VISC, ARTV, MLP, stage_minb<T>()>;
+  auto kern = stage_kernel<T, VISC, ARTV, MLP, stage_minb<T>(), BATCH>;
   constexpr int NV = VISC ? 5 : 4;
   const size_t smem = stage_smem_per_warp<T, NV>();
   static bool configured[MAX_DEVICES] = {false};
@@ -314,6 +322,7 @@ cudaError_t launch_stage(jxs_solver* s, const void* Uin, const void* U0, void* U
   A.plane = s->plane; A.nx = s->nx; A.ny = s->ny; A.pitch = s->pitch;
   A.nstrips = s->nstrips; A.rows_per_seg = s->rows_per_seg; A.ntasks = s->ntasks;
   A.nseg_a = s->nseg_a; A.rows_b = s->rows_b;
+  A.nb = s->nb; A.nseg = s->nseg; A.state_stride = (long long)sizeof(StepState); A.vtab = (const T*)s->d_vtab;
   A.mode = mode;
   A.gamma = (T)s->gamma; A.g1 = (T)(s->gamma - 1.0); A.g1inv = (T)(1.0 / (s->gamma - 1.0));
   A.dxi = (T)(1.0 / s->dx); A.dyi = (T)(1.0 / s->dy);
@@ -345,6 +354,9 @@ cudaError_t launch_stage(jxs_solver* s, const void* Uin, const void* U0, void* U
   if (s->ny == 1) {  // one-dimensional problems: stage1d_kernel.cuh
     stage1d_kernel<T><<<(s->nx + S1D_OUT - 1) / S1D_OUT, S1D_TB, 0, s->stream>>>(A);
     e = cudaGetLastError();
+  } else if (s->nb > 1) {  // batch: one launch over all members (no nu-term: jxs_set_artificial_viscosity refuses)
+    if (s->mlp_on) e = visc ? launch_stage_t<T, true, false, true, true>(s, A) : launch_stage_t<T, false, false, true, true>(s, A);
+    else e = visc ? launch_stage_t<T, true, false, false, true>(s, A) : launch_stage_t<T, false, false, false, true>(s, A);
   } else if (s->mlp_on || s->cnn_on) {
     if (visc) e = artv ? launch_stage_t<T, true, true, true>(s, A) : launch_stage_t<T, true, false, true>(s, A);
     else e = artv ? launch_stage_t<T, false, true, true>(s, A) : launch_stage_t<T, false, false, true>(s, A);
@@ -365,13 +377,15 @@ cudaError_t stage(jxs_solver* s, const void* Uin, const void* U0, void* Uout, in
 
 cudaError_t ghost_fill(jxs_solver* s, void* U) {
   const int nframe = 6 * s->ny + (s->ny > 1 ? 6 * (s->nx + 6) : 0);
-  const int total = nframe + s->n_ghost;
+  const int total = nframe * s->nb + s->n_ghost;
   IbmList L{s->d_cell, s->d_donor, s->d_w, s->d_nrm, s->n_ghost};
   const int bs = 128;
   if (s->dtype == JXS_F64)
-    ghost_fill_kernel<double><<<(total + bs - 1) / bs, bs, 0, s->stream>>>((double*)U, dims(s), bcspec(s), L, s->gamma);
+    ghost_fill_kernel<double><<<(total + bs - 1) / bs, bs, 0, s->stream>>>((double*)U, dims(s), bcspec(s), L, s->gamma,
+                                                                          s->d_inflow_tab);
   else
-    ghost_fill_kernel<float><<<(total + bs - 1) / bs, bs, 0, s->stream>>>((float*)U, dims(s), bcspec(s), L, (float)s->gamma);
+    ghost_fill_kernel<float><<<(total + bs - 1) / bs, bs, 0, s->stream>>>((float*)U, dims(s), bcspec(s), L, (float)s->gamma,
+                                                                         s->d_inflow_tab);
   s->launches++;
   return cudaGetLastError();
 }
@@ -382,7 +396,7 @@ cudaError_t launch_flux_mlp(jxs_solver* s, const void* U) {
   MlpArgs<T> A;
   A.U = (const T*)U; A.dF = s->d_dF; A.dG = s->d_dG; A.blob = s->d_mlp_blob;
   A.plane = s->plane; A.nx = s->nx; A.ny = s->ny; A.pitch = s->pitch;
-  A.nstrips = s->mlp_strips; A.rows_per_seg = s->mlp_rows_per_seg;
+  A.nstrips = s->mlp_strips; A.rows_per_seg = s->mlp_rows_per_seg; A.nseg = s->mlp_nseg;
   A.g1 = (T)(s->gamma - 1.0);
   for (int k = 0; k < 4; ++k) A.inv_scale[k] = (T)(1.0 / s->in_scale[k]);
   std::memcpy(A.bias, s->mlp_bias, sizeof(A.bias));
@@ -539,13 +553,17 @@ cudaError_t unpad(jxs_solver* s, const void* src, void* U) {
 }
 
 cudaError_t wavespeed(jxs_solver* s, const void* Upad, unsigned long long* out_bits) {
-  cudaError_t e = cudaMemsetAsync(out_bits, 0, sizeof(unsigned long long), s->stream);
+  // out_bits: the word of member 0; member m's lies m StepStates further on
+  cudaError_t e = cudaMemset2DAsync(out_bits, sizeof(StepState), 0, sizeof(unsigned long long), s->nb, s->stream);
   if (e != cudaSuccess) return e;
-  const int bs = 256, gs = s->num_sms * 8;
+  const int bs = 256;
+  const dim3 gs(std::max(1, s->num_sms * 8 / s->nb), s->nb);
   if (s->dtype == JXS_F64)
-    wavespeed_kernel<double><<<gs, bs, 0, s->stream>>>((const double*)Upad, dims(s), s->d_fluid, s->gamma, out_bits);
+    wavespeed_kernel<double><<<gs, bs, 0, s->stream>>>((const double*)Upad, dims(s), s->d_fluid, s->gamma, out_bits,
+                                                       (long long)sizeof(StepState));
   else
-    wavespeed_kernel<float><<<gs, bs, 0, s->stream>>>((const float*)Upad, dims(s), s->d_fluid, (float)s->gamma, out_bits);
+    wavespeed_kernel<float><<<gs, bs, 0, s->stream>>>((const float*)Upad, dims(s), s->d_fluid, (float)s->gamma, out_bits,
+                                                      (long long)sizeof(StepState));
   s->launches++;
   return cudaGetLastError();
 }
@@ -564,7 +582,7 @@ void free_ibm(jxs_solver* s) {
 // the two buffers every step; SSP-RK3 always starts and ends in buf[0]).
 // SSP-RK3 (R5): three stages.  Forward Euler (Eq. 10 as printed): one stage with (a,b) = (0,1).
 int one_step(jxs_solver* s, double cfl_h, double fixed_dt, int& cur, int& at) {
-  prepare_step_kernel<<<1, 1, 0, s->stream>>>(s->d_state, cur, cfl_h, fixed_dt);
+  prepare_step_kernel<<<(s->nb + 63) / 64, 64, 0, s->stream>>>(s->d_state, cur, cfl_h, fixed_dt, s->nb);
   s->launches++;
   CU(cudaGetLastError());
   unsigned long long* next = &s->d_state->smax_bits[cur ^ 1];
@@ -651,9 +669,15 @@ int run_steps(jxs_solver* s, double cfl, double fixed_dt, int nsteps, int* where
 }
 
 int finish_steps(jxs_solver* s, int nsteps) {
-  StepState st;
-  CU(cudaMemcpyAsync(&st, s->d_state, sizeof(st), cudaMemcpyDeviceToHost, s->stream));
+  std::vector<StepState> sts(s->nb);
+  CU(cudaMemcpyAsync(sts.data(), s->d_state, sizeof(StepState) * s->nb, cudaMemcpyDeviceToHost, s->stream));
   CU(cudaStreamSynchronize(s->stream));
+  StepState st = sts[0];
+  for (int m = 0; m < s->nb; ++m) {
+    s->t_b[m] = sts[m].t;
+    if (nsteps > 0) s->dt_b[m] = sts[m].dt;
+    st.bad |= sts[m].bad;
+  }
   s->t = st.t;
   if (nsteps > 0) s->last_dt = st.dt;
   if (s->profiling) {
@@ -674,7 +698,8 @@ int finish_steps(jxs_solver* s, int nsteps) {
   }
   if (st.bad) {
     int zero = 0;
-    cudaMemcpyAsync(&s->d_state->bad, &zero, sizeof(int), cudaMemcpyHostToDevice, s->stream);
+    for (int m = 0; m < s->nb; ++m)
+      cudaMemcpyAsync(&s->d_state[m].bad, &zero, sizeof(int), cudaMemcpyHostToDevice, s->stream);
     return fail(s, JXS_ENUMERIC, "non-finite or non-positive wavespeed met while stepping");
   }
   const double sm = 0;  (void)sm;
@@ -735,7 +760,7 @@ int step_common(jxs_solver* s, void* U, double cfl, double fixed_dt, int nsteps,
   if (!U) return fail(s, JXS_EINVAL, "U is NULL");
   if (nsteps < 0) return fail(s, JXS_EINVAL, "nsteps < 0");
   if (!(fixed_dt > 0) && !(cfl > 0)) return fail(s, JXS_EINVAL, "cfl must be > 0");
-  const size_t bytes = (size_t)4 * s->nx * s->ny * s->elem;
+  const size_t bytes = (size_t)4 * s->nx * s->ny * s->nb * s->elem;
   const void* Ud = U;
   if (host) {
     CU(cudaMemcpyAsync(s->stage_io, U, bytes, cudaMemcpyHostToDevice, s->stream));
@@ -860,6 +885,7 @@ int tangent_common(jxs_solver* s, void* U, void* Udot, double gamma_dot, double 
   if (!(dt > 0)) return fail(s, JXS_EINVAL, "dt must be > 0");
   if (!std::isfinite(gamma_dot)) return fail(s, JXS_EINVAL, "gamma_dot is not finite");
   if (s->dtype != JXS_F64) return fail(s, JXS_EINVAL, "the tangent is fp64 only");
+  if (s->nb > 1) return fail(s, JXS_EINVAL, "no derivatives on a batch handle");
   if (s->mlp_on || s->cnn_on || s->mlp1d_on) return fail(s, JXS_ESTATE, "the tangent does not differentiate the networks");
   if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
   if (s->ny != 1) return tangent2d_common(s, U, Udot, gamma_dot, dt, nsteps);
@@ -924,6 +950,7 @@ double* compact_state(const jxs_solver* s, double* base, long long i) {
 
 int adjoint_checks(jxs_solver* s) {
   if (s->dtype != JXS_F64) return fail(s, JXS_EINVAL, "the adjoint is fp64 only");
+  if (s->nb > 1) return fail(s, JXS_EINVAL, "no derivatives on a batch handle");
   if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
   return JXS_OK;
 }
@@ -1468,26 +1495,39 @@ int adjoint2d_common(jxs_solver* s, void* Ubar, double* gamma_bar, const double*
 
 extern "C" {
 
-int jxs_create(int nx, int ny, double dx, double dy, double gamma, double mu, double Pr, const jxs_bc* bc, int dtype,
-               void* cuda_stream, jxs_solver** out) {
+static int create_common(int nb, int nx, int ny, double dx, double dy, double gamma, const double* mu_b, double Pr,
+                         const jxs_bc* bc_b, int dtype, void* cuda_stream, jxs_solver** out) {
   if (!out) return JXS_EINVAL;
   *out = nullptr;
-  if (!bc) return JXS_EINVAL;
-  if (nx < 8 || (ny < 8 && ny != 1) || !(dx > 0) || !(dy > 0) || !(gamma > 1) || !(mu >= 0) || (mu > 0 && !(Pr > 0)))
-    return JXS_EINVAL;
+  if (!bc_b || !mu_b || nb < 1) return JXS_EINVAL;
+  if (nb > 1 && ny == 1) return JXS_EINVAL;  // batches are two-dimensional
+  if (nx < 8 || (ny < 8 && ny != 1) || !(dx > 0) || !(dy > 0) || !(gamma > 1)) return JXS_EINVAL;
   if (dtype != JXS_F64 && dtype != JXS_F32) return JXS_EINVAL;
-  const int kinds[4] = {bc->xlo, bc->xhi, bc->ylo, bc->yhi};
-  for (int k : kinds)
-    if (k < 0 || k > 3) return JXS_EINVAL;
-  if ((bc->xlo == JXS_BC_PERIODIC) != (bc->xhi == JXS_BC_PERIODIC)) return JXS_EINVAL;
-  if ((bc->ylo == JXS_BC_PERIODIC) != (bc->yhi == JXS_BC_PERIODIC)) return JXS_EINVAL;
-  for (int k = 0; k < 4; ++k)
-    if (!std::isfinite(bc->inflow[k])) return JXS_EINVAL;
+  for (int m = 0; m < nb; ++m) {
+    const jxs_bc* bc = bc_b + m;
+    if (!(mu_b[m] >= 0) || (mu_b[m] > 0 && !(Pr > 0)) || (mu_b[m] > 0) != (mu_b[0] > 0)) return JXS_EINVAL;
+    const int kinds[4] = {bc->xlo, bc->xhi, bc->ylo, bc->yhi};
+    for (int k : kinds)
+      if (k < 0 || k > 3) return JXS_EINVAL;
+    if ((bc->xlo == JXS_BC_PERIODIC) != (bc->xhi == JXS_BC_PERIODIC)) return JXS_EINVAL;
+    if ((bc->ylo == JXS_BC_PERIODIC) != (bc->yhi == JXS_BC_PERIODIC)) return JXS_EINVAL;
+    for (int k = 0; k < 4; ++k)
+      if (!std::isfinite(bc->inflow[k])) return JXS_EINVAL;
+    // the members of a batch share the kinds of their boundary conditions; the inflow states may differ
+    if (bc->xlo != bc_b->xlo || bc->xhi != bc_b->xhi || bc->ylo != bc_b->ylo || bc->yhi != bc_b->yhi) return JXS_EINVAL;
+  }
+  const jxs_bc* bc = bc_b;
+  const double mu = mu_b[0];
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return JXS_ECUDA;
   jxs_solver* s = new (std::nothrow) jxs_solver;
   if (!s) return JXS_ENOMEM;
   s->nx = nx; s->ny = ny; s->dx = dx; s->dy = dy; s->gamma = gamma; s->mu = mu; s->Pr = Pr; s->bc = *bc;
+  s->nb = nb;
+  s->mu_b.assign(mu_b, mu_b + nb);
+  s->bc_b.assign(bc_b, bc_b + nb);
+  s->t_b.assign(nb, 0.0);
+  s->dt_b.assign(nb, 0.0);
   if (ny == 1) s->bc.ylo = s->bc.yhi = JXS_BC_TRANSMISSIVE;  // the ghost rows of a single row are copies of it
   s->dtype = dtype;
   s->elem = dtype == JXS_F64 ? 8 : 4;
@@ -1501,14 +1541,36 @@ int jxs_create(int nx, int ny, double dx, double dy, double gamma, double mu, do
   choose_decomposition(s);
   const int SOUT = dtype == JXS_F64 ? sout<double>() : sout<float>();
   s->pitch = ((SOUT * s->nstrips + 6 + 15) / 16) * 16;
-  s->plane = (long long)(ny + 6) * s->pitch;
+  s->plane = (long long)nb * (ny + 6) * s->pitch;
   if (s->plane > 0x7fffffffLL) { delete s; return JXS_EINVAL; }
   const size_t pbytes = (size_t)4 * s->plane * s->elem;
   cudaError_t e = cudaSuccess;
   for (int b = 0; b < 3 && e == cudaSuccess; ++b) e = cudaMalloc(&s->buf[b], pbytes);
-  if (e == cudaSuccess) e = cudaMalloc(&s->stage_io, (size_t)4 * nx * ny * s->elem);
-  if (e == cudaSuccess) e = cudaMalloc(&s->d_state, sizeof(StepState));
-  if (e == cudaSuccess) e = cudaMemsetAsync(s->d_state, 0, sizeof(StepState), s->stream);
+  if (e == cudaSuccess) e = cudaMalloc(&s->stage_io, (size_t)4 * nx * ny * nb * s->elem);
+  if (e == cudaSuccess) e = cudaMalloc(&s->d_state, sizeof(StepState) * nb);
+  if (e == cudaSuccess) e = cudaMemsetAsync(s->d_state, 0, sizeof(StepState) * nb, s->stream);
+  if (e == cudaSuccess && nb > 1) {  // per-member inflow states and viscous coefficients (the order of StageArgs)
+    std::vector<double> inflow(4 * (size_t)nb), vt(10 * (size_t)nb);
+    for (int m = 0; m < nb; ++m) {
+      const double r = bc_b[m].inflow[0], u = bc_b[m].inflow[1], v = bc_b[m].inflow[2], p = bc_b[m].inflow[3];
+      inflow[4 * m] = r; inflow[4 * m + 1] = r * u; inflow[4 * m + 2] = r * v;
+      inflow[4 * m + 3] = p / (gamma - 1.0) + 0.5 * r * (u * u + v * v);
+      const double mm = mu_b[m], kap = mm > 0 ? mm * gamma / ((gamma - 1.0) * Pr) : 0.0, dxi = 1.0 / dx, dyi = 1.0 / dy;
+      const double c[10] = {4.0 / 3.0 * mm * dyi, 2.0 / 3.0 * mm * 0.25 * dxi, mm * dyi, mm * 0.25 * dxi, kap * dyi,
+                            4.0 / 3.0 * mm * dxi, 2.0 / 3.0 * mm * 0.25 * dyi, mm * dxi, mm * 0.25 * dyi, kap * dxi};
+      for (int q = 0; q < 10; ++q) vt[10 * m + q] = c[q];
+    }
+    e = cudaMalloc(&s->d_inflow_tab, inflow.size() * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemcpy(s->d_inflow_tab, inflow.data(), inflow.size() * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_vtab, vt.size() * s->elem);
+    if (e == cudaSuccess) {
+      if (dtype == JXS_F64) e = cudaMemcpy(s->d_vtab, vt.data(), vt.size() * sizeof(double), cudaMemcpyHostToDevice);
+      else {
+        std::vector<float> vf(vt.begin(), vt.end());
+        e = cudaMemcpy(s->d_vtab, vf.data(), vf.size() * sizeof(float), cudaMemcpyHostToDevice);
+      }
+    }
+  }
   if (e != cudaSuccess) {
     const int rc = e == cudaErrorMemoryAllocation ? JXS_ENOMEM : JXS_ECUDA;
     jxs_destroy(s);
@@ -1531,6 +1593,15 @@ int jxs_create(int nx, int ny, double dx, double dy, double gamma, double mu, do
   return JXS_OK;
 }
 
+int jxs_create(int nx, int ny, double dx, double dy, double gamma, double mu, double Pr, const jxs_bc* bc, int dtype,
+               void* cuda_stream, jxs_solver** out) {
+  return create_common(1, nx, ny, dx, dy, gamma, &mu, Pr, bc, dtype, cuda_stream, out);
+}
+int jxs_create_batch(int nbatch, int nx, int ny, double dx, double dy, double gamma, const double* mu, double Pr,
+                     const jxs_bc* bc, int dtype, void* cuda_stream, jxs_solver** out) {
+  return create_common(nbatch, nx, ny, dx, dy, gamma, mu, Pr, bc, dtype, cuda_stream, out);
+}
+
 void jxs_destroy(jxs_solver* s) {
   if (!s) return;
   cudaStreamSynchronize(s->stream);
@@ -1549,6 +1620,7 @@ void jxs_destroy(jxs_solver* s) {
   cudaFree(s->ckpt);
   cudaFree(s->adj);
   cudaFree(s->d_state);
+  cudaFree(s->d_inflow_tab); cudaFree(s->d_vtab);
   free_ibm(s);
   cudaFree(s->d_mlp_blob); cudaFree(s->d_dF); cudaFree(s->d_dG);
   for (int d = 0; d < 2; ++d) {
@@ -1574,11 +1646,16 @@ int jxs_set_ibm(jxs_solver* s, const double* phi) {
   const double dx = s->dx, dy = s->dy;
   // classification (R9 I1, I2): 1 = fluid in `fl`; ghost = non-fluid cell that some fluid cell's
   // WENO stencil (3 cells along an axis) or viscous stencil (3x3 box) touches
-  std::vector<uint8_t> fl((size_t)nx * ny);
-  for (size_t c = 0; c < fl.size(); ++c) fl[c] = phi[c] > 0.0 ? 1 : 0;
-  auto is_fluid = [&](int i, int j) { return i >= 0 && i < nx && j >= 0 && j < ny && fl[(size_t)j * nx + i]; };
+  std::vector<uint8_t> fl_all((size_t)nx * ny * s->nb);
+  for (size_t c = 0; c < fl_all.size(); ++c) fl_all[c] = phi[c] > 0.0 ? 1 : 0;
   std::vector<int> cell, donor;
   std::vector<double> wts, nrm;
+  const double* const phi_all = phi;
+  for (int member = 0; member < s->nb; ++member) {  // a batch: one level set per member, [nb][ny][nx]
+  const uint8_t* fl = fl_all.data() + (size_t)member * nx * ny;
+  phi = phi_all + (size_t)member * nx * ny;
+  const int moff = member * (ny + 6) * s->pitch;  // this member's rows in the padded buffers
+  auto is_fluid = [&](int i, int j) { return i >= 0 && i < nx && j >= 0 && j < ny && fl[(size_t)j * nx + i]; };
   static const int off[16][2] = {{1, 0}, {-1, 0}, {0, 1}, {0, -1}, {2, 0}, {-2, 0}, {0, 2}, {0, -2},
                                  {3, 0}, {-3, 0}, {0, 3}, {0, -3}, {1, 1}, {-1, 1}, {1, -1}, {-1, -1}};
   const double h = std::min(dx, dy);
@@ -1618,14 +1695,17 @@ int jxs_set_ibm(jxs_solver* s, const double* phi) {
         xi += h * n0; yi += h * n1;
       }
       if (!(sum > 0.0)) return fail(s, JXS_EINVAL, "IBM: ghost cell without a fluid donor");
-      cell.push_back((j + 3) * s->pitch + i + 3);
+      cell.push_back(moff + (j + 3) * s->pitch + i + 3);
       for (int d = 0; d < 4; ++d) {
         const double wd = w[d] / sum;
         wts.push_back(wd);
-        donor.push_back(wd > 0.0 ? (dj[d] + 3) * s->pitch + di[d] + 3 : (j + 3) * s->pitch + i + 3);
+        donor.push_back(moff + (wd > 0.0 ? (dj[d] + 3) * s->pitch + di[d] + 3 : (j + 3) * s->pitch + i + 3));
       }
       nrm.push_back(n0); nrm.push_back(n1);
     }
+  }  // members
+  phi = phi_all;
+  const std::vector<uint8_t>& fl = fl_all;
   const int ng = (int)cell.size();
   CU(cudaMalloc(&s->d_fluid, fl.size()));
   CU(cudaMemcpy(s->d_fluid, fl.data(), fl.size(), cudaMemcpyHostToDevice));
@@ -1643,7 +1723,7 @@ int jxs_set_ibm(jxs_solver* s, const double* phi) {
   // for the reverse sweep (deriv2d_kernels.cuh): the fluid mask transposed, and the gather list transposed —
   // every donor cell with the entries 16 q + 4 d of the ghost cells q it feeds, in increasing order (a fixed
   // summation order instead of atomics)
-  {
+  if (s->nb == 1) {
     std::vector<uint8_t> flt((size_t)nx * ny);
     for (int j = 0; j < ny; ++j)
       for (int i = 0; i < nx; ++i) flt[(size_t)i * ny + j] = fl[(size_t)j * nx + i];
@@ -1725,10 +1805,11 @@ int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[
   s->mlp_strips = (s->nx + 1 + MLP_TILE - 1) / MLP_TILE;
   const int nrows = s->ny + 1;
   const long long slots = (long long)s->num_sms * 4;
-  int segs = (int)std::max<long long>(1, slots / s->mlp_strips);
+  int segs = (int)std::max<long long>(1, slots / ((long long)s->mlp_strips * s->nb));
   int rps = std::max((nrows + segs - 1) / segs, std::min(nrows, 16));
   s->mlp_rows_per_seg = rps;
-  s->mlp_grid = s->mlp_strips * ((nrows + rps - 1) / rps);
+  s->mlp_nseg = (nrows + rps - 1) / rps;
+  s->mlp_grid = s->mlp_strips * s->mlp_nseg * s->nb;
   s->mlp_on = true;
   return JXS_OK;
 }
@@ -1740,6 +1821,7 @@ int jxs_set_flux_cnn(jxs_solver* s, const float* weights, const double in_scale[
   CU(cudaStreamSynchronize(s->stream));
   if (!weights) { s->cnn_on = false; return JXS_OK; }
   if (s->ny == 1) return fail(s, JXS_EINVAL, "no CNN flux in one-dimensional problems");
+  if (s->nb > 1) return fail(s, JXS_EINVAL, "no CNN flux on a batch handle");
   if (s->mlp_on) return fail(s, JXS_ESTATE, "the flux MLP is set: disable it first (jxs_set_flux_mlp(NULL))");
   if (!in_scale || !out_scale) return fail(s, JXS_EINVAL, "in_scale / out_scale is NULL");
   for (int k = 0; k < 4; ++k)
@@ -1794,6 +1876,7 @@ int jxs_flux_cnn_inputs(jxs_solver* s, const void* U, float* Xx, float* Xy) {
 int jxs_set_artificial_viscosity(jxs_solver* s, double nu) {
   if (!s) return JXS_EINVAL;
   if (!(nu >= 0) || !std::isfinite(nu)) return fail(s, JXS_EINVAL, "nu must be finite and >= 0");
+  if (s->nb > 1 && nu > 0) return fail(s, JXS_EINVAL, "no nu-term on a batch handle");
   if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
   drop_graph(s);
   s->tape_steps = 0;  // a recording made with another nu cannot be reversed
@@ -1826,7 +1909,7 @@ int jxs_rhs_host(jxs_solver* s, const void* U, void* dUdt) {
   if (!s) return JXS_EINVAL;
   DEV(s);
   if (!U || !dUdt) return fail(s, JXS_EINVAL, "NULL array");
-  const size_t bytes = (size_t)4 * s->nx * s->ny * s->elem;
+  const size_t bytes = (size_t)4 * s->nx * s->ny * s->nb * s->elem;
   CU(cudaMemcpyAsync(s->stage_io, U, bytes, cudaMemcpyHostToDevice, s->stream));
   CU(pad(s, s->stage_io, s->buf[0]));
   CU(ghost_fill(s, s->buf[0]));
@@ -1844,12 +1927,11 @@ int jxs_max_wavespeed(jxs_solver* s, const void* U, double* smax) {
   CU(pad(s, U, s->buf[1]));
   unsigned long long* bits = &s->d_state->smax_bits[0];
   CU(wavespeed(s, s->buf[1], bits));
-  unsigned long long h = 0;
-  CU(cudaMemcpyAsync(&h, bits, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+  std::vector<unsigned long long> h(s->nb);
+  CU(cudaMemcpy2DAsync(h.data(), sizeof(unsigned long long), bits, sizeof(StepState), sizeof(unsigned long long), s->nb,
+                       cudaMemcpyDeviceToHost, s->stream));
   CU(cudaStreamSynchronize(s->stream));
-  double v;
-  std::memcpy(&v, &h, sizeof(v));
-  *smax = v;
+  std::memcpy(smax, h.data(), sizeof(double) * s->nb);  // one value per member of a batch
   return JXS_OK;
 }
 
@@ -1948,6 +2030,7 @@ int jxs_set_time_integrator(jxs_solver* s, int scheme) {
   if (!s) return JXS_EINVAL;
   drop_graph(s);
   if (scheme != JXS_SSPRK3 && scheme != JXS_EULER) return fail(s, JXS_EINVAL, "unknown time integrator");
+  if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
   s->scheme = scheme;
   return JXS_OK;
 }
@@ -1958,6 +2041,16 @@ int jxs_get_time(const jxs_solver* s, double* t, double* last_dt) {
   if (last_dt) *last_dt = s->last_dt;
   return JXS_OK;
 }
+
+int jxs_get_time_batch(const jxs_solver* s, double* t, double* last_dt) {
+  if (!s) return JXS_EINVAL;
+  for (int m = 0; m < s->nb; ++m) {
+    if (t) t[m] = s->t_b[m];
+    if (last_dt) last_dt[m] = s->dt_b[m];
+  }
+  return JXS_OK;
+}
+int jxs_batch_size(const jxs_solver* s) { return s ? s->nb : -1; }
 
 long long jxs_launch_count(const jxs_solver* s) { return s ? s->launches : -1; }
 
@@ -1994,6 +2087,7 @@ int jxs_flux_correction(jxs_solver* s, const void* U, float* dFx, float* dGy) {
   DEV(s);
   if (!U || !dFx || !dGy) return fail(s, JXS_EINVAL, "NULL array");
   if (!s->mlp_on && !s->cnn_on) return fail(s, JXS_ESTATE, "no flux network set (jxs_set_flux_mlp / jxs_set_flux_cnn)");
+  if (s->nb > 1) return fail(s, JXS_EINVAL, "jxs_flux_correction inspects single handles");
   CU(pad(s, U, s->buf[0]));
   CU(ghost_fill(s, s->buf[0]));
   CU(flux_mlp(s, s->buf[0]));

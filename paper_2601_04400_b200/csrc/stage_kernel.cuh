@@ -50,6 +50,12 @@ struct StageArgs {
   int nx, ny, pitch;
   int nstrips, rows_per_seg, ntasks;
   int nseg_a, rows_b;    // the first nseg_a row segments of a strip have rows_per_seg rows, the later ones rows_b
+  // batch (BATCH instantiations): nb members stacked along y, nseg row segments per strip and member; dt and
+  // smax_bits of member m lie state_stride bytes further on per member, its ten viscous coefficients (the order of
+  // vy_n .. vx_q below) at vtab[10 m], its fluid mask and (mode 1) output at member strides
+  int nb, nseg;
+  long long state_stride;
+  const T* vtab;
   int mode;
   T gamma, g1, g1inv, dxi, dyi, mu, kappa, nu;
   T rk_a, rk_b;          // Uout = a*U0 + b*(Uin + dt*L)
@@ -459,7 +465,7 @@ __host__ __device__ constexpr size_t stage_smem_per_warp() {
 }
 
 // ------------------------------------------------------------------ the kernel
-template <typename T, bool VISC, bool ARTV, bool MLP, int MINB>
+template <typename T, bool VISC, bool ARTV, bool MLP, int MINB, bool BATCH = false>
 __global__ void __launch_bounds__(STAGE_WARPS * 32, MINB)
 stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, const __grid_constant__ CUtensorMap tm_epi,
              const __grid_constant__ CUtensorMap tm_epi0) {
@@ -471,12 +477,14 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
   constexpr int EW = Epi<T>::W, EOFF = Epi<T>::OFF;
   const int lane = threadIdx.x;
   const int task = blockIdx.x;
-  const int strip = task % A.nstrips, seg = task / A.nstrips;
+  const int strip = task % A.nstrips, seg_all = task / A.nstrips;
+  const int member = BATCH ? seg_all / A.nseg : 0, seg = BATCH ? seg_all - member * A.nseg : seg_all;
+  const int rb = BATCH ? member * (A.ny + 6) : 0;  // first padded row of my member
   // first output row (padded index) and one past the last; tasks are handed out in blockIdx order, segment-major, and
   // the last segments are the short ones: the kernel's tail (SMs running out of tasks) shrinks with the task length
   const bool seg_long = seg < A.nseg_a;
-  const int jbeg = 3 + (seg_long ? seg * A.rows_per_seg : A.nseg_a * A.rows_per_seg + (seg - A.nseg_a) * A.rows_b);
-  const int jend = min(jbeg + (seg_long ? A.rows_per_seg : A.rows_b), 3 + A.ny);
+  const int jbeg = rb + 3 + (seg_long ? seg * A.rows_per_seg : A.nseg_a * A.rows_per_seg + (seg - A.nseg_a) * A.rows_b);
+  const int jend = min(jbeg + (seg_long ? A.rows_per_seg : A.rows_b), rb + 3 + A.ny);
   if (jbeg >= jend) return;
   const int w0 = 2 + SOUT * strip;  // padded column of lane 0's cell
   const int ic = w0 + lane - 3;     // interior x index of my cell
@@ -521,7 +529,14 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
   }
 
   const T gamma = A.gamma, g1inv = A.g1inv, g1 = A.g1;
-  const T dtv = T(*A.dt);
+  const T dtv = T(*reinterpret_cast<const double*>(reinterpret_cast<const char*>(A.dt) + (BATCH ? member * A.state_stride : 0)));
+  const uint8_t* const fluid = A.fluid ? A.fluid + (BATCH ? (size_t)member * A.nx * A.ny : 0) : nullptr;
+  // viscous-flux coefficients: kernel parameters (constant-bank operands), or this member's row of the table
+  T vc[10] = {A.vy_n, A.vy_c, A.vy_s, A.vy_t, A.vy_q, A.vx_n, A.vx_c, A.vx_s, A.vx_t, A.vx_q};
+  if (BATCH && VISC) {
+#pragma unroll
+    for (int c = 0; c < 10; ++c) vc[c] = A.vtab[10 * member + c];
+  }
 
   // state carried from one row to the next
   T Ly[4];  // left state (rho,u,v,p) at the face below the next centre row
@@ -665,11 +680,11 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
       if (VISC) {
         const T dn[N] = {pC[2 * CW] - pB[2 * CW]}, dt_[N] = {pC[CW] - pB[CW]}, xt[N] = {cuP + cuC}, xn[N] = {cvP + cvC};
         const T sn[N] = {pB[2 * CW] + pC[2 * CW]}, st[N] = {pB[CW] + pC[CW]}, dT[N] = {pC[4 * CW] - pB[4 * CW]};
-        const T cn[N] = {A.vy_n}, cc[N] = {A.vy_c}, cs[N] = {A.vy_s}, ct[N] = {A.vy_t}, cq[N] = {A.vy_q};
+        const T cn[N] = {vc[0]}, cc[N] = {vc[1]}, cs[N] = {vc[2]}, ct[N] = {vc[3]}, cq[N] = {vc[4]};
         viscous_n<T, N>(dn, dt_, xt, xn, sn, st, dT, cn, cc, cs, ct, cq, f1, f2, f3);
       }
       Gp[0] = f0[0]; Gp[1] = f1[0]; Gp[2] = f2[0]; Gp[3] = f3[0];
-      if (A.fluid && in_x) fl_next = A.fluid[(size_t)(jo + 1 - 3) * A.nx + ic];
+      if (fluid && in_x) fl_next = fluid[(size_t)(jo + 1 - 3 - rb) * A.nx + ic];
     }
 #pragma unroll
     for (int k = 0; k < 4; ++k) Ly[k] = Lnew[k];
@@ -687,7 +702,7 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
     take_row(n, it, A.mode == 0, EpO);
     const int jo = n - 3;  // output row = pB; pC = jc
     const unsigned fl = fl_next;
-    if (n < nlast && A.fluid && in_x) fl_next = A.fluid[(size_t)(jo + 1 - 3) * A.nx + ic];
+    if (n < nlast && fluid && in_x) fl_next = fluid[(size_t)(jo + 1 - 3 - rb) * A.nx + ic];
     float yF[4], yG[4];  // S5': network outputs at my right face and my top face (row jo)
     if (MLP) {
       const size_t o = (size_t)jo * A.pitch + (w0 + lane);
@@ -737,8 +752,8 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
         const T xt[N] = {cuI + cuC, cv0 + cv1}, xn[N] = {cvI + cvC, cu0 + cu1};
         const T sn[N] = {pB[2 * CW] + pC[2 * CW], wc[1] + u1}, st[N] = {pB[CW] + pC[CW], wc[2] + v1};
         const T dT[N] = {pC[4 * CW] - pB[4 * CW], pB[4 * CW + 1] - pB[4 * CW]};
-        const T cn[N] = {A.vy_n, A.vx_n}, cc[N] = {A.vy_c, A.vx_c}, cs[N] = {A.vy_s, A.vx_s}, ct[N] = {A.vy_t, A.vx_t},
-                cq[N] = {A.vy_q, A.vx_q};
+        const T cn[N] = {vc[0], vc[5]}, cc[N] = {vc[1], vc[6]}, cs[N] = {vc[2], vc[7]}, ct[N] = {vc[3], vc[8]},
+                cq[N] = {vc[4], vc[9]};
         viscous_n<T, N>(dn, dt_, xt, xn, sn, st, dT, cn, cc, cs, ct, cq, f1, f2, f3);
       }
     }
@@ -782,7 +797,7 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
     // -------------------------------------------------------------- S8, S9: combine, store, wavespeed
     const bool ok = lane >= 1 && lane <= SOUT && in_x;  // lanes 0 and > SOUT are support cells
     if (A.mode == 1) {
-      const size_t o = (size_t)(jo - 3) * A.nx + ic, pl = (size_t)A.nx * A.ny;
+      const size_t pl = (size_t)A.nx * A.ny, o = (size_t)(jo - 3 - rb) * A.nx + ic + (BATCH ? 4 * pl * member : 0);
       if (ok) {
 #pragma unroll
         for (int k = 0; k < 4; ++k) A.Uout[k * pl + o] = fl ? Lc[k] : T(0);
@@ -831,7 +846,9 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
       const T other = __shfl_xor_sync(0xffffffffu, smax, o);
       smax = (other > smax || other != other) ? other : smax;
     }
-    if (lane == 0) atomic_max_pos(A.smax_bits, (double)smax);
+    if (lane == 0)
+      atomic_max_pos(reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(A.smax_bits) + (BATCH ? member * A.state_stride : 0)),
+                     (double)smax);
   }
 }
 

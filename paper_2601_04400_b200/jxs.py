@@ -26,7 +26,8 @@ EXPORTS = ("jxs_create", "jxs_destroy", "jxs_last_error", "jxs_set_ibm", "jxs_se
            "jxs_set_concurrent_handles", "jxs_set_flux_cnn", "jxs_flux_cnn_inputs",
            "jxs_step_fixed_dt_tangent", "jxs_mse_tangent", "jxs_step_fixed_dt_record", "jxs_adjoint_steps", "jxs_set_gamma",
            "jxs_set_adjoint_checkpointing", "jxs_flux_mlp_gradient", "jxs_adjoint_steps_mse",
-           "jxs_tune", "jxs_set_rows_per_segment", "jxs_set_graph_replay")
+           "jxs_tune", "jxs_set_rows_per_segment", "jxs_set_graph_replay", "jxs_create_batch", "jxs_batch_size",
+           "jxs_get_time_batch")
 
 
 class jxs_bc(C.Structure):
@@ -55,6 +56,10 @@ def lib():
         vp, dp = C.c_void_p, C.POINTER(C.c_double)
         L.jxs_create.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
                                  C.POINTER(jxs_bc), C.c_int, vp, C.POINTER(vp)]
+        L.jxs_create_batch.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, dp, C.c_double,
+                                       C.POINTER(jxs_bc), C.c_int, vp, C.POINTER(vp)]
+        L.jxs_batch_size.argtypes = [vp]
+        L.jxs_get_time_batch.argtypes = [vp, dp, dp]
         L.jxs_destroy.argtypes = [vp]
         L.jxs_destroy.restype = None
         L.jxs_last_error.argtypes = [vp]
@@ -136,6 +141,33 @@ class Solver:
             raise JxsError(rc, "jxs_create")
 
     @classmethod
+    def from_cases(cls, cases, dtype=torch.float64, stream=None):
+        """jxs_create_batch: one handle for len(cases) independent cases of one grid size; fields are [nb, 4, ny, nx]."""
+        if not torch.cuda.is_available():
+            raise JxsError(ECUDA, "no CUDA device: jxs has no CPU fallback")
+        c0, nb = cases[0], len(cases)
+        self = cls.__new__(cls)
+        self.nx, self.ny, self.nb, self.dtype = int(c0["nx"]), int(c0["ny"]), nb, dtype
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        self._bcs = (jxs_bc * nb)(*[make_bc(c["bc"]) for c in cases])
+        mu = (C.c_double * nb)(*[float(c["mu"]) for c in cases])
+        self._h = C.c_void_p()
+        rc = lib().jxs_create_batch(nb, self.nx, self.ny, float(c0["dx"]), float(c0["dy"]), float(c0["gamma"]), mu,
+                                    float(c0["Pr"]), self._bcs, F64 if dtype == torch.float64 else F32,
+                                    C.c_void_p(self.stream.cuda_stream), C.byref(self._h))
+        if rc != OK:
+            raise JxsError(rc, "jxs_create_batch")
+        if cases[0].get("phi") is not None:
+            self.set_ibm(np.stack([c["phi"] for c in cases]))
+        return self
+
+    def time_batch(self):
+        n = getattr(self, "nb", 1)
+        t, dt = (C.c_double * n)(), (C.c_double * n)()
+        self._chk(lib().jxs_get_time_batch(self._h, t, dt))
+        return list(t), list(dt)
+
+    @classmethod
     def from_case(cls, case, dtype=torch.float64, stream=None):
         s = cls(case["nx"], case["ny"], case["dx"], case["dy"], case["gamma"], case["mu"], case["Pr"], case["bc"],
                 dtype=dtype, stream=stream)
@@ -156,12 +188,16 @@ class Solver:
 
     def _dev(self, U):
         assert isinstance(U, torch.Tensor) and U.is_cuda and U.is_contiguous(), "device tensor expected"
-        assert U.dtype == self.dtype and tuple(U.shape) == (4, self.ny, self.nx), (U.dtype, tuple(U.shape))
+        assert U.dtype == self.dtype and tuple(U.shape) == self._shape(), (U.dtype, tuple(U.shape))
         return C.c_void_p(U.data_ptr())
+
+    def _shape(self):
+        nb = getattr(self, "nb", 1)
+        return (4, self.ny, self.nx) if nb == 1 else (nb, 4, self.ny, self.nx)
 
     def _host(self, U):
         assert isinstance(U, torch.Tensor) and not U.is_cuda and U.is_contiguous(), "host tensor expected"
-        assert U.dtype == self.dtype and tuple(U.shape) == (4, self.ny, self.nx)
+        assert U.dtype == self.dtype and tuple(U.shape) == self._shape()
         return C.c_void_p(U.data_ptr())
 
     def set_ibm(self, phi):
@@ -169,7 +205,8 @@ class Solver:
             self._chk(lib().jxs_set_ibm(self._h, None))
             return
         phi = np.ascontiguousarray(phi, dtype=np.float64)
-        assert phi.shape == (self.ny, self.nx)
+        nb = getattr(self, "nb", 1)
+        assert phi.shape == ((self.ny, self.nx) if nb == 1 else (nb, self.ny, self.nx))
         self._chk(lib().jxs_set_ibm(self._h, phi.ctypes.data))
 
     def set_flux_mlp(self, weights, in_scale=None, out_scale=None):
@@ -231,9 +268,11 @@ class Solver:
         return dUdt
 
     def max_wavespeed(self, U):
-        s = C.c_double()
-        self._chk(lib().jxs_max_wavespeed(self._h, self._dev(U), C.byref(s)))
-        return s.value
+        """s_max (a single handle) or the list of every member's s_max (a batch handle)"""
+        nb = getattr(self, "nb", 1)
+        s = (C.c_double * nb)()
+        self._chk(lib().jxs_max_wavespeed(self._h, self._dev(U), s))
+        return s[0] if nb == 1 else list(s)
 
     def step(self, U, cfl, nsteps):
         """In place on the device tensor U."""
