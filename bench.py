@@ -539,14 +539,28 @@ def run_c5(args, rank, world, local_rank, dist, barrier, tdt):
     from paper_2601_04400_b200 import jxs, workloads as wl
     cases = wl.batch_cases(16)
     w, (ins, outs) = wl.mlp_weights(), wl.mlp_scales()
-    streams = [torch.cuda.Stream() for _ in cases]
+    ngroups = args.batch_groups if args.batch_groups > 0 else len(cases)
+    streams = [torch.cuda.Stream() for _ in range(ngroups)]
     solvers, Us = [], []
-    for c, st in zip(cases, streams):
-        s = jxs.Solver.from_case(c, dtype=tdt, stream=st)
-        s.set_flux_mlp(w, ins, outs)
-        s.set_concurrent_handles(len(cases))
-        solvers.append(s)
-        Us.append(torch.tensor(c["U0"], dtype=tdt, device="cuda"))
+    if args.batch_groups > 0:
+        # batched handles (jxs_create_batch): the 16 cases in `batch_groups` handles, one stream each — one launch per
+        # kernel and stage for all members of a handle; two or more handles let the MUFU-bound network kernel of one
+        # overlap the FP64-bound stage kernel of another
+        per = (len(cases) + ngroups - 1) // ngroups
+        for gi, st in enumerate(streams):
+            grp = cases[gi * per:(gi + 1) * per]
+            s = jxs.Solver.from_cases(grp, dtype=tdt, stream=st)
+            s.set_flux_mlp(w, ins, outs)
+            s.set_concurrent_handles(ngroups)
+            solvers.append(s)
+            Us.append(torch.tensor(np.stack([c["U0"] for c in grp]), dtype=tdt, device="cuda"))
+    else:
+        for c, st in zip(cases, streams):
+            s = jxs.Solver.from_case(c, dtype=tdt, stream=st)
+            s.set_flux_mlp(w, ins, outs)
+            s.set_concurrent_handles(len(cases))
+            solvers.append(s)
+            Us.append(torch.tensor(c["U0"], dtype=tdt, device="cuda"))
     ncell = sum(c["nx"] * c["ny"] for c in cases)
     K, W = args.steps, args.warmup
     torch.cuda.synchronize()
@@ -595,7 +609,8 @@ def run_c5(args, rank, world, local_rank, dist, barrier, tdt):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
         "config": {"workload": "batch_16x1024x512_flux_mlp (BASELINE.json configs[4]: 16 independent shock-cylinder runs, "
                                "Mach ~ U[1.5,3], per-face MLP 24-64-64-4 in bf16 fused into the HLLC flux)",
-                   "cfl": 0.4, "rk": "SSP-RK3", "cells": ncell, "handles": len(cases), "streams": len(streams),
+                   "cfl": 0.4, "rk": "SSP-RK3", "cells": ncell, "handles": len(solvers), "streams": len(streams),
+                   "batched": args.batch_groups > 0,
                    "l2": "16 x 3 x 17 MB of state buffers = 800 MB vs 126 MB of L2, no flush needed",
                    "parallelism": "replicas" if world > 1 else "single GPU"},
         "clocks": clocks, "gpu_launches": launches,
@@ -623,6 +638,9 @@ def main():
     ap.add_argument("--euler", action="store_true", help="mu = 0, no IBM (not the headline config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile-kernels", action="store_true", help="c5 only: per-kernel CUDA-event spans")
+    ap.add_argument("--batch-groups", type=int, default=0,
+                    help="c5 only: 0 = 16 single handles on 16 streams; G > 0 = the 16 cases in G batched handles "
+                         "(jxs_create_batch), one stream each")
     ap.add_argument("--rows-per-segment", type=int, default=0,
                     help="fix the stage kernel's row-segment length (jxs_set_rows_per_segment) instead of measuring it at the "
                          "first step call: used for ncu captures, which would otherwise land in the ~40 tuning launches")

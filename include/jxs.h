@@ -244,6 +244,30 @@ int jxs_set_graph_replay(jxs_solver*, int on);
  * its tasks for 1/n of the GPU (longer row segments, fewer warm-up rows) instead of trying to fill it alone.
  * Results do not change.  Default 1.                                                           */
 int jxs_set_concurrent_handles(jxs_solver*, int n);
+/* y-slab sharding of ONE simulation over several GPUs: the pieces a multi-rank
+ * driver composes — paper_2601_04400_b200/sharded.py does, with torch.distributed (NCCL) carrying the rows.  Every
+ * rank runs an ordinary handle on its slab extended by 12 overlap rows per cut side.
+ *   jxs_set_active_rows   rows outside [j_lo, j_hi) are the overlap: L = 0 there, they do not enter s_max, and an
+ *                         immersed body may cross the slab edge behind them (the 8-cell edge rule applies to the
+ *                         domain's real edges only).  Call before jxs_set_ibm (JXS_ESTATE otherwise).
+ *   jxs_shard_begin       U (DEVICE, [4][ny][nx]) -> the handle's buffers; local s_max of the active rows
+ *   jxs_shard_smax        set = 0: *d_smax (DEVICE double) <- the current local s_max; set = 1: the handle's s_max <-
+ *                         *d_smax (after the MAX all-reduce over the ranks)
+ *   jxs_shard_step_begin  dt = cfl min(dx,dy) / s_max (or fixed_dt > 0), clock advanced
+ *   jxs_shard_rows        rows [row0, row0 + nrows) of the INPUT buffer of stage k (0..2) -> rows (DEVICE, contiguous
+ *                         [4][nrows][nx]) (unpack = 0), or back (unpack = 1): the halo pack / unpack kernels
+ *   jxs_shard_stage       ghost fills + [flux MLP] + the fused stage kernel of SSP-RK3 stage k
+ *   jxs_shard_end         the result -> U; synchronises, returns JXS_ENUMERIC like jxs_step
+ * All asynchronous on the handle's stream except jxs_shard_end.  JXS_EINVAL on batch or one-dimensional handles,
+ * JXS_ESTATE out of order, with forward Euler, or with the CNN flux.                                              */
+int jxs_set_active_rows(jxs_solver*, int j_lo, int j_hi);
+int jxs_shard_begin(jxs_solver*, const void* U);
+int jxs_shard_smax(jxs_solver*, double* d_smax, int set);
+int jxs_shard_step_begin(jxs_solver*, double cfl, double fixed_dt);
+int jxs_shard_rows(jxs_solver*, int k, int row0, int nrows, void* rows, int unpack);
+int jxs_shard_stage(jxs_solver*, int k);
+int jxs_shard_end(jxs_solver*, void* U, int nsteps);
+
 /* Time integrator of jxs_step*: JXS_SSPRK3 (default, R5) or JXS_EULER, the forward-Euler update the paper
  * prints (Eq. 10; with jxs_set_artificial_viscosity it is Eq. 10 term by term) = one stage
  * with (a,b) = (0,1).  SURVEY.md section 8(f) rank 2.                                           */

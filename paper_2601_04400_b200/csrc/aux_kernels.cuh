@@ -259,4 +259,25 @@ __global__ void dfma_peak_kernel(double* out, int iters, double a, double b) {
   if (s == 123.456) out[0] = s;  // never true; keeps the loop alive
 }
 
+// y-slab sharding: rows [row0, row0 + nrows) x the interior columns x the 4 fields of a padded
+// buffer <-> a contiguous array [4][nrows][nx] that the caller sends to / receives from the neighbouring rank.
+// row0 is an interior row index (0 = the first interior row).
+template <typename T>
+__global__ void rows_copy_kernel(T* __restrict__ U, T* __restrict__ rows, GridDims g, int row0, int nrows, int unpack) {
+  const long long n = (long long)g.nx * nrows;
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < 4 * n; t += (long long)gridDim.x * blockDim.x) {
+    const int k = (int)(t / n);
+    const long long r = t - k * n;
+    const int j = (int)(r / g.nx), i = (int)(r - (long long)j * g.nx);
+    T* p = U + k * g.plane + (long long)(row0 + j + 3) * g.pitch + i + 3;
+    if (unpack) *p = rows[t];
+    else rows[t] = *p;
+  }
+}
+// s_max as a double <-> its bit pattern in the stepping state (for the MAX all-reduce over the ranks)
+__global__ void smax_copy_kernel(unsigned long long* bits, double* v, int set) {
+  if (set) *bits = (unsigned long long)__double_as_longlong(*v);
+  else *v = __longlong_as_double((long long)*bits);
+}
+
 }  // namespace jxs

@@ -53,6 +53,13 @@ struct jxs_solver {
   double* d_inflow_tab = nullptr;  // [nb][4] conserved inflow states
   void* d_vtab = nullptr;          // [nb][10] viscous coefficients in the handle's dtype
   int mlp_nseg = 1;
+  // y-slab sharding: rows outside [act_lo, act_hi) are inactive (overlap rows refreshed from the neighbouring rank before
+  // every stage: L = 0 there and they do not enter s_max); shard_cur = which s_max slot is current
+  int act_lo = 0, act_hi = 0;
+  bool act_set = false;
+  std::vector<uint8_t> fluid_host;  // the fluid mask as jxs_set_ibm built it (all ones without a body)
+  int shard_cur = 0;
+  bool shard_open = false;
   double dx = 0, dy = 0, gamma = 0, mu = 0, Pr = 0, nu = 0;
   jxs_bc bc{};
   cudaStream_t stream = nullptr;
@@ -1634,13 +1641,24 @@ void jxs_destroy(jxs_solver* s) {
 
 const char* jxs_last_error(const jxs_solver* s) { return s ? s->err.c_str() : "null handle"; }
 
+// the device mask = the body's fluid mask with the inactive rows cleared (single handles only)
+static int apply_active_rows(jxs_solver* s) {
+  std::vector<uint8_t> m = s->fluid_host.empty() ? std::vector<uint8_t>((size_t)s->nx * s->ny, 1) : s->fluid_host;
+  for (int j = 0; j < s->ny; ++j)
+    if (j < s->act_lo || j >= s->act_hi) std::fill(m.begin() + (size_t)j * s->nx, m.begin() + (size_t)(j + 1) * s->nx, 0);
+  if (!s->d_fluid) CU(cudaMalloc(&s->d_fluid, m.size()));
+  CU(cudaMemcpy(s->d_fluid, m.data(), m.size(), cudaMemcpyHostToDevice));
+  return JXS_OK;
+}
+
 int jxs_set_ibm(jxs_solver* s, const double* phi) {
   if (!s) return JXS_EINVAL;
   DEV(s);
   drop_graph(s);
   CU(cudaStreamSynchronize(s->stream));
   free_ibm(s);
-  if (!phi) return JXS_OK;
+  s->fluid_host.clear();
+  if (!phi) return s->act_set ? apply_active_rows(s) : JXS_OK;
   if (s->ny == 1) return fail(s, JXS_EINVAL, "no immersed boundary in one-dimensional problems");
   const int nx = s->nx, ny = s->ny;
   const double dx = s->dx, dy = s->dy;
@@ -1662,11 +1680,20 @@ int jxs_set_ibm(jxs_solver* s, const double* phi) {
   for (int j = 0; j < ny; ++j)
     for (int i = 0; i < nx; ++i) {
       if (fl[(size_t)j * nx + i]) continue;
-      if (i < 8 || j < 8 || i >= nx - 8 || j >= ny - 8)
+      // y-slab sharding: an edge behind inactive rows is a cut through the domain, not its boundary; bodies may cross
+      // it, and ghost cells of inactive rows whose stencils leave the slab are skipped (their rows are refreshed from
+      // the rank that owns them before every stage)
+      const bool inactive = s->act_set && (j < s->act_lo || j >= s->act_hi);
+      const bool cut_lo = s->act_set && s->act_lo > 0, cut_hi = s->act_set && s->act_hi < ny;
+      if (i < 8 || i >= nx - 8 || (j < 8 && !cut_lo) || (j >= ny - 8 && !cut_hi))
         return fail(s, JXS_EINVAL, "IBM body closer than 8 cells to a domain edge");
       bool ghost = false;
       for (int q = 0; q < 16 && !ghost; ++q) ghost = is_fluid(i + off[q][0], j + off[q][1]);
       if (!ghost) continue;
+      if (j == 0 || j == ny - 1) {
+        if (inactive) continue;
+        return fail(s, JXS_EINVAL, "IBM: a ghost cell of an active row lies on a slab edge (overlap too small)");
+      }
       // I3: unit normal from central differences of the sampled level set
       const double px = (phi[(size_t)j * nx + i + 1] - phi[(size_t)j * nx + i - 1]) / (2.0 * dx);
       const double py = (phi[(size_t)(j + 1) * nx + i] - phi[(size_t)(j - 1) * nx + i]) / (2.0 * dy);
@@ -1675,15 +1702,16 @@ int jxs_set_ibm(jxs_solver* s, const double* phi) {
       const double n0 = px / pn, n1 = py / pn;
       // I4: image point, mirrored through the surface along the normal
       const double depth = std::fabs(phi[(size_t)j * nx + i]);
-      double xi = (i + 0.5) * dx + 2.0 * depth * n0;
-      double yi = (j + 0.5) * dy + 2.0 * depth * n1;
+      // kept as its offset from the ghost cell's centre, in cells: x_I = (i + 0.5 + ox) dx.  The donors and weights
+      // then do not depend on where the cell sits in the array (a slab of a sharded run builds the same list)
+      double ox = 2.0 * depth * n0 / dx, oy = 2.0 * depth * n1 / dy;
       // I5: bilinear donors, non-fluid ones dropped, weights renormalised; probe outwards if empty
       int di[4], dj[4];
       double w[4], sum = 0.0;
       for (int attempt = 0; attempt < 9; ++attempt) {
-        const double fx = xi / dx - 0.5, fy = yi / dy - 0.5;
-        const int i0 = (int)std::floor(fx), j0 = (int)std::floor(fy);
-        const double tx = fx - i0, ty = fy - j0;
+        const double flx = std::floor(ox), fly = std::floor(oy);
+        const int i0 = i + (int)flx, j0 = j + (int)fly;
+        const double tx = ox - flx, ty = oy - fly;
         const double bw[4] = {(1 - tx) * (1 - ty), tx * (1 - ty), (1 - tx) * ty, tx * ty};
         sum = 0.0;
         for (int d = 0; d < 4; ++d) {
@@ -1692,9 +1720,12 @@ int jxs_set_ibm(jxs_solver* s, const double* phi) {
           sum += w[d];
         }
         if (sum > 0.0) break;
-        xi += h * n0; yi += h * n1;
+        ox += h * n0 / dx; oy += h * n1 / dy;
       }
-      if (!(sum > 0.0)) return fail(s, JXS_EINVAL, "IBM: ghost cell without a fluid donor");
+      if (!(sum > 0.0)) {
+        if (inactive) continue;
+        return fail(s, JXS_EINVAL, "IBM: ghost cell without a fluid donor");
+      }
       cell.push_back(moff + (j + 3) * s->pitch + i + 3);
       for (int d = 0; d < 4; ++d) {
         const double wd = w[d] / sum;
@@ -1707,8 +1738,13 @@ int jxs_set_ibm(jxs_solver* s, const double* phi) {
   phi = phi_all;
   const std::vector<uint8_t>& fl = fl_all;
   const int ng = (int)cell.size();
+  s->fluid_host = fl;
   CU(cudaMalloc(&s->d_fluid, fl.size()));
   CU(cudaMemcpy(s->d_fluid, fl.data(), fl.size(), cudaMemcpyHostToDevice));
+  if (s->act_set) {
+    const int rc_ = apply_active_rows(s);
+    if (rc_ != JXS_OK) return rc_;
+  }
   if (ng > 0) {
     CU(cudaMalloc(&s->d_cell, sizeof(int) * ng));
     CU(cudaMalloc(&s->d_donor, sizeof(int) * 4 * ng));
@@ -2026,6 +2062,95 @@ int jxs_tune(jxs_solver* s) {
   drop_graph(s);
   return tune_decomposition(s);
 }
+// ---- y-slab sharding: the pieces a multi-rank driver composes (paper_2601_04400_b200/sharded.py)
+int jxs_set_active_rows(jxs_solver* s, int j_lo, int j_hi) {
+  if (!s) return JXS_EINVAL;
+  DEV(s);
+  if (s->nb > 1 || s->ny == 1) return fail(s, JXS_EINVAL, "active rows: single two-dimensional handles only");
+  if (j_lo < 0 || j_hi > s->ny || j_lo >= j_hi) return fail(s, JXS_EINVAL, "bad row range");
+  if (s->n_ghost > 0 || !s->fluid_host.empty()) return fail(s, JXS_ESTATE, "set the active rows before jxs_set_ibm");
+  drop_graph(s);
+  CU(cudaStreamSynchronize(s->stream));
+  s->act_lo = j_lo; s->act_hi = j_hi;
+  s->act_set = !(j_lo == 0 && j_hi == s->ny);
+  if (!s->act_set) { cudaFree(s->d_fluid); s->d_fluid = nullptr; return JXS_OK; }
+  return apply_active_rows(s);
+}
+static int shard_checks(jxs_solver* s) {
+  if (s->nb > 1 || s->ny == 1) return fail(s, JXS_EINVAL, "sharded stepping: single two-dimensional handles only");
+  if (s->scheme != JXS_SSPRK3) return fail(s, JXS_ESTATE, "sharded stepping is SSP-RK3");
+  if (s->cnn_on) return fail(s, JXS_ESTATE, "no CNN flux in sharded stepping (its receptive field needs a deeper exchange)");
+  if (s->pending_steps) return fail(s, JXS_ESTATE, "jxs_wait first");
+  return JXS_OK;
+}
+int jxs_shard_begin(jxs_solver* s, const void* U) {
+  if (!s) return JXS_EINVAL;
+  DEV(s);
+  if (!U) return fail(s, JXS_EINVAL, "U is NULL");
+  int rc = shard_checks(s);
+  if (rc != JXS_OK) return rc;
+  CU(pad(s, U, s->buf[0]));
+  s->shard_cur = 0;
+  CU(wavespeed(s, s->buf[0], &s->d_state->smax_bits[0]));
+  s->shard_open = true;
+  return JXS_OK;
+}
+int jxs_shard_smax(jxs_solver* s, double* d_smax, int set) {
+  if (!s) return JXS_EINVAL;
+  DEV(s);
+  if (!d_smax) return fail(s, JXS_EINVAL, "d_smax is NULL");
+  if (!s->shard_open) return fail(s, JXS_ESTATE, "jxs_shard_begin first");
+  smax_copy_kernel<<<1, 1, 0, s->stream>>>(&s->d_state->smax_bits[s->shard_cur], d_smax, set);
+  s->launches++;
+  CU(cudaGetLastError());
+  return JXS_OK;
+}
+int jxs_shard_step_begin(jxs_solver* s, double cfl, double fixed_dt) {
+  if (!s) return JXS_EINVAL;
+  DEV(s);
+  if (!s->shard_open) return fail(s, JXS_ESTATE, "jxs_shard_begin first");
+  if (!(fixed_dt > 0) && !(cfl > 0)) return fail(s, JXS_EINVAL, "cfl must be > 0");
+  prepare_step_kernel<<<1, 64, 0, s->stream>>>(s->d_state, s->shard_cur, cfl * std::min(s->dx, s->dy), fixed_dt > 0 ? fixed_dt : 0.0, 1);
+  s->launches++;
+  CU(cudaGetLastError());
+  return JXS_OK;
+}
+int jxs_shard_stage(jxs_solver* s, int k) {
+  if (!s) return JXS_EINVAL;
+  DEV(s);
+  if (!s->shard_open) return fail(s, JXS_ESTATE, "jxs_shard_begin first");
+  if (k < 0 || k > 2) return fail(s, JXS_EINVAL, "stage index 0..2");
+  static const double ab[3][2] = {{0.0, 1.0}, {0.75, 0.25}, {1.0 / 3.0, 2.0 / 3.0}};
+  const int in = k, out = (k + 1) % 3;
+  CU(ghost_fill(s, s->buf[in]));
+  CU(flux_mlp(s, s->buf[in]));
+  unsigned long long* next = k == 2 ? &s->d_state->smax_bits[s->shard_cur ^ 1] : nullptr;
+  CU(stage(s, s->buf[in], k == 0 ? nullptr : s->buf[0], s->buf[out], 0, ab[k][0], ab[k][1], next));
+  if (k == 2) s->shard_cur ^= 1;
+  return JXS_OK;
+}
+int jxs_shard_rows(jxs_solver* s, int k, int row0, int nrows, void* rows, int unpack) {
+  if (!s) return JXS_EINVAL;
+  DEV(s);
+  if (!s->shard_open) return fail(s, JXS_ESTATE, "jxs_shard_begin first");
+  if (!rows || k < 0 || k > 2 || nrows < 1 || row0 < 0 || row0 + nrows > s->ny) return fail(s, JXS_EINVAL, "bad rows");
+  const int bs = 256, gs = std::max(1, std::min(s->num_sms * 4, (int)((4LL * s->nx * nrows + bs - 1) / bs)));
+  if (s->dtype == JXS_F64) rows_copy_kernel<double><<<gs, bs, 0, s->stream>>>((double*)s->buf[k], (double*)rows, dims(s), row0, nrows, unpack);
+  else rows_copy_kernel<float><<<gs, bs, 0, s->stream>>>((float*)s->buf[k], (float*)rows, dims(s), row0, nrows, unpack);
+  s->launches++;
+  CU(cudaGetLastError());
+  return JXS_OK;
+}
+int jxs_shard_end(jxs_solver* s, void* U, int nsteps) {
+  if (!s) return JXS_EINVAL;
+  DEV(s);
+  if (!U) return fail(s, JXS_EINVAL, "U is NULL");
+  if (!s->shard_open) return fail(s, JXS_ESTATE, "jxs_shard_begin first");
+  s->shard_open = false;
+  CU(unpad(s, s->buf[0], U));
+  return finish_steps(s, nsteps);
+}
+
 int jxs_set_time_integrator(jxs_solver* s, int scheme) {
   if (!s) return JXS_EINVAL;
   drop_graph(s);

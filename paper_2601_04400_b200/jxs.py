@@ -27,7 +27,8 @@ EXPORTS = ("jxs_create", "jxs_destroy", "jxs_last_error", "jxs_set_ibm", "jxs_se
            "jxs_step_fixed_dt_tangent", "jxs_mse_tangent", "jxs_step_fixed_dt_record", "jxs_adjoint_steps", "jxs_set_gamma",
            "jxs_set_adjoint_checkpointing", "jxs_flux_mlp_gradient", "jxs_adjoint_steps_mse",
            "jxs_tune", "jxs_set_rows_per_segment", "jxs_set_graph_replay", "jxs_create_batch", "jxs_batch_size",
-           "jxs_get_time_batch")
+           "jxs_get_time_batch", "jxs_set_active_rows", "jxs_shard_begin", "jxs_shard_smax", "jxs_shard_step_begin",
+           "jxs_shard_rows", "jxs_shard_stage", "jxs_shard_end")
 
 
 class jxs_bc(C.Structure):
@@ -60,6 +61,13 @@ def lib():
                                        C.POINTER(jxs_bc), C.c_int, vp, C.POINTER(vp)]
         L.jxs_batch_size.argtypes = [vp]
         L.jxs_get_time_batch.argtypes = [vp, dp, dp]
+        L.jxs_set_active_rows.argtypes = [vp, C.c_int, C.c_int]
+        L.jxs_shard_begin.argtypes = [vp, vp]
+        L.jxs_shard_smax.argtypes = [vp, vp, C.c_int]
+        L.jxs_shard_step_begin.argtypes = [vp, C.c_double, C.c_double]
+        L.jxs_shard_rows.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, C.c_int]
+        L.jxs_shard_stage.argtypes = [vp, C.c_int]
+        L.jxs_shard_end.argtypes = [vp, vp, C.c_int]
         L.jxs_destroy.argtypes = [vp]
         L.jxs_destroy.restype = None
         L.jxs_last_error.argtypes = [vp]
@@ -160,6 +168,40 @@ class Solver:
         if cases[0].get("phi") is not None:
             self.set_ibm(np.stack([c["phi"] for c in cases]))
         return self
+
+    # ---- y-slab sharding (driven by sharded.ShardedSolver)
+    def set_active_rows(self, j_lo, j_hi):
+        self._chk(lib().jxs_set_active_rows(self._h, int(j_lo), int(j_hi)))
+
+    def shard_begin(self, U):
+        self._chk(lib().jxs_shard_begin(self._h, self._dev(U)))
+
+    def shard_smax(self, v, set):
+        assert v.is_cuda and v.dtype == torch.float64 and v.numel() == 1
+        self._chk(lib().jxs_shard_smax(self._h, C.c_void_p(v.data_ptr()), int(bool(set))))
+
+    def shard_step_begin(self, cfl, fixed_dt=0.0):
+        self._chk(lib().jxs_shard_step_begin(self._h, float(cfl), float(fixed_dt)))
+
+    def shard_rows(self, k, row0, nrows, rows, unpack):
+        assert rows.is_cuda and rows.is_contiguous() and rows.dtype == self.dtype and tuple(rows.shape) == (4, nrows, self.nx)
+        self._chk(lib().jxs_shard_rows(self._h, int(k), int(row0), int(nrows), C.c_void_p(rows.data_ptr()), int(bool(unpack))))
+
+    def shard_stage(self, k):
+        self._chk(lib().jxs_shard_stage(self._h, int(k)))
+
+    def shard_end(self, U, nsteps):
+        self._chk(lib().jxs_shard_end(self._h, self._dev(U), int(nsteps)))
+
+    @classmethod
+    def from_slab(cls, case, active, dtype=torch.float64, stream=None):
+        """a rank's handle of a sharded run: the active rows are set before the immersed boundary"""
+        s = cls(case["nx"], case["ny"], case["dx"], case["dy"], case["gamma"], case["mu"], case["Pr"], case["bc"],
+                dtype=dtype, stream=stream)
+        s.set_active_rows(*active)
+        if case.get("phi") is not None:
+            s.set_ibm(case["phi"])
+        return s
 
     def time_batch(self):
         n = getattr(self, "nb", 1)
