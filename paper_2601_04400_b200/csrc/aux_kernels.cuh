@@ -4,6 +4,7 @@
 //   S9 stand-alone wavespeed reduction, the per-step device-side dt computation,
 //   and the register-resident DFMA loop that measures the FP64 roofline denominator.
 #pragma once
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -51,7 +52,7 @@ __global__ void fill_benign_kernel(T* U, GridDims g, T e_rest) {
 // network outputs in padded indexing -> the caller's face arrays, scaled by out_scale (Eq. 11):
 // dFx[4][ny][nx+1] (face f of row j lies between cells f-1 and f), dGy[4][ny+1][nx]; components are
 // corrections to the (rho, rho u, rho v, E) fluxes (the y-faces' normal momentum is rho v)
-__global__ void gather_faces_kernel(const float* __restrict__ dF, const float* __restrict__ dG, float* __restrict__ dFx,
+__global__ void gather_faces_kernel(const uint4* __restrict__ dFG, float* __restrict__ dFx,
                                     float* __restrict__ dGy, GridDims g, double s0, double s1, double s2, double s3) {
   const double sc[4] = {s0, s1, s2, s3};
   const long long nfx = (long long)g.ny * (g.nx + 1), nfy = (long long)(g.ny + 1) * g.nx;
@@ -61,14 +62,16 @@ __global__ void gather_faces_kernel(const float* __restrict__ dF, const float* _
       const int k = (int)(t / nfx);
       const long long r = t - k * nfx;
       const int j = (int)(r / (g.nx + 1)), f = (int)(r - (long long)j * (g.nx + 1));
-      dFx[t] = (float)(sc[k] * (double)dF[k * g.plane + (long long)(j + 3) * g.pitch + f + 2]);
+      const __half* h = reinterpret_cast<const __half*>(dFG + (long long)(j + 3) * g.pitch + f + 2);
+      dFx[t] = (float)(sc[k] * (double)__half2float(h[k]));
     } else {
       const long long u = t - 4 * nfx;
       const int k = (int)(u / nfy);  // conserved component; network output index swaps the momenta
       const int ko = k == 1 ? 2 : (k == 2 ? 1 : k);
       const long long r = u - k * nfy;
       const int f = (int)(r / g.nx), i = (int)(r - (long long)f * g.nx);
-      dGy[u] = (float)(sc[ko] * (double)dG[ko * g.plane + (long long)(f + 2) * g.pitch + i + 3]);
+      const __half* h = reinterpret_cast<const __half*>(dFG + (long long)(f + 2) * g.pitch + i + 3);
+      dGy[u] = (float)(sc[ko] * (double)__half2float(h[4 + ko]));
     }
   }
 }

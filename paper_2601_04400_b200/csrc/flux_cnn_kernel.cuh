@@ -145,8 +145,10 @@ struct CnnLayerArgs {
   CnnField in, out;      // out unused by the last layer
   const uint8_t* blob;   // weights + biases of this layer (for this direction: y-faces use transposed taps)
   int rows_per_seg;
-  // last layer only: y[k] -> dst[k * plane + (row + row_off) * pitch + face + col_off], fp32 (the stage kernel's dF / dG)
-  float* dst;
+  // last layer only: y[0..3] -> half `slot` (0: right faces, 1: top faces) of dst[(row + row_off) * pitch + face + col_off],
+  // as fp16 (the stage kernel's dFG)
+  uint4* dst;
+  int slot;
   long long plane;
   int pitch, row_off, col_off;
 };
@@ -291,9 +293,12 @@ __global__ void __launch_bounds__(CNN_TILE) cnn_layer3_kernel(const CnnLayerArgs
       tmem_ld4(tg, y);
       tmem_ld_wait();
       if (live) {
-        float* o = A.dst + (size_t)(row + A.row_off) * A.pitch + p + A.col_off;
+        // my half (x-faces: the first 8 bytes, y-faces: the second) of the cell's eight fp16 network outputs
+        uint2* o = reinterpret_cast<uint2*>(A.dst + (size_t)(row + A.row_off) * A.pitch + p + A.col_off) + A.slot;
+        float t4[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) o[k * A.plane] = tanh_f32(__uint_as_float(y[k]) + bias[k]);
+        for (int k = 0; k < 4; ++k) t4[k] = tanh_f32(__uint_as_float(y[k]) + bias[k]);
+        *o = make_uint2(pack_half2(t4[0], t4[1]), pack_half2(t4[2], t4[3]));
       }
     }
     tmem_zero<NOUT>(tg);  // the group starts over with output row r+2

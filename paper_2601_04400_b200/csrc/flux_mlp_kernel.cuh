@@ -20,8 +20,8 @@
 // registers.  Completion of the MMAs is tracked with
 // tcgen05.commit on an mbarrier.
 // The scaled bf16 primitives of the last 6 rows are kept in a shared-memory ring; a row is converted
-// once.  Output: y (fp32, before out_scale) per face, in padded indexing: dF[k][row][col] = right face,
-// dG[k][row][col] = top face of padded cell (row, col), k = (mass, normal, tangential momentum, energy).
+// once.  Output: y (before out_scale) per face as fp16, one uint4 per padded cell (row, col): {right face: 4, top
+// face: 4}, k = (mass, normal, tangential momentum, energy).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -52,8 +52,7 @@ static_assert(MLP_OFF_BAR % 8 == 0, "mbarrier alignment");
 template <typename T>
 struct MlpArgs {
   const T* U;            // padded [4][ny+6][pitch], ghosts filled
-  float* dF;             // [4][ny+6][pitch] right-face corrections
-  float* dG;             // [4][ny+6][pitch] top-face corrections
+  uint4* dFG;            // [rows][pitch]: per padded cell eight fp16 network outputs {right face: 4, top face: 4}
   const uint8_t* blob;   // MLP_BLOB bytes: canonical bf16 weights + fp32 biases
   long long plane;
   int nx, ny, pitch;
@@ -116,6 +115,11 @@ __host__ __device__ constexpr uint32_t umma_idesc(int M, int N) {
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   uint32_t d;
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+  return d;
+}
+__device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
+  uint32_t d;
+  asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
   return d;
 }
 __device__ __forceinline__ float tanh_f32(float x) {
@@ -310,12 +314,14 @@ __global__ void __launch_bounds__(MLP_TILE, 4) flux_mlp_kernel(const MlpArgs<T> 
       tmem_ld4(tlane + 64, yy);
       tmem_ld_wait();
       if (col <= A.nx + 2) {
-        const size_t o = (size_t)r * A.pitch + col;
+        float fx[4], fy[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-          A.dF[k * A.plane + o] = __uint_as_float(yx[k]) + A.bias[128 + k];
-          A.dG[k * A.plane + o] = __uint_as_float(yy[k]) + A.bias[128 + k];
+          fx[k] = __uint_as_float(yx[k]) + A.bias[128 + k];
+          fy[k] = __uint_as_float(yy[k]) + A.bias[128 + k];
         }
+        A.dFG[(size_t)r * A.pitch + col] = make_uint4(pack_half2(fx[0], fx[1]), pack_half2(fx[2], fx[3]),
+                                                      pack_half2(fy[0], fy[1]), pack_half2(fy[2], fy[3]));
       }
     }
     tc_fence_before();  // the next iteration's MMAs overwrite the columns just read

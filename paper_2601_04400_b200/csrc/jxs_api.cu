@@ -128,12 +128,11 @@ struct jxs_solver {
   // per-face MLP flux correction (S5')
   bool mlp_on = false;
   uint8_t* d_mlp_blob = nullptr;
-  float* d_dF = nullptr;   // [4][ny+6][pitch] network outputs at right faces
-  float* d_dG = nullptr;   // same at top faces
+  uint4* d_dFG = nullptr;  // [rows][pitch]: per padded cell eight fp16 network outputs {right face: 4, top face: 4}
   double in_scale[4] = {1, 1, 1, 1}, out_scale[4] = {1, 1, 1, 1};
   float mlp_bias[132] = {0};
   // the paper's 2D CNN flux (flux_cnn_kernel.cuh): per direction (x, y) the input field, the two hidden fields and
-  // the three layers' weight blobs; shares d_dF / d_dG / out_scale with the MLP path (one of the two at a time)
+  // the three layers' weight blobs; shares d_dFG / out_scale with the MLP path (one of the two at a time)
   bool cnn_on = false;
   CnnField cnn_X[2] = {}, cnn_H1[2] = {}, cnn_H2[2] = {};
   uint8_t* d_cnn_blob3[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};  // for cnn_layer3_kernel
@@ -346,8 +345,7 @@ cudaError_t launch_stage(jxs_solver* s, const void* Uin, const void* U0, void* U
     A.vx_n = (T)(4.0 / 3.0 * mu * dxi); A.vx_c = (T)(2.0 / 3.0 * mu * 0.25 * dyi); A.vx_s = (T)(mu * dxi);
     A.vx_t = (T)(mu * 0.25 * dyi); A.vx_q = (T)(kap * dxi);
   }
-  A.dF = (s->mlp_on || s->cnn_on) ? s->d_dF : nullptr;
-  A.dG = (s->mlp_on || s->cnn_on) ? s->d_dG : nullptr;
+  A.dFG = (s->mlp_on || s->cnn_on) ? s->d_dFG : nullptr;
   for (int k = 0; k < 4; ++k) A.oscale[k] = (T)s->out_scale[k];
   A.dF1d = s->mlp1d_on ? s->d_dF1d : nullptr;
   const bool visc = s->mu > 0, artv = s->nu > 0;
@@ -397,11 +395,11 @@ cudaError_t ghost_fill(jxs_solver* s, void* U) {
   return cudaGetLastError();
 }
 
-// S5': network outputs of every face of the padded, ghost-filled state U -> d_dF, d_dG
+// S5': network outputs of every face of the padded, ghost-filled state U -> d_dFG
 template <typename T>
 cudaError_t launch_flux_mlp(jxs_solver* s, const void* U) {
   MlpArgs<T> A;
-  A.U = (const T*)U; A.dF = s->d_dF; A.dG = s->d_dG; A.blob = s->d_mlp_blob;
+  A.U = (const T*)U; A.dFG = s->d_dFG; A.blob = s->d_mlp_blob;
   A.plane = s->plane; A.nx = s->nx; A.ny = s->ny; A.pitch = s->pitch;
   A.nstrips = s->mlp_strips; A.rows_per_seg = s->mlp_rows_per_seg; A.nseg = s->mlp_nseg;
   A.g1 = (T)(s->gamma - 1.0);
@@ -421,7 +419,7 @@ cudaError_t launch_flux_mlp(jxs_solver* s, const void* U) {
   s->launches++;
   return cudaGetLastError();
 }
-// the CNN flux of the padded, ghost-filled state U -> d_dF, d_dG: reconstruction pass, then three convolution
+// the CNN flux of the padded, ghost-filled state U -> d_dFG: reconstruction pass, then three convolution
 // layers per direction
 template <int KC, int CIN8, int NOUT, bool LAST>
 cudaError_t launch_cnn_layer3(jxs_solver* s, const CnnLayerArgs& A0) {
@@ -461,7 +459,7 @@ cudaError_t launch_flux_cnn(jxs_solver* s, const void* U) {
     e = launch_cnn_layer3<2, 4, 16, false>(s, A);
     if (e != cudaSuccess) break;
     A.in = s->cnn_H2[d]; A.blob = s->d_cnn_blob3[d][2];
-    A.dst = d == 0 ? s->d_dF : s->d_dG;
+    A.dst = s->d_dFG; A.slot = d;
     A.row_off = d == 0 ? 3 : 2; A.col_off = d == 0 ? 2 : 3;
     e = launch_cnn_layer3<1, 2, 16, true>(s, A);
   }
@@ -1629,7 +1627,7 @@ void jxs_destroy(jxs_solver* s) {
   cudaFree(s->d_state);
   cudaFree(s->d_inflow_tab); cudaFree(s->d_vtab);
   free_ibm(s);
-  cudaFree(s->d_mlp_blob); cudaFree(s->d_dF); cudaFree(s->d_dG);
+  cudaFree(s->d_mlp_blob); cudaFree(s->d_dFG);
   for (int d = 0; d < 2; ++d) {
     cudaFree(s->cnn_X[d].data); cudaFree(s->cnn_H1[d].data); cudaFree(s->cnn_H2[d].data);
     for (int l = 0; l < 3; ++l) cudaFree(s->d_cnn_blob3[d][l]);
@@ -1831,10 +1829,9 @@ int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[
   float* bias = reinterpret_cast<float*>(blob.data() + MLP_OFF_BIAS);
   std::memcpy(bias, b1, 64 * 4); std::memcpy(bias + 64, b2, 64 * 4); std::memcpy(bias + 128, b3, 4 * 4);
   std::memcpy(s->mlp_bias, bias, sizeof(s->mlp_bias));
-  const size_t fbytes = (size_t)4 * s->plane * sizeof(float);
+  const size_t fbytes = (size_t)s->plane * sizeof(uint4);
   if (!s->d_mlp_blob) CU(cudaMalloc(&s->d_mlp_blob, MLP_BLOB));
-  if (!s->d_dF) { CU(cudaMalloc(&s->d_dF, fbytes)); CU(cudaMemset(s->d_dF, 0, fbytes)); }
-  if (!s->d_dG) { CU(cudaMalloc(&s->d_dG, fbytes)); CU(cudaMemset(s->d_dG, 0, fbytes)); }
+  if (!s->d_dFG) { CU(cudaMalloc(&s->d_dFG, fbytes)); CU(cudaMemset(s->d_dFG, 0, fbytes)); }
   CU(cudaMemcpy(s->d_mlp_blob, blob.data(), MLP_BLOB, cudaMemcpyHostToDevice));
   for (int k = 0; k < 4; ++k) { s->in_scale[k] = in_scale[k]; s->out_scale[k] = out_scale[k]; }
   // strips of 128 faces x row segments: fill 4 resident CTAs per SM, 5 warm-up rows per segment
@@ -1886,9 +1883,8 @@ int jxs_set_flux_cnn(jxs_solver* s, const float* weights, const double in_scale[
       f[q]->na = na; f[q]->nb = nb; f[q]->nbp = nbp; f[q]->C = chunks[q];
     }
   }
-  const size_t fbytes = (size_t)4 * s->plane * sizeof(float);
-  if (!s->d_dF) { CU(cudaMalloc(&s->d_dF, fbytes)); CU(cudaMemset(s->d_dF, 0, fbytes)); }
-  if (!s->d_dG) { CU(cudaMalloc(&s->d_dG, fbytes)); CU(cudaMemset(s->d_dG, 0, fbytes)); }
+  const size_t fbytes = (size_t)s->plane * sizeof(uint4);
+  if (!s->d_dFG) { CU(cudaMalloc(&s->d_dFG, fbytes)); CU(cudaMemset(s->d_dFG, 0, fbytes)); }
   for (int k = 0; k < 4; ++k) { s->cnn_in_scale[k] = in_scale[k]; s->out_scale[k] = out_scale[k]; }
   s->cnn_on = true;
   return JXS_OK;
@@ -2217,7 +2213,7 @@ int jxs_flux_correction(jxs_solver* s, const void* U, float* dFx, float* dGy) {
   CU(ghost_fill(s, s->buf[0]));
   CU(flux_mlp(s, s->buf[0]));
   const int bs = 256, gs = s->num_sms * 8;
-  gather_faces_kernel<<<gs, bs, 0, s->stream>>>(s->d_dF, s->d_dG, dFx, dGy, dims(s), s->out_scale[0], s->out_scale[1],
+  gather_faces_kernel<<<gs, bs, 0, s->stream>>>(s->d_dFG, dFx, dGy, dims(s), s->out_scale[0], s->out_scale[1],
                                                  s->out_scale[2], s->out_scale[3]);
   s->launches++;
   CU(cudaGetLastError());

@@ -21,6 +21,7 @@
 // Neither reconstructed states nor fluxes ever leave the SM.
 #pragma once
 #include <cuda.h>
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -67,10 +68,10 @@ struct StageArgs {
   // tangential part), heat flux; n = the face's normal direction
   T vy_n, vy_c, vy_s, vy_t, vy_q;  // y-faces: 4/3 mu/dy, (2/3) mu/(4 dx), mu/dy, mu/(4 dx), kappa/dy
   T vx_n, vx_c, vx_s, vx_t, vx_q;  // x-faces: 4/3 mu/dx, (2/3) mu/(4 dy), mu/dx, mu/(4 dy), kappa/dx
-  // S5' (optional): network outputs y per face from flux_mlp_kernel, padded indexing [4][ny+6][pitch]:
-  // dF = right face, dG = top face of the cell; k = (mass, normal, tangential momentum, energy) (R14)
-  const float* dF;
-  const float* dG;
+  // S5' (optional): network outputs y per face from flux_mlp_kernel / the CNN's last layer, one uint4 per padded cell
+  // [rows][pitch]: eight fp16 values {right face: 4, top face: 4}, k = (mass, normal, tangential momentum, energy) (R14).
+  // 16 bytes per cell-stage instead of the 32 of fp32 planes; fp16 keeps 11 bits (5e-4) of a correction held to 1e-2.
+  const uint4* dFG;
   T oscale[4];
   // one-dimensional problems (stage1d_kernel.cuh): the per-face MLP's flux correction from mlp1d_kernel.cuh, already
   // scaled, indexed like U (right face of the cell); nullptr = none
@@ -411,6 +412,12 @@ __device__ __forceinline__ void hllc_n(const T (&rL)[N], const T (&unL)[N], cons
   JXS_V f3[k] = fma_(sc[k], dE[k], f3[k]);
 }
 
+// four fp16 values in two 32-bit words -> floats
+__device__ __forceinline__ void unpack_half4(uint32_t lo, uint32_t hi, float (&y)[4]) {
+  const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&lo)), b = __half22float2(*reinterpret_cast<const __half2*>(&hi));
+  y[0] = a.x; y[1] = a.y; y[2] = b.x; y[3] = b.y;
+}
+
 template <typename T>
 __device__ __forceinline__ T shfl_down1(T v) { return __shfl_down_sync(0xffffffffu, v, 1); }
 template <typename T>
@@ -549,6 +556,7 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
   T Ep0[4], Ep1[4];
   T smax = T(0);
   unsigned fl_next = 1;  // fluid flag of my cell in the next output row, fetched one iteration ahead
+  uint4 y_next = make_uint4(0, 0, 0, 0);  // S5': the network outputs of my cell in the next output row
 
   // Ring rows as loop-carried per-lane pointers (to my column q), rotated once per iteration: the row
   // accesses below become LDS with immediate offsets, no slot arithmetic.  pN = slot written next.
@@ -671,11 +679,14 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
       const T rR[N] = {Ry[0]}, unR[N] = {Ry[2]}, utR[N] = {Ry[1]}, pR[N] = {Ry[3]};
       hllc_n<T, N>(rL, unL, utL, pL, rR, unR, utR, pR, gamma, g1inv, f0, f1, f2, f3);
       if (MLP) {  // Eq. 11
-        const size_t o = (size_t)jo * A.pitch + (w0 + lane);
-        f0[0] = fma_(A.oscale[0], T(__ldg(A.dG + o)), f0[0]);
-        f1[0] = fma_(A.oscale[1], T(__ldg(A.dG + A.plane + o)), f1[0]);
-        f2[0] = fma_(A.oscale[2], T(__ldg(A.dG + 2 * A.plane + o)), f2[0]);
-        f3[0] = fma_(A.oscale[3], T(__ldg(A.dG + 3 * A.plane + o)), f3[0]);
+        const uint4 y8 = __ldg(A.dFG + (size_t)jo * A.pitch + (w0 + lane));
+        float yG[4];
+        unpack_half4(y8.z, y8.w, yG);
+        f0[0] = fma_(A.oscale[0], T(yG[0]), f0[0]);
+        f1[0] = fma_(A.oscale[1], T(yG[1]), f1[0]);
+        f2[0] = fma_(A.oscale[2], T(yG[2]), f2[0]);
+        f3[0] = fma_(A.oscale[3], T(yG[3]), f3[0]);
+        y_next = __ldg(A.dFG + (size_t)(jo + 1) * A.pitch + (w0 + lane));
       }
       if (VISC) {
         const T dn[N] = {pC[2 * CW] - pB[2 * CW]}, dt_[N] = {pC[CW] - pB[CW]}, xt[N] = {cuP + cuC}, xn[N] = {cvP + cvC};
@@ -703,12 +714,10 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
     const int jo = n - 3;  // output row = pB; pC = jc
     const unsigned fl = fl_next;
     if (n < nlast && fluid && in_x) fl_next = fluid[(size_t)(jo + 1 - 3 - rb) * A.nx + ic];
-    float yF[4], yG[4];  // S5': network outputs at my right face and my top face (row jo)
-    if (MLP) {
-      const size_t o = (size_t)jo * A.pitch + (w0 + lane);
-#pragma unroll
-      for (int k = 0; k < 4; ++k) { yF[k] = __ldg(A.dF + k * A.plane + o); yG[k] = __ldg(A.dG + k * A.plane + o); }
-    }
+    // S5': network outputs at my right face and my top face (row jo): one 16-byte load per cell, fetched a whole row
+    // ahead (like the fluid flag) so that its latency never meets the use
+    const uint4 y8 = y_next;
+    if (MLP && n < nlast) y_next = __ldg(A.dFG + (size_t)(jo + 1) * A.pitch + (w0 + lane));
 
     // -------------------------------------------------------------- S4 along y (centre jc) and along x (row jo)
     T Ry[4], Lnew[4], cuC = T(0), cvC = T(0);
@@ -736,6 +745,9 @@ stage_kernel(const StageArgs<T> A, const __grid_constant__ CUtensorMap tm_row, c
               utR[N] = {Ry[1], shfl_down1(Rm[2])}, pR[N] = {Ry[3], shfl_down1(Rm[3])};
       hllc_n<T, N>(rL, unL, utL, pL, rR, unR, utR, pR, gamma, g1inv, f0, f1, f2, f3);
       if (MLP) {  // Eq. 11
+        float yF[4], yG[4];
+        unpack_half4(y8.x, y8.y, yF);
+        unpack_half4(y8.z, y8.w, yG);
         f0[0] = fma_(A.oscale[0], T(yG[0]), f0[0]); f0[1] = fma_(A.oscale[0], T(yF[0]), f0[1]);
         f1[0] = fma_(A.oscale[1], T(yG[1]), f1[0]); f1[1] = fma_(A.oscale[1], T(yF[1]), f1[1]);
         f2[0] = fma_(A.oscale[2], T(yG[2]), f2[0]); f2[1] = fma_(A.oscale[2], T(yF[2]), f2[1]);

@@ -152,9 +152,11 @@ def test_adjoint_rejects_what_it_does_not_do():
     s32 = jxs().Solver.from_case(case, dtype=torch.float32)
     with pytest.raises(E):
         s32.step_fixed_dt_record(dev(case["U0"], torch.float32), 1e-3, 1)
-    v = wl.vortex(32)
+    v = wl.vortex(32)                             # two-dimensional handles: tests/test_gpu_deriv2d.py; not with a network
+    sv = jxs().Solver.from_case(v)
+    sv.set_flux_mlp(wl.mlp_weights(), *wl.mlp_scales())
     with pytest.raises(E):
-        jxs().Solver.from_case(v).step_fixed_dt_record(dev(v["U0"]), 1e-3, 1)
+        sv.step_fixed_dt_record(dev(v["U0"]), 1e-3, 1)
     # a zero adjoint stays zero
     s3 = jxs().Solver.from_case(case)
     s3.step_fixed_dt_record(dev(case["U0"]), 1e-3, 2)

@@ -214,7 +214,8 @@ def test_tangent_rejects_what_it_does_not_do():
     s32 = jxs().Solver.from_case(case, dtype=torch.float32)
     with pytest.raises(E):
         s32.step_fixed_dt_tangent(dev(case["U0"], torch.float32), dev(case["U0"], torch.float32), 1.0, 1e-3, 1)
-    c2 = wl.vortex(32)
+    c2 = wl.vortex(32)                            # two-dimensional handles: tests/test_gpu_deriv2d.py; not with a network
     s2 = jxs().Solver.from_case(c2)
+    s2.set_flux_mlp(wl.mlp_weights(), *wl.mlp_scales())
     with pytest.raises(E):
         s2.step_fixed_dt_tangent(dev(c2["U0"]), dev(c2["U0"]), 1.0, 1e-3, 1)
