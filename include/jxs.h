@@ -147,10 +147,12 @@ int jxs_max_wavespeed(jxs_solver*, const void* U, double* smax_host);
 int jxs_step(jxs_solver*, void* U, double cfl, int nsteps);
 /* Same with a fixed time step.                                                              */
 int jxs_step_fixed_dt(jxs_solver*, void* U, double dt, int nsteps);
-/* Tangent (forward-mode derivative) of jxs_step_fixed_dt for one-dimensional problems: PAPER.md Eq. 15-16 (the step
+/* Tangent (forward-mode derivative) of jxs_step_fixed_dt, in one and in two dimensions: PAPER.md Eq. 15-16 (the step
  * U^{n+k} = S(U^{n+k-1}, theta) and the chain of its Jacobians) applied to ONE direction of perturbation, for the
  * paper's inference of the specific-heat ratio from Sod data (L149, Fig. 3b; R21).
- *   U, Udot   DEVICE pointers, [4][1][nx] doubles, read and overwritten: the state and a direction of perturbation
+ * In 2D (ny > 1; Fig. 5d-f; R25) the boundary conditions and the immersed-boundary fill are
+ * differentiated with the scheme (deriv2d_kernels.cuh); the 2D networks are not (JXS_ESTATE).
+ *   U, Udot   DEVICE pointers, [4][ny][nx] doubles, read and overwritten: the state and a direction of perturbation
  *             of it (owned by the caller; Udot = 0 differentiates with respect to gamma at fixed conserved state,
  *             Udot[3] = -p/(gamma-1)^2 at fixed primitives)
  *   gamma_dot perturbation of gamma along the same direction
@@ -159,7 +161,7 @@ int jxs_step_fixed_dt(jxs_solver*, void* U, double dt, int nsteps);
  * On return U = S^nsteps(U; gamma) (the same arithmetic as the tangent's value part, equal to jxs_step_fixed_dt to
  * round-off) and Udot = dS^nsteps/dU . Udot + dS^nsteps/dgamma . gamma_dot.  Branches of the scheme (min / max of wave
  * speeds, sign of the contact speed, positivity guard) carry the derivative of the branch taken.
- * Errors: JXS_EINVAL for NULL pointers, dt <= 0, nsteps < 0, a non-finite gamma_dot, an fp32 handle or ny != 1;
+ * Errors: JXS_EINVAL for NULL pointers, dt <= 0, nsteps < 0, a non-finite gamma_dot, an fp32 or a batch handle;
  * JXS_ESTATE with a network set or with steps pending (jxs_wait);
  * JXS_ENOMEM / JXS_ECUDA from the first call's allocation of the tangent buffers.  Synchronises the stream.      */
 int jxs_step_fixed_dt_tangent(jxs_solver*, void* U, void* Udot, double gamma_dot, double dt, int nsteps);
@@ -171,19 +173,21 @@ int jxs_step_fixed_dt_tangent(jxs_solver*, void* U, void* Udot, double gamma_dot
  * reproducible.  Errors: JXS_EINVAL for NULL pointers or an fp32 handle.  Synchronises the stream.               */
 int jxs_mse_tangent(jxs_solver*, const void* U, const void* Udot, const void* Utarget, double* loss, double* dloss);
 
-/* Reverse mode (adjoint) of jxs_step_fixed_dt for one-dimensional problems (Euler or Navier-Stokes, nu-term): Eq. 15-16 —
+/* Reverse mode (adjoint) of jxs_step_fixed_dt, in one and in two dimensions (Euler or Navier-Stokes, nu-term; in 2D with the
+ * immersed boundary and the frame's corners, R25): Eq. 15-16 —
  * "backpropagation through the full sequence of unrolled solver steps" (R21, R24).
  * Two calls: the forward sweep that records the trajectory, then the reverse sweep.
  *
- * jxs_step_fixed_dt_record: as jxs_step_fixed_dt (U: DEVICE pointer, [4][1][nx] doubles, advanced in place by nsteps
+ * jxs_step_fixed_dt_record: as jxs_step_fixed_dt (U: DEVICE pointer, [4][ny][nx] doubles, advanced in place by nsteps
  * >= 1 steps of size dt > 0 of the handle's time integrator), keeping the stage states of every step (3 for SSP-RK3, 1
- * for forward Euler) in device memory owned by the handle (32 nx bytes per state).
- * jxs_adjoint_steps: Ubar (DEVICE pointer, [4][1][nx] doubles) holds on entry the adjoint of the final state, e.g.
+ * for forward Euler) in device memory owned by the handle (32 nx bytes per state in 1D, a padded buffer of
+ * 32 (nx+6..) (ny+6) bytes in 2D).
+ * jxs_adjoint_steps: Ubar (DEVICE pointer, [4][ny][nx] doubles) holds on entry the adjoint of the final state, e.g.
  * dL/dU^{n+m} of the loss of Eq. 14; on return the adjoint of the initial state, (dU^{n+m}/dU^n)^T Ubar.
  * *gamma_bar (HOST) = <dU^{n+m}/dgamma at fixed initial conserved state, Ubar>.  For every direction (Udot, gamma_dot),
  * with Udot_end from jxs_step_fixed_dt_tangent: <Ubar on entry, Udot_end> = <Ubar on return, Udot> + gamma_bar gamma_dot.
  * May be called repeatedly on one recording.  Branches of the scheme carry the derivative of the branch taken.
- * Errors: JXS_EINVAL for NULL pointers, dt <= 0, nsteps < 1, an fp32 handle or ny != 1; JXS_ESTATE with steps
+ * Errors: JXS_EINVAL for NULL pointers, dt <= 0, nsteps < 1, an fp32 or a batch handle; JXS_ESTATE with a 2D network, steps
  * pending, or (adjoint) nothing recorded (changing gamma, nu or the network drops a recording); JXS_ENOMEM when the
  * trajectory does not fit.  With the per-face MLP set on the handle (see jxs_flux_mlp_gradient below) both calls include it.  The recording stays (and its memory is reused by the next record call) until jxs_destroy.  Both
  * synchronise the stream.                                                                                         */
@@ -191,9 +195,9 @@ int jxs_step_fixed_dt_record(jxs_solver*, void* U, double dt, int nsteps);
 int jxs_adjoint_steps(jxs_solver*, void* Ubar, double* gamma_bar);
 /* The reverse sweep driven by the loss of PAPER.md Eq. 14 itself, the mean over the m recorded steps of the mean
  * squared error against one target per step (R22):  L = (1/m) sum_{s=1..m} mean((U^{n+s} - targets[s-1])^2).
- *   targets  DEVICE, [m][4][1][nx] doubles, m = the nsteps of the last jxs_step_fixed_dt_record: the downsampled
+ *   targets  DEVICE, [m][4][ny][nx] doubles, m = the nsteps of the last jxs_step_fixed_dt_record: the downsampled
  *            reference states U~^{n+s} (read only)
- *   Ubar     DEVICE, [4][1][nx] doubles, OUT: dL/dU^n
+ *   Ubar     DEVICE, [4][ny][nx] doubles, OUT: dL/dU^n
  *   loss, gamma_bar  HOST, OUT: L and dL/dgamma at fixed U^n; the weights' gradient dL/dtheta is read with
  *            jxs_flux_mlp_gradient
  * Every intermediate loss L_s enters the sweep where its state does (Eq. 16 summed over s), so the cost is that of
