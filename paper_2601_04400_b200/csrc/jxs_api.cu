@@ -414,7 +414,7 @@ cudaError_t launch_flux_mlp(jxs_solver* s, const void* U) {
     e1 = s->mlp_events[s->mlp_events_used++];
     cudaEventRecord(e0, s->stream);
   }
-  kern<<<s->mlp_grid, MLP_TILE, MLP_SMEM, s->stream>>>(A);
+  kern<<<s->mlp_grid, MLP_THREADS, MLP_SMEM, s->stream>>>(A);
   if (e1) cudaEventRecord(e1, s->stream);
   s->launches++;
   return cudaGetLastError();
@@ -1834,12 +1834,19 @@ int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[
   if (!s->d_dFG) { CU(cudaMalloc(&s->d_dFG, fbytes)); CU(cudaMemset(s->d_dFG, 0, fbytes)); }
   CU(cudaMemcpy(s->d_mlp_blob, blob.data(), MLP_BLOB, cudaMemcpyHostToDevice));
   for (int k = 0; k < 4; ++k) { s->in_scale[k] = in_scale[k]; s->out_scale[k] = out_scale[k]; }
-  // strips of 128 faces x row segments: fill 4 resident CTAs per SM, 5 warm-up rows per segment
+  // strips of 128 cells x row segments: 2 resident CTAs per SM, 5 warm-up rows per segment; the segment count
+  // that minimises (waves of CTAs) x (rows a CTA streams)
   s->mlp_strips = (s->nx + 1 + MLP_TILE - 1) / MLP_TILE;
   const int nrows = s->ny + 1;
-  const long long slots = (long long)s->num_sms * 4;
-  int segs = (int)std::max<long long>(1, slots / ((long long)s->mlp_strips * s->nb));
-  int rps = std::max((nrows + segs - 1) / segs, std::min(nrows, 16));
+  const long long slots = (long long)s->num_sms * 2, columns = (long long)s->mlp_strips * s->nb;
+  long long best_cost = -1;
+  int rps = nrows;
+  for (int nseg = 1; nseg <= std::max(1, nrows / 8); ++nseg) {
+    const int r = (nrows + nseg - 1) / nseg;
+    const long long waves = (columns * ((nrows + r - 1) / r) + slots - 1) / slots;
+    const long long cost = waves * (r + 5);
+    if (best_cost < 0 || cost < best_cost) { best_cost = cost; rps = r; }
+  }
   s->mlp_rows_per_seg = rps;
   s->mlp_nseg = (nrows + rps - 1) / rps;
   s->mlp_grid = s->mlp_strips * s->mlp_nseg * s->nb;
