@@ -3,28 +3,33 @@
 //
 //   x (24 stencil primitives / in_scale, bf16) -> tanh(W1 x + b1) -> tanh(W2 h1 + b2) -> W3 h2 + b3
 //
-// One CTA = 8 warps = two warpgroups marches a strip of 128 cells upwards, one row per iteration.  Thread lt
-// (0..127) of warpgroup 0 owns the RIGHT face of the cell in column c0+lt (x-face i+1/2: cells i-2..i+3 of the
-// row), thread lt of warpgroup 1 its TOP face (y-face j+1/2: rows j-2..j+3 of the column, normal velocity
-// first).  The 128 faces of a warpgroup are the M = 128 rows of its own chain of tcgen05.mma tiles:
+// One CTA per SM = 11 warps marches a strip of 128 cells upwards:
+//   warps 0-3  (warpgroup 0)  the RIGHT faces of the cells (x-face i+1/2: cells i-2..i+3 of the row); thread lt owns
+//                             the face of the cell in column c0+lt
+//   warps 4-7  (warpgroup 1)  their TOP faces (y-face j+1/2: rows j-2..j+3 of the column, normal velocity first)
+//   warp 8, 9                 one lane each issues the tcgen05.mma of warpgroup 0 / 1
+//   warp 10                   the producer: conserved rows from HBM -> scaled bf16 primitives in a shared-memory ring
+// The 128 faces of a warpgroup and row are the M = 128 rows of a chain of tcgen05.mma tiles:
 //   layer 1  D[128 x 64] = A1[128 x 32] W1^T     (K = 24 padded to 32, 2 MMAs of K = 16)
 //   layer 2  D[128 x 64] = A2[128 x 64] W2^T     (4 MMAs)
 //   layer 3  D[128 x 16] = A3[128 x 64] W3^T     (N = 4 padded to 16, 4 MMAs)
 // The A operands live in TENSOR MEMORY (tcgen05.mma with [a_tmem]: lane m = row m, 32-bit column c = the bf16
 // pair k = 2c, 2c+1): every thread writes the row of its own face with tcgen05.st and the tensor core reads
 // it from there, so an MMA fetches only its 0.5-2 KB weight tile from shared memory and runs at the
-// 128 N / 256-cycle floor (32 cycles for N = 64) instead of the ~100 cycles that the 4 KB A tile in shared
-// memory cost (profiles/r02_flux_mlp.md).  Per warpgroup 96 TMEM columns: X = [0, 32) the A operand of the
-// current layer, Y = [32, 96) its accumulator; TMEM lane m = face m = thread m, so tcgen05.ld (32x32b)
-// hands every thread the pre-activations of its own face; bias, tanh (tanh.approx.f32, then one rounding to
-// bf16 — the rounding points of the oracle's emulating mode; the packed tanh.approx.bf16x2 was measured: SASS
-// splits it into two MUFU operations, so it is no faster, and its extra input rounding costs 1e-2 of
-// accuracy) and the tcgen05.st of the next A operand follow in registers.  The two warpgroups run their
-// chains independently (a named barrier and an mbarrier each) and meet once per row, when the new row of
-// primitives enters the ring; two CTAs per SM (all 512 TMEM columns) = four independent chains that keep the
-// SFU (tanh: the binding unit, 128 per face) busy while one of them waits for its MMAs.
-// The scaled bf16 primitives of the last 7 rows are kept in a shared-memory ring; a row is converted
-// once.  Output: y (before out_scale) per face as fp16, one uint4 per padded cell (row, col): {right face: 4, top
+// 128 N / 256-cycle floor (32 cycles for N = 64) instead of the ~100 cycles that a 4 KB A tile in shared
+// memory cost (profiles/r02_flux_mlp.md).  A tile slot is 96 TMEM columns: X = [0, 32) the A operand of the
+// current layer, Y = [32, 96) its accumulator; TMEM lane m = face m = thread m, so tcgen05.ld (32x32b) hands
+// every thread the pre-activations of its own face; bias, tanh (tanh.approx.f32, then one rounding to bf16 —
+// the rounding points of the oracle's emulating mode; the packed tanh.approx.bf16x2 was measured: SASS splits
+// it into two MUFU operations, so it is no faster, and its extra input rounding costs 1e-2 of accuracy) and
+// the tcgen05.st of the next A operand follow in registers.
+// What binds is the SFU (128 tanh per face at 16 per clock and SM), so the schedule exists to keep MUFU.TANH
+// issuing: each warpgroup works on TWO rows at once (two tile slots, 4 x 96 of the 512 TMEM columns per SM) and
+// alternates between them, so the MMAs of one slot (and their completion latency) run under the tanh phase of
+// the other.  Hand-over is by mbarriers only: a_full[g][s] (128 arrivals: the A operand of slot s is in TMEM)
+// -> the MMA lane issues the layer and commits to d_full[g][s] -> the threads read the accumulator.  The ring
+// has its own full / empty barriers per row slot; nothing in the loop is a CTA-wide barrier.
+// Output: y (before out_scale) per face as fp16, one uint4 per padded cell (row, col): {right face: 4, top
 // face: 4}, k = (mass, normal, tangential momentum, energy).
 #pragma once
 #include <cuda_runtime.h>
@@ -33,10 +38,10 @@
 namespace jxs {
 
 constexpr int MLP_TILE = 128;               // faces per MMA tile = threads per warpgroup
-constexpr int MLP_THREADS = 2 * MLP_TILE;   // warpgroup 0: x-faces, warpgroup 1: y-faces
-constexpr int MLP_RING = 7;                 // rows of bf16 primitives kept (6 read + the one being written)
+constexpr int MLP_THREADS = 2 * MLP_TILE + 3 * 32;  // two warpgroups, two MMA warps, the producer warp
+constexpr int MLP_RING = 10;                // rows of bf16 primitives kept (rows r-2 .. r+4 of a row pair + slack)
 constexpr int MLP_RW = MLP_TILE + 5;        // ring row width: 2 halo cells left, 3 right
-constexpr int MLP_TMEM_COLS = 256;          // 128 per warpgroup, 96 used: X = [0, 32), Y = [32, 96)
+constexpr int MLP_TMEM_COLS = 512;          // [warpgroup][slot] x 128, 96 used: X = [0, 32), Y = [32, 96)
 // shared-memory carve-up (bytes)
 constexpr int MLP_OFF_W1 = 0;                         // [64 x 32] bf16 canonical, 4 KB
 constexpr int MLP_OFF_W2 = MLP_OFF_W1 + 64 * 32 * 2;  // [64 x 64] 8 KB
@@ -44,9 +49,10 @@ constexpr int MLP_OFF_W3 = MLP_OFF_W2 + 64 * 64 * 2;  // [16 x 64] 2 KB
 constexpr int MLP_WBLOB = MLP_OFF_W3 + 16 * 64 * 2;   // 14336 B of weights, then 132 floats of biases
 constexpr int MLP_OFF_BIAS = MLP_WBLOB;               // b1[64] b2[64] b3[4]
 constexpr int MLP_BLOB = MLP_OFF_BIAS + 132 * 4;      // what jxs_set_flux_mlp uploads
-constexpr int MLP_OFF_RING = 14976;                   // [7][133] uint2
-constexpr int MLP_OFF_BAR = MLP_OFF_RING + MLP_RING * MLP_RW * 8 + 8;  // one mbarrier per warpgroup
-constexpr int MLP_SMEM = MLP_OFF_BAR + 16;
+constexpr int MLP_OFF_RING = 14976;                   // [10][133] uint2
+// mbarriers: a_full[2][2], d_full[2][2], ring_full[MLP_RING], ring_empty[MLP_RING]
+constexpr int MLP_OFF_BAR = MLP_OFF_RING + MLP_RING * MLP_RW * 8 + 8;
+constexpr int MLP_SMEM = MLP_OFF_BAR + (8 + 2 * MLP_RING) * 8;
 static_assert(MLP_OFF_RING >= MLP_BLOB && MLP_OFF_RING % 16 == 0, "the ring must not overlap the weights");
 static_assert(MLP_OFF_BAR % 8 == 0, "mbarrier alignment");
 
@@ -148,5 +154,227 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&w)[16
                  "r"(w[9]), "r"(w[10]), "r"(w[11]), "r"(w[12]), "r"(w[13]), "r"(w[14]), "r"(w[15]) : "memory");
 }
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-__device__ __forceinline__ void wg_barrier(int wg) { asm volatile("bar.sync %0, 128;" ::"r"(1 + wg) : "memory"); }
+__device__ __forceinline__ void mlp_bar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
 
+
+// hidden layer epilogue of one tile slot: the 64 pre-activations of my face (TMEM columns y .. y+63) -> + bias -> tanh
+// -> bf16 pairs -> the next layer's A operand (TMEM columns x .. x+31)
+__device__ __forceinline__ void hidden_epilogue_ts(uint32_t y, uint32_t x, const float (&bias)[64]) {
+  uint32_t v0[32], v1[32];
+  tmem_ld32(y, v0);
+  tmem_ld32(y + 32, v1);  // both halves in flight: the second one's latency passes under the first half's tanh
+  tmem_ld_wait();
+  uint32_t w[16];
+#pragma unroll
+  for (int e = 0; e < 16; ++e)
+    w[e] = pack_bf16(tanh_f32(__uint_as_float(v0[2 * e]) + bias[2 * e]), tanh_f32(__uint_as_float(v0[2 * e + 1]) + bias[2 * e + 1]));
+  tmem_st16(x, w);
+#pragma unroll
+  for (int e = 0; e < 16; ++e)
+    w[e] = pack_bf16(tanh_f32(__uint_as_float(v1[2 * e]) + bias[32 + 2 * e]), tanh_f32(__uint_as_float(v1[2 * e + 1]) + bias[33 + 2 * e]));
+  tmem_st16(x + 16, w);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(MLP_THREADS, 1) flux_mlp_kernel(const MlpArgs<T> A) {
+  extern __shared__ __align__(128) unsigned char sm[];
+  __shared__ uint32_t tmem_slot;
+  const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
+  const int strip = blockIdx.x % A.nstrips, seg_all = blockIdx.x / A.nstrips;
+  const int member = seg_all / A.nseg, seg = seg_all - member * A.nseg;
+  const int rb = member * (A.ny + 6);  // first padded row of my member
+  // cell rows whose faces this CTA evaluates: padded rows [rbeg, rend) of this member's [2, ny+3)
+  const int rbeg = rb + 2 + seg * A.rows_per_seg;
+  const int rend = min(rbeg + A.rows_per_seg, rb + A.ny + 3);
+  if (rbeg >= rend) return;
+  const int c0 = 2 + MLP_TILE * strip;            // padded column of the cell of lt = 0
+  const int nfirst = rbeg - 2, nlast = rend + 2;  // rows the producer streams, inclusive
+  const int n0 = (rend - rbeg + 1) / 2, n1 = (rend - rbeg) / 2;  // rows of tile slot 0 (even) and 1 (odd)
+
+  const uint32_t sm_u32 = (uint32_t)__cvta_generic_to_shared(sm);
+  const uint32_t bars = sm_u32 + MLP_OFF_BAR;
+  auto a_full = [&](int g, int s) { return bars + 8 * (2 * g + s); };
+  auto d_full = [&](int g, int s) { return bars + 8 * (4 + 2 * g + s); };
+  auto ring_full = [&](int slot) { return bars + 8 * (8 + slot); };
+  auto ring_empty = [&](int slot) { return bars + 8 * (8 + MLP_RING + slot); };
+  uint2* ring = reinterpret_cast<uint2*>(sm + MLP_OFF_RING);
+
+  // ---- one-time set-up: weights -> smem, TMEM, mbarriers
+  for (int i = t; i < MLP_BLOB / 16; i += MLP_THREADS)
+    reinterpret_cast<uint4*>(sm)[i] = reinterpret_cast<const uint4*>(A.blob)[i];
+  if (t == 0) {
+    for (int q = 0; q < 4; ++q) { mlp_bar_init(bars + 8 * q, MLP_TILE); mlp_bar_init(bars + 8 * (4 + q), 1); }
+    for (int q = 0; q < MLP_RING; ++q) { mlp_bar_init(ring_full(q), 32); mlp_bar_init(ring_empty(q), 2 * MLP_TILE); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 0) tmem_alloc((uint32_t)__cvta_generic_to_shared(&tmem_slot), MLP_TMEM_COLS);
+  fence_async_smem();
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+
+  if (warp == 10) {
+    // ================= producer: conserved row n -> scaled bf16 primitives (rho, u, v, p) of ring columns lane + 32 q
+    constexpr int NQ = (MLP_RW + 31) / 32;
+    T q[2][NQ][4];
+    auto load_row = [&](int n, T (&dst)[NQ][4]) {
+#pragma unroll
+      for (int c = 0; c < NQ; ++c) {
+        const int gc = min(c0 - 2 + lane + 32 * c, A.pitch - 1);
+        const T* s = A.U + (size_t)n * A.pitch + gc;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) dst[c][k] = s[k * A.plane];
+      }
+    };
+    auto convert_row = [&](int n, const T (&src)[NQ][4]) {
+      const int it = n - nfirst, slot = it % MLP_RING;
+      if (it >= MLP_RING) mbar_wait_spin(ring_empty(slot), (uint32_t)((it / MLP_RING - 1) & 1));
+#pragma unroll
+      for (int c = 0; c < NQ; ++c) {
+        const T ri = T(1) / src[c][0];
+        const T u = src[c][1] * ri, v = src[c][2] * ri;
+        const T p = A.g1 * (src[c][3] - T(0.5) * (src[c][1] * u + src[c][2] * v));
+        uint2 o;
+        o.x = pack_bf16((float)(src[c][0] * A.inv_scale[0]), (float)(u * A.inv_scale[1]));
+        o.y = pack_bf16((float)(v * A.inv_scale[2]), (float)(p * A.inv_scale[3]));
+        if (lane + 32 * c < MLP_RW) ring[slot * MLP_RW + lane + 32 * c] = o;
+      }
+      mbar_arrive(ring_full(slot));
+    };
+    load_row(nfirst, q[0]);
+    for (int n = nfirst; n <= nlast; n += 2) {  // two rows per trip: the register buffers are indexed at compile time
+      if (n + 1 <= nlast) load_row(n + 1, q[1]);
+      convert_row(n, q[0]);
+      if (n + 1 <= nlast) {
+        if (n + 2 <= nlast) load_row(n + 2, q[0]);
+        convert_row(n + 1, q[1]);
+      }
+    }
+  } else if (warp >= 8) {
+    // ================= MMA issue for warpgroup g: one lane, in the order the warpgroup fills its A operands
+    const int g = warp - 8;
+    if (lane == 0) {
+      constexpr uint32_t IDESC_H = umma_idesc(128, 64), IDESC_O = umma_idesc(128, 16);
+      uint32_t ph[2] = {0, 0};
+      auto issue = [&](int s, int layer) {
+        const uint32_t X = tmem + 256 * g + 128 * s, Y = X + 32;
+        mbar_wait_spin(a_full(g, s), ph[s]); ph[s] ^= 1;
+        tc_fence_after();
+        if (layer == 0) {
+#pragma unroll
+          for (int ks = 0; ks < 2; ++ks)
+            umma_bf16_ts(Y, X + 8 * ks, umma_desc(sm_u32 + MLP_OFF_W1 + ks * 2048, 1024, 128), IDESC_H, ks);
+        } else if (layer == 1) {
+#pragma unroll
+          for (int ks = 0; ks < 4; ++ks)
+            umma_bf16_ts(Y, X + 8 * ks, umma_desc(sm_u32 + MLP_OFF_W2 + ks * 2048, 1024, 128), IDESC_H, ks);
+        } else {
+#pragma unroll
+          for (int ks = 0; ks < 4; ++ks)
+            umma_bf16_ts(Y, X + 8 * ks, umma_desc(sm_u32 + MLP_OFF_W3 + ks * 512, 256, 128), IDESC_O, ks);
+        }
+        umma_commit(d_full(g, s));
+      };
+      for (int i = 0; i <= n0; ++i) {  // the order in which the warpgroup fills its A operands (see below)
+        const bool t0 = i < n0, t1 = i < n1, p1 = i > 0 && i - 1 < n1;
+        if (t0) issue(0, 0);
+        if (p1) issue(1, 2);
+        if (t0) issue(0, 1);
+        if (t1) issue(1, 0);
+        if (t0) issue(0, 2);
+        if (t1) issue(1, 1);
+      }
+    }
+    __syncwarp();
+  } else {
+    // ================= the two warpgroups: g = 0 right faces, g = 1 top faces; lt = my face = my TMEM lane
+    const int g = t >> 7, lt = t & (MLP_TILE - 1);
+    const int col = c0 + lt;
+    float b1[64], b2[64];  // compile-time indexed below: they stay constant-bank operands
+#pragma unroll
+    for (int k = 0; k < 64; ++k) { b1[k] = A.bias[k]; b2[k] = A.bias[64 + k]; }
+    const uint32_t lane_base = tmem + 256 * g + ((uint32_t)(32 * (warp & 3)) << 16);  // my lane quarter, slot 0
+    uint32_t ph[2] = {0, 0};
+
+    // layer-1 A operand of my face of cell row r: 24 inputs as 12 bf16 pairs, K padded to 32 with zeros
+    auto build_a1 = [&](int s, int r) {
+      const int it = r - nfirst;  // ring rows are numbered from nfirst
+      uint32_t w[16];
+      if (g == 0) {  // cells c-2 .. c+3 of row r
+        mbar_wait_spin(ring_full(it % MLP_RING), (uint32_t)((it / MLP_RING) & 1));
+        const uint2* rx = ring + (it % MLP_RING) * MLP_RW + lt;
+#pragma unroll
+        for (int c = 0; c < 6; ++c) { const uint2 e = rx[c]; w[2 * c] = e.x; w[2 * c + 1] = e.y; }
+        mbar_arrive(ring_empty(it % MLP_RING));  // the x-faces of row r were the last reader of ring row r in this warpgroup
+      } else {       // rows r-2 .. r+3 of column c, normal velocity first: (rho, v, u, p)
+        mbar_wait_spin(ring_full((it + 3) % MLP_RING), (uint32_t)(((it + 3) / MLP_RING) & 1));
+#pragma unroll
+        for (int c = 0; c < 6; ++c) {
+          const uint2 f = ring[((it - 2 + c) % MLP_RING) * MLP_RW + lt + 2];
+          w[2 * c] = __byte_perm(f.x, f.y, 0x5410); w[2 * c + 1] = __byte_perm(f.x, f.y, 0x7632);
+        }
+        mbar_arrive(ring_empty((it - 2) % MLP_RING));  // row r-2 is not read again
+      }
+      w[12] = w[13] = w[14] = w[15] = 0u;
+      tmem_st16(lane_base + 128 * s, w);
+      tmem_st_wait();
+      tc_fence_before();
+      mbar_arrive(a_full(g, s));
+    };
+    auto hidden = [&](int s, const float (&bias)[64]) {
+      mbar_wait_spin(d_full(g, s), ph[s]); ph[s] ^= 1;
+      tc_fence_after();
+      hidden_epilogue_ts(lane_base + 128 * s + 32, lane_base + 128 * s, bias);
+      tmem_st_wait();
+      tc_fence_before();
+      mbar_arrive(a_full(g, s));
+    };
+    // y = W3 h2 + b3 of my face -> my half of the cell's uint4 (x-faces: the first 8 bytes, y-faces: the second)
+    auto output = [&](int s, int r) {
+      mbar_wait_spin(d_full(g, s), ph[s]); ph[s] ^= 1;
+      tc_fence_after();
+      uint32_t y[4];
+      tmem_ld4(lane_base + 128 * s + 32, y);
+      tmem_ld_wait();
+      if (col <= A.nx + 2) {
+        float f[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) f[k] = __uint_as_float(y[k]) + A.bias[128 + k];
+        uint2* o = reinterpret_cast<uint2*>(A.dFG + (size_t)r * A.pitch + col) + g;
+        *o = make_uint2(pack_half2(f[0], f[1]), pack_half2(f[2], f[3]));
+      }
+      tc_fence_before();  // the next layer-1 MMA of this slot overwrites the columns just read
+    };
+
+    if (g == 0) {  // ring rows rbeg-2, rbeg-1 have no x-face reader: release them for this warpgroup
+      mbar_arrive(ring_empty(0));
+      mbar_arrive(ring_empty(1));
+    }
+    // Slot 0 takes the even rows of the segment, slot 1 the odd ones, one and a half steps behind: a step without tanh
+    // (output of the finished row + the layer-1 operand of the next one) always lies between two tanh steps of the
+    // other slot, and every MMA has a whole step of the other slot to complete in.
+    for (int i = 0; i <= n0; ++i) {
+      const bool t0 = i < n0, t1 = i < n1, p1 = i > 0 && i - 1 < n1;
+      const int ra = rbeg + 2 * i, rb1 = ra + 1;
+      if (i > 0) output(0, ra - 2);
+      if (t0) build_a1(0, ra);
+      if (p1) hidden(1, b2);
+      if (t0) hidden(0, b1);
+      if (p1) output(1, rb1 - 2);
+      if (t1) build_a1(1, rb1);
+      if (t0) hidden(0, b2);
+      if (t1) hidden(1, b1);
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tmem, MLP_TMEM_COLS);
+}
+
+}  // namespace jxs

@@ -1834,11 +1834,11 @@ int jxs_set_flux_mlp(jxs_solver* s, const float* weights, const double in_scale[
   if (!s->d_dFG) { CU(cudaMalloc(&s->d_dFG, fbytes)); CU(cudaMemset(s->d_dFG, 0, fbytes)); }
   CU(cudaMemcpy(s->d_mlp_blob, blob.data(), MLP_BLOB, cudaMemcpyHostToDevice));
   for (int k = 0; k < 4; ++k) { s->in_scale[k] = in_scale[k]; s->out_scale[k] = out_scale[k]; }
-  // strips of 128 cells x row segments: 2 resident CTAs per SM, 5 warm-up rows per segment; the segment count
+  // strips of 128 cells x row segments: 1 resident CTA per SM, 5 extra rows per segment; the segment count
   // that minimises (waves of CTAs) x (rows a CTA streams)
   s->mlp_strips = (s->nx + 1 + MLP_TILE - 1) / MLP_TILE;
   const int nrows = s->ny + 1;
-  const long long slots = (long long)s->num_sms * 2, columns = (long long)s->mlp_strips * s->nb;
+  const long long slots = (long long)s->num_sms, columns = (long long)s->mlp_strips * s->nb;
   long long best_cost = -1;
   int rps = nrows;
   for (int nseg = 1; nseg <= std::max(1, nrows / 8); ++nseg) {
