@@ -38,9 +38,16 @@
 namespace jxs {
 
 constexpr int MLP_TILE = 128;               // faces per MMA tile = threads per warpgroup
-constexpr int MLP_THREADS = 2 * MLP_TILE + 3 * 32;  // two warpgroups, two MMA warps, the producer warp
+constexpr int MLP_PRODUCERS = 4;           // producer warps: warp p converts the rows n = p (mod 4) of the segment
+constexpr int MLP_THREADS = 5 * MLP_TILE + (2 + MLP_PRODUCERS) * 32;  // four tanh warpgroups, one builder warpgroup, two MMA warps, the producers
 constexpr int MLP_RING = 10;                // rows of bf16 primitives kept (rows r-2 .. r+4 of a row pair + slack)
 constexpr int MLP_RW = MLP_TILE + 5;        // ring row width: 2 halo cells left, 3 right
+#ifndef PAUSE_T
+#define PAUSE_T 32
+#define PAUSE_B 64
+#define PAUSE_P 128
+#define PAUSE_M 20
+#endif
 constexpr int MLP_TMEM_COLS = 512;          // [warpgroup][slot] x 128, 96 used: X = [0, 32), Y = [32, 96)
 // shared-memory carve-up (bytes)
 constexpr int MLP_OFF_W1 = 0;                         // [64 x 32] bf16 canonical, 4 KB
@@ -50,9 +57,9 @@ constexpr int MLP_WBLOB = MLP_OFF_W3 + 16 * 64 * 2;   // 14336 B of weights, the
 constexpr int MLP_OFF_BIAS = MLP_WBLOB;               // b1[64] b2[64] b3[4]
 constexpr int MLP_BLOB = MLP_OFF_BIAS + 132 * 4;      // what jxs_set_flux_mlp uploads
 constexpr int MLP_OFF_RING = 14976;                   // [10][133] uint2
-// mbarriers: a_full[2][2], d_full[2][2], ring_full[MLP_RING], ring_empty[MLP_RING]
+// mbarriers: a_full, d_full, o_full, a1_full, l1_done, o_free (each [2 directions][2 slots]), ring_full[MLP_RING], ring_empty[MLP_RING]
 constexpr int MLP_OFF_BAR = MLP_OFF_RING + MLP_RING * MLP_RW * 8 + 8;
-constexpr int MLP_SMEM = MLP_OFF_BAR + (8 + 2 * MLP_RING) * 8;
+constexpr int MLP_SMEM = MLP_OFF_BAR + (24 + 2 * MLP_RING) * 8;
 static_assert(MLP_OFF_RING >= MLP_BLOB && MLP_OFF_RING % 16 == 0, "the ring must not overlap the weights");
 static_assert(MLP_OFF_BAR % 8 == 0, "mbarrier alignment");
 
@@ -154,30 +161,47 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&w)[16
                  "r"(w[9]), "r"(w[10]), "r"(w[11]), "r"(w[12]), "r"(w[13]), "r"(w[14]), "r"(w[15]) : "memory");
 }
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// wait with a pause between the polls: a waiting warp must not crowd the SM's MIO queue, through which the working warps'
+// MUFU, tcgen05.ld / st and shared-memory instructions are issued as well
+template <unsigned NS>
+__device__ __forceinline__ void mbar_wait_pause(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  for (;;) {
+    asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (ok) break;
+    __nanosleep(NS);
+  }
+}
 __device__ __forceinline__ void mlp_bar_init(uint32_t bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+// one arrival for the whole warp: 128 or 256 separate arrivals on one barrier serialise in the shared-memory atomic unit
+__device__ __forceinline__ void mbar_arrive_warp(uint32_t bar) {
+  __syncwarp();
+  if ((threadIdx.x & 31) == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive2(uint32_t bar) {  // counts as two arrivals
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], 2;" ::"r"(bar) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 
 
-// hidden layer epilogue of one tile slot: the 64 pre-activations of my face (TMEM columns y .. y+63) -> + bias -> tanh
-// -> bf16 pairs -> the next layer's A operand (TMEM columns x .. x+31)
+// hidden layer epilogue of one tile slot, column half H: 32 of the 64 pre-activations of my face (TMEM columns
+// y + 32 H ..) -> + bias -> tanh -> bf16 pairs -> my half of the next layer's A operand (TMEM columns x + 16 H ..)
+template <int H>
 __device__ __forceinline__ void hidden_epilogue_ts(uint32_t y, uint32_t x, const float (&bias)[64]) {
-  uint32_t v0[32], v1[32];
-  tmem_ld32(y, v0);
-  tmem_ld32(y + 32, v1);  // both halves in flight: the second one's latency passes under the first half's tanh
+  uint32_t v[32];
+  tmem_ld32(y + 32 * H, v);
   tmem_ld_wait();
   uint32_t w[16];
 #pragma unroll
   for (int e = 0; e < 16; ++e)
-    w[e] = pack_bf16(tanh_f32(__uint_as_float(v0[2 * e]) + bias[2 * e]), tanh_f32(__uint_as_float(v0[2 * e + 1]) + bias[2 * e + 1]));
-  tmem_st16(x, w);
-#pragma unroll
-  for (int e = 0; e < 16; ++e)
-    w[e] = pack_bf16(tanh_f32(__uint_as_float(v1[2 * e]) + bias[32 + 2 * e]), tanh_f32(__uint_as_float(v1[2 * e + 1]) + bias[33 + 2 * e]));
-  tmem_st16(x + 16, w);
+    w[e] = pack_bf16(tanh_f32(__uint_as_float(v[2 * e]) + bias[32 * H + 2 * e]),
+                     tanh_f32(__uint_as_float(v[2 * e + 1]) + bias[32 * H + 2 * e + 1]));
+  tmem_st16(x + 16 * H, w);
 }
 
 template <typename T>
@@ -198,18 +222,27 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) flux_mlp_kernel(const MlpArgs<
 
   const uint32_t sm_u32 = (uint32_t)__cvta_generic_to_shared(sm);
   const uint32_t bars = sm_u32 + MLP_OFF_BAR;
-  auto a_full = [&](int g, int s) { return bars + 8 * (2 * g + s); };
-  auto d_full = [&](int g, int s) { return bars + 8 * (4 + 2 * g + s); };
-  auto ring_full = [&](int slot) { return bars + 8 * (8 + slot); };
-  auto ring_empty = [&](int slot) { return bars + 8 * (8 + MLP_RING + slot); };
+  auto bar6 = [&](int kind, int g, int s) { return bars + 8 * (4 * kind + 2 * g + s); };
+  auto a_full = [&](int g, int s) { return bar6(0, g, s); };   // 8 warps: the A operand of layer 2 / 3 is in X (tanh warps)
+  auto d_full = [&](int g, int s) { return bar6(1, g, s); };   // commit: layer 1 / 2 has written Y
+  auto o_full = [&](int g, int s) { return bar6(2, g, s); };   // commit: layer 3 has written O
+  auto a1_full = [&](int g, int s) { return bar6(3, g, s); };  // 4 warps: the next row's layer-1 operand is in A1 (builders)
+  auto l1_done = [&](int g, int s) { return bar6(4, g, s); };  // commit: layer 1 has read A1
+  auto o_free = [&](int g, int s) { return bar6(5, g, s); };   // 4 warps: the builders have read O
+  auto ring_full = [&](int slot) { return bars + 8 * (24 + slot); };
+  auto ring_empty = [&](int slot) { return bars + 8 * (24 + MLP_RING + slot); };
   uint2* ring = reinterpret_cast<uint2*>(sm + MLP_OFF_RING);
 
   // ---- one-time set-up: weights -> smem, TMEM, mbarriers
   for (int i = t; i < MLP_BLOB / 16; i += MLP_THREADS)
     reinterpret_cast<uint4*>(sm)[i] = reinterpret_cast<const uint4*>(A.blob)[i];
   if (t == 0) {
-    for (int q = 0; q < 4; ++q) { mlp_bar_init(bars + 8 * q, MLP_TILE); mlp_bar_init(bars + 8 * (4 + q), 1); }
-    for (int q = 0; q < MLP_RING; ++q) { mlp_bar_init(ring_full(q), 32); mlp_bar_init(ring_empty(q), 2 * MLP_TILE); }
+    for (int q = 0; q < 4; ++q) {
+      mlp_bar_init(a_full(q >> 1, q & 1), 8); mlp_bar_init(d_full(q >> 1, q & 1), 1);
+      mlp_bar_init(o_full(q >> 1, q & 1), 1); mlp_bar_init(a1_full(q >> 1, q & 1), 4);
+      mlp_bar_init(l1_done(q >> 1, q & 1), 1); mlp_bar_init(o_free(q >> 1, q & 1), 4);
+    }
+    for (int q = 0; q < MLP_RING; ++q) { mlp_bar_init(ring_full(q), 1); mlp_bar_init(ring_empty(q), 8); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 0) tmem_alloc((uint32_t)__cvta_generic_to_shared(&tmem_slot), MLP_TMEM_COLS);
@@ -219,157 +252,191 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) flux_mlp_kernel(const MlpArgs<
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
 
-  if (warp == 10) {
-    // ================= producer: conserved row n -> scaled bf16 primitives (rho, u, v, p) of ring columns lane + 32 q
+  if (warp >= 22) {
+    // ================= producers: conserved row n -> scaled bf16 primitives (rho, u, v, p) of ring columns lane + 32 q
     constexpr int NQ = (MLP_RW + 31) / 32;
-    T q[2][NQ][4];
-    auto load_row = [&](int n, T (&dst)[NQ][4]) {
+    T q[NQ][4];
+    for (int n = nfirst + (warp - 22); n <= nlast; n += MLP_PRODUCERS) {
+      const int it = n - nfirst, slot = it % MLP_RING;
 #pragma unroll
       for (int c = 0; c < NQ; ++c) {
         const int gc = min(c0 - 2 + lane + 32 * c, A.pitch - 1);
-        const T* s = A.U + (size_t)n * A.pitch + gc;
+        const T* src = A.U + (size_t)n * A.pitch + gc;
 #pragma unroll
-        for (int k = 0; k < 4; ++k) dst[c][k] = s[k * A.plane];
+        for (int k = 0; k < 4; ++k) q[c][k] = src[k * A.plane];
       }
-    };
-    auto convert_row = [&](int n, const T (&src)[NQ][4]) {
-      const int it = n - nfirst, slot = it % MLP_RING;
-      if (it >= MLP_RING) mbar_wait_spin(ring_empty(slot), (uint32_t)((it / MLP_RING - 1) & 1));
+      if (it >= MLP_RING) mbar_wait_pause<PAUSE_P>(ring_empty(slot), (uint32_t)((it / MLP_RING - 1) & 1));
 #pragma unroll
       for (int c = 0; c < NQ; ++c) {
-        const T ri = T(1) / src[c][0];
-        const T u = src[c][1] * ri, v = src[c][2] * ri;
-        const T p = A.g1 * (src[c][3] - T(0.5) * (src[c][1] * u + src[c][2] * v));
+        // fp32 is plenty ahead of a rounding to bf16 (8 significant bits), and the fp64 division was what made the
+        // producers the slowest stage of the pipeline
+        const float r = (float)q[c][0], ru = (float)q[c][1], rv = (float)q[c][2], E = (float)q[c][3];
+        const float ri = 1.0f / r;
+        const float u = ru * ri, v = rv * ri;
+        const float p = (float)A.g1 * (E - 0.5f * (ru * u + rv * v));
         uint2 o;
-        o.x = pack_bf16((float)(src[c][0] * A.inv_scale[0]), (float)(u * A.inv_scale[1]));
-        o.y = pack_bf16((float)(v * A.inv_scale[2]), (float)(p * A.inv_scale[3]));
+        o.x = pack_bf16(r * (float)A.inv_scale[0], u * (float)A.inv_scale[1]);
+        o.y = pack_bf16(v * (float)A.inv_scale[2], p * (float)A.inv_scale[3]);
         if (lane + 32 * c < MLP_RW) ring[slot * MLP_RW + lane + 32 * c] = o;
       }
-      mbar_arrive(ring_full(slot));
-    };
-    load_row(nfirst, q[0]);
-    for (int n = nfirst; n <= nlast; n += 2) {  // two rows per trip: the register buffers are indexed at compile time
-      if (n + 1 <= nlast) load_row(n + 1, q[1]);
-      convert_row(n, q[0]);
-      if (n + 1 <= nlast) {
-        if (n + 2 <= nlast) load_row(n + 2, q[0]);
-        convert_row(n + 1, q[1]);
-      }
+      mbar_arrive_warp(ring_full(slot));
     }
-  } else if (warp >= 8) {
-    // ================= MMA issue for warpgroup g: one lane, in the order the warpgroup fills its A operands
-    const int g = warp - 8;
+  } else if (warp >= 20 && warp < 22) {
+    // ================= MMA issue for direction g: one lane, in the order the warpgroup fills its A operands
+    const int g = warp - 20;
     if (lane == 0) {
       constexpr uint32_t IDESC_H = umma_idesc(128, 64), IDESC_O = umma_idesc(128, 16);
-      uint32_t ph[2] = {0, 0};
-      auto issue = [&](int s, int layer) {
-        const uint32_t X = tmem + 256 * g + 128 * s, Y = X + 32;
-        mbar_wait_spin(a_full(g, s), ph[s]); ph[s] ^= 1;
+      uint32_t pa[2] = {0, 0}, p1[2] = {0, 0}, pf[2] = {0, 0};
+      int rows3[2] = {0, 0};  // output layers issued per slot
+      auto layer1 = [&](int s) {  // A1 = [96, 112) -> Y
+        const uint32_t base = tmem + 256 * g + 128 * s;
+        mbar_wait_pause<PAUSE_M>(a1_full(g, s), p1[s]); p1[s] ^= 1;
         tc_fence_after();
-        if (layer == 0) {
 #pragma unroll
-          for (int ks = 0; ks < 2; ++ks)
-            umma_bf16_ts(Y, X + 8 * ks, umma_desc(sm_u32 + MLP_OFF_W1 + ks * 2048, 1024, 128), IDESC_H, ks);
-        } else if (layer == 1) {
+        for (int ks = 0; ks < 2; ++ks)
+          umma_bf16_ts(base + 32, base + 96 + 8 * ks, umma_desc(sm_u32 + MLP_OFF_W1 + ks * 2048, 1024, 128), IDESC_H, ks);
+        umma_commit(d_full(g, s));
+        umma_commit(l1_done(g, s));
+      };
+      auto layer2 = [&](int s) {  // X -> Y
+        const uint32_t base = tmem + 256 * g + 128 * s;
+        mbar_wait_pause<PAUSE_M>(a_full(g, s), pa[s]); pa[s] ^= 1;
+        tc_fence_after();
 #pragma unroll
-          for (int ks = 0; ks < 4; ++ks)
-            umma_bf16_ts(Y, X + 8 * ks, umma_desc(sm_u32 + MLP_OFF_W2 + ks * 2048, 1024, 128), IDESC_H, ks);
-        } else {
-#pragma unroll
-          for (int ks = 0; ks < 4; ++ks)
-            umma_bf16_ts(Y, X + 8 * ks, umma_desc(sm_u32 + MLP_OFF_W3 + ks * 512, 256, 128), IDESC_O, ks);
-        }
+        for (int ks = 0; ks < 4; ++ks)
+          umma_bf16_ts(base + 32, base + 8 * ks, umma_desc(sm_u32 + MLP_OFF_W2 + ks * 2048, 1024, 128), IDESC_H, ks);
         umma_commit(d_full(g, s));
       };
-      for (int i = 0; i <= n0; ++i) {  // the order in which the warpgroup fills its A operands (see below)
-        const bool t0 = i < n0, t1 = i < n1, p1 = i > 0 && i - 1 < n1;
-        if (t0) issue(0, 0);
-        if (p1) issue(1, 2);
-        if (t0) issue(0, 1);
-        if (t1) issue(1, 0);
-        if (t0) issue(0, 2);
-        if (t1) issue(1, 1);
+      auto layer3 = [&](int s) {  // X -> O = [112, 128), once the builders have read the previous row's output
+        const uint32_t base = tmem + 256 * g + 128 * s;
+        mbar_wait_pause<PAUSE_M>(a_full(g, s), pa[s]); pa[s] ^= 1;
+        if (rows3[s] > 0) { mbar_wait_pause<PAUSE_M>(o_free(g, s), pf[s]); pf[s] ^= 1; }
+        ++rows3[s];
+        tc_fence_after();
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks)
+          umma_bf16_ts(base + 112, base + 8 * ks, umma_desc(sm_u32 + MLP_OFF_W3 + ks * 512, 256, 128), IDESC_O, ks);
+        umma_commit(o_full(g, s));
+      };
+      // per slot: layer 1, 2, 3 of a row, and layer 1 of the slot's next row right behind layer 3 (its operand A1 was
+      // built long before and Y is free as soon as the tanh warps have read it for layer 3's operand)
+      layer1(0);
+      if (n1 > 0) layer1(1);
+      for (int i = 0; i < n0; ++i) {
+        layer2(0);
+        if (i < n1) layer2(1);
+        layer3(0);
+        if (i + 1 < n0) layer1(0);
+        if (i < n1) {
+          layer3(1);
+          if (i + 1 < n1) layer1(1);
+        }
       }
     }
     __syncwarp();
-  } else {
-    // ================= the two warpgroups: g = 0 right faces, g = 1 top faces; lt = my face = my TMEM lane
-    const int g = t >> 7, lt = t & (MLP_TILE - 1);
-    const int col = c0 + lt;
-    float b1[64], b2[64];  // compile-time indexed below: they stay constant-bank operands
-#pragma unroll
-    for (int k = 0; k < 64; ++k) { b1[k] = A.bias[k]; b2[k] = A.bias[64 + k]; }
+  } else if (warp < 16) {
+    // ================= four tanh warpgroups: g = 0 right faces, g = 1 top faces; h = which 32 of the 64 hidden units.
+    // lt = my face = my TMEM lane; warps w, w + 8 (and builder warp 16 + w % 4) reach the same lanes 32 (w % 4) .. + 31.
+    const int g = (warp >> 2) & 1, h = warp >> 3;
     const uint32_t lane_base = tmem + 256 * g + ((uint32_t)(32 * (warp & 3)) << 16);  // my lane quarter, slot 0
     uint32_t ph[2] = {0, 0};
-
-    // layer-1 A operand of my face of cell row r: 24 inputs as 12 bf16 pairs, K padded to 32 with zeros
-    auto build_a1 = [&](int s, int r) {
+    float b1[64], b2[64];  // compile-time indexed below: they stay constant-bank operands
+#pragma unroll
+    for (int q = 0; q < 64; ++q) { b1[q] = A.bias[q]; b2[q] = A.bias[64 + q]; }
+    auto hidden = [&](int s, const float (&bias)[64]) {
+      mbar_wait_pause<PAUSE_T>(d_full(g, s), ph[s]); ph[s] ^= 1;
+      tc_fence_after();
+      if (h == 0) hidden_epilogue_ts<0>(lane_base + 128 * s + 32, lane_base + 128 * s, bias);
+      else hidden_epilogue_ts<1>(lane_base + 128 * s + 32, lane_base + 128 * s, bias);
+      tmem_st_wait();
+      tc_fence_before();
+      mbar_arrive_warp(a_full(g, s));
+    };
+    // Slot 0 takes the even rows of the segment, slot 1 the odd ones; the steps alternate between the slots, so that the
+    // MMAs a step asks for have the other slot's step to complete in.
+    for (int i = 0; i < n0; ++i) {
+      hidden(0, b1);
+      if (i < n1) hidden(1, b1);
+      hidden(0, b2);
+      if (i < n1) hidden(1, b2);
+    }
+  } else {
+    // ================= the builder warpgroup (warps 16-19), both directions, off the critical path: the layer-1 operand
+    // of a slot's NEXT row goes to the columns A1 = [96, 112) as soon as layer 1 of the current row has read them, and the
+    // output layer writes to its own columns O = [112, 128), which are read here
+    const int lt = 32 * (warp & 3) + lane, col = c0 + lt;
+    const uint32_t lane_q = (uint32_t)(32 * (warp & 3)) << 16;
+    uint32_t pl[2][2] = {{0, 0}, {0, 0}}, po[2][2] = {{0, 0}, {0, 0}};
+    // layer-1 A operand of face lt of cell row r: 24 inputs as 12 bf16 pairs, K padded to 32 with zeros
+    auto build_a1 = [&](int g, int s, int r) {
       const int it = r - nfirst;  // ring rows are numbered from nfirst
       uint32_t w[16];
       if (g == 0) {  // cells c-2 .. c+3 of row r
-        mbar_wait_spin(ring_full(it % MLP_RING), (uint32_t)((it / MLP_RING) & 1));
+        mbar_wait_pause<PAUSE_B>(ring_full(it % MLP_RING), (uint32_t)((it / MLP_RING) & 1));
         const uint2* rx = ring + (it % MLP_RING) * MLP_RW + lt;
 #pragma unroll
         for (int c = 0; c < 6; ++c) { const uint2 e = rx[c]; w[2 * c] = e.x; w[2 * c + 1] = e.y; }
-        mbar_arrive(ring_empty(it % MLP_RING));  // the x-faces of row r were the last reader of ring row r in this warpgroup
+        mbar_arrive_warp(ring_empty(it % MLP_RING));  // the x-faces of row r were the last right-face reader of ring row r
       } else {       // rows r-2 .. r+3 of column c, normal velocity first: (rho, v, u, p)
-        mbar_wait_spin(ring_full((it + 3) % MLP_RING), (uint32_t)(((it + 3) / MLP_RING) & 1));
+        // the producers fill the ring rows out of order: the first top-face row waits for all six rows it reads, every
+        // later one for the one row that is new to it
+        for (int q = (r == rbeg ? it - 2 : it + 3); q <= it + 3; ++q)
+          mbar_wait_pause<PAUSE_B>(ring_full(q % MLP_RING), (uint32_t)((q / MLP_RING) & 1));
 #pragma unroll
         for (int c = 0; c < 6; ++c) {
           const uint2 f = ring[((it - 2 + c) % MLP_RING) * MLP_RW + lt + 2];
           w[2 * c] = __byte_perm(f.x, f.y, 0x5410); w[2 * c + 1] = __byte_perm(f.x, f.y, 0x7632);
         }
-        mbar_arrive(ring_empty((it - 2) % MLP_RING));  // row r-2 is not read again
+        mbar_arrive_warp(ring_empty((it - 2) % MLP_RING));  // row r-2 is not read again by the top faces
       }
       w[12] = w[13] = w[14] = w[15] = 0u;
-      tmem_st16(lane_base + 128 * s, w);
+      tmem_st16(tmem + 256 * g + 128 * s + 96 + lane_q, w);
       tmem_st_wait();
       tc_fence_before();
-      mbar_arrive(a_full(g, s));
+      mbar_arrive_warp(a1_full(g, s));
     };
-    auto hidden = [&](int s, const float (&bias)[64]) {
-      mbar_wait_spin(d_full(g, s), ph[s]); ph[s] ^= 1;
-      tc_fence_after();
-      hidden_epilogue_ts(lane_base + 128 * s + 32, lane_base + 128 * s, bias);
-      tmem_st_wait();
-      tc_fence_before();
-      mbar_arrive(a_full(g, s));
-    };
-    // y = W3 h2 + b3 of my face -> my half of the cell's uint4 (x-faces: the first 8 bytes, y-faces: the second)
-    auto output = [&](int s, int r) {
-      mbar_wait_spin(d_full(g, s), ph[s]); ph[s] ^= 1;
+    // y = W3 h2 + b3 of face lt -> its half of the cell's uint4 (x-faces: the first 8 bytes, y-faces: the second)
+    auto output = [&](int g, int s, int r) {
+      mbar_wait_pause<PAUSE_B>(o_full(g, s), po[g][s]); po[g][s] ^= 1;
       tc_fence_after();
       uint32_t y[4];
-      tmem_ld4(lane_base + 128 * s + 32, y);
+      tmem_ld4(tmem + 256 * g + 128 * s + 112 + lane_q, y);
       tmem_ld_wait();
+      tc_fence_before();
+      mbar_arrive_warp(o_free(g, s));
       if (col <= A.nx + 2) {
         float f[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) f[k] = __uint_as_float(y[k]) + A.bias[128 + k];
+        for (int q = 0; q < 4; ++q) f[q] = __uint_as_float(y[q]) + A.bias[128 + q];
         uint2* o = reinterpret_cast<uint2*>(A.dFG + (size_t)r * A.pitch + col) + g;
         *o = make_uint2(pack_half2(f[0], f[1]), pack_half2(f[2], f[3]));
       }
-      tc_fence_before();  // the next layer-1 MMA of this slot overwrites the columns just read
     };
-
-    if (g == 0) {  // ring rows rbeg-2, rbeg-1 have no x-face reader: release them for this warpgroup
-      mbar_arrive(ring_empty(0));
-      mbar_arrive(ring_empty(1));
+    // ring rows rbeg-2, rbeg-1 have no right-face reader: release them for that direction
+    mbar_arrive_warp(ring_empty(0));
+    mbar_arrive_warp(ring_empty(1));
+#pragma unroll
+    for (int g = 0; g < 2; ++g) {
+      build_a1(g, 0, rbeg);
+      if (n1 > 0) build_a1(g, 1, rbeg + 1);
     }
-    // Slot 0 takes the even rows of the segment, slot 1 the odd ones, one and a half steps behind: a step without tanh
-    // (output of the finished row + the layer-1 operand of the next one) always lies between two tanh steps of the
-    // other slot, and every MMA has a whole step of the other slot to complete in.
-    for (int i = 0; i <= n0; ++i) {
-      const bool t0 = i < n0, t1 = i < n1, p1 = i > 0 && i - 1 < n1;
-      const int ra = rbeg + 2 * i, rb1 = ra + 1;
-      if (i > 0) output(0, ra - 2);
-      if (t0) build_a1(0, ra);
-      if (p1) hidden(1, b2);
-      if (t0) hidden(0, b1);
-      if (p1) output(1, rb1 - 2);
-      if (t1) build_a1(1, rb1);
-      if (t0) hidden(0, b2);
-      if (t1) hidden(1, b1);
+    for (int i = 0; i < n0; ++i) {
+#pragma unroll
+      for (int s = 0; s < 2; ++s) {
+        if (s == 1 && i >= n1) break;
+        const int r = rbeg + 2 * i + s;
+        const bool next = s == 0 ? i + 1 < n0 : i + 1 < n1;
+#pragma unroll
+        for (int g = 0; g < 2; ++g) {
+          if (next) {  // layer 1 of row r has read A1: build row r + 2's
+            mbar_wait_pause<PAUSE_B>(l1_done(g, s), pl[g][s]); pl[g][s] ^= 1;
+            tc_fence_after();
+            build_a1(g, s, r + 2);
+          }
+        }
+#pragma unroll
+        for (int g = 0; g < 2; ++g) output(g, s, r);
+      }
     }
   }
   tc_fence_before();
