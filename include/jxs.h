@@ -294,6 +294,17 @@ int jxs_ibm_ghost_count(const jxs_solver*);
 /* Sustained FP64 FMA rate of the device, in TFLOP/s (2 flops per FMA), from a register-
  * resident DFMA loop run for about `ms` milliseconds: the ALU-roofline denominator.         */
 int jxs_measure_fp64_peak(void* cuda_stream, double ms, double* tflops);
+/* Sustained rate of one execution unit of the current device, from a register-resident loop run for about `ms`
+ * milliseconds on `cuda_stream` (synchronous): the measured denominators of the "alu"-bound rooflines.
+ *   JXS_RATE_DFMA   FP64 FMAs of the form x = x * a + b (two register operands), TFLOP/s at 2 flop per FMA: what
+ *                   jxs_measure_fp64_peak returns; 64 per clock and SM;
+ *   JXS_RATE_DFMA3  FP64 FMAs with three distinct register operands (x = p * q + x), TFLOP/s;
+ *   JXS_RATE_TANH   MUFU.TANH (tanh.approx.f32), in 10^12 results per second: 16 per clock and SM.
+ * Errors: JXS_EINVAL (rate NULL, ms <= 0, unknown `what`), JXS_ENOMEM, JXS_ECUDA.                              */
+#define JXS_RATE_DFMA 0
+#define JXS_RATE_DFMA3 1
+#define JXS_RATE_TANH 2
+int jxs_measure_unit_rate(void* cuda_stream, int what, double ms, double* rate);
 
 #ifdef __cplusplus
 }

@@ -262,6 +262,40 @@ __global__ void dfma_peak_kernel(double* out, int iters, double a, double b) {
   if (s == 123.456) out[0] = s;  // never true; keeps the loop alive
 }
 
+// The same loop with three DISTINCT register operands per DFMA (x = p * q + x, p and q varying from one instruction to
+// the next): measured beside the loop above so that the bench line shows what operand mix the peak was taken with.
+__global__ void dfma3_peak_kernel(double* out, int iters, const double* in) {
+  double x[8], p[8], q[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) { x[k] = threadIdx.x + k; p[k] = in[k]; q[k] = in[8 + k]; }
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u)
+#pragma unroll
+      for (int k = 0; k < 8; ++k) x[k] = fma(p[k], q[k], x[k]);
+  }
+  double s = 0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) s += x[k];
+  if (s == 123.456) out[0] = s;
+}
+// MUFU.TANH rate (the roofline denominator of the flux-MLP kernel): 8 independent chains of tanh.approx.f32
+__global__ void tanh_peak_kernel(double* out, int iters) {
+  float x[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) x[k] = 0.1f * k + 1e-3f * threadIdx.x;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u)
+#pragma unroll
+      for (int k = 0; k < 8; ++k) asm volatile("tanh.approx.f32 %0, %0;" : "+f"(x[k]));
+  }
+  float s = 0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) s += x[k];
+  if (s == 123.456f) out[0] = s;
+}
+
 // y-slab sharding: rows [row0, row0 + nrows) x the interior columns x the 4 fields of a padded
 // buffer <-> a contiguous array [4][nrows][nx] that the caller sends to / receives from the neighbouring rank.
 // row0 is an interior row index (0 = the first interior row).

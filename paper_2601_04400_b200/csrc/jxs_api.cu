@@ -2227,15 +2227,18 @@ int jxs_flux_correction(jxs_solver* s, const void* U, float* dFx, float* dGy) {
   return JXS_OK;
 }
 
-int jxs_measure_fp64_peak(void* cuda_stream, double ms, double* tflops) {
-  if (!tflops || !(ms > 0)) return JXS_EINVAL;
+int jxs_measure_unit_rate(void* cuda_stream, int what, double ms, double* rate) {
+  if (!rate || !(ms > 0) || what < 0 || what > 2) return JXS_EINVAL;
   int ndev = 0, dev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return JXS_ECUDA;
   cudaDeviceProp prop;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return JXS_ECUDA;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   double* d_out = nullptr;
-  if (cudaMalloc(&d_out, 8) != cudaSuccess) return JXS_ENOMEM;
+  if (cudaMalloc(&d_out, 17 * sizeof(double)) != cudaSuccess) return JXS_ENOMEM;
+  double seed[16];
+  for (int k = 0; k < 16; ++k) seed[k] = k < 8 ? 1.0 + 1e-7 * (k + 1) : 1e-9 * (k - 7);
+  cudaMemcpyAsync(d_out + 1, seed, sizeof(seed), cudaMemcpyHostToDevice, st);
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0); cudaEventCreate(&e1);
   const int bs = 256, gs = prop.multiProcessorCount * 8;
@@ -2244,19 +2247,26 @@ int jxs_measure_fp64_peak(void* cuda_stream, double ms, double* tflops) {
   float el = 0;
   for (int rep = 0; rep < 6; ++rep) {
     cudaEventRecord(e0, st);
-    dfma_peak_kernel<<<gs, bs, 0, st>>>(d_out, iters, 1.0000001, 1e-9);
+    if (what == JXS_RATE_DFMA) dfma_peak_kernel<<<gs, bs, 0, st>>>(d_out, iters, 1.0000001, 1e-9);
+    else if (what == JXS_RATE_DFMA3) dfma3_peak_kernel<<<gs, bs, 0, st>>>(d_out, iters, d_out + 1);
+    else tanh_peak_kernel<<<gs, bs, 0, st>>>(d_out, iters);
     cudaEventRecord(e1, st);
     if (cudaEventSynchronize(e1) != cudaSuccess) break;
     cudaEventElapsedTime(&el, e0, e1);
-    const double fl = (double)gs * bs * (double)iters * 64.0 * 2.0;
-    if (rep > 0) best = std::max(best, fl / (el * 1e-3) / 1e12);
+    // 64 operations per thread and trip; an FMA counts as 2 flop, a tanh as 1
+    const double ops = (double)gs * bs * (double)iters * 64.0 * (what == JXS_RATE_TANH ? 1.0 : 2.0);
+    if (rep > 0) best = std::max(best, ops / (el * 1e-3) / 1e12);
     if (el < ms) iters = (int)std::min(2.0e6, iters * std::max(1.5, ms / std::max(el, 1e-3f)));
   }
   cudaEventDestroy(e0); cudaEventDestroy(e1);
   cudaFree(d_out);
   if (cudaGetLastError() != cudaSuccess) return JXS_ECUDA;
-  *tflops = best;
+  *rate = best;
   return JXS_OK;
+}
+
+int jxs_measure_fp64_peak(void* cuda_stream, double ms, double* tflops) {
+  return jxs_measure_unit_rate(cuda_stream, JXS_RATE_DFMA, ms, tflops);
 }
 
 }  // extern "C"

@@ -28,7 +28,7 @@ EXPORTS = ("jxs_create", "jxs_destroy", "jxs_last_error", "jxs_set_ibm", "jxs_se
            "jxs_set_adjoint_checkpointing", "jxs_flux_mlp_gradient", "jxs_adjoint_steps_mse",
            "jxs_tune", "jxs_set_rows_per_segment", "jxs_set_graph_replay", "jxs_create_batch", "jxs_batch_size",
            "jxs_get_time_batch", "jxs_set_active_rows", "jxs_shard_begin", "jxs_shard_smax", "jxs_shard_step_begin",
-           "jxs_shard_rows", "jxs_shard_stage", "jxs_shard_end")
+           "jxs_shard_rows", "jxs_shard_stage", "jxs_shard_end", "jxs_measure_unit_rate")
 
 
 class jxs_bc(C.Structure):
@@ -105,6 +105,7 @@ def lib():
         L.jxs_stage_time.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
         L.jxs_ibm_ghost_count.argtypes = [vp]
         L.jxs_measure_fp64_peak.argtypes = [vp, C.c_double, dp]
+        L.jxs_measure_unit_rate.argtypes = [vp, C.c_int, C.c_double, dp]
         L.jxs_flux_correction.argtypes = [vp, vp, vp, vp]
         L.jxs_flux_mlp_time.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
         _lib = L
@@ -127,6 +128,18 @@ def measure_fp64_peak(ms=200.0, stream=None):
     rc = lib().jxs_measure_fp64_peak(C.c_void_p(st), float(ms), C.byref(t))
     if rc != OK:
         raise JxsError(rc, "jxs_measure_fp64_peak")
+    return t.value
+
+
+RATE_DFMA, RATE_DFMA3, RATE_TANH = 0, 1, 2
+
+
+def measure_unit_rate(what, ms=200.0, stream=None):
+    t = C.c_double()
+    st = stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream
+    rc = lib().jxs_measure_unit_rate(C.c_void_p(st), int(what), float(ms), C.byref(t))
+    if rc != OK:
+        raise JxsError(rc, "jxs_measure_unit_rate")
     return t.value
 
 
