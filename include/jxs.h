@@ -173,6 +173,26 @@ int jxs_step_fixed_dt_tangent(jxs_solver*, void* U, void* Udot, double gamma_dot
  * reproducible.  Errors: JXS_EINVAL for NULL pointers or an fp32 handle.  Synchronises the stream.               */
 int jxs_mse_tangent(jxs_solver*, const void* U, const void* Udot, const void* Utarget, double* loss, double* dloss);
 
+/* jxs_mse_tangent for callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): the same two launches in the same fixed summation order, hence the same bits, but
+ *   - the partial sums go to a file-scope device array of the library (2 x 1024 doubles = 16 KB, held by every GPU
+ *     that loads the library until exit) instead of a buffer the handle allocates on first use;
+ *   - the result goes to out_dev, a DEVICE array of 2 doubles the caller owns: out_dev[0] = mean((U - Utarget)^2),
+ *     out_dev[1] = mean(2 (U - Utarget) Udot); nothing is copied to the host and the stream is NOT synchronised:
+ *     the call only enqueues two kernels on the handle's stream.
+ * It calls no cudaMalloc / cudaFree and no allocating library routine.  The first call on a device looks up the
+ * array's device address (cudaGetSymbolAddress, no allocation): make one call before starting a graph capture.
+ * U, Udot, Utarget: DEVICE pointers, [4][ny][nx] doubles, read only (as for jxs_mse_tangent).
+ * Limit: 4 nx ny <= JXS_MSE_NOALLOC_MAX_N = 2^26 entries (twice the 4 x 4096 x 2048 of the largest BASELINE
+ * configuration: the size the array is stated and tested for); beyond it JXS_EINVAL with a message naming the limit.
+ * ALL calls on a device share the one array, which keeps the last call's partial sums (every value a call reads it
+ * has written itself, so nothing needs clearing): calls that overlap on the GPU (different streams, or graph
+ * launches running concurrently) race on it and return garbage - order them.
+ * Errors: JXS_EINVAL (NULL pointers, fp32 handle, size beyond the limit), JXS_ESTATE (wrong current device),
+ * JXS_ECUDA.                                                                                                       */
+#define JXS_MSE_NOALLOC_MAX_N (1LL << 26)
+int jxs_mse_tangent_noalloc(jxs_solver*, const void* U, const void* Udot, const void* Utarget, double* out_dev);
+
 /* Reverse mode (adjoint) of jxs_step_fixed_dt, in one and in two dimensions (Euler or Navier-Stokes, nu-term; in 2D with the
  * immersed boundary and the frame's corners, R25): Eq. 15-16 —
  * "backpropagation through the full sequence of unrolled solver steps" (R21, R24).

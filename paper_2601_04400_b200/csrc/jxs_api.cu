@@ -2026,6 +2026,40 @@ int jxs_mse_tangent(jxs_solver* s, const void* U, const void* Udot, const void* 
   return JXS_OK;
 }
 
+// ---- the allocation-free variant of jxs_mse_tangent (include/jxs.h): the partial sums of the first launch live in a
+// file-scope device array instead of a lazily cudaMalloc'ed buffer of the handle.  Every GPU that loads the library holds
+// the array (16 KB) until exit.  In host code `g_mse_noalloc_scratch` is only a stand-in for the symbol: its device
+// address is looked up once per device (with that device current) and it is that address the kernels are given.
+constexpr long long MSE_NOALLOC_MAX_N = JXS_MSE_NOALLOC_MAX_N;
+static __device__ __align__(256) double g_mse_noalloc_scratch[2 * MSE_PARTS];
+static double* g_mse_noalloc_ptr[MAX_DEVICES] = {nullptr};
+
+int jxs_mse_tangent_noalloc(jxs_solver* s, const void* U, const void* Udot, const void* Utarget, double* out_dev) {
+  if (!s) return JXS_EINVAL;
+  DEV(s);
+  if (!U || !Udot || !Utarget || !out_dev) return fail(s, JXS_EINVAL, "NULL argument");
+  if (s->dtype != JXS_F64) return fail(s, JXS_EINVAL, "the tangent is fp64 only");
+  const long long n = 4LL * s->nx * s->ny;  // as in jxs_mse_tangent
+  if (n > MSE_NOALLOC_MAX_N)
+    return fail(s, JXS_EINVAL, "jxs_mse_tangent_noalloc: 4 nx ny entries exceed JXS_MSE_NOALLOC_MAX_N (2^26), the size its "
+                               "fixed scratch array is stated for; use jxs_mse_tangent");
+  if (s->dev < 0 || s->dev >= MAX_DEVICES) return fail(s, JXS_EINVAL, "device index out of range");
+  double* scratch = g_mse_noalloc_ptr[s->dev];
+  if (!scratch) {  // set-up, once per device: the device address of the symbol on the CURRENT device (= s->dev, checked above)
+    const cudaError_t e = cudaGetSymbolAddress((void**)&scratch, g_mse_noalloc_scratch);
+    if (e != cudaSuccess || !scratch) return fail(s, JXS_ECUDA, cudaGetErrorString(e));
+    g_mse_noalloc_ptr[s->dev] = scratch;
+  }
+  // same launches as jxs_mse_tangent: every partial sum that the second launch reads is written by the first one, so
+  // nothing in the array has to start at zero and the contents the last call left behind are never read
+  const int parts = (int)std::min<long long>(MSE_PARTS, (n + MSE_TB - 1) / MSE_TB);
+  mse_partial_kernel<<<parts, MSE_TB, 0, s->stream>>>((const double*)U, (const double*)Udot, (const double*)Utarget, n, scratch);
+  mse_final_kernel<<<1, MSE_TB, 0, s->stream>>>(scratch, parts, 1.0 / (double)n, out_dev);
+  s->launches += 2;
+  if (const cudaError_t e = cudaGetLastError(); e != cudaSuccess) return fail(s, JXS_ECUDA, cudaGetErrorString(e));
+  return JXS_OK;
+}
+
 int jxs_step_host(jxs_solver* s, void* U, double cfl, int nsteps) { return step_common(s, U, cfl, 0.0, nsteps, true); }
 int jxs_step_async(jxs_solver* s, void* U, double cfl, int nsteps) { return step_common(s, U, cfl, 0.0, nsteps, false, false); }
 int jxs_wait(jxs_solver* s) {

@@ -28,7 +28,7 @@ EXPORTS = ("jxs_create", "jxs_destroy", "jxs_last_error", "jxs_set_ibm", "jxs_se
            "jxs_set_adjoint_checkpointing", "jxs_flux_mlp_gradient", "jxs_adjoint_steps_mse",
            "jxs_tune", "jxs_set_rows_per_segment", "jxs_set_graph_replay", "jxs_create_batch", "jxs_batch_size",
            "jxs_get_time_batch", "jxs_set_active_rows", "jxs_shard_begin", "jxs_shard_smax", "jxs_shard_step_begin",
-           "jxs_shard_rows", "jxs_shard_stage", "jxs_shard_end", "jxs_measure_unit_rate")
+           "jxs_shard_rows", "jxs_shard_stage", "jxs_shard_end", "jxs_measure_unit_rate", "jxs_mse_tangent_noalloc")
 
 
 class jxs_bc(C.Structure):
@@ -92,6 +92,7 @@ def lib():
         L.jxs_flux_cnn_inputs.argtypes = [vp, vp, vp, vp]
         L.jxs_step_fixed_dt_tangent.argtypes = [vp, vp, vp, C.c_double, C.c_double, C.c_int]
         L.jxs_mse_tangent.argtypes = [vp, vp, vp, vp, dp, dp]
+        L.jxs_mse_tangent_noalloc.argtypes = [vp, vp, vp, vp, vp]
         L.jxs_step_fixed_dt_record.argtypes = [vp, vp, C.c_double, C.c_int]
         L.jxs_adjoint_steps.argtypes = [vp, vp, dp]
         L.jxs_set_gamma.argtypes = [vp, C.c_double]
@@ -132,6 +133,7 @@ def measure_fp64_peak(ms=200.0, stream=None):
 
 
 RATE_DFMA, RATE_DFMA3, RATE_TANH = 0, 1, 2
+MSE_NOALLOC_MAX_N = 1 << 26   # JXS_MSE_NOALLOC_MAX_N of include/jxs.h
 
 
 def measure_unit_rate(what, ms=200.0, stream=None):
@@ -373,6 +375,13 @@ class Solver:
         self._chk(lib().jxs_mse_tangent(self._h, self._dev(U), self._dev(Udot), self._dev(Utarget),
                                         C.byref(loss), C.byref(dloss)))
         return loss.value, dloss.value
+
+    def mse_tangent_noalloc(self, U, Udot, Utarget, out):
+        """jxs_mse_tangent without any allocation or synchronisation: out (device tensor, 2 float64) receives
+        (loss, dloss) when the handle's stream reaches the two kernels.  Shares one scratch array per device."""
+        assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() >= 2
+        self._chk(lib().jxs_mse_tangent_noalloc(self._h, self._dev(U), self._dev(Udot), self._dev(Utarget),
+                                                C.c_void_p(out.data_ptr())))
 
     def set_gamma(self, gamma):
         self._chk(lib().jxs_set_gamma(self._h, float(gamma)))
