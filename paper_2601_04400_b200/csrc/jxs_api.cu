@@ -83,6 +83,13 @@ struct jxs_solver {
   double* d_theta_bar = nullptr;
   double* d_Wmlp = nullptr;
   cudaGraphExec_t tan_exec = nullptr;  // one tangent step (10 launches), replayed: small grids are launch-bound
+  // the whole recorded forward sweep and the whole reverse sweep of the 1D path as graphs (run_sweep): a sweep whose
+  // parameters equal those of the call before is captured, and replayed from then on (22 launches per unrolled step)
+  struct SweepGraph {
+    cudaGraphExec_t exec = nullptr;
+    std::vector<long long> key, seen;
+    long long launches = 0;
+  } rec_graph, adj_graph;
   double tan_dt = 0, tan_gdot = 0;
   long long tan_launches = 0;
   // recorded trajectory and adjoint buffers of the one-dimensional reverse sweep (adjoint1d_kernel.cuh), compact
@@ -616,6 +623,60 @@ void drop_graph(jxs_solver* s) {
   s->pair_exec = nullptr;
   if (s->tan_exec) cudaGraphExecDestroy(s->tan_exec);
   s->tan_exec = nullptr;
+  for (jxs_solver::SweepGraph* g : {&s->rec_graph, &s->adj_graph}) {
+    if (g->exec) cudaGraphExecDestroy(g->exec);
+    g->exec = nullptr;
+    g->key.clear();
+    g->seen.clear();
+  }
+}
+
+// Run `body` (stream-ordered launches on s->stream only: no allocation, no synchronisation) either as it is, or - when
+// the call before had the same `key` - captured into a graph that is replayed from then on.  The key holds every
+// value and pointer that the launches bake in.
+template <typename Body>
+int run_sweep(jxs_solver* s, jxs_solver::SweepGraph& G, const std::vector<long long>& key, Body body) {
+  if (s->profiling || !s->use_graph) return body();
+  if (G.exec && G.key == key) {
+    CU(cudaGraphLaunch(G.exec, s->stream));
+    s->launches += G.launches;
+    return JXS_OK;
+  }
+  if (G.seen != key) {  // first sight of these parameters: plain launches (they also set the kernels' attributes)
+    G.seen = key;
+    return body();
+  }
+  if (G.exec) cudaGraphExecDestroy(G.exec);
+  G.exec = nullptr;
+  if (!s->cap_stream && cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+    cudaGetLastError();
+    return body();
+  }
+  cudaStream_t user = s->stream;
+  const long long l0 = s->launches;
+  s->stream = s->cap_stream;
+  bool ok = cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+  if (ok) {
+    ok = body() == JXS_OK;
+    cudaGraph_t g = nullptr;
+    if (cudaStreamEndCapture(s->cap_stream, &g) != cudaSuccess) ok = false;
+    if (ok && cudaGraphInstantiate(&G.exec, g, 0) != cudaSuccess) ok = false;
+    if (g) cudaGraphDestroy(g);
+  }
+  s->stream = user;
+  G.launches = s->launches - l0;
+  s->launches = l0;
+  if (!ok) {
+    cudaGetLastError();
+    if (G.exec) cudaGraphExecDestroy(G.exec);
+    G.exec = nullptr;
+    G.seen.clear();
+    return body();
+  }
+  G.key = key;
+  CU(cudaGraphLaunch(G.exec, s->stream));
+  s->launches += G.launches;
+  return JXS_OK;
 }
 
 // capture two steps (from the state cur = 0, at = 0) on a private stream; false = use plain launches
@@ -994,6 +1055,7 @@ int record_common(jxs_solver* s, void* U, double dt, int nsteps) {
   CU(pad(s, U, T(0)));
   s->events_used = 0;
   s->mlp_events_used = 0;
+  auto sweep = [&]() -> int {
   for (long long n = 0; n < nsteps; ++n) {
     prepare_step_kernel<<<1, 1, 0, s->stream>>>(s->d_state, 0, 0.0, dt);
     s->launches++;
@@ -1027,6 +1089,16 @@ int record_common(jxs_solver* s, void* U, double dt, int nsteps) {
     CU(ghost_fill(s, T(3 * n + 2)));
     CU(flux_mlp(s, T(3 * n + 2)));
     CU(stage(s, T(3 * n + 2), T(3 * n), T(3 * n + 3), 0, 1.0 / 3.0, 2.0 / 3.0, nullptr));
+  }
+  return JXS_OK;
+  };
+  {
+    long long dt_bits;
+    std::memcpy(&dt_bits, &dt, 8);
+    const std::vector<long long> key = {nsteps, dt_bits, s->scheme, ckpt, s->mlp1d_on, (long long)(size_t)s->tape,
+                                        (long long)(size_t)s->ckpt};
+    rc = run_sweep(s, s->rec_graph, key, sweep);
+    if (rc != JXS_OK) return rc;
   }
   CU(unpad(s, T((long long)per_step * nsteps), U));
   rc = finish_steps(s, nsteps);
@@ -1117,6 +1189,8 @@ int adjoint_common(jxs_solver* s, void* Ubar, double* gamma_bar, const double* t
   if (s->mlp1d_on) CU(cudaMemsetAsync(s->d_theta_bar, 0, MLP1D_NPARAM * sizeof(double), s->stream));
   s->events_used = 0;
   int x = 0;  // which adjoint state holds the adjoint of U^{n+1}
+  auto sweep = [&]() -> int {
+  x = 0;
   for (long long n = s->tape_steps - 1; n >= 0; --n) {
     // (Eq. 14) the adjoint of U^{n+1} so far comes from the later steps: add this state's own term of the loss
     if (targets && n + 1 < s->tape_steps) CU(inject(n + 1, x, 1));
@@ -1149,6 +1223,23 @@ int adjoint_common(jxs_solver* s, void* Ubar, double* gamma_bar, const double* t
     CU(adjoint_stage(s, T(3 * n), B(y1), B(y0), 1.0, B(x), 1.0 / 3.0, B(y2), 0.75));
     x = y0;
   }
+  return JXS_OK;
+  };
+  if (s->tape_ckpt) {  // the checkpointed sweep copies dt from a host variable inside the loop: plain launches
+    rc = sweep();
+  } else {
+    long long dt_bits;
+    std::memcpy(&dt_bits, &s->tape_dt, 8);
+    const std::vector<long long> key = {s->tape_steps, dt_bits, s->tape_scheme, s->mlp1d_on, (long long)(size_t)s->tape,
+                                        (long long)(size_t)s->adj, (long long)(size_t)targets, s->adj_parts};
+    rc = run_sweep(s, s->adj_graph, key, sweep);
+    if (rc == JXS_OK) {  // where the adjoint of U^0 ends up does not depend on how the sweep was run
+      x = 0;
+      if (s->tape_scheme == JXS_EULER) x = (int)(s->tape_steps & 1);
+      else for (long long n = 0; n < s->tape_steps; ++n) x = (x + 3) & 3;
+    }
+  }
+  if (rc != JXS_OK) return rc;
   CU(unpad(s, B(x), Ubar));
   double out[2];
   CU(cudaMemcpyAsync(out, s->adj + 4 * state + parts, sizeof(out), cudaMemcpyDeviceToHost, s->stream));

@@ -161,3 +161,59 @@ def test_adjoint_rejects_what_it_does_not_do():
     s3 = jxs().Solver.from_case(case)
     s3.step_fixed_dt_record(dev(case["U0"]), 1e-3, 2)
     assert s3.adjoint_steps(B) == 0.0 and float(B.abs().max()) == 0.0
+
+
+@pytest.mark.parametrize("with_mlp", [False, True])
+def test_sweep_graphs_replay_bitwise(with_mlp):
+    """The recorded forward sweep and the reverse sweep run as plain launches on the first call with given parameters,
+    are captured into CUDA graphs on the second and replayed from the third on (run_sweep in csrc/jxs_api.cu): all of
+    them must give the same bits as a handle with graph replay switched off (to round-off where the network's reverse
+    sums with atomics), also after the parameters change."""
+    case = wl.sod1d(500)
+    dt = 0.2 * case["dx"]
+    rng = np.random.default_rng(5)
+    seed_bar = torch.tensor(rng.normal(size=case["U0"].shape), device="cuda")
+    m = 6
+    targets = torch.tensor(rng.normal(size=(m,) + case["U0"].shape) * 0.01 + case["U0"], device="cuda")
+
+    def make(graph):
+        s = jxs().Solver.from_case(case)
+        if with_mlp:
+            s.set_flux_mlp(wl.mlp_weights(3), *wl.mlp_scales(out_factor=1e-2))
+        s.set_graph_replay(graph)
+        return s
+
+    def run(s, steps):
+        U = torch.tensor(case["U0"], device="cuda")
+        s.step_fixed_dt_record(U, dt, steps)
+        B = seed_bar.clone()
+        g = s.adjoint_steps(B)
+        out = [U.clone(), B.clone(), g]
+        if steps == m:
+            U2 = torch.tensor(case["U0"], device="cuda")
+            s.step_fixed_dt_record(U2, dt, steps)
+            B2 = torch.zeros_like(U2)
+            loss, g2 = s.adjoint_steps_mse(targets, B2)
+            out += [B2.clone(), loss, g2]
+            if with_mlp:
+                out.append(s.flux_mlp_gradient().copy())
+        return out
+
+    plain, graphed = make(False), make(True)
+    launches = []
+    for steps in (m, m, m, m, 4, 4, 4, m, m):   # plain / capture / replay, a change of key, and back
+        want = run(plain, steps)
+        l0 = graphed.launch_count()
+        got = run(graphed, steps)
+        launches.append(graphed.launch_count() - l0)
+        for a, b in zip(got, want):
+            if isinstance(a, torch.Tensor):
+                if with_mlp:   # the network's reverse adds into the cells' adjoints with fp64 atomics
+                    assert float((a - b).abs().max()) <= 1e-12 * float(b.abs().max())
+                else:
+                    assert torch.equal(a, b)
+            elif isinstance(a, np.ndarray):   # the weights' gradient is summed with fp64 atomics: order varies
+                assert np.allclose(a, b, rtol=1e-11, atol=1e-13 * np.abs(b).max())
+            else:   # gamma_bar is a fixed-order sum; the loss of Eq. 14 is accumulated with atomics
+                assert a == pytest.approx(b, rel=1e-13, abs=1e-300)
+    assert launches[0] == launches[1] == launches[2]    # the replayed launches are still counted
