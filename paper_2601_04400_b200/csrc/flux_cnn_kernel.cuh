@@ -314,4 +314,180 @@ __global__ void __launch_bounds__(CNN_TILE) cnn_layer3_kernel(const CnnLayerArgs
   if (warp == 0) tmem_dealloc(tmem, TCOLS);
 }
 
+// ------------------------------------------------------------------ all three layers in one kernel
+// The hidden fields (32 and 16 channels, 64 + 32 B per face) never leave the SM: a CTA marches a strip of faces row by
+// row and keeps, in shared memory, the one row of each hidden layer that the next layer's MMAs read.  With the row taps
+// stacked along N (above), input row r of a layer completes output row r-1, so one step of the march is
+//   X row r -> [layer 1] -> H1 row r-1 -> [layer 2, one step later] -> H2 row r-3 -> [layer 3, one step later] -> out row r-5.
+// The MMAs of the three layers of a step (3 + 6 + 3) are issued back to back and committed ONCE: layer 2 reads the H1
+// row that the previous step's epilogue wrote, layer 3 the H2 row likewise, so a step costs one MMA round trip instead
+// of three.  A layer's 3-wide face taps eat one face on each side: the 128-face tile yields 128 faces of H1, 126 valid
+// faces of H2 and CNNF_OUT = 124 valid output faces, so the strips advance by 124 (3 % recomputed).  The "SAME" zero
+// padding of every layer: hidden values at faces or rows outside the field are stored as zeros (not as the layer's
+// response to padded inputs).  8 extra steps per row segment fill and drain the pipeline.
+constexpr int CNNF_OUT = CNN_TILE - 4;
+constexpr int CNNF_W1 = cnn3_wbytes<1, 32>() + 32 * 4, CNNF_W2 = cnn3_wbytes<2, 16>() + 16 * 4, CNNF_W3 = cnn3_wbytes<1, 16>() + 16 * 4;
+constexpr int cnnf_align(int x) { return (x + 127) / 128 * 128; }
+constexpr int CNNF_OFF_W2 = cnnf_align(CNNF_W1), CNNF_OFF_W3 = CNNF_OFF_W2 + cnnf_align(CNNF_W2);
+constexpr int CNNF_OFF_X = CNNF_OFF_W3 + cnnf_align(CNNF_W3);          // two X row buffers (K = 16: 2 chunks)
+constexpr int CNNF_OFF_H1 = CNNF_OFF_X + 2 * cnn_slot_bytes<1>();      // one H1 row (4 chunks)
+constexpr int CNNF_OFF_H2 = CNNF_OFF_H1 + cnn_slot_bytes<2>();         // one H2 row (2 chunks)
+constexpr int CNNF_OFF_BAR = CNNF_OFF_H2 + cnn_slot_bytes<1>();
+constexpr int CNNF_SMEM = CNNF_OFF_BAR + 16;
+constexpr int CNNF_TCOLS = 256;  // accumulators: layer 1 [0, 96), layer 2 [96, 144), layer 3 [144, 192)
+
+struct CnnFusedArgs {
+  CnnField in;                 // the input field X of this direction
+  const uint8_t* blob[3];      // the three layers' blobs (cnn_layer3_kernel's format)
+  int rows_per_seg, nstrips;
+  uint4* dst;                  // as CnnLayerArgs (last layer)
+  int slot, pitch, row_off, col_off;
+};
+
+__device__ __forceinline__ void tmem_ld16u(uint32_t taddr, uint32_t (&v)[16]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                 "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+               : "r"(taddr) : "memory");
+}
+// 16 accumulator columns of my face -> + bias -> ReLU -> bf16 -> two 16-byte chunks of a row buffer (zeros if !keep)
+__device__ __forceinline__ void cnnf_hidden16(uint32_t taddr, const float* bias, unsigned char* rowbuf, int chunk0, int m, bool keep) {
+  uint32_t v[16];
+  tmem_ld16u(taddr, v);
+  tmem_ld_wait();
+#pragma unroll
+  for (int c = 0; c < 2; ++c) {
+    uint32_t w[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const int k = 8 * c + 2 * e;
+      w[e] = pack_bf16(fmaxf(__uint_as_float(v[k]) + bias[k], 0.f), fmaxf(__uint_as_float(v[k + 1]) + bias[k + 1], 0.f));
+    }
+    *reinterpret_cast<uint4*>(rowbuf + (chunk0 + c) * (CNN_ROWP * 16) + m * 16) = keep ? make_uint4(w[0], w[1], w[2], w[3]) : make_uint4(0, 0, 0, 0);
+  }
+}
+
+__global__ void __launch_bounds__(CNN_TILE, 2) cnn_fused_kernel(const CnnFusedArgs A) {
+  extern __shared__ __align__(128) unsigned char sm[];
+  __shared__ uint32_t tmem_slot;
+  constexpr int LBO_A = CNN_ROWP * 16;
+  constexpr int SLOTX = cnn_slot_bytes<1>();
+  const int t = threadIdx.x, warp = t >> 5;
+  const int strip = blockIdx.x % A.nstrips, seg = blockIdx.x / A.nstrips;
+  const int na = A.in.na, nb = A.in.nb;
+  const int abeg = seg * A.rows_per_seg, aend = min(abeg + A.rows_per_seg, na);
+  if (abeg >= aend) return;
+  const int b0 = strip * CNNF_OUT;  // first output face of the strip
+  const uint32_t sm_u32 = (uint32_t)__cvta_generic_to_shared(sm);
+  const uint32_t bar = sm_u32 + CNNF_OFF_BAR;
+  const float* bias1 = reinterpret_cast<const float*>(sm + cnn3_wbytes<1, 32>());
+  const float* bias2 = reinterpret_cast<const float*>(sm + CNNF_OFF_W2 + cnn3_wbytes<2, 16>());
+  const float* bias3 = reinterpret_cast<const float*>(sm + CNNF_OFF_W3 + cnn3_wbytes<1, 16>());
+
+  for (int i = t; i < CNNF_W1 / 16; i += CNN_TILE) reinterpret_cast<uint4*>(sm)[i] = reinterpret_cast<const uint4*>(A.blob[0])[i];
+  for (int i = t; i < CNNF_W2 / 16; i += CNN_TILE) reinterpret_cast<uint4*>(sm + CNNF_OFF_W2)[i] = reinterpret_cast<const uint4*>(A.blob[1])[i];
+  for (int i = t; i < CNNF_W3 / 16; i += CNN_TILE) reinterpret_cast<uint4*>(sm + CNNF_OFF_W3)[i] = reinterpret_cast<const uint4*>(A.blob[2])[i];
+  for (int i = t; i < (CNNF_OFF_BAR - CNNF_OFF_X) / 16; i += CNN_TILE) reinterpret_cast<uint4*>(sm + CNNF_OFF_X)[i] = make_uint4(0, 0, 0, 0);
+  if (t == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(1) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 0) tmem_alloc((uint32_t)__cvta_generic_to_shared(&tmem_slot), CNNF_TCOLS);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+  const uint32_t tlane = tmem + ((uint32_t)(32 * warp) << 16);
+  constexpr uint32_t ID1 = umma_idesc(128, 96), ID2 = umma_idesc(128, 48);
+  constexpr int PERM1 = 3 * 1 * 96 * 32, PERM2 = 3 * 2 * 48 * 32, PERM3 = 3 * 1 * 48 * 32;
+  uint32_t phase = 0;
+  tmem_zero<96>(tlane);
+  tmem_zero<48>(tlane + 96);
+  tmem_zero<48>(tlane + 144);
+
+  // X row buffer entry i = face b0 - 3 + i, i = 0 .. 129: thread t takes entry t, threads 0 and 1 also 128 + t.  Faces
+  // and rows outside the field read as zeros.  The loads are issued two steps before the stores.
+  uint4 pre[2], pre2[2];
+  auto fetch_row = [&](int r, int q) {
+    const bool row_in = r >= 0 && r < na;
+    const int p = b0 - 3 + t, p2 = b0 - 3 + CNN_TILE + t;
+    pre[q] = (row_in && p >= 0 && p < nb) ? A.in.data[A.in.at(r, 0, p)] : make_uint4(0, 0, 0, 0);
+    if (t < 2) pre2[q] = (row_in && p2 >= 0 && p2 < nb) ? A.in.data[A.in.at(r, 0, p2)] : make_uint4(0, 0, 0, 0);
+  };
+  const int r_first = abeg - 3, r_last = aend + 4;  // X rows of the march; out row r - 5 completes at step r
+  auto step = [&](int r, int q) {
+    unsigned char* xbuf = sm + CNNF_OFF_X + (r & 1) * SLOTX;
+    reinterpret_cast<uint4*>(xbuf)[t] = pre[q];
+    if (t < 2) reinterpret_cast<uint4*>(xbuf)[CNN_TILE + t] = pre2[q];
+    if (r + 2 <= r_last) fetch_row(r + 2, q);
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    if (t == 0) {
+      tc_fence_after();
+      const uint32_t xb = sm_u32 + CNNF_OFF_X + (r & 1) * SLOTX;
+      const uint32_t w1 = sm_u32 + ((r + 12) % 3) * PERM1;                       // layer 1: input row r
+      const uint32_t w2 = sm_u32 + CNNF_OFF_W2 + ((r - 2 + 12) % 3) * PERM2;     // layer 2: input row r - 2 (of H1)
+      const uint32_t w3 = sm_u32 + CNNF_OFF_W3 + ((r - 4 + 12) % 3) * PERM3;     // layer 3: input row r - 4 (of H2)
+#pragma unroll
+      for (int db = 0; db < 3; ++db)
+        umma_bf16(tmem, umma_desc(xb + db * 16, LBO_A, 128), umma_desc(w1 + db * 96 * 32, 96 * 16, 128), ID1, 1u);
+#pragma unroll
+      for (int db = 0; db < 3; ++db)
+#pragma unroll
+        for (int ks = 0; ks < 2; ++ks)
+          umma_bf16(tmem + 96, umma_desc(sm_u32 + CNNF_OFF_H1 + ks * 2 * LBO_A + db * 16, LBO_A, 128),
+                    umma_desc(w2 + (db * 2 + ks) * 48 * 32, 48 * 16, 128), ID2, 1u);
+#pragma unroll
+      for (int db = 0; db < 3; ++db)
+        umma_bf16(tmem + 144, umma_desc(sm_u32 + CNNF_OFF_H2 + db * 16, LBO_A, 128), umma_desc(w3 + db * 48 * 32, 48 * 16, 128), ID2, 1u);
+      umma_commit(bar);
+    }
+    mbar_wait_spin(bar, phase); phase ^= 1;
+    tc_fence_after();
+    // H1 row r - 1 is complete (group (r - 1) mod 3): tile row t = face b0 - 2 + t
+    {
+      const int row = r - 1, p = b0 - 2 + t;
+      const bool keep = row >= 0 && row < na && p >= 0 && p < nb;
+      const uint32_t tg = tlane + ((row + 12) % 3) * 32;
+      cnnf_hidden16(tg, bias1, sm + CNNF_OFF_H1, 0, t, keep);
+      cnnf_hidden16(tg + 16, bias1 + 16, sm + CNNF_OFF_H1, 2, t, keep);
+      tmem_zero<32>(tg);
+    }
+    // H2 row r - 3 (input row r - 2 of layer 2 completes its row - 1): tile row t = face b0 - 1 + t
+    {
+      const int row = r - 3, p = b0 - 1 + t;
+      const bool keep = row >= 0 && row < na && p >= 0 && p < nb;
+      const uint32_t tg = tlane + 96 + ((row + 12) % 3) * 16;
+      cnnf_hidden16(tg, bias2, sm + CNNF_OFF_H2, 0, t, keep);
+      tmem_zero<16>(tg);
+    }
+    // out row r - 5: tile row t = face b0 + t, of which the first CNNF_OUT are valid
+    {
+      const int row = r - 5, p = b0 + t;
+      const uint32_t tg = tlane + 144 + ((row + 12) % 3) * 16;
+      uint32_t y[4];
+      tmem_ld4(tg, y);
+      tmem_ld_wait();
+      if (row >= abeg && row < aend && t < CNNF_OUT && p < nb) {
+        uint2* o = reinterpret_cast<uint2*>(A.dst + (size_t)(row + A.row_off) * A.pitch + p + A.col_off) + A.slot;
+        float t4[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) t4[k] = tanh_f32(__uint_as_float(y[k]) + bias3[k]);
+        *o = make_uint2(pack_half2(t4[0], t4[1]), pack_half2(t4[2], t4[3]));
+      }
+      tmem_zero<16>(tg);
+    }
+    tc_fence_before();
+  };
+  fetch_row(r_first, 0);
+  fetch_row(r_first + 1, 1);
+  for (int r = r_first; r <= r_last; r += 2) {  // steps are taken in pairs: the register buffers are indexed at compile time
+    step(r, 0);
+    if (r + 1 <= r_last) step(r + 1, 1);
+  }
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tmem, CNNF_TCOLS);
+}
+
 }  // namespace jxs

@@ -456,19 +456,30 @@ cudaError_t launch_flux_cnn(jxs_solver* s, const void* U) {
   cnn_recon_kernel<T><<<grid, CNN_RX * CNN_RY, 0, s->stream>>>(R);
   s->launches++;
   cudaError_t e = cudaGetLastError();
-  for (int d = 0; d < 2 && e == cudaSuccess; ++d) {
-    CnnLayerArgs A{};
-    A.plane = s->plane; A.pitch = s->pitch;
-    A.in = s->cnn_X[d]; A.out = s->cnn_H1[d]; A.blob = s->d_cnn_blob3[d][0];
-    e = launch_cnn_layer3<1, 1, 32, false>(s, A);
-    if (e != cudaSuccess) break;
-    A.in = s->cnn_H1[d]; A.out = s->cnn_H2[d]; A.blob = s->d_cnn_blob3[d][1];
-    e = launch_cnn_layer3<2, 4, 16, false>(s, A);
-    if (e != cudaSuccess) break;
-    A.in = s->cnn_H2[d]; A.blob = s->d_cnn_blob3[d][2];
-    A.dst = s->d_dFG; A.slot = d;
+  static bool configured[MAX_DEVICES] = {false};
+  if (e == cudaSuccess) e = configure_smem(s, cnn_fused_kernel, configured, CNNF_SMEM);
+  for (int d = 0; d < 2 && e == cudaSuccess; ++d) {  // one launch per direction: the three layers fused
+    CnnFusedArgs A{};
+    A.in = s->cnn_X[d];
+    for (int l = 0; l < 3; ++l) A.blob[l] = s->d_cnn_blob3[d][l];
+    A.nstrips = (A.in.nb + CNNF_OUT - 1) / CNNF_OUT;
+    // two CTAs per SM, 8 extra steps per row segment: the segment count that minimises (waves of CTAs) x (steps per CTA)
+    const long long slots = 2LL * s->num_sms;
+    long long best = -1;
+    int rps = A.in.na;
+    for (int nseg = 1; nseg <= std::max(1, A.in.na / 16); ++nseg) {
+      const int r = (A.in.na + nseg - 1) / nseg;
+      const long long waves = ((long long)A.nstrips * ((A.in.na + r - 1) / r) + slots - 1) / slots;
+      const long long cost = waves * (r + 8);
+      if (best < 0 || cost < best) { best = cost; rps = r; }
+    }
+    A.rows_per_seg = rps;
+    A.dst = s->d_dFG; A.slot = d; A.pitch = s->pitch;
     A.row_off = d == 0 ? 3 : 2; A.col_off = d == 0 ? 2 : 3;
-    e = launch_cnn_layer3<1, 2, 16, true>(s, A);
+    const int grid = A.nstrips * ((A.in.na + rps - 1) / rps);
+    cnn_fused_kernel<<<grid, CNN_TILE, CNNF_SMEM, s->stream>>>(A);
+    s->launches++;
+    e = cudaGetLastError();
   }
   return e;
 }
