@@ -329,12 +329,16 @@ constexpr int CNNF_OUT = CNN_TILE - 4;
 constexpr int CNNF_W1 = cnn3_wbytes<1, 32>() + 32 * 4, CNNF_W2 = cnn3_wbytes<2, 16>() + 16 * 4, CNNF_W3 = cnn3_wbytes<1, 16>() + 16 * 4;
 constexpr int cnnf_align(int x) { return (x + 127) / 128 * 128; }
 constexpr int CNNF_OFF_W2 = cnnf_align(CNNF_W1), CNNF_OFF_W3 = CNNF_OFF_W2 + cnnf_align(CNNF_W2);
-constexpr int CNNF_OFF_X = CNNF_OFF_W3 + cnnf_align(CNNF_W3);          // two X row buffers (K = 16: 2 chunks)
-constexpr int CNNF_OFF_H1 = CNNF_OFF_X + 2 * cnn_slot_bytes<1>();      // one H1 row (4 chunks)
-constexpr int CNNF_OFF_H2 = CNNF_OFF_H1 + cnn_slot_bytes<2>();         // one H2 row (2 chunks)
-constexpr int CNNF_OFF_BAR = CNNF_OFF_H2 + cnn_slot_bytes<1>();
-constexpr int CNNF_SMEM = CNNF_OFF_BAR + 16;
+constexpr int CNNF_XS = 3;                                             // X row ring slots
+constexpr int CNNF_OFF_X = CNNF_OFF_W3 + cnnf_align(CNNF_W3);          // X row ring (K = 16: 2 chunks per row)
+constexpr int CNNF_OFF_H1 = CNNF_OFF_X + CNNF_XS * cnn_slot_bytes<1>();  // two H1 rows (4 chunks each)
+constexpr int CNNF_OFF_H2 = CNNF_OFF_H1 + 2 * cnn_slot_bytes<2>();     // two H2 rows (2 chunks each)
+// mbarriers: x_full[XS], x_empty[XS], acc_full[3] (a layer's MMAs of a step are complete), eps_done[3] (its epilogue has
+// read the accumulator, zeroed it and written its row)
+constexpr int CNNF_OFF_BAR = CNNF_OFF_H2 + 2 * cnn_slot_bytes<1>();
+constexpr int CNNF_SMEM = CNNF_OFF_BAR + (2 * CNNF_XS + 6) * 8;
 constexpr int CNNF_TCOLS = 256;  // accumulators: layer 1 [0, 96), layer 2 [96, 144), layer 3 [144, 192)
+constexpr int CNNF_THREADS = 3 * CNN_TILE + 64;  // one epilogue warpgroup per layer, the X producer warp, the MMA warp
 
 struct CnnFusedArgs {
   CnnField in;                 // the input field X of this direction
@@ -367,125 +371,177 @@ __device__ __forceinline__ void cnnf_hidden16(uint32_t taddr, const float* bias,
   }
 }
 
-__global__ void __launch_bounds__(CNN_TILE, 2) cnn_fused_kernel(const CnnFusedArgs A) {
+
+// Roles of the 14 warps (two CTAs per SM): warps 0-3 / 4-7 / 8-11 are the epilogue warpgroups of layers 1 / 2 / 3 (thread
+// m of a warpgroup owns tile row m = TMEM lane m), warp 12 streams the X rows from HBM into a ring, one lane of warp 13
+// issues every MMA.  A layer's cycle is: MMAs of step r -> commit -> its warpgroup reads the completed group, zeroes
+// it, writes its row (bias, ReLU, bf16, zeros outside the field) into one of two row buffers -> the MMAs of step r + 1 of
+// this layer (the group is free) and of the next layer (its input row is there) may be issued.  The three cycles run
+// against each other, so the tensor pipe works on one layer while the other two are in their epilogues; MMAs of one
+// thread complete in issue order, which is also what keeps a row buffer from being overwritten while it is still read.
+__global__ void __launch_bounds__(CNNF_THREADS, 2) cnn_fused_kernel(const CnnFusedArgs A) {
   extern __shared__ __align__(128) unsigned char sm[];
   __shared__ uint32_t tmem_slot;
   constexpr int LBO_A = CNN_ROWP * 16;
-  constexpr int SLOTX = cnn_slot_bytes<1>();
-  const int t = threadIdx.x, warp = t >> 5;
+  constexpr int SLOTX = cnn_slot_bytes<1>(), SLOTH1 = cnn_slot_bytes<2>(), SLOTH2 = cnn_slot_bytes<1>();
+  const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
   const int strip = blockIdx.x % A.nstrips, seg = blockIdx.x / A.nstrips;
   const int na = A.in.na, nb = A.in.nb;
   const int abeg = seg * A.rows_per_seg, aend = min(abeg + A.rows_per_seg, na);
   if (abeg >= aend) return;
   const int b0 = strip * CNNF_OUT;  // first output face of the strip
   const uint32_t sm_u32 = (uint32_t)__cvta_generic_to_shared(sm);
-  const uint32_t bar = sm_u32 + CNNF_OFF_BAR;
+  const uint32_t bars = sm_u32 + CNNF_OFF_BAR;
+  auto x_full = [&](int s) { return bars + 8 * s; };
+  auto x_empty = [&](int s) { return bars + 8 * (CNNF_XS + s); };
+  auto acc_full = [&](int l) { return bars + 8 * (2 * CNNF_XS + l); };
+  auto eps_done = [&](int l) { return bars + 8 * (2 * CNNF_XS + 3 + l); };
   const float* bias1 = reinterpret_cast<const float*>(sm + cnn3_wbytes<1, 32>());
   const float* bias2 = reinterpret_cast<const float*>(sm + CNNF_OFF_W2 + cnn3_wbytes<2, 16>());
   const float* bias3 = reinterpret_cast<const float*>(sm + CNNF_OFF_W3 + cnn3_wbytes<1, 16>());
 
-  for (int i = t; i < CNNF_W1 / 16; i += CNN_TILE) reinterpret_cast<uint4*>(sm)[i] = reinterpret_cast<const uint4*>(A.blob[0])[i];
-  for (int i = t; i < CNNF_W2 / 16; i += CNN_TILE) reinterpret_cast<uint4*>(sm + CNNF_OFF_W2)[i] = reinterpret_cast<const uint4*>(A.blob[1])[i];
-  for (int i = t; i < CNNF_W3 / 16; i += CNN_TILE) reinterpret_cast<uint4*>(sm + CNNF_OFF_W3)[i] = reinterpret_cast<const uint4*>(A.blob[2])[i];
-  for (int i = t; i < (CNNF_OFF_BAR - CNNF_OFF_X) / 16; i += CNN_TILE) reinterpret_cast<uint4*>(sm + CNNF_OFF_X)[i] = make_uint4(0, 0, 0, 0);
+  for (int i = t; i < CNNF_W1 / 16; i += CNNF_THREADS) reinterpret_cast<uint4*>(sm)[i] = reinterpret_cast<const uint4*>(A.blob[0])[i];
+  for (int i = t; i < CNNF_W2 / 16; i += CNNF_THREADS) reinterpret_cast<uint4*>(sm + CNNF_OFF_W2)[i] = reinterpret_cast<const uint4*>(A.blob[1])[i];
+  for (int i = t; i < CNNF_W3 / 16; i += CNNF_THREADS) reinterpret_cast<uint4*>(sm + CNNF_OFF_W3)[i] = reinterpret_cast<const uint4*>(A.blob[2])[i];
+  for (int i = t; i < (CNNF_OFF_BAR - CNNF_OFF_X) / 16; i += CNNF_THREADS) reinterpret_cast<uint4*>(sm + CNNF_OFF_X)[i] = make_uint4(0, 0, 0, 0);
   if (t == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(1) : "memory");
+    for (int s = 0; s < CNNF_XS; ++s) { mlp_bar_init(x_full(s), 1); mlp_bar_init(x_empty(s), 1); }
+    for (int l = 0; l < 3; ++l) { mlp_bar_init(acc_full(l), 1); mlp_bar_init(eps_done(l), 4); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 0) tmem_alloc((uint32_t)__cvta_generic_to_shared(&tmem_slot), CNNF_TCOLS);
+  fence_async_smem();
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
-  const uint32_t tlane = tmem + ((uint32_t)(32 * warp) << 16);
-  constexpr uint32_t ID1 = umma_idesc(128, 96), ID2 = umma_idesc(128, 48);
-  constexpr int PERM1 = 3 * 1 * 96 * 32, PERM2 = 3 * 2 * 48 * 32, PERM3 = 3 * 1 * 48 * 32;
-  uint32_t phase = 0;
-  tmem_zero<96>(tlane);
-  tmem_zero<48>(tlane + 96);
-  tmem_zero<48>(tlane + 144);
-
-  // X row buffer entry i = face b0 - 3 + i, i = 0 .. 129: thread t takes entry t, threads 0 and 1 also 128 + t.  Faces
-  // and rows outside the field read as zeros.  The loads are issued two steps before the stores.
-  uint4 pre[2], pre2[2];
-  auto fetch_row = [&](int r, int q) {
-    const bool row_in = r >= 0 && r < na;
-    const int p = b0 - 3 + t, p2 = b0 - 3 + CNN_TILE + t;
-    pre[q] = (row_in && p >= 0 && p < nb) ? A.in.data[A.in.at(r, 0, p)] : make_uint4(0, 0, 0, 0);
-    if (t < 2) pre2[q] = (row_in && p2 >= 0 && p2 < nb) ? A.in.data[A.in.at(r, 0, p2)] : make_uint4(0, 0, 0, 0);
-  };
+  const uint32_t tlane = tmem + ((uint32_t)(32 * (warp & 3)) << 16);
+  if (warp < 4) tmem_zero<96>(tlane);
+  else if (warp < 8) tmem_zero<48>(tlane + 96);
+  else if (warp < 12) tmem_zero<48>(tlane + 144);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
   const int r_first = abeg - 3, r_last = aend + 4;  // X rows of the march; out row r - 5 completes at step r
-  auto step = [&](int r, int q) {
-    unsigned char* xbuf = sm + CNNF_OFF_X + (r & 1) * SLOTX;
-    reinterpret_cast<uint4*>(xbuf)[t] = pre[q];
-    if (t < 2) reinterpret_cast<uint4*>(xbuf)[CNN_TILE + t] = pre2[q];
-    if (r + 2 <= r_last) fetch_row(r + 2, q);
-    fence_async_smem();
-    tc_fence_before();
-    __syncthreads();
-    if (t == 0) {
-      tc_fence_after();
-      const uint32_t xb = sm_u32 + CNNF_OFF_X + (r & 1) * SLOTX;
-      const uint32_t w1 = sm_u32 + ((r + 12) % 3) * PERM1;                       // layer 1: input row r
-      const uint32_t w2 = sm_u32 + CNNF_OFF_W2 + ((r - 2 + 12) % 3) * PERM2;     // layer 2: input row r - 2 (of H1)
-      const uint32_t w3 = sm_u32 + CNNF_OFF_W3 + ((r - 4 + 12) % 3) * PERM3;     // layer 3: input row r - 4 (of H2)
+
+  if (warp == 12) {
+    // ================= X producer: ring entry i = face b0 - 3 + i, i = 0 .. 129 (lane + 32 k); zeros outside the field.
+    // The loads of a row are issued two rows before its stores.
+    uint4 pre[2][5];
+    auto fetch_row = [&](int r, int q) {
+      const bool row_in = r >= 0 && r < na;
 #pragma unroll
-      for (int db = 0; db < 3; ++db)
-        umma_bf16(tmem, umma_desc(xb + db * 16, LBO_A, 128), umma_desc(w1 + db * 96 * 32, 96 * 16, 128), ID1, 1u);
-#pragma unroll
-      for (int db = 0; db < 3; ++db)
-#pragma unroll
-        for (int ks = 0; ks < 2; ++ks)
-          umma_bf16(tmem + 96, umma_desc(sm_u32 + CNNF_OFF_H1 + ks * 2 * LBO_A + db * 16, LBO_A, 128),
-                    umma_desc(w2 + (db * 2 + ks) * 48 * 32, 48 * 16, 128), ID2, 1u);
-#pragma unroll
-      for (int db = 0; db < 3; ++db)
-        umma_bf16(tmem + 144, umma_desc(sm_u32 + CNNF_OFF_H2 + db * 16, LBO_A, 128), umma_desc(w3 + db * 48 * 32, 48 * 16, 128), ID2, 1u);
-      umma_commit(bar);
-    }
-    mbar_wait_spin(bar, phase); phase ^= 1;
-    tc_fence_after();
-    // H1 row r - 1 is complete (group (r - 1) mod 3): tile row t = face b0 - 2 + t
-    {
-      const int row = r - 1, p = b0 - 2 + t;
-      const bool keep = row >= 0 && row < na && p >= 0 && p < nb;
-      const uint32_t tg = tlane + ((row + 12) % 3) * 32;
-      cnnf_hidden16(tg, bias1, sm + CNNF_OFF_H1, 0, t, keep);
-      cnnf_hidden16(tg + 16, bias1 + 16, sm + CNNF_OFF_H1, 2, t, keep);
-      tmem_zero<32>(tg);
-    }
-    // H2 row r - 3 (input row r - 2 of layer 2 completes its row - 1): tile row t = face b0 - 1 + t
-    {
-      const int row = r - 3, p = b0 - 1 + t;
-      const bool keep = row >= 0 && row < na && p >= 0 && p < nb;
-      const uint32_t tg = tlane + 96 + ((row + 12) % 3) * 16;
-      cnnf_hidden16(tg, bias2, sm + CNNF_OFF_H2, 0, t, keep);
-      tmem_zero<16>(tg);
-    }
-    // out row r - 5: tile row t = face b0 + t, of which the first CNNF_OUT are valid
-    {
-      const int row = r - 5, p = b0 + t;
-      const uint32_t tg = tlane + 144 + ((row + 12) % 3) * 16;
-      uint32_t y[4];
-      tmem_ld4(tg, y);
-      tmem_ld_wait();
-      if (row >= abeg && row < aend && t < CNNF_OUT && p < nb) {
-        uint2* o = reinterpret_cast<uint2*>(A.dst + (size_t)(row + A.row_off) * A.pitch + p + A.col_off) + A.slot;
-        float t4[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) t4[k] = tanh_f32(__uint_as_float(y[k]) + bias3[k]);
-        *o = make_uint2(pack_half2(t4[0], t4[1]), pack_half2(t4[2], t4[3]));
+      for (int k = 0; k < 5; ++k) {
+        const int i = lane + 32 * k, p = b0 - 3 + i;
+        pre[q][k] = (row_in && i < CNN_TILE + 2 && p >= 0 && p < nb) ? A.in.data[A.in.at(r, 0, p)] : make_uint4(0, 0, 0, 0);
       }
-      tmem_zero<16>(tg);
+    };
+    auto put_row = [&](int r, int q) {
+      const int k0 = r - r_first, s = k0 % CNNF_XS;
+      if (k0 >= CNNF_XS) mbar_wait_spin(x_empty(s), (uint32_t)((k0 / CNNF_XS - 1) & 1));
+      uint4* xbuf = reinterpret_cast<uint4*>(sm + CNNF_OFF_X + s * SLOTX);
+#pragma unroll
+      for (int k = 0; k < 5; ++k)
+        if (lane + 32 * k < CNN_TILE + 2) xbuf[lane + 32 * k] = pre[q][k];
+      if (r + 2 <= r_last) fetch_row(r + 2, q);
+      fence_async_smem();
+      mbar_arrive_warp(x_full(s));
+    };
+    fetch_row(r_first, 0);
+    fetch_row(r_first + 1, 1);
+    for (int r = r_first; r <= r_last; r += 2) {
+      put_row(r, 0);
+      if (r + 1 <= r_last) put_row(r + 1, 1);
     }
-    tc_fence_before();
-  };
-  fetch_row(r_first, 0);
-  fetch_row(r_first + 1, 1);
-  for (int r = r_first; r <= r_last; r += 2) {  // steps are taken in pairs: the register buffers are indexed at compile time
-    step(r, 0);
-    if (r + 1 <= r_last) step(r + 1, 1);
+  } else if (warp == 13) {
+    // ================= MMA issue
+    if (lane == 0) {
+      constexpr uint32_t ID1 = umma_idesc(128, 96), ID2 = umma_idesc(128, 48);
+      constexpr int PERM1 = 3 * 1 * 96 * 32, PERM2 = 3 * 2 * 48 * 32, PERM3 = 3 * 1 * 48 * 32;
+      uint32_t pe[3] = {0, 0, 0};
+      for (int r = r_first; r <= r_last; ++r) {
+        const int k0 = r - r_first, s = k0 % CNNF_XS;
+        const bool first = r == r_first;
+        // layer 1: X row r; its accumulator group of output row r + 2 was read and zeroed by epilogue 1 of step r - 1
+        mbar_wait_spin(x_full(s), (uint32_t)((k0 / CNNF_XS) & 1));
+        if (!first) { mbar_wait_spin(eps_done(0), pe[0]); pe[0] ^= 1; }
+        tc_fence_after();
+        {
+          const uint32_t xb = sm_u32 + CNNF_OFF_X + s * SLOTX, w1 = sm_u32 + ((r + 12) % 3) * PERM1;
+#pragma unroll
+          for (int db = 0; db < 3; ++db)
+            umma_bf16(tmem, umma_desc(xb + db * 16, LBO_A, 128), umma_desc(w1 + db * 96 * 32, 96 * 16, 128), ID1, 1u);
+          umma_commit(acc_full(0));
+          umma_commit(x_empty(s));
+        }
+        // layer 2: H1 row r - 2 (written by epilogue 1 of step r - 1, waited for above)
+        if (!first) { mbar_wait_spin(eps_done(1), pe[1]); pe[1] ^= 1; }
+        tc_fence_after();
+        {
+          const uint32_t hb = sm_u32 + CNNF_OFF_H1 + ((r - 2) & 1) * SLOTH1, w2 = sm_u32 + CNNF_OFF_W2 + ((r - 2 + 12) % 3) * PERM2;
+#pragma unroll
+          for (int db = 0; db < 3; ++db)
+#pragma unroll
+            for (int ks = 0; ks < 2; ++ks)
+              umma_bf16(tmem + 96, umma_desc(hb + ks * 2 * LBO_A + db * 16, LBO_A, 128),
+                        umma_desc(w2 + (db * 2 + ks) * 48 * 32, 48 * 16, 128), ID2, 1u);
+          umma_commit(acc_full(1));
+        }
+        // layer 3: H2 row r - 4 (written by epilogue 2 of step r - 1, waited for above)
+        if (!first) { mbar_wait_spin(eps_done(2), pe[2]); pe[2] ^= 1; }
+        tc_fence_after();
+        {
+          const uint32_t hb = sm_u32 + CNNF_OFF_H2 + ((r - 4) & 1) * SLOTH2, w3 = sm_u32 + CNNF_OFF_W3 + ((r - 4 + 12) % 3) * PERM3;
+#pragma unroll
+          for (int db = 0; db < 3; ++db)
+            umma_bf16(tmem + 144, umma_desc(hb + db * 16, LBO_A, 128), umma_desc(w3 + db * 48 * 32, 48 * 16, 128), ID2, 1u);
+          umma_commit(acc_full(2));
+        }
+      }
+    }
+    __syncwarp();
+  } else {
+    // ================= the three epilogue warpgroups
+    const int layer = warp >> 2, m = t & (CNN_TILE - 1);
+    uint32_t pf = 0;
+    for (int r = r_first; r <= r_last; ++r) {
+      mbar_wait_spin(acc_full(layer), pf); pf ^= 1;
+      tc_fence_after();
+      if (layer == 0) {         // H1 row r - 1 (group (r - 1) mod 3): tile row m = face b0 - 2 + m
+        const int row = r - 1, p = b0 - 2 + m;
+        const bool keep = row >= 0 && row < na && p >= 0 && p < nb;
+        const uint32_t tg = tlane + ((row + 12) % 3) * 32;
+        unsigned char* buf = sm + CNNF_OFF_H1 + (row & 1) * SLOTH1;
+        cnnf_hidden16(tg, bias1, buf, 0, m, keep);
+        cnnf_hidden16(tg + 16, bias1 + 16, buf, 2, m, keep);
+        tmem_zero<32>(tg);
+      } else if (layer == 1) {  // H2 row r - 3: tile row m = face b0 - 1 + m
+        const int row = r - 3, p = b0 - 1 + m;
+        const bool keep = row >= 0 && row < na && p >= 0 && p < nb;
+        const uint32_t tg = tlane + 96 + ((row + 12) % 3) * 16;
+        cnnf_hidden16(tg, bias2, sm + CNNF_OFF_H2 + (row & 1) * SLOTH2, 0, m, keep);
+        tmem_zero<16>(tg);
+      } else {                  // out row r - 5: tile row m = face b0 + m, of which the first CNNF_OUT are valid
+        const int row = r - 5, p = b0 + m;
+        const uint32_t tg = tlane + 144 + ((row + 12) % 3) * 16;
+        uint32_t y[4];
+        tmem_ld4(tg, y);
+        tmem_ld_wait();
+        tmem_zero<16>(tg);
+        if (row >= abeg && row < aend && m < CNNF_OUT && p < nb) {
+          uint2* o = reinterpret_cast<uint2*>(A.dst + (size_t)(row + A.row_off) * A.pitch + p + A.col_off) + A.slot;
+          float t4[4];
+#pragma unroll
+          for (int k = 0; k < 4; ++k) t4[k] = tanh_f32(__uint_as_float(y[k]) + bias3[k]);
+          *o = make_uint2(pack_half2(t4[0], t4[1]), pack_half2(t4[2], t4[3]));
+        }
+      }
+      fence_async_smem();
+      tc_fence_before();
+      mbar_arrive_warp(eps_done(layer));
+    }
   }
+  tc_fence_before();
   __syncthreads();
   if (warp == 0) tmem_dealloc(tmem, CNNF_TCOLS);
 }

@@ -477,7 +477,7 @@ cudaError_t launch_flux_cnn(jxs_solver* s, const void* U) {
     A.dst = s->d_dFG; A.slot = d; A.pitch = s->pitch;
     A.row_off = d == 0 ? 3 : 2; A.col_off = d == 0 ? 2 : 3;
     const int grid = A.nstrips * ((A.in.na + rps - 1) / rps);
-    cnn_fused_kernel<<<grid, CNN_TILE, CNNF_SMEM, s->stream>>>(A);
+    cnn_fused_kernel<<<grid, CNNF_THREADS, CNNF_SMEM, s->stream>>>(A);
     s->launches++;
     e = cudaGetLastError();
   }
