@@ -608,7 +608,7 @@ def run_cnn(args, rank, world, local_rank, dist, barrier, tdt):
         "clocks": clocks, "gpu_launches": solver.launch_count() - launches0,
         "roofline": {"bound": "tensor", "achieved": flop / (avg * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
                      "frac": flop / (avg * 1e-3) / 1e12 / peak, "traffic": None,
-                     "kernel": "jxs::cnn_recon_kernel + 6 x jxs::cnn_layer_kernel (one network pass)",
+                     "kernel": "jxs::cnn_recon_kernel + 2 x jxs::cnn_fused_kernel (one network pass)",
                      "avg_launch_ms": avg, "launches_timed": net_n, "stage_kernel_avg_launch_ms": stage_ms / max(stage_n, 1),
                      "alg_flop_per_cell_stage": 2.0 * 12672.0,
                      "peak_source": "MEASURED_PEAKS.json bf16_tflops_sustained (dense bf16)"},

@@ -4,18 +4,13 @@
 //   F^Neural = out_scale o tanh(conv3x3(relu(conv3x3(relu(conv3x3(X; 4->32)); 32->16)); 16->4)),  zero padding
 //
 // where X is, at every face of one direction, the mean of the left and right WENO5 states as conservative
-// variables (rho, rho u_n, rho u_t, E) / in_scale (R19).  Three passes per direction, one kernel each:
+// variables (rho, rho u_n, rho u_t, E) / in_scale (R19).  Two kernels:
 //
 //   cnn_recon_kernel   U (padded, ghosts filled) -> the two input fields, bf16, 16 bytes per face
-//   cnn_layer3_kernel  one 3x3 convolution as an implicit GEMM on tcgen05: a CTA marches a strip of 128 faces
-//                      row by row; the current input row sits in shared memory in the K-major core-matrix layout
-//                      [8-channel chunk][face][16 B], so that face tap db of the convolution is a tcgen05.mma whose
-//                      A descriptor points 16*db bytes into the row buffer: im2col without a copy.  The three ROW
-//                      taps are stacked along N (one MMA feeds three output rows): 3 * Cin/16 MMAs per row accumulate
-//                      in TMEM; bias, ReLU (tanh in the last layer) and the rounding to bf16 follow in registers.
+//   cnn_fused_kernel   one launch per direction: the three 3x3 convolutions as implicit GEMMs on tcgen05, the hidden
+//                      activations kept in shared memory (see the kernel's comment)
 //
-// Activation fields in HBM use the same chunked layout with a one-face border of zeros all around (the "SAME"
-// padding of every layer is then just what the loads find): element (row r, chunk c, face p) is the uint4 at
+// The input fields in HBM have a one-face border of zeros all around: element (row r, chunk c, face p) is the uint4 at
 //   ((r + 1) * C + c) * nbp + (p + 1),      r in [-1, na], p in [-1, nbp - 2].
 // Rows are indexed along the field's first axis, faces along its second.  x-faces: rows = j (tangential), faces
 // = f (normal).  y-faces are kept in their natural order, rows = f (normal), faces = i (tangential), and use the
@@ -137,43 +132,25 @@ __global__ void cnn_inputs_gather_kernel(CnnField fx, CnnField fy, float* __rest
   }
 }
 
-// ------------------------------------------------------------------ passes 2-4: one 3x3 convolution each
+// ------------------------------------------------------------------ the three 3x3 convolutions
 // KC = 16-channel K steps per tap (input channels / 16, at least 1), NOUT = output channels padded to 16.
-// Weight blob of a layer (bf16, packed on the host): [9 taps][KC][NOUT x 16] tiles in the K-major no-swizzle
-// canonical layout (element (n, k) at (n/8)*128 + (k/8)*(NOUT*16) + (n%8)*16 + (k%8)*2), then NOUT fp32 biases.
-struct CnnLayerArgs {
-  CnnField in, out;      // out unused by the last layer
-  const uint8_t* blob;   // weights + biases of this layer (for this direction: y-faces use transposed taps)
-  int rows_per_seg;
-  // last layer only: y[0..3] -> half `slot` (0: right faces, 1: top faces) of dst[(row + row_off) * pitch + face + col_off],
-  // as fp16 (the stage kernel's dFG)
-  uint4* dst;
-  int slot;
-  long long plane;
-  int pitch, row_off, col_off;
-};
-
 template <int KC>
-__host__ __device__ constexpr int cnn_slot_bytes() { return 2 * KC * CNN_ROWP * 16; }  // 2 chunks per K step
-// CIN8 (below) = 8-channel chunks the input field really has (1 for the first layer: its second chunk stays zero)
+__host__ __device__ constexpr int cnn_slot_bytes() { return 2 * KC * CNN_ROWP * 16; }  // one row buffer: 2 chunks per K step
 
-// ------------------------------------------------------------------ the layer, with the row taps stacked along N
-// A 128 x N x 16 MMA with N <= 32 costs ~64 cycles whatever it computes (measured: the tensor core's fetch of the
-// 4 KB activation tile), so a layer with one MMA per tap is bound by its 9 * KC MMAs per row.  Input row r feeds THREE output
-// rows (r+1 with row tap 0, r with tap 1, r-1 with tap 2) from the same shifted windows, so one MMA with the three
-// taps' weights side by side (N = 3 * NOUT) does the work of three: 3 * KC MMAs per row.  The three accumulators
-// (TMEM column groups g = output row mod 3) are always accumulated into; the group whose output row is complete
-// after input row r (row r-1) is read by the epilogue and zeroed with tcgen05.st.  Which tap a group needs depends
-// on r mod 3, hence three permutations of the weight tiles (packed on the host):
-//   blob = [3 permutations][3 face taps db][KC][3 NOUT x 16] canonical tiles, then NOUT fp32 biases;
+// A 128 x N x 16 MMA with N <= 64 costs ~50 cycles whatever it computes, so a layer with one MMA per tap would be bound
+// by its 9 * KC MMAs per row.  Input row r feeds THREE output rows (r+1 with row tap 0, r with tap 1, r-1 with tap 2)
+// from the same shifted windows, so one MMA with the three taps' weights side by side (N = 3 * NOUT) does the work of
+// three: 3 * KC MMAs per row.  The three accumulators (TMEM column groups g = output row mod 3) are always
+// accumulated into; the group whose output row is complete after input row r (row r-1) is read by the epilogue and
+// zeroed with tcgen05.st.  Which tap a group needs depends on r mod 3, hence three permutations of the weight tiles
+// (packed on the host):
+//   blob of a layer = [3 permutations][3 face taps db][KC][3 NOUT x 16] tiles in the K-major no-swizzle canonical layout
+//   (element (n, k) at (n/8)*128 + (k/8)*(N*16) + (n%8)*16 + (k%8)*2), then NOUT fp32 biases;
 //   in permutation q = r mod 3, rows g * NOUT .. of a tile hold row tap da = (q + 1 - g) mod 3.
-// Only the current input row is needed in shared memory (double-buffered).
+// Face tap db of the convolution is an MMA whose A descriptor points 16*db bytes into the row buffer (layout
+// [8-channel chunk][face][16 B]): im2col without a copy.
 template <int KC, int NOUT>
 __host__ __device__ constexpr int cnn3_wbytes() { return 3 * 3 * KC * 3 * NOUT * 16 * 2; }
-template <int KC, int NOUT>
-__host__ __device__ constexpr int cnn3_smem_bytes() {
-  return (cnn3_wbytes<KC, NOUT>() + NOUT * 4 + 127) / 128 * 128 + 2 * cnn_slot_bytes<KC>() + 16;
-}
 
 template <int NCOL>
 __device__ __forceinline__ void tmem_zero(uint32_t taddr) {  // NCOL (multiple of 16) columns of my lane <- 0
@@ -182,136 +159,6 @@ __device__ __forceinline__ void tmem_zero(uint32_t taddr) {  // NCOL (multiple o
     asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1,%1};"
                  ::"r"(taddr + 16 * h), "r"(0u) : "memory");
   asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-}
-
-template <int KC, int CIN8, int NOUT, bool LAST>
-__global__ void __launch_bounds__(CNN_TILE) cnn_layer3_kernel(const CnnLayerArgs A) {
-  extern __shared__ __align__(128) unsigned char sm[];
-  __shared__ uint32_t tmem_slot;
-  constexpr int WB = cnn3_wbytes<KC, NOUT>();
-  constexpr int OFF_ROWS = (WB + NOUT * 4 + 127) / 128 * 128;
-  constexpr int SLOT = cnn_slot_bytes<KC>();
-  constexpr int LBO_A = CNN_ROWP * 16;
-  constexpr int N3 = 3 * NOUT;
-  constexpr int TCOLS = N3 <= 64 ? 64 : 128;
-  constexpr int PERM = 3 * KC * N3 * 32;  // bytes of one permutation of the tiles
-  const int t = threadIdx.x, warp = t >> 5;
-  const int nstrips = (A.in.nb + CNN_TILE - 1) / CNN_TILE;
-  const int strip = blockIdx.x % nstrips, seg = blockIdx.x / nstrips;
-  const int abeg = seg * A.rows_per_seg, aend = min(abeg + A.rows_per_seg, A.in.na);
-  if (abeg >= aend) return;
-  const int b0 = strip * CNN_TILE;
-  const uint32_t sm_u32 = (uint32_t)__cvta_generic_to_shared(sm);
-  const uint32_t bar = sm_u32 + OFF_ROWS + 2 * SLOT;
-  const float* bias = reinterpret_cast<const float*>(sm + WB);
-
-  for (int i = t; i < (WB + NOUT * 4) / 16; i += CNN_TILE)
-    reinterpret_cast<uint4*>(sm)[i] = reinterpret_cast<const uint4*>(A.blob)[i];
-  for (int i = t; i < 2 * SLOT / 16; i += CNN_TILE) reinterpret_cast<uint4*>(sm + OFF_ROWS)[i] = make_uint4(0, 0, 0, 0);
-  if (t == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(1) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  if (warp == 0) tmem_alloc((uint32_t)__cvta_generic_to_shared(&tmem_slot), TCOLS);
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = tmem_slot;
-  const uint32_t tlane = tmem + ((uint32_t)(32 * warp) << 16);
-  constexpr uint32_t IDESC = umma_idesc(128, N3);
-  uint32_t phase = 0;
-  tmem_zero<N3>(tlane);  // the three accumulators start at zero and are only ever added to
-
-  // the global loads of a row are issued TWO iterations before its stores (registers pre[r & 1]): one iteration is
-  // shorter than the memory latency under load
-  uint4 pre[2][CIN8], pre2[2][CIN8];
-  auto fetch_row = [&](int r, int q) {
-#pragma unroll
-    for (int c = 0; c < CIN8; ++c) {
-      const uint4* src = A.in.data + A.in.at(r, c, b0 - 1);
-      pre[q][c] = src[t];
-      if (t < 2) pre2[q][c] = src[CNN_TILE + t];
-    }
-  };
-  auto store_row = [&](int r, int q) {
-    unsigned char* dst = sm + OFF_ROWS + ((r + 2) & 1) * SLOT;
-#pragma unroll
-    for (int c = 0; c < CIN8; ++c) {
-      reinterpret_cast<uint4*>(dst + c * LBO_A)[t] = pre[q][c];
-      if (t < 2) reinterpret_cast<uint4*>(dst + c * LBO_A)[CNN_TILE + t] = pre2[q][c];
-    }
-  };
-  // rows are taken in pairs so that the register buffers are indexed at compile time
-  auto row_step = [&](int r, int q) {
-    store_row(r, q);
-    if (r + 2 <= aend) fetch_row(r + 2, q);
-    fence_async_smem();
-    tc_fence_before();
-    __syncthreads();
-    if (t == 0) {
-      tc_fence_after();
-      const uint32_t rowbuf = sm_u32 + OFF_ROWS + ((r + 2) & 1) * SLOT;
-      const uint32_t wperm = sm_u32 + ((r + 3) % 3) * PERM;
-#pragma unroll
-      for (int db = 0; db < 3; ++db)
-#pragma unroll
-        for (int ks = 0; ks < KC; ++ks)
-          umma_bf16(tmem, umma_desc(rowbuf + ks * 2 * LBO_A + db * 16, LBO_A, 128),
-                    umma_desc(wperm + (db * KC + ks) * N3 * 32, N3 * 16, 128), IDESC, 1u);
-      umma_commit(bar);
-    }
-    mbar_wait_spin(bar, phase); phase ^= 1;
-    tc_fence_after();
-    // output row r-1 is complete: its accumulator is column group (r-1) mod 3
-    const int row = r - 1, p = b0 + t;
-    const uint32_t tg = tlane + ((row + 3) % 3) * NOUT;
-    const bool live = row >= abeg && row < aend && p < A.in.nb;
-    if (!LAST) {
-#pragma unroll
-      for (int h = 0; h < NOUT / 16; ++h) {
-        uint32_t v[16];
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                       "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                     : "r"(tg + 16 * h) : "memory");
-        tmem_ld_wait();
-        if (live) {
-#pragma unroll
-          for (int c = 0; c < 2; ++c) {
-            uint32_t w[4];
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              const int k = 8 * c + 2 * e;
-              w[e] = pack_bf16(fmaxf(__uint_as_float(v[k]) + bias[16 * h + k], 0.f), fmaxf(__uint_as_float(v[k + 1]) + bias[16 * h + k + 1], 0.f));
-            }
-            A.out.data[A.out.at(row, 2 * h + c, p)] = make_uint4(w[0], w[1], w[2], w[3]);
-          }
-        }
-      }
-    } else {
-      uint32_t y[4];
-      tmem_ld4(tg, y);
-      tmem_ld_wait();
-      if (live) {
-        // my half (x-faces: the first 8 bytes, y-faces: the second) of the cell's eight fp16 network outputs
-        uint2* o = reinterpret_cast<uint2*>(A.dst + (size_t)(row + A.row_off) * A.pitch + p + A.col_off) + A.slot;
-        float t4[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) t4[k] = tanh_f32(__uint_as_float(y[k]) + bias[k]);
-        *o = make_uint2(pack_half2(t4[0], t4[1]), pack_half2(t4[2], t4[3]));
-      }
-    }
-    tmem_zero<NOUT>(tg);  // the group starts over with output row r+2
-    tc_fence_before();
-  };
-  fetch_row(abeg - 1, 0);
-  fetch_row(abeg, 1);
-  for (int r = abeg - 1; r <= aend; r += 2) {  // input rows; rows -1 and na are the zero border of the field
-    row_step(r, 0);
-    if (r + 1 <= aend) row_step(r + 1, 1);
-  }
-  __syncthreads();
-  if (warp == 0) tmem_dealloc(tmem, TCOLS);
 }
 
 // ------------------------------------------------------------------ all three layers in one kernel

@@ -141,8 +141,8 @@ struct jxs_solver {
   // the paper's 2D CNN flux (flux_cnn_kernel.cuh): per direction (x, y) the input field, the two hidden fields and
   // the three layers' weight blobs; shares d_dFG / out_scale with the MLP path (one of the two at a time)
   bool cnn_on = false;
-  CnnField cnn_X[2] = {}, cnn_H1[2] = {}, cnn_H2[2] = {};
-  uint8_t* d_cnn_blob3[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};  // for cnn_layer3_kernel
+  CnnField cnn_X[2] = {};
+  uint8_t* d_cnn_blob3[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};  // per direction and layer, for cnn_fused_kernel
   double cnn_in_scale[4] = {1, 1, 1, 1};
   int mlp_strips = 0, mlp_rows_per_seg = 0, mlp_grid = 0;
   double mlp_ms = 0;
@@ -426,23 +426,8 @@ cudaError_t launch_flux_mlp(jxs_solver* s, const void* U) {
   s->launches++;
   return cudaGetLastError();
 }
-// the CNN flux of the padded, ghost-filled state U -> d_dFG: reconstruction pass, then three convolution
-// layers per direction
-template <int KC, int CIN8, int NOUT, bool LAST>
-cudaError_t launch_cnn_layer3(jxs_solver* s, const CnnLayerArgs& A0) {
-  CnnLayerArgs A = A0;
-  auto kern = cnn_layer3_kernel<KC, CIN8, NOUT, LAST>;
-  constexpr int smem = cnn3_smem_bytes<KC, NOUT>();
-  static bool configured[MAX_DEVICES] = {false};
-  if (cudaError_t e = configure_smem(s, kern, configured, smem); e != cudaSuccess) return e;
-  const int nstrips = (A.in.nb + CNN_TILE - 1) / CNN_TILE;
-  const int segs = std::max(1, s->num_sms * 8 / nstrips);
-  A.rows_per_seg = std::max((A.in.na + segs - 1) / segs, std::min(A.in.na, 8));
-  const int grid = nstrips * ((A.in.na + A.rows_per_seg - 1) / A.rows_per_seg);
-  kern<<<grid, CNN_TILE, smem, s->stream>>>(A);
-  s->launches++;
-  return cudaGetLastError();
-}
+// the CNN flux of the padded, ghost-filled state U -> d_dFG: reconstruction pass, then one fused three-layer launch
+// per direction
 template <typename T>
 cudaError_t launch_flux_cnn(jxs_solver* s, const void* U) {
   CnnReconArgs<T> R;
@@ -500,7 +485,7 @@ cudaError_t flux_mlp(jxs_solver* s, const void* U) {  // whichever network is se
     s->launches++;
     return cudaGetLastError();
   }
-  if (s->cnn_on) {  // jxs_flux_mlp_time then reports the whole network pass (reconstruction + 6 layer launches)
+  if (s->cnn_on) {  // jxs_flux_mlp_time then reports the whole network pass (reconstruction + one fused launch per direction)
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (s->profiling && s->mlp_events_used + 2 <= (int)s->mlp_events.size()) {
       e0 = s->mlp_events[s->mlp_events_used++];
@@ -536,7 +521,7 @@ void pack_canonical(const float* W, int N, int Kin, int Npad, int Kpad, uint8_t*
 
 // W is OIHW [cout][cin][3 tangential taps][3 normal taps]; the kernel's tap (row offset, face offset) is
 // (tangential, normal) for x-faces and (normal, tangential) for y-faces (transposed = true).
-// one convolution layer's blob for cnn_layer3_kernel: [3 permutations q][3 face taps dp][KC][3 NOUT x 16] tiles + NOUT biases; rows
+// one convolution layer's blob for cnn_fused_kernel: [3 permutations q][3 face taps dp][KC][3 NOUT x 16] tiles + NOUT biases; rows
 // g * NOUT .. of a tile hold row tap dr = (q + 1 - g) mod 3
 std::vector<uint8_t> pack_cnn_layer3(const float* W, const float* b, int cout, int cin, int KC, int NOUT, bool transposed) {
   const int N3 = 3 * NOUT;
@@ -1731,7 +1716,7 @@ void jxs_destroy(jxs_solver* s) {
   free_ibm(s);
   cudaFree(s->d_mlp_blob); cudaFree(s->d_dFG);
   for (int d = 0; d < 2; ++d) {
-    cudaFree(s->cnn_X[d].data); cudaFree(s->cnn_H1[d].data); cudaFree(s->cnn_H2[d].data);
+    cudaFree(s->cnn_X[d].data);
     for (int l = 0; l < 3; ++l) cudaFree(s->d_cnn_blob3[d][l]);
   }
   for (cudaEvent_t ev : s->events) cudaEventDestroy(ev);
@@ -1983,14 +1968,11 @@ int jxs_set_flux_cnn(jxs_solver* s, const float* weights, const double in_scale[
     // fields: x-faces rows j (ny), faces f (nx+1); y-faces rows f (ny+1), faces i (nx); zero border all around
     const int na = d == 0 ? s->ny : s->ny + 1, nb = d == 0 ? s->nx + 1 : s->nx;
     const int nbp = (nb + CNN_TILE - 1) / CNN_TILE * CNN_TILE + 2;
-    CnnField* f[3] = {&s->cnn_X[d], &s->cnn_H1[d], &s->cnn_H2[d]};
-    const int chunks[3] = {1, 4, 2};
-    for (int q = 0; q < 3; ++q) {
-      const size_t bytes = (size_t)(na + 2) * chunks[q] * nbp * sizeof(uint4);
-      if (!f[q]->data) CU(cudaMalloc(&f[q]->data, bytes));
-      CU(cudaMemset(f[q]->data, 0, bytes));
-      f[q]->na = na; f[q]->nb = nb; f[q]->nbp = nbp; f[q]->C = chunks[q];
-    }
+    CnnField* f = &s->cnn_X[d];   // the hidden fields never leave the SM (cnn_fused_kernel)
+    const size_t bytes = (size_t)(na + 2) * nbp * sizeof(uint4);
+    if (!f->data) CU(cudaMalloc(&f->data, bytes));
+    CU(cudaMemset(f->data, 0, bytes));
+    f->na = na; f->nb = nb; f->nbp = nbp; f->C = 1;
   }
   const size_t fbytes = (size_t)s->plane * sizeof(uint4);
   if (!s->d_dFG) { CU(cudaMalloc(&s->d_dFG, fbytes)); CU(cudaMemset(s->d_dFG, 0, fbytes)); }
