@@ -263,11 +263,13 @@ __global__ void dfma_peak_kernel(double* out, int iters, double a, double b) {
 }
 
 // The same loop with three DISTINCT register operands per DFMA (x = p * q + x, p and q varying from one instruction to
-// the next): measured beside the loop above so that the bench line shows what operand mix the peak was taken with.
+// the next): the register file hands the FP64 pipe two 64-bit operands per issue slot, so such a DFMA occupies the pipe for 3
+// cycles instead of 2 (measured: 24.8 against 37.2 TFLOP/s).  Real code is a mix of the two forms.
 __global__ void dfma3_peak_kernel(double* out, int iters, const double* in) {
   double x[8], p[8], q[8];
 #pragma unroll
-  for (int k = 0; k < 8; ++k) { x[k] = threadIdx.x + k; p[k] = in[k]; q[k] = in[8 + k]; }
+  // p and q depend on the thread: uniform values would be kept in uniform registers, which are not register-file reads
+  for (int k = 0; k < 8; ++k) { x[k] = threadIdx.x + k; p[k] = in[k] + 1e-13 * threadIdx.x; q[k] = in[8 + k] * (1.0 + 1e-13 * threadIdx.x); }
   for (int i = 0; i < iters; ++i) {
 #pragma unroll
     for (int u = 0; u < 8; ++u)
