@@ -166,14 +166,15 @@ __device__ __forceinline__ void tmem_zero(uint32_t taddr) {  // NCOL (multiple o
 // row and keeps, in shared memory, the one row of each hidden layer that the next layer's MMAs read.  With the row taps
 // stacked along N (above), input row r of a layer completes output row r-1, so one step of the march is
 //   X row r -> [layer 1] -> H1 row r-1 -> [layer 2, one step later] -> H2 row r-3 -> [layer 3, one step later] -> out row r-5.
-// The MMAs of the three layers of a step (3 + 6 + 3) are issued back to back and committed ONCE: layer 2 reads the H1
+// The MMAs of the three layers of a step (1 + 6 + 3) are issued back to back and committed ONCE: layer 2 reads the H1
 // row that the previous step's epilogue wrote, layer 3 the H2 row likewise, so a step costs one MMA round trip instead
 // of three.  A layer's 3-wide face taps eat one face on each side: the 128-face tile yields 128 faces of H1, 126 valid
 // faces of H2 and CNNF_OUT = 124 valid output faces, so the strips advance by 124 (3 % recomputed).  The "SAME" zero
 // padding of every layer: hidden values at faces or rows outside the field are stored as zeros (not as the layer's
 // response to padded inputs).  8 extra steps per row segment fill and drain the pipeline.
 constexpr int CNNF_OUT = CNN_TILE - 4;
-constexpr int CNNF_W1 = cnn3_wbytes<1, 32>() + 32 * 4, CNNF_W2 = cnn3_wbytes<2, 16>() + 16 * 4, CNNF_W3 = cnn3_wbytes<1, 16>() + 16 * 4;
+constexpr int CNNF_W1T = 3 * 96 * 16 * 2;  // layer 1: one [96 x 16] tile per permutation (its 3 face taps x 4 channels share one K step)
+constexpr int CNNF_W1 = CNNF_W1T + 32 * 4, CNNF_W2 = cnn3_wbytes<2, 16>() + 16 * 4, CNNF_W3 = cnn3_wbytes<1, 16>() + 16 * 4;
 constexpr int cnnf_align(int x) { return (x + 127) / 128 * 128; }
 constexpr int CNNF_OFF_W2 = cnnf_align(CNNF_W1), CNNF_OFF_W3 = CNNF_OFF_W2 + cnnf_align(CNNF_W2);
 constexpr int CNNF_XS = 3;                                             // X row ring slots
@@ -189,7 +190,7 @@ constexpr int CNNF_THREADS = 3 * CNN_TILE + 64;  // one epilogue warpgroup per l
 
 struct CnnFusedArgs {
   CnnField in;                 // the input field X of this direction
-  const uint8_t* blob[3];      // the three layers' blobs (cnn_layer3_kernel's format)
+  const uint8_t* blob[3];      // the three layers' blobs (layer 1: [3 permutations][96 x 16 tile], its taps side by side in K)
   int rows_per_seg, nstrips;
   uint4* dst;                  // as CnnLayerArgs (last layer)
   int slot, pitch, row_off, col_off;
@@ -243,7 +244,7 @@ __global__ void __launch_bounds__(CNNF_THREADS, 2) cnn_fused_kernel(const CnnFus
   auto x_empty = [&](int s) { return bars + 8 * (CNNF_XS + s); };
   auto acc_full = [&](int l) { return bars + 8 * (2 * CNNF_XS + l); };
   auto eps_done = [&](int l) { return bars + 8 * (2 * CNNF_XS + 3 + l); };
-  const float* bias1 = reinterpret_cast<const float*>(sm + cnn3_wbytes<1, 32>());
+  const float* bias1 = reinterpret_cast<const float*>(sm + CNNF_W1T);
   const float* bias2 = reinterpret_cast<const float*>(sm + CNNF_OFF_W2 + cnn3_wbytes<2, 16>());
   const float* bias3 = reinterpret_cast<const float*>(sm + CNNF_OFF_W3 + cnn3_wbytes<1, 16>());
 
@@ -286,10 +287,23 @@ __global__ void __launch_bounds__(CNNF_THREADS, 2) cnn_fused_kernel(const CnnFus
     auto put_row = [&](int r, int q) {
       const int k0 = r - r_first, s = k0 % CNNF_XS;
       if (k0 >= CNNF_XS) mbar_wait_spin(x_empty(s), (uint32_t)((k0 / CNNF_XS - 1) & 1));
-      uint4* xbuf = reinterpret_cast<uint4*>(sm + CNNF_OFF_X + s * SLOTX);
+      // layer 1's im2col along the faces: the K = 16 operand row of ring entry i is (X[i], X[i+1]) in chunk 0 and
+      // (X[i+2], 0) in chunk 1, 4 channels = 8 bytes each: the three face taps of the first layer in ONE MMA
+      uint4* c0 = reinterpret_cast<uint4*>(sm + CNNF_OFF_X + s * SLOTX);
+      uint4* c1 = c0 + CNN_ROWP;
 #pragma unroll
-      for (int k = 0; k < 5; ++k)
-        if (lane + 32 * k < CNN_TILE + 2) xbuf[lane + 32 * k] = pre[q][k];
+      for (int k = 0; k < 4; ++k) {
+        const uint2 me = make_uint2(pre[q][k].x, pre[q][k].y), up = make_uint2(pre[q][k + 1].x, pre[q][k + 1].y);
+        uint2 n1, n2, w0, w1;
+        n1.x = __shfl_down_sync(0xffffffffu, me.x, 1); n1.y = __shfl_down_sync(0xffffffffu, me.y, 1);
+        n2.x = __shfl_down_sync(0xffffffffu, me.x, 2); n2.y = __shfl_down_sync(0xffffffffu, me.y, 2);
+        w0.x = __shfl_sync(0xffffffffu, up.x, 0); w0.y = __shfl_sync(0xffffffffu, up.y, 0);   // entry 32 (k + 1)
+        w1.x = __shfl_sync(0xffffffffu, up.x, 1); w1.y = __shfl_sync(0xffffffffu, up.y, 1);   // entry 32 (k + 1) + 1
+        if (lane == 31) { n1 = w0; n2 = w1; }
+        if (lane == 30) n2 = w0;
+        c0[lane + 32 * k] = make_uint4(me.x, me.y, n1.x, n1.y);
+        c1[lane + 32 * k] = make_uint4(n2.x, n2.y, 0u, 0u);
+      }
       if (r + 2 <= r_last) fetch_row(r + 2, q);
       fence_async_smem();
       mbar_arrive_warp(x_full(s));
@@ -304,7 +318,7 @@ __global__ void __launch_bounds__(CNNF_THREADS, 2) cnn_fused_kernel(const CnnFus
     // ================= MMA issue
     if (lane == 0) {
       constexpr uint32_t ID1 = umma_idesc(128, 96), ID2 = umma_idesc(128, 48);
-      constexpr int PERM1 = 3 * 1 * 96 * 32, PERM2 = 3 * 2 * 48 * 32, PERM3 = 3 * 1 * 48 * 32;
+      constexpr int PERM1 = 96 * 32, PERM2 = 3 * 2 * 48 * 32, PERM3 = 3 * 1 * 48 * 32;
       uint32_t pe[3] = {0, 0, 0};
       for (int r = r_first; r <= r_last; ++r) {
         const int k0 = r - r_first, s = k0 % CNNF_XS;
@@ -315,9 +329,7 @@ __global__ void __launch_bounds__(CNNF_THREADS, 2) cnn_fused_kernel(const CnnFus
         tc_fence_after();
         {
           const uint32_t xb = sm_u32 + CNNF_OFF_X + s * SLOTX, w1 = sm_u32 + ((r + 12) % 3) * PERM1;
-#pragma unroll
-          for (int db = 0; db < 3; ++db)
-            umma_bf16(tmem, umma_desc(xb + db * 16, LBO_A, 128), umma_desc(w1 + db * 96 * 32, 96 * 16, 128), ID1, 1u);
+          umma_bf16(tmem, umma_desc(xb, LBO_A, 128), umma_desc(w1, 96 * 16, 128), ID1, 1u);
           umma_commit(acc_full(0));
           umma_commit(x_empty(s));
         }

@@ -544,6 +544,29 @@ std::vector<uint8_t> pack_cnn_layer3(const float* W, const float* b, int cout, i
   return blob;
 }
 
+// the first layer's blob for cnn_fused_kernel: its 3 face taps x 4 channels fit one K = 16 step (k = 4 dp + channel), so one
+// [3 NOUT x 16] tile per permutation q; rows g * NOUT .. hold row tap dr = (q + 1 - g) mod 3 as above
+std::vector<uint8_t> pack_cnn_layer1_im2col(const float* W, const float* b, int cout, int cin, int NOUT, bool transposed) {
+  const int N3 = 3 * NOUT;
+  std::vector<uint8_t> blob((size_t)3 * N3 * 32 + NOUT * 4, 0);
+  std::vector<float> tile((size_t)N3 * 16);
+  for (int q = 0; q < 3; ++q) {
+    std::fill(tile.begin(), tile.end(), 0.f);
+    for (int g = 0; g < 3; ++g) {
+      const int dr = ((q + 1 - g) % 3 + 3) % 3;
+      for (int dp = 0; dp < 3; ++dp) {
+        const int ta = transposed ? dp : dr, tb = transposed ? dr : dp;
+        for (int n = 0; n < cout; ++n)
+          for (int k = 0; k < cin; ++k)
+            tile[(size_t)(g * NOUT + n) * 16 + 4 * dp + k] = W[(((size_t)n * cin + k) * 3 + ta) * 3 + tb];
+      }
+    }
+    pack_canonical(tile.data(), N3, 16, N3, 16, blob.data() + (size_t)q * N3 * 32);
+  }
+  std::memcpy(blob.data() + (size_t)3 * N3 * 32, b, (size_t)cout * 4);
+  return blob;
+}
+
 cudaError_t pad(jxs_solver* s, const void* U, void* dst) {
   const int bs = 256, gs = s->num_sms * 8;
   if (s->dtype == JXS_F64) pad_kernel<double><<<gs, bs, 0, s->stream>>>((const double*)U, (double*)dst, dims(s));
@@ -1959,7 +1982,7 @@ int jxs_set_flux_cnn(jxs_solver* s, const float* weights, const double in_scale[
   // OIHW: W1[32][4][3][3], b1[32], W2[16][32][3][3], b2[16], W3[4][16][3][3], b3[4]
   const float *W1 = weights, *b1 = W1 + 32 * 4 * 9, *W2 = b1 + 32, *b2 = W2 + 16 * 32 * 9, *W3 = b2 + 16, *b3 = W3 + 4 * 16 * 9;
   for (int d = 0; d < 2; ++d) {
-    const std::vector<uint8_t> blobs3[3] = {pack_cnn_layer3(W1, b1, 32, 4, 1, 32, d == 1), pack_cnn_layer3(W2, b2, 16, 32, 2, 16, d == 1),
+    const std::vector<uint8_t> blobs3[3] = {pack_cnn_layer1_im2col(W1, b1, 32, 4, 32, d == 1), pack_cnn_layer3(W2, b2, 16, 32, 2, 16, d == 1),
                                             pack_cnn_layer3(W3, b3, 4, 16, 1, 16, d == 1)};
     for (int l = 0; l < 3; ++l) {
       if (!s->d_cnn_blob3[d][l]) CU(cudaMalloc(&s->d_cnn_blob3[d][l], blobs3[l].size()));

@@ -13,7 +13,7 @@ pytestmark = pytest.mark.gpu
 
 CASES = {
     "vortex_48": lambda: wl.vortex(48),
-    "jumps_mixed_bc_300x70": lambda: smooth_case(300, 70, 2, MIXED, mu=5e-3, jump=True),   # 3 strips of 128 faces
+    "jumps_mixed_bc_300x70": lambda: smooth_case(300, 70, 2, MIXED, mu=5e-3, jump=True),   # 3 strips of 124 output faces
     "shock_cylinder_256x136": lambda: wl.shock_cylinder(256, 136, Ms=2.0),                 # IBM, exactly 2 strips in y
 }
 
