@@ -89,7 +89,7 @@ struct jxs_solver {
     cudaGraphExec_t exec = nullptr;
     std::vector<long long> key, seen;
     long long launches = 0;
-  } rec_graph, adj_graph;
+  } rec_graph, adj_graph, rec2_graph, adj2_graph;   // 1D and 2D sweeps
   double tan_dt = 0, tan_gdot = 0;
   long long tan_launches = 0;
   // recorded trajectory and adjoint buffers of the one-dimensional reverse sweep (adjoint1d_kernel.cuh), compact
@@ -642,7 +642,7 @@ void drop_graph(jxs_solver* s) {
   s->pair_exec = nullptr;
   if (s->tan_exec) cudaGraphExecDestroy(s->tan_exec);
   s->tan_exec = nullptr;
-  for (jxs_solver::SweepGraph* g : {&s->rec_graph, &s->adj_graph}) {
+  for (jxs_solver::SweepGraph* g : {&s->rec_graph, &s->adj_graph, &s->rec2_graph, &s->adj2_graph}) {
     if (g->exec) cudaGraphExecDestroy(g->exec);
     g->exec = nullptr;
     g->key.clear();
@@ -1434,6 +1434,7 @@ int record2d_common(jxs_solver* s, void* U, double dt, int nsteps) {
   const size_t sb = state * sizeof(double);
   // The fused stage kernel reads through the tensor maps of buf[0..2]; the recording therefore steps in the handle's
   // buffers exactly like jxs_step_fixed_dt and copies each stage's (ghost-filled) input to the tape.
+  auto sweep = [&]() -> int {
   long long rec = 0;
   for (long long n = 0; n < nsteps; ++n) {
     prepare_step_kernel<<<1, 1, 0, s->stream>>>(s->d_state, 0, 0.0, dt);
@@ -1458,6 +1459,16 @@ int record2d_common(jxs_solver* s, void* U, double dt, int nsteps) {
   }
   const int at = s->scheme == JXS_EULER ? (nsteps & 1) : 0;
   CU(cudaMemcpyAsync(T(rec), s->buf[at], sb, cudaMemcpyDeviceToDevice, s->stream));
+  return JXS_OK;
+  };
+  {
+    long long dt_bits;
+    std::memcpy(&dt_bits, &dt, 8);
+    const std::vector<long long> key = {nsteps, dt_bits, s->scheme, ckpt, (long long)(size_t)s->tape2, s->rows_per_seg, s->grid};
+    rc = run_sweep(s, s->rec2_graph, key, sweep);
+    if (rc != JXS_OK) return rc;
+  }
+  const int at = s->scheme == JXS_EULER ? (nsteps & 1) : 0;
   CU(unpad(s, s->buf[at], U));
   rc = finish_steps(s, nsteps);
   if (rc != JXS_OK) return rc;
@@ -1561,6 +1572,8 @@ int adjoint2d_common(jxs_solver* s, void* Ubar, double* gamma_bar, const double*
   else CU(pad(s, Ubar, B(0)));
   s->events_used = 0;
   int x = 0;
+  auto sweep = [&]() -> int {
+  x = 0;
   for (long long n = s->tape_steps - 1; n >= 0; --n) {
     if (targets && n + 1 < s->tape_steps) CU(inject(n + 1, x, 1));
     int rc;
@@ -1587,6 +1600,26 @@ int adjoint2d_common(jxs_solver* s, void* Ubar, double* gamma_bar, const double*
     if (rc == JXS_OK) rc = adjoint_stage2d(s, S0, B(y1), B(y0), 1.0, B(x), 1.0 / 3.0, B(y2), 0.75);
     if (rc != JXS_OK) return rc;
     x = y0;
+  }
+  return JXS_OK;
+  };
+  {
+    int rc;
+    if (s->tape_ckpt) {  // the checkpointed sweep copies dt from a host variable inside the loop: plain launches
+      rc = sweep();
+    } else {
+      long long dt_bits;
+      std::memcpy(&dt_bits, &s->tape_dt, 8);
+      const std::vector<long long> key = {s->tape_steps, dt_bits, s->tape_scheme, (long long)(size_t)s->tape2,
+                                          (long long)(size_t)s->adj2, (long long)(size_t)targets};
+      rc = run_sweep(s, s->adj2_graph, key, sweep);
+      if (rc == JXS_OK) {  // where the adjoint of U^0 ends up does not depend on how the sweep was run
+        x = 0;
+        if (s->tape_scheme == JXS_EULER) x = (int)(s->tape_steps & 1);
+        else for (long long n = 0; n < s->tape_steps; ++n) x = (x + 3) & 3;
+      }
+    }
+    if (rc != JXS_OK) return rc;
   }
   CU(unpad(s, B(x), Ubar));
   double out[2];

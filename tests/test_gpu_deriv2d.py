@@ -238,3 +238,36 @@ def test_adjoint2d_mse_sweep_and_argument_checks():
     with pytest.raises(m.JxsError) as e:
         s.step_fixed_dt_record(U, dt, 1)
     assert e.value.code == m.ESTATE
+
+
+def test_sweep_graphs_of_the_2d_path_replay_bitwise():
+    """The 2D recorded sweep and reverse sweep run as plain launches on the first call with given parameters, are captured
+    as CUDA graphs on the second and replayed afterwards (run_sweep in csrc/jxs_api.cu): same bits as with graph replay
+    switched off (the 2D reverse sweep has no atomics), also after a change of the step count and back."""
+    case = wl.shock_cylinder(96, 48, Ms=2.0, Re=300.0, x_shock=0.28)
+    s0 = solver_of(case)
+    U0 = dev(case["U0"])
+    s0.step(U0, 0.4, 10)
+    dt = s0.time()[1]
+    rng = np.random.default_rng(2)
+    Ubar = dev(rng.normal(size=case["U0"].shape))
+    targets = dev(rng.normal(size=(3,) + case["U0"].shape) * 0.01) + U0
+
+    def run(s, steps):
+        U, B = U0.clone(), Ubar.clone()
+        s.step_fixed_dt_record(U, dt, steps)
+        g = s.adjoint_steps(B)
+        out = [U, B, g]
+        if steps == 3:
+            U2, B2 = U0.clone(), torch.zeros_like(U0)
+            s.step_fixed_dt_record(U2, dt, steps)
+            loss, g2 = s.adjoint_steps_mse(targets, B2)
+            out += [B2, loss, g2]
+        return out
+
+    plain, graphed = solver_of(case), solver_of(case)
+    plain.set_graph_replay(False)
+    for steps in (3, 3, 3, 3, 2, 2, 2, 3, 3):
+        want, got = run(plain, steps), run(graphed, steps)
+        for a, b in zip(got, want):
+            assert torch.equal(a, b) if isinstance(a, torch.Tensor) else a == b
