@@ -222,6 +222,48 @@ __global__ void wavespeed_kernel(const T* __restrict__ U, GridDims g, const uint
   }
 }
 
+// pad_kernel and wavespeed_kernel in one pass over the caller's array (jxs_step with a CFL step: the state is read once
+// instead of twice).  The per-cell arithmetic and the reduction are wavespeed_kernel's, so s_max has the same bits.
+template <typename T>
+__global__ void pad_wavespeed_kernel(const T* __restrict__ src, T* __restrict__ dst, GridDims g, const uint8_t* __restrict__ fluid,
+                                     T gamma, unsigned long long* out_bits, long long out_stride) {
+  const long long n = (long long)g.nx * g.ny;
+  const int member = blockIdx.y;
+  src += 4 * n * member;
+  dst += (long long)member * (g.ny + 6) * g.pitch;
+  if (fluid) fluid += member * n;
+  out_bits = reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(out_bits) + member * out_stride);
+  T smax = T(0);
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+    const int j = (int)(t / g.nx), i = (int)(t - (long long)j * g.nx);
+    const long long o = (long long)(j + 3) * g.pitch + i + 3;
+    const T r = src[t], ru = src[n + t], rv = src[2 * n + t], E = src[3 * n + t];
+    dst[o] = r; dst[g.plane + o] = ru; dst[2 * g.plane + o] = rv; dst[3 * g.plane + o] = E;
+    if (fluid && !fluid[t]) continue;
+    const T u = ru / r, v = rv / r;
+    const T p = (gamma - T(1)) * (E - T(0.5) * r * (u * u + v * v));
+    const T a = sqrt(gamma * p / r);
+    const T s = max(fabs(u), fabs(v)) + a;
+    smax = (s > smax || s != s) ? s : smax;
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    const T other = __shfl_xor_sync(0xffffffffu, smax, o);
+    smax = (other > smax || other != other) ? other : smax;
+  }
+  __shared__ T wmax[32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) wmax[warp] = smax;
+  __syncthreads();
+  if (warp == 0) {
+    smax = lane < (int)(blockDim.x >> 5) ? wmax[lane] : T(0);
+    for (int o = 16; o > 0; o >>= 1) {
+      const T other = __shfl_xor_sync(0xffffffffu, smax, o);
+      smax = (other > smax || other != other) ? other : smax;
+    }
+    if (lane == 0) atomic_max_bits(out_bits, (double)smax);
+  }
+}
+
 // device-resident stepping state
 struct StepState {
   unsigned long long smax_bits[2];  // wavespeed of U^n (cur) and accumulator for U^{n+1} (next)

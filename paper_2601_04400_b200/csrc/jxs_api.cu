@@ -599,6 +599,22 @@ cudaError_t wavespeed(jxs_solver* s, const void* Upad, unsigned long long* out_b
   return cudaGetLastError();
 }
 
+// pad + wavespeed in one pass (the entry of jxs_step with a CFL step)
+cudaError_t pad_wavespeed(jxs_solver* s, const void* U, void* dst, unsigned long long* out_bits) {
+  cudaError_t e = cudaMemset2DAsync(out_bits, sizeof(StepState), 0, sizeof(unsigned long long), s->nb, s->stream);
+  if (e != cudaSuccess) return e;
+  const int bs = 256;
+  const dim3 gs(std::max(1, s->num_sms * 8 / s->nb), s->nb);
+  if (s->dtype == JXS_F64)
+    pad_wavespeed_kernel<double><<<gs, bs, 0, s->stream>>>((const double*)U, (double*)dst, dims(s), s->d_fluid, s->gamma,
+                                                           out_bits, (long long)sizeof(StepState));
+  else
+    pad_wavespeed_kernel<float><<<gs, bs, 0, s->stream>>>((const float*)U, (float*)dst, dims(s), s->d_fluid, (float)s->gamma,
+                                                          out_bits, (long long)sizeof(StepState));
+  s->launches++;
+  return cudaGetLastError();
+}
+
 void free_ibm(jxs_solver* s) {
   cudaFree(s->d_fluid); cudaFree(s->d_cell); cudaFree(s->d_donor); cudaFree(s->d_w); cudaFree(s->d_nrm);
   s->d_fluid = nullptr; s->d_cell = nullptr; s->d_donor = nullptr; s->d_w = nullptr; s->d_nrm = nullptr;
@@ -731,12 +747,12 @@ bool capture_pair(jxs_solver* s, double cfl_h, double fixed_dt) {
 }
 
 // advance the padded state in buf[0] by nsteps steps; returns in *where the buffer that holds the result
-int run_steps(jxs_solver* s, double cfl, double fixed_dt, int nsteps, int* where) {
+int run_steps(jxs_solver* s, double cfl, double fixed_dt, int nsteps, int* where, bool smax_ready = false) {
   const double cfl_h = cfl * std::min(s->dx, s->dy);
   int cur = 0, at = 0;
   s->events_used = 0;
   s->mlp_events_used = 0;
-  if (!(fixed_dt > 0)) CU(wavespeed(s, s->buf[0], &s->d_state->smax_bits[0]));
+  if (!(fixed_dt > 0) && !smax_ready) CU(wavespeed(s, s->buf[0], &s->d_state->smax_bits[0]));
   int n = 0;
   if (!s->profiling && s->use_graph && nsteps >= 6) {
     // the first pair runs as plain launches (it also configures the kernels' attributes outside any capture)
@@ -851,13 +867,16 @@ int step_common(jxs_solver* s, void* U, double cfl, double fixed_dt, int nsteps,
     CU(cudaMemcpyAsync(s->stage_io, U, bytes, cudaMemcpyHostToDevice, s->stream));
     Ud = s->stage_io;
   }
-  CU(pad(s, Ud, s->buf[0]));
+  // with a CFL step the wavespeed of the incoming state is taken in the same pass that pads it
+  const bool fused_entry = !(fixed_dt > 0) && nsteps > 0;
+  if (fused_entry) CU(pad_wavespeed(s, Ud, s->buf[0], &s->d_state->smax_bits[0]));
+  else CU(pad(s, Ud, s->buf[0]));
   if (!s->tuned && nsteps > 0 && wait) {  // never inside jxs_step_async: it must only enqueue (jxs_tune does it explicitly)
     const int rc = tune_decomposition(s);
     if (rc != JXS_OK) return rc;
   }
   int at = 0;
-  int rc = run_steps(s, cfl, fixed_dt, nsteps, &at);
+  int rc = run_steps(s, cfl, fixed_dt, nsteps, &at, fused_entry);
   if (rc != JXS_OK) return rc;
   if (host) {
     CU(unpad(s, s->buf[at], s->stage_io));

@@ -49,7 +49,7 @@ def test_batch_equals_separate_handles_bitwise(dtype, mlp):
     n0 = b2.launch_count()
     b2.step(Ub, 0.4, 10)
     per_step = 1 + 3 * (3 if mlp else 2)
-    assert b2.launch_count() - n0 == 10 * per_step + 3      # + pad, wavespeed, unpad
+    assert b2.launch_count() - n0 == 10 * per_step + 2      # + pad-with-wavespeed, unpad
 
 
 def test_batch_member_against_the_oracle_and_fixed_dt():
