@@ -27,17 +27,32 @@ __device__ __forceinline__ long long padded_offset(const GridDims& g, long long 
   const int j = (int)(r / g.nx), i = (int)(r - (long long)j * g.nx);
   return k * g.plane + ((long long)m * (g.ny + 6) + j + 3) * g.pitch + i + 3;
 }
+// one piece of a row of one variable of one member at a time (the index arithmetic once per piece, not per element);
+// rows are cut into pieces of PAD_PIECE elements so that one-dimensional problems (4 rows in all) still fill the GPU
+constexpr int PAD_PIECE = 4096;
 template <typename T>
 __global__ void pad_kernel(const T* __restrict__ src, T* __restrict__ dst, GridDims g) {
-  const long long n = (long long)g.nx * g.ny * g.nb;
-  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < 4 * n; t += (long long)gridDim.x * blockDim.x)
-    dst[padded_offset(g, t)] = src[t];
+  const int npiece = (g.nx + PAD_PIECE - 1) / PAD_PIECE;
+  const long long nitems = 4LL * g.ny * g.nb * npiece;
+  for (long long it = blockIdx.x; it < nitems; it += gridDim.x) {
+    const int L = (int)(it / npiece), i0 = (int)(it - (long long)L * npiece) * PAD_PIECE, i1 = min(i0 + PAD_PIECE, g.nx);
+    const int mk = L / g.ny, j = L - mk * g.ny, m = mk >> 2, k = mk & 3;
+    const T* a = src + (long long)L * g.nx;
+    T* b = dst + k * g.plane + ((long long)m * (g.ny + 6) + j + 3) * g.pitch + 3;
+    for (int i = i0 + threadIdx.x; i < i1; i += blockDim.x) b[i] = a[i];
+  }
 }
 template <typename T>
 __global__ void unpad_kernel(const T* __restrict__ src, T* __restrict__ dst, GridDims g) {
-  const long long n = (long long)g.nx * g.ny * g.nb;
-  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < 4 * n; t += (long long)gridDim.x * blockDim.x)
-    dst[t] = src[padded_offset(g, t)];
+  const int npiece = (g.nx + PAD_PIECE - 1) / PAD_PIECE;
+  const long long nitems = 4LL * g.ny * g.nb * npiece;
+  for (long long it = blockIdx.x; it < nitems; it += gridDim.x) {
+    const int L = (int)(it / npiece), i0 = (int)(it - (long long)L * npiece) * PAD_PIECE, i1 = min(i0 + PAD_PIECE, g.nx);
+    const int mk = L / g.ny, j = L - mk * g.ny, m = mk >> 2, k = mk & 3;
+    const T* a = src + k * g.plane + ((long long)m * (g.ny + 6) + j + 3) * g.pitch + 3;
+    T* b = dst + (long long)L * g.nx;
+    for (int i = i0 + threadIdx.x; i < i1; i += blockDim.x) b[i] = a[i];
+  }
 }
 // every element of the padded buffers starts as a benign state so that support cells outside the
 // frame never feed denormals/NaNs into the division slow paths
@@ -234,8 +249,11 @@ __global__ void pad_wavespeed_kernel(const T* __restrict__ src, T* __restrict__ 
   if (fluid) fluid += member * n;
   out_bits = reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(out_bits) + member * out_stride);
   T smax = T(0);
-  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
-    const int j = (int)(t / g.nx), i = (int)(t - (long long)j * g.nx);
+  const int npiece = (g.nx + PAD_PIECE - 1) / PAD_PIECE;
+  for (long long it = blockIdx.x; it < (long long)g.ny * npiece; it += gridDim.x)   // one piece of a row at a time
+  for (int j = (int)(it / npiece), i0 = (int)(it - (long long)j * npiece) * PAD_PIECE, i = i0 + threadIdx.x;
+       i < min(i0 + PAD_PIECE, g.nx); i += blockDim.x) {
+    const long long t = (long long)j * g.nx + i;
     const long long o = (long long)(j + 3) * g.pitch + i + 3;
     const T r = src[t], ru = src[n + t], rv = src[2 * n + t], E = src[3 * n + t];
     dst[o] = r; dst[g.plane + o] = ru; dst[2 * g.plane + o] = rv; dst[3 * g.plane + o] = E;
