@@ -3,32 +3,37 @@
 //
 //   x (24 stencil primitives / in_scale, bf16) -> tanh(W1 x + b1) -> tanh(W2 h1 + b2) -> W3 h2 + b3
 //
-// One CTA per SM = 11 warps marches a strip of 128 cells upwards:
-//   warps 0-3  (warpgroup 0)  the RIGHT faces of the cells (x-face i+1/2: cells i-2..i+3 of the row); thread lt owns
-//                             the face of the cell in column c0+lt
-//   warps 4-7  (warpgroup 1)  their TOP faces (y-face j+1/2: rows j-2..j+3 of the column, normal velocity first)
-//   warp 8, 9                 one lane each issues the tcgen05.mma of warpgroup 0 / 1
-//   warp 10                   the producer: conserved rows from HBM -> scaled bf16 primitives in a shared-memory ring
-// The 128 faces of a warpgroup and row are the M = 128 rows of a chain of tcgen05.mma tiles:
+// One CTA per SM = 26 warps marches a strip of 128 cells upwards.  The 128 RIGHT faces of a cell row (x-face i+1/2:
+// cells i-2..i+3 of the row) and its 128 TOP faces (y-face j+1/2: rows j-2..j+3 of the column, normal velocity
+// first) are the M = 128 rows of two chains (directions g = 0, 1) of tcgen05.mma tiles:
 //   layer 1  D[128 x 64] = A1[128 x 32] W1^T     (K = 24 padded to 32, 2 MMAs of K = 16)
 //   layer 2  D[128 x 64] = A2[128 x 64] W2^T     (4 MMAs)
 //   layer 3  D[128 x 16] = A3[128 x 64] W3^T     (N = 4 padded to 16, 4 MMAs)
+// and each direction works on TWO rows at once (tile slots s = 0: even rows of the segment, s = 1: odd rows): four
+// independent chains, so that the MMAs of one (and the ~230 cycles a commit takes to come back) run under the tanh of
+// the others.  What binds is the SFU (128 tanh per face at 16 per clock and SM); the schedule exists to keep
+// MUFU.TANH issuing.
 // The A operands live in TENSOR MEMORY (tcgen05.mma with [a_tmem]: lane m = row m, 32-bit column c = the bf16
-// pair k = 2c, 2c+1): every thread writes the row of its own face with tcgen05.st and the tensor core reads
-// it from there, so an MMA fetches only its 0.5-2 KB weight tile from shared memory and runs at the
-// 128 N / 256-cycle floor (32 cycles for N = 64) instead of the ~100 cycles that a 4 KB A tile in shared
-// memory cost (profiles/r02_flux_mlp.md).  A tile slot is 96 TMEM columns: X = [0, 32) the A operand of the
-// current layer, Y = [32, 96) its accumulator; TMEM lane m = face m = thread m, so tcgen05.ld (32x32b) hands
-// every thread the pre-activations of its own face; bias, tanh (tanh.approx.f32, then one rounding to bf16 —
-// the rounding points of the oracle's emulating mode; the packed tanh.approx.bf16x2 was measured: SASS splits
-// it into two MUFU operations, so it is no faster, and its extra input rounding costs 1e-2 of accuracy) and
-// the tcgen05.st of the next A operand follow in registers.
-// What binds is the SFU (128 tanh per face at 16 per clock and SM), so the schedule exists to keep MUFU.TANH
-// issuing: each warpgroup works on TWO rows at once (two tile slots, 4 x 96 of the 512 TMEM columns per SM) and
-// alternates between them, so the MMAs of one slot (and their completion latency) run under the tanh phase of
-// the other.  Hand-over is by mbarriers only: a_full[g][s] (128 arrivals: the A operand of slot s is in TMEM)
-// -> the MMA lane issues the layer and commits to d_full[g][s] -> the threads read the accumulator.  The ring
-// has its own full / empty barriers per row slot; nothing in the loop is a CTA-wide barrier.
+// pair k = 2c, 2c+1): threads write the row of their own face with tcgen05.st and the tensor core reads it there;
+// only the 0.5-2 KB weight tile of an MMA comes from shared memory.  A slot owns 128 of the SM's 512 TMEM columns:
+//   X  = [0, 32)     A operand of layers 2 and 3 (the bf16 hidden activations)
+//   Y  = [32, 96)    accumulator of layers 1 and 2 (64 pre-activations per face)
+//   A1 = [96, 112)   layer-1 operand of the slot's NEXT row (24 inputs + padding)
+//   O  = [112, 128)  accumulator of the output layer
+// TMEM lane m = face m, so tcgen05.ld (32x32b) hands a thread the pre-activations of its own face; bias, tanh
+// (tanh.approx.f32, then one rounding to bf16 - the rounding points of the oracle's emulating mode; the packed
+// tanh.approx.bf16x2 was measured: SASS splits it into two MUFU operations, so it is no faster, and its extra input
+// rounding costs 1e-2 of accuracy) and the tcgen05.st of the next operand follow in registers.
+// Warp roles:
+//   warps 0-15   four tanh warpgroups, (direction g, half h of the 64 hidden units): wait d_full[g][s] -> load 32
+//                pre-activations -> tanh -> store 16 packed columns of X -> arrive a_full[g][s]; slots alternate
+//   warps 16-19  the builder warpgroup, both directions, off the critical path: once layer 1 of a row has read A1
+//                (l1_done) it builds the slot's next row there from the ring (a1_full); it reads the output layer's
+//                accumulator (o_full), frees it (o_free) and writes y + b3 as fp16 to HBM
+//   warps 20, 21 one lane each issues the MMAs of a direction as their operands become ready and commits them
+//   warps 22-25  producers: conserved row n (n = p mod 4 for producer p) from HBM -> scaled bf16 primitives (fp32
+//                arithmetic: they are rounded to 8 bits next) in a 10-row shared-memory ring (ring_full / ring_empty)
+// Hand-over is by mbarriers only, one arrival per warp; nothing in the loop is a CTA-wide barrier.
 // Output: y (before out_scale) per face as fp16, one uint4 per padded cell (row, col): {right face: 4, top
 // face: 4}, k = (mass, normal, tangential momentum, energy).
 #pragma once
