@@ -662,23 +662,34 @@ def run_c5(args, rank, world, local_rank, dist, barrier, tdt):
     sampler = ClockSampler(local_rank)
     main_stream = torch.cuda.current_stream()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def one_pass():   # K steps of every simulation, all streams released together and joined again
+        for st in streams:
+            st.wait_stream(main_stream)
+        for s, U in zip(solvers, Us):
+            s.step_async(U, 0.4, K)
+        for st in streams:
+            main_stream.wait_stream(st)
+
+    e0.record(main_stream)
+    one_pass()                    # untimed: how long one pass lasts decides the repetitions below
+    e1.record(main_stream)
+    for s in solvers:
+        s.wait()
+    R = 1 if args.profile_kernels else repeats_for(e0.elapsed_time(e1))
     launches0 = sum(s.launch_count() for s in solvers)
     barrier()
     sampler.start()
     e0.record(main_stream)
-    for st in streams:
-        st.wait_event(e0)
-    for s, U in zip(solvers, Us):
-        s.step_async(U, 0.4, K)
-    for st in streams:
-        main_stream.wait_stream(st)
+    for _ in range(R):
+        one_pass()
     e1.record(main_stream)
     for s in solvers:
         s.wait()
     barrier()
     clocks = sampler.stop()
-    ms = max_over_ranks(e0.elapsed_time(e1), dist, "cuda")
-    launches = sum(s.launch_count() for s in solvers) - launches0
+    ms = max_over_ranks(e0.elapsed_time(e1), dist, "cuda") / R
+    launches = (sum(s.launch_count() for s in solvers) - launches0) // R
     if not all(bool(torch.isfinite(U).all()) for U in Us):
         raise SystemExit("bench.py: non-finite state after the timed region")
     value = aggregate_rate(ncell, K, world, ms)
@@ -700,6 +711,9 @@ def run_c5(args, rank, world, local_rank, dist, barrier, tdt):
                                "Mach ~ U[1.5,3], per-face MLP 24-64-64-4 in bf16 fused into the HLLC flux)",
                    "cfl": 0.4, "rk": "SSP-RK3", "cells": ncell, "handles": len(solvers), "streams": len(streams),
                    "batched": args.batch_groups > 0,
+                   "timed_region": f"{R} back-to-back passes of {K} steps of all the simulations (>= {MIN_REGION_S} s in all); "
+                                   "ms_per_step and value are the mean pass",
+                   "repeats": R,
                    "l2": "16 x 3 x 17 MB of state buffers = 800 MB vs 126 MB of L2, no flush needed",
                    "parallelism": "replicas" if world > 1 else "single GPU"},
         "clocks": clocks, "gpu_launches": launches,
