@@ -15,6 +15,9 @@ CASES = {
     "vortex_48": lambda: wl.vortex(48),
     "jumps_mixed_bc_300x70": lambda: smooth_case(300, 70, 2, MIXED, mu=5e-3, jump=True),   # 3 strips of 124 output faces
     "shock_cylinder_256x136": lambda: wl.shock_cylinder(256, 136, Ms=2.0),                 # IBM, exactly 2 strips in y
+    "tiny_8x8": lambda: wl.vortex(8),                                                      # the smallest grid the library takes
+    "strip_edge_124x9": lambda: smooth_case(124, 9, 4, MIXED, mu=5e-3),                    # 125 x-faces: a second strip of one face
+    "thin_16x150": lambda: smooth_case(16, 150, 5, MIXED, mu=5e-3),                        # one narrow strip, several row segments
 }
 
 
@@ -43,7 +46,8 @@ def test_input_fields_and_corrections(name):
     for got, want in ((gx, bf16(Xx)), (gy, bf16(Xy))):
         d = np.abs(got - want)
         assert d.max() <= 2.0 ** -7 * np.abs(want).max()          # at most one bf16 step where a value sits on a tie
-        assert (d > 0).mean() < 0.02
+        # (a wall's normal momentum is zero up to round-off on both sides, 1e-17 here and 1e-8 there: not a mismatch)
+        assert (d > 1e-6 * np.abs(want).max()).mean() < 0.02
     dFx, dGy = [a.cpu().numpy().astype(np.float64) for a in s.flux_correction(dev(case["U0"]))]
     outs = scales[1]
     for k in range(4):

@@ -78,7 +78,17 @@ CASES = {
     "shock_cylinder_256x128": lambda: wl.shock_cylinder(256, 128, Ms=2.0),
     "shock_cylinder_ragged_301x77": lambda: wl.shock_cylinder(301, 77, Ms=2.5, bodies=((0.5, 0.5, 0.12),)),
     "vortex_64": lambda: wl.vortex(64),
+    # the smallest grid the library takes (one strip of 9 face columns, 9 face rows) and two lopsided ones: a strip and a
+    # half wide with 10 rows (every CTA starts and ends inside its pipeline's warm-up), 17 columns with 151 rows
+    "tiny_8x8": lambda: wl.vortex(8),
+    "wide_190x9": lambda: _smooth(190, 9),
+    "thin_16x150": lambda: _smooth(16, 150),
 }
+
+
+def _smooth(nx, ny):
+    from test_gpu_parity import MIXED, smooth_case
+    return smooth_case(nx, ny, 3, MIXED, mu=2e-3, jump=True)
 
 
 @pytest.mark.parametrize("name", list(CASES))
