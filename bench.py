@@ -743,9 +743,9 @@ def main():
     ap.add_argument("--euler", action="store_true", help="mu = 0, no IBM (not the headline config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile-kernels", action="store_true", help="c5 only: per-kernel CUDA-event spans")
-    ap.add_argument("--batch-groups", type=int, default=0,
-                    help="c5 only: 0 = 16 single handles on 16 streams; G > 0 = the 16 cases in G batched handles "
-                         "(jxs_create_batch), one stream each")
+    ap.add_argument("--batch-groups", type=int, default=2,
+                    help="c5 only: G > 0 = the 16 cases in G batched handles (jxs_create_batch), one stream each (default 2, "
+                         "the fastest measured); 0 = 16 single handles on 16 streams")
     ap.add_argument("--rows-per-segment", type=int, default=0,
                     help="fix the stage kernel's row-segment length (jxs_set_rows_per_segment) instead of measuring it at the "
                          "first step call: used for ncu captures, which would otherwise land in the ~40 tuning launches")
