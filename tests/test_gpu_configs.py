@@ -140,7 +140,7 @@ def test_c5_one_1024x512_handle_correction_after_20_steps():
 
 
 def test_c5_concurrent_handles_with_the_network_equal_the_synchronous_path():
-    """bench.py --workload c5's configuration: 16 handles x 1024x512 with the flux MLP, one stream each,
+    """bench.py --workload c5 --batch-groups 0: 16 handles x 1024x512 with the flux MLP, one stream each,
     jxs_step_async + jxs_wait — bitwise equal to jxs_step on a handle of its own."""
     m = jxs()
     cases = wl.batch_cases(16)
